@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the all-sky stochtrack hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5]
+
+A "step" is one pass of the whole hot path over one synthetic map: S0 map preparation
+(st_set_map) + S1-S4 (st_search: template generation, rasterisation, Eq. 8 scoring for
+every (template, delay), max/argmax/histogram) -- see DESIGN.md.  The default workload
+is BASELINE.json configs[4] (the largest single-GPU configuration: 1000 x 2461 map, 1e7
+templates, 512 delays = 2.6e12 track-pixel evaluations per step).  `value` is track-pixel
+evaluations per second over all ranks, device-timed with the map resident in HBM; `e2e`
+is the same metric through the C ABI with host buffers (H2D of the map and D2H of the
+result inside the timed region).  Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import synth  # noqa: E402
+
+METRIC = "track_pixel_evals_per_s"
+UNIT = "evals/s"
+N_SM, FP32_LANES = 148, 128           # B200: 148 SMs x 128 FP32 lanes (B200_PROFILING.md, blackwell guide)
+FLOP_PER_EVAL = 4                     # Eq. 8 needs 2 FMA per (pixel, delay) once the phase factor is known
+# ncu --set full, dominant kernel, config 5 sub-range (profiles/); None until measured
+DRAM_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    sm_mhz, src = 1965.0, "fallback clock 1965 MHz"
+    if os.path.exists(p):
+        with open(p) as f:
+            sm_mhz = float(json.load(f).get("sm_max_mhz", sm_mhz))
+        src = "MEASURED_PEAKS.json sm_max_mhz"
+    return N_SM * FP32_LANES * 2 * sm_mhz * 1e6 / 1e12, f"148 SMs x 128 FP32 lanes x 2 flop x {sm_mhz:.0f} MHz ({src})"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.rows, self.proc, self.index = [], None, index
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([x.strip() for x in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        self.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        load = sorted(sm)[len(sm) // 2:] if sm else []      # upper half = samples under load
+        return {"sm_mhz": float(np.median(load)) if load else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def build_inputs(cfg, st, m=0):
+    """Seeded synthetic map of the config; injections rasterised by the CUDA path (product side)."""
+    def rast(inj):
+        return st.debug_rasterise_track(inj.N, inj.j0, inj.a, inj.y0, inj.y1, inj.y2)
+    return synth.config_inputs(cfg, m, rasterise=rast)
+
+
+def search_kwargs(cfg, tau):
+    kw = dict(n_bins=cfg.n_bins, hist_lo=cfg.hist_lo, hist_hi=cfg.hist_hi)
+    if cfg.tau_mode == "grid":
+        kw["tau_grid"] = tau
+    else:
+        kw["tau_range"] = (-synth.TAU_MAX, synth.TAU_MAX)
+    return kw
+
+
+def run_ours(args):
+    import torch
+    import paper_1401_8060_b200 as pkg
+    from paper_1401_8060_b200 import build, sharding
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    build.build()
+    pkg.load_library()
+    dev = f"cuda:{local}"
+    cfg = synth.CONFIGS[args.config]
+    n_tracks = args.tracks or cfg.n_tracks
+    st = pkg.Stochtrack(cfg.n_t, cfg.n_f, cfg.df, cfg.f_min, max_n_tau=max(cfg.n_tau, 64), device=dev)
+    csd, sigma, tau = build_inputs(cfg, st)
+    seed = synth.map_seed(cfg, 0)
+    # weak scaling: rank r scores its own template-id range on its own copy of the map
+    first, n_mine = sharding.rank_range(n_tracks, rank)
+    kw = search_kwargs(cfg, tau)
+    csd_d = torch.from_numpy(csd).to(dev)
+    sigma_d = torch.from_numpy(sigma).to(dev) if sigma is not None else None
+    csd_h = torch.from_numpy(csd).pin_memory()
+    sigma_h = torch.from_numpy(sigma).pin_memory() if sigma is not None else None
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
+
+    def step_device():
+        st.set_map(csd_d, sigma_d)
+        return st.search(n_mine, seed, cfg.n_min, cfg.n_max, track_offset=first, **kw)
+
+    def step_host():
+        st.set_map(csd_h.numpy(), sigma_h.numpy() if sigma_h is not None else None)
+        return st.search(n_mine, seed, cfg.n_min, cfg.n_max, track_offset=first, **kw)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        flush.zero_()
+        r = step_device()
+    # ---- device-timed steps (inputs resident in HBM; L2 flushed between steps)
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    barrier()
+    t_wall0 = time.perf_counter()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kernel_ms, launches, evals = 0.0, 0, 0
+    for a, b in ev:
+        flush.zero_()
+        a.record()
+        r = step_device()
+        b.record()
+        kernel_ms += r.gpu_ms
+        launches += r.n_launches + 1               # + k_prepare_map
+        evals += r.n_evals
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    dev_ms = sum(a.elapsed_time(b) for a, b in ev)
+    # ---- end to end through the C ABI with host buffers
+    step_host()
+    barrier()
+    e2e_evals, t0 = 0, time.perf_counter()
+    for _ in range(args.steps):
+        e2e_evals += step_host().n_evals
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([dev_ms, e2e_s, float(evals), float(e2e_evals), float(launches), kernel_ms], dtype=torch.float64,
+                     device=dev)
+    if dist is not None:
+        mx = t.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = t.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        dev_ms, e2e_s, kernel_ms = mx[0].item(), mx[1].item(), mx[5].item()
+        evals, e2e_evals, launches = sm[2].item(), sm[3].item(), sm[4].item()
+        combined = sharding.all_combine(r)
+    else:
+        combined = r
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    peak, peak_how = peaks()
+    value = evals / (dev_ms * 1e-3)
+    per_launch_evals = evals / world / args.steps            # one scoring launch sequence per step per rank
+    achieved = FLOP_PER_EVAL * per_launch_evals / (kernel_ms / args.steps * 1e-3) / 1e12
+    n_tau = cfg.n_tau if cfg.tau_mode == "grid" else 1
+    h2d = csd.nbytes + (sigma.nbytes if sigma is not None else 0)
+    d2h = 128 + 8 * cfg.n_bins
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({cfg.name}): {cfg.n_t}x{cfg.n_f} map, "
+                               f"{n_tracks:.0e} templates per GPU, {n_tau} delays ({cfg.tau_mode})",
+                   "n_t": cfg.n_t, "n_f": cfg.n_f, "n_tracks_per_gpu": n_tracks, "n_tau": n_tau,
+                   "tau_mode": cfg.tau_mode, "kernel": r.kernel_name, "l2": "flushed between timed steps (256 MB write)",
+                   "parallelism": f"independent template-id ranges x{world}, no data-path collective"},
+        "tracks_tau_per_s": world * args.steps * n_mine * n_tau / (dev_ms * 1e-3),
+        "wall_s_timed_region": t_wall,
+        "e2e": {"value": e2e_evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": {"bound": "alu", "kernel": f"k_score_recur ({r.kernel_name})", "achieved": achieved, "peak": peak,
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES_PER_LAUNCH,
+                     "peak_how": peak_how + "; algorithmic 4 flop per track-pixel evaluation (DESIGN.md)"},
+        "result": {"max_snr": combined["max_snr_f64"], "arg_track": combined["arg_track"],
+                   "arg_tau_index": combined["arg_tau_index"]},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(cfg, csd, sigma, tau, seed, budget_s=args.cpu_budget)
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def oracle_inputs(cfg):
+    from oracle import oracle
+
+    def rast(inj):
+        return oracle.rasterise(oracle.make_track(inj.N, inj.j0, inj.a, inj.y0, inj.y1, inj.y2), cfg.n_f)
+    return synth.config_inputs(cfg, 0, rasterise=rast)
+
+
+def oracle_sample(oracle, p, cfg, tau, seed, n, first=0):
+    kw = dict(tau_grid=tau) if cfg.tau_mode == "grid" else dict(tau_range=(-synth.TAU_MAX, synth.TAU_MAX))
+    t0 = time.perf_counter()
+    r = oracle.search(p, cfg.f_min, cfg.df, n, seed, cfg.n_min, cfg.n_max, n_bins=cfg.n_bins, hist_lo=cfg.hist_lo,
+                      hist_hi=cfg.hist_hi, track_offset=first, **kw)
+    return r, time.perf_counter() - t0
+
+
+def cpu_baseline(cfg, csd, sigma, tau, seed, budget_s=15.0):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample."""
+    from oracle import oracle
+    oracle.build()
+    p = oracle.prepare_map(csd, sigma)
+    r, dt = oracle_sample(oracle, p, cfg, tau, seed, 256)
+    rate = r["n_evals"] / dt
+    n = int(max(256, min(cfg.n_tracks, budget_s * rate / (r["n_evals"] / 256))))
+    r, dt = oracle_sample(oracle, p, cfg, tau, seed, n)
+    return {"value": r["n_evals"] / dt, "unit": UNIT, "cores": r["threads_used"], "kind": "oracle",
+            "sample": f"first {n} templates of the workload ({r['n_evals']:.3e} evals, {dt:.1f} s), float64, OpenMP"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle
+    oracle.build()
+    cfg = synth.CONFIGS[args.config]
+    csd, sigma, tau = oracle_inputs(cfg)
+    seed = synth.map_seed(cfg, 0)
+    p = oracle.prepare_map(csd, sigma)
+    r, dt = oracle_sample(oracle, p, cfg, tau, seed, 256)
+    per_track = dt / 256
+    n = int(max(256, min(cfg.n_tracks, args.ref_step_s / per_track)))
+    for i in range(args.warmup):
+        oracle_sample(oracle, p, cfg, tau, seed, n, first=i * n)
+    evals, t = 0, 0.0
+    for i in range(args.steps):
+        r, dt = oracle_sample(oracle, p, cfg, tau, seed, n, first=(args.warmup + i) * n)
+        evals += r["n_evals"]; t += dt
+    n_tau = cfg.n_tau if cfg.tau_mode == "grid" else 1
+    value = evals / t
+    sample = f"{n} templates per step of the workload's id range ({evals / args.steps:.3e} evals per step), float64, OpenMP"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({cfg.name}): {cfg.n_t}x{cfg.n_f} map, "
+                               f"{n_tau} delays ({cfg.tau_mode}); bounded sample of {n} templates per step",
+                   "n_t": cfg.n_t, "n_f": cfg.n_f, "n_tau": n_tau, "tau_mode": cfg.tau_mode},
+        "cpu_baseline": {"value": value, "unit": UNIT, "kind": "oracle", "cores": r["threads_used"], "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--tracks", type=int, default=0, help="override templates per GPU (debugging)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--ref-step-s", type=float, default=6.0, help="seconds of oracle work per reference step")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = max(args.warmup, 1)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,180 @@
+/*
+ * stochtrack.h -- C ABI of the B200 (sm_100a) all-sky stochtrack hot path.
+ *
+ * Method: Thrane & Coughlin, "Seedless clustering in all-sky searches for
+ * gravitational-wave transients" (arXiv:1401.8060).  Citations are lines of the
+ * paper text (PAPER.md:<line>) with the section / equation they fall in, and
+ * readings G<n> of DESIGN.md where the paper is silent.
+ *
+ * What the library computes (one GPU, one stream, no collectives):
+ *   S0  p(t;f) = CSD(t;f) / sigma          complex SNR map, Eq. 7
+ *   S1  template i -> 3 Bezier control points + delay, from Philox4x32-10(seed, i)
+ *                                            "six random numbers"
+ *   S2  Eq. 6 curve -> one frequency bin per time column (the cluster Gamma)
+ *
+ *   S3  SNR(i, tau) = N^-alpha * sum_Gamma Re[ e^{2 pi i f tau} p(t;f) ], Eq. 8
+ *
+ *   S4  max / argmax over (i, tau) and a histogram of all SNR(i, tau)
+ *
+ *
+ * Conventions
+ *   - plain C types only; every pointer is marked HOST or DEVICE below;
+ *   - the caller owns every buffer it passes; the library allocates no device
+ *     memory: the caller hands in one workspace (st_workspace_bytes / st_set_workspace);
+ *   - every call returns 0 (ST_OK) or a negative ST_E* code, never throws or aborts;
+ *     st_last_error() returns a message for the last failing call on that context;
+ *   - a context is bound to one CUDA stream and is not thread-safe;
+ *   - st_search / st_set_map_host are synchronous on return (they end with a
+ *     stream synchronisation); st_set_map and the debug calls are stream-ordered.
+ *   - there is NO CPU fallback: without a CUDA device every device call fails
+ *     with ST_ECUDA.
+ */
+#ifndef STOCHTRACK_H
+#define STOCHTRACK_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ST_OK       0
+#define ST_EINVAL  -1   /* bad argument                                   */
+#define ST_ESTATE  -2   /* search before workspace / map were set         */
+#define ST_ENOSPC  -3   /* workspace too small for the request            */
+#define ST_ECUDA   -4   /* CUDA runtime error (message in st_last_error)  */
+
+/* sigma layouts for st_set_map (Eq. 7: p = lambda sI* sJ, sigma = 1/lambda; G11) */
+#define ST_SIGMA_NONE      0   /* sigma == 1 everywhere, pointer ignored   */
+#define ST_SIGMA_PER_FREQ  1   /* float32 [n_f]                            */
+#define ST_SIGMA_PER_PIXEL 2   /* float32 [n_t][n_f]                       */
+
+/* delay modes (one random Delta tau per template; the grid mode
+ * scores every template against every trial delay, BASELINE.json north_star) */
+#define ST_TAU_GRID   0
+#define ST_TAU_RANDOM 1
+
+/* normalisation N^-alpha of Eq. 8 (G1): alpha = 1/2 gives a unit-variance
+ * statistic; alpha = 1 is Eq. 8 exactly as printed.           */
+#define ST_NORM_SQRT_N 0
+#define ST_NORM_MEAN   1
+
+/* scoring kernel selection (grid mode).  AUTO picks REINSCH when the grid is
+ * uniform and well conditioned, else ROTATION when uniform, else TABLE.       */
+#define ST_KERNEL_AUTO     0
+#define ST_KERNEL_TABLE    1   /* twiddle table W[k][m] read from L2, any grid          */
+#define ST_KERNEL_ROTATION 2   /* complex rotation recurrence along a uniform tau grid  */
+#define ST_KERNEL_REINSCH  3   /* real three-term (Reinsch) recurrence, uniform grid    */
+#define ST_KERNEL_RANDOM   4   /* reported in st_result for ST_TAU_RANDOM searches      */
+
+typedef struct st_ctx st_ctx;   /* opaque */
+
+/* One template: quadratic Bezier through P0 = (j0, y0),
+ * P1 = (j0 + a, y1), P2 = (j0 + N, y2); times in columns, frequencies in bins
+ * (bin k covers [k, k+1)); tau is the template's own delay in random mode.    */
+typedef struct {
+    int32_t N;      /* number of time columns = pixels in Gamma  */
+    int32_t j0;     /* first column                                             */
+    double  a;      /* t_mid - t_start in columns, 0 < a < N (G3)               */
+    double  y0, y1, y2;
+    double  tau;    /* seconds                                                  */
+} st_track;
+
+typedef struct {
+    uint64_t n_tracks;       /* T: templates scored, ids [track_offset, track_offset+T) */
+    uint64_t track_offset;   /* lets runs be combined exactly by max     */
+    uint64_t seed;           /* Philox key ("different random seed")       */
+    int32_t  n_min, n_max;   /* track duration range in columns, 1 <= n_min <= n_max <= n_t
+                                (the t_min constraint of PAPER.md:75)                   */
+    int32_t  tau_mode;       /* ST_TAU_GRID | ST_TAU_RANDOM                             */
+    int32_t  n_tau;          /* grid size (grid mode), ignored in random mode           */
+    const double *tau_grid;  /* HOST, n_tau delays in seconds (grid mode)               */
+    double   tau_lo, tau_hi; /* random mode: tau ~ U(tau_lo, tau_hi)     */
+    int32_t  norm;           /* ST_NORM_SQRT_N | ST_NORM_MEAN                           */
+    int32_t  n_bins;         /* histogram bins, 0 = no histogram, <= ST_MAX_BINS        */
+    double   hist_lo, hist_hi; /* bin = floor((snr-lo)/(hi-lo)*n_bins) clamped (G14)    */
+    uint64_t *hist_out;      /* HOST, n_bins counts (overwritten) or NULL               */
+    int32_t  kernel;         /* ST_KERNEL_* request (grid mode)                         */
+    int32_t  reserved;       /* must be 0                                               */
+} st_search_params;
+
+typedef struct {
+    float    max_snr;        /* largest float32 SNR(i, tau) the scoring kernel produced  */
+    int32_t  arg_tau_index;  /* grid index m of the argmax (0 in random mode)            */
+    double   max_snr_f64;    /* SNR of the argmax re-scored in float64 on the device     */
+    uint64_t arg_track;      /* template id of the argmax (G12 total order)              */
+    double   arg_tau;        /* its delay in seconds                                     */
+    st_track arg_params;     /* its control points                                       */
+    uint64_t n_evals;        /* sum_i N_i * n_tau  (track-pixel x delay evaluations)     */
+    uint64_t n_pixels;       /* sum_i N_i                                                */
+    int32_t  n_candidates;   /* near-max samples re-scored in float64                    */
+    int32_t  kernel_used;    /* ST_KERNEL_* actually launched                            */
+    int32_t  n_launches;     /* kernels launched by this call                            */
+    int32_t  flags;          /* bit 0: candidate list overflowed, argmax from float32    */
+    float    gpu_ms;         /* device time of the scoring launches (CUDA events)        */
+    float    reserved;
+} st_result;
+
+#define ST_MAX_BINS 4096
+#define ST_MAX_N_T  1048576
+#define ST_MAX_N_F  65535
+#define ST_MAX_N_TAU 4096
+
+/* Create a context for maps of n_t time columns x n_f frequency bins, bin k at
+ * frequency f_min + k*df [Hz] (G6).  HOST only, no CUDA call.
+ * Errors: ST_EINVAL unless 1<=n_t<=ST_MAX_N_T, 1<=n_f<=ST_MAX_N_F, df>0, f_min>=0. */
+int st_create(st_ctx **out, int32_t n_t, int32_t n_f, double df, double f_min);
+void st_destroy(st_ctx *ctx);
+
+/* Bytes of DEVICE workspace needed for searches with up to max_n_tau grid
+ * delays (0 on bad arguments).  Includes a staging area for st_set_map_host. */
+size_t st_workspace_bytes(const st_ctx *ctx, int32_t max_n_tau);
+
+/* Hand in the workspace (DEVICE, 256-byte aligned, caller-owned, must outlive the
+ * context's use) and the CUDA stream (cudaStream_t as void*, NULL = default
+ * stream) every later call is ordered on.  Errors: ST_ENOSPC, ST_EINVAL, ST_ECUDA. */
+int st_set_workspace(st_ctx *ctx, void *workspace_dev, size_t bytes, void *cuda_stream);
+
+/* S0 (Eq. 7): p = CSD / sigma into the workspace.  csd_dev: DEVICE
+ * complex64 [n_t][n_f] (frequency contiguous, interleaved re/im); sigma_dev: DEVICE
+ * float32 per sigma_kind.  sigma <= 0 or non-finite masks the pixel (p = 0, G11).
+ * Stream-ordered; inputs may be freed once the stream has passed the call.   */
+int st_set_map(st_ctx *ctx, const void *csd_dev, const float *sigma_dev, int32_t sigma_kind);
+
+/* Same with HOST buffers (pinned or pageable): copies them into the workspace
+ * staging area on the stream, then runs S0.  Synchronous on return.          */
+int st_set_map_host(st_ctx *ctx, const void *csd_host, const float *sigma_host, int32_t sigma_kind);
+
+/* S1-S4 over the current map.  Fills *out (HOST) and params->hist_out (HOST).
+ * Errors: ST_ESTATE (no workspace / map), ST_EINVAL, ST_ENOSPC (n_tau beyond the
+ * workspace), ST_ECUDA.                                                        */
+int st_search(st_ctx *ctx, const st_search_params *params, st_result *out);
+
+/* S1 as a pure HOST function: the control points of template `track_id`
+ * (same arithmetic as the device generator).                                   */
+int st_track_params(const st_ctx *ctx, uint64_t seed, uint64_t track_id,
+                    int32_t n_min, int32_t n_max, double tau_lo, double tau_hi, st_track *out);
+
+/* Parity exports (stream-ordered, outputs DEVICE).  Ids [first, first+count):
+ * k_out_dev int32 [count][n_t] (-1 beyond N), j0_dev / N_dev int32 [count].
+ * Uses params->seed, n_min, n_max.                                             */
+int st_debug_rasterise(st_ctx *ctx, const st_search_params *params, uint64_t first, uint64_t count,
+                       int32_t *k_out_dev, int32_t *j0_dev, int32_t *N_dev);
+/* Rasterise one explicit template (HOST st_track in, DEVICE int32 [N] out).    */
+int st_debug_rasterise_track(st_ctx *ctx, const st_track *track, int32_t *k_out_dev);
+/* snr_dev float32 [count][n_tau] (n_tau = 1 in random mode): every SNR(i, tau)
+ * the scoring kernel selected by params->kernel produces.                      */
+int st_debug_scores(st_ctx *ctx, const st_search_params *params, uint64_t first, uint64_t count,
+                    float *snr_dev);
+/* The 8 Philox words of a template (HOST out[8]); pure host function.          */
+int st_debug_track_words(uint64_t seed, uint64_t track_id, uint32_t *out_host);
+
+const char *st_last_error(const st_ctx *ctx);
+/* Library / build identification, e.g. "stochtrack-b200 sm_100a".              */
+const char *st_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STOCHTRACK_H */

@@ -1,0 +1,272 @@
+"""ctypes binding of include/stochtrack.h.  Marshalling only; PyTorch supplies
+device memory and the CUDA stream (nothing else)."""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libstochtrack_b200.so")
+
+ST_OK, ST_EINVAL, ST_ESTATE, ST_ENOSPC, ST_ECUDA = 0, -1, -2, -3, -4
+_CODES = {ST_EINVAL: "ST_EINVAL", ST_ESTATE: "ST_ESTATE", ST_ENOSPC: "ST_ENOSPC", ST_ECUDA: "ST_ECUDA"}
+SIGMA_NONE, SIGMA_PER_FREQ, SIGMA_PER_PIXEL = 0, 1, 2
+TAU_GRID, TAU_RANDOM = 0, 1
+NORM_SQRT_N, NORM_MEAN = 0, 1
+KERNEL_AUTO, KERNEL_TABLE, KERNEL_ROTATION, KERNEL_REINSCH, KERNEL_RANDOM = 0, 1, 2, 3, 4
+KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random"}
+
+# every symbol include/stochtrack.h declares
+exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_workspace", "st_set_map",
+                    "st_set_map_host", "st_search", "st_track_params", "st_debug_rasterise",
+                    "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words",
+                    "st_last_error", "st_version")
+
+
+class StError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{_CODES.get(code, code)}: {msg}")
+        self.code = code
+
+
+class CTrack(C.Structure):
+    _fields_ = [("N", C.c_int32), ("j0", C.c_int32), ("a", C.c_double), ("y0", C.c_double),
+                ("y1", C.c_double), ("y2", C.c_double), ("tau", C.c_double)]
+
+    def as_dict(self):
+        return {f: getattr(self, f) for f, _ in self._fields_}
+
+
+class CSearchParams(C.Structure):
+    _fields_ = [("n_tracks", C.c_uint64), ("track_offset", C.c_uint64), ("seed", C.c_uint64),
+                ("n_min", C.c_int32), ("n_max", C.c_int32), ("tau_mode", C.c_int32), ("n_tau", C.c_int32),
+                ("tau_grid", C.POINTER(C.c_double)), ("tau_lo", C.c_double), ("tau_hi", C.c_double),
+                ("norm", C.c_int32), ("n_bins", C.c_int32), ("hist_lo", C.c_double), ("hist_hi", C.c_double),
+                ("hist_out", C.POINTER(C.c_uint64)), ("kernel", C.c_int32), ("reserved", C.c_int32)]
+
+
+class CResult(C.Structure):
+    _fields_ = [("max_snr", C.c_float), ("arg_tau_index", C.c_int32), ("max_snr_f64", C.c_double),
+                ("arg_track", C.c_uint64), ("arg_tau", C.c_double), ("arg_params", CTrack),
+                ("n_evals", C.c_uint64), ("n_pixels", C.c_uint64), ("n_candidates", C.c_int32),
+                ("kernel_used", C.c_int32), ("n_launches", C.c_int32), ("flags", C.c_int32),
+                ("gpu_ms", C.c_float), ("reserved", C.c_float)]
+
+
+_lib = None
+
+
+def library_path():
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen the C-ABI library.  Fails loudly when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_1401_8060_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(_LIB_PATH)
+    vp = C.c_void_p
+    L.st_create.argtypes = [C.POINTER(vp), C.c_int32, C.c_int32, C.c_double, C.c_double]
+    L.st_destroy.argtypes = [vp]
+    L.st_destroy.restype = None
+    L.st_workspace_bytes.argtypes = [vp, C.c_int32]
+    L.st_workspace_bytes.restype = C.c_size_t
+    L.st_set_workspace.argtypes = [vp, vp, C.c_size_t, vp]
+    L.st_set_map.argtypes = [vp, vp, vp, C.c_int32]
+    L.st_set_map_host.argtypes = [vp, vp, vp, C.c_int32]
+    L.st_search.argtypes = [vp, C.POINTER(CSearchParams), C.POINTER(CResult)]
+    L.st_track_params.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_int32, C.c_int32, C.c_double, C.c_double,
+                                  C.POINTER(CTrack)]
+    L.st_debug_rasterise.argtypes = [vp, C.POINTER(CSearchParams), C.c_uint64, C.c_uint64, vp, vp, vp]
+    L.st_debug_rasterise_track.argtypes = [vp, C.POINTER(CTrack), vp]
+    L.st_debug_scores.argtypes = [vp, C.POINTER(CSearchParams), C.c_uint64, C.c_uint64, vp]
+    L.st_debug_track_words.argtypes = [C.c_uint64, C.c_uint64, C.POINTER(C.c_uint32)]
+    L.st_last_error.argtypes = [vp]
+    L.st_last_error.restype = C.c_char_p
+    L.st_version.argtypes = []
+    L.st_version.restype = C.c_char_p
+    for name in ("st_create", "st_set_workspace", "st_set_map", "st_set_map_host", "st_search", "st_track_params",
+                 "st_debug_rasterise", "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words"):
+        getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def st_track_words(seed, track_id):
+    out = (C.c_uint32 * 8)()
+    rc = load_library().st_debug_track_words(seed, track_id, out)
+    if rc:
+        raise StError(rc, "st_debug_track_words")
+    return np.array(list(out), dtype=np.uint32)
+
+
+class SearchResult(dict):
+    __getattr__ = dict.__getitem__
+
+
+class Stochtrack:
+    """One context = one map shape on one GPU / stream.  Mirrors the C ABI:
+    st_create / st_workspace_bytes / st_set_workspace at construction, then
+    set_map(), search(), and the parity exports."""
+
+    def __init__(self, n_t, n_f, df, f_min, max_n_tau=512, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the stochtrack hot path has no CPU fallback")
+        self._torch = torch
+        self._L = load_library()
+        self.n_t, self.n_f, self.df, self.f_min = int(n_t), int(n_f), float(df), float(f_min)
+        self.device = torch.device(device)
+        self._ctx = C.c_void_p()
+        rc = self._L.st_create(C.byref(self._ctx), self.n_t, self.n_f, self.df, self.f_min)
+        if rc:
+            raise StError(rc, "st_create: invalid map shape / frequency axis")
+        nbytes = self._L.st_workspace_bytes(self._ctx, int(max_n_tau))
+        if nbytes == 0:
+            raise StError(ST_EINVAL, "st_workspace_bytes: bad max_n_tau")
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.workspace_bytes = nbytes
+        self._check(self._L.st_set_workspace(self._ctx, self._ws.data_ptr(), nbytes, self._stream.cuda_stream))
+        self._keep = []
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self._L.st_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    __del__ = close
+
+    def _check(self, rc):
+        if rc:
+            raise StError(rc, (self._L.st_last_error(self._ctx) or b"").decode())
+
+    def synchronize(self):
+        self._stream.synchronize()
+
+    # ---------------------------------------------------------------- S0
+    def set_map(self, csd, sigma=None):
+        """csd: complex64 [n_t][n_f] torch CUDA tensor (device path) or numpy array /
+        CPU tensor (host path: copied inside the C call).  sigma: None, [n_f] or [n_t][n_f] float32."""
+        torch = self._torch
+        kind = SIGMA_NONE
+        if sigma is not None:
+            shp = tuple(sigma.shape)
+            kind = SIGMA_PER_FREQ if shp == (self.n_f,) else SIGMA_PER_PIXEL if shp == (self.n_t, self.n_f) else -1
+            if kind < 0:
+                raise ValueError("sigma must be None, [n_f] or [n_t][n_f]")
+        if tuple(csd.shape) != (self.n_t, self.n_f):
+            raise ValueError("csd must be [n_t][n_f]")
+        if isinstance(csd, torch.Tensor) and csd.is_cuda:
+            if csd.dtype != torch.complex64 or not csd.is_contiguous():
+                raise ValueError("csd must be a contiguous complex64 tensor")
+            sp = 0
+            if sigma is not None:
+                if not (isinstance(sigma, torch.Tensor) and sigma.is_cuda and sigma.dtype == torch.float32
+                        and sigma.is_contiguous()):
+                    raise ValueError("sigma must be a contiguous float32 CUDA tensor")
+                sp = sigma.data_ptr()
+            self._check(self._L.st_set_map(self._ctx, csd.data_ptr(), sp, kind))
+            self._keep = [csd, sigma]          # inputs must outlive the stream-ordered call
+        else:
+            c = csd.numpy() if isinstance(csd, torch.Tensor) else np.ascontiguousarray(csd, dtype=np.complex64)
+            s = None
+            if sigma is not None:
+                s = sigma.numpy() if isinstance(sigma, torch.Tensor) else np.ascontiguousarray(sigma, dtype=np.float32)
+            if c.dtype != np.complex64 or (s is not None and s.dtype != np.float32):
+                raise ValueError("host csd must be complex64 and sigma float32")
+            self._check(self._L.st_set_map_host(self._ctx, c.ctypes.data, s.ctypes.data if s is not None else 0, kind))
+
+    # ------------------------------------------------------------ S1-S4
+    def _params(self, n_tracks, seed, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
+                track_offset, kernel):
+        p = CSearchParams()
+        p.n_tracks, p.track_offset, p.seed = int(n_tracks), int(track_offset), int(seed)
+        p.n_min, p.n_max = int(n_min), int(n_max)
+        keep = []
+        if tau_grid is not None:
+            g = np.ascontiguousarray(tau_grid, dtype=np.float64)
+            keep.append(g)
+            p.tau_mode, p.n_tau = TAU_GRID, g.size
+            p.tau_grid = g.ctypes.data_as(C.POINTER(C.c_double))
+        else:
+            p.tau_mode, p.n_tau = TAU_RANDOM, 1
+            p.tau_lo, p.tau_hi = float(tau_range[0]), float(tau_range[1])
+        p.norm, p.n_bins = int(norm), int(n_bins)
+        p.hist_lo, p.hist_hi = float(hist_lo), float(hist_hi)
+        p.kernel = int(kernel)
+        return p, keep
+
+    def search(self, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=None, norm=NORM_SQRT_N,
+               n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO):
+        p, keep = self._params(n_tracks, seed, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
+                               track_offset, kernel)
+        hist = None
+        if n_bins > 0:
+            hist = np.zeros(n_bins, dtype=np.uint64)
+            p.hist_out = hist.ctypes.data_as(C.POINTER(C.c_uint64))
+        r = CResult()
+        self._check(self._L.st_search(self._ctx, C.byref(p), C.byref(r)))
+        return SearchResult(max_snr=float(r.max_snr), max_snr_f64=float(r.max_snr_f64), arg_track=int(r.arg_track),
+                            arg_tau_index=int(r.arg_tau_index), arg_tau=float(r.arg_tau),
+                            arg_params=r.arg_params.as_dict(), n_evals=int(r.n_evals), n_pixels=int(r.n_pixels),
+                            n_candidates=int(r.n_candidates), kernel_used=int(r.kernel_used),
+                            kernel_name=KERNEL_NAMES.get(int(r.kernel_used), "?"), n_launches=int(r.n_launches),
+                            flags=int(r.flags), gpu_ms=float(r.gpu_ms), hist=hist)
+
+    def track_params(self, seed, track_id, n_min, n_max, tau_lo=0.0, tau_hi=0.0):
+        t = CTrack()
+        self._check(self._L.st_track_params(self._ctx, seed, track_id, n_min, n_max, tau_lo, tau_hi, C.byref(t)))
+        return t
+
+    # ------------------------------------------------------ parity exports
+    def debug_rasterise(self, seed, n_min, n_max, first, count):
+        torch = self._torch
+        p, _ = self._params(count, seed, n_min, n_max, None, (0.0, 0.0), 0, 0, -10, 10, 0, 0)
+        k = torch.empty((count, self.n_t), dtype=torch.int32, device=self.device)
+        j0 = torch.empty(count, dtype=torch.int32, device=self.device)
+        N = torch.empty(count, dtype=torch.int32, device=self.device)
+        self._check(self._L.st_debug_rasterise(self._ctx, C.byref(p), int(first), int(count), k.data_ptr(),
+                                               j0.data_ptr(), N.data_ptr()))
+        self.synchronize()
+        return k.cpu().numpy(), j0.cpu().numpy(), N.cpu().numpy()
+
+    def debug_rasterise_track(self, N, j0, a, y0, y1, y2):
+        torch = self._torch
+        t = CTrack(int(N), int(j0), float(a), float(y0), float(y1), float(y2), 0.0)
+        k = torch.empty(int(N), dtype=torch.int32, device=self.device)
+        self._check(self._L.st_debug_rasterise_track(self._ctx, C.byref(t), k.data_ptr()))
+        self.synchronize()
+        return k.cpu().numpy()
+
+    def debug_scores(self, seed, n_min, n_max, first, count, tau_grid=None, tau_range=None, norm=NORM_SQRT_N,
+                     kernel=KERNEL_AUTO):
+        torch = self._torch
+        p, keep = self._params(count, seed, n_min, n_max, tau_grid, tau_range, norm, 0, -10, 10, first, kernel)
+        n_tau = p.n_tau if p.tau_mode == TAU_GRID else 1
+        snr = torch.empty((count, n_tau), dtype=torch.float32, device=self.device)
+        self._check(self._L.st_debug_scores(self._ctx, C.byref(p), int(first), int(count), snr.data_ptr()))
+        self.synchronize()
+        return snr.cpu().numpy()
+
+
+def st_track_params(n_t, n_f, seed, track_id, n_min, n_max, tau_lo=0.0, tau_hi=0.0, df=1.0, f_min=0.0):
+    """S1 as a pure host function (no GPU needed)."""
+    L = load_library()
+    ctx = C.c_void_p()
+    rc = L.st_create(C.byref(ctx), n_t, n_f, df, f_min)
+    if rc:
+        raise StError(rc, "st_create")
+    try:
+        t = CTrack()
+        rc = L.st_track_params(ctx, seed, track_id, n_min, n_max, tau_lo, tau_hi, C.byref(t))
+        if rc:
+            raise StError(rc, "st_track_params: invalid arguments")
+        return t
+    finally:
+        L.st_destroy(ctx)

@@ -1,0 +1,645 @@
+// st_kernels.cuh -- the sm_100a kernels of the all-sky stochtrack hot path.
+//
+//   k_prepare_map      S0  p = CSD / sigma                     Eq. 7
+//   k_build_w_table    twiddles W[k][m] = e^{2 pi i f_k tau_m}        (G6, G7)
+//   k_build_bin_tables per-bin constants of the uniform-grid recurrences
+//   k_score_table      S1-S4, any tau grid: lanes over tau, W read through L1/L2
+//   k_score_recur      S1-S4, uniform tau grid: lanes over pixels, the phase factor
+//                      advanced along tau by a recurrence in registers
+//   k_score_random     S1-S4, the paper's mode: one random delay per template
+//   k_finalize         S4: float64 re-score of the near-max candidates, argmax (G12)
+//   k_debug_rasterise  parity export of S1+S2
+//
+// One warp owns one template at a time (templates are independent: PAPER.md:25,
+// :242 "embarrassingly parallel").  No tensor cores: per template the sum of
+// Eq. 8 is a gather along the track, not a dense contraction.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "st_track.cuh"
+
+namespace st {
+
+constexpr int kWarp = 32;
+constexpr unsigned kFull = 0xFFFFFFFFu;
+constexpr double kTwoPi = 6.283185307179586476925286766559;
+
+struct Cand {            // a near-max sample kept for the float64 re-score
+    float snr;
+    uint32_t m;
+    uint64_t id;
+};
+
+struct WarpBest {        // per-warp best under the G12 total order (overflow fallback)
+    float snr;
+    uint32_t m;
+    uint64_t id;
+    uint32_t valid;
+    uint32_t pad;
+};
+
+struct Scalars {         // device scalars of one search, zeroed by the host
+    unsigned long long counter;     // next template index of the current launch
+    unsigned long long n_pixels;    // sum of N_i
+    uint32_t gmax_bits;             // ordered-uint encoding of the float32 maximum
+    uint32_t cand_count;
+    uint32_t overflow;
+    uint32_t pad;
+};
+
+struct DeviceResult {
+    float    max_snr;
+    int32_t  arg_m;
+    double   snr_f64;
+    uint64_t arg_id;
+    double   arg_tau;
+    Track    track;
+    int32_t  n_candidates;
+    int32_t  flags;
+    unsigned long long n_pixels;
+};
+
+struct ScoreArgs {
+    const float2* map;        // p[j * n_f + k]
+    BankParams bp;
+    double f_min, df;
+    uint64_t track_offset;    // id of template 0 of this launch
+    uint64_t n_tracks;        // templates in this launch
+    int32_t n_tau;
+    int32_t norm;
+    const float2* W;          // [n_f][n_tau]      (table kernel)
+    const float2* E0;         // [n_f] e^{2 pi i f_k tau_0}  (recurrence kernels)
+    const float4* bintab;     // [n_f] per-bin recurrence constants
+    Scalars* sc;
+    Cand* cand;
+    uint32_t cand_cap;
+    WarpBest* warp_best;
+    unsigned long long* hist; // [n_bins] global counts
+    int32_t n_bins;
+    float hist_lo, hist_scale;
+    float* dump;              // [n_tracks][n_tau] or null
+    int32_t pool_stride;      // pixels of pool space per warp (>= n_max, multiple of 32)
+};
+
+// ------------------------------------------------------------------ helpers --
+__device__ __forceinline__ uint32_t enc_f32(float f)
+{
+    const uint32_t b = __float_as_uint(f);
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float dec_f32(uint32_t e)
+{
+    return __uint_as_float((e & 0x80000000u) ? (e & 0x7FFFFFFFu) : ~e);
+}
+// Near-max margin: float32 SNRs within this distance of the running maximum are
+// kept and re-scored in float64 (G12).  Far above the float32 error of a score.
+__host__ __device__ __forceinline__ float near_margin(float mx)
+{
+    const float a = fabsf(mx);
+    return 5e-5f * (a > 1.0f ? a : 1.0f);
+}
+__device__ __forceinline__ bool better(float s, uint64_t id, uint32_t m,
+                                       float bs, uint64_t bid, uint32_t bm)
+{
+    if (s != bs) return s > bs;
+    if (id != bid) return id < bid;
+    return m < bm;
+}
+__host__ __device__ __forceinline__ float norm_scale(int32_t N, int32_t norm)
+{
+    // N^-alpha: alpha = 1/2 (G1 default) or 1 (Eq. 8 as printed)
+    return norm == 0 ? (float)(1.0 / sqrt((double)N)) : (float)(1.0 / (double)N);
+}
+
+// Per-warp reduction state (S4).
+struct WarpReduce {
+    float cached_max;      // last seen global float32 maximum
+    WarpBest best;
+    unsigned long long pixels;
+};
+
+__device__ __forceinline__ void reduce_init(WarpReduce& wr)
+{
+    wr.cached_max = -INFINITY;
+    wr.best.snr = -INFINITY; wr.best.m = 0; wr.best.id = 0; wr.best.valid = 0; wr.best.pad = 0;
+    wr.pixels = 0;
+}
+
+// Called by all 32 lanes with NV values per lane (sample (id, m[i]) = v[i], ignored
+// where !valid[i]).  Histogram + running max + near-max candidate capture.
+template <int NV>
+__device__ __forceinline__ void reduce_samples(const ScoreArgs& a, WarpReduce& wr, uint32_t* sm_hist,
+                                               uint64_t id, uint64_t q, const float (&v)[NV],
+                                               const uint32_t (&m)[NV], const bool (&valid)[NV])
+{
+    float lmax = -INFINITY;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        if (valid[i]) {
+            lmax = fmaxf(lmax, v[i]);
+            if (a.n_bins > 0) {
+                int b = __float2int_rd((v[i] - a.hist_lo) * a.hist_scale);
+                b = b < 0 ? 0 : (b >= a.n_bins ? a.n_bins - 1 : b);
+                atomicAdd(&sm_hist[b], 1u);
+            }
+            if (a.dump) a.dump[q * (uint64_t)a.n_tau + m[i]] = v[i];
+        }
+    }
+    float wmax = lmax;
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) wmax = fmaxf(wmax, __shfl_xor_sync(kFull, wmax, off));
+    if (wmax >= wr.cached_max - near_margin(wr.cached_max)) {
+        // slow path: this template comes within the margin of the global maximum
+        const int lane = threadIdx.x & 31;
+        uint32_t old = 0;
+        if (lane == 0) old = atomicMax(&a.sc->gmax_bits, enc_f32(wmax));
+        old = __shfl_sync(kFull, old, 0);
+        const float gm = fmaxf(dec_f32(old), wmax);
+        wr.cached_max = gm;
+        const float thr = gm - near_margin(gm);
+        const bool full = *(volatile uint32_t*)&a.sc->overflow != 0;
+        float bs = -INFINITY; uint32_t bm = 0;
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            if (valid[i] && v[i] >= thr) {
+                if (!full) {
+                    const uint32_t slot = atomicAdd(&a.sc->cand_count, 1u);
+                    if (slot < a.cand_cap) { Cand c; c.snr = v[i]; c.m = m[i]; c.id = id; a.cand[slot] = c; }
+                    else a.sc->overflow = 1u;
+                }
+                if (v[i] > bs || (v[i] == bs && m[i] < bm)) { bs = v[i]; bm = m[i]; }
+            }
+        }
+        // warp-wide best of this template under (snr desc, m asc), then against the warp's record
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) {
+            const float os = __shfl_xor_sync(kFull, bs, off);
+            const uint32_t om = __shfl_xor_sync(kFull, bm, off);
+            if (os > bs || (os == bs && om < bm)) { bs = os; bm = om; }
+        }
+        if (bs > -INFINITY && (!wr.best.valid || better(bs, id, bm, wr.best.snr, wr.best.id, wr.best.m))) {
+            wr.best.snr = bs; wr.best.m = bm; wr.best.id = id; wr.best.valid = 1;
+        }
+    }
+}
+
+__device__ __forceinline__ void reduce_finish(const ScoreArgs& a, WarpReduce& wr)
+{
+    const int lane = threadIdx.x & 31;
+    if (lane == 0) {
+        if (wr.pixels) atomicAdd(&a.sc->n_pixels, wr.pixels);
+        if (wr.best.valid) {
+            const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+            WarpBest cur = a.warp_best[gw];     // slot owned by this warp across launches
+            if (!cur.valid || better(wr.best.snr, wr.best.id, wr.best.m, cur.snr, cur.id, cur.m))
+                a.warp_best[gw] = wr.best;
+        }
+    }
+}
+
+__device__ __forceinline__ void hist_init(uint32_t* sm_hist, int n_bins)
+{
+    for (int b = threadIdx.x; b < n_bins; b += blockDim.x) sm_hist[b] = 0;
+    __syncthreads();
+}
+__device__ __forceinline__ void hist_flush(uint32_t* sm_hist, unsigned long long* hist, int n_bins)
+{
+    __syncthreads();
+    for (int b = threadIdx.x; b < n_bins; b += blockDim.x) {
+        const uint32_t c = sm_hist[b];
+        if (c) atomicAdd(&hist[b], (unsigned long long)c);
+    }
+}
+
+// Next template of the launch for this warp (dynamic: durations vary 100x).
+__device__ __forceinline__ uint64_t next_track(const ScoreArgs& a)
+{
+    unsigned long long q = 0;
+    if ((threadIdx.x & 31) == 0) q = atomicAdd(&a.sc->counter, 1ull);
+    return __shfl_sync(kFull, q, 0);
+}
+
+__device__ __forceinline__ uint32_t hist_smem_words(int n_bins) { return (uint32_t)((n_bins + 3) & ~3); }
+
+// ----------------------------------------------------------------------- S0 --
+// p = CSD / sigma (Eq. 7); sigma <= 0 or non-finite masks the pixel (G11).
+__global__ void k_prepare_map(const float2* __restrict__ csd, const float* __restrict__ sigma,
+                              int sigma_kind, int n_f, size_t n_pix, float2* __restrict__ p)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_pix;
+         i += (size_t)gridDim.x * blockDim.x) {
+        float2 c = csd[i];
+        if (sigma_kind != 0) {
+            const float s = sigma_kind == 1 ? sigma[i % (size_t)n_f] : sigma[i];
+            if (!(s > 0.0f) || isinf(s)) { c.x = 0.0f; c.y = 0.0f; }
+            else { c.x = __fdiv_rn(c.x, s); c.y = __fdiv_rn(c.y, s); }
+        }
+        p[i] = c;
+    }
+}
+
+// ------------------------------------------------------------------ twiddles --
+// W[k][m] = e^{2 pi i (f_min + k df) tau_m}, formed in float64, stored as float32
+// (cos, sin).  Sign as printed in Eq. 8 (G7); f is the bin frequency (G6).
+__global__ void k_build_w_table(const double* __restrict__ tau, int n_tau, int n_f,
+                                double f_min, double df, float2* __restrict__ W)
+{
+    const size_t n = (size_t)n_f * (size_t)n_tau;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (size_t)gridDim.x * blockDim.x) {
+        const int k = (int)(i / (size_t)n_tau), m = (int)(i % (size_t)n_tau);
+        const double cyc = (f_min + (double)k * df) * tau[m];
+        double s, c;
+        sincospi(2.0 * (cyc - rint(cyc)), &s, &c);
+        W[i] = make_float2((float)c, (float)s);
+    }
+}
+
+// Uniform grid tau_m = tau0 + m * dtau.  With theta_k = 2 pi f_k dtau:
+//   E0[k]     = e^{2 pi i f_k tau0}
+//   mode 0 (rotation): bintab[k] = (cos theta, sin theta, cos(CH theta), sin(CH theta))
+//   mode 1 (Reinsch):  bintab[k] = (4 sin^2(theta/2), sin theta, cos(CH theta), sin(CH theta))
+__global__ void k_build_bin_tables(double tau0, double dtau, int ch, int mode, int n_f,
+                                   double f_min, double df, float2* __restrict__ E0,
+                                   float4* __restrict__ bintab)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_f) return;
+    const double f = f_min + (double)k * df;
+    double s, c;
+    const double c0 = f * tau0;
+    sincospi(2.0 * (c0 - rint(c0)), &s, &c);
+    E0[k] = make_float2((float)c, (float)s);
+    double cyc = f * dtau;
+    cyc -= rint(cyc);                       // theta / 2 pi in [-1/2, 1/2]
+    double zs, zc, hs, hc, cs, cc;
+    sincospi(2.0 * cyc, &zs, &zc);
+    sincospi(cyc, &hs, &hc);                // sin(theta/2)
+    double cch = cyc * (double)ch;
+    cch -= rint(cch);
+    sincospi(2.0 * cch, &cs, &cc);
+    float4 t;
+    t.x = mode == 0 ? (float)zc : (float)(4.0 * hs * hs);
+    t.y = (float)zs;
+    t.z = (float)cc;
+    t.w = (float)cs;
+    bintab[k] = t;
+}
+
+// --------------------------------------------------- S1-S4, table, any grid --
+// Warp per template.  The warp rasterises the track (lanes over columns), parks
+// (p, k) of every pixel in its shared-memory pool, then lanes own delays: for each
+// block of 32 delays every lane walks the track in column order and accumulates
+// Re[W(k_c, m) p_c] in float32.
+__global__ void __launch_bounds__(256) k_score_table(const ScoreArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_warps = blockDim.x >> 5;
+    float2* pool_p = reinterpret_cast<float2*>(sm_hist + hist_smem_words(a.n_bins)) + (size_t)warp * a.pool_stride;
+    uint16_t* pool_k = reinterpret_cast<uint16_t*>(reinterpret_cast<float2*>(sm_hist + hist_smem_words(a.n_bins))
+                                                   + (size_t)n_warps * a.pool_stride) + (size_t)warp * a.pool_stride;
+    hist_init(sm_hist, a.n_bins);
+    WarpReduce wr;
+    reduce_init(wr);
+    for (;;) {
+        const uint64_t q = next_track(a);
+        if (q >= a.n_tracks) break;
+        const uint64_t id = a.track_offset + q;
+        const Track t = make_track(a.bp, id);
+        const Raster r = make_raster(t, a.bp.n_f);
+        for (int c = lane; c < t.N; c += kWarp) {
+            const int k = raster_bin(r, c);
+            pool_p[c] = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k]);
+            pool_k[c] = (uint16_t)k;
+        }
+        __syncwarp();
+        wr.pixels += (unsigned long long)t.N;
+        const float scale = norm_scale(t.N, a.norm);
+        for (int mb = 0; mb < a.n_tau; mb += kWarp) {
+            const int m = mb + lane;
+            const int mm = m < a.n_tau ? m : a.n_tau - 1;
+            const float2* Wm = a.W + mm;
+            float acc = 0.0f;
+#pragma unroll 4
+            for (int c = 0; c < t.N; ++c) {
+                const float2 p = pool_p[c];
+                const float2 w = __ldg(Wm + (size_t)pool_k[c] * (size_t)a.n_tau);
+                acc = fmaf(w.x, p.x, acc);
+                acc = fmaf(-w.y, p.y, acc);
+            }
+            const float v[1] = {acc * scale};
+            const uint32_t ms[1] = {(uint32_t)m};
+            const bool ok[1] = {m < a.n_tau};
+            reduce_samples<1>(a, wr, sm_hist, id, q, v, ms, ok);
+        }
+        __syncwarp();
+    }
+    reduce_finish(a, wr);
+    hist_flush(sm_hist, a.hist, a.n_bins);
+}
+
+// ----------------------------------------- S1-S4, the paper's random-tau mode --
+// One delay per template.  Lanes over columns; the phase
+// 2 pi f_k tau is reduced in float64 (f tau reaches 25 cycles), its sine and
+// cosine taken in float32; partial sums meet in a warp shuffle tree.
+__global__ void __launch_bounds__(256) k_score_random(const ScoreArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
+    const int lane = threadIdx.x & 31;
+    hist_init(sm_hist, a.n_bins);
+    WarpReduce wr;
+    reduce_init(wr);
+    for (;;) {
+        const uint64_t q = next_track(a);
+        if (q >= a.n_tracks) break;
+        const uint64_t id = a.track_offset + q;
+        const Track t = make_track(a.bp, id);
+        const Raster r = make_raster(t, a.bp.n_f);
+        float acc = 0.0f;
+#pragma unroll 2
+        for (int c = lane; c < t.N; c += kWarp) {
+            const int k = raster_bin(r, c);
+            const float2 p = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k]);
+            const double cyc = (a.f_min + (double)k * a.df) * t.tau;
+            float s, co;
+            sincospif(2.0f * (float)(cyc - rint(cyc)), &s, &co);
+            acc = fmaf(co, p.x, acc);
+            acc = fmaf(-s, p.y, acc);
+        }
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) acc += __shfl_xor_sync(kFull, acc, off);
+        wr.pixels += (unsigned long long)t.N;
+        const float v[1] = {acc * norm_scale(t.N, a.norm)};
+        const uint32_t ms[1] = {0u};
+        const bool ok[1] = {lane == 0};
+        reduce_samples<1>(a, wr, sm_hist, id, q, v, ms, ok);
+    }
+    reduce_finish(a, wr);
+    hist_flush(sm_hist, a.hist, a.n_bins);
+}
+
+// ------------------------------- S1-S4, uniform tau grid, recurrence along tau --
+// Warp per template, lanes over PIXELS.  Phase A rasterises the track and parks
+// v_c = p_c * e^{2 pi i f_k tau_0} (the term of Eq. 8 at the first delay) and k_c in
+// the warp's pool.  Phase B walks the delays in chunks of CH: a lane takes its
+// pixels two at a time, and advances each term along tau in registers,
+//   MODE 0 (rotation):  v <- v * e^{i theta_k}                     (4 flop + 1 add / eval)
+//   MODE 1 (Reinsch):   d <- d - 4 sin^2(theta_k/2) x ; x <- x + d (2 flop + 1 add / eval)
+// where x = Re v; both are exact identities for x_m = Re[p e^{2 pi i f (tau_0 + m dtau)}].
+// CH accumulators per lane hold the partial sums over that lane's pixels; a
+// transposing shuffle tree folds them across the warp, leaving CH/32 finished
+// delays per lane.  Anchors are re-derived every chunk from v_c * e^{i CH theta_k}
+// (tabulated from float64), so recurrence error never spans more than CH steps.
+template <int MODE, int CH, bool BT_SMEM>
+__global__ void __launch_bounds__(512, 1) k_score_recur(const ScoreArgs a)
+{
+    static_assert(CH == 32 || CH == 64, "chunk of 32 or 64 delays");
+    constexpr int NV = CH / 32;
+    extern __shared__ __align__(16) unsigned char smem[];
+    uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_warps = blockDim.x >> 5;
+    float4* sm_bt = reinterpret_cast<float4*>(sm_hist + hist_smem_words(a.n_bins));
+    float2* pools = reinterpret_cast<float2*>(sm_bt + (BT_SMEM ? a.bp.n_f : 0));
+    float2* pool_v = pools + (size_t)warp * a.pool_stride;
+    uint16_t* pool_k = reinterpret_cast<uint16_t*>(pools + (size_t)n_warps * a.pool_stride) + (size_t)warp * a.pool_stride;
+    if (BT_SMEM)
+        for (int k = threadIdx.x; k < a.bp.n_f; k += blockDim.x) sm_bt[k] = a.bintab[k];
+    hist_init(sm_hist, a.n_bins);   // includes __syncthreads
+    const float4* bt = BT_SMEM ? sm_bt : a.bintab;
+    const int n_chunks = (a.n_tau + CH - 1) / CH;
+    WarpReduce wr;
+    reduce_init(wr);
+    for (;;) {
+        const uint64_t q = next_track(a);
+        if (q >= a.n_tracks) break;
+        const uint64_t id = a.track_offset + q;
+        const Track t = make_track(a.bp, id);
+        const Raster r = make_raster(t, a.bp.n_f);
+        // ---- phase A: rasterise, gather, rotate to tau_0
+        const int n_pad = (t.N + 63) & ~63;          // pairs of 32-pixel rows
+#pragma unroll 2
+        for (int c = lane; c < n_pad; c += kWarp) {
+            float2 v = make_float2(0.0f, 0.0f);
+            int k = 0;
+            if (c < t.N) {
+                k = raster_bin(r, c);
+                const float2 p = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k]);
+                const float2 e = __ldg(&a.E0[k]);
+                v.x = p.x * e.x - p.y * e.y;
+                v.y = p.x * e.y + p.y * e.x;
+            }
+            pool_v[c] = v;
+            pool_k[c] = (uint16_t)k;
+        }
+        __syncwarp();
+        wr.pixels += (unsigned long long)t.N;
+        const float scale = norm_scale(t.N, a.norm);
+        // ---- phase B: chunks of CH delays
+        for (int j = 0; j < n_chunks; ++j) {
+            float acc[CH];
+#pragma unroll
+            for (int i = 0; i < CH; ++i) acc[i] = 0.0f;
+            for (int c = lane; c < n_pad; c += 2 * kWarp) {
+                const float2 v1 = pool_v[c], v2 = pool_v[c + kWarp];
+                const float4 b1 = bt[pool_k[c]], b2 = bt[pool_k[c + kWarp]];
+                // anchors of the next chunk: v * e^{i CH theta}
+                pool_v[c] = make_float2(v1.x * b1.z - v1.y * b1.w, v1.x * b1.w + v1.y * b1.z);
+                pool_v[c + kWarp] = make_float2(v2.x * b2.z - v2.y * b2.w, v2.x * b2.w + v2.y * b2.z);
+                if (MODE == 0) {
+                    float xr1 = v1.x, xi1 = v1.y, xr2 = v2.x, xi2 = v2.y;
+#pragma unroll
+                    for (int i = 0; i < CH; ++i) {
+                        acc[i] += xr1;
+                        acc[i] += xr2;
+                        const float nr1 = fmaf(xr1, b1.x, -(xi1 * b1.y));
+                        const float ni1 = fmaf(xr1, b1.y, xi1 * b1.x);
+                        const float nr2 = fmaf(xr2, b2.x, -(xi2 * b2.y));
+                        const float ni2 = fmaf(xr2, b2.y, xi2 * b2.x);
+                        xr1 = nr1; xi1 = ni1; xr2 = nr2; xi2 = ni2;
+                    }
+                } else {
+                    // x_m - x_{m-1} = 2 sin^2(theta/2) Re v - sin(theta) Im v
+                    float x1 = v1.x, d1 = fmaf(0.5f * b1.x, v1.x, -(b1.y * v1.y));
+                    float x2 = v2.x, d2 = fmaf(0.5f * b2.x, v2.x, -(b2.y * v2.y));
+#pragma unroll
+                    for (int i = 0; i < CH; ++i) {
+                        acc[i] += x1;
+                        acc[i] += x2;
+                        d1 = fmaf(-b1.x, x1, d1);
+                        d2 = fmaf(-b2.x, x2, d2);
+                        x1 += d1;
+                        x2 += d2;
+                    }
+                }
+            }
+            // ---- fold the CH partial sums across the 32 lanes (transposing tree):
+            // after the stage with offset `off` a lane keeps the half of the delays
+            // selected by that lane bit; lane l ends with delays NV*l .. NV*l + NV-1.
+#pragma unroll
+            for (int off = 16, n = CH / 2; off >= 1; off >>= 1, n >>= 1) {
+                const bool upper = (lane & off) != 0;
+#pragma unroll
+                for (int i = 0; i < n; ++i) {
+                    const float send = upper ? acc[i] : acc[i + n];
+                    const float keep = upper ? acc[i + n] : acc[i];
+                    acc[i] = keep + __shfl_xor_sync(kFull, send, off);
+                }
+            }
+            float v[NV]; uint32_t ms[NV]; bool ok[NV];
+#pragma unroll
+            for (int i = 0; i < NV; ++i) {
+                ms[i] = (uint32_t)(j * CH + NV * lane + i);
+                ok[i] = (int)ms[i] < a.n_tau;
+                v[i] = acc[i] * scale;
+            }
+            reduce_samples<NV>(a, wr, sm_hist, id, q, v, ms, ok);
+            __syncwarp();
+        }
+    }
+    reduce_finish(a, wr);
+    hist_flush(sm_hist, a.hist, a.n_bins);
+}
+
+// ----------------------------------------------------------------------- S4 --
+// Float64 score of one (template, delay): Eq. 8 with cos/sin of 2 pi f tau in
+// double, lanes over columns, fixed-order shuffle tree.  All lanes return it.
+__device__ __forceinline__ double score_f64(const float2* __restrict__ map, const BankParams& bp,
+                                            double f_min, double df, const Track& t, double tau, int norm)
+{
+    const int lane = threadIdx.x & 31;
+    const Raster r = make_raster(t, bp.n_f);
+    double acc = 0.0;
+    for (int c = lane; c < t.N; c += kWarp) {
+        const int k = raster_bin(r, c);
+        const float2 p = map[(size_t)(t.j0 + c) * (size_t)bp.n_f + (size_t)k];
+        const double phi = kTwoPi * (f_min + (double)k * df) * tau;
+        double s, co;
+        sincos(phi, &s, &co);
+        acc += co * (double)p.x - s * (double)p.y;
+    }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) acc += __shfl_xor_sync(kFull, acc, off);
+    return acc / (norm == 0 ? sqrt((double)t.N) : (double)t.N);
+}
+
+struct FinalArgs {
+    const float2* map;
+    BankParams bp;
+    double f_min, df;
+    int32_t norm, tau_mode, n_tau;
+    const double* tau_d;       // device grid (grid mode)
+    const Scalars* sc;
+    const Cand* cand;
+    uint32_t cand_cap;
+    const WarpBest* warp_best;
+    uint32_t n_warp_slots;
+    DeviceResult* out;
+};
+
+// One block.  Near-max candidates (float32 SNR within the margin of the float32
+// maximum) are re-scored in float64; the answer is the best under the G12 total
+// order (larger SNR, then smaller template id, then smaller delay index).  If the
+// candidate list overflowed (degenerate maps with massive ties) the per-warp
+// float32 records decide instead and flags bit 0 is set.
+__global__ void __launch_bounds__(256) k_finalize(const FinalArgs a)
+{
+    __shared__ double s_snr[8];
+    __shared__ uint64_t s_id[8];
+    __shared__ uint32_t s_m[8];
+    __shared__ int s_valid[8];
+    __shared__ float s_f32[8];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+    const float gmax = dec_f32(a.sc->gmax_bits);
+    const uint32_t n_cand = a.sc->cand_count < a.cand_cap ? a.sc->cand_count : a.cand_cap;
+    const bool overflow = a.sc->overflow != 0 || a.sc->cand_count > a.cand_cap;
+    double best = 0.0; uint64_t bid = 0; uint32_t bm = 0; int have = 0; float bf32 = 0.0f;
+    int n_scored = 0;
+    if (!overflow) {
+        const float thr = gmax - near_margin(gmax);
+        for (uint32_t i = warp; i < n_cand; i += n_warps) {
+            const Cand c = a.cand[i];
+            if (!(c.snr >= thr)) continue;
+            const Track t = make_track(a.bp, c.id);
+            const double tau = a.tau_mode == 0 ? a.tau_d[c.m] : t.tau;
+            const double s = score_f64(a.map, a.bp, a.f_min, a.df, t, tau, a.norm);
+            ++n_scored;
+            if (!have || s > best || (s == best && (c.id < bid || (c.id == bid && c.m < bm)))) {
+                have = 1; best = s; bid = c.id; bm = c.m; bf32 = c.snr;
+            }
+        }
+    } else {
+        // float32 records: every lane scans a slice, warp-reduce, one re-score at the end
+        float fs = -INFINITY; uint64_t fid = 0; uint32_t fm = 0; int fh = 0;
+        for (uint32_t i = threadIdx.x; i < a.n_warp_slots; i += blockDim.x) {
+            const WarpBest w = a.warp_best[i];
+            if (w.valid && (!fh || better(w.snr, w.id, w.m, fs, fid, fm))) { fh = 1; fs = w.snr; fid = w.id; fm = w.m; }
+        }
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) {
+            const float os = __shfl_xor_sync(kFull, fs, off);
+            const uint64_t oid = __shfl_xor_sync(kFull, fid, off);
+            const uint32_t om = __shfl_xor_sync(kFull, fm, off);
+            const int oh = __shfl_xor_sync(kFull, fh, off);
+            if (oh && (!fh || better(os, oid, om, fs, fid, fm))) { fh = 1; fs = os; fid = oid; fm = om; }
+        }
+        // carried as (float32 snr promoted) so that the block reduce below keeps float32 order
+        if (fh) { have = 1; best = (double)fs; bid = fid; bm = fm; bf32 = fs; }
+    }
+    if (lane == 0) { s_snr[warp] = best; s_id[warp] = bid; s_m[warp] = bm; s_valid[warp] = have; s_f32[warp] = bf32; }
+    __shared__ int s_nscored[8];
+    if (lane == 0) s_nscored[warp] = n_scored;
+    __syncthreads();
+    if (warp == 0) {
+        have = 0;
+        int total = 0;
+        for (int w = 0; w < n_warps; ++w) {
+            total += s_nscored[w];
+            if (!s_valid[w]) continue;
+            if (!have || s_snr[w] > best || (s_snr[w] == best && (s_id[w] < bid || (s_id[w] == bid && s_m[w] < bm)))) {
+                have = 1; best = s_snr[w]; bid = s_id[w]; bm = s_m[w]; bf32 = s_f32[w];
+            }
+        }
+        DeviceResult res;
+        res.max_snr = gmax; res.arg_m = 0; res.snr_f64 = 0.0; res.arg_id = 0; res.arg_tau = 0.0;
+        res.track.N = 0; res.track.j0 = 0; res.track.a = res.track.y0 = res.track.y1 = res.track.y2 = res.track.tau = 0.0;
+        res.n_candidates = total; res.flags = overflow ? 1 : 0; res.n_pixels = a.sc->n_pixels;
+        if (have) {
+            const Track t = make_track(a.bp, bid);
+            const double tau = a.tau_mode == 0 ? a.tau_d[bm] : t.tau;
+            const double s = overflow ? score_f64(a.map, a.bp, a.f_min, a.df, t, tau, a.norm) : best;
+            res.arg_m = (int32_t)bm; res.snr_f64 = s; res.arg_id = bid; res.arg_tau = tau; res.track = t;
+            if (overflow) res.n_candidates = 1;
+        }
+        if (lane == 0) *a.out = res;
+    }
+}
+
+// ------------------------------------------------------------- parity export --
+// S1 + S2 for ids [first, first + count): k_out[q][c] (-1 beyond N), j0, N.
+__global__ void k_debug_rasterise(BankParams bp, uint64_t first, uint64_t count, int32_t* __restrict__ k_out,
+                                  int32_t* __restrict__ j0_out, int32_t* __restrict__ N_out)
+{
+    const int lane = threadIdx.x & 31;
+    const uint64_t gw = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const uint64_t n_w = ((uint64_t)gridDim.x * blockDim.x) >> 5;
+    for (uint64_t q = gw; q < count; q += n_w) {
+        const Track t = make_track(bp, first + q);
+        const Raster r = make_raster(t, bp.n_f);
+        int32_t* row = k_out + q * (uint64_t)bp.n_t;
+        for (int c = lane; c < bp.n_t; c += kWarp) row[c] = c < t.N ? raster_bin(r, c) : -1;
+        if (lane == 0) { j0_out[q] = t.j0; N_out[q] = t.N; }
+    }
+}
+
+__global__ void k_debug_rasterise_track(Track t, int32_t n_f, int32_t* __restrict__ k_out)
+{
+    const Raster r = make_raster(t, n_f);
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < t.N; c += gridDim.x * blockDim.x)
+        k_out[c] = raster_bin(r, c);
+}
+
+}  // namespace st

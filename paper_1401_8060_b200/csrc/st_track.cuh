@@ -1,0 +1,147 @@
+// st_track.cuh -- S1 (template generation) and S2 (rasterisation) of the hot path.
+//
+// S1: PAPER.md:75, :86 ("each template can be quickly generated from just six
+//     random numbers"), :100 (Delta tau ~ U(+-Delta tau_max)); readings G3-G5 of DESIGN.md.
+// S2: PAPER.md:83 (Eq. 6), :73 (N = pixels in Gamma); readings G2, G15.
+//
+// Everything here is __host__ __device__ so that st_track_params (host, pure)
+// and the kernels share one statement of the arithmetic.  The rasteriser is a
+// fixed sequence of single IEEE-754 double operations: on the device every
+// operation is a *_rn intrinsic (never contracted into an FMA); on the host the
+// file is compiled with -ffp-contract=off.
+#pragma once
+#include <stdint.h>
+#include <math.h>
+
+#if defined(__CUDA_ARCH__)
+#define ST_DMUL(x, y) __dmul_rn((x), (y))
+#define ST_DADD(x, y) __dadd_rn((x), (y))
+#define ST_DSUB(x, y) __dsub_rn((x), (y))
+#define ST_DDIV(x, y) __ddiv_rn((x), (y))
+#define ST_DSQRT(x)   __dsqrt_rn((x))
+#define ST_MULHI(x, y) __umulhi((x), (y))
+#else
+#define ST_DMUL(x, y) ((x) * (y))
+#define ST_DADD(x, y) ((x) + (y))
+#define ST_DSUB(x, y) ((x) - (y))
+#define ST_DDIV(x, y) ((x) / (y))
+#define ST_DSQRT(x)   sqrt((x))
+#define ST_MULHI(x, y) ((uint32_t)(((uint64_t)(x) * (uint64_t)(y)) >> 32))
+#endif
+
+#define ST_HD __host__ __device__ __forceinline__
+
+namespace st {
+
+// Domain tag of the template stream: fourth Philox counter word (G5).
+constexpr uint32_t kTrackTag = 0x5354524Bu;  // "STRK"
+
+struct Words8 { uint32_t r[8]; };
+
+// Philox4x32-10 (Salmon et al., SC'11): ten rounds of two 32x32->64 multiplies
+// with xor of the neighbouring word and the round key; key += Weyl constants.
+ST_HD void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                         uint32_t k0, uint32_t k1, uint32_t* out)
+{
+    constexpr uint32_t kMulA = 0xD2511F53u, kMulB = 0xCD9E8D57u;
+    constexpr uint32_t kWeylA = 0x9E3779B9u, kWeylB = 0xBB67AE85u;
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        const uint32_t hiA = ST_MULHI(kMulA, c0), loA = kMulA * c0;
+        const uint32_t hiB = ST_MULHI(kMulB, c2), loB = kMulB * c2;
+        c0 = hiB ^ c1 ^ k0;
+        c1 = loB;
+        c2 = hiA ^ c3 ^ k1;
+        c3 = loA;
+        k0 += kWeylA;
+        k1 += kWeylB;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// The eight words of template `id`: counter (id_lo, id_hi, b, tag), b = 0, 1.
+ST_HD Words8 track_words(uint64_t seed, uint64_t id)
+{
+    Words8 w;
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    const uint32_t i0 = (uint32_t)id, i1 = (uint32_t)(id >> 32);
+    philox4x32_10(i0, i1, 0u, kTrackTag, k0, k1, w.r);
+    philox4x32_10(i0, i1, 1u, kTrackTag, k0, k1, w.r + 4);
+    return w;
+}
+
+struct Track {
+    int32_t N, j0;
+    double a, y0, y1, y2, tau;
+};
+
+struct BankParams {       // what S1 needs besides (seed, id)
+    uint64_t seed;
+    int32_t n_t, n_f, n_min, n_max;
+    double tau_lo, tau_hi;
+};
+
+// S1.  N uniform in [n_min, n_max]; first column uniform among the feasible
+// ones; t_mid strictly inside (t_start, t_end); three frequency control points
+// uniform over the band; tau uniform in (tau_lo, tau_hi).  The (r + 1/2) * n *
+// 2^-32 products are exact in double (n < 2^20).
+ST_HD Track make_track(const BankParams& bp, uint64_t id)
+{
+    const Words8 w = track_words(bp.seed, id);
+    constexpr double kTwoM32 = 1.0 / 4294967296.0;
+    Track t;
+    t.N  = bp.n_min + (int32_t)ST_MULHI(w.r[0], (uint32_t)(bp.n_max - bp.n_min + 1));
+    t.j0 = (int32_t)ST_MULHI(w.r[1], (uint32_t)(bp.n_t - t.N + 1));
+    const double dN = (double)t.N, dF = (double)bp.n_f;
+    t.a  = ST_DMUL(ST_DMUL((double)w.r[2] + 0.5, dN), kTwoM32);
+    t.y0 = ST_DMUL(ST_DMUL((double)w.r[3] + 0.5, dF), kTwoM32);
+    t.y1 = ST_DMUL(ST_DMUL((double)w.r[4] + 0.5, dF), kTwoM32);
+    t.y2 = ST_DMUL(ST_DMUL((double)w.r[5] + 0.5, dF), kTwoM32);
+    const double u = ST_DMUL((double)w.r[6] + 0.5, kTwoM32);
+    t.tau = ST_DADD(bp.tau_lo, ST_DMUL(ST_DSUB(bp.tau_hi, bp.tau_lo), u));
+    return t;
+}
+
+// Per-track constants of S2.
+struct Raster {
+    double a, cc, aa, y0, y1, y2;
+    int32_t kmax;
+};
+
+ST_HD Raster make_raster(const Track& t, int32_t n_f)
+{
+    Raster r;
+    r.a  = t.a;
+    r.cc = ST_DSUB((double)t.N, ST_DMUL(2.0, t.a));   // N - 2a
+    r.aa = ST_DMUL(t.a, t.a);
+    r.y0 = t.y0; r.y1 = t.y1; r.y2 = t.y2;
+    r.kmax = n_f - 1;
+    return r;
+}
+
+// S2 for column c of the track: the Bezier time polynomial t(xi) - j0 =
+// (N - 2a) xi^2 + 2a xi is solved at the column centre u = c + 1/2 with the
+// cancellation-free root xi = u / (a + sqrt(a^2 + (N-2a) u)); f(xi) follows
+// Eq. 6 and is floored to a bin.
+ST_HD int32_t raster_bin(const Raster& r, int32_t c)
+{
+    const double u   = (double)c + 0.5;
+    double D         = ST_DADD(r.aa, ST_DMUL(r.cc, u));
+    D                = D < 0.0 ? 0.0 : D;
+    const double s   = ST_DSQRT(D);
+    const double den = ST_DADD(r.a, s);
+    const double xi  = ST_DDIV(u, den);
+    const double om  = ST_DSUB(1.0, xi);
+    const double b0  = ST_DMUL(om, om);
+    const double b1  = ST_DMUL(2.0, ST_DMUL(om, xi));
+    const double b2  = ST_DMUL(xi, xi);
+    const double y   = ST_DADD(ST_DADD(ST_DMUL(b0, r.y0), ST_DMUL(b1, r.y1)), ST_DMUL(b2, r.y2));
+    const double fl  = floor(y);
+    int32_t k;
+    if (!(fl >= 0.0)) k = 0;
+    else if (fl > (double)r.kmax) k = r.kmax;
+    else k = (int32_t)fl;
+    return k;
+}
+
+}  // namespace st

@@ -1,0 +1,584 @@
+// stochtrack_api.cu -- the C ABI of include/stochtrack.h over the kernels of
+// st_kernels.cuh.  Host logic only: validation, workspace layout, twiddle-table
+// caching, kernel selection and launch, result copy-back.  No device memory is
+// allocated here (the caller's workspace is carved up); the only allocations are
+// a few KB of pinned host memory for results and two CUDA events per context.
+#include <cuda_runtime.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <math.h>
+#include <vector>
+#include <new>
+
+#include "../../include/stochtrack.h"
+#include "st_kernels.cuh"
+
+namespace {
+
+constexpr size_t kAlign = 256;
+constexpr uint32_t kCandCap = 1u << 16;
+constexpr uint32_t kWarpSlots = 1u << 14;
+constexpr uint64_t kMaxSamplesPerLaunch = 1ull << 31;   // keeps per-block u32 histogram bins exact
+
+size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {
+    size_t map, e0, bintab, w, tau, hist, scalars, result, cand, warp_best, stage_csd, stage_sigma, total;
+};
+
+Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
+{
+    const size_t n_pix = (size_t)n_t * (size_t)n_f;
+    Layout L;
+    size_t o = 0;
+    L.map = o;         o += align_up(n_pix * sizeof(float2));
+    L.e0 = o;          o += align_up((size_t)n_f * sizeof(float2));
+    L.bintab = o;      o += align_up((size_t)n_f * sizeof(float4));
+    L.w = o;           o += align_up((size_t)n_f * (size_t)max_n_tau * sizeof(float2));
+    L.tau = o;         o += align_up((size_t)max_n_tau * sizeof(double));
+    L.hist = o;        o += align_up((size_t)ST_MAX_BINS * sizeof(unsigned long long));
+    L.scalars = o;     o += align_up(sizeof(st::Scalars));
+    L.result = o;      o += align_up(sizeof(st::DeviceResult));
+    L.cand = o;        o += align_up((size_t)kCandCap * sizeof(st::Cand));
+    L.warp_best = o;   o += align_up((size_t)kWarpSlots * sizeof(st::WarpBest));
+    L.stage_csd = o;   o += align_up(n_pix * sizeof(float2));
+    L.stage_sigma = o; o += align_up(n_pix * sizeof(float));
+    L.total = o;
+    return L;
+}
+
+enum TableKind { kNoTable = 0, kWTable = 1, kRotTable = 2, kReinschTable = 3 };
+
+}  // namespace
+
+struct st_ctx {
+    int32_t n_t, n_f;
+    double df, f_min;
+    unsigned char* ws;
+    size_t ws_bytes;
+    int32_t max_n_tau;
+    Layout L;
+    cudaStream_t stream;
+    bool have_ws, have_map;
+    std::vector<double> tau_cached;    // grid currently on the device
+    int table_kind, table_ch;          // which tables are currently built for tau_cached
+    bool w_built;
+    cudaEvent_t ev0, ev1;
+    st::DeviceResult* h_res;           // pinned
+    unsigned long long* h_hist;        // pinned, ST_MAX_BINS
+    int n_sm, smem_optin;
+    int recur_threads;                 // tunable: threads per block of k_score_recur
+    char err[512];
+};
+
+namespace {
+
+int fail(st_ctx* c, int code, const char* fmt, ...)
+{
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define ST_CUDA(ctx, call)                                                                   \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess)                                                               \
+            return fail((ctx), ST_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));           \
+    } while (0)
+
+template <typename T>
+T* at(st_ctx* c, size_t off) { return reinterpret_cast<T*>(c->ws + off); }
+
+st::BankParams bank(const st_ctx* c, const st_search_params* p)
+{
+    st::BankParams bp;
+    bp.seed = p->seed;
+    bp.n_t = c->n_t; bp.n_f = c->n_f; bp.n_min = p->n_min; bp.n_max = p->n_max;
+    bp.tau_lo = p->tau_mode == ST_TAU_RANDOM ? p->tau_lo : 0.0;
+    bp.tau_hi = p->tau_mode == ST_TAU_RANDOM ? p->tau_hi : 0.0;
+    return bp;
+}
+
+int validate(st_ctx* c, const st_search_params* p, bool need_map)
+{
+    if (!c) return ST_EINVAL;
+    if (!p) return fail(c, ST_EINVAL, "params is NULL");
+    if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
+    if (need_map && !c->have_map) return fail(c, ST_ESTATE, "no map: call st_set_map first");
+    if (p->n_min < 1 || p->n_max < p->n_min || p->n_max > c->n_t)
+        return fail(c, ST_EINVAL, "need 1 <= n_min <= n_max <= n_t (got %d, %d, n_t %d)", p->n_min, p->n_max, c->n_t);
+    if (p->tau_mode != ST_TAU_GRID && p->tau_mode != ST_TAU_RANDOM) return fail(c, ST_EINVAL, "bad tau_mode %d", p->tau_mode);
+    if (p->tau_mode == ST_TAU_GRID) {
+        if (p->n_tau < 1 || p->n_tau > ST_MAX_N_TAU) return fail(c, ST_EINVAL, "n_tau %d outside [1, %d]", p->n_tau, ST_MAX_N_TAU);
+        if (p->n_tau > c->max_n_tau) return fail(c, ST_ENOSPC, "n_tau %d exceeds the workspace's max_n_tau %d", p->n_tau, c->max_n_tau);
+        if (!p->tau_grid) return fail(c, ST_EINVAL, "tau_grid is NULL");
+        for (int m = 0; m < p->n_tau; ++m)
+            if (!isfinite(p->tau_grid[m])) return fail(c, ST_EINVAL, "tau_grid[%d] is not finite", m);
+    } else {
+        if (!isfinite(p->tau_lo) || !isfinite(p->tau_hi) || p->tau_hi < p->tau_lo)
+            return fail(c, ST_EINVAL, "bad random-tau range");
+    }
+    if (p->norm != ST_NORM_SQRT_N && p->norm != ST_NORM_MEAN) return fail(c, ST_EINVAL, "bad norm %d", p->norm);
+    if (p->n_bins < 0 || p->n_bins > ST_MAX_BINS) return fail(c, ST_EINVAL, "n_bins %d outside [0, %d]", p->n_bins, ST_MAX_BINS);
+    if (p->n_bins > 0 && !(p->hist_hi > p->hist_lo)) return fail(c, ST_EINVAL, "need hist_hi > hist_lo");
+    if (p->kernel < ST_KERNEL_AUTO || p->kernel > ST_KERNEL_REINSCH) return fail(c, ST_EINVAL, "bad kernel %d", p->kernel);
+    if (p->reserved != 0) return fail(c, ST_EINVAL, "reserved must be 0");
+    if (p->n_tracks > (1ull << 62) || p->track_offset > (1ull << 62)) return fail(c, ST_EINVAL, "n_tracks / track_offset too large");
+    return ST_OK;
+}
+
+// Is the grid tau_0 + m * dtau to within a phase error of 1e-8 rad at the top of the band?
+bool grid_uniform(const st_ctx* c, const double* tau, int n, double* tau0, double* dtau)
+{
+    *tau0 = tau[0];
+    *dtau = n > 1 ? (tau[n - 1] - tau[0]) / (double)(n - 1) : 0.0;
+    const double f_top = c->f_min + c->df * (double)(c->n_f - 1);
+    const double tol = 1e-8 / (st::kTwoPi * (f_top > 1.0 ? f_top : 1.0));
+    for (int m = 0; m < n; ++m)
+        if (fabs(tau[m] - (*tau0 + (double)m * *dtau)) > tol) return false;
+    return true;
+}
+
+// The three-term recurrence amplifies rounding by 1/|sin theta|: refuse it when a
+// bin's step angle theta_k = 2 pi f_k dtau (mod 2 pi) comes within 0.1 rad of pi.
+bool reinsch_well_conditioned(const st_ctx* c, double dtau)
+{
+    for (int k = 0; k < c->n_f; ++k) {
+        double cyc = (c->f_min + (double)k * c->df) * dtau;
+        cyc -= rint(cyc);                               // [-1/2, 1/2]
+        if (0.5 - fabs(cyc) < 0.1 / st::kTwoPi) return false;
+    }
+    return true;
+}
+
+int pick_chunk(int n_tau)
+{
+    const int pad32 = (n_tau + 31) / 32 * 32, pad64 = (n_tau + 63) / 64 * 64;
+    return pad32 < pad64 ? 32 : 64;
+}
+
+struct Plan {
+    int kernel;       // ST_KERNEL_*
+    int ch;           // recurrence chunk
+    double tau0, dtau;
+};
+
+int make_plan(st_ctx* c, const st_search_params* p, Plan* plan)
+{
+    plan->ch = 0; plan->tau0 = 0.0; plan->dtau = 0.0;
+    if (p->tau_mode == ST_TAU_RANDOM) { plan->kernel = ST_KERNEL_RANDOM; return ST_OK; }
+    const bool uni = grid_uniform(c, p->tau_grid, p->n_tau, &plan->tau0, &plan->dtau);
+    int k = p->kernel;
+    if (k == ST_KERNEL_AUTO) {
+        if (!uni || p->n_tau < 8) k = ST_KERNEL_TABLE;
+        else k = reinsch_well_conditioned(c, plan->dtau) ? ST_KERNEL_REINSCH : ST_KERNEL_ROTATION;
+    }
+    if ((k == ST_KERNEL_ROTATION || k == ST_KERNEL_REINSCH) && !uni)
+        return fail(c, ST_EINVAL, "recurrence kernels need a uniform tau grid");
+    plan->kernel = k;
+    if (k != ST_KERNEL_TABLE) plan->ch = pick_chunk(p->n_tau);
+    return ST_OK;
+}
+
+// Upload the grid and (re)build whichever twiddle tables the plan needs.
+int ensure_tables(st_ctx* c, const st_search_params* p, const Plan& plan, int* n_launches)
+{
+    if (p->tau_mode != ST_TAU_GRID) return ST_OK;
+    const bool same_grid = (int)c->tau_cached.size() == p->n_tau &&
+                           memcmp(c->tau_cached.data(), p->tau_grid, sizeof(double) * (size_t)p->n_tau) == 0;
+    if (!same_grid) {
+        c->tau_cached.assign(p->tau_grid, p->tau_grid + p->n_tau);
+        c->table_kind = kNoTable; c->w_built = false;
+        ST_CUDA(c, cudaMemcpyAsync(at<double>(c, c->L.tau), c->tau_cached.data(), sizeof(double) * (size_t)p->n_tau,
+                                   cudaMemcpyHostToDevice, c->stream));
+    }
+    if (plan.kernel == ST_KERNEL_TABLE) {
+        if (!c->w_built) {
+            const size_t n = (size_t)c->n_f * (size_t)p->n_tau;
+            const int blocks = (int)((n + 255) / 256 < 4096 ? (n + 255) / 256 : 4096);
+            st::k_build_w_table<<<blocks, 256, 0, c->stream>>>(at<double>(c, c->L.tau), p->n_tau, c->n_f, c->f_min, c->df,
+                                                                at<float2>(c, c->L.w));
+            ST_CUDA(c, cudaGetLastError());
+            c->w_built = true; ++*n_launches;
+        }
+    } else {
+        const int want = plan.kernel == ST_KERNEL_ROTATION ? kRotTable : kReinschTable;
+        if (c->table_kind != want || c->table_ch != plan.ch) {
+            st::k_build_bin_tables<<<(c->n_f + 127) / 128, 128, 0, c->stream>>>(
+                plan.tau0, plan.dtau, plan.ch, want == kRotTable ? 0 : 1, c->n_f, c->f_min, c->df,
+                at<float2>(c, c->L.e0), at<float4>(c, c->L.bintab));
+            ST_CUDA(c, cudaGetLastError());
+            c->table_kind = want; c->table_ch = plan.ch; ++*n_launches;
+        }
+    }
+    return ST_OK;
+}
+
+template <typename K>
+int set_smem(st_ctx* c, K kernel, size_t bytes)
+{
+    if (bytes > 48 * 1024)
+        ST_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return ST_OK;
+}
+
+size_t hist_bytes(int n_bins) { return (size_t)((n_bins + 3) & ~3) * sizeof(uint32_t); }
+
+// Launch the scoring kernel of the plan on templates [a.track_offset, +a.n_tracks).
+int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
+{
+    const int stride = (n_max + 63) & ~63;
+    a.pool_stride = stride;
+    const uint64_t want_warps = a.n_tracks;
+    ST_CUDA(c, cudaMemsetAsync(&a.sc->counter, 0, sizeof(unsigned long long), c->stream));
+    if (plan.kernel == ST_KERNEL_RANDOM) {
+        const int threads = 256;
+        const size_t smem = hist_bytes(a.n_bins);
+        uint64_t blocks = (uint64_t)c->n_sm * 8;
+        const uint64_t need = (want_warps + 7) / 8;
+        if (blocks > need) blocks = need;
+        st::k_score_random<<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+    } else if (plan.kernel == ST_KERNEL_TABLE) {
+        int threads = 256;
+        size_t smem;
+        for (;; threads -= 32) {
+            smem = hist_bytes(a.n_bins) + (size_t)(threads / 32) * (size_t)stride * (sizeof(float2) + sizeof(uint16_t));
+            if (smem <= (size_t)c->smem_optin || threads == 32) break;
+        }
+        if (smem > (size_t)c->smem_optin) return fail(c, ST_ENOSPC, "n_max %d needs more shared memory than one SM has", n_max);
+        int rc = set_smem(c, st::k_score_table, smem);
+        if (rc) return rc;
+        int per_sm = (int)((size_t)c->smem_optin / (smem + 1024));
+        per_sm = per_sm < 1 ? 1 : (per_sm > 8 ? 8 : per_sm);
+        uint64_t blocks = (uint64_t)c->n_sm * (uint64_t)per_sm;
+        const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
+        if (blocks > need) blocks = need;
+        st::k_score_table<<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+    } else {
+        int threads = c->recur_threads;
+        const size_t bt_bytes = (size_t)c->n_f * sizeof(float4);
+        bool bt_smem = true;
+        size_t smem;
+        for (;;) {
+            smem = hist_bytes(a.n_bins) + (bt_smem ? bt_bytes : 0) +
+                   (size_t)(threads / 32) * (size_t)stride * (sizeof(float2) + sizeof(uint16_t));
+            if (smem <= (size_t)c->smem_optin) break;
+            if (threads > 256) threads -= 64;           // fewer warps first, down to 8
+            else if (bt_smem) bt_smem = false;          // then the bin table stays in L2
+            else if (threads > 32) threads -= 32;
+            else return fail(c, ST_ENOSPC, "n_max %d needs more shared memory than one SM has", n_max);
+        }
+        uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
+        const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
+        if (blocks > need) blocks = need;
+        const bool rot = plan.kernel == ST_KERNEL_ROTATION;
+#define ST_LAUNCH_RECUR(MODE, CH, BT)                                                              \
+    do {                                                                                           \
+        int rc_ = set_smem(c, st::k_score_recur<MODE, CH, BT>, smem);                              \
+        if (rc_) return rc_;                                                                       \
+        st::k_score_recur<MODE, CH, BT><<<(unsigned)blocks, threads, smem, c->stream>>>(a);        \
+    } while (0)
+        if (rot) {
+            if (plan.ch == 32) { if (bt_smem) ST_LAUNCH_RECUR(0, 32, true); else ST_LAUNCH_RECUR(0, 32, false); }
+            else               { if (bt_smem) ST_LAUNCH_RECUR(0, 64, true); else ST_LAUNCH_RECUR(0, 64, false); }
+        } else {
+            if (plan.ch == 32) { if (bt_smem) ST_LAUNCH_RECUR(1, 32, true); else ST_LAUNCH_RECUR(1, 32, false); }
+            else               { if (bt_smem) ST_LAUNCH_RECUR(1, 64, true); else ST_LAUNCH_RECUR(1, 64, false); }
+        }
+#undef ST_LAUNCH_RECUR
+    }
+    ST_CUDA(c, cudaGetLastError());
+    return ST_OK;
+}
+
+st::ScoreArgs base_args(st_ctx* c, const st_search_params* p)
+{
+    st::ScoreArgs a;
+    memset(&a, 0, sizeof(a));
+    a.map = at<float2>(c, c->L.map);
+    a.bp = bank(c, p);
+    a.f_min = c->f_min; a.df = c->df;
+    a.n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
+    a.norm = p->norm;
+    a.W = at<float2>(c, c->L.w);
+    a.E0 = at<float2>(c, c->L.e0);
+    a.bintab = at<float4>(c, c->L.bintab);
+    a.sc = at<st::Scalars>(c, c->L.scalars);
+    a.cand = at<st::Cand>(c, c->L.cand);
+    a.cand_cap = kCandCap;
+    a.warp_best = at<st::WarpBest>(c, c->L.warp_best);
+    a.hist = at<unsigned long long>(c, c->L.hist);
+    a.n_bins = 0; a.hist_lo = 0.0f; a.hist_scale = 0.0f;
+    a.dump = nullptr;
+    return a;
+}
+
+int reset_search_state(st_ctx* c, int n_bins)
+{
+    ST_CUDA(c, cudaMemsetAsync(at<void>(c, c->L.scalars), 0, sizeof(st::Scalars), c->stream));
+    ST_CUDA(c, cudaMemsetAsync(at<void>(c, c->L.warp_best), 0, (size_t)kWarpSlots * sizeof(st::WarpBest), c->stream));
+    if (n_bins > 0)
+        ST_CUDA(c, cudaMemsetAsync(at<void>(c, c->L.hist), 0, (size_t)n_bins * sizeof(unsigned long long), c->stream));
+    // gmax_bits = 0 encodes "below every float" (enc(-inf) = 0x007FFFFF > 0)
+    return ST_OK;
+}
+
+}  // namespace
+
+// ================================================================== C ABI ====
+extern "C" {
+
+const char* st_version(void) { return "stochtrack-b200 0.1 (sm_100a)"; }
+
+const char* st_last_error(const st_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
+{
+    if (!out) return ST_EINVAL;
+    *out = nullptr;
+    if (n_t < 1 || n_t > ST_MAX_N_T || n_f < 1 || n_f > ST_MAX_N_F) return ST_EINVAL;
+    if (!(df > 0.0) || !(f_min >= 0.0) || !isfinite(df) || !isfinite(f_min)) return ST_EINVAL;
+    st_ctx* c = new (std::nothrow) st_ctx();
+    if (!c) return ST_EINVAL;
+    c->n_t = n_t; c->n_f = n_f; c->df = df; c->f_min = f_min;
+    c->ws = nullptr; c->ws_bytes = 0; c->max_n_tau = 0; c->stream = nullptr;
+    c->have_ws = c->have_map = false;
+    c->table_kind = kNoTable; c->table_ch = 0; c->w_built = false;
+    c->ev0 = c->ev1 = nullptr; c->h_res = nullptr; c->h_hist = nullptr;
+    c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512;
+    c->err[0] = 0;
+    const char* e = getenv("ST_RECUR_THREADS");
+    if (e) { int t = atoi(e); if (t >= 32 && t <= 512 && t % 32 == 0) c->recur_threads = t; }
+    *out = c;
+    return ST_OK;
+}
+
+void st_destroy(st_ctx* c)
+{
+    if (!c) return;
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->h_res) cudaFreeHost(c->h_res);
+    if (c->h_hist) cudaFreeHost(c->h_hist);
+    delete c;
+}
+
+size_t st_workspace_bytes(const st_ctx* c, int32_t max_n_tau)
+{
+    if (!c || max_n_tau < 1 || max_n_tau > ST_MAX_N_TAU) return 0;
+    return make_layout(c->n_t, c->n_f, max_n_tau).total;
+}
+
+int st_set_workspace(st_ctx* c, void* ws, size_t bytes, void* cuda_stream)
+{
+    if (!c) return ST_EINVAL;
+    if (!ws || ((uintptr_t)ws % kAlign) != 0) return fail(c, ST_EINVAL, "workspace must be a non-null, 256-byte aligned device pointer");
+    // largest max_n_tau the buffer supports
+    const size_t base = make_layout(c->n_t, c->n_f, 1).total;
+    if (bytes < base) return fail(c, ST_ENOSPC, "workspace of %zu bytes is below the minimum %zu", bytes, base);
+    int lo = 1, hi = ST_MAX_N_TAU;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) / 2;
+        if (make_layout(c->n_t, c->n_f, mid).total <= bytes) lo = mid; else hi = mid - 1;
+    }
+    int dev = 0;
+    ST_CUDA(c, cudaGetDevice(&dev));
+    cudaPointerAttributes pa;
+    ST_CUDA(c, cudaPointerGetAttributes(&pa, ws));
+    if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)
+        return fail(c, ST_EINVAL, "workspace is not device memory");
+    ST_CUDA(c, cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev));
+    ST_CUDA(c, cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    if (!c->ev0) ST_CUDA(c, cudaEventCreate(&c->ev0));
+    if (!c->ev1) ST_CUDA(c, cudaEventCreate(&c->ev1));
+    if (!c->h_res) ST_CUDA(c, cudaHostAlloc((void**)&c->h_res, sizeof(st::DeviceResult), cudaHostAllocDefault));
+    if (!c->h_hist) ST_CUDA(c, cudaHostAlloc((void**)&c->h_hist, ST_MAX_BINS * sizeof(unsigned long long), cudaHostAllocDefault));
+    c->ws = (unsigned char*)ws; c->ws_bytes = bytes; c->max_n_tau = lo;
+    c->L = make_layout(c->n_t, c->n_f, lo);
+    c->stream = (cudaStream_t)cuda_stream;
+    c->have_ws = true; c->have_map = false;
+    c->tau_cached.clear(); c->table_kind = kNoTable; c->w_built = false;
+    return ST_OK;
+}
+
+int st_set_map(st_ctx* c, const void* csd_dev, const float* sigma_dev, int32_t sigma_kind)
+{
+    if (!c) return ST_EINVAL;
+    if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
+    if (!csd_dev) return fail(c, ST_EINVAL, "csd is NULL");
+    if (sigma_kind < ST_SIGMA_NONE || sigma_kind > ST_SIGMA_PER_PIXEL) return fail(c, ST_EINVAL, "bad sigma_kind %d", sigma_kind);
+    if (sigma_kind != ST_SIGMA_NONE && !sigma_dev) return fail(c, ST_EINVAL, "sigma is NULL");
+    const size_t n_pix = (size_t)c->n_t * (size_t)c->n_f;
+    const int blocks = (int)((n_pix + 255) / 256 < (size_t)(8 * c->n_sm) ? (n_pix + 255) / 256 : (size_t)(8 * c->n_sm));
+    st::k_prepare_map<<<blocks, 256, 0, c->stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, c->n_f, n_pix,
+                                                     at<float2>(c, c->L.map));
+    ST_CUDA(c, cudaGetLastError());
+    c->have_map = true;
+    return ST_OK;
+}
+
+int st_set_map_host(st_ctx* c, const void* csd_host, const float* sigma_host, int32_t sigma_kind)
+{
+    if (!c) return ST_EINVAL;
+    if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
+    if (!csd_host) return fail(c, ST_EINVAL, "csd is NULL");
+    if (sigma_kind < ST_SIGMA_NONE || sigma_kind > ST_SIGMA_PER_PIXEL) return fail(c, ST_EINVAL, "bad sigma_kind %d", sigma_kind);
+    if (sigma_kind != ST_SIGMA_NONE && !sigma_host) return fail(c, ST_EINVAL, "sigma is NULL");
+    const size_t n_pix = (size_t)c->n_t * (size_t)c->n_f;
+    ST_CUDA(c, cudaMemcpyAsync(at<void>(c, c->L.stage_csd), csd_host, n_pix * sizeof(float2), cudaMemcpyHostToDevice, c->stream));
+    if (sigma_kind != ST_SIGMA_NONE) {
+        const size_t n_s = sigma_kind == ST_SIGMA_PER_FREQ ? (size_t)c->n_f : n_pix;
+        ST_CUDA(c, cudaMemcpyAsync(at<void>(c, c->L.stage_sigma), sigma_host, n_s * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    }
+    const int rc = st_set_map(c, at<void>(c, c->L.stage_csd), at<float>(c, c->L.stage_sigma), sigma_kind);
+    if (rc) return rc;
+    ST_CUDA(c, cudaStreamSynchronize(c->stream));
+    return ST_OK;
+}
+
+int st_search(st_ctx* c, const st_search_params* p, st_result* out)
+{
+    int rc = validate(c, p, true);
+    if (rc) return rc;
+    if (!out) return fail(c, ST_EINVAL, "result is NULL");
+    if (p->n_bins > 0 && !p->hist_out) return fail(c, ST_EINVAL, "n_bins > 0 but hist_out is NULL");
+    memset(out, 0, sizeof(*out));
+    Plan plan;
+    rc = make_plan(c, p, &plan);
+    if (rc) return rc;
+    out->kernel_used = plan.kernel;
+    const int n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
+    if (p->n_tracks == 0) {                       // empty search: nothing scored
+        out->max_snr = -INFINITY; out->max_snr_f64 = -INFINITY;
+        if (p->n_bins > 0) memset(p->hist_out, 0, sizeof(uint64_t) * (size_t)p->n_bins);
+        return ST_OK;
+    }
+    int n_launches = 0;
+    rc = ensure_tables(c, p, plan, &n_launches);
+    if (rc) return rc;
+    rc = reset_search_state(c, p->n_bins);
+    if (rc) return rc;
+    st::ScoreArgs a = base_args(c, p);
+    a.n_bins = p->n_bins;
+    a.hist_lo = (float)p->hist_lo;
+    a.hist_scale = p->n_bins > 0 ? (float)((double)p->n_bins / (p->hist_hi - p->hist_lo)) : 0.0f;
+    uint64_t per_launch = kMaxSamplesPerLaunch / (uint64_t)n_tau;
+    if (per_launch < 1) per_launch = 1;
+    ST_CUDA(c, cudaEventRecord(c->ev0, c->stream));
+    for (uint64_t done = 0; done < p->n_tracks; done += per_launch) {
+        a.track_offset = p->track_offset + done;
+        a.n_tracks = p->n_tracks - done < per_launch ? p->n_tracks - done : per_launch;
+        rc = launch_score(c, plan, a, p->n_max);
+        if (rc) return rc;
+        ++n_launches;
+    }
+    ST_CUDA(c, cudaEventRecord(c->ev1, c->stream));
+    st::FinalArgs f;
+    memset(&f, 0, sizeof(f));
+    f.map = a.map; f.bp = a.bp; f.f_min = c->f_min; f.df = c->df;
+    f.norm = p->norm; f.tau_mode = p->tau_mode; f.n_tau = n_tau;
+    f.tau_d = at<double>(c, c->L.tau);
+    f.sc = a.sc; f.cand = a.cand; f.cand_cap = kCandCap; f.warp_best = a.warp_best; f.n_warp_slots = kWarpSlots;
+    f.out = at<st::DeviceResult>(c, c->L.result);
+    st::k_finalize<<<1, 256, 0, c->stream>>>(f);
+    ST_CUDA(c, cudaGetLastError());
+    ++n_launches;
+    ST_CUDA(c, cudaMemcpyAsync(c->h_res, f.out, sizeof(st::DeviceResult), cudaMemcpyDeviceToHost, c->stream));
+    if (p->n_bins > 0)
+        ST_CUDA(c, cudaMemcpyAsync(c->h_hist, a.hist, sizeof(unsigned long long) * (size_t)p->n_bins, cudaMemcpyDeviceToHost, c->stream));
+    ST_CUDA(c, cudaStreamSynchronize(c->stream));
+    const st::DeviceResult& r = *c->h_res;
+    out->max_snr = r.max_snr; out->arg_tau_index = r.arg_m; out->max_snr_f64 = r.snr_f64;
+    out->arg_track = r.arg_id; out->arg_tau = r.arg_tau;
+    out->arg_params.N = r.track.N; out->arg_params.j0 = r.track.j0; out->arg_params.a = r.track.a;
+    out->arg_params.y0 = r.track.y0; out->arg_params.y1 = r.track.y1; out->arg_params.y2 = r.track.y2;
+    out->arg_params.tau = r.track.tau;
+    out->n_pixels = r.n_pixels; out->n_evals = r.n_pixels * (uint64_t)n_tau;
+    out->n_candidates = r.n_candidates; out->flags = r.flags; out->n_launches = n_launches;
+    float ms = 0.0f;
+    ST_CUDA(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+    out->gpu_ms = ms;
+    if (p->n_bins > 0)
+        for (int b = 0; b < p->n_bins; ++b) p->hist_out[b] = (uint64_t)c->h_hist[b];
+    return ST_OK;
+}
+
+int st_track_params(const st_ctx* c, uint64_t seed, uint64_t track_id, int32_t n_min, int32_t n_max,
+                    double tau_lo, double tau_hi, st_track* out)
+{
+    if (!c || !out) return ST_EINVAL;
+    if (n_min < 1 || n_max < n_min || n_max > c->n_t) return ST_EINVAL;
+    st::BankParams bp;
+    bp.seed = seed; bp.n_t = c->n_t; bp.n_f = c->n_f; bp.n_min = n_min; bp.n_max = n_max;
+    bp.tau_lo = tau_lo; bp.tau_hi = tau_hi;
+    const st::Track t = st::make_track(bp, track_id);
+    out->N = t.N; out->j0 = t.j0; out->a = t.a; out->y0 = t.y0; out->y1 = t.y1; out->y2 = t.y2; out->tau = t.tau;
+    return ST_OK;
+}
+
+int st_debug_track_words(uint64_t seed, uint64_t track_id, uint32_t* out_host)
+{
+    if (!out_host) return ST_EINVAL;
+    const st::Words8 w = st::track_words(seed, track_id);
+    for (int i = 0; i < 8; ++i) out_host[i] = w.r[i];
+    return ST_OK;
+}
+
+int st_debug_rasterise(st_ctx* c, const st_search_params* p, uint64_t first, uint64_t count,
+                       int32_t* k_out_dev, int32_t* j0_dev, int32_t* N_dev)
+{
+    if (!c) return ST_EINVAL;
+    if (!p) return fail(c, ST_EINVAL, "params is NULL");
+    if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
+    if (p->n_min < 1 || p->n_max < p->n_min || p->n_max > c->n_t) return fail(c, ST_EINVAL, "need 1 <= n_min <= n_max <= n_t");
+    if (!k_out_dev || !j0_dev || !N_dev) return fail(c, ST_EINVAL, "output pointer is NULL");
+    if (count == 0) return ST_OK;
+    const uint64_t need = (count + 7) / 8;
+    const unsigned blocks = (unsigned)(need < (uint64_t)(c->n_sm * 8) ? need : (uint64_t)(c->n_sm * 8));
+    st::k_debug_rasterise<<<blocks, 256, 0, c->stream>>>(bank(c, p), first, count, k_out_dev, j0_dev, N_dev);
+    ST_CUDA(c, cudaGetLastError());
+    return ST_OK;
+}
+
+int st_debug_rasterise_track(st_ctx* c, const st_track* t, int32_t* k_out_dev)
+{
+    if (!c) return ST_EINVAL;
+    if (!t || !k_out_dev) return fail(c, ST_EINVAL, "NULL argument");
+    if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
+    if (t->N < 1 || t->j0 < 0 || t->j0 + t->N > c->n_t) return fail(c, ST_EINVAL, "track outside the map");
+    st::Track d;
+    d.N = t->N; d.j0 = t->j0; d.a = t->a; d.y0 = t->y0; d.y1 = t->y1; d.y2 = t->y2; d.tau = t->tau;
+    st::k_debug_rasterise_track<<<(t->N + 127) / 128, 128, 0, c->stream>>>(d, c->n_f, k_out_dev);
+    ST_CUDA(c, cudaGetLastError());
+    return ST_OK;
+}
+
+int st_debug_scores(st_ctx* c, const st_search_params* p, uint64_t first, uint64_t count, float* snr_dev)
+{
+    int rc = validate(c, p, true);
+    if (rc) return rc;
+    if (!snr_dev) return fail(c, ST_EINVAL, "snr_dev is NULL");
+    if (count == 0) return ST_OK;
+    Plan plan;
+    rc = make_plan(c, p, &plan);
+    if (rc) return rc;
+    const int n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
+    if (count > kMaxSamplesPerLaunch / (uint64_t)n_tau) return fail(c, ST_EINVAL, "count too large for one debug launch");
+    int n_launches = 0;
+    rc = ensure_tables(c, p, plan, &n_launches);
+    if (rc) return rc;
+    rc = reset_search_state(c, 0);
+    if (rc) return rc;
+    st::ScoreArgs a = base_args(c, p);
+    a.track_offset = first; a.n_tracks = count; a.dump = snr_dev;
+    return launch_score(c, plan, a, p->n_max);
+}
+
+}  // extern "C"

@@ -1,0 +1,346 @@
+"""Parity of the CUDA path (through the C ABI) against the float64 CPU oracle, element by
+element on the same seeded inputs.  Bars: template parameters, pixel indices and argmax
+bit-exact; SNRs within 1e-4 * max(|SNR|, s0) (G13); histogram by the edge rule (G14)."""
+import numpy as np
+import pytest
+
+from workloads import synth
+from helpers import config_inputs, snr_close, hist_rule_ok, S0_UNIT
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = {"table": 1, "rotation": 2, "reinsch": 3}
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1401_8060_b200 as pkg
+    from paper_1401_8060_b200 import build
+    build.build()
+    pkg.load_library()          # fails loudly if the extension is missing
+    return pkg
+
+
+def make_ctx(P, cfg, max_n_tau=None):
+    return P.Stochtrack(cfg.n_t, cfg.n_f, cfg.df, cfg.f_min, max_n_tau=max_n_tau or max(cfg.n_tau, 64))
+
+
+def s0_of(cfg):
+    return S0_UNIT
+
+
+# ------------------------------------------------------------------ S1 + S2
+@pytest.mark.parametrize("cid,first,count", [(1, 0, 1000), (2, 0, 3000), (3, 0, 2000), (5, 0, 2000),
+                                             (5, 9_990_000, 1500), (4, 2 ** 33 + 5, 700)])
+def test_rasteriser_indices_bit_exact(P, orc, cid, first, count):
+    cfg = synth.CONFIGS[cid]
+    st = make_ctx(P, cfg)
+    seed = synth.map_seed(cfg, 0)
+    k, j0, N = st.debug_rasterise(seed, cfg.n_min, cfg.n_max, first, count)
+    # the oracle's pixel lists via its search dump (tiny noise map; scores unused)
+    p = np.zeros((cfg.n_t, cfg.n_f), dtype=np.complex128)
+    ref = orc.search(p, cfg.f_min, cfg.df, count, seed, cfg.n_min, cfg.n_max, tau_grid=np.zeros(1),
+                     track_offset=first, dump_tracks=True)
+    assert np.array_equal(N, ref["N"]) and np.array_equal(j0, ref["j0"])
+    assert np.array_equal(k, ref["k"])
+    assert (N >= cfg.n_min).all() and (N <= cfg.n_max).all()
+
+
+def test_rasteriser_explicit_tracks(P, orc):
+    """Injection tracks of SURVEY 8(d) and the degenerate shapes: flat, straight, a -> 0, a -> N."""
+    cfg = synth.CONFIGS[5]
+    st = make_ctx(P, cfg)
+    tracks = [(inj.N, inj.j0, inj.a, inj.y0, inj.y1, inj.y2) for inj in cfg.injections]
+    tracks += [(1000, 0, 500.0, 7.5, 7.5, 7.5), (1000, 0, 500.0, 0.25, 1230.25, 2460.25),
+               (1, 999, 0.5, 2460.99, 0.01, 1200.0), (10, 5, 1e-9, 100.0, 2000.0, 50.0),
+               (10, 5, 10 - 1e-9, 100.0, 2000.0, 50.0), (777, 100, 3.0, 2460.999999, 0.0000001, 2460.999999)]
+    for tr in tracks:
+        got = st.debug_rasterise_track(*tr)
+        want = orc.rasterise(orc.make_track(*tr), cfg.n_f)
+        assert np.array_equal(got, want), tr
+
+
+# ------------------------------------------------------------------ S3 per kernel
+def _score_case(P, orc, cfg, kernel, count, first=0, norm=0, n_tau=None, tau=None):
+    csd, sigma, tau_cfg = config_inputs(orc, cfg)
+    if tau is None:
+        tau = tau_cfg if n_tau is None else synth.tau_linspace(n_tau)
+    st = make_ctx(P, cfg, max_n_tau=max(len(tau), 64))
+    st.set_map(csd, sigma)
+    got = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, first, count, tau_grid=tau, norm=norm, kernel=kernel)
+    p = orc.prepare_map(csd, sigma)
+    ref = orc.search(p, cfg.f_min, cfg.df, count, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, norm=norm,
+                     track_offset=first, dump_snr=True)["snr"]
+    return got, ref
+
+
+@pytest.mark.parametrize("kname", ["table", "rotation", "reinsch"])
+@pytest.mark.parametrize("cid,count", [(1, 1000), (2, 4000)])
+def test_scores_grid_kernels_vs_oracle(P, orc, kname, cid, count):
+    cfg = synth.CONFIGS[cid]
+    got, ref = _score_case(P, orc, cfg, KERNELS[kname], count)
+    ok, worst = snr_close(got, ref)
+    assert ok, f"{kname} config {cid}: worst error {worst:.3f} x tolerance"
+    assert worst < 0.5          # float32 leaves an order of magnitude of headroom (DESIGN.md error budget)
+
+
+@pytest.mark.parametrize("kname", ["table", "rotation", "reinsch"])
+@pytest.mark.parametrize("n_tau", [1, 7, 33, 50, 128, 200])
+def test_scores_ragged_tau_counts(P, orc, kname, n_tau):
+    """Grid sizes that are not multiples of the 32/64-delay chunks, on the config-5 shape
+    with per-pixel sigma (several 32-column rows and a ragged tail per track)."""
+    cfg = synth.CONFIGS[5]
+    got, ref = _score_case(P, orc, cfg, KERNELS[kname], 300, first=12345, n_tau=n_tau)
+    ok, worst = snr_close(got, ref)
+    assert ok, f"{kname} n_tau {n_tau}: worst error {worst:.3f} x tolerance"
+
+
+@pytest.mark.parametrize("kname", ["table", "reinsch"])
+def test_scores_mean_normalisation(P, orc, kname):
+    """alpha = 1: Eq. 8 exactly as printed."""
+    cfg = synth.CONFIGS[2]
+    got, ref = _score_case(P, orc, cfg, KERNELS[kname], 1500, norm=1)
+    # null scale of the mean statistic is s0 / sqrt(N) <= s0 / sqrt(n_min): keep G13 with that floor
+    ok, worst = snr_close(got, ref, s0=S0_UNIT / np.sqrt(cfg.n_max))
+    assert ok, worst
+
+
+def test_scores_nonuniform_grid_uses_table(P, orc):
+    cfg = synth.CONFIGS[2]
+    rng = np.random.default_rng(5)
+    tau = np.sort(rng.uniform(-0.01, 0.01, 40))
+    got, ref = _score_case(P, orc, cfg, 0, 800, tau=tau)
+    ok, worst = snr_close(got, ref)
+    assert ok, worst
+    csd, sigma, _ = config_inputs(orc, cfg)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    r = st.search(100, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau)
+    assert r.kernel_name == "table"
+    with pytest.raises(P.StError):
+        st.search(100, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, kernel=P.KERNEL_REINSCH)
+
+
+def test_scores_random_tau_mode(P, orc):
+    """The paper's mode: one delay per template."""
+    cfg = synth.CONFIGS[3]
+    csd, sigma, _ = config_inputs(orc, cfg)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    count = 20000
+    got = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, 0, count, tau_range=(-synth.TAU_MAX, synth.TAU_MAX))
+    p = orc.prepare_map(csd, sigma)
+    ref = orc.search(p, cfg.f_min, cfg.df, count, cfg.seed, cfg.n_min, cfg.n_max,
+                     tau_range=(-synth.TAU_MAX, synth.TAU_MAX), dump_snr=True)["snr"]
+    ok, worst = snr_close(got, ref)
+    assert ok, worst
+
+
+def test_auto_picks_rotation_when_reinsch_ill_conditioned(P, orc):
+    """A grid step with f * dtau = 1/2 for some bin (theta = pi) must not use the three-term form."""
+    cfg = synth.CONFIGS[1]            # 40..103 Hz
+    dtau = 0.5 / 80.0                 # theta = pi at 80 Hz
+    tau = -0.01 + dtau * np.arange(16)
+    csd, sigma, _ = config_inputs(orc, cfg)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    r = st.search(1000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=1000)
+    assert r.kernel_name == "rotation"
+    p = orc.prepare_map(csd, sigma)
+    ref = orc.search(p, cfg.f_min, cfg.df, 1000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, dump_snr=True)
+    assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+    got = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, 0, 1000, tau_grid=tau)
+    ok, worst = snr_close(got, ref["snr"])
+    assert ok, worst
+
+
+# ------------------------------------------------------------------ S4: whole searches
+def _search_both(P, orc, cfg, n_tracks, kernel=0, norm=0, offset=0, m=0, st=None, inputs=None, dump=True):
+    csd, sigma, tau = inputs if inputs is not None else config_inputs(orc, cfg, m)
+    seed = synth.map_seed(cfg, m)
+    if st is None:
+        st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    kw = dict(tau_grid=tau) if cfg.tau_mode == "grid" else dict(tau_range=(-synth.TAU_MAX, synth.TAU_MAX))
+    r = st.search(n_tracks, seed, cfg.n_min, cfg.n_max, norm=norm, n_bins=cfg.n_bins, hist_lo=cfg.hist_lo,
+                  hist_hi=cfg.hist_hi, track_offset=offset, kernel=kernel, **kw)
+    p = orc.prepare_map(csd, sigma)
+    ref = orc.search(p, cfg.f_min, cfg.df, n_tracks, seed, cfg.n_min, cfg.n_max, norm=norm, n_bins=cfg.n_bins,
+                     hist_lo=cfg.hist_lo, hist_hi=cfg.hist_hi, track_offset=offset, dump_snr=dump, **kw)
+    return r, ref
+
+
+def _assert_search_parity(r, ref, cfg, check_hist=True):
+    assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"]), (r, ref["max_snr"])
+    assert r.n_pixels == ref["n_pixels"] and r.n_evals == ref["n_evals"]
+    assert abs(r.max_snr - ref["max_snr"]) <= 1e-4 * abs(ref["max_snr"])          # float32 kernel value
+    assert abs(r.max_snr_f64 - ref["max_snr"]) <= 1e-9 * abs(ref["max_snr"])      # float64 re-score
+    assert r.arg_tau == pytest.approx(ref["arg_tau"], abs=1e-15)
+    assert r.flags == 0 and r.n_candidates >= 1
+    if check_hist:
+        assert int(r.hist.sum()) == int(ref["hist"].sum())
+        if ref["snr"] is not None:
+            ok, why = hist_rule_ok(r.hist, ref["snr"], cfg.hist_lo, cfg.hist_hi, cfg.n_bins)
+            assert ok, why
+
+
+@pytest.mark.parametrize("kname", ["auto", "table", "rotation", "reinsch"])
+def test_search_config1(P, orc, kname):
+    cfg = synth.CONFIGS[1]
+    r, ref = _search_both(P, orc, cfg, cfg.n_tracks, kernel=KERNELS.get(kname, 0))
+    _assert_search_parity(r, ref, cfg)
+    assert r.n_evals == 1000 * 64 * 16
+
+
+@pytest.mark.parametrize("kname", ["auto", "table", "rotation"])
+def test_search_config2_full_size(P, orc, kname):
+    """Config 2 at its full size (1e5 tracks x 64 delays, injected chirp), every output."""
+    cfg = synth.CONFIGS[2]
+    r, ref = _search_both(P, orc, cfg, cfg.n_tracks, kernel=KERNELS.get(kname, 0))
+    _assert_search_parity(r, ref, cfg)
+    if kname == "auto":
+        assert r.kernel_name == "reinsch"
+    # the argmax template's control points are the oracle's (bit-exact)
+    o = orc.track_params(cfg.seed, ref["arg_track"], cfg.n_t, cfg.n_f, cfg.n_min, cfg.n_max)
+    for f in ("N", "j0", "a", "y0", "y1", "y2"):
+        assert r.arg_params[f] == getattr(o, f)
+
+
+def test_search_config3_full_size_random_tau(P, orc):
+    """Config 3 at its full size: 1e6 templates, one random delay each, 1000-bin histogram."""
+    cfg = synth.CONFIGS[3]
+    r, ref = _search_both(P, orc, cfg, cfg.n_tracks)
+    _assert_search_parity(r, ref, cfg)
+    assert r.kernel_name == "random" and int(r.hist.sum()) == cfg.n_tracks
+
+
+def test_search_mean_norm_and_offsets(P, orc):
+    cfg = synth.CONFIGS[2]
+    r, ref = _search_both(P, orc, cfg, 20000, norm=1, offset=777_000)
+    assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+    assert abs(r.max_snr_f64 - ref["max_snr"]) <= 1e-9 * abs(ref["max_snr"])
+
+
+@pytest.mark.parametrize("cid,m,ranges", [
+    (4, 0, [(0, 6000), (994_000, 6000)]), (4, 57, [(500_000, 6000)]), (4, 99, [(123_456, 6000)]),
+    (5, 0, [(0, 1500), (9_998_500, 1500), (5_000_000, 1500)])])
+def test_search_large_configs_subranges(P, orc, cid, m, ranges):
+    """Configs 4 (three of the 100 maps) and 5 at full map size and full delay grid, on id
+    sub-ranges the oracle finishes in seconds (SURVEY 8(d) sub-range protocol)."""
+    cfg = synth.CONFIGS[cid]
+    inputs = config_inputs(orc, cfg, m)
+    st = make_ctx(P, cfg)
+    for first, n in ranges:
+        r, ref = _search_both(P, orc, cfg, n, offset=first, m=m, st=st, inputs=inputs)
+        _assert_search_parity(r, ref, cfg)
+        assert r.kernel_name == "reinsch"
+
+
+def test_chunk_combination_P9(P, orc):
+    """runs combine by max; histograms add exactly; ids are global."""
+    cfg = synth.CONFIGS[2]
+    csd, sigma, tau = config_inputs(orc, cfg)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    kw = dict(tau_grid=tau, n_bins=1000)
+    T = 7001
+    whole = st.search(3 * T, cfg.seed, cfg.n_min, cfg.n_max, **kw)
+    parts = [st.search(T, cfg.seed, cfg.n_min, cfg.n_max, track_offset=i * T, **kw) for i in range(3)]
+    best = max(parts, key=lambda r: (r.max_snr_f64, -r.arg_track, -r.arg_tau_index))
+    assert (whole.arg_track, whole.arg_tau_index, whole.max_snr_f64) == (best.arg_track, best.arg_tau_index, best.max_snr_f64)
+    assert np.array_equal(whole.hist, sum(r.hist for r in parts))
+    assert whole.n_evals == sum(r.n_evals for r in parts)
+    # repeatability: the same search twice gives identical outputs (atomics only on integers)
+    again = st.search(3 * T, cfg.seed, cfg.n_min, cfg.n_max, **kw)
+    assert np.array_equal(again.hist, whole.hist) and again.max_snr == whole.max_snr
+    assert (again.arg_track, again.arg_tau_index) == (whole.arg_track, whole.arg_tau_index)
+
+
+def test_injected_track_self_recovery_P7(P, orc):
+    """A bank member injected noise-free at a grid delay is returned exactly, with SNR = A sqrt(N)...
+    here A = snr/sqrt(N) so the recovered SNR is `snr`."""
+    cfg = synth.CONFIGS[2]
+    tau = synth.tau_linspace(64)
+    i_star, m_star, snr = 4321, 17, 9.0
+    t = orc.track_params(cfg.seed, i_star, cfg.n_t, cfg.n_f, cfg.n_min, cfg.n_max)
+    k = orc.rasterise(t, cfg.n_f)
+    csd = np.zeros((cfg.n_t, cfg.n_f), dtype=np.complex64)
+    sigma = synth.make_sigma("per_f", 0.2, cfg.n_t, cfg.n_f, 11)
+    synth.add_injection(csd, sigma, t.j0 + np.arange(t.N), k, tau[m_star], snr, cfg.f_min, cfg.df)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    r = st.search(10000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau)
+    assert (r.arg_track, r.arg_tau_index) == (i_star, m_star)
+    assert r.max_snr_f64 == pytest.approx(snr, rel=1e-6) and r.max_snr == pytest.approx(snr, rel=1e-5)
+    assert r.arg_params["a"] == t.a and r.arg_params["y1"] == t.y1 and r.arg_params["N"] == t.N
+
+
+# ------------------------------------------------------------------ edge cases
+def test_edge_cases(P, orc):
+    cfg = synth.CONFIGS[2]
+    csd, sigma, tau = config_inputs(orc, cfg)
+    st = make_ctx(P, cfg)
+    # search before a map -> ST_ESTATE
+    with pytest.raises(P.StError) as e:
+        st.search(10, 0, 10, 250, tau_grid=tau)
+    assert e.value.code == -2
+    st.set_map(csd, sigma)
+    # empty search
+    r = st.search(0, 0, 10, 250, tau_grid=tau, n_bins=100)
+    assert r.n_evals == 0 and r.max_snr == -np.inf and int(r.hist.sum()) == 0
+    # invalid arguments come back as codes, not crashes
+    for bad in (dict(n_min=0), dict(n_max=251), dict(n_min=200, n_max=100)):
+        kw = dict(n_min=10, n_max=250)
+        kw.update(bad)
+        with pytest.raises(P.StError):
+            st.search(10, 0, kw["n_min"], kw["n_max"], tau_grid=tau)
+    with pytest.raises(P.StError) as e:
+        st.search(10, 0, 10, 250, tau_grid=synth.tau_linspace(1024))    # beyond the workspace
+    assert e.value.code == -3
+    # single template, single delay, single column
+    r = st.search(1, 5, 1, 1, tau_grid=np.array([0.001]), n_bins=10)
+    p = orc.prepare_map(csd, sigma)
+    ref = orc.search(p, cfg.f_min, cfg.df, 1, 5, 1, 1, tau_grid=np.array([0.001]), n_bins=10)
+    assert r.n_evals == 1 and (r.arg_track, r.arg_tau_index) == (0, 0)
+    assert r.max_snr_f64 == pytest.approx(ref["max_snr"], rel=1e-12)
+    assert np.array_equal(r.hist, ref["hist"])
+    # maximum-length tracks only (n_min = n_max = n_t), per-pixel sigma with masked pixels (G11)
+    sig2 = np.ones((cfg.n_t, cfg.n_f), dtype=np.float32)
+    sig2[:, 100:140] = 0.0
+    sig2[7, :] = np.inf
+    sig2[9, 5] = np.nan
+    sig2[11, :] = -1.0
+    st.set_map(csd, sig2)
+    p2 = orc.prepare_map(csd, sig2)
+    got = st.debug_scores(3, cfg.n_t, cfg.n_t, 0, 500, tau_grid=tau)
+    ref = orc.search(p2, cfg.f_min, cfg.df, 500, 3, cfg.n_t, cfg.n_t, tau_grid=tau, dump_snr=True)["snr"]
+    ok, worst = snr_close(got, ref)
+    assert ok, worst
+
+
+def test_degenerate_all_zero_map(P, orc):
+    """Every SNR ties at 0: the G12 total order picks the smallest id and delay index; the
+    candidate list overflows and the float32 records decide (flags bit 0)."""
+    cfg = synth.CONFIGS[1]
+    st = make_ctx(P, cfg)
+    st.set_map(np.zeros((cfg.n_t, cfg.n_f), dtype=np.complex64))
+    tau = synth.tau_linspace(16)
+    r = st.search(20000, 0, 64, 64, tau_grid=tau, n_bins=1000, track_offset=100)
+    assert (r.arg_track, r.arg_tau_index, r.max_snr, r.max_snr_f64) == (100, 0, 0.0, 0.0)
+    assert int(r.hist[500]) == 20000 * 16 and int(r.hist.sum()) == 20000 * 16
+    assert r.flags & 1
+
+
+def test_host_buffer_entry_point(P, orc):
+    """st_set_map_host (numpy in) == st_set_map (CUDA tensors in)."""
+    import torch
+    cfg = synth.CONFIGS[2]
+    csd, sigma, tau = config_inputs(orc, cfg)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)                                   # host path
+    a = st.search(5000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=1000)
+    st.set_map(torch.from_numpy(csd).cuda(), torch.from_numpy(sigma).cuda())   # device path
+    b = st.search(5000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=1000)
+    assert a.max_snr == b.max_snr and a.arg_track == b.arg_track and np.array_equal(a.hist, b.hist)

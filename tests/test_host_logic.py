@@ -1,0 +1,114 @@
+"""CPU-side checks of the product library (no GPU needed): the C-ABI library loads and
+exports every symbol include/stochtrack.h declares, the host-only entry points validate
+their arguments, and the host copy of S1 (st_track_params / st_debug_track_words) agrees
+bit for bit with the oracle.  No compute call touches a device here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_1401_8060_b200 as P
+from paper_1401_8060_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return P.load_library()
+
+
+def test_library_exports_every_declared_symbol(lib):
+    header = open(os.path.join(ROOT, "include", "stochtrack.h")).read()
+    declared = set(re.findall(r"\b(st_[a-z_]+)\s*\(", header))
+    assert declared == set(binding.exported_symbols), declared ^ set(binding.exported_symbols)
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert b"sm_100a" in lib.st_version()
+
+
+def test_struct_layouts_match_header(tmp_path):
+    """ctypes mirrors of the header's structs have the sizes / offsets gcc gives them."""
+    import subprocess
+    src = tmp_path / "layout.c"
+    src.write_text(r"""
+#include <stdio.h>
+#include <stddef.h>
+#include "stochtrack.h"
+int main(void) {
+  printf("%zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(st_track), sizeof(st_search_params), sizeof(st_result),
+         offsetof(st_search_params, tau_grid), offsetof(st_search_params, hist_out), offsetof(st_search_params, kernel),
+         offsetof(st_result, arg_params), offsetof(st_result, gpu_ms));
+  return 0; }
+""")
+    exe = tmp_path / "layout"
+    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
+    got = [int(x) for x in subprocess.check_output([str(exe)]).split()]
+    B = binding
+    want = [C.sizeof(B.CTrack), C.sizeof(B.CSearchParams), C.sizeof(B.CResult), B.CSearchParams.tau_grid.offset,
+            B.CSearchParams.hist_out.offset, B.CSearchParams.kernel.offset, B.CResult.arg_params.offset,
+            B.CResult.gpu_ms.offset]
+    assert got == want
+
+
+def test_create_validates_arguments(lib):
+    ctx = C.c_void_p()
+    for args in [(0, 64, 1.0, 40.0), (64, 0, 1.0, 40.0), (64, 70000, 1.0, 40.0), (64, 64, 0.0, 40.0),
+                 (64, 64, 1.0, -1.0), (2 ** 20 + 1, 64, 1.0, 0.0), (64, 64, float("nan"), 0.0)]:
+        assert lib.st_create(C.byref(ctx), *args) == binding.ST_EINVAL, args
+        assert not ctx.value
+    assert lib.st_create(C.byref(ctx), 1000, 2461, 1.0, 40.0) == 0
+    try:
+        b512, b64 = lib.st_workspace_bytes(ctx, 512), lib.st_workspace_bytes(ctx, 64)
+        assert b512 > b64 > 1000 * 2461 * 8
+        assert b512 - b64 >= (512 - 64) * 2461 * 8
+        assert lib.st_workspace_bytes(ctx, 0) == 0 and lib.st_workspace_bytes(ctx, 5000) == 0
+        # calls that need a workspace fail with ST_ESTATE, never crash
+        p = binding.CSearchParams()
+        p.n_tracks, p.n_min, p.n_max, p.tau_mode, p.tau_hi = 10, 10, 100, binding.TAU_RANDOM, 0.01
+        r = binding.CResult()
+        assert lib.st_search(ctx, C.byref(p), C.byref(r)) == binding.ST_ESTATE
+        assert b"workspace" in lib.st_last_error(ctx)
+        assert lib.st_set_map(ctx, 0, 0, 0) == binding.ST_ESTATE
+        assert lib.st_set_workspace(ctx, 0, 1 << 30, 0) == binding.ST_EINVAL
+        t = binding.CTrack()
+        assert lib.st_track_params(ctx, 0, 0, 10, 1001, 0.0, 0.0, C.byref(t)) == binding.ST_EINVAL
+        assert lib.st_track_params(ctx, 0, 0, 0, 10, 0.0, 0.0, C.byref(t)) == binding.ST_EINVAL
+    finally:
+        lib.st_destroy(ctx)
+
+
+def test_host_track_generator_matches_oracle_bit_for_bit(lib, orc):
+    """S1 on the host side of the product == O1 + O2 of the oracle (words and parameters)."""
+    shapes = [(0, 64, 64, 64, 64), (1, 250, 961, 10, 250), (2, 500, 2461, 10, 500), (4, 1000, 2461, 10, 1000),
+              (3 * 2 ** 32 + 7, 500, 2461, 10, 500)]
+    ids = list(range(300)) + [2 ** 32 - 1, 2 ** 32, 2 ** 40 + 17, 2 ** 62]
+    for seed, n_t, n_f, n_min, n_max in shapes:
+        for tid in ids:
+            assert np.array_equal(P.st_track_words(seed, tid), orc.track_words(seed, tid))
+            g = P.st_track_params(n_t, n_f, seed, tid, n_min, n_max, -0.01, 0.01)
+            o = orc.track_params(seed, tid, n_t, n_f, n_min, n_max, -0.01, 0.01)
+            for f in ("N", "j0", "a", "y0", "y1", "y2", "tau"):
+                assert getattr(g, f) == getattr(o, f), (seed, tid, f)
+
+
+def test_binding_fails_loudly_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        P.Stochtrack(64, 64, 1.0, 40.0)
+
+
+def test_product_does_not_import_oracle():
+    """The product path must not route through oracle/ (or read _work/)."""
+    pkg = os.path.join(ROOT, "paper_1401_8060_b200")
+    bad = re.compile(r"(^|\s)(from|import)\s+oracle\b|oracle/|oracle\.py|stochtrack_oracle|_work/|/_work")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not bad.search(src), f
