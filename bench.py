@@ -124,6 +124,8 @@ def run_ours(args):
     # weak scaling: rank r scores its own template-id range on its own copy of the map
     first, n_mine = sharding.rank_range(n_tracks, rank)
     kw = search_kwargs(cfg, tau)
+    if cfg.tau_mode == "grid":
+        kw["kernel"] = {"auto": 0, "table": 1, "rotation": 2, "reinsch": 3}[args.kernel]
     csd_d = torch.from_numpy(csd).to(dev)
     sigma_d = torch.from_numpy(sigma).to(dev) if sigma is not None else None
     csd_h = torch.from_numpy(csd).pin_memory()
@@ -294,6 +296,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--tracks", type=int, default=0, help="override templates per GPU (debugging)")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "table", "rotation", "reinsch"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--ref-step-s", type=float, default=6.0, help="seconds of oracle work per reference step")

@@ -69,7 +69,9 @@ struct ScoreArgs {
     int32_t norm;
     const float2* W;          // [n_f][n_tau]      (table kernel)
     const float2* E0;         // [n_f] e^{2 pi i f_k tau_0}  (recurrence kernels)
-    const float4* bintab;     // [n_f] per-bin recurrence constants
+    const float4* bintab;     // [n_f] per-bin recurrence constants (rotation kernel)
+    const float2* Es;         // [n_super][n_f] e^{2 pi i f_k tau_{s R}}: anchors of the Reinsch kernel
+    const float2* kz;         // [n_f] (-4 sin^2(theta_k/2), sin theta_k)
     Scalars* sc;
     Cand* cand;
     uint32_t cand_cap;
@@ -286,6 +288,29 @@ __global__ void k_build_bin_tables(double tau0, double dtau, int ch, int mode, i
     bintab[k] = t;
 }
 
+// Tables of k_score_reinsch on the uniform grid tau_m = tau0 + m dtau, theta_k = 2 pi f_k dtau:
+//   Es[s][k] = e^{2 pi i f_k (tau0 + s R dtau)}   anchor phase factors, one row per super-chunk of R delays
+//   kz[k]    = (-4 sin^2(theta_k / 2), sin theta_k)
+__global__ void k_build_reinsch_tables(double tau0, double dtau, int r_super, int n_super, int n_f,
+                                       double f_min, double df, float2* __restrict__ Es, float2* __restrict__ kz)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_f) return;
+    const double f = f_min + (double)k * df;
+    for (int s = 0; s < n_super; ++s) {
+        const double cyc = f * (tau0 + (double)(s * r_super) * dtau);
+        double sn, cs;
+        sincospi(2.0 * (cyc - rint(cyc)), &sn, &cs);
+        Es[(size_t)s * (size_t)n_f + (size_t)k] = make_float2((float)cs, (float)sn);
+    }
+    double cyc = f * dtau;
+    cyc -= rint(cyc);
+    double zs, zc, hs, hc;
+    sincospi(2.0 * cyc, &zs, &zc);
+    sincospi(cyc, &hs, &hc);
+    kz[k] = make_float2((float)(-4.0 * hs * hs), (float)zs);
+}
+
 // --------------------------------------------------- S1-S4, table, any grid --
 // Warp per template.  The warp rasterises the track (lanes over columns), parks
 // (p, k) of every pixel in its shared-memory pool, then lanes own delays: for each
@@ -498,6 +523,183 @@ __global__ void __launch_bounds__(512, 1) k_score_recur(const ScoreArgs a)
             }
             reduce_samples<NV>(a, wr, sm_hist, id, q, v, ms, ok);
             __syncwarp();
+        }
+    }
+    reduce_finish(a, wr);
+    hist_flush(sm_hist, a.hist, a.n_bins);
+}
+
+
+// --------------------- S1-S4, uniform tau grid, packed three-term recurrence --
+// The production kernel of the grid mode.  Warp per template, lanes over pixels.
+// For x_m = Re[p e^{2 pi i f (tau_0 + m dtau)}] the exact identities
+//     d_{m+1} = d_m - kappa x_m ,   x_{m+1} = x_m + d_{m+1} ,   kappa = 4 sin^2(theta/2)
+// (Reinsch's form of the Chebyshev three-term recurrence, stable as theta -> 0)
+// advance a pixel's term of Eq. 8 along the delay grid with one FMA and one add;
+// a third add accumulates it.  Two pixels of a lane are packed into one f32x2
+// register pair (sm_100 fma.rn.f32x2 / add.rn.f32x2), two such pairs are in flight.
+//   anchor phase (every R = 256 delays): rasterise (first time), gather p from the
+//     L2-resident map, x = Re[p Es], d = x_m - x_{m-1}, parked with the bin in the
+//     warp's shared-memory pool (10 B per pixel);
+//   chunk of 32 delays: 32 packed accumulators per lane; states are read from the
+//     pool, advanced 32 steps in registers and written back; a transposing shuffle
+//     tree folds the accumulators across the warp: lane l ends with delay m0 + l.
+// Float32 error of a term after R steps stays below 1e-5 |p| (tests).
+typedef unsigned long long f32x2_t;
+__device__ __forceinline__ f32x2_t pk_fma(f32x2_t a, f32x2_t b, f32x2_t c)
+{
+    f32x2_t r;
+    asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2_t pk_add(f32x2_t a, f32x2_t b)
+{
+    f32x2_t r;
+    asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2_t pk_make(float lo, float hi)
+{
+    f32x2_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ float pk_sum(f32x2_t a)
+{
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a));
+    return lo + hi;
+}
+
+constexpr int kChunk = 32;        // delays per accumulator chunk
+constexpr int kSuper = 256;       // delays between re-anchoring (8 chunks)
+
+template <int NCHAIN>
+__global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_warps = blockDim.x >> 5;
+    // shared memory: hist | kz[n_f] | x2[n_warps][P] | d2[n_warps][P] | kk[n_warps][P],  P = pool_stride / 2
+    float2* sm_kz = reinterpret_cast<float2*>(sm_hist + hist_smem_words(a.n_bins));
+    const int P = a.pool_stride >> 1;               // packed entries (pixel pairs) per warp
+    f32x2_t* pool_x = reinterpret_cast<f32x2_t*>(sm_kz + a.bp.n_f + (a.bp.n_f & 1)) + (size_t)warp * P;
+    f32x2_t* pool_d = pool_x + (size_t)n_warps * P;
+    uint32_t* pool_k = reinterpret_cast<uint32_t*>(reinterpret_cast<f32x2_t*>(sm_kz + a.bp.n_f + (a.bp.n_f & 1))
+                                                   + 2 * (size_t)n_warps * P) + (size_t)warp * P;
+    for (int k = threadIdx.x; k < a.bp.n_f; k += blockDim.x) sm_kz[k] = a.kz[k];
+    hist_init(sm_hist, a.n_bins);
+    const float* sm_negk = reinterpret_cast<const float*>(sm_kz);     // sm_negk[2k] = -kappa_k
+    const int n_chunks = (a.n_tau + kChunk - 1) / kChunk;
+    WarpReduce wr;
+    reduce_init(wr);
+    for (;;) {
+        const uint64_t q = next_track(a);
+        if (q >= a.n_tracks) break;
+        const uint64_t id = a.track_offset + q;
+        const Track t = make_track(a.bp, id);
+        const Raster r = make_raster(t, a.bp.n_f);
+        const int n_prows = (t.N + 63) >> 6;         // packed rows: columns [64 pr, 64 pr + 64)
+        wr.pixels += (unsigned long long)t.N;
+        const float scale = norm_scale(t.N, a.norm);
+#pragma unroll 1
+        for (int j = 0; j < n_chunks; ++j) {
+            if ((j & (kSuper / kChunk - 1)) == 0) {
+                // ---- anchor phase of super-chunk s: state (x, d) of every pixel at delay s * R
+                const int s = j / (kSuper / kChunk);
+                const float2* Es = a.Es + (size_t)s * (size_t)a.bp.n_f;
+#pragma unroll 1
+                for (int pr = 0; pr < n_prows; ++pr) {
+                    const int e = pr * kWarp + lane;
+                    const int cA = pr * 64 + lane, cB = cA + kWarp;
+                    int kA = 0, kB = 0;
+                    if (s == 0) {
+                        if (cA < t.N) kA = raster_bin(r, cA);
+                        if (cB < t.N) kB = raster_bin(r, cB);
+                        pool_k[e] = (uint32_t)kA | ((uint32_t)kB << 16);
+                    } else {
+                        const uint32_t kk = pool_k[e];
+                        kA = (int)(kk & 0xFFFFu); kB = (int)(kk >> 16);
+                    }
+                    float xA = 0.f, dA = 0.f, xB = 0.f, dB = 0.f;
+                    if (cA < t.N) {
+                        const float2 p = __ldg(&a.map[(size_t)(t.j0 + cA) * (size_t)a.bp.n_f + (size_t)kA]);
+                        const float2 w = __ldg(&Es[kA]);
+                        const float2 z = sm_kz[kA];
+                        const float vr = p.x * w.x - p.y * w.y, vi = p.x * w.y + p.y * w.x;
+                        xA = vr;                                   // x_m
+                        dA = fmaf(-0.5f * z.x, vr, -(z.y * vi));   // x_m - x_{m-1} = 2 sin^2(theta/2) Re v - sin(theta) Im v
+                    }
+                    if (cB < t.N) {
+                        const float2 p = __ldg(&a.map[(size_t)(t.j0 + cB) * (size_t)a.bp.n_f + (size_t)kB]);
+                        const float2 w = __ldg(&Es[kB]);
+                        const float2 z = sm_kz[kB];
+                        const float vr = p.x * w.x - p.y * w.y, vi = p.x * w.y + p.y * w.x;
+                        xB = vr;
+                        dB = fmaf(-0.5f * z.x, vr, -(z.y * vi));
+                    }
+                    pool_x[e] = pk_make(xA, xB);
+                    pool_d[e] = pk_make(dA, dB);
+                }
+            }
+            // ---- one chunk of 32 delays
+            f32x2_t acc[kChunk];
+#pragma unroll
+            for (int i = 0; i < kChunk; ++i) acc[i] = 0ull;
+            int pr = 0;
+            if (NCHAIN == 2) {
+#pragma unroll 1
+                for (; pr + 2 <= n_prows; pr += 2) {
+                    const int e0 = pr * kWarp + lane, e1 = e0 + kWarp;
+                    f32x2_t x0 = pool_x[e0], d0 = pool_d[e0], x1 = pool_x[e1], d1 = pool_d[e1];
+                    const uint32_t kk0 = pool_k[e0], kk1 = pool_k[e1];
+                    const f32x2_t nk0 = pk_make(sm_negk[2 * (kk0 & 0xFFFFu)], sm_negk[2 * (kk0 >> 16)]);
+                    const f32x2_t nk1 = pk_make(sm_negk[2 * (kk1 & 0xFFFFu)], sm_negk[2 * (kk1 >> 16)]);
+#pragma unroll
+                    for (int i = 0; i < kChunk; ++i) {
+                        acc[i] = pk_add(acc[i], x0);
+                        d0 = pk_fma(nk0, x0, d0);
+                        d1 = pk_fma(nk1, x1, d1);
+                        acc[i] = pk_add(acc[i], x1);
+                        x0 = pk_add(x0, d0);
+                        x1 = pk_add(x1, d1);
+                    }
+                    pool_x[e0] = x0; pool_d[e0] = d0; pool_x[e1] = x1; pool_d[e1] = d1;
+                }
+            }
+#pragma unroll 1
+            for (; pr < n_prows; ++pr) {
+                const int e0 = pr * kWarp + lane;
+                f32x2_t x0 = pool_x[e0], d0 = pool_d[e0];
+                const uint32_t kk0 = pool_k[e0];
+                const f32x2_t nk0 = pk_make(sm_negk[2 * (kk0 & 0xFFFFu)], sm_negk[2 * (kk0 >> 16)]);
+#pragma unroll
+                for (int i = 0; i < kChunk; ++i) {
+                    acc[i] = pk_add(acc[i], x0);
+                    d0 = pk_fma(nk0, x0, d0);
+                    x0 = pk_add(x0, d0);
+                }
+                pool_x[e0] = x0; pool_d[e0] = d0;
+            }
+            // ---- fold: packed halves, then the transposing tree across the 32 lanes
+            float f[kChunk];
+#pragma unroll
+            for (int i = 0; i < kChunk; ++i) f[i] = pk_sum(acc[i]);
+#pragma unroll
+            for (int off = 16, n = kChunk / 2; off >= 1; off >>= 1, n >>= 1) {
+                const bool upper = (lane & off) != 0;
+#pragma unroll
+                for (int i = 0; i < n; ++i) {
+                    const float send = upper ? f[i] : f[i + n];
+                    const float keep = upper ? f[i + n] : f[i];
+                    f[i] = keep + __shfl_xor_sync(kFull, send, off);
+                }
+            }
+            const float v[1] = {f[0] * scale};
+            const uint32_t ms[1] = {(uint32_t)(j * kChunk + lane)};
+            const bool ok[1] = {(int)ms[0] < a.n_tau};
+            reduce_samples<1>(a, wr, sm_hist, id, q, v, ms, ok);
         }
     }
     reduce_finish(a, wr);

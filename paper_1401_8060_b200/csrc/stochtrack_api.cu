@@ -25,7 +25,7 @@ constexpr uint64_t kMaxSamplesPerLaunch = 1ull << 31;   // keeps per-block u32 h
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t map, e0, bintab, w, tau, hist, scalars, result, cand, warp_best, stage_csd, stage_sigma, total;
+    size_t map, e0, bintab, es, kz, w, tau, hist, scalars, result, cand, warp_best, stage_csd, stage_sigma, total;
 };
 
 Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
@@ -36,6 +36,8 @@ Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
     L.map = o;         o += align_up(n_pix * sizeof(float2));
     L.e0 = o;          o += align_up((size_t)n_f * sizeof(float2));
     L.bintab = o;      o += align_up((size_t)n_f * sizeof(float4));
+    L.es = o;          o += align_up((size_t)n_f * (size_t)((max_n_tau + st::kSuper - 1) / st::kSuper) * sizeof(float2));
+    L.kz = o;          o += align_up((size_t)n_f * sizeof(float2));
     L.w = o;           o += align_up((size_t)n_f * (size_t)max_n_tau * sizeof(float2));
     L.tau = o;         o += align_up((size_t)max_n_tau * sizeof(double));
     L.hist = o;        o += align_up((size_t)ST_MAX_BINS * sizeof(unsigned long long));
@@ -69,7 +71,8 @@ struct st_ctx {
     st::DeviceResult* h_res;           // pinned
     unsigned long long* h_hist;        // pinned, ST_MAX_BINS
     int n_sm, smem_optin;
-    int recur_threads;                 // tunable: threads per block of k_score_recur
+    int recur_threads;                 // tunable: threads per block of the recurrence kernels
+    int reinsch_chains;                // tunable: packed recurrence chains in flight per lane (1 or 2)
     char err[512];
 };
 
@@ -183,7 +186,8 @@ int make_plan(st_ctx* c, const st_search_params* p, Plan* plan)
     if ((k == ST_KERNEL_ROTATION || k == ST_KERNEL_REINSCH) && !uni)
         return fail(c, ST_EINVAL, "recurrence kernels need a uniform tau grid");
     plan->kernel = k;
-    if (k != ST_KERNEL_TABLE) plan->ch = pick_chunk(p->n_tau);
+    if (k == ST_KERNEL_ROTATION) plan->ch = pick_chunk(p->n_tau);
+    if (k == ST_KERNEL_REINSCH) plan->ch = st::kChunk;
     return ST_OK;
 }
 
@@ -208,14 +212,22 @@ int ensure_tables(st_ctx* c, const st_search_params* p, const Plan& plan, int* n
             ST_CUDA(c, cudaGetLastError());
             c->w_built = true; ++*n_launches;
         }
-    } else {
-        const int want = plan.kernel == ST_KERNEL_ROTATION ? kRotTable : kReinschTable;
-        if (c->table_kind != want || c->table_ch != plan.ch) {
+    } else if (plan.kernel == ST_KERNEL_ROTATION) {
+        if (c->table_kind != kRotTable || c->table_ch != plan.ch) {
             st::k_build_bin_tables<<<(c->n_f + 127) / 128, 128, 0, c->stream>>>(
-                plan.tau0, plan.dtau, plan.ch, want == kRotTable ? 0 : 1, c->n_f, c->f_min, c->df,
+                plan.tau0, plan.dtau, plan.ch, 0, c->n_f, c->f_min, c->df,
                 at<float2>(c, c->L.e0), at<float4>(c, c->L.bintab));
             ST_CUDA(c, cudaGetLastError());
-            c->table_kind = want; c->table_ch = plan.ch; ++*n_launches;
+            c->table_kind = kRotTable; c->table_ch = plan.ch; ++*n_launches;
+        }
+    } else {
+        if (c->table_kind != kReinschTable) {
+            const int n_super = (p->n_tau + st::kSuper - 1) / st::kSuper;
+            st::k_build_reinsch_tables<<<(c->n_f + 127) / 128, 128, 0, c->stream>>>(
+                plan.tau0, plan.dtau, st::kSuper, n_super, c->n_f, c->f_min, c->df,
+                at<float2>(c, c->L.es), at<float2>(c, c->L.kz));
+            ST_CUDA(c, cudaGetLastError());
+            c->table_kind = kReinschTable; c->table_ch = plan.ch; ++*n_launches;
         }
     }
     return ST_OK;
@@ -261,6 +273,24 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
         st::k_score_table<<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+    } else if (plan.kernel == ST_KERNEL_REINSCH) {
+        int threads = c->recur_threads;
+        size_t smem;
+        for (;; threads -= 32) {
+            smem = hist_bytes(a.n_bins) + (size_t)(c->n_f + (c->n_f & 1)) * sizeof(float2) +
+                   (size_t)(threads / 32) * (size_t)(stride / 2) * (8 + 8 + 4);
+            if (smem <= (size_t)c->smem_optin || threads == 32) break;
+        }
+        if (smem > (size_t)c->smem_optin)
+            return fail(c, ST_ENOSPC, "n_f %d / n_max %d need more shared memory than one SM has", c->n_f, n_max);
+        const bool two = c->reinsch_chains == 2;
+        int rc = two ? set_smem(c, st::k_score_reinsch<2>, smem) : set_smem(c, st::k_score_reinsch<1>, smem);
+        if (rc) return rc;
+        uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
+        const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
+        if (blocks > need) blocks = need;
+        if (two) st::k_score_reinsch<2><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        else st::k_score_reinsch<1><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
     } else {
         int threads = c->recur_threads;
         const size_t bt_bytes = (size_t)c->n_f * sizeof(float4);
@@ -278,20 +308,14 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
-        const bool rot = plan.kernel == ST_KERNEL_ROTATION;
 #define ST_LAUNCH_RECUR(MODE, CH, BT)                                                              \
     do {                                                                                           \
         int rc_ = set_smem(c, st::k_score_recur<MODE, CH, BT>, smem);                              \
         if (rc_) return rc_;                                                                       \
         st::k_score_recur<MODE, CH, BT><<<(unsigned)blocks, threads, smem, c->stream>>>(a);        \
     } while (0)
-        if (rot) {
-            if (plan.ch == 32) { if (bt_smem) ST_LAUNCH_RECUR(0, 32, true); else ST_LAUNCH_RECUR(0, 32, false); }
-            else               { if (bt_smem) ST_LAUNCH_RECUR(0, 64, true); else ST_LAUNCH_RECUR(0, 64, false); }
-        } else {
-            if (plan.ch == 32) { if (bt_smem) ST_LAUNCH_RECUR(1, 32, true); else ST_LAUNCH_RECUR(1, 32, false); }
-            else               { if (bt_smem) ST_LAUNCH_RECUR(1, 64, true); else ST_LAUNCH_RECUR(1, 64, false); }
-        }
+        if (plan.ch == 32) { if (bt_smem) ST_LAUNCH_RECUR(0, 32, true); else ST_LAUNCH_RECUR(0, 32, false); }
+        else               { if (bt_smem) ST_LAUNCH_RECUR(0, 64, true); else ST_LAUNCH_RECUR(0, 64, false); }
 #undef ST_LAUNCH_RECUR
     }
     ST_CUDA(c, cudaGetLastError());
@@ -310,6 +334,8 @@ st::ScoreArgs base_args(st_ctx* c, const st_search_params* p)
     a.W = at<float2>(c, c->L.w);
     a.E0 = at<float2>(c, c->L.e0);
     a.bintab = at<float4>(c, c->L.bintab);
+    a.Es = at<float2>(c, c->L.es);
+    a.kz = at<float2>(c, c->L.kz);
     a.sc = at<st::Scalars>(c, c->L.scalars);
     a.cand = at<st::Cand>(c, c->L.cand);
     a.cand_cap = kCandCap;
@@ -354,6 +380,9 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->ev0 = c->ev1 = nullptr; c->h_res = nullptr; c->h_hist = nullptr;
     c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512;
     c->err[0] = 0;
+    c->reinsch_chains = 2;
+    const char* e2 = getenv("ST_REINSCH_CHAINS");
+    if (e2 && atoi(e2) == 1) c->reinsch_chains = 1;
     const char* e = getenv("ST_RECUR_THREADS");
     if (e) { int t = atoi(e); if (t >= 32 && t <= 512 && t % 32 == 0) c->recur_threads = t; }
     *out = c;

@@ -87,7 +87,7 @@ def test_scores_grid_kernels_vs_oracle(P, orc, kname, cid, count):
 
 
 @pytest.mark.parametrize("kname", ["table", "rotation", "reinsch"])
-@pytest.mark.parametrize("n_tau", [1, 7, 33, 50, 128, 200])
+@pytest.mark.parametrize("n_tau", [1, 7, 33, 50, 128, 200, 600])
 def test_scores_ragged_tau_counts(P, orc, kname, n_tau):
     """Grid sizes that are not multiples of the 32/64-delay chunks, on the config-5 shape
     with per-pixel sigma (several 32-column rows and a ragged tail per track)."""
@@ -176,7 +176,10 @@ def _assert_search_parity(r, ref, cfg, check_hist=True):
     assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"]), (r, ref["max_snr"])
     assert r.n_pixels == ref["n_pixels"] and r.n_evals == ref["n_evals"]
     assert abs(r.max_snr - ref["max_snr"]) <= 1e-4 * abs(ref["max_snr"])          # float32 kernel value
-    assert abs(r.max_snr_f64 - ref["max_snr"]) <= 1e-9 * abs(ref["max_snr"])      # float64 re-score
+    # float64 re-score of the argmax: float64 arithmetic on the library's float32 map p = CSD/sigma
+    # (2^-24 relative rounding per pixel when sigma != 1; exact when sigma is absent)
+    rel64 = 1e-11 if cfg.sigma == "none" else 2e-7
+    assert abs(r.max_snr_f64 - ref["max_snr"]) <= rel64 * abs(ref["max_snr"])
     assert r.arg_tau == pytest.approx(ref["arg_tau"], abs=1e-15)
     assert r.flags == 0 and r.n_candidates >= 1
     if check_hist:
@@ -220,7 +223,7 @@ def test_search_mean_norm_and_offsets(P, orc):
     cfg = synth.CONFIGS[2]
     r, ref = _search_both(P, orc, cfg, 20000, norm=1, offset=777_000)
     assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
-    assert abs(r.max_snr_f64 - ref["max_snr"]) <= 1e-9 * abs(ref["max_snr"])
+    assert abs(r.max_snr_f64 - ref["max_snr"]) <= 2e-7 * abs(ref["max_snr"])
 
 
 @pytest.mark.parametrize("cid,m,ranges", [
@@ -304,7 +307,7 @@ def test_edge_cases(P, orc):
     p = orc.prepare_map(csd, sigma)
     ref = orc.search(p, cfg.f_min, cfg.df, 1, 5, 1, 1, tau_grid=np.array([0.001]), n_bins=10)
     assert r.n_evals == 1 and (r.arg_track, r.arg_tau_index) == (0, 0)
-    assert r.max_snr_f64 == pytest.approx(ref["max_snr"], rel=1e-12)
+    assert r.max_snr_f64 == pytest.approx(ref["max_snr"], rel=2e-7)      # float32 map p = CSD/sigma
     assert np.array_equal(r.hist, ref["hist"])
     # maximum-length tracks only (n_min = n_max = n_t), per-pixel sigma with masked pixels (G11)
     sig2 = np.ones((cfg.n_t, cfg.n_f), dtype=np.float32)
