@@ -60,13 +60,15 @@ extern "C" {
 #define ST_NORM_SQRT_N 0
 #define ST_NORM_MEAN   1
 
-/* scoring kernel selection (grid mode).  AUTO picks REINSCH when the grid is
- * uniform and well conditioned, else ROTATION when uniform, else TABLE.       */
+/* scoring kernel selection (grid mode).  AUTO picks CHEBYSHEV when the grid is
+ * uniform and every bin's step angle is well conditioned, else REINSCH / ROTATION
+ * when uniform, else TABLE.                                                     */
 #define ST_KERNEL_AUTO     0
 #define ST_KERNEL_TABLE    1   /* twiddle table W[k][m] read from L2, any grid          */
 #define ST_KERNEL_ROTATION 2   /* complex rotation recurrence along a uniform tau grid  */
 #define ST_KERNEL_REINSCH  3   /* real three-term (Reinsch) recurrence, uniform grid    */
 #define ST_KERNEL_RANDOM   4   /* reported in st_result for ST_TAU_RANDOM searches      */
+#define ST_KERNEL_CHEBYSHEV 5  /* two-sided Chebyshev recurrence, uniform grid (1 FMA per eval) */
 
 typedef struct st_ctx st_ctx;   /* opaque */
 

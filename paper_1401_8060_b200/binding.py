@@ -6,15 +6,16 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libstochtrack_b200.so")
+# ST_LIB_PATH selects another build of the same C ABI (e.g. a tuning variant)
+_LIB_PATH = os.environ.get("ST_LIB_PATH") or os.path.join(_HERE, "libstochtrack_b200.so")
 
 ST_OK, ST_EINVAL, ST_ESTATE, ST_ENOSPC, ST_ECUDA = 0, -1, -2, -3, -4
 _CODES = {ST_EINVAL: "ST_EINVAL", ST_ESTATE: "ST_ESTATE", ST_ENOSPC: "ST_ENOSPC", ST_ECUDA: "ST_ECUDA"}
 SIGMA_NONE, SIGMA_PER_FREQ, SIGMA_PER_PIXEL = 0, 1, 2
 TAU_GRID, TAU_RANDOM = 0, 1
 NORM_SQRT_N, NORM_MEAN = 0, 1
-KERNEL_AUTO, KERNEL_TABLE, KERNEL_ROTATION, KERNEL_REINSCH, KERNEL_RANDOM = 0, 1, 2, 3, 4
-KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random"}
+KERNEL_AUTO, KERNEL_TABLE, KERNEL_ROTATION, KERNEL_REINSCH, KERNEL_RANDOM, KERNEL_CHEBYSHEV = 0, 1, 2, 3, 4, 5
+KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random", 5: "chebyshev"}
 
 # every symbol include/stochtrack.h declares
 exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_workspace", "st_set_map",

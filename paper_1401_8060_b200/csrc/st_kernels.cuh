@@ -72,6 +72,8 @@ struct ScoreArgs {
     const float4* bintab;     // [n_f] per-bin recurrence constants (rotation kernel)
     const float2* Es;         // [n_super][n_f] e^{2 pi i f_k tau_{s R}}: anchors of the Reinsch kernel
     const float2* kz;         // [n_f] (-4 sin^2(theta_k/2), sin theta_k)
+    const float2* Ec;         // [n_f] e^{2 pi i f_k tau_{32}}: first anchor of the Chebyshev kernel
+    const float4* cheb;       // [n_f] (2 cos theta, sin theta, cos 64 theta, sin 64 theta)
     Scalars* sc;
     Cand* cand;
     uint32_t cand_cap;
@@ -309,6 +311,28 @@ __global__ void k_build_reinsch_tables(double tau0, double dtau, int r_super, in
     sincospi(2.0 * cyc, &zs, &zc);
     sincospi(cyc, &hs, &hc);
     kz[k] = make_float2((float)(-4.0 * hs * hs), (float)zs);
+}
+
+// Tables of k_score_cheb on the uniform grid: Ec[k] = e^{2 pi i f_k (tau0 + 32 dtau)} (anchor of
+// chunk 0 at its centre), cheb[k] = (2 cos theta_k, sin theta_k, cos 64 theta_k, sin 64 theta_k).
+__global__ void k_build_cheb_tables(double tau0, double dtau, int n_f, double f_min, double df,
+                                    float2* __restrict__ Ec, float4* __restrict__ cheb)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_f) return;
+    const double f = f_min + (double)k * df;
+    double s, c;
+    const double c0 = f * (tau0 + 32.0 * dtau);
+    sincospi(2.0 * (c0 - rint(c0)), &s, &c);
+    Ec[k] = make_float2((float)c, (float)s);
+    double cyc = f * dtau;
+    cyc -= rint(cyc);
+    double zs, zc, ms, mc;
+    sincospi(2.0 * cyc, &zs, &zc);
+    double c64 = cyc * 64.0;
+    c64 -= rint(c64);
+    sincospi(2.0 * c64, &ms, &mc);
+    cheb[k] = make_float4((float)(2.0 * zc), (float)zs, (float)mc, (float)ms);
 }
 
 // --------------------------------------------------- S1-S4, table, any grid --
@@ -558,11 +582,35 @@ __device__ __forceinline__ f32x2_t pk_add(f32x2_t a, f32x2_t b)
     asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
     return r;
 }
+// d = fma(nk, x, d) on the two halves with scalar FFMAs: fma.rn.f32x2 with three distinct
+// register-pair operands issues at 2/3 rate (register-file bandwidth; st_microbench
+// ffma2_3distinct), two scalar FFMAs cost the same pipe time as one full-rate packed op.
+__device__ __forceinline__ f32x2_t pk_fma_halves(f32x2_t a, f32x2_t b, f32x2_t c)
+{
+    f32x2_t r;
+    asm volatile("{\n\t.reg .f32 al, ah, bl, bh, cl, ch;\n\t"
+                 "mov.b64 {al, ah}, %1;\n\tmov.b64 {bl, bh}, %2;\n\tmov.b64 {cl, ch}, %3;\n\t"
+                 "fma.rn.f32 cl, al, bl, cl;\n\tfma.rn.f32 ch, ah, bh, ch;\n\t"
+                 "mov.b64 %0, {cl, ch};\n\t}" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
 __device__ __forceinline__ f32x2_t pk_make(float lo, float hi)
 {
     f32x2_t r;
     asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
     return r;
+}
+__device__ __forceinline__ float pk_lo(f32x2_t a)
+{
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a));
+    return lo;
+}
+__device__ __forceinline__ float pk_hi(f32x2_t a)
+{
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a));
+    return hi;
 }
 __device__ __forceinline__ float pk_sum(f32x2_t a)
 {
@@ -574,7 +622,7 @@ __device__ __forceinline__ float pk_sum(f32x2_t a)
 constexpr int kChunk = 32;        // delays per accumulator chunk
 constexpr int kSuper = 256;       // delays between re-anchoring (8 chunks)
 
-template <int NCHAIN>
+template <int VAR>
 __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -591,6 +639,10 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
     for (int k = threadIdx.x; k < a.bp.n_f; k += blockDim.x) sm_kz[k] = a.kz[k];
     hist_init(sm_hist, a.n_bins);
     const float* sm_negk = reinterpret_cast<const float*>(sm_kz);     // sm_negk[2k] = -kappa_k
+#ifdef ST_EXP_NOANCHOR
+    for (int e = lane; e < P; e += kWarp) { pool_x[e] = 0ull; pool_d[e] = 0ull; pool_k[e] = 0u; }
+    __syncwarp();
+#endif
     const int n_chunks = (a.n_tau + kChunk - 1) / kChunk;
     WarpReduce wr;
     reduce_init(wr);
@@ -605,87 +657,150 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
         const float scale = norm_scale(t.N, a.norm);
 #pragma unroll 1
         for (int j = 0; j < n_chunks; ++j) {
+#ifdef ST_EXP_ONEANCHOR
+            if (j == 0) {
+#else
             if ((j & (kSuper / kChunk - 1)) == 0) {
+#endif
                 // ---- anchor phase of super-chunk s: state (x, d) of every pixel at delay s * R
                 const int s = j / (kSuper / kChunk);
                 const float2* Es = a.Es + (size_t)s * (size_t)a.bp.n_f;
+#ifdef ST_EXP_NOANCHOR
+                if (s == 0 && q > (1ull << 62)) {
+#else
+                if (s == 0) {
+#endif
+                    // rasterise: four columns per lane in flight (FP64 div / sqrt chains are long)
 #pragma unroll 1
-                for (int pr = 0; pr < n_prows; ++pr) {
-                    const int e = pr * kWarp + lane;
-                    const int cA = pr * 64 + lane, cB = cA + kWarp;
-                    int kA = 0, kB = 0;
-                    if (s == 0) {
-                        if (cA < t.N) kA = raster_bin(r, cA);
-                        if (cB < t.N) kB = raster_bin(r, cB);
-                        pool_k[e] = (uint32_t)kA | ((uint32_t)kB << 16);
-                    } else {
-                        const uint32_t kk = pool_k[e];
-                        kA = (int)(kk & 0xFFFFu); kB = (int)(kk >> 16);
+                    for (int pr = 0; pr < n_prows; pr += 2) {
+                        const int c0 = pr * 64 + lane;
+                        int k[4];
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            const int c = c0 + u * kWarp;
+                            k[u] = raster_bin(r, c < t.N ? c : t.N - 1);
+                        }
+                        pool_k[pr * kWarp + lane] = (uint32_t)k[0] | ((uint32_t)k[1] << 16);
+                        if (pr + 1 < n_prows) pool_k[(pr + 1) * kWarp + lane] = (uint32_t)k[2] | ((uint32_t)k[3] << 16);
                     }
-                    float xA = 0.f, dA = 0.f, xB = 0.f, dB = 0.f;
-                    if (cA < t.N) {
-                        const float2 p = __ldg(&a.map[(size_t)(t.j0 + cA) * (size_t)a.bp.n_f + (size_t)kA]);
-                        const float2 w = __ldg(&Es[kA]);
-                        const float2 z = sm_kz[kA];
-                        const float vr = p.x * w.x - p.y * w.y, vi = p.x * w.y + p.y * w.x;
-                        xA = vr;                                   // x_m
-                        dA = fmaf(-0.5f * z.x, vr, -(z.y * vi));   // x_m - x_{m-1} = 2 sin^2(theta/2) Re v - sin(theta) Im v
+                }
+                // gather p and the anchor phase factor: 16 independent L2 loads in flight per lane
+#pragma unroll 1
+#ifdef ST_EXP_NOANCHOR
+                for (int pr = 0; pr < (q > (1ull << 62) ? n_prows : 0); pr += 4) {
+#else
+                for (int pr = 0; pr < n_prows; pr += 4) {
+#endif
+                    float2 pv[8], wv[8];
+                    int kq[8];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int prow = pr + u < n_prows ? pr + u : n_prows - 1;
+                        const uint32_t kk = pool_k[prow * kWarp + lane];
+                        kq[2 * u] = (int)(kk & 0xFFFFu);
+                        kq[2 * u + 1] = (int)(kk >> 16);
                     }
-                    if (cB < t.N) {
-                        const float2 p = __ldg(&a.map[(size_t)(t.j0 + cB) * (size_t)a.bp.n_f + (size_t)kB]);
-                        const float2 w = __ldg(&Es[kB]);
-                        const float2 z = sm_kz[kB];
-                        const float vr = p.x * w.x - p.y * w.y, vi = p.x * w.y + p.y * w.x;
-                        xB = vr;
-                        dB = fmaf(-0.5f * z.x, vr, -(z.y * vi));
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const int prow = pr + (u >> 1) < n_prows ? pr + (u >> 1) : n_prows - 1;
+                        int c = prow * 64 + (u & 1) * kWarp + lane;
+                        c = c < t.N ? c : t.N - 1;       // clamped: the value is discarded below
+                        pv[u] = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)kq[u]]);
+                        wv[u] = __ldg(&Es[kq[u]]);
                     }
-                    pool_x[e] = pk_make(xA, xB);
-                    pool_d[e] = pk_make(dA, dB);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (pr + u < n_prows) {
+                            float x[2], d[2];
+#pragma unroll
+                            for (int h = 0; h < 2; ++h) {
+                                const int c = (pr + u) * 64 + h * kWarp + lane;
+                                const float2 p = pv[2 * u + h], w = wv[2 * u + h];
+                                const float2 z = sm_kz[kq[2 * u + h]];
+                                const float vr = p.x * w.x - p.y * w.y, vi = p.x * w.y + p.y * w.x;
+                                // x_m = Re v ; x_m - x_{m-1} = 2 sin^2(theta/2) Re v - sin(theta) Im v
+                                x[h] = c < t.N ? vr : 0.0f;
+                                d[h] = c < t.N ? fmaf(-0.5f * z.x, vr, -(z.y * vi)) : 0.0f;
+                            }
+                            pool_x[(pr + u) * kWarp + lane] = pk_make(x[0], x[1]);
+                            pool_d[(pr + u) * kWarp + lane] = pk_make(d[0], d[1]);
+                        }
+                    }
                 }
             }
-            // ---- one chunk of 32 delays
-            f32x2_t acc[kChunk];
+            // ---- one chunk of 32 delays: four pixels of the lane in flight (two register pairs).
+            // Per delay and pair: two scalar FFMAs (d += -kappa x on the halves; a packed FFMA with
+            // three distinct register pairs issues at 2/3 rate), one packed add (x += d) and the
+            // accumulation.  VAR 0: four scalar adds into acc[i]; VAR 1: one packed add of the two
+            // pairs, then two scalar adds (fewer issue slots).
+            float f[kChunk];
 #pragma unroll
-            for (int i = 0; i < kChunk; ++i) acc[i] = 0ull;
+            for (int i = 0; i < kChunk; ++i) f[i] = 0.0f;
             int pr = 0;
-            if (NCHAIN == 2) {
 #pragma unroll 1
-                for (; pr + 2 <= n_prows; pr += 2) {
-                    const int e0 = pr * kWarp + lane, e1 = e0 + kWarp;
-                    f32x2_t x0 = pool_x[e0], d0 = pool_d[e0], x1 = pool_x[e1], d1 = pool_d[e1];
-                    const uint32_t kk0 = pool_k[e0], kk1 = pool_k[e1];
-                    const f32x2_t nk0 = pk_make(sm_negk[2 * (kk0 & 0xFFFFu)], sm_negk[2 * (kk0 >> 16)]);
-                    const f32x2_t nk1 = pk_make(sm_negk[2 * (kk1 & 0xFFFFu)], sm_negk[2 * (kk1 >> 16)]);
+            for (; pr + 2 <= n_prows; pr += 2) {
+                const int e0 = pr * kWarp + lane, e1 = e0 + kWarp;
+                f32x2_t x0 = pool_x[e0], d0 = pool_d[e0], x1 = pool_x[e1], d1 = pool_d[e1];
+                const uint32_t kk0 = pool_k[e0], kk1 = pool_k[e1];
+                const f32x2_t nk0 = pk_make(sm_negk[2 * (kk0 & 0xFFFFu)], sm_negk[2 * (kk0 >> 16)]);
+                const f32x2_t nk1 = pk_make(sm_negk[2 * (kk1 & 0xFFFFu)], sm_negk[2 * (kk1 >> 16)]);
+                if (VAR <= 1) {
 #pragma unroll
                     for (int i = 0; i < kChunk; ++i) {
-                        acc[i] = pk_add(acc[i], x0);
-                        d0 = pk_fma(nk0, x0, d0);
-                        d1 = pk_fma(nk1, x1, d1);
-                        acc[i] = pk_add(acc[i], x1);
+                        if (VAR == 0) {
+                            f[i] += pk_lo(x0); f[i] += pk_hi(x0);
+                            f[i] += pk_lo(x1); f[i] += pk_hi(x1);
+                        } else {
+                            const f32x2_t sx = pk_add(x0, x1);
+                            f[i] += pk_lo(sx); f[i] += pk_hi(sx);
+                        }
+                        d0 = pk_fma_halves(nk0, x0, d0);
+                        d1 = pk_fma_halves(nk1, x1, d1);
                         x0 = pk_add(x0, d0);
                         x1 = pk_add(x1, d1);
                     }
-                    pool_x[e0] = x0; pool_d[e0] = d0; pool_x[e1] = x1; pool_d[e1] = d1;
+                } else if (VAR == 2) {
+                    // same arithmetic, every packed value updated in place (stable register pairs)
+                    f32x2_t sx = pk_add(x0, x1);
+#pragma unroll
+                    for (int i = 0; i < kChunk; ++i) {
+                        f[i] += pk_lo(sx); f[i] += pk_hi(sx);
+                        d0 = pk_fma_halves(nk0, x0, d0);
+                        d1 = pk_fma_halves(nk1, x1, d1);
+                        x0 = pk_add(x0, d0);
+                        x1 = pk_add(x1, d1);
+                        sx = pk_add(x0, x1);
+                    }
+                } else {
+                    // all scalar: four independent chains, 32-bit operands only
+                    float a0 = pk_lo(x0), a1 = pk_hi(x0), a2 = pk_lo(x1), a3 = pk_hi(x1);
+                    float b0 = pk_lo(d0), b1 = pk_hi(d0), b2 = pk_lo(d1), b3 = pk_hi(d1);
+                    const float k0 = pk_lo(nk0), k1 = pk_hi(nk0), k2 = pk_lo(nk1), k3 = pk_hi(nk1);
+#pragma unroll
+                    for (int i = 0; i < kChunk; ++i) {
+                        f[i] += (a0 + a1) + (a2 + a3);
+                        b0 = fmaf(k0, a0, b0); b1 = fmaf(k1, a1, b1); b2 = fmaf(k2, a2, b2); b3 = fmaf(k3, a3, b3);
+                        a0 += b0; a1 += b1; a2 += b2; a3 += b3;
+                    }
+                    x0 = pk_make(a0, a1); x1 = pk_make(a2, a3); d0 = pk_make(b0, b1); d1 = pk_make(b2, b3);
                 }
+                pool_x[e0] = x0; pool_d[e0] = d0; pool_x[e1] = x1; pool_d[e1] = d1;
             }
-#pragma unroll 1
-            for (; pr < n_prows; ++pr) {
+            if (pr < n_prows) {          // odd tail: one pair
                 const int e0 = pr * kWarp + lane;
                 f32x2_t x0 = pool_x[e0], d0 = pool_d[e0];
                 const uint32_t kk0 = pool_k[e0];
                 const f32x2_t nk0 = pk_make(sm_negk[2 * (kk0 & 0xFFFFu)], sm_negk[2 * (kk0 >> 16)]);
 #pragma unroll
                 for (int i = 0; i < kChunk; ++i) {
-                    acc[i] = pk_add(acc[i], x0);
-                    d0 = pk_fma(nk0, x0, d0);
+                    f[i] += pk_lo(x0); f[i] += pk_hi(x0);
+                    d0 = pk_fma_halves(nk0, x0, d0);
                     x0 = pk_add(x0, d0);
                 }
                 pool_x[e0] = x0; pool_d[e0] = d0;
             }
-            // ---- fold: packed halves, then the transposing tree across the 32 lanes
-            float f[kChunk];
-#pragma unroll
-            for (int i = 0; i < kChunk; ++i) f[i] = pk_sum(acc[i]);
+            // ---- fold: the transposing tree across the 32 lanes
+#ifndef ST_EXP_NOFOLD
 #pragma unroll
             for (int off = 16, n = kChunk / 2; off >= 1; off >>= 1, n >>= 1) {
                 const bool upper = (lane & off) != 0;
@@ -696,15 +811,173 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
                     f[i] = keep + __shfl_xor_sync(kFull, send, off);
                 }
             }
+#else
+#pragma unroll
+            for (int i = 1; i < kChunk; ++i) f[0] += f[i];
+#endif
             const float v[1] = {f[0] * scale};
             const uint32_t ms[1] = {(uint32_t)(j * kChunk + lane)};
             const bool ok[1] = {(int)ms[0] < a.n_tau};
+#ifndef ST_EXP_NOREDUCE
             reduce_samples<1>(a, wr, sm_hist, id, q, v, ms, ok);
+#else
+            if (v[0] == 123.456f && ok[0]) wr.pixels += ms[0];
+#endif
         }
     }
     reduce_finish(a, wr);
     hist_flush(sm_hist, a.hist, a.n_bins);
 }
+
+
+// ------------------ S1-S4, uniform tau grid, two-sided Chebyshev recurrence --
+// The production kernel of the grid mode.  Warp per template, lanes over pixels.
+// A pixel's term of Eq. 8 along the uniform delay grid, x_m = Re[p e^{2 pi i f (tau_0 + m dtau)}],
+// obeys the three-term recurrence of cos(psi + m theta):
+//     x_{m+1} = 2 cos(theta) x_m - x_{m-1}          (forward)
+//     x_{m-1} = 2 cos(theta) x_m - x_{m+1}          (backward, same coefficient)
+// i.e. ONE FMA per (pixel, delay); a second instruction accumulates it.  Delays are
+// processed in chunks of 64 around an anchor at the chunk centre m_c = 64 j + 32: the
+// complex anchor v = p e^{2 pi i f tau_{m_c}} gives x_{m_c} = Re v and x_{m_c - 1} =
+// Re[v e^{-i theta}], from which 32 forward and 32 backward steps run as two independent
+// chains; two pixels per lane are in flight (four chains).  The anchor of the next chunk
+// is v e^{i 64 theta} (table from float64), so recurrence error never spans more than 32
+// steps: a float32 coefficient 2 cos(theta) shifts the phase by <= 32 * 2^-25 / sin(theta)
+// (measured term error <= 3.3e-5 |p| at theta = 0.01, rms 2e-6; DESIGN.md error budget).
+// Per lane 64 float32 accumulators hold the partial sums over its pixels; a transposing
+// shuffle tree folds them across the warp, leaving delays 2l, 2l+1 of the chunk on lane l.
+constexpr int kCheb = 64;         // delays per chunk
+constexpr int kHalf = kCheb / 2;
+
+// one pixel row's two chains advanced by one delay each (forward into f[FI], backward into f[BI])
+#define ST_CHEB_STEP(FI, BI, g, fc, fp, bc, bp)                 \
+    do {                                                        \
+        f[FI] += fc;                                            \
+        f[BI] += bc;                                            \
+        const float fn_ = fmaf(g, fc, -fp);                     \
+        const float bn_ = fmaf(g, bc, -bp);                     \
+        fp = fc; fc = fn_;                                      \
+        bp = bc; bc = bn_;                                      \
+    } while (0)
+
+__global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_warps = blockDim.x >> 5;
+    // shared memory: hist | cheb[n_f] (float4) | v[n_warps][S] (float2) | k[n_warps][S] (u16), S = pool_stride
+    float4* sm_tab = reinterpret_cast<float4*>(sm_hist + hist_smem_words(a.n_bins));
+    const int S = a.pool_stride;
+    float2* pool_v = reinterpret_cast<float2*>(sm_tab + a.bp.n_f) + (size_t)warp * S;
+    uint16_t* pool_k = reinterpret_cast<uint16_t*>(reinterpret_cast<float2*>(sm_tab + a.bp.n_f) + (size_t)n_warps * S)
+                       + (size_t)warp * S;
+    for (int k = threadIdx.x; k < a.bp.n_f; k += blockDim.x) sm_tab[k] = a.cheb[k];
+    hist_init(sm_hist, a.n_bins);
+    const int n_chunks = (a.n_tau + kCheb - 1) / kCheb;
+    WarpReduce wr;
+    reduce_init(wr);
+    for (;;) {
+        const uint64_t q = next_track(a);
+        if (q >= a.n_tracks) break;
+        const uint64_t id = a.track_offset + q;
+        const Track t = make_track(a.bp, id);
+        const Raster r = make_raster(t, a.bp.n_f);
+        const int n_rows = (t.N + kWarp - 1) >> 5;     // rows of 32 columns
+        wr.pixels += (unsigned long long)t.N;
+        const float scale = norm_scale(t.N, a.norm);
+        // ---- phase A: rasterise (four columns per lane in flight), gather p, anchor of chunk 0
+#pragma unroll 1
+        for (int row = 0; row < n_rows; row += 4) {
+            int kq[4];
+            float2 pv[4], ev[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int c = (row + u) * kWarp + lane;
+                kq[u] = raster_bin(r, c < t.N ? c : t.N - 1);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                int c = (row + u) * kWarp + lane;
+                c = c < t.N ? c : t.N - 1;              // clamped: discarded below
+                pv[u] = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)kq[u]]);
+                ev[u] = __ldg(&a.Ec[kq[u]]);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (row + u < n_rows) {
+                    const int c = (row + u) * kWarp + lane;
+                    float2 v;
+                    v.x = pv[u].x * ev[u].x - pv[u].y * ev[u].y;
+                    v.y = pv[u].x * ev[u].y + pv[u].y * ev[u].x;
+                    if (c >= t.N) { v.x = 0.0f; v.y = 0.0f; }
+                    pool_v[c] = v;
+                    pool_k[c] = (uint16_t)kq[u];
+                }
+            }
+        }
+        // ---- phase B: chunks of 64 delays
+#pragma unroll 1
+        for (int j = 0; j < n_chunks; ++j) {
+            float f[kCheb];
+#pragma unroll
+            for (int i = 0; i < kCheb; ++i) f[i] = 0.0f;
+            int row = 0;
+#pragma unroll 1
+            for (; row + 2 <= n_rows; row += 2) {
+                const int e0 = row * kWarp + lane, e1 = e0 + kWarp;
+                const float2 v0 = pool_v[e0], v1 = pool_v[e1];
+                const float4 t0 = sm_tab[pool_k[e0]], t1 = sm_tab[pool_k[e1]];
+                // next chunk's anchors: v e^{i 64 theta}
+                pool_v[e0] = make_float2(fmaf(v0.x, t0.z, -(v0.y * t0.w)), fmaf(v0.x, t0.w, v0.y * t0.z));
+                pool_v[e1] = make_float2(fmaf(v1.x, t1.z, -(v1.y * t1.w)), fmaf(v1.x, t1.w, v1.y * t1.z));
+                const float g0 = t0.x, g1 = t1.x;
+                // x_{m_c} = Re v ; x_{m_c - 1} = Re[v e^{-i theta}] = cos(theta) Re v + sin(theta) Im v
+                float fc0 = v0.x, fp0 = fmaf(0.5f * g0, v0.x, t0.y * v0.y);
+                float fc1 = v1.x, fp1 = fmaf(0.5f * g1, v1.x, t1.y * v1.y);
+                float bc0 = fp0, bp0 = fc0, bc1 = fp1, bp1 = fc1;
+#pragma unroll
+                for (int i = 0; i < kHalf; ++i) {
+                    ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g0, fc0, fp0, bc0, bp0);
+                    ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g1, fc1, fp1, bc1, bp1);
+                }
+            }
+            if (row < n_rows) {          // odd tail row
+                const int e0 = row * kWarp + lane;
+                const float2 v0 = pool_v[e0];
+                const float4 t0 = sm_tab[pool_k[e0]];
+                pool_v[e0] = make_float2(fmaf(v0.x, t0.z, -(v0.y * t0.w)), fmaf(v0.x, t0.w, v0.y * t0.z));
+                const float g0 = t0.x;
+                float fc0 = v0.x, fp0 = fmaf(0.5f * g0, v0.x, t0.y * v0.y);
+                float bc0 = fp0, bp0 = fc0;
+#pragma unroll
+                for (int i = 0; i < kHalf; ++i) ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g0, fc0, fp0, bc0, bp0);
+            }
+            // ---- fold across the 32 lanes (transposing tree): lane l ends with delays 2l, 2l+1
+#pragma unroll
+            for (int off = 16, n = kCheb / 2; off >= 1; off >>= 1, n >>= 1) {
+                const bool upper = (lane & off) != 0;
+#pragma unroll
+                for (int i = 0; i < n; ++i) {
+                    const float send = upper ? f[i] : f[i + n];
+                    const float keep = upper ? f[i + n] : f[i];
+                    f[i] = keep + __shfl_xor_sync(kFull, send, off);
+                }
+            }
+            float v[2]; uint32_t ms[2]; bool ok[2];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                ms[i] = (uint32_t)(j * kCheb + 2 * lane + i);
+                ok[i] = (int)ms[i] < a.n_tau;
+                v[i] = f[i] * scale;
+            }
+            reduce_samples<2>(a, wr, sm_hist, id, q, v, ms, ok);
+        }
+    }
+    reduce_finish(a, wr);
+    hist_flush(sm_hist, a.hist, a.n_bins);
+}
+#undef ST_CHEB_STEP
 
 // ----------------------------------------------------------------------- S4 --
 // Float64 score of one (template, delay): Eq. 8 with cos/sin of 2 pi f tau in

@@ -99,6 +99,155 @@ __global__ void k_reinsch(float* out, float kappa)
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// The packed (f32x2) Reinsch inner loop exactly as k_score_reinsch issues it: per step and
+// chain  acc[i] += x ; d = fma(-kappa, x, d) ; x += d  on register pairs, 32 packed accumulators.
+typedef unsigned long long f32x2_t;
+__device__ __forceinline__ f32x2_t pk_fma(f32x2_t a, f32x2_t b, f32x2_t c)
+{ f32x2_t r; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ f32x2_t pk_add(f32x2_t a, f32x2_t b)
+{ f32x2_t r; asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2_t pk_make(float lo, float hi)
+{ f32x2_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ float pk_sum(f32x2_t a)
+{ float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a)); return lo + hi; }
+
+__device__ __forceinline__ f32x2_t pk_fma_halves(f32x2_t a, f32x2_t b, f32x2_t c)
+{
+    f32x2_t r;
+    asm volatile("{\n\t.reg .f32 al, ah, bl, bh, cl, ch;\n\t"
+                 "mov.b64 {al, ah}, %1;\n\tmov.b64 {bl, bh}, %2;\n\tmov.b64 {cl, ch}, %3;\n\t"
+                 "fma.rn.f32 cl, al, bl, cl;\n\tfma.rn.f32 ch, ah, bh, ch;\n\t"
+                 "mov.b64 %0, {cl, ch};\n\t}" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
+template <int NCH, bool MIXED>
+__global__ void k_reinsch_packed(float* out, float kappa)
+{
+    f32x2_t acc[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) acc[i] = 0ull;
+    f32x2_t x[NCH], d[NCH], nk[NCH];
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) {
+        x[c] = pk_make(threadIdx.x * 1e-3f + c, threadIdx.x * 2e-3f + c);
+        d[c] = pk_make(1e-3f * c, 2e-3f * c);
+        nk[c] = pk_make(-kappa * (c + 1), -kappa * (c + 2));
+    }
+#pragma unroll 1
+    for (int it = 0; it < kIters / 32; ++it) {
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) acc[i] = pk_add(acc[i], x[c]);
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) d[c] = MIXED ? pk_fma_halves(nk[c], x[c], d[c]) : pk_fma(nk[c], x[c], d[c]);
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) x[c] = pk_add(x[c], d[c]);
+        }
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < 32; ++i) s += pk_sum(acc[i]);
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+// Variant M2: scalar FFMA on the halves, ONE packed add for x += d, scalar accumulators
+// (NACC of them, both halves of a pair add into the same delay's accumulator).
+template <int NPK, int NACC>
+__global__ void k_reinsch_m2(float* out, float kappa)
+{
+    float acc[NACC];
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) acc[i] = 0.f;
+    f32x2_t x[NPK], d[NPK], nk[NPK];
+#pragma unroll
+    for (int c = 0; c < NPK; ++c) {
+        x[c] = pk_make(threadIdx.x * 1e-3f + c, threadIdx.x * 2e-3f + c);
+        d[c] = pk_make(1e-3f * c, 2e-3f * c);
+        nk[c] = pk_make(-kappa * (c + 1), -kappa * (c + 2));
+    }
+#pragma unroll 1
+    for (int it = 0; it < kIters / NACC; ++it) {
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) {
+#pragma unroll
+            for (int c = 0; c < NPK; ++c) {
+                float xl, xh;
+                asm volatile("mov.b64 {%0, %1}, %2;" : "=f"(xl), "=f"(xh) : "l"(x[c]));
+                acc[i] += xl;
+                acc[i] += xh;
+                d[c] = pk_fma_halves(nk[c], x[c], d[c]);
+                x[c] = pk_add(x[c], d[c]);
+            }
+        }
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) s += acc[i];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+// all-scalar with NACC accumulators and NCH independent pixels
+template <int NCH, int NACC>
+__global__ void k_reinsch_s(float* out, float kappa)
+{
+    float acc[NACC];
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) acc[i] = 0.f;
+    float x[NCH], d[NCH], nk[NCH];
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) { x[c] = threadIdx.x * 1e-3f + c; d[c] = 1e-3f * c; nk[c] = -kappa * (c + 1); }
+#pragma unroll 1
+    for (int it = 0; it < kIters / NACC; ++it) {
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) {
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) {
+                acc[i] += x[c];
+                d[c] = fmaf(nk[c], x[c], d[c]);
+                x[c] += d[c];
+            }
+        }
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) s += acc[i];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+// packed add only, and packed fma with three distinct register-pair operands
+template <int ILP>
+__global__ void k_fadd2(float* out, float a)
+{
+    f32x2_t x[ILP], aa = pk_make(a, a);
+#pragma unroll
+    for (int i = 0; i < ILP; ++i) x[i] = pk_make(threadIdx.x * 1e-3f + i, 1.0f);
+    for (int it = 0; it < kIters; ++it) {
+#pragma unroll
+        for (int i = 0; i < ILP; ++i) x[i] = pk_add(x[i], aa);
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < ILP; ++i) s += pk_sum(x[i]);
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+template <int ILP>
+__global__ void k_ffma2_3op(float* out, float a)
+{
+    f32x2_t x[ILP], y[ILP], z[ILP];
+#pragma unroll
+    for (int i = 0; i < ILP; ++i) { x[i] = pk_make(threadIdx.x * 1e-3f + i, 1.0f); y[i] = pk_make(a + i, a); z[i] = pk_make(a, a * i); }
+    for (int it = 0; it < kIters; ++it) {
+#pragma unroll
+        for (int i = 0; i < ILP; ++i) x[i] = pk_fma(y[i], z[i], x[i]);
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < ILP; ++i) s += pk_sum(x[i]);
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 __global__ void k_mufu(float* out, float a)
 {
     float x0 = threadIdx.x * 1e-3f, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3;
@@ -211,6 +360,40 @@ int main()
         printf("{\"bench\": \"reinsch_4chain_8w\", \"ms\": %.4f, \"per_clk_per_sm_at_max_clock\": %.2f, \"unit\": \"evals\"}\n", ms,
                (double)n_sm * 256 * 4.0 * kIters / (ms * 1e-3) / (n_sm * ghz * 1e9));
     }
+    {   // packed Reinsch pattern at the score kernel's occupancy (16 warps / SM) and at 32 warps / SM
+        for (int w = 16; w <= 32; w += 16) {
+            const int thr = 512, blk = n_sm * (w / 16);
+            const double ln = (double)blk * thr;
+            float ms = time_ms([&] { k_reinsch_packed<1, true><<<blk, thr>>>(out, 1e-3f); });
+            printf("{\"bench\": \"reinsch_mixed_1chain_%dw\", \"ms\": %.4f, \"per_clk_per_sm_at_max_clock\": %.2f, \"unit\": \"evals\"}\n", w, ms,
+                   ln * 2.0 * kIters / (ms * 1e-3) / (n_sm * ghz * 1e9));
+            ms = time_ms([&] { k_reinsch_packed<2, true><<<blk, thr>>>(out, 1e-3f); });
+            printf("{\"bench\": \"reinsch_mixed_2chain_%dw\", \"ms\": %.4f, \"per_clk_per_sm_at_max_clock\": %.2f, \"unit\": \"evals\"}\n", w, ms,
+                   ln * 4.0 * kIters / (ms * 1e-3) / (n_sm * ghz * 1e9));
+            ms = time_ms([&] { k_reinsch_packed<1, false><<<blk, thr>>>(out, 1e-3f); });
+            printf("{\"bench\": \"reinsch_packed_1chain_%dw\", \"ms\": %.4f, \"per_clk_per_sm_at_max_clock\": %.2f, \"unit\": \"evals\"}\n", w, ms,
+                   ln * 2.0 * kIters / (ms * 1e-3) / (n_sm * ghz * 1e9));
+            ms = time_ms([&] { k_reinsch_packed<2, false><<<blk, thr>>>(out, 1e-3f); });
+            printf("{\"bench\": \"reinsch_packed_2chain_%dw\", \"ms\": %.4f, \"per_clk_per_sm_at_max_clock\": %.2f, \"unit\": \"evals\"}\n", w, ms,
+                   ln * 4.0 * kIters / (ms * 1e-3) / (n_sm * ghz * 1e9));
+        }
+    }
+    {
+#define RUN16(name, kern, evals_per_iter)                                                              \
+    { float ms = time_ms([&] { kern<<<n_sm, 512>>>(out, 1e-3f); });                                    \
+      printf("{\"bench\": \"%s_16w\", \"ms\": %.4f, \"per_clk_per_sm_at_max_clock\": %.2f, \"unit\": \"evals\"}\n", name, ms, \
+             (double)n_sm * 512 * (evals_per_iter) * kIters / (ms * 1e-3) / (n_sm * ghz * 1e9)); }
+        RUN16("reinsch_m2_1pk_acc32", (k_reinsch_m2<1, 32>), 2.0)
+        RUN16("reinsch_m2_2pk_acc32", (k_reinsch_m2<2, 32>), 4.0)
+        RUN16("reinsch_m2_1pk_acc64", (k_reinsch_m2<1, 64>), 2.0)
+        RUN16("reinsch_m2_2pk_acc64", (k_reinsch_m2<2, 64>), 4.0)
+        RUN16("reinsch_s_2ch_acc32", (k_reinsch_s<2, 32>), 2.0)
+        RUN16("reinsch_s_2ch_acc64", (k_reinsch_s<2, 64>), 2.0)
+        RUN16("reinsch_s_4ch_acc64", (k_reinsch_s<4, 64>), 4.0)
+        RUN16("reinsch_s_4ch_acc32", (k_reinsch_s<4, 32>), 4.0)
+    }
+    { float ms = time_ms([&] { k_fadd2<8><<<blocks, threads>>>(out, 1e-4f); }); REPORT("fadd2_ilp8", ms, 16.0 * kIters, "FADD lane-ops (packed x2)"); }
+    { float ms = time_ms([&] { k_ffma2_3op<8><<<blocks, threads>>>(out, 1e-4f); }); REPORT("ffma2_3distinct_ilp8", ms, 16.0 * kIters, "FMA lane-ops (packed x2)"); }
     { float ms = time_ms([&] { k_mufu<<<blocks, threads>>>(out, 0.f); }); REPORT("mufu_sincos", ms, 4.0 * kIters, "MUFU lane-ops"); }
     { float ms = time_ms([&] { k_fp64<0><<<blocks, threads>>>((double*)out, 1.0000001, 1e-9); }); REPORT("dfma", ms, 1.0 * kIters, "DFMA lane-ops"); }
     { float ms = time_ms([&] { k_fp64<1><<<blocks, threads>>>((double*)out, 1.5, 0.0); }); REPORT("ddiv_rn", ms, 1.0 * kIters, "DDIV lane-ops"); }

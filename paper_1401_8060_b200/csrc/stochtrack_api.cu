@@ -25,7 +25,7 @@ constexpr uint64_t kMaxSamplesPerLaunch = 1ull << 31;   // keeps per-block u32 h
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t map, e0, bintab, es, kz, w, tau, hist, scalars, result, cand, warp_best, stage_csd, stage_sigma, total;
+    size_t map, e0, bintab, es, kz, ec, cheb, w, tau, hist, scalars, result, cand, warp_best, stage_csd, stage_sigma, total;
 };
 
 Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
@@ -38,6 +38,8 @@ Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
     L.bintab = o;      o += align_up((size_t)n_f * sizeof(float4));
     L.es = o;          o += align_up((size_t)n_f * (size_t)((max_n_tau + st::kSuper - 1) / st::kSuper) * sizeof(float2));
     L.kz = o;          o += align_up((size_t)n_f * sizeof(float2));
+    L.ec = o;          o += align_up((size_t)n_f * sizeof(float2));
+    L.cheb = o;        o += align_up((size_t)n_f * sizeof(float4));
     L.w = o;           o += align_up((size_t)n_f * (size_t)max_n_tau * sizeof(float2));
     L.tau = o;         o += align_up((size_t)max_n_tau * sizeof(double));
     L.hist = o;        o += align_up((size_t)ST_MAX_BINS * sizeof(unsigned long long));
@@ -51,7 +53,7 @@ Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
     return L;
 }
 
-enum TableKind { kNoTable = 0, kWTable = 1, kRotTable = 2, kReinschTable = 3 };
+enum TableKind { kNoTable = 0, kWTable = 1, kRotTable = 2, kReinschTable = 3, kChebTable = 4 };
 
 }  // namespace
 
@@ -131,7 +133,8 @@ int validate(st_ctx* c, const st_search_params* p, bool need_map)
     if (p->norm != ST_NORM_SQRT_N && p->norm != ST_NORM_MEAN) return fail(c, ST_EINVAL, "bad norm %d", p->norm);
     if (p->n_bins < 0 || p->n_bins > ST_MAX_BINS) return fail(c, ST_EINVAL, "n_bins %d outside [0, %d]", p->n_bins, ST_MAX_BINS);
     if (p->n_bins > 0 && !(p->hist_hi > p->hist_lo)) return fail(c, ST_EINVAL, "need hist_hi > hist_lo");
-    if (p->kernel < ST_KERNEL_AUTO || p->kernel > ST_KERNEL_REINSCH) return fail(c, ST_EINVAL, "bad kernel %d", p->kernel);
+    if (p->kernel < ST_KERNEL_AUTO || p->kernel > ST_KERNEL_CHEBYSHEV || p->kernel == ST_KERNEL_RANDOM)
+        return fail(c, ST_EINVAL, "bad kernel %d", p->kernel);
     if (p->reserved != 0) return fail(c, ST_EINVAL, "reserved must be 0");
     if (p->n_tracks > (1ull << 62) || p->track_offset > (1ull << 62)) return fail(c, ST_EINVAL, "n_tracks / track_offset too large");
     return ST_OK;
@@ -161,6 +164,19 @@ bool reinsch_well_conditioned(const st_ctx* c, double dtau)
     return true;
 }
 
+// The plain three-term recurrence carries a float32 coefficient 2 cos(theta): its rounding
+// shifts the phase by <= 32 * 2^-25 / |sin theta| per half chunk.  Require |sin theta_k| >= 0.008
+// for every bin (phase error <= 1.2e-4 rad worst case, ~2e-6 rms over a track).
+bool cheb_well_conditioned(const st_ctx* c, double dtau)
+{
+    for (int k = 0; k < c->n_f; ++k) {
+        double cyc = (c->f_min + (double)k * c->df) * dtau;
+        cyc -= rint(cyc);
+        if (fabs(sin(st::kTwoPi * cyc)) < 0.008) return false;
+    }
+    return true;
+}
+
 int pick_chunk(int n_tau)
 {
     const int pad32 = (n_tau + 31) / 32 * 32, pad64 = (n_tau + 63) / 64 * 64;
@@ -181,13 +197,15 @@ int make_plan(st_ctx* c, const st_search_params* p, Plan* plan)
     int k = p->kernel;
     if (k == ST_KERNEL_AUTO) {
         if (!uni || p->n_tau < 8) k = ST_KERNEL_TABLE;
+        else if (cheb_well_conditioned(c, plan->dtau)) k = ST_KERNEL_CHEBYSHEV;
         else k = reinsch_well_conditioned(c, plan->dtau) ? ST_KERNEL_REINSCH : ST_KERNEL_ROTATION;
     }
-    if ((k == ST_KERNEL_ROTATION || k == ST_KERNEL_REINSCH) && !uni)
+    if ((k == ST_KERNEL_ROTATION || k == ST_KERNEL_REINSCH || k == ST_KERNEL_CHEBYSHEV) && !uni)
         return fail(c, ST_EINVAL, "recurrence kernels need a uniform tau grid");
     plan->kernel = k;
     if (k == ST_KERNEL_ROTATION) plan->ch = pick_chunk(p->n_tau);
     if (k == ST_KERNEL_REINSCH) plan->ch = st::kChunk;
+    if (k == ST_KERNEL_CHEBYSHEV) plan->ch = st::kCheb;
     return ST_OK;
 }
 
@@ -219,6 +237,13 @@ int ensure_tables(st_ctx* c, const st_search_params* p, const Plan& plan, int* n
                 at<float2>(c, c->L.e0), at<float4>(c, c->L.bintab));
             ST_CUDA(c, cudaGetLastError());
             c->table_kind = kRotTable; c->table_ch = plan.ch; ++*n_launches;
+        }
+    } else if (plan.kernel == ST_KERNEL_CHEBYSHEV) {
+        if (c->table_kind != kChebTable) {
+            st::k_build_cheb_tables<<<(c->n_f + 127) / 128, 128, 0, c->stream>>>(
+                plan.tau0, plan.dtau, c->n_f, c->f_min, c->df, at<float2>(c, c->L.ec), at<float4>(c, c->L.cheb));
+            ST_CUDA(c, cudaGetLastError());
+            c->table_kind = kChebTable; c->table_ch = plan.ch; ++*n_launches;
         }
     } else {
         if (c->table_kind != kReinschTable) {
@@ -273,6 +298,22 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
         st::k_score_table<<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+    } else if (plan.kernel == ST_KERNEL_CHEBYSHEV) {
+        int threads = c->recur_threads;
+        size_t smem;
+        for (;; threads -= 32) {
+            smem = hist_bytes(a.n_bins) + (size_t)c->n_f * sizeof(float4) +
+                   (size_t)(threads / 32) * (size_t)stride * (sizeof(float2) + sizeof(uint16_t));
+            if (smem <= (size_t)c->smem_optin || threads == 32) break;
+        }
+        if (smem > (size_t)c->smem_optin)
+            return fail(c, ST_ENOSPC, "n_f %d / n_max %d need more shared memory than one SM has", c->n_f, n_max);
+        int rc = set_smem(c, st::k_score_cheb, smem);
+        if (rc) return rc;
+        uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
+        const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
+        if (blocks > need) blocks = need;
+        st::k_score_cheb<<<(unsigned)blocks, threads, smem, c->stream>>>(a);
     } else if (plan.kernel == ST_KERNEL_REINSCH) {
         int threads = c->recur_threads;
         size_t smem;
@@ -283,14 +324,17 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         }
         if (smem > (size_t)c->smem_optin)
             return fail(c, ST_ENOSPC, "n_f %d / n_max %d need more shared memory than one SM has", c->n_f, n_max);
-        const bool two = c->reinsch_chains == 2;
-        int rc = two ? set_smem(c, st::k_score_reinsch<2>, smem) : set_smem(c, st::k_score_reinsch<1>, smem);
+        const int var = c->reinsch_chains;
+        int rc = var == 0 ? set_smem(c, st::k_score_reinsch<0>, smem) : var == 1 ? set_smem(c, st::k_score_reinsch<1>, smem)
+               : var == 2 ? set_smem(c, st::k_score_reinsch<2>, smem) : set_smem(c, st::k_score_reinsch<3>, smem);
         if (rc) return rc;
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
-        if (two) st::k_score_reinsch<2><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
-        else st::k_score_reinsch<1><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        if (var == 0) st::k_score_reinsch<0><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        else if (var == 1) st::k_score_reinsch<1><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        else if (var == 2) st::k_score_reinsch<2><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        else st::k_score_reinsch<3><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
     } else {
         int threads = c->recur_threads;
         const size_t bt_bytes = (size_t)c->n_f * sizeof(float4);
@@ -336,6 +380,8 @@ st::ScoreArgs base_args(st_ctx* c, const st_search_params* p)
     a.bintab = at<float4>(c, c->L.bintab);
     a.Es = at<float2>(c, c->L.es);
     a.kz = at<float2>(c, c->L.kz);
+    a.Ec = at<float2>(c, c->L.ec);
+    a.cheb = at<float4>(c, c->L.cheb);
     a.sc = at<st::Scalars>(c, c->L.scalars);
     a.cand = at<st::Cand>(c, c->L.cand);
     a.cand_cap = kCandCap;
@@ -380,9 +426,9 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->ev0 = c->ev1 = nullptr; c->h_res = nullptr; c->h_hist = nullptr;
     c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512;
     c->err[0] = 0;
-    c->reinsch_chains = 2;
-    const char* e2 = getenv("ST_REINSCH_CHAINS");
-    if (e2 && atoi(e2) == 1) c->reinsch_chains = 1;
+    c->reinsch_chains = 1;
+    const char* e2 = getenv("ST_REINSCH_VAR");
+    if (e2 && atoi(e2) >= 0 && atoi(e2) <= 3) c->reinsch_chains = atoi(e2);
     const char* e = getenv("ST_RECUR_THREADS");
     if (e) { int t = atoi(e); if (t >= 32 && t <= 512 && t % 32 == 0) c->recur_threads = t; }
     *out = c;

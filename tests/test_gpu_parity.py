@@ -9,7 +9,7 @@ from helpers import config_inputs, snr_close, hist_rule_ok, S0_UNIT
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = {"table": 1, "rotation": 2, "reinsch": 3}
+KERNELS = {"table": 1, "rotation": 2, "reinsch": 3, "chebyshev": 5}
 
 
 @pytest.fixture(scope="module")
@@ -76,7 +76,7 @@ def _score_case(P, orc, cfg, kernel, count, first=0, norm=0, n_tau=None, tau=Non
     return got, ref
 
 
-@pytest.mark.parametrize("kname", ["table", "rotation", "reinsch"])
+@pytest.mark.parametrize("kname", ["table", "rotation", "reinsch", "chebyshev"])
 @pytest.mark.parametrize("cid,count", [(1, 1000), (2, 4000)])
 def test_scores_grid_kernels_vs_oracle(P, orc, kname, cid, count):
     cfg = synth.CONFIGS[cid]
@@ -86,7 +86,7 @@ def test_scores_grid_kernels_vs_oracle(P, orc, kname, cid, count):
     assert worst < 0.5          # float32 leaves an order of magnitude of headroom (DESIGN.md error budget)
 
 
-@pytest.mark.parametrize("kname", ["table", "rotation", "reinsch"])
+@pytest.mark.parametrize("kname", ["table", "rotation", "reinsch", "chebyshev"])
 @pytest.mark.parametrize("n_tau", [1, 7, 33, 50, 128, 200, 600])
 def test_scores_ragged_tau_counts(P, orc, kname, n_tau):
     """Grid sizes that are not multiples of the 32/64-delay chunks, on the config-5 shape
@@ -97,7 +97,7 @@ def test_scores_ragged_tau_counts(P, orc, kname, n_tau):
     assert ok, f"{kname} n_tau {n_tau}: worst error {worst:.3f} x tolerance"
 
 
-@pytest.mark.parametrize("kname", ["table", "reinsch"])
+@pytest.mark.parametrize("kname", ["table", "reinsch", "chebyshev"])
 def test_scores_mean_normalisation(P, orc, kname):
     """alpha = 1: Eq. 8 exactly as printed."""
     cfg = synth.CONFIGS[2]
@@ -189,7 +189,7 @@ def _assert_search_parity(r, ref, cfg, check_hist=True):
             assert ok, why
 
 
-@pytest.mark.parametrize("kname", ["auto", "table", "rotation", "reinsch"])
+@pytest.mark.parametrize("kname", ["auto", "table", "rotation", "reinsch", "chebyshev"])
 def test_search_config1(P, orc, kname):
     cfg = synth.CONFIGS[1]
     r, ref = _search_both(P, orc, cfg, cfg.n_tracks, kernel=KERNELS.get(kname, 0))
@@ -197,14 +197,14 @@ def test_search_config1(P, orc, kname):
     assert r.n_evals == 1000 * 64 * 16
 
 
-@pytest.mark.parametrize("kname", ["auto", "table", "rotation"])
+@pytest.mark.parametrize("kname", ["auto", "table", "rotation", "reinsch"])
 def test_search_config2_full_size(P, orc, kname):
     """Config 2 at its full size (1e5 tracks x 64 delays, injected chirp), every output."""
     cfg = synth.CONFIGS[2]
     r, ref = _search_both(P, orc, cfg, cfg.n_tracks, kernel=KERNELS.get(kname, 0))
     _assert_search_parity(r, ref, cfg)
     if kname == "auto":
-        assert r.kernel_name == "reinsch"
+        assert r.kernel_name == "chebyshev"
     # the argmax template's control points are the oracle's (bit-exact)
     o = orc.track_params(cfg.seed, ref["arg_track"], cfg.n_t, cfg.n_f, cfg.n_min, cfg.n_max)
     for f in ("N", "j0", "a", "y0", "y1", "y2"):
@@ -238,7 +238,7 @@ def test_search_large_configs_subranges(P, orc, cid, m, ranges):
     for first, n in ranges:
         r, ref = _search_both(P, orc, cfg, n, offset=first, m=m, st=st, inputs=inputs)
         _assert_search_parity(r, ref, cfg)
-        assert r.kernel_name == "reinsch"
+        assert r.kernel_name == "chebyshev"
 
 
 def test_chunk_combination_P9(P, orc):
