@@ -846,6 +846,18 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
 // (measured term error <= 3.3e-5 |p| at theta = 0.01, rms 2e-6; DESIGN.md error budget).
 // Per lane 64 float32 accumulators hold the partial sums over its pixels; a transposing
 // shuffle tree folds them across the warp, leaving delays 2l, 2l+1 of the chunk on lane l.
+// (nl, nh) = g * (cl, ch) - (pl, ph): two scalar FFMAs on the halves of register pairs
+__device__ __forceinline__ f32x2_t pk_cheb(float g, f32x2_t cur, f32x2_t prev)
+{
+    f32x2_t r;
+    asm volatile("{\n\t.reg .f32 cl, ch, pl, ph;\n\t"
+                 "mov.b64 {cl, ch}, %2;\n\tmov.b64 {pl, ph}, %3;\n\t"
+                 "neg.f32 pl, pl;\n\tneg.f32 ph, ph;\n\t"
+                 "fma.rn.f32 pl, %1, cl, pl;\n\tfma.rn.f32 ph, %1, ch, ph;\n\t"
+                 "mov.b64 %0, {pl, ph};\n\t}" : "=l"(r) : "f"(g), "l"(cur), "l"(prev));
+    return r;
+}
+
 constexpr int kCheb = 64;         // delays per chunk
 constexpr int kHalf = kCheb / 2;
 
@@ -860,6 +872,7 @@ constexpr int kHalf = kCheb / 2;
         bp = bc; bc = bn_;                                      \
     } while (0)
 
+template <int VAR>
 __global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -920,8 +933,11 @@ __global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
 #pragma unroll 1
         for (int j = 0; j < n_chunks; ++j) {
             float f[kCheb];
+            f32x2_t f2[kHalf];           // VAR 1: f2[i] = (f[32 + i], f[31 - i]) as a register pair
 #pragma unroll
             for (int i = 0; i < kCheb; ++i) f[i] = 0.0f;
+#pragma unroll
+            for (int i = 0; i < kHalf; ++i) f2[i] = 0ull;
             int row = 0;
 #pragma unroll 1
             for (; row + 2 <= n_rows; row += 2) {
@@ -935,11 +951,28 @@ __global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
                 // x_{m_c} = Re v ; x_{m_c - 1} = Re[v e^{-i theta}] = cos(theta) Re v + sin(theta) Im v
                 float fc0 = v0.x, fp0 = fmaf(0.5f * g0, v0.x, t0.y * v0.y);
                 float fc1 = v1.x, fp1 = fmaf(0.5f * g1, v1.x, t1.y * v1.y);
-                float bc0 = fp0, bp0 = fc0, bc1 = fp1, bp1 = fc1;
+                if (VAR == 0) {
+                    float bc0 = fp0, bp0 = fc0, bc1 = fp1, bp1 = fc1;
 #pragma unroll
-                for (int i = 0; i < kHalf; ++i) {
-                    ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g0, fc0, fp0, bc0, bp0);
-                    ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g1, fc1, fp1, bc1, bp1);
+                    for (int i = 0; i < kHalf; ++i) {
+                        ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g0, fc0, fp0, bc0, bp0);
+                        ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g1, fc1, fp1, bc1, bp1);
+                    }
+                } else {
+                    // pairs (forward value, backward value): cur = (x_{mc+i}, x_{mc-1-i}), prev = (x_{mc+i-1}, x_{mc-i})
+                    f32x2_t ca = pk_make(fc0, fp0), pa = pk_make(fp0, fc0);
+                    f32x2_t cb = pk_make(fc1, fp1), pb = pk_make(fp1, fc1);
+#pragma unroll
+                    for (int i = 0; i < kHalf; i += 2) {
+                        f2[i] = pk_add(f2[i], ca);
+                        f2[i] = pk_add(f2[i], cb);
+                        pa = pk_cheb(g0, ca, pa);            // pa now holds step i+1's values
+                        pb = pk_cheb(g1, cb, pb);
+                        f2[i + 1] = pk_add(f2[i + 1], pa);
+                        f2[i + 1] = pk_add(f2[i + 1], pb);
+                        ca = pk_cheb(g0, pa, ca);            // ca holds step i+2's values
+                        cb = pk_cheb(g1, pb, cb);
+                    }
                 }
             }
             if (row < n_rows) {          // odd tail row
@@ -949,9 +982,24 @@ __global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
                 pool_v[e0] = make_float2(fmaf(v0.x, t0.z, -(v0.y * t0.w)), fmaf(v0.x, t0.w, v0.y * t0.z));
                 const float g0 = t0.x;
                 float fc0 = v0.x, fp0 = fmaf(0.5f * g0, v0.x, t0.y * v0.y);
-                float bc0 = fp0, bp0 = fc0;
+                if (VAR == 0) {
+                    float bc0 = fp0, bp0 = fc0;
 #pragma unroll
-                for (int i = 0; i < kHalf; ++i) ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g0, fc0, fp0, bc0, bp0);
+                    for (int i = 0; i < kHalf; ++i) ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g0, fc0, fp0, bc0, bp0);
+                } else {
+                    f32x2_t ca = pk_make(fc0, fp0), pa = pk_make(fp0, fc0);
+#pragma unroll
+                    for (int i = 0; i < kHalf; i += 2) {
+                        f2[i] = pk_add(f2[i], ca);
+                        pa = pk_cheb(g0, ca, pa);
+                        f2[i + 1] = pk_add(f2[i + 1], pa);
+                        ca = pk_cheb(g0, pa, ca);
+                    }
+                }
+            }
+            if (VAR == 1) {
+#pragma unroll
+                for (int i = 0; i < kHalf; ++i) { f[kHalf + i] = pk_lo(f2[i]); f[kHalf - 1 - i] = pk_hi(f2[i]); }
             }
             // ---- fold across the 32 lanes (transposing tree): lane l ends with delays 2l, 2l+1
 #pragma unroll

@@ -74,6 +74,7 @@ struct st_ctx {
     unsigned long long* h_hist;        // pinned, ST_MAX_BINS
     int n_sm, smem_optin;
     int recur_threads;                 // tunable: threads per block of the recurrence kernels
+    int cheb_var;                      // tunable: 0 scalar accumulators, 1 packed (f32x2) accumulators
     int reinsch_chains;                // tunable: packed recurrence chains in flight per lane (1 or 2)
     char err[512];
 };
@@ -308,12 +309,14 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         }
         if (smem > (size_t)c->smem_optin)
             return fail(c, ST_ENOSPC, "n_f %d / n_max %d need more shared memory than one SM has", c->n_f, n_max);
-        int rc = set_smem(c, st::k_score_cheb, smem);
+        const bool pk = c->cheb_var == 1;
+        int rc = pk ? set_smem(c, st::k_score_cheb<1>, smem) : set_smem(c, st::k_score_cheb<0>, smem);
         if (rc) return rc;
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
-        st::k_score_cheb<<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        if (pk) st::k_score_cheb<1><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        else st::k_score_cheb<0><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
     } else if (plan.kernel == ST_KERNEL_REINSCH) {
         int threads = c->recur_threads;
         size_t smem;
@@ -426,6 +429,9 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->ev0 = c->ev1 = nullptr; c->h_res = nullptr; c->h_hist = nullptr;
     c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512;
     c->err[0] = 0;
+    c->cheb_var = 1;
+    const char* e3 = getenv("ST_CHEB_VAR");
+    if (e3 && atoi(e3) == 0) c->cheb_var = 0;
     c->reinsch_chains = 1;
     const char* e2 = getenv("ST_REINSCH_VAR");
     if (e2 && atoi(e2) >= 0 && atoi(e2) <= 3) c->reinsch_chains = atoi(e2);
