@@ -896,12 +896,16 @@ __global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
         const uint64_t id = a.track_offset + q;
         const Track t = make_track(a.bp, id);
         const Raster r = make_raster(t, a.bp.n_f);
-        const int n_rows = (t.N + kWarp - 1) >> 5;     // rows of 32 columns
+        const int n_rows_raw = (t.N + kWarp - 1) >> 5;     // rows of 32 columns
         wr.pixels += (unsigned long long)t.N;
         const float scale = norm_scale(t.N, a.norm);
-        // ---- phase A: rasterise (four columns per lane in flight), gather p, anchor of chunk 0
+        // ---- phase A: rasterise (four columns per lane in flight), gather p, merge runs of
+        // consecutive columns that fall in the same bin (their terms share the phase factor, so
+        // Eq. 8 only needs the sum of their p), compact, rotate to the anchor of chunk 0.
+        int n_merged = 0;                             // warp-uniform count of merged pixels
+        __syncwarp();                                 // the previous template's pool reads are done
 #pragma unroll 1
-        for (int row = 0; row < n_rows; row += 4) {
+        for (int row = 0; row < n_rows_raw; row += 4) {
             int kq[4];
             float2 pv[4], ev[4];
 #pragma unroll
@@ -918,17 +922,41 @@ __global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                if (row + u < n_rows) {
+                if (row + u < n_rows_raw) {             // warp-uniform
                     const int c = (row + u) * kWarp + lane;
-                    float2 v;
-                    v.x = pv[u].x * ev[u].x - pv[u].y * ev[u].y;
-                    v.y = pv[u].x * ev[u].y + pv[u].y * ev[u].x;
-                    if (c >= t.N) { v.x = 0.0f; v.y = 0.0f; }
-                    pool_v[c] = v;
-                    pool_k[c] = (uint16_t)kq[u];
+                    const bool valid = c < t.N;
+                    const int k_left = __shfl_up_sync(kFull, kq[u], 1);
+                    const bool head = valid && (lane == 0 || kq[u] != k_left);
+                    const uint32_t heads = __ballot_sync(kFull, head);
+                    const uint32_t vmask = __ballot_sync(kFull, valid);
+                    // first lane of this lane's run, then an inclusive segmented sum of p along the run
+                    const int run0 = 31 - __clz((int)(heads & (0xFFFFFFFFu >> (31 - lane))));
+                    float sx = valid ? pv[u].x : 0.0f, sy = valid ? pv[u].y : 0.0f;
+#pragma unroll
+                    for (int d = 1; d < kWarp; d <<= 1) {
+                        if (__ballot_sync(kFull, lane - d >= run0) == 0u) break;   // no run is longer than d
+                        const float tx = __shfl_up_sync(kFull, sx, d), ty = __shfl_up_sync(kFull, sy, d);
+                        if (lane - d >= run0) { sx += tx; sy += ty; }
+                    }
+                    // the last lane of a run holds its total: compact those
+                    const uint32_t nxt = lane == 31 ? 0u : ((vmask & ~heads) >> (lane + 1)) & 1u;   // next lane continues the run
+                    const bool tail = valid && !nxt;
+                    const uint32_t tails = __ballot_sync(kFull, tail);
+                    if (tail) {
+                        const int e = n_merged + __popc(tails & ((1u << lane) - 1u));
+                        pool_v[e] = make_float2(sx * ev[u].x - sy * ev[u].y, sx * ev[u].y + sy * ev[u].x);
+                        pool_k[e] = (uint16_t)kq[u];
+                    }
+                    n_merged += __popc(tails);
                 }
             }
         }
+        {   // zero-fill the unused slots of the last row
+            const int e = n_merged + lane;
+            if (e < ((n_merged + kWarp - 1) & ~(kWarp - 1))) { pool_v[e] = make_float2(0.0f, 0.0f); pool_k[e] = 0; }
+        }
+        __syncwarp();
+        const int n_rows = (n_merged + kWarp - 1) >> 5;
         // ---- phase B: chunks of 64 delays
 #pragma unroll 1
         for (int j = 0; j < n_chunks; ++j) {
