@@ -212,7 +212,8 @@ def run_ours(args):
         "e2e": {"value": e2e_evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": {"bound": "alu", "kernel": f"k_score_recur ({r.kernel_name})", "achieved": achieved, "peak": peak,
+        "roofline": {"bound": "alu", "kernel": {"chebyshev": "k_score_cheb", "reinsch": "k_score_reinsch", "rotation": "k_score_recur",
+                                                "table": "k_score_table", "random": "k_score_random"}.get(r.kernel_name, r.kernel_name), "achieved": achieved, "peak": peak,
                      "unit": "TFLOP/s", "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES_PER_LAUNCH,
                      "peak_how": peak_how + "; algorithmic 4 flop per track-pixel evaluation (DESIGN.md)"},
         "result": {"max_snr": combined["max_snr_f64"], "arg_track": combined["arg_track"],
@@ -246,9 +247,9 @@ def cpu_baseline(cfg, csd, sigma, tau, seed, budget_s=15.0):
     from oracle import oracle
     oracle.build()
     p = oracle.prepare_map(csd, sigma)
-    r, dt = oracle_sample(oracle, p, cfg, tau, seed, 256)
-    rate = r["n_evals"] / dt
-    n = int(max(256, min(cfg.n_tracks, budget_s * rate / (r["n_evals"] / 256))))
+    oracle_sample(oracle, p, cfg, tau, seed, 256)                 # thread start-up, table build
+    r, dt = oracle_sample(oracle, p, cfg, tau, seed, 4096)        # pilot
+    n = int(max(256, min(cfg.n_tracks, budget_s * 4096 / dt)))
     r, dt = oracle_sample(oracle, p, cfg, tau, seed, n)
     return {"value": r["n_evals"] / dt, "unit": UNIT, "cores": r["threads_used"], "kind": "oracle",
             "sample": f"first {n} templates of the workload ({r['n_evals']:.3e} evals, {dt:.1f} s), float64, OpenMP"}
@@ -264,8 +265,9 @@ def run_reference(args):
     csd, sigma, tau = oracle_inputs(cfg)
     seed = synth.map_seed(cfg, 0)
     p = oracle.prepare_map(csd, sigma)
-    r, dt = oracle_sample(oracle, p, cfg, tau, seed, 256)
-    per_track = dt / 256
+    oracle_sample(oracle, p, cfg, tau, seed, 256)
+    r, dt = oracle_sample(oracle, p, cfg, tau, seed, 4096)
+    per_track = dt / 4096
     n = int(max(256, min(cfg.n_tracks, args.ref_step_s / per_track)))
     for i in range(args.warmup):
         oracle_sample(oracle, p, cfg, tau, seed, n, first=i * n)
