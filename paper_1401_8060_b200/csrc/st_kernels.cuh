@@ -73,7 +73,8 @@ struct ScoreArgs {
     const float2* Es;         // [n_super][n_f] e^{2 pi i f_k tau_{s R}}: anchors of the Reinsch kernel
     const float2* kz;         // [n_f] (-4 sin^2(theta_k/2), sin theta_k)
     const float2* Ec;         // [n_f] e^{2 pi i f_k tau_{32}}: first anchor of the Chebyshev kernel
-    const float4* cheb;       // [n_f] (2 cos theta, sin theta, cos 64 theta, sin 64 theta)
+    const float4* cheb;       // [n_f] (G = 2 cos(S theta), cos theta, sin theta, cos 64 theta), built on the host
+    const float* cheb_zi;     // [n_f] sin 64 theta
     Scalars* sc;
     Cand* cand;
     uint32_t cand_cap;
@@ -311,28 +312,6 @@ __global__ void k_build_reinsch_tables(double tau0, double dtau, int r_super, in
     sincospi(2.0 * cyc, &zs, &zc);
     sincospi(cyc, &hs, &hc);
     kz[k] = make_float2((float)(-4.0 * hs * hs), (float)zs);
-}
-
-// Tables of k_score_cheb on the uniform grid: Ec[k] = e^{2 pi i f_k (tau0 + 32 dtau)} (anchor of
-// chunk 0 at its centre), cheb[k] = (2 cos theta_k, sin theta_k, cos 64 theta_k, sin 64 theta_k).
-__global__ void k_build_cheb_tables(double tau0, double dtau, int n_f, double f_min, double df,
-                                    float2* __restrict__ Ec, float4* __restrict__ cheb)
-{
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n_f) return;
-    const double f = f_min + (double)k * df;
-    double s, c;
-    const double c0 = f * (tau0 + 32.0 * dtau);
-    sincospi(2.0 * (c0 - rint(c0)), &s, &c);
-    Ec[k] = make_float2((float)c, (float)s);
-    double cyc = f * dtau;
-    cyc -= rint(cyc);
-    double zs, zc, ms, mc;
-    sincospi(2.0 * cyc, &zs, &zc);
-    double c64 = cyc * 64.0;
-    c64 -= rint(c64);
-    sincospi(2.0 * c64, &ms, &mc);
-    cheb[k] = make_float4((float)(2.0 * zc), (float)zs, (float)mc, (float)ms);
 }
 
 // --------------------------------------------------- S1-S4, table, any grid --
@@ -832,20 +811,22 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
 
 // ------------------ S1-S4, uniform tau grid, two-sided Chebyshev recurrence --
 // The production kernel of the grid mode.  Warp per template, lanes over pixels.
-// A pixel's term of Eq. 8 along the uniform delay grid, x_m = Re[p e^{2 pi i f (tau_0 + m dtau)}],
-// obeys the three-term recurrence of cos(psi + m theta):
-//     x_{m+1} = 2 cos(theta) x_m - x_{m-1}          (forward)
-//     x_{m-1} = 2 cos(theta) x_m - x_{m+1}          (backward, same coefficient)
-// i.e. ONE FMA per (pixel, delay); a second instruction accumulates it.  Delays are
-// processed in chunks of 64 around an anchor at the chunk centre m_c = 64 j + 32: the
-// complex anchor v = p e^{2 pi i f tau_{m_c}} gives x_{m_c} = Re v and x_{m_c - 1} =
-// Re[v e^{-i theta}], from which 32 forward and 32 backward steps run as two independent
-// chains; two pixels per lane are in flight (four chains).  The anchor of the next chunk
-// is v e^{i 64 theta} (table from float64), so recurrence error never spans more than 32
-// steps: a float32 coefficient 2 cos(theta) shifts the phase by <= 32 * 2^-25 / sin(theta)
-// (measured term error <= 3.3e-5 |p| at theta = 0.01, rms 2e-6; DESIGN.md error budget).
-// Per lane 64 float32 accumulators hold the partial sums over its pixels; a transposing
-// shuffle tree folds them across the warp, leaving delays 2l, 2l+1 of the chunk on lane l.
+// A pixel's term of Eq. 8 along the uniform delay grid, x_m = Re[p e^{2 pi i f (tau_0 + m dtau)}]
+// = |p| cos(psi + m theta), obeys for any stride S the three-term recurrence
+//     x_{m+S} = 2 cos(S theta) x_m - x_{m-S}        (and the same backwards),
+// i.e. ONE FMA per (pixel, delay); half a packed add accumulates it.  Delays are processed
+// in chunks of 64 around an anchor at the chunk centre m_c = 64 j + 32: the complex anchor
+// v = p e^{2 pi i f tau_{m_c}} gives x_{m_c}, x_{m_c +- 1} (and x_{m_c - 2} for S = 2), from
+// which 32 forward and 32 backward delays run as 2 S independent chains per pixel; two
+// pixels per lane are in flight.  Forward and backward values of the same offset share a
+// register pair, so the accumulation is one add.rn.f32x2 into 32 packed accumulators.  The
+// anchor of the next chunk is v e^{i 64 theta} (table built in float64), so recurrence
+// error never spans more than 32 delays.  The float32 coefficient G = fl(2 cos(S theta))
+// stands for a slightly different angle: the host measures that drift per bin (it builds
+// the table) and picks S = 1 or 2 so that 32 delays of drift stay below 3e-5 rad, else the
+// search falls back to k_score_reinsch / k_score_recur (stochtrack_api.cu).
+// A transposing shuffle tree folds the packed accumulators across the warp: lane l ends
+// with delays m_c + l and m_c - 1 - l.
 // (nl, nh) = g * (cl, ch) - (pl, ph): two scalar FFMAs on the halves of register pairs
 __device__ __forceinline__ f32x2_t pk_cheb(float g, f32x2_t cur, f32x2_t prev)
 {
@@ -861,31 +842,48 @@ __device__ __forceinline__ f32x2_t pk_cheb(float g, f32x2_t cur, f32x2_t prev)
 constexpr int kCheb = 64;         // delays per chunk
 constexpr int kHalf = kCheb / 2;
 
-// one pixel row's two chains advanced by one delay each (forward into f[FI], backward into f[BI])
-#define ST_CHEB_STEP(FI, BI, g, fc, fp, bc, bp)                 \
-    do {                                                        \
-        f[FI] += fc;                                            \
-        f[BI] += bc;                                            \
-        const float fn_ = fmaf(g, fc, -fp);                     \
-        const float bn_ = fmaf(g, bc, -bp);                     \
-        fp = fc; fc = fn_;                                      \
-        bp = bc; bc = bn_;                                      \
-    } while (0)
+// The register pairs of one pixel at the anchor of a chunk.
+//   stride 1: one chain pair   cur = (x_mc, x_mc-1)            prev = (x_mc-1, x_mc)
+//   stride 2: even offsets     cur = (x_mc, x_mc-1)            prev = (x_mc-2, x_mc+1)
+//             odd offsets      cur = (x_mc+1, x_mc-2)          prev = (x_mc-1, x_mc)
+template <int STRIDE>
+struct ChebPixel {
+    f32x2_t ce, pe, co, po;
+    float G;
+    __device__ __forceinline__ void anchor(const float2 v, const float4 t)
+    {
+        // t = (G, cos theta, sin theta, .);  x_{mc+-1} = Re[v e^{+-i theta}] = c Re v -+ s Im v
+        G = t.x;
+        const float w = v.y * t.z;
+        const float xm1 = fmaf(v.x, t.y, w);
+        if (STRIDE == 1) {
+            ce = pk_make(v.x, xm1);
+            pe = pk_make(xm1, v.x);
+        } else {
+            const float xp1 = fmaf(v.x, t.y, -w);
+            const float xm2 = fmaf(t.y + t.y, xm1, -v.x);     // one stride-1 step: x_{mc-2} = 2c x_{mc-1} - x_mc
+            ce = pk_make(v.x, xm1);
+            pe = pk_make(xm2, xp1);
+            co = pk_make(xp1, xm2);
+            po = pk_make(xm1, v.x);
+        }
+    }
+};
 
-template <int VAR>
+template <int STRIDE>
 __global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_warps = blockDim.x >> 5;
-    // shared memory: hist | cheb[n_f] (float4) | v[n_warps][S] (float2) | k[n_warps][S] (u16), S = pool_stride
+    // shared memory: hist | cheb[n_f] float4 | v[n_warps][S] float2 | z64i[n_f (padded)] float | k[n_warps][S] u16
     float4* sm_tab = reinterpret_cast<float4*>(sm_hist + hist_smem_words(a.n_bins));
     const int S = a.pool_stride;
     float2* pool_v = reinterpret_cast<float2*>(sm_tab + a.bp.n_f) + (size_t)warp * S;
-    uint16_t* pool_k = reinterpret_cast<uint16_t*>(reinterpret_cast<float2*>(sm_tab + a.bp.n_f) + (size_t)n_warps * S)
-                       + (size_t)warp * S;
-    for (int k = threadIdx.x; k < a.bp.n_f; k += blockDim.x) sm_tab[k] = a.cheb[k];
+    float* sm_zi = reinterpret_cast<float*>(reinterpret_cast<float2*>(sm_tab + a.bp.n_f) + (size_t)n_warps * S);
+    uint16_t* pool_k = reinterpret_cast<uint16_t*>(sm_zi + ((a.bp.n_f + 1) & ~1)) + (size_t)warp * S;
+    for (int k = threadIdx.x; k < a.bp.n_f; k += blockDim.x) { sm_tab[k] = a.cheb[k]; sm_zi[k] = a.cheb_zi[k]; }
     hist_init(sm_hist, a.n_bins);
     const int n_chunks = (a.n_tau + kCheb - 1) / kCheb;
     WarpReduce wr;
@@ -957,13 +955,10 @@ __global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
         }
         __syncwarp();
         const int n_rows = (n_merged + kWarp - 1) >> 5;
-        // ---- phase B: chunks of 64 delays
+        // ---- phase B: chunks of 64 delays; f2[i] = (sum x_{mc+i}, sum x_{mc-1-i}) over this lane's pixels
 #pragma unroll 1
         for (int j = 0; j < n_chunks; ++j) {
-            float f[kCheb];
-            f32x2_t f2[kHalf];           // VAR 1: f2[i] = (f[32 + i], f[31 - i]) as a register pair
-#pragma unroll
-            for (int i = 0; i < kCheb; ++i) f[i] = 0.0f;
+            f32x2_t f2[kHalf];
 #pragma unroll
             for (int i = 0; i < kHalf; ++i) f2[i] = 0ull;
             int row = 0;
@@ -971,89 +966,100 @@ __global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
             for (; row + 2 <= n_rows; row += 2) {
                 const int e0 = row * kWarp + lane, e1 = e0 + kWarp;
                 const float2 v0 = pool_v[e0], v1 = pool_v[e1];
-                const float4 t0 = sm_tab[pool_k[e0]], t1 = sm_tab[pool_k[e1]];
-                // next chunk's anchors: v e^{i 64 theta}
-                pool_v[e0] = make_float2(fmaf(v0.x, t0.z, -(v0.y * t0.w)), fmaf(v0.x, t0.w, v0.y * t0.z));
-                pool_v[e1] = make_float2(fmaf(v1.x, t1.z, -(v1.y * t1.w)), fmaf(v1.x, t1.w, v1.y * t1.z));
-                const float g0 = t0.x, g1 = t1.x;
-                // x_{m_c} = Re v ; x_{m_c - 1} = Re[v e^{-i theta}] = cos(theta) Re v + sin(theta) Im v
-                float fc0 = v0.x, fp0 = fmaf(0.5f * g0, v0.x, t0.y * v0.y);
-                float fc1 = v1.x, fp1 = fmaf(0.5f * g1, v1.x, t1.y * v1.y);
-                if (VAR == 0) {
-                    float bc0 = fp0, bp0 = fc0, bc1 = fp1, bp1 = fc1;
-#pragma unroll
-                    for (int i = 0; i < kHalf; ++i) {
-                        ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g0, fc0, fp0, bc0, bp0);
-                        ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g1, fc1, fp1, bc1, bp1);
-                    }
-                } else {
-                    // pairs (forward value, backward value): cur = (x_{mc+i}, x_{mc-1-i}), prev = (x_{mc+i-1}, x_{mc-i})
-                    f32x2_t ca = pk_make(fc0, fp0), pa = pk_make(fp0, fc0);
-                    f32x2_t cb = pk_make(fc1, fp1), pb = pk_make(fp1, fc1);
+                const int k0 = pool_k[e0], k1 = pool_k[e1];
+                const float4 t0 = sm_tab[k0], t1 = sm_tab[k1];
+                const float zi0 = sm_zi[k0], zi1 = sm_zi[k1];
+                // next chunk's anchors: v e^{i 64 theta}   (t.w = cos 64 theta, zi = sin 64 theta)
+                pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
+                pool_v[e1] = make_float2(fmaf(v1.x, t1.w, -(v1.y * zi1)), fmaf(v1.x, zi1, v1.y * t1.w));
+                ChebPixel<STRIDE> A, B;
+                A.anchor(v0, t0);
+                B.anchor(v1, t1);
+                if (STRIDE == 1) {
 #pragma unroll
                     for (int i = 0; i < kHalf; i += 2) {
-                        f2[i] = pk_add(f2[i], ca);
-                        f2[i] = pk_add(f2[i], cb);
-                        pa = pk_cheb(g0, ca, pa);            // pa now holds step i+1's values
-                        pb = pk_cheb(g1, cb, pb);
-                        f2[i + 1] = pk_add(f2[i + 1], pa);
-                        f2[i + 1] = pk_add(f2[i + 1], pb);
-                        ca = pk_cheb(g0, pa, ca);            // ca holds step i+2's values
-                        cb = pk_cheb(g1, pb, cb);
+                        f2[i] = pk_add(f2[i], A.ce);
+                        f2[i] = pk_add(f2[i], B.ce);
+                        A.pe = pk_cheb(A.G, A.ce, A.pe);            // pe now holds offset i + 1
+                        B.pe = pk_cheb(B.G, B.ce, B.pe);
+                        f2[i + 1] = pk_add(f2[i + 1], A.pe);
+                        f2[i + 1] = pk_add(f2[i + 1], B.pe);
+                        A.ce = pk_cheb(A.G, A.pe, A.ce);            // ce holds offset i + 2
+                        B.ce = pk_cheb(B.G, B.pe, B.ce);
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < kHalf; i += 4) {
+                        f2[i] = pk_add(f2[i], A.ce);
+                        f2[i] = pk_add(f2[i], B.ce);
+                        f2[i + 1] = pk_add(f2[i + 1], A.co);
+                        f2[i + 1] = pk_add(f2[i + 1], B.co);
+                        A.pe = pk_cheb(A.G, A.ce, A.pe);            // offset i + 2
+                        B.pe = pk_cheb(B.G, B.ce, B.pe);
+                        A.po = pk_cheb(A.G, A.co, A.po);            // offset i + 3
+                        B.po = pk_cheb(B.G, B.co, B.po);
+                        f2[i + 2] = pk_add(f2[i + 2], A.pe);
+                        f2[i + 2] = pk_add(f2[i + 2], B.pe);
+                        f2[i + 3] = pk_add(f2[i + 3], A.po);
+                        f2[i + 3] = pk_add(f2[i + 3], B.po);
+                        A.ce = pk_cheb(A.G, A.pe, A.ce);            // offset i + 4
+                        B.ce = pk_cheb(B.G, B.pe, B.ce);
+                        A.co = pk_cheb(A.G, A.po, A.co);            // offset i + 5
+                        B.co = pk_cheb(B.G, B.po, B.co);
                     }
                 }
             }
             if (row < n_rows) {          // odd tail row
                 const int e0 = row * kWarp + lane;
                 const float2 v0 = pool_v[e0];
-                const float4 t0 = sm_tab[pool_k[e0]];
-                pool_v[e0] = make_float2(fmaf(v0.x, t0.z, -(v0.y * t0.w)), fmaf(v0.x, t0.w, v0.y * t0.z));
-                const float g0 = t0.x;
-                float fc0 = v0.x, fp0 = fmaf(0.5f * g0, v0.x, t0.y * v0.y);
-                if (VAR == 0) {
-                    float bc0 = fp0, bp0 = fc0;
-#pragma unroll
-                    for (int i = 0; i < kHalf; ++i) ST_CHEB_STEP(kHalf + i, kHalf - 1 - i, g0, fc0, fp0, bc0, bp0);
-                } else {
-                    f32x2_t ca = pk_make(fc0, fp0), pa = pk_make(fp0, fc0);
+                const int k0 = pool_k[e0];
+                const float4 t0 = sm_tab[k0];
+                const float zi0 = sm_zi[k0];
+                pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
+                ChebPixel<STRIDE> A;
+                A.anchor(v0, t0);
+                if (STRIDE == 1) {
 #pragma unroll
                     for (int i = 0; i < kHalf; i += 2) {
-                        f2[i] = pk_add(f2[i], ca);
-                        pa = pk_cheb(g0, ca, pa);
-                        f2[i + 1] = pk_add(f2[i + 1], pa);
-                        ca = pk_cheb(g0, pa, ca);
+                        f2[i] = pk_add(f2[i], A.ce);
+                        A.pe = pk_cheb(A.G, A.ce, A.pe);
+                        f2[i + 1] = pk_add(f2[i + 1], A.pe);
+                        A.ce = pk_cheb(A.G, A.pe, A.ce);
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < kHalf; i += 4) {
+                        f2[i] = pk_add(f2[i], A.ce);
+                        f2[i + 1] = pk_add(f2[i + 1], A.co);
+                        A.pe = pk_cheb(A.G, A.ce, A.pe);
+                        A.po = pk_cheb(A.G, A.co, A.po);
+                        f2[i + 2] = pk_add(f2[i + 2], A.pe);
+                        f2[i + 3] = pk_add(f2[i + 3], A.po);
+                        A.ce = pk_cheb(A.G, A.pe, A.ce);
+                        A.co = pk_cheb(A.G, A.po, A.co);
                     }
                 }
             }
-            if (VAR == 1) {
+            // ---- fold across the 32 lanes (transposing tree on register pairs): lane l keeps pair l
 #pragma unroll
-                for (int i = 0; i < kHalf; ++i) { f[kHalf + i] = pk_lo(f2[i]); f[kHalf - 1 - i] = pk_hi(f2[i]); }
-            }
-            // ---- fold across the 32 lanes (transposing tree): lane l ends with delays 2l, 2l+1
-#pragma unroll
-            for (int off = 16, n = kCheb / 2; off >= 1; off >>= 1, n >>= 1) {
+            for (int off = 16, n = kHalf / 2; off >= 1; off >>= 1, n >>= 1) {
                 const bool upper = (lane & off) != 0;
 #pragma unroll
                 for (int i = 0; i < n; ++i) {
-                    const float send = upper ? f[i] : f[i + n];
-                    const float keep = upper ? f[i + n] : f[i];
-                    f[i] = keep + __shfl_xor_sync(kFull, send, off);
+                    const f32x2_t send = upper ? f2[i] : f2[i + n];
+                    const f32x2_t keep = upper ? f2[i + n] : f2[i];
+                    f2[i] = pk_add(keep, __shfl_xor_sync(kFull, send, off));
                 }
             }
-            float v[2]; uint32_t ms[2]; bool ok[2];
-#pragma unroll
-            for (int i = 0; i < 2; ++i) {
-                ms[i] = (uint32_t)(j * kCheb + 2 * lane + i);
-                ok[i] = (int)ms[i] < a.n_tau;
-                v[i] = f[i] * scale;
-            }
+            const float v[2] = {pk_lo(f2[0]) * scale, pk_hi(f2[0]) * scale};
+            const uint32_t ms[2] = {(uint32_t)(j * kCheb + kHalf + lane), (uint32_t)(j * kCheb + kHalf - 1 - lane)};
+            const bool ok[2] = {(int)ms[0] < a.n_tau, (int)ms[1] < a.n_tau};
             reduce_samples<2>(a, wr, sm_hist, id, q, v, ms, ok);
         }
     }
     reduce_finish(a, wr);
     hist_flush(sm_hist, a.hist, a.n_bins);
 }
-#undef ST_CHEB_STEP
 
 // ----------------------------------------------------------------------- S4 --
 // Float64 score of one (template, delay): Eq. 8 with cos/sin of 2 pi f tau in

@@ -25,7 +25,7 @@ constexpr uint64_t kMaxSamplesPerLaunch = 1ull << 31;   // keeps per-block u32 h
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t map, e0, bintab, es, kz, ec, cheb, w, tau, hist, scalars, result, cand, warp_best, stage_csd, stage_sigma, total;
+    size_t map, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, warp_best, stage_csd, stage_sigma, total;
 };
 
 Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
@@ -40,6 +40,7 @@ Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
     L.kz = o;          o += align_up((size_t)n_f * sizeof(float2));
     L.ec = o;          o += align_up((size_t)n_f * sizeof(float2));
     L.cheb = o;        o += align_up((size_t)n_f * sizeof(float4));
+    L.cheb_zi = o;     o += align_up((size_t)n_f * sizeof(float));
     L.w = o;           o += align_up((size_t)n_f * (size_t)max_n_tau * sizeof(float2));
     L.tau = o;         o += align_up((size_t)max_n_tau * sizeof(double));
     L.hist = o;        o += align_up((size_t)ST_MAX_BINS * sizeof(unsigned long long));
@@ -74,7 +75,9 @@ struct st_ctx {
     unsigned long long* h_hist;        // pinned, ST_MAX_BINS
     int n_sm, smem_optin;
     int recur_threads;                 // tunable: threads per block of the recurrence kernels
-    int cheb_var;                      // tunable: 0 scalar accumulators, 1 packed (f32x2) accumulators
+    int cheb_stride;                   // stride of the tables currently on the device
+    bool pick_valid; double pick_dtau; int pick_stride;   // memo of cheb_pick_stride
+    std::vector<float> h_cheb;         // host-built Chebyshev tables: [n_f] float4, [n_f] float2 Ec, [n_f] float zi
     int reinsch_chains;                // tunable: packed recurrence chains in flight per lane (1 or 2)
     char err[512];
 };
@@ -165,17 +168,60 @@ bool reinsch_well_conditioned(const st_ctx* c, double dtau)
     return true;
 }
 
-// The plain three-term recurrence carries a float32 coefficient 2 cos(theta): its rounding
-// shifts the phase by <= 32 * 2^-25 / |sin theta| per half chunk.  Require |sin theta_k| >= 0.008
-// for every bin (phase error <= 1.2e-4 rad worst case, ~2e-6 rms over a track).
-bool cheb_well_conditioned(const st_ctx* c, double dtau)
+// Chebyshev tables for stride S (built on the host so that the conditioning test sees the very
+// float32 coefficients the kernel uses).  The coefficient G = fl32(2 cos(S theta)) is the exact
+// coefficient of a slightly different angle; over the 32 delays between an anchor and the edge of
+// its chunk the phase drifts by (32 / S) |acos(G/2) - S theta|.  Returns the worst drift over bins.
+double build_cheb_tables(const st_ctx* c, double tau0, double dtau, int stride, std::vector<float>* out)
 {
+    const int n_f = c->n_f;
+    if (out) out->assign((size_t)n_f * 7, 0.0f);
+    double worst = 0.0;
+    for (int k = 0; k < n_f; ++k) {
+        const double f = c->f_min + (double)k * c->df;
+        double cyc = f * dtau;
+        cyc -= rint(cyc);                                   // theta / 2 pi in [-1/2, 1/2]
+        const double theta = st::kTwoPi * cyc;
+        double sth = (double)stride * theta;                // S theta reduced to (-pi, pi]
+        sth -= st::kTwoPi * rint(sth / st::kTwoPi);
+        const float G = (float)(2.0 * cos(sth));
+        double half = 0.5 * (double)G;
+        half = half > 1.0 ? 1.0 : (half < -1.0 ? -1.0 : half);
+        const double drift = (32.0 / (double)stride) * fabs(acos(half) - fabs(sth));
+        if (drift > worst) worst = drift;
+        if (out) {
+            double c64 = cyc * 64.0;
+            c64 -= rint(c64);
+            double c0 = f * (tau0 + 32.0 * dtau);
+            c0 -= rint(c0);
+            float* t4 = out->data() + (size_t)k * 4;
+            t4[0] = G; t4[1] = (float)cos(theta); t4[2] = (float)sin(theta); t4[3] = (float)cos(st::kTwoPi * c64);
+            float* ec = out->data() + (size_t)n_f * 4 + (size_t)k * 2;
+            ec[0] = (float)cos(st::kTwoPi * c0); ec[1] = (float)sin(st::kTwoPi * c0);
+            (*out)[(size_t)n_f * 6 + (size_t)k] = (float)sin(st::kTwoPi * c64);
+        }
+    }
+    return worst;
+}
+
+constexpr double kChebMaxDrift = 3e-5;   // rad: worst-case relative error of a coherent signal's SNR
+
+// Stride 2 needs 2 theta inside (0, pi) for every bin; pick the stride with the smaller drift.
+int cheb_pick_stride(st_ctx* c, double dtau)
+{
+    if (c->pick_valid && c->pick_dtau == dtau) return c->pick_stride;
+    double max_abs_cyc = 0.0;
     for (int k = 0; k < c->n_f; ++k) {
         double cyc = (c->f_min + (double)k * c->df) * dtau;
         cyc -= rint(cyc);
-        if (fabs(sin(st::kTwoPi * cyc)) < 0.008) return false;
+        if (fabs(cyc) > max_abs_cyc) max_abs_cyc = fabs(cyc);
     }
-    return true;
+    const double d1 = build_cheb_tables(c, 0.0, dtau, 1, nullptr);
+    const double d2 = max_abs_cyc < 0.22 ? build_cheb_tables(c, 0.0, dtau, 2, nullptr) : 1e9;
+    const int s = d2 < d1 ? 2 : 1;
+    c->pick_valid = true; c->pick_dtau = dtau;
+    c->pick_stride = (s == 2 ? d2 : d1) <= kChebMaxDrift ? s : 0;
+    return c->pick_stride;
 }
 
 int pick_chunk(int n_tau)
@@ -187,19 +233,25 @@ int pick_chunk(int n_tau)
 struct Plan {
     int kernel;       // ST_KERNEL_*
     int ch;           // recurrence chunk
+    int stride;       // Chebyshev stride (1 or 2)
     double tau0, dtau;
 };
 
 int make_plan(st_ctx* c, const st_search_params* p, Plan* plan)
 {
-    plan->ch = 0; plan->tau0 = 0.0; plan->dtau = 0.0;
+    plan->ch = 0; plan->tau0 = 0.0; plan->dtau = 0.0; plan->stride = 0;
     if (p->tau_mode == ST_TAU_RANDOM) { plan->kernel = ST_KERNEL_RANDOM; return ST_OK; }
     const bool uni = grid_uniform(c, p->tau_grid, p->n_tau, &plan->tau0, &plan->dtau);
     int k = p->kernel;
     if (k == ST_KERNEL_AUTO) {
         if (!uni || p->n_tau < 8) k = ST_KERNEL_TABLE;
-        else if (cheb_well_conditioned(c, plan->dtau)) k = ST_KERNEL_CHEBYSHEV;
+        else if ((plan->stride = cheb_pick_stride(c, plan->dtau)) != 0) k = ST_KERNEL_CHEBYSHEV;
         else k = reinsch_well_conditioned(c, plan->dtau) ? ST_KERNEL_REINSCH : ST_KERNEL_ROTATION;
+    }
+    if (k == ST_KERNEL_CHEBYSHEV && plan->stride == 0) {
+        if (uni) plan->stride = cheb_pick_stride(c, plan->dtau);
+        if (uni && plan->stride == 0)
+            return fail(c, ST_EINVAL, "the Chebyshev kernel is ill conditioned on this delay grid (drift > %.1e rad)", kChebMaxDrift);
     }
     if ((k == ST_KERNEL_ROTATION || k == ST_KERNEL_REINSCH || k == ST_KERNEL_CHEBYSHEV) && !uni)
         return fail(c, ST_EINVAL, "recurrence kernels need a uniform tau grid");
@@ -240,11 +292,13 @@ int ensure_tables(st_ctx* c, const st_search_params* p, const Plan& plan, int* n
             c->table_kind = kRotTable; c->table_ch = plan.ch; ++*n_launches;
         }
     } else if (plan.kernel == ST_KERNEL_CHEBYSHEV) {
-        if (c->table_kind != kChebTable) {
-            st::k_build_cheb_tables<<<(c->n_f + 127) / 128, 128, 0, c->stream>>>(
-                plan.tau0, plan.dtau, c->n_f, c->f_min, c->df, at<float2>(c, c->L.ec), at<float4>(c, c->L.cheb));
-            ST_CUDA(c, cudaGetLastError());
-            c->table_kind = kChebTable; c->table_ch = plan.ch; ++*n_launches;
+        if (c->table_kind != kChebTable || c->cheb_stride != plan.stride) {
+            build_cheb_tables(c, plan.tau0, plan.dtau, plan.stride, &c->h_cheb);
+            const size_t n = (size_t)c->n_f;
+            ST_CUDA(c, cudaMemcpyAsync(at<void>(c, c->L.cheb), c->h_cheb.data(), n * 4 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+            ST_CUDA(c, cudaMemcpyAsync(at<void>(c, c->L.ec), c->h_cheb.data() + n * 4, n * 2 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+            ST_CUDA(c, cudaMemcpyAsync(at<void>(c, c->L.cheb_zi), c->h_cheb.data() + n * 6, n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+            c->table_kind = kChebTable; c->table_ch = plan.ch; c->cheb_stride = plan.stride;
         }
     } else {
         if (c->table_kind != kReinschTable) {
@@ -303,20 +357,20 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         int threads = c->recur_threads;
         size_t smem;
         for (;; threads -= 32) {
-            smem = hist_bytes(a.n_bins) + (size_t)c->n_f * sizeof(float4) +
+            smem = hist_bytes(a.n_bins) + (size_t)c->n_f * sizeof(float4) + (size_t)((c->n_f + 1) & ~1) * sizeof(float) +
                    (size_t)(threads / 32) * (size_t)stride * (sizeof(float2) + sizeof(uint16_t));
             if (smem <= (size_t)c->smem_optin || threads == 32) break;
         }
         if (smem > (size_t)c->smem_optin)
             return fail(c, ST_ENOSPC, "n_f %d / n_max %d need more shared memory than one SM has", c->n_f, n_max);
-        const bool pk = c->cheb_var == 1;
-        int rc = pk ? set_smem(c, st::k_score_cheb<1>, smem) : set_smem(c, st::k_score_cheb<0>, smem);
+        const bool pk = plan.stride == 2;
+        int rc = pk ? set_smem(c, st::k_score_cheb<2>, smem) : set_smem(c, st::k_score_cheb<1>, smem);
         if (rc) return rc;
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
-        if (pk) st::k_score_cheb<1><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
-        else st::k_score_cheb<0><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        if (pk) st::k_score_cheb<2><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        else st::k_score_cheb<1><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
     } else if (plan.kernel == ST_KERNEL_REINSCH) {
         int threads = c->recur_threads;
         size_t smem;
@@ -385,6 +439,7 @@ st::ScoreArgs base_args(st_ctx* c, const st_search_params* p)
     a.kz = at<float2>(c, c->L.kz);
     a.Ec = at<float2>(c, c->L.ec);
     a.cheb = at<float4>(c, c->L.cheb);
+    a.cheb_zi = at<float>(c, c->L.cheb_zi);
     a.sc = at<st::Scalars>(c, c->L.scalars);
     a.cand = at<st::Cand>(c, c->L.cand);
     a.cand_cap = kCandCap;
@@ -429,9 +484,7 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->ev0 = c->ev1 = nullptr; c->h_res = nullptr; c->h_hist = nullptr;
     c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512;
     c->err[0] = 0;
-    c->cheb_var = 1;
-    const char* e3 = getenv("ST_CHEB_VAR");
-    if (e3 && atoi(e3) == 0) c->cheb_var = 0;
+    c->cheb_stride = 0; c->pick_valid = false; c->pick_dtau = 0.0; c->pick_stride = 0;
     c->reinsch_chains = 1;
     const char* e2 = getenv("ST_REINSCH_VAR");
     if (e2 && atoi(e2) >= 0 && atoi(e2) <= 3) c->reinsch_chains = atoi(e2);

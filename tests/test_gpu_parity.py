@@ -92,7 +92,13 @@ def test_scores_ragged_tau_counts(P, orc, kname, n_tau):
     """Grid sizes that are not multiples of the 32/64-delay chunks, on the config-5 shape
     with per-pixel sigma (several 32-column rows and a ragged tail per track)."""
     cfg = synth.CONFIGS[5]
-    got, ref = _score_case(P, orc, cfg, KERNELS[kname], 300, first=12345, n_tau=n_tau)
+    try:
+        got, ref = _score_case(P, orc, cfg, KERNELS[kname], 300, first=12345, n_tau=n_tau)
+    except P.StError as e:
+        # coarse grids alias some bins onto theta ~ 0 or pi: the Chebyshev kernel refuses them
+        # (ST_EINVAL) rather than lose accuracy; AUTO must then pick another kernel and still agree
+        assert kname == "chebyshev" and e.code == -1 and n_tau in (7, 33, 50)
+        got, ref = _score_case(P, orc, cfg, 0, 300, first=12345, n_tau=n_tau)
     ok, worst = snr_close(got, ref)
     assert ok, f"{kname} n_tau {n_tau}: worst error {worst:.3f} x tolerance"
 
@@ -138,22 +144,28 @@ def test_scores_random_tau_mode(P, orc):
     assert ok, worst
 
 
-def test_auto_picks_rotation_when_reinsch_ill_conditioned(P, orc):
-    """A grid step with f * dtau = 1/2 for some bin (theta = pi) must not use the three-term form."""
+def test_auto_falls_back_to_rotation_on_ill_conditioned_grids(P, orc):
+    """A grid step that puts a bin's step angle theta within 3e-3 rad of pi: the float32 Chebyshev
+    coefficient would drift the phase by > 3e-5 rad over 32 delays and Reinsch amplifies rounding by
+    1/sin(theta), so AUTO must pick the complex rotation; at theta == pi exactly (coefficient -2, no
+    drift) Chebyshev is fine.  Either way the scores agree with the oracle."""
     cfg = synth.CONFIGS[1]            # 40..103 Hz
-    dtau = 0.5 / 80.0                 # theta = pi at 80 Hz
-    tau = -0.01 + dtau * np.arange(16)
     csd, sigma, _ = config_inputs(orc, cfg)
     st = make_ctx(P, cfg)
     st.set_map(csd, sigma)
-    r = st.search(1000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=1000)
-    assert r.kernel_name == "rotation"
     p = orc.prepare_map(csd, sigma)
-    ref = orc.search(p, cfg.f_min, cfg.df, 1000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, dump_snr=True)
-    assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
-    got = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, 0, 1000, tau_grid=tau)
-    ok, worst = snr_close(got, ref["snr"])
-    assert ok, worst
+    for dtau, want in ((0.5005 / 80.0, "rotation"), (0.5 / 80.0, "chebyshev")):
+        tau = -0.01 + dtau * np.arange(16)
+        r = st.search(1000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=1000)
+        assert r.kernel_name == want
+        ref = orc.search(p, cfg.f_min, cfg.df, 1000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, dump_snr=True)
+        assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+        got = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, 0, 1000, tau_grid=tau)
+        ok, worst = snr_close(got, ref["snr"])
+        assert ok, worst
+    with pytest.raises(P.StError):      # an explicit request for the refused kernel is an error, not a silent downgrade
+        st.search(10, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=-0.01 + (0.5005 / 80.0) * np.arange(16),
+                  kernel=P.KERNEL_CHEBYSHEV)
 
 
 # ------------------------------------------------------------------ S4: whole searches
