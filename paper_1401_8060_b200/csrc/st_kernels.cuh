@@ -338,7 +338,7 @@ __global__ void __launch_bounds__(256) k_score_table(const ScoreArgs a)
         const Track t = make_track(a.bp, id);
         const Raster r = make_raster(t, a.bp.n_f);
         for (int c = lane; c < t.N; c += kWarp) {
-            const int k = raster_bin(r, c);
+            const int k = raster_bin_fast(r, c);
             pool_p[c] = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k]);
             pool_k[c] = (uint16_t)k;
         }
@@ -389,7 +389,7 @@ __global__ void __launch_bounds__(256) k_score_random(const ScoreArgs a)
         float acc = 0.0f;
 #pragma unroll 2
         for (int c = lane; c < t.N; c += kWarp) {
-            const int k = raster_bin(r, c);
+            const int k = raster_bin_fast(r, c);
             const float2 p = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k]);
             const double cyc = (a.f_min + (double)k * a.df) * t.tau;
             float s, co;
@@ -454,7 +454,7 @@ __global__ void __launch_bounds__(512, 1) k_score_recur(const ScoreArgs a)
             float2 v = make_float2(0.0f, 0.0f);
             int k = 0;
             if (c < t.N) {
-                k = raster_bin(r, c);
+                k = raster_bin_fast(r, c);
                 const float2 p = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k]);
                 const float2 e = __ldg(&a.E0[k]);
                 v.x = p.x * e.x - p.y * e.y;
@@ -657,7 +657,7 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
 #pragma unroll
                         for (int u = 0; u < 4; ++u) {
                             const int c = c0 + u * kWarp;
-                            k[u] = raster_bin(r, c < t.N ? c : t.N - 1);
+                            k[u] = raster_bin_fast(r, c < t.N ? c : t.N - 1);
                         }
                         pool_k[pr * kWarp + lane] = (uint32_t)k[0] | ((uint32_t)k[1] << 16);
                         if (pr + 1 < n_prows) pool_k[(pr + 1) * kWarp + lane] = (uint32_t)k[2] | ((uint32_t)k[3] << 16);
@@ -906,10 +906,18 @@ __global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
         for (int row = 0; row < n_rows_raw; row += 4) {
             int kq[4];
             float2 pv[4], ev[4];
+            bool redo[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const int c = (row + u) * kWarp + lane;
-                kq[u] = raster_bin(r, c < t.N ? c : t.N - 1);
+                kq[u] = raster_bin_fast(r, c < t.N ? c : t.N - 1, redo[u]);     // branch-free: the four chains interleave
+            }
+            if (redo[0] | redo[1] | redo[2] | redo[3]) {                       // ~1e-5 of the time: normative sequence
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int c = (row + u) * kWarp + lane;
+                    if (redo[u]) kq[u] = raster_bin(r, c < t.N ? c : t.N - 1);
+                }
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
@@ -1071,7 +1079,7 @@ __device__ __forceinline__ double score_f64(const float2* __restrict__ map, cons
     const Raster r = make_raster(t, bp.n_f);
     double acc = 0.0;
     for (int c = lane; c < t.N; c += kWarp) {
-        const int k = raster_bin(r, c);
+        const int k = raster_bin_fast(r, c);
         const float2 p = map[(size_t)(t.j0 + c) * (size_t)bp.n_f + (size_t)k];
         const double phi = kTwoPi * (f_min + (double)k * df) * tau;
         double s, co;
@@ -1187,7 +1195,7 @@ __global__ void k_debug_rasterise(BankParams bp, uint64_t first, uint64_t count,
         const Track t = make_track(bp, first + q);
         const Raster r = make_raster(t, bp.n_f);
         int32_t* row = k_out + q * (uint64_t)bp.n_t;
-        for (int c = lane; c < bp.n_t; c += kWarp) row[c] = c < t.N ? raster_bin(r, c) : -1;
+        for (int c = lane; c < bp.n_t; c += kWarp) row[c] = c < t.N ? raster_bin_fast(r, c) : -1;
         if (lane == 0) { j0_out[q] = t.j0; N_out[q] = t.N; }
     }
 }
@@ -1196,7 +1204,7 @@ __global__ void k_debug_rasterise_track(Track t, int32_t n_f, int32_t* __restric
 {
     const Raster r = make_raster(t, n_f);
     for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < t.N; c += gridDim.x * blockDim.x)
-        k_out[c] = raster_bin(r, c);
+        k_out[c] = raster_bin_fast(r, c);
 }
 
 }  // namespace st
