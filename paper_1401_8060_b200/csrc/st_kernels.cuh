@@ -387,15 +387,39 @@ __global__ void __launch_bounds__(256) k_score_random(const ScoreArgs a)
         const Track t = make_track(a.bp, id);
         const Raster r = make_raster(t, a.bp.n_f);
         float acc = 0.0f;
-#pragma unroll 2
-        for (int c = lane; c < t.N; c += kWarp) {
-            const int k = raster_bin_fast(r, c);
-            const float2 p = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k]);
-            const double cyc = (a.f_min + (double)k * a.df) * t.tau;
-            float s, co;
-            sincospif(2.0f * (float)(cyc - rint(cyc)), &s, &co);
-            acc = fmaf(co, p.x, acc);
-            acc = fmaf(-s, p.y, acc);
+        // four columns per lane in flight: branch-free bins, then the four L2 gathers together
+#pragma unroll 1
+        for (int c0 = lane; c0 < t.N; c0 += 4 * kWarp) {
+            int kq[4];
+            bool redo[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int c = c0 + u * kWarp;
+                kq[u] = raster_bin_fast(r, c < t.N ? c : t.N - 1, redo[u]);
+            }
+            if (redo[0] | redo[1] | redo[2] | redo[3]) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int c = c0 + u * kWarp;
+                    if (redo[u]) kq[u] = raster_bin(r, c < t.N ? c : t.N - 1);
+                }
+            }
+            float2 pv[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int c = c0 + u * kWarp;
+                pv[u] = __ldg(&a.map[(size_t)(t.j0 + (c < t.N ? c : t.N - 1)) * (size_t)a.bp.n_f + (size_t)kq[u]]);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const double cyc = (a.f_min + (double)kq[u] * a.df) * t.tau;
+                float s, co;
+                sincospif(2.0f * (float)(cyc - rint(cyc)), &s, &co);
+                if (c0 + u * kWarp < t.N) {
+                    acc = fmaf(co, pv[u].x, acc);
+                    acc = fmaf(-s, pv[u].y, acc);
+                }
+            }
         }
 #pragma unroll
         for (int off = 16; off >= 1; off >>= 1) acc += __shfl_xor_sync(kFull, acc, off);
@@ -583,12 +607,14 @@ __device__ __forceinline__ float pk_lo(f32x2_t a)
 {
     float lo, hi;
     asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a));
+    (void)hi;
     return lo;
 }
 __device__ __forceinline__ float pk_hi(f32x2_t a)
 {
     float lo, hi;
     asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a));
+    (void)lo;
     return hi;
 }
 __device__ __forceinline__ float pk_sum(f32x2_t a)
@@ -870,8 +896,11 @@ struct ChebPixel {
     }
 };
 
+#ifndef ST_CHEB_MAX_THREADS
+#define ST_CHEB_MAX_THREADS 512
+#endif
 template <int STRIDE>
-__global__ void __launch_bounds__(512, 1) k_score_cheb(const ScoreArgs a)
+__global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);

@@ -489,7 +489,7 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     const char* e2 = getenv("ST_REINSCH_VAR");
     if (e2 && atoi(e2) >= 0 && atoi(e2) <= 3) c->reinsch_chains = atoi(e2);
     const char* e = getenv("ST_RECUR_THREADS");
-    if (e) { int t = atoi(e); if (t >= 32 && t <= 512 && t % 32 == 0) c->recur_threads = t; }
+    if (e) { int t = atoi(e); if (t >= 32 && t <= 1024 && t % 32 == 0) c->recur_threads = t; }
     *out = c;
     return ST_OK;
 }

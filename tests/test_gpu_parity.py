@@ -359,3 +359,45 @@ def test_host_buffer_entry_point(P, orc):
     st.set_map(torch.from_numpy(csd).cuda(), torch.from_numpy(sigma).cuda())   # device path
     b = st.search(5000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=1000)
     assert a.max_snr == b.max_snr and a.arg_track == b.arg_track and np.array_equal(a.hist, b.hist)
+
+
+# ------------------------------------------------------------------ full sizes, bench launch configuration
+@pytest.mark.parametrize("cid", [4, 5])
+def test_full_size_search_subrange_protocol(P, orc, cid):
+    """Configs 4 (map 0) and 5 at BASELINE.json's full sizes (1e6 x 128 and 1e7 x 512), launched exactly
+    as bench.py launches them.  The oracle cannot finish these, so (SURVEY 8(d) sub-range protocol):
+    (1) properties that hold at any size: histogram total, n_evals, P9 chunk combination of four
+    quarter searches == the full search (bit for bit); (2) the oracle runs the 1500-template sub-range
+    that contains the GPU's global argmax and must agree on it exactly; (3) the oracle re-scores the GPU's
+    argmax sample on its own (Eq. 8 directly)."""
+    cfg = synth.CONFIGS[cid]
+    csd, sigma, tau = config_inputs(orc, cfg, 0)
+    seed = synth.map_seed(cfg, 0)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    kw = dict(tau_grid=tau, n_bins=cfg.n_bins, hist_lo=cfg.hist_lo, hist_hi=cfg.hist_hi)
+    T = cfg.n_tracks
+    full = st.search(T, seed, cfg.n_min, cfg.n_max, **kw)
+    assert full.kernel_name == "chebyshev" and full.flags == 0
+    assert int(full.hist.sum()) == T * cfg.n_tau and full.n_evals == full.n_pixels * cfg.n_tau
+    mean_n = full.n_pixels / T
+    assert abs(mean_n - (cfg.n_min + cfg.n_max) / 2) < 5 * (cfg.n_max - cfg.n_min) / np.sqrt(12 * T)
+    quarters = [st.search(T // 4, seed, cfg.n_min, cfg.n_max, track_offset=i * (T // 4), **kw) for i in range(4)]
+    best = max(quarters, key=lambda r: (r.max_snr_f64, -r.arg_track, -r.arg_tau_index))
+    assert (full.arg_track, full.arg_tau_index, full.max_snr_f64) == (best.arg_track, best.arg_tau_index, best.max_snr_f64)
+    assert np.array_equal(full.hist, sum(r.hist for r in quarters))
+    assert full.n_pixels == sum(r.n_pixels for r in quarters)
+    # (2) oracle on the sub-range holding the argmax
+    p = orc.prepare_map(csd, sigma)
+    first = (full.arg_track // 1500) * 1500
+    ref = orc.search(p, cfg.f_min, cfg.df, 1500, seed, cfg.n_min, cfg.n_max, tau_grid=tau, track_offset=first)
+    assert (ref["arg_track"], ref["arg_tau_index"]) == (full.arg_track, full.arg_tau_index)
+    rel64 = 1e-11 if cfg.sigma == "none" else 2e-7
+    assert abs(full.max_snr_f64 - ref["max_snr"]) <= rel64 * abs(ref["max_snr"])
+    assert abs(full.max_snr - ref["max_snr"]) <= 1e-4 * abs(ref["max_snr"])
+    # (3) the oracle's own Eq. 8 on that one (template, delay)
+    t = orc.track_params(seed, full.arg_track, cfg.n_t, cfg.n_f, cfg.n_min, cfg.n_max)
+    one = orc.score_direct(p, t, orc.rasterise(t, cfg.n_f), cfg.f_min, cfg.df, tau[full.arg_tau_index])
+    assert abs(one - ref["max_snr"]) <= 1e-12 * abs(one)
+    for f in ("N", "j0", "a", "y0", "y1", "y2"):
+        assert full.arg_params[f] == getattr(t, f)
