@@ -84,6 +84,7 @@ struct ScoreArgs {
     float hist_lo, hist_scale;
     float* dump;              // [n_tracks][n_tau] or null
     int32_t pool_stride;      // pixels of pool space per warp (>= n_max, multiple of 32)
+    int32_t n_prod, n_slots;  // warp-specialised kernel: producer warps, pixel pools in the ring
 };
 
 // ------------------------------------------------------------------ helpers --
@@ -369,14 +370,19 @@ __global__ void __launch_bounds__(256) k_score_table(const ScoreArgs a)
 }
 
 // ----------------------------------------- S1-S4, the paper's random-tau mode --
-// One delay per template.  Lanes over columns; the phase
-// 2 pi f_k tau is reduced in float64 (f tau reaches 25 cycles), its sine and
-// cosine taken in float32; partial sums meet in a warp shuffle tree.
+// One delay per template.  Lanes over columns, four columns per lane in flight:
+// branch-free bins, then the four L2 gathers together.  The phase f_k tau (up to 25 cycles) is
+// formed and reduced to [-1/2, 1/2] in float64, its sine and cosine taken by MUFU in float32
+// (abs error 5e-7); partial sums meet in a warp shuffle tree.  Per pixel the XU pipe sees five
+// operations (two float64 seeds of the rasteriser, one F2F, MUFU.SIN, MUFU.COS): everything else
+// (floor, int <-> double, rounding to the nearest cycle) runs on the FP64 pipe through the
+// 1.5 * 2^52 constant, so that the binding unit is the L2 sector gather, not conversions.
 __global__ void __launch_bounds__(256) k_score_random(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
     const int lane = threadIdx.x & 31;
+    const double u_lane = (double)lane + 0.5;
     hist_init(sm_hist, a.n_bins);
     WarpReduce wr;
     reduce_init(wr);
@@ -386,35 +392,36 @@ __global__ void __launch_bounds__(256) k_score_random(const ScoreArgs a)
         const uint64_t id = a.track_offset + q;
         const Track t = make_track(a.bp, id);
         const Raster r = make_raster(t, a.bp.n_f);
+        const double u_last = int_to_double_fast(t.N - 1) + 0.5;
+        const float2* col0 = a.map + (size_t)t.j0 * (size_t)a.bp.n_f;
         float acc = 0.0f;
-        // four columns per lane in flight: branch-free bins, then the four L2 gathers together
+        double ub = u_lane;                               // column centre of this lane in the current group
 #pragma unroll 1
-        for (int c0 = lane; c0 < t.N; c0 += 4 * kWarp) {
-            int kq[4];
+        for (int c0 = lane; c0 < t.N; c0 += 4 * kWarp, ub += 128.0) {
+            int kq[4], cq[4];
             bool redo[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const int c = c0 + u * kWarp;
-                kq[u] = raster_bin_fast(r, c < t.N ? c : t.N - 1, redo[u]);
+                const bool in = c < t.N;
+                cq[u] = in ? c : t.N - 1;                 // clamped: discarded below
+                kq[u] = raster_bin_fast_u(r, in ? ub + 32.0 * u : u_last, redo[u]);
             }
-            if (redo[0] | redo[1] | redo[2] | redo[3]) {
+            if (redo[0] | redo[1] | redo[2] | redo[3]) {  // ~1e-5 of the time: normative sequence
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int c = c0 + u * kWarp;
-                    if (redo[u]) kq[u] = raster_bin(r, c < t.N ? c : t.N - 1);
-                }
+                for (int u = 0; u < 4; ++u)
+                    if (redo[u]) kq[u] = raster_bin(r, cq[u]);
             }
             float2 pv[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int c = c0 + u * kWarp;
-                pv[u] = __ldg(&a.map[(size_t)(t.j0 + (c < t.N ? c : t.N - 1)) * (size_t)a.bp.n_f + (size_t)kq[u]]);
-            }
+            for (int u = 0; u < 4; ++u)
+                pv[u] = __ldg(col0 + (size_t)cq[u] * (size_t)a.bp.n_f + (size_t)kq[u]);
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const double cyc = (a.f_min + (double)kq[u] * a.df) * t.tau;
-                float s, co;
-                sincospif(2.0f * (float)(cyc - rint(cyc)), &s, &co);
+                const double cyc = (a.f_min + int_to_double_fast(kq[u]) * a.df) * t.tau;
+                const double fr = cyc - ((cyc + kRoundMagic) - kRoundMagic);     // cyc - rint(cyc), |cyc| < 2^51
+                const float ph = 6.283185307179586f * (float)fr;
+                const float s = __sinf(ph), co = __cosf(ph);
                 if (c0 + u * kWarp < t.N) {
                     acc = fmaf(co, pv[u].x, acc);
                     acc = fmaf(-s, pv[u].y, acc);
@@ -853,15 +860,21 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
 // search falls back to k_score_reinsch / k_score_recur (stochtrack_api.cu).
 // A transposing shuffle tree folds the packed accumulators across the warp: lane l ends
 // with delays m_c + l and m_c - 1 - l.
-// (nl, nh) = g * (cl, ch) - (pl, ph): two scalar FFMAs on the halves of register pairs
-__device__ __forceinline__ f32x2_t pk_cheb(float g, f32x2_t cur, f32x2_t prev)
+// One recurrence step on a register pair: (g, g) * cur + prev as ONE packed fma.rn.f32x2.  ptxas
+// turns the (g, g) pair into FFMA2's scalar-broadcast operand (R.F32, with a free negation), so the
+// instruction reads one 32-bit and two 64-bit registers and issues at full rate: measured 60.8
+// evaluations/clk/SM for this loop against 37.5 with two scalar FFMAs (profiles/microbench).
+// The recurrence x_{n+1} = G x_n - x_{n-1} has a subtraction FFMA2 cannot express on a pair, so
+// the chains carry w_n = s_n x_n with the sign pattern s = + + - - + + - - ...:
+//     w_{n+1} = (+G) w_n + w_{n-1}  (n even),     w_{n+1} = (-G) w_n + w_{n-1}  (n odd),
+// started from w_0 = x_0, w_{-1} = -x_{-1}; the accumulators collect sum_pixels w_n and the sign
+// s_n (a function of the accumulator index only) is applied once after the fold.  Every product
+// and sum has the magnitude the plain recurrence has: the rounding is identical.
+__device__ __forceinline__ f32x2_t pk_step(float g, f32x2_t cur, f32x2_t prev)
 {
     f32x2_t r;
-    asm volatile("{\n\t.reg .f32 cl, ch, pl, ph;\n\t"
-                 "mov.b64 {cl, ch}, %2;\n\tmov.b64 {pl, ph}, %3;\n\t"
-                 "neg.f32 pl, pl;\n\tneg.f32 ph, ph;\n\t"
-                 "fma.rn.f32 pl, %1, cl, pl;\n\tfma.rn.f32 ph, %1, ch, ph;\n\t"
-                 "mov.b64 %0, {pl, ph};\n\t}" : "=l"(r) : "f"(g), "l"(cur), "l"(prev));
+    asm volatile("{\n\t.reg .b64 gg;\n\tmov.b64 gg, {%1, %1};\n\t"
+                 "fma.rn.f32x2 %0, gg, %2, %3;\n\t}" : "=l"(r) : "f"(g), "l"(cur), "l"(prev));
     return r;
 }
 
@@ -869,9 +882,10 @@ constexpr int kCheb = 64;         // delays per chunk
 constexpr int kHalf = kCheb / 2;
 
 // The register pairs of one pixel at the anchor of a chunk.
-//   stride 1: one chain pair   cur = (x_mc, x_mc-1)            prev = (x_mc-1, x_mc)
-//   stride 2: even offsets     cur = (x_mc, x_mc-1)            prev = (x_mc-2, x_mc+1)
-//             odd offsets      cur = (x_mc+1, x_mc-2)          prev = (x_mc-1, x_mc)
+//   stride 1: one chain pair   cur = (x_mc, x_mc-1)            prev = -(x_mc-1, x_mc)
+//   stride 2: even offsets     cur = (x_mc, x_mc-1)            prev = -(x_mc-2, x_mc+1)
+//             odd offsets      cur = (x_mc+1, x_mc-2)          prev = -(x_mc-1, x_mc)
+// (prev negated: the chains run in the sign pattern of pk_step)
 template <int STRIDE>
 struct ChebPixel {
     f32x2_t ce, pe, co, po;
@@ -884,14 +898,14 @@ struct ChebPixel {
         const float xm1 = fmaf(v.x, t.y, w);
         if (STRIDE == 1) {
             ce = pk_make(v.x, xm1);
-            pe = pk_make(xm1, v.x);
+            pe = pk_make(-xm1, -v.x);                          // w_{-1} = -x_{-1}
         } else {
             const float xp1 = fmaf(v.x, t.y, -w);
             const float xm2 = fmaf(t.y + t.y, xm1, -v.x);     // one stride-1 step: x_{mc-2} = 2c x_{mc-1} - x_mc
             ce = pk_make(v.x, xm1);
-            pe = pk_make(xm2, xp1);
+            pe = pk_make(-xm2, -xp1);
             co = pk_make(xp1, xm2);
-            po = pk_make(xm1, v.x);
+            po = pk_make(-xm1, -v.x);
         }
     }
 };
@@ -899,6 +913,226 @@ struct ChebPixel {
 #ifndef ST_CHEB_MAX_THREADS
 #define ST_CHEB_MAX_THREADS 512
 #endif
+// ---- Phase A of the Chebyshev kernels: rasterise, gather p, merge runs of consecutive columns
+// that fall in the same bin (their terms share the phase factor, so Eq. 8 only needs the sum of
+// their p), compact into the pool, rotate to the anchor of chunk 0.  A lane owns L = ceil(N / 32)
+// CONSECUTIVE columns, so runs are merged by a sequential compare-and-add in registers (runs are
+// cut at lane boundaries: <= 31 extra pixels per template); finished runs are appended to the pool
+// through a ballot.  The work is cut into ELEMENTS of four columns per lane: cheb_fetch issues the
+// four rasteriser chains and the L2 gathers of an element, cheb_merge consumes them, so that a
+// caller can keep the next element in flight while it merges the current one.
+struct ChebFetchCtx {          // what fetching needs to know about a template
+    Raster r;
+    double u_last;             // centre of the last column (clamp target of out-of-range lanes)
+    const float2* col0;        // map row of the template's first column
+    int32_t N, L, cbase;       // columns, columns per lane, first column of this lane
+};
+struct ChebElem { int k[4]; float2 p[4], e[4]; };
+struct ChebMergeState { int run_k, n_merged; float ax, ay; float2 run_e; };
+
+__device__ __forceinline__ void cheb_fetch_ctx(const ScoreArgs& a, const Track& t, const int lane, ChebFetchCtx& f)
+{
+    f.r = make_raster(t, a.bp.n_f);
+    f.N = t.N;
+    f.L = (t.N + kWarp - 1) >> 5;
+    f.cbase = lane * f.L;
+    f.u_last = int_to_double_fast(t.N - 1) + 0.5;
+    f.col0 = a.map + (size_t)t.j0 * (size_t)a.bp.n_f;
+}
+__device__ __forceinline__ void cheb_fetch(const ScoreArgs& a, const ChebFetchCtx& f, const int i, ChebElem& E)
+{
+    bool redo[4];
+    int cc[4];
+    const double ub = int_to_double_fast(f.cbase + i) + 0.5;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int c = f.cbase + i + u;
+        const bool in = c < f.N;
+        cc[u] = in ? c : f.N - 1;                      // clamped: discarded by the merge
+        E.k[u] = raster_bin_fast_u(f.r, in ? ub + (double)u : f.u_last, redo[u]);   // branch-free: the four chains interleave
+    }
+    if (redo[0] | redo[1] | redo[2] | redo[3]) {       // ~1e-5 of the time: normative sequence
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (redo[u]) E.k[u] = raster_bin(f.r, cc[u]);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        E.p[u] = __ldg(f.col0 + (size_t)cc[u] * (size_t)a.bp.n_f + (size_t)E.k[u]);
+        E.e[u] = __ldg(&a.Ec[E.k[u]]);
+    }
+}
+__device__ __forceinline__ void cheb_merge_init(ChebMergeState& m)
+{
+    m.run_k = -1; m.n_merged = 0; m.ax = 0.0f; m.ay = 0.0f; m.run_e = make_float2(0.0f, 0.0f);
+}
+// append the finished runs of the lanes flagged `emit` (a warp-wide ballot keeps the pool compact)
+__device__ __forceinline__ void cheb_emit(ChebMergeState& m, const bool emit, float2* pool_v, uint16_t* pool_k, const int lane)
+{
+    const uint32_t em = __ballot_sync(kFull, emit);
+    if (emit) {
+        const int e = m.n_merged + __popc(em & ((1u << lane) - 1u));
+        pool_v[e] = make_float2(m.ax * m.run_e.x - m.ay * m.run_e.y, m.ax * m.run_e.y + m.ay * m.run_e.x);
+        pool_k[e] = (uint16_t)m.run_k;
+    }
+    m.n_merged += __popc(em);
+}
+__device__ __forceinline__ void cheb_merge(const int N, const int L, const int cbase, const int i, const ChebElem& E,
+                                           ChebMergeState& m, float2* pool_v, uint16_t* pool_k, const int lane)
+{
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const bool valid = (i + u < L) && (cbase + i + u < N);
+        const bool brk = valid && E.k[u] != m.run_k;   // a new run starts at this column
+        cheb_emit(m, brk && m.run_k >= 0, pool_v, pool_k, lane);
+        if (brk) { m.ax = E.p[u].x; m.ay = E.p[u].y; m.run_k = E.k[u]; m.run_e = E.e[u]; }
+        else if (valid) { m.ax += E.p[u].x; m.ay += E.p[u].y; }
+    }
+}
+// the lanes' last runs, then zero-fill up to a multiple of 32 entries; returns the merged count
+__device__ __forceinline__ int cheb_merge_finish(ChebMergeState& m, float2* pool_v, uint16_t* pool_k, const int lane)
+{
+    cheb_emit(m, m.run_k >= 0, pool_v, pool_k, lane);
+    const int e = m.n_merged + lane;
+    if (e < ((m.n_merged + kWarp - 1) & ~(kWarp - 1))) { pool_v[e] = make_float2(0.0f, 0.0f); pool_k[e] = 0; }
+    __syncwarp();
+    return m.n_merged;
+}
+
+// Phase A for one template, start to finish (the next element is in flight while one is merged).
+__device__ __forceinline__ int cheb_phase_a(const ScoreArgs& a, const Track& t, float2* pool_v, uint16_t* pool_k,
+                                            const int lane)
+{
+    ChebFetchCtx f;
+    cheb_fetch_ctx(a, t, lane, f);
+    ChebMergeState m;
+    cheb_merge_init(m);
+    ChebElem E, En;
+    __syncwarp();                                      // the previous template's pool reads are done
+    cheb_fetch(a, f, 0, E);
+#pragma unroll 1
+    for (int i = 0; i < f.L; i += 4) {
+        if (i + 4 < f.L) cheb_fetch(a, f, i + 4, En);  // warp-uniform
+        cheb_merge(f.N, f.L, f.cbase, i, E, m, pool_v, pool_k, lane);
+        E = En;
+    }
+    return cheb_merge_finish(m, pool_v, pool_k, lane);
+}
+
+// Phase B for one template whose merged pixels sit in (pool_v, pool_k): every delay of the grid,
+// fused S4.  pool_v is advanced in place from chunk to chunk.
+template <int STRIDE>
+__device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr, uint32_t* sm_hist,
+                                             const float4* sm_tab, const float* sm_zi, float2* pool_v,
+                                             const uint16_t* pool_k, const int n_merged, const float scale,
+                                             const uint64_t id, const uint64_t q, const int n_chunks, const int lane)
+{
+    const int n_rows = (n_merged + kWarp - 1) >> 5;
+    // ---- phase B: chunks of 64 delays; f2[i] = (sum x_{mc+i}, sum x_{mc-1-i}) over this lane's pixels
+#pragma unroll 1
+    for (int j = 0; j < n_chunks; ++j) {
+        f32x2_t f2[kHalf];
+#pragma unroll
+        for (int i = 0; i < kHalf; ++i) f2[i] = 0ull;
+        int row = 0;
+#pragma unroll 1
+        for (; row + 2 <= n_rows; row += 2) {
+            const int e0 = row * kWarp + lane, e1 = e0 + kWarp;
+            const float2 v0 = pool_v[e0], v1 = pool_v[e1];
+            const int k0 = pool_k[e0], k1 = pool_k[e1];
+            const float4 t0 = sm_tab[k0], t1 = sm_tab[k1];
+            const float zi0 = sm_zi[k0], zi1 = sm_zi[k1];
+            // next chunk's anchors: v e^{i 64 theta}   (t.w = cos 64 theta, zi = sin 64 theta)
+            pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
+            pool_v[e1] = make_float2(fmaf(v1.x, t1.w, -(v1.y * zi1)), fmaf(v1.x, zi1, v1.y * t1.w));
+            ChebPixel<STRIDE> A, B;
+            A.anchor(v0, t0);
+            B.anchor(v1, t1);
+            if (STRIDE == 1) {
+#pragma unroll
+                for (int i = 0; i < kHalf; i += 2) {
+                    f2[i] = pk_add(f2[i], A.ce);
+                    f2[i] = pk_add(f2[i], B.ce);
+                    A.pe = pk_step(A.G, A.ce, A.pe);            // pe now holds offset i + 1
+                    B.pe = pk_step(B.G, B.ce, B.pe);
+                    f2[i + 1] = pk_add(f2[i + 1], A.pe);
+                    f2[i + 1] = pk_add(f2[i + 1], B.pe);
+                    A.ce = pk_step(-A.G, A.pe, A.ce);            // ce holds offset i + 2
+                    B.ce = pk_step(-B.G, B.pe, B.ce);
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < kHalf; i += 4) {
+                    f2[i] = pk_add(f2[i], A.ce);
+                    f2[i] = pk_add(f2[i], B.ce);
+                    f2[i + 1] = pk_add(f2[i + 1], A.co);
+                    f2[i + 1] = pk_add(f2[i + 1], B.co);
+                    A.pe = pk_step(A.G, A.ce, A.pe);            // offset i + 2
+                    B.pe = pk_step(B.G, B.ce, B.pe);
+                    A.po = pk_step(A.G, A.co, A.po);            // offset i + 3
+                    B.po = pk_step(B.G, B.co, B.po);
+                    f2[i + 2] = pk_add(f2[i + 2], A.pe);
+                    f2[i + 2] = pk_add(f2[i + 2], B.pe);
+                    f2[i + 3] = pk_add(f2[i + 3], A.po);
+                    f2[i + 3] = pk_add(f2[i + 3], B.po);
+                    A.ce = pk_step(-A.G, A.pe, A.ce);            // offset i + 4
+                    B.ce = pk_step(-B.G, B.pe, B.ce);
+                    A.co = pk_step(-A.G, A.po, A.co);            // offset i + 5
+                    B.co = pk_step(-B.G, B.po, B.co);
+                }
+            }
+        }
+        if (row < n_rows) {          // odd tail row
+            const int e0 = row * kWarp + lane;
+            const float2 v0 = pool_v[e0];
+            const int k0 = pool_k[e0];
+            const float4 t0 = sm_tab[k0];
+            const float zi0 = sm_zi[k0];
+            pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
+            ChebPixel<STRIDE> A;
+            A.anchor(v0, t0);
+            if (STRIDE == 1) {
+#pragma unroll
+                for (int i = 0; i < kHalf; i += 2) {
+                    f2[i] = pk_add(f2[i], A.ce);
+                    A.pe = pk_step(A.G, A.ce, A.pe);
+                    f2[i + 1] = pk_add(f2[i + 1], A.pe);
+                    A.ce = pk_step(-A.G, A.pe, A.ce);
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < kHalf; i += 4) {
+                    f2[i] = pk_add(f2[i], A.ce);
+                    f2[i + 1] = pk_add(f2[i + 1], A.co);
+                    A.pe = pk_step(A.G, A.ce, A.pe);
+                    A.po = pk_step(A.G, A.co, A.po);
+                    f2[i + 2] = pk_add(f2[i + 2], A.pe);
+                    f2[i + 3] = pk_add(f2[i + 3], A.po);
+                    A.ce = pk_step(-A.G, A.pe, A.ce);
+                    A.co = pk_step(-A.G, A.po, A.co);
+                }
+            }
+        }
+        // ---- fold across the 32 lanes (transposing tree on register pairs): lane l keeps pair l
+#pragma unroll
+        for (int off = 16, n = kHalf / 2; off >= 1; off >>= 1, n >>= 1) {
+            const bool upper = (lane & off) != 0;
+#pragma unroll
+            for (int i = 0; i < n; ++i) {
+                const f32x2_t send = upper ? f2[i] : f2[i + n];
+                const f32x2_t keep = upper ? f2[i + n] : f2[i];
+                f2[i] = pk_add(keep, __shfl_xor_sync(kFull, send, off));
+            }
+        }
+        // sign s_n of the chains: accumulator l holds chain index n = l (stride 1) or l >> 1 (stride 2)
+    const float sscale = ((lane >> STRIDE) & 1) ? -scale : scale;
+    const float v[2] = {pk_lo(f2[0]) * sscale, pk_hi(f2[0]) * sscale};
+        const uint32_t ms[2] = {(uint32_t)(j * kCheb + kHalf + lane), (uint32_t)(j * kCheb + kHalf - 1 - lane)};
+        const bool ok[2] = {(int)ms[0] < a.n_tau, (int)ms[1] < a.n_tau};
+        reduce_samples<2>(a, wr, sm_hist, id, q, v, ms, ok);
+    }
+}
+
 template <int STRIDE>
 __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const ScoreArgs a)
 {
@@ -922,176 +1156,189 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
         if (q >= a.n_tracks) break;
         const uint64_t id = a.track_offset + q;
         const Track t = make_track(a.bp, id);
-        const Raster r = make_raster(t, a.bp.n_f);
-        const int n_rows_raw = (t.N + kWarp - 1) >> 5;     // rows of 32 columns
         wr.pixels += (unsigned long long)t.N;
-        const float scale = norm_scale(t.N, a.norm);
-        // ---- phase A: rasterise (four columns per lane in flight), gather p, merge runs of
-        // consecutive columns that fall in the same bin (their terms share the phase factor, so
-        // Eq. 8 only needs the sum of their p), compact, rotate to the anchor of chunk 0.
-        int n_merged = 0;                             // warp-uniform count of merged pixels
-        __syncwarp();                                 // the previous template's pool reads are done
-#pragma unroll 1
-        for (int row = 0; row < n_rows_raw; row += 4) {
-            int kq[4];
-            float2 pv[4], ev[4];
-            bool redo[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int c = (row + u) * kWarp + lane;
-                kq[u] = raster_bin_fast(r, c < t.N ? c : t.N - 1, redo[u]);     // branch-free: the four chains interleave
-            }
-            if (redo[0] | redo[1] | redo[2] | redo[3]) {                       // ~1e-5 of the time: normative sequence
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int c = (row + u) * kWarp + lane;
-                    if (redo[u]) kq[u] = raster_bin(r, c < t.N ? c : t.N - 1);
+        const int n_merged = cheb_phase_a(a, t, pool_v, pool_k, lane);
+        cheb_phase_b<STRIDE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, n_merged, norm_scale(t.N, a.norm), id, q,
+                             n_chunks, lane);
+    }
+    reduce_finish(a, wr);
+    hist_flush(sm_hist, a.hist, a.n_bins);
+}
+
+// ------- S1-S4, uniform tau grid, Chebyshev recurrence, warp-specialised variant --
+// Same arithmetic as k_score_cheb, but the two phases run in different warps of the persistent
+// block: PRODUCER warps (the first n_prod) generate templates, rasterise, gather and merge
+// (phase A: FP64 chains and L2 latency, almost no FP32 work) into a ring of n_slots pixel pools
+// in shared memory; CONSUMER warps take filled pools in ticket order and run phase B (FP32-pipe
+// bound) plus the fused S4.  A consumer therefore never waits for a rasteriser or an L2 gather:
+// the FP32 pipe stays fed while phase A latency is absorbed by the ring.
+//   slot s % n_slots of ticket s:  gen[slot] == s / n_slots  -> free for the producer of s
+//                                  full[slot] == s + 1        -> filled, for the consumer of s
+// All outputs are order independent (integer histogram adds, max under a total order), so the
+// result does not depend on which warp scores which template.
+struct WsDesc { unsigned long long q; int32_t N; int32_t n_merged; };
+struct WsQueue {
+    uint32_t prod_ticket, cons_ticket, done_producers, pad;
+};
+constexpr int kWsMaxSlots = 64;
+
+// mbarrier (shared::cta) wrappers: a waiting warp sleeps in hardware instead of spinning on a flag
+// (spinning consumers took half of the issue slots away from the producers they were waiting for).
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)      // release.cta
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)   // acquire.cta
+{
+    asm volatile("{\n\t.reg .pred P1;\n\tLAB_WAIT:\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+                 "@P1 bra DONE;\n\tbra LAB_WAIT;\n\tDONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
+// Ring protocol.  Ticket s uses slot s % n_slots in generation g = s / n_slots.
+//   full[slot]  : phase g completes when the producer of ticket s has filled the pool
+//   empty[slot] : phase g completes when the consumer of ticket s has released it
+// The producer of generation g waits for empty phase g - 1 (parity (g + 1) & 1: passes at once for
+// g = 0), the consumer of generation g waits for full phase g (parity g & 1).  The last producer to
+// run out of templates sends one poison ticket (N = -1) per consumer through the same ring.
+// A parity wait cannot tell phase g from phase g - 2: a fast consumer may hold a ticket two
+// generations ahead of a pool that a slow consumer is still scoring, and would sail through.  So
+// each pool also carries plain generation counters (written before the arrive, read after the
+// wait); a waiter that finds the wrong generation goes back to waiting.
+__device__ __forceinline__ void ws_wait(uint64_t* bar, const uint32_t* counter, uint32_t want_gen)
+{
+    for (;;) {
+        mbar_wait(bar, (want_gen + 1u) & 1u);         // phase want_gen - 1 complete
+        if (*(const volatile uint32_t*)counter >= want_gen) return;
+        __nanosleep(200);
+    }
+}
+template <int STRIDE>
+__global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb_ws(const ScoreArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_slots = a.n_slots, n_prod = a.n_prod, n_cons = (blockDim.x >> 5) - a.n_prod;
+    // shared memory: hist | cheb[n_f] float4 | v[n_slots][S] float2 | z64i[n_f (padded)] float | desc[n_slots] |
+    //                queue | full[n_slots] | empty[n_slots] | k[n_slots][S] u16
+    float4* sm_tab = reinterpret_cast<float4*>(sm_hist + hist_smem_words(a.n_bins));
+    const int S = a.pool_stride;
+    float2* slots_v = reinterpret_cast<float2*>(sm_tab + a.bp.n_f);
+    float* sm_zi = reinterpret_cast<float*>(slots_v + (size_t)n_slots * S);
+    WsDesc* desc = reinterpret_cast<WsDesc*>(sm_zi + ((a.bp.n_f + 3) & ~3));
+    WsQueue* wq = reinterpret_cast<WsQueue*>(desc + n_slots);
+    uint64_t* full = reinterpret_cast<uint64_t*>(wq + 1);
+    uint64_t* empty = full + n_slots;
+    uint32_t* filled = reinterpret_cast<uint32_t*>(empty + n_slots);    // generations filled / released so far
+    uint32_t* released = filled + n_slots;
+    uint16_t* slots_k = reinterpret_cast<uint16_t*>(released + n_slots);
+    for (int k = threadIdx.x; k < a.bp.n_f; k += blockDim.x) { sm_tab[k] = a.cheb[k]; sm_zi[k] = a.cheb_zi[k]; }
+    for (int i = threadIdx.x; i < n_slots; i += blockDim.x) {
+        mbar_init(&full[i], 1u); mbar_init(&empty[i], 1u);
+        filled[i] = 0u; released[i] = 0u;
+    }
+    if (threadIdx.x == 0) { wq->prod_ticket = 0u; wq->cons_ticket = 0u; wq->done_producers = 0u; wq->pad = 0u; }
+    hist_init(sm_hist, a.n_bins);   // includes __syncthreads
+    const int n_chunks = (a.n_tau + kCheb - 1) / kCheb;
+    WarpReduce wr;
+    reduce_init(wr);
+    if (warp < n_prod) {
+        // ------------------------------------------------------------- producer
+        // A stream of elements (four columns per lane) runs through the warp: while element e is
+        // merged into its template's pool, element e + 1 -- of the same template or, at a template
+        // boundary, of the next one (generated and ticketed early) -- has its rasteriser chains and
+        // L2 gathers in flight.  The template-counter atomic for the template after that is in
+        // flight too (its result stays in lane 0 until needed).
+        struct Open { uint32_t s, slot, g; unsigned long long q; int32_t N, L, cbase; };
+        unsigned long long q_pref = 0;
+        if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
+        auto take_ticket = [&](Open& o) {
+            uint32_t s = 0;
+            if (lane == 0) s = atomicAdd(&wq->prod_ticket, 1u);
+            s = __shfl_sync(kFull, s, 0);
+            o.s = s; o.slot = s % (uint32_t)n_slots; o.g = s / (uint32_t)n_slots;
+        };
+        auto open = [&](ChebFetchCtx& f, Open& o) -> bool {
+            const unsigned long long q = __shfl_sync(kFull, q_pref, 0);
+            if (q >= a.n_tracks) return false;
+            if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
+            const Track t = make_track(a.bp, a.track_offset + q);
+            cheb_fetch_ctx(a, t, lane, f);
+            take_ticket(o);
+            o.q = q; o.N = f.N; o.L = f.L; o.cbase = f.cbase;
+            return true;
+        };
+        ChebFetchCtx F;
+        Open A, P;
+        ChebElem E, En;
+        ChebMergeState m;
+        bool have = open(F, A);
+        int i_f = 0, i_a = 0;
+        if (have) {
+            cheb_fetch(a, F, 0, E);
+            ws_wait(&empty[A.slot], &released[A.slot], A.g);   // only now: our previous ticket is already published
+            cheb_merge_init(m);
+        }
+        while (have) {
+            // fetch cursor: one element ahead of the merge cursor
+            bool have_next = true, switched = false;
+            i_f += 4;
+            if (i_f >= F.L) { have_next = open(F, P); i_f = 0; switched = true; }
+            if (have_next) cheb_fetch(a, F, i_f, En);
+            float2* pool_v = slots_v + (size_t)A.slot * S;
+            uint16_t* pool_k = slots_k + (size_t)A.slot * S;
+            cheb_merge(A.N, A.L, A.cbase, i_a, E, m, pool_v, pool_k, lane);
+            i_a += 4;
+            if (switched) {                          // that was the template's last element: publish it
+                const int n_merged = cheb_merge_finish(m, pool_v, pool_k, lane);   // ends with __syncwarp
+                if (lane == 0) {
+                    WsDesc d; d.q = A.q; d.N = A.N; d.n_merged = n_merged;
+                    desc[A.slot] = d;
+                    filled[A.slot] = A.g + 1u;
+                    mbar_arrive(&full[A.slot]);
                 }
+                have = have_next;
+                if (have) { A = P; i_a = 0; ws_wait(&empty[A.slot], &released[A.slot], A.g); cheb_merge_init(m); }
             }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                int c = (row + u) * kWarp + lane;
-                c = c < t.N ? c : t.N - 1;              // clamped: discarded below
-                pv[u] = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)kq[u]]);
-                ev[u] = __ldg(&a.Ec[kq[u]]);
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                if (row + u < n_rows_raw) {             // warp-uniform
-                    const int c = (row + u) * kWarp + lane;
-                    const bool valid = c < t.N;
-                    const int k_left = __shfl_up_sync(kFull, kq[u], 1);
-                    const bool head = valid && (lane == 0 || kq[u] != k_left);
-                    const uint32_t heads = __ballot_sync(kFull, head);
-                    const uint32_t vmask = __ballot_sync(kFull, valid);
-                    // first lane of this lane's run, then an inclusive segmented sum of p along the run
-                    const int run0 = 31 - __clz((int)(heads & (0xFFFFFFFFu >> (31 - lane))));
-                    float sx = valid ? pv[u].x : 0.0f, sy = valid ? pv[u].y : 0.0f;
-#pragma unroll
-                    for (int d = 1; d < kWarp; d <<= 1) {
-                        if (__ballot_sync(kFull, lane - d >= run0) == 0u) break;   // no run is longer than d
-                        const float tx = __shfl_up_sync(kFull, sx, d), ty = __shfl_up_sync(kFull, sy, d);
-                        if (lane - d >= run0) { sx += tx; sy += ty; }
-                    }
-                    // the last lane of a run holds its total: compact those
-                    const uint32_t nxt = lane == 31 ? 0u : ((vmask & ~heads) >> (lane + 1)) & 1u;   // next lane continues the run
-                    const bool tail = valid && !nxt;
-                    const uint32_t tails = __ballot_sync(kFull, tail);
-                    if (tail) {
-                        const int e = n_merged + __popc(tails & ((1u << lane) - 1u));
-                        pool_v[e] = make_float2(sx * ev[u].x - sy * ev[u].y, sx * ev[u].y + sy * ev[u].x);
-                        pool_k[e] = (uint16_t)kq[u];
-                    }
-                    n_merged += __popc(tails);
+            E = En;
+        }
+        uint32_t last = 0;
+        if (lane == 0) last = atomicAdd(&wq->done_producers, 1u) == (uint32_t)(n_prod - 1);
+        if (__shfl_sync(kFull, last, 0)) {
+            for (int c = 0; c < n_cons; ++c) {       // one poison ticket per consumer
+                take_ticket(A);
+                ws_wait(&empty[A.slot], &released[A.slot], A.g);
+                if (lane == 0) {
+                    WsDesc d; d.q = 0ull; d.N = -1; d.n_merged = 0;
+                    desc[A.slot] = d;
+                    filled[A.slot] = A.g + 1u;
+                    mbar_arrive(&full[A.slot]);
                 }
             }
         }
-        {   // zero-fill the unused slots of the last row
-            const int e = n_merged + lane;
-            if (e < ((n_merged + kWarp - 1) & ~(kWarp - 1))) { pool_v[e] = make_float2(0.0f, 0.0f); pool_k[e] = 0; }
-        }
-        __syncwarp();
-        const int n_rows = (n_merged + kWarp - 1) >> 5;
-        // ---- phase B: chunks of 64 delays; f2[i] = (sum x_{mc+i}, sum x_{mc-1-i}) over this lane's pixels
-#pragma unroll 1
-        for (int j = 0; j < n_chunks; ++j) {
-            f32x2_t f2[kHalf];
-#pragma unroll
-            for (int i = 0; i < kHalf; ++i) f2[i] = 0ull;
-            int row = 0;
-#pragma unroll 1
-            for (; row + 2 <= n_rows; row += 2) {
-                const int e0 = row * kWarp + lane, e1 = e0 + kWarp;
-                const float2 v0 = pool_v[e0], v1 = pool_v[e1];
-                const int k0 = pool_k[e0], k1 = pool_k[e1];
-                const float4 t0 = sm_tab[k0], t1 = sm_tab[k1];
-                const float zi0 = sm_zi[k0], zi1 = sm_zi[k1];
-                // next chunk's anchors: v e^{i 64 theta}   (t.w = cos 64 theta, zi = sin 64 theta)
-                pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
-                pool_v[e1] = make_float2(fmaf(v1.x, t1.w, -(v1.y * zi1)), fmaf(v1.x, zi1, v1.y * t1.w));
-                ChebPixel<STRIDE> A, B;
-                A.anchor(v0, t0);
-                B.anchor(v1, t1);
-                if (STRIDE == 1) {
-#pragma unroll
-                    for (int i = 0; i < kHalf; i += 2) {
-                        f2[i] = pk_add(f2[i], A.ce);
-                        f2[i] = pk_add(f2[i], B.ce);
-                        A.pe = pk_cheb(A.G, A.ce, A.pe);            // pe now holds offset i + 1
-                        B.pe = pk_cheb(B.G, B.ce, B.pe);
-                        f2[i + 1] = pk_add(f2[i + 1], A.pe);
-                        f2[i + 1] = pk_add(f2[i + 1], B.pe);
-                        A.ce = pk_cheb(A.G, A.pe, A.ce);            // ce holds offset i + 2
-                        B.ce = pk_cheb(B.G, B.pe, B.ce);
-                    }
-                } else {
-#pragma unroll
-                    for (int i = 0; i < kHalf; i += 4) {
-                        f2[i] = pk_add(f2[i], A.ce);
-                        f2[i] = pk_add(f2[i], B.ce);
-                        f2[i + 1] = pk_add(f2[i + 1], A.co);
-                        f2[i + 1] = pk_add(f2[i + 1], B.co);
-                        A.pe = pk_cheb(A.G, A.ce, A.pe);            // offset i + 2
-                        B.pe = pk_cheb(B.G, B.ce, B.pe);
-                        A.po = pk_cheb(A.G, A.co, A.po);            // offset i + 3
-                        B.po = pk_cheb(B.G, B.co, B.po);
-                        f2[i + 2] = pk_add(f2[i + 2], A.pe);
-                        f2[i + 2] = pk_add(f2[i + 2], B.pe);
-                        f2[i + 3] = pk_add(f2[i + 3], A.po);
-                        f2[i + 3] = pk_add(f2[i + 3], B.po);
-                        A.ce = pk_cheb(A.G, A.pe, A.ce);            // offset i + 4
-                        B.ce = pk_cheb(B.G, B.pe, B.ce);
-                        A.co = pk_cheb(A.G, A.po, A.co);            // offset i + 5
-                        B.co = pk_cheb(B.G, B.po, B.co);
-                    }
-                }
-            }
-            if (row < n_rows) {          // odd tail row
-                const int e0 = row * kWarp + lane;
-                const float2 v0 = pool_v[e0];
-                const int k0 = pool_k[e0];
-                const float4 t0 = sm_tab[k0];
-                const float zi0 = sm_zi[k0];
-                pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
-                ChebPixel<STRIDE> A;
-                A.anchor(v0, t0);
-                if (STRIDE == 1) {
-#pragma unroll
-                    for (int i = 0; i < kHalf; i += 2) {
-                        f2[i] = pk_add(f2[i], A.ce);
-                        A.pe = pk_cheb(A.G, A.ce, A.pe);
-                        f2[i + 1] = pk_add(f2[i + 1], A.pe);
-                        A.ce = pk_cheb(A.G, A.pe, A.ce);
-                    }
-                } else {
-#pragma unroll
-                    for (int i = 0; i < kHalf; i += 4) {
-                        f2[i] = pk_add(f2[i], A.ce);
-                        f2[i + 1] = pk_add(f2[i + 1], A.co);
-                        A.pe = pk_cheb(A.G, A.ce, A.pe);
-                        A.po = pk_cheb(A.G, A.co, A.po);
-                        f2[i + 2] = pk_add(f2[i + 2], A.pe);
-                        f2[i + 3] = pk_add(f2[i + 3], A.po);
-                        A.ce = pk_cheb(A.G, A.pe, A.ce);
-                        A.co = pk_cheb(A.G, A.po, A.co);
-                    }
-                }
-            }
-            // ---- fold across the 32 lanes (transposing tree on register pairs): lane l keeps pair l
-#pragma unroll
-            for (int off = 16, n = kHalf / 2; off >= 1; off >>= 1, n >>= 1) {
-                const bool upper = (lane & off) != 0;
-#pragma unroll
-                for (int i = 0; i < n; ++i) {
-                    const f32x2_t send = upper ? f2[i] : f2[i + n];
-                    const f32x2_t keep = upper ? f2[i + n] : f2[i];
-                    f2[i] = pk_add(keep, __shfl_xor_sync(kFull, send, off));
-                }
-            }
-            const float v[2] = {pk_lo(f2[0]) * scale, pk_hi(f2[0]) * scale};
-            const uint32_t ms[2] = {(uint32_t)(j * kCheb + kHalf + lane), (uint32_t)(j * kCheb + kHalf - 1 - lane)};
-            const bool ok[2] = {(int)ms[0] < a.n_tau, (int)ms[1] < a.n_tau};
-            reduce_samples<2>(a, wr, sm_hist, id, q, v, ms, ok);
+    } else {
+        // ------------------------------------------------------------- consumer
+        for (;;) {
+            uint32_t s = 0;
+            if (lane == 0) s = atomicAdd(&wq->cons_ticket, 1u);
+            s = __shfl_sync(kFull, s, 0);
+            const uint32_t slot = s % (uint32_t)n_slots, g = s / (uint32_t)n_slots;
+            ws_wait(&full[slot], &filled[slot], g + 1u);   // full phase g complete <=> filled >= g + 1
+            const WsDesc d = desc[slot];
+            if (d.N < 0) break;                       // poison: the bank is exhausted
+            float2* pool_v = slots_v + (size_t)slot * S;
+            const uint16_t* pool_k = slots_k + (size_t)slot * S;
+            wr.pixels += (unsigned long long)d.N;
+            cheb_phase_b<STRIDE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, d.n_merged, norm_scale(d.N, a.norm),
+                                 a.track_offset + d.q, d.q, n_chunks, lane);
+            __syncwarp();
+            if (lane == 0) { released[slot] = g + 1u; mbar_arrive(&empty[slot]); }
         }
     }
     reduce_finish(a, wr);

@@ -105,6 +105,7 @@ ST_HD Track make_track(const BankParams& bp, uint64_t id)
 // Per-track constants of S2.
 struct Raster {
     double a, cc, aa, y0, y1, y2;
+    double guard;      // fast path: distance from a bin edge below which the normative sequence decides
     int32_t kmax;
 };
 
@@ -116,6 +117,7 @@ ST_HD Raster make_raster(const Track& t, int32_t n_f)
     r.aa = ST_DMUL(t.a, t.a);
     r.y0 = t.y0; r.y1 = t.y1; r.y2 = t.y2;
     r.kmax = n_f - 1;
+    r.guard = 4e-11 * (double)n_f > 1e-6 ? 4e-11 * (double)n_f : 1e-6;
     return r;
 }
 
@@ -145,43 +147,64 @@ ST_HD int32_t raster_bin(const Raster& r, int32_t c)
 }
 
 #if defined(__CUDACC__)
-// S2, fast path (device).  The same bin as raster_bin, at about half the instructions and
-// without branches (so that several columns interleave): y is evaluated to ~1e-8 bins with
-// float32 seeds (one MUFU rsqrt, one MUFU rcp) refined by one float64 Newton step each, instead
-// of correctly rounded sqrt and division.  `redo` is set when y lands within 1e-6 of a bin edge
-// (probability ~2e-6 per pixel) or is not finite; the caller then runs the normative sequence,
-// so the index used is ALWAYS floor of the normative y: bit-exact by construction
-// (|y_fast - y_normative| < 1e-7 << 1e-6: xi is good to ~1e-13 and |dy/dxi| <= 2 n_f <= 1.3e5).
+// S2, fast path (device).  The same bin as raster_bin, at about half the instructions, without
+// branches (so that several columns interleave) and with only two operations on the XU pipe:
+// y is evaluated to ~1e-8 bins with the float64 MUFU seeds rsqrt.approx.f64 / rcp.approx.f64
+// (~20 bits) refined by one float64 Newton step each, instead of correctly rounded sqrt and
+// division; floor and the fractional part come from the 1.5 * 2^52 rounding constant on the FP64
+// pipe (no F2I / I2F / FRND conversions).  `redo` is set when y lands within r.guard of a bin edge
+// (probability ~2e-6 per pixel) or is not finite; the caller then runs the normative sequence, so
+// the index used is ALWAYS floor of the normative y: bit-exact by construction
+// (|y_fast - y_normative| <= 2 n_f * 6e-12: xi is good to ~6e-12 after the Newton steps, and
+// |dy/dxi| <= 2 n_f; guard = max(1e-6, 4e-11 n_f) leaves a factor 3).
+constexpr double kRoundMagic = 6755399441055744.0;   // 1.5 * 2^52: x + M - M rounds x to the nearest integer
+
+__device__ __forceinline__ double raster_y_fast(const Raster& r, double u)
+{
+    const double D  = fma(r.cc, u, r.aa);                       // >= min(a, N - a)^2 > 0
+    double rs, rc;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(rs) : "d"(D));    // ~ 1 / sqrt(D), ~2^-20
+    const double s0 = D * rs;
+    const double s  = fma(fma(-s0, s0, D), 0.5 * rs, s0);       // one Newton step  s <- s + (D - s^2) / (2 s)
+    const double den = r.a + s;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(den));
+    const double q0 = u * rc;
+    const double xi = fma(fma(-den, q0, u), rc, q0);            // one Newton step on the quotient u / den
+    const double om = 1.0 - xi;
+    return fma(om * om, r.y0, fma(2.0 * (om * xi), r.y1, (xi * xi) * r.y2));
+}
+// floor(y) as an int (clamped to [0, kmax]); redo when y is within the guard of an integer or NaN
+__device__ __forceinline__ int32_t floor_guarded(const Raster& r, double y, bool& redo)
+{
+    const double tm = y + kRoundMagic;
+    int32_t k = __double2loint(tm);                             // the low mantissa word holds the integer
+    double yr = tm - kRoundMagic;                               // nearest integer
+    const bool above = yr > y;
+    yr = above ? yr - 1.0 : yr;                                 // floor
+    k  = above ? k - 1 : k;
+    const double fr = y - yr;
+    redo = !(fr > r.guard && fr < 1.0 - r.guard) || !(fabs(y) < 1e9);   // also true for NaN
+    return k < 0 ? 0 : (k > r.kmax ? r.kmax : k);
+}
+// u = column + 1/2 given as a double (callers step it without int -> double conversions)
+__device__ __forceinline__ int32_t raster_bin_fast_u(const Raster& r, double u, bool& redo)
+{
+    return floor_guarded(r, raster_y_fast(r, u), redo);
+}
 __device__ __forceinline__ int32_t raster_bin_fast(const Raster& r, int32_t c, bool& redo)
 {
-    const double u  = (double)c + 0.5;
-    const double D  = fma(r.cc, u, r.aa);                       // >= min(a, N - a)^2 > 0
-    // s = sqrt(D): float32 seed, one Newton step  s <- s + (D - s^2) / (2 s)
-    const float  Df = (float)D;
-    float rs;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rs) : "f"(Df));   // ~ 1 / sqrt(D), 2^-22
-    const double s0 = (double)(Df * rs);
-    const double s  = fma(fma(-s0, s0, D), (double)(0.5f * rs), s0);
-    const double den = r.a + s;
-    // xi = u / den: float32 reciprocal seed, one Newton step on the quotient
-    float rcf;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rcf) : "f"((float)den));
-    const double rc = (double)rcf;
-    const double q0 = u * rc;
-    const double xi = fma(fma(-den, q0, u), rc, q0);
-    const double om = 1.0 - xi;
-    const double y  = fma(om * om, r.y0, fma(2.0 * (om * xi), r.y1, (xi * xi) * r.y2));
-    const double fr = y - floor(y);
-    redo = !(fr > 1e-6 && fr < 1.0 - 1e-6);                     // also true for NaN
-    int32_t k = __double2int_rd(y);                             // saturating; NaN -> 0
-    k = k < 0 ? 0 : (k > r.kmax ? r.kmax : k);
-    return k;
+    return raster_bin_fast_u(r, (double)c + 0.5, redo);
 }
 __device__ __forceinline__ int32_t raster_bin_fast(const Raster& r, int32_t c)
 {
     bool redo;
     const int32_t k = raster_bin_fast(r, c, redo);
     return redo ? raster_bin(r, c) : k;
+}
+// exact (double)k for 0 <= k < 2^31 without the I2F conversion
+__device__ __forceinline__ double int_to_double_fast(int32_t k)
+{
+    return __hiloint2double(0x43380000, k) - kRoundMagic;
 }
 #endif
 
