@@ -84,7 +84,6 @@ struct ScoreArgs {
     float hist_lo, hist_scale;
     float* dump;              // [n_tracks][n_tau] or null
     int32_t pool_stride;      // pixels of pool space per warp (>= n_max, multiple of 32)
-    int32_t n_prod, n_slots;  // warp-specialised kernel: producer warps, pixel pools in the ring
 };
 
 // ------------------------------------------------------------------ helpers --
@@ -114,7 +113,15 @@ __device__ __forceinline__ bool better(float s, uint64_t id, uint32_t m,
 __host__ __device__ __forceinline__ float norm_scale(int32_t N, int32_t norm)
 {
     // N^-alpha: alpha = 1/2 (G1 default) or 1 (Eq. 8 as printed)
+#if defined(__CUDA_ARCH__)
+    // float32 throughout (the score it multiplies is float32): rsqrt seed + one Newton step, <= 1 ulp
+    const float n = (float)N;                  // exact: N <= 2^20
+    if (norm != 0) return __frcp_rn(n);
+    const float y = rsqrtf(n);
+    return y * fmaf(-0.5f * n * y, y, 1.5f);
+#else
     return norm == 0 ? (float)(1.0 / sqrt((double)N)) : (float)(1.0 / (double)N);
+#endif
 }
 
 // Per-warp reduction state (S4).
@@ -985,8 +992,13 @@ __device__ __forceinline__ void cheb_merge(const int N, const int L, const int c
         const bool valid = (i + u < L) && (cbase + i + u < N);
         const bool brk = valid && E.k[u] != m.run_k;   // a new run starts at this column
         cheb_emit(m, brk && m.run_k >= 0, pool_v, pool_k, lane);
-        if (brk) { m.ax = E.p[u].x; m.ay = E.p[u].y; m.run_k = E.k[u]; m.run_e = E.e[u]; }
-        else if (valid) { m.ax += E.p[u].x; m.ay += E.p[u].y; }
+        // branch-free update: a break restarts the sums, a column outside the template adds zero
+        const float px = valid ? E.p[u].x : 0.0f, py = valid ? E.p[u].y : 0.0f;
+        m.ax = brk ? px : m.ax + px;
+        m.ay = brk ? py : m.ay + py;
+        m.run_k = brk ? E.k[u] : m.run_k;
+        m.run_e.x = brk ? E.e[u].x : m.run_e.x;
+        m.run_e.y = brk ? E.e[u].y : m.run_e.y;
     }
 }
 // the lanes' last runs, then zero-fill up to a multiple of 32 entries; returns the merged count
@@ -1007,14 +1019,16 @@ __device__ __forceinline__ int cheb_phase_a(const ScoreArgs& a, const Track& t, 
     cheb_fetch_ctx(a, t, lane, f);
     ChebMergeState m;
     cheb_merge_init(m);
-    ChebElem E, En;
+    ChebElem E0, E1;                                   // ping-pong: no register copies between elements
     __syncwarp();                                      // the previous template's pool reads are done
-    cheb_fetch(a, f, 0, E);
+    cheb_fetch(a, f, 0, E0);
 #pragma unroll 1
-    for (int i = 0; i < f.L; i += 4) {
-        if (i + 4 < f.L) cheb_fetch(a, f, i + 4, En);  // warp-uniform
-        cheb_merge(f.N, f.L, f.cbase, i, E, m, pool_v, pool_k, lane);
-        E = En;
+    for (int i = 0; i < f.L; i += 8) {
+        if (i + 4 < f.L) cheb_fetch(a, f, i + 4, E1);  // warp-uniform
+        cheb_merge(f.N, f.L, f.cbase, i, E0, m, pool_v, pool_k, lane);
+        if (i + 4 >= f.L) break;
+        if (i + 8 < f.L) cheb_fetch(a, f, i + 8, E0);
+        cheb_merge(f.N, f.L, f.cbase, i + 4, E1, m, pool_v, pool_k, lane);
     }
     return cheb_merge_finish(m, pool_v, pool_k, lane);
 }
@@ -1151,195 +1165,20 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
     const int n_chunks = (a.n_tau + kCheb - 1) / kCheb;
     WarpReduce wr;
     reduce_init(wr);
+    // the template counter's L2 atomic (~1 us round trip) is issued one template ahead; its result
+    // stays in lane 0 until the next iteration broadcasts it
+    unsigned long long q_pref = 0;
+    if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
     for (;;) {
-        const uint64_t q = next_track(a);
+        const uint64_t q = __shfl_sync(kFull, q_pref, 0);
         if (q >= a.n_tracks) break;
+        if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
         const uint64_t id = a.track_offset + q;
         const Track t = make_track(a.bp, id);
         wr.pixels += (unsigned long long)t.N;
         const int n_merged = cheb_phase_a(a, t, pool_v, pool_k, lane);
         cheb_phase_b<STRIDE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, n_merged, norm_scale(t.N, a.norm), id, q,
                              n_chunks, lane);
-    }
-    reduce_finish(a, wr);
-    hist_flush(sm_hist, a.hist, a.n_bins);
-}
-
-// ------- S1-S4, uniform tau grid, Chebyshev recurrence, warp-specialised variant --
-// Same arithmetic as k_score_cheb, but the two phases run in different warps of the persistent
-// block: PRODUCER warps (the first n_prod) generate templates, rasterise, gather and merge
-// (phase A: FP64 chains and L2 latency, almost no FP32 work) into a ring of n_slots pixel pools
-// in shared memory; CONSUMER warps take filled pools in ticket order and run phase B (FP32-pipe
-// bound) plus the fused S4.  A consumer therefore never waits for a rasteriser or an L2 gather:
-// the FP32 pipe stays fed while phase A latency is absorbed by the ring.
-//   slot s % n_slots of ticket s:  gen[slot] == s / n_slots  -> free for the producer of s
-//                                  full[slot] == s + 1        -> filled, for the consumer of s
-// All outputs are order independent (integer histogram adds, max under a total order), so the
-// result does not depend on which warp scores which template.
-struct WsDesc { unsigned long long q; int32_t N; int32_t n_merged; };
-struct WsQueue {
-    uint32_t prod_ticket, cons_ticket, done_producers, pad;
-};
-constexpr int kWsMaxSlots = 64;
-
-// mbarrier (shared::cta) wrappers: a waiting warp sleeps in hardware instead of spinning on a flag
-// (spinning consumers took half of the issue slots away from the producers they were waiting for).
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)      // release.cta
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)   // acquire.cta
-{
-    asm volatile("{\n\t.reg .pred P1;\n\tLAB_WAIT:\n\t"
-                 "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
-                 "@P1 bra DONE;\n\tbra LAB_WAIT;\n\tDONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-
-// Ring protocol.  Ticket s uses slot s % n_slots in generation g = s / n_slots.
-//   full[slot]  : phase g completes when the producer of ticket s has filled the pool
-//   empty[slot] : phase g completes when the consumer of ticket s has released it
-// The producer of generation g waits for empty phase g - 1 (parity (g + 1) & 1: passes at once for
-// g = 0), the consumer of generation g waits for full phase g (parity g & 1).  The last producer to
-// run out of templates sends one poison ticket (N = -1) per consumer through the same ring.
-// A parity wait cannot tell phase g from phase g - 2: a fast consumer may hold a ticket two
-// generations ahead of a pool that a slow consumer is still scoring, and would sail through.  So
-// each pool also carries plain generation counters (written before the arrive, read after the
-// wait); a waiter that finds the wrong generation goes back to waiting.
-__device__ __forceinline__ void ws_wait(uint64_t* bar, const uint32_t* counter, uint32_t want_gen)
-{
-    for (;;) {
-        mbar_wait(bar, (want_gen + 1u) & 1u);         // phase want_gen - 1 complete
-        if (*(const volatile uint32_t*)counter >= want_gen) return;
-        __nanosleep(200);
-    }
-}
-template <int STRIDE>
-__global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb_ws(const ScoreArgs a)
-{
-    extern __shared__ __align__(16) unsigned char smem[];
-    uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n_slots = a.n_slots, n_prod = a.n_prod, n_cons = (blockDim.x >> 5) - a.n_prod;
-    // shared memory: hist | cheb[n_f] float4 | v[n_slots][S] float2 | z64i[n_f (padded)] float | desc[n_slots] |
-    //                queue | full[n_slots] | empty[n_slots] | k[n_slots][S] u16
-    float4* sm_tab = reinterpret_cast<float4*>(sm_hist + hist_smem_words(a.n_bins));
-    const int S = a.pool_stride;
-    float2* slots_v = reinterpret_cast<float2*>(sm_tab + a.bp.n_f);
-    float* sm_zi = reinterpret_cast<float*>(slots_v + (size_t)n_slots * S);
-    WsDesc* desc = reinterpret_cast<WsDesc*>(sm_zi + ((a.bp.n_f + 3) & ~3));
-    WsQueue* wq = reinterpret_cast<WsQueue*>(desc + n_slots);
-    uint64_t* full = reinterpret_cast<uint64_t*>(wq + 1);
-    uint64_t* empty = full + n_slots;
-    uint32_t* filled = reinterpret_cast<uint32_t*>(empty + n_slots);    // generations filled / released so far
-    uint32_t* released = filled + n_slots;
-    uint16_t* slots_k = reinterpret_cast<uint16_t*>(released + n_slots);
-    for (int k = threadIdx.x; k < a.bp.n_f; k += blockDim.x) { sm_tab[k] = a.cheb[k]; sm_zi[k] = a.cheb_zi[k]; }
-    for (int i = threadIdx.x; i < n_slots; i += blockDim.x) {
-        mbar_init(&full[i], 1u); mbar_init(&empty[i], 1u);
-        filled[i] = 0u; released[i] = 0u;
-    }
-    if (threadIdx.x == 0) { wq->prod_ticket = 0u; wq->cons_ticket = 0u; wq->done_producers = 0u; wq->pad = 0u; }
-    hist_init(sm_hist, a.n_bins);   // includes __syncthreads
-    const int n_chunks = (a.n_tau + kCheb - 1) / kCheb;
-    WarpReduce wr;
-    reduce_init(wr);
-    if (warp < n_prod) {
-        // ------------------------------------------------------------- producer
-        // A stream of elements (four columns per lane) runs through the warp: while element e is
-        // merged into its template's pool, element e + 1 -- of the same template or, at a template
-        // boundary, of the next one (generated and ticketed early) -- has its rasteriser chains and
-        // L2 gathers in flight.  The template-counter atomic for the template after that is in
-        // flight too (its result stays in lane 0 until needed).
-        struct Open { uint32_t s, slot, g; unsigned long long q; int32_t N, L, cbase; };
-        unsigned long long q_pref = 0;
-        if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
-        auto take_ticket = [&](Open& o) {
-            uint32_t s = 0;
-            if (lane == 0) s = atomicAdd(&wq->prod_ticket, 1u);
-            s = __shfl_sync(kFull, s, 0);
-            o.s = s; o.slot = s % (uint32_t)n_slots; o.g = s / (uint32_t)n_slots;
-        };
-        auto open = [&](ChebFetchCtx& f, Open& o) -> bool {
-            const unsigned long long q = __shfl_sync(kFull, q_pref, 0);
-            if (q >= a.n_tracks) return false;
-            if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
-            const Track t = make_track(a.bp, a.track_offset + q);
-            cheb_fetch_ctx(a, t, lane, f);
-            take_ticket(o);
-            o.q = q; o.N = f.N; o.L = f.L; o.cbase = f.cbase;
-            return true;
-        };
-        ChebFetchCtx F;
-        Open A, P;
-        ChebElem E, En;
-        ChebMergeState m;
-        bool have = open(F, A);
-        int i_f = 0, i_a = 0;
-        if (have) {
-            cheb_fetch(a, F, 0, E);
-            ws_wait(&empty[A.slot], &released[A.slot], A.g);   // only now: our previous ticket is already published
-            cheb_merge_init(m);
-        }
-        while (have) {
-            // fetch cursor: one element ahead of the merge cursor
-            bool have_next = true, switched = false;
-            i_f += 4;
-            if (i_f >= F.L) { have_next = open(F, P); i_f = 0; switched = true; }
-            if (have_next) cheb_fetch(a, F, i_f, En);
-            float2* pool_v = slots_v + (size_t)A.slot * S;
-            uint16_t* pool_k = slots_k + (size_t)A.slot * S;
-            cheb_merge(A.N, A.L, A.cbase, i_a, E, m, pool_v, pool_k, lane);
-            i_a += 4;
-            if (switched) {                          // that was the template's last element: publish it
-                const int n_merged = cheb_merge_finish(m, pool_v, pool_k, lane);   // ends with __syncwarp
-                if (lane == 0) {
-                    WsDesc d; d.q = A.q; d.N = A.N; d.n_merged = n_merged;
-                    desc[A.slot] = d;
-                    filled[A.slot] = A.g + 1u;
-                    mbar_arrive(&full[A.slot]);
-                }
-                have = have_next;
-                if (have) { A = P; i_a = 0; ws_wait(&empty[A.slot], &released[A.slot], A.g); cheb_merge_init(m); }
-            }
-            E = En;
-        }
-        uint32_t last = 0;
-        if (lane == 0) last = atomicAdd(&wq->done_producers, 1u) == (uint32_t)(n_prod - 1);
-        if (__shfl_sync(kFull, last, 0)) {
-            for (int c = 0; c < n_cons; ++c) {       // one poison ticket per consumer
-                take_ticket(A);
-                ws_wait(&empty[A.slot], &released[A.slot], A.g);
-                if (lane == 0) {
-                    WsDesc d; d.q = 0ull; d.N = -1; d.n_merged = 0;
-                    desc[A.slot] = d;
-                    filled[A.slot] = A.g + 1u;
-                    mbar_arrive(&full[A.slot]);
-                }
-            }
-        }
-    } else {
-        // ------------------------------------------------------------- consumer
-        for (;;) {
-            uint32_t s = 0;
-            if (lane == 0) s = atomicAdd(&wq->cons_ticket, 1u);
-            s = __shfl_sync(kFull, s, 0);
-            const uint32_t slot = s % (uint32_t)n_slots, g = s / (uint32_t)n_slots;
-            ws_wait(&full[slot], &filled[slot], g + 1u);   // full phase g complete <=> filled >= g + 1
-            const WsDesc d = desc[slot];
-            if (d.N < 0) break;                       // poison: the bank is exhausted
-            float2* pool_v = slots_v + (size_t)slot * S;
-            const uint16_t* pool_k = slots_k + (size_t)slot * S;
-            wr.pixels += (unsigned long long)d.N;
-            cheb_phase_b<STRIDE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, d.n_merged, norm_scale(d.N, a.norm),
-                                 a.track_offset + d.q, d.q, n_chunks, lane);
-            __syncwarp();
-            if (lane == 0) { released[slot] = g + 1u; mbar_arrive(&empty[slot]); }
-        }
     }
     reduce_finish(a, wr);
     hist_flush(sm_hist, a.hist, a.n_bins);

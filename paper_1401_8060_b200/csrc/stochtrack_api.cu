@@ -79,7 +79,6 @@ struct st_ctx {
     bool pick_valid; double pick_dtau; int pick_stride;   // memo of cheb_pick_stride
     std::vector<float> h_cheb;         // host-built Chebyshev tables: [n_f] float4, [n_f] float2 Ec, [n_f] float zi
     int reinsch_chains;                // tunable: packed recurrence chains in flight per lane (1 or 2)
-    int cheb_ws, cheb_prod, cheb_slots; // tunables: warp-specialised Chebyshev kernel, its producer warps, ring size cap
     char err[512];
 };
 
@@ -365,26 +364,6 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         if (smem > (size_t)c->smem_optin)
             return fail(c, ST_ENOSPC, "n_f %d / n_max %d need more shared memory than one SM has", c->n_f, n_max);
         const bool pk = plan.stride == 2;
-        // warp-specialised variant: producers fill a ring of pixel pools, consumers score them
-        const int ws_threads = c->recur_threads;
-        const int n_prod = c->cheb_prod;
-        const size_t fixed = hist_bytes(a.n_bins) + (size_t)c->n_f * sizeof(float4) + (size_t)((c->n_f + 3) & ~3) * sizeof(float) +
-                             sizeof(st::WsQueue);
-        const size_t per_slot = (size_t)stride * (sizeof(float2) + sizeof(uint16_t)) + sizeof(st::WsDesc) + 2 * sizeof(uint64_t) + 2 * sizeof(uint32_t);
-        int n_slots = (size_t)c->smem_optin > fixed ? (int)(((size_t)c->smem_optin - fixed) / per_slot) : 0;
-        if (n_slots > st::kWsMaxSlots) n_slots = st::kWsMaxSlots;
-        if (c->cheb_slots > 0 && c->cheb_slots < n_slots) n_slots = c->cheb_slots;
-        const int n_cons = ws_threads / 32 - n_prod;
-        if (c->cheb_ws && n_prod >= 1 && n_cons >= 1 && n_slots >= n_cons + 1 && want_warps >= (uint64_t)(4 * c->n_sm)) {
-            const size_t ws_smem = fixed + (size_t)n_slots * per_slot;
-            int rc = pk ? set_smem(c, st::k_score_cheb_ws<2>, ws_smem) : set_smem(c, st::k_score_cheb_ws<1>, ws_smem);
-            if (rc) return rc;
-            a.n_prod = n_prod; a.n_slots = n_slots;
-            if (pk) st::k_score_cheb_ws<2><<<(unsigned)c->n_sm, ws_threads, ws_smem, c->stream>>>(a);
-            else st::k_score_cheb_ws<1><<<(unsigned)c->n_sm, ws_threads, ws_smem, c->stream>>>(a);
-            ST_CUDA(c, cudaGetLastError());
-            return ST_OK;
-        }
         int rc = pk ? set_smem(c, st::k_score_cheb<2>, smem) : set_smem(c, st::k_score_cheb<1>, smem);
         if (rc) return rc;
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
@@ -507,13 +486,6 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->err[0] = 0;
     c->cheb_stride = 0; c->pick_valid = false; c->pick_dtau = 0.0; c->pick_stride = 0;
     c->reinsch_chains = 1;
-    c->cheb_ws = 0; c->cheb_prod = 4; c->cheb_slots = 0;   // warp-specialised variant: opt-in (ST_CHEB_WS=1) until it beats the plain kernel
-    const char* e3 = getenv("ST_CHEB_WS");
-    if (e3) c->cheb_ws = atoi(e3) != 0;
-    const char* e4 = getenv("ST_CHEB_PROD");
-    if (e4 && atoi(e4) >= 1 && atoi(e4) <= 16) c->cheb_prod = atoi(e4);
-    const char* e5 = getenv("ST_CHEB_SLOTS");
-    if (e5 && atoi(e5) >= 2) c->cheb_slots = atoi(e5);
     const char* e2 = getenv("ST_REINSCH_VAR");
     if (e2 && atoi(e2) >= 0 && atoi(e2) <= 3) c->reinsch_chains = atoi(e2);
     const char* e = getenv("ST_RECUR_THREADS");
