@@ -32,8 +32,10 @@ METRIC = "track_pixel_evals_per_s"
 UNIT = "evals/s"
 N_SM, FP32_LANES = 148, 128           # B200: 148 SMs x 128 FP32 lanes (B200_PROFILING.md, blackwell guide)
 FLOP_PER_EVAL = 4                     # Eq. 8 needs 2 FMA per (pixel, delay) once the phase factor is known
-# ncu --set full, dominant kernel, config 5 sub-range (profiles/); None until measured
-DRAM_TRAFFIC_BYTES_PER_LAUNCH = None
+# dram__bytes_read.sum + dram__bytes_write.sum of k_score_cheb from the ncu --set full capture in
+# profiles/r01_kernels.md (config 5: the 19.69 MB map is read from HBM once, then served by L2)
+DRAM_TRAFFIC_BYTES_PER_LAUNCH = {5: 19.87e6, 3: 9.88e6}
+L2_GATHER_PEAK_GBS = 9200.0          # random 32-byte sector gathers, measured (profiles/microbench_r01.md)
 
 
 def peaks():
@@ -214,11 +216,18 @@ def run_ours(args):
         "clocks": clocks,
         "roofline": {"bound": "alu", "kernel": {"chebyshev": "k_score_cheb", "reinsch": "k_score_reinsch", "rotation": "k_score_recur",
                                                 "table": "k_score_table", "random": "k_score_random"}.get(r.kernel_name, r.kernel_name), "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES_PER_LAUNCH,
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
                      "peak_how": peak_how + "; algorithmic 4 flop per track-pixel evaluation (DESIGN.md)"},
         "result": {"max_snr": combined["max_snr_f64"], "arg_track": combined["arg_track"],
                    "arg_tau_index": combined["arg_tau_index"]},
     }
+    if cfg.tau_mode == "random":
+        # the paper's one-delay mode is a gather: one 32-byte L2 sector per track pixel
+        gbs = 32.0 * per_launch_evals / (kernel_ms / args.steps * 1e-3) / 1e9
+        line["roofline"].update({"bound": "l2-gather", "achieved": gbs, "peak": L2_GATHER_PEAK_GBS, "unit": "GB/s",
+                                 "frac": gbs / L2_GATHER_PEAK_GBS,
+                                 "peak_how": "random 8-byte gathers from an L2-resident 19.7 MB buffer, one 32-byte sector each, "
+                                             "measured by st_microbench (profiles/microbench_r01.md)"})
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(cfg, csd, sigma, tau, seed, budget_s=args.cpu_budget)
     print(json.dumps(line))

@@ -236,18 +236,52 @@ __device__ __forceinline__ uint32_t hist_smem_words(int n_bins) { return (uint32
 
 // ----------------------------------------------------------------------- S0 --
 // p = CSD / sigma (Eq. 7); sigma <= 0 or non-finite masks the pixel (G11).
-__global__ void k_prepare_map(const float2* __restrict__ csd, const float* __restrict__ sigma,
-                              int sigma_kind, int n_f, size_t n_pix, float2* __restrict__ p)
+__device__ __forceinline__ float2 prepare_pixel(float2 c, float s)
 {
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_pix;
-         i += (size_t)gridDim.x * blockDim.x) {
-        float2 c = csd[i];
-        if (sigma_kind != 0) {
-            const float s = sigma_kind == 1 ? sigma[i % (size_t)n_f] : sigma[i];
-            if (!(s > 0.0f) || isinf(s)) { c.x = 0.0f; c.y = 0.0f; }
-            else { c.x = __fdiv_rn(c.x, s); c.y = __fdiv_rn(c.y, s); }
+    if (!(s > 0.0f) || isinf(s)) return make_float2(0.0f, 0.0f);
+    return make_float2(__fdiv_rn(c.x, s), __fdiv_rn(c.y, s));
+}
+// HBM bound (16 B read + 8 B written per pixel with a per-pixel sigma).  VEC: two pixels per thread
+// per iteration through 16-byte loads and stores (the host checks alignment and parity), two
+// iterations in flight.
+template <bool VEC>
+__global__ void __launch_bounds__(256) k_prepare_map(const float2* __restrict__ csd, const float* __restrict__ sigma,
+                                                     int sigma_kind, int n_f, size_t n_pix, float2* __restrict__ p)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x, t0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (VEC) {
+        const size_t n2 = n_pix >> 1;
+        const float4* c4 = reinterpret_cast<const float4*>(csd);
+        float4* p4 = reinterpret_cast<float4*>(p);
+        for (size_t i = t0; i < n2; i += 2 * stride) {
+            const size_t j = i + stride;
+            const bool two = j < n2;
+            const float4 a = __ldcs(&c4[i]);
+            const float4 b = two ? __ldcs(&c4[j]) : make_float4(0.f, 0.f, 0.f, 0.f);
+            float2 sa = make_float2(1.0f, 1.0f), sb = sa;
+            if (sigma_kind == 2) {
+                sa = __ldcs(reinterpret_cast<const float2*>(sigma) + i);
+                if (two) sb = __ldcs(reinterpret_cast<const float2*>(sigma) + j);
+            } else if (sigma_kind == 1) {
+                const size_t ka = (2 * i) % (size_t)n_f, kb = (2 * j) % (size_t)n_f;
+                sa = make_float2(__ldg(&sigma[ka]), __ldg(&sigma[ka + 1 < (size_t)n_f ? ka + 1 : 0]));
+                if (two) sb = make_float2(__ldg(&sigma[kb]), __ldg(&sigma[kb + 1 < (size_t)n_f ? kb + 1 : 0]));
+            }
+            float2 r0 = make_float2(a.x, a.y), r1 = make_float2(a.z, a.w);
+            float2 r2 = make_float2(b.x, b.y), r3 = make_float2(b.z, b.w);
+            if (sigma_kind != 0) {
+                r0 = prepare_pixel(r0, sa.x); r1 = prepare_pixel(r1, sa.y);
+                r2 = prepare_pixel(r2, sb.x); r3 = prepare_pixel(r3, sb.y);
+            }
+            p4[i] = make_float4(r0.x, r0.y, r1.x, r1.y);
+            if (two) p4[j] = make_float4(r2.x, r2.y, r3.x, r3.y);
         }
-        p[i] = c;
+    } else {
+        for (size_t i = t0; i < n_pix; i += stride) {
+            float2 c = csd[i];
+            if (sigma_kind != 0) c = prepare_pixel(c, sigma_kind == 1 ? sigma[i % (size_t)n_f] : sigma[i]);
+            p[i] = c;
+        }
     }
 }
 
@@ -384,7 +418,10 @@ __global__ void __launch_bounds__(256) k_score_table(const ScoreArgs a)
 // operations (two float64 seeds of the rasteriser, one F2F, MUFU.SIN, MUFU.COS): everything else
 // (floor, int <-> double, rounding to the nearest cycle) runs on the FP64 pipe through the
 // 1.5 * 2^52 constant, so that the binding unit is the L2 sector gather, not conversions.
-__global__ void __launch_bounds__(256) k_score_random(const ScoreArgs a)
+#ifndef ST_RANDOM_MIN_BLOCKS
+#define ST_RANDOM_MIN_BLOCKS 3
+#endif
+__global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);

@@ -551,8 +551,13 @@ int st_set_map(st_ctx* c, const void* csd_dev, const float* sigma_dev, int32_t s
     if (sigma_kind != ST_SIGMA_NONE && !sigma_dev) return fail(c, ST_EINVAL, "sigma is NULL");
     const size_t n_pix = (size_t)c->n_t * (size_t)c->n_f;
     const int blocks = (int)((n_pix + 255) / 256 < (size_t)(8 * c->n_sm) ? (n_pix + 255) / 256 : (size_t)(8 * c->n_sm));
-    st::k_prepare_map<<<blocks, 256, 0, c->stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, c->n_f, n_pix,
-                                                     at<float2>(c, c->L.map));
+    // two pixels per thread through 16-byte accesses when the pointers and the pixel count allow
+    const bool vec = (n_pix % 2 == 0) && ((uintptr_t)csd_dev % 16 == 0) &&
+                     (sigma_kind != ST_SIGMA_PER_PIXEL || (uintptr_t)sigma_dev % 8 == 0);
+    if (vec) st::k_prepare_map<true><<<blocks, 256, 0, c->stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, c->n_f, n_pix,
+                                                                    at<float2>(c, c->L.map));
+    else st::k_prepare_map<false><<<blocks, 256, 0, c->stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, c->n_f, n_pix,
+                                                                  at<float2>(c, c->L.map));
     ST_CUDA(c, cudaGetLastError());
     c->have_map = true;
     return ST_OK;
