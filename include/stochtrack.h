@@ -153,6 +153,31 @@ int st_set_map_host(st_ctx *ctx, const void *csd_host, const float *sigma_host, 
  * workspace), ST_ECUDA.                                                        */
 int st_search(st_ctx *ctx, const st_search_params *params, st_result *out);
 
+/* Batch / background mode (the background is estimated from many
+ * time-shifted maps, every one searched with its own template bank; BASELINE.json configs[3]):
+ * S0-S4 over n_maps maps in ONE call.  Map m is searched exactly as
+ *     st_set_map(csd[m], sigma[m]);  st_search(params with seed = seeds[m])
+ * would search it (same kernels, same results bit for bit), but nothing synchronises with the host
+ * between maps: per-map results and histograms accumulate on the device and come back once per
+ * group of ST_BATCH_GROUP maps, and with HOST buffers the copy of map m + 1 overlaps the search of
+ * map m (a second, internal stream and two staging buffers).                                   */
+#define ST_BATCH_GROUP 256
+typedef struct {
+    int32_t  n_maps;
+    int32_t  host_buffers;        /* 0: csd[m] / sigma[m] are DEVICE pointers, 1: HOST (pinned for overlap) */
+    const void  *const *csd;      /* HOST array of n_maps pointers: complex64 [n_t][n_f] each            */
+    const float *const *sigma;    /* HOST array of n_maps pointers per sigma_kind, or NULL when NONE      */
+    int32_t  sigma_kind;          /* ST_SIGMA_*                                                            */
+    int32_t  reserved;            /* must be 0                                                             */
+    const uint64_t *seeds;        /* HOST, n_maps template seeds (G16), or NULL: params->seed for every map */
+} st_batch;
+/* results: HOST [n_maps].  params->hist_out (when params->n_bins > 0): HOST [n_maps][n_bins], one
+ * histogram per map.  results[m].gpu_ms is 0; *gpu_ms_total (optional) receives the device time of
+ * the whole batch (CUDA events around everything the call enqueues).  Synchronous on return.
+ * Errors as st_search, plus ST_EINVAL for n_maps < 1 or a NULL entry.                           */
+int st_search_batch(st_ctx *ctx, const st_batch *batch, const st_search_params *params,
+                    st_result *results, float *gpu_ms_total);
+
 /* S1 as a pure HOST function: the control points of template `track_id`
  * (same arithmetic as the device generator).                                   */
 int st_track_params(const st_ctx *ctx, uint64_t seed, uint64_t track_id,

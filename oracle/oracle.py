@@ -209,3 +209,16 @@ def search(p, f_min, df, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=
             "n_evals": int(res.n_evals), "n_pixels": int(res.n_pixels),
             "threads_used": int(res.threads_used), "hist": hist, "snr": snr,
             "k": kd, "j0": j0, "N": Nn}
+
+
+def search_batch(csd_maps, sigma_maps, seeds, f_min, df, n_tracks, n_min, n_max, **kw):
+    """Batch / background mode: the background of the search is estimated from many (time-shifted)
+    maps, each searched on its own with its own template bank (PAPER.md:173, :232-234, :346
+    "different random seed for each run").  By definition a loop: map m -> O0 (prepare_map) and
+    O1-O5 (search) with seed seeds[m].  Returns the list of per-map result dicts."""
+    out = []
+    for m, csd in enumerate(csd_maps):
+        p = prepare_map(csd, None if sigma_maps is None else sigma_maps[m])
+        seed = int(seeds[m]) if np.ndim(seeds) else int(seeds)
+        out.append(search(p, f_min, df, n_tracks, seed, n_min, n_max, **kw))
+    return out

@@ -19,7 +19,7 @@ KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random",
 
 # every symbol include/stochtrack.h declares
 exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_workspace", "st_set_map",
-                    "st_set_map_host", "st_search", "st_track_params", "st_debug_rasterise",
+                    "st_set_map_host", "st_search", "st_search_batch", "st_track_params", "st_debug_rasterise",
                     "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words",
                     "st_last_error", "st_version")
 
@@ -53,6 +53,14 @@ class CResult(C.Structure):
                 ("kernel_used", C.c_int32), ("n_launches", C.c_int32), ("flags", C.c_int32),
                 ("gpu_ms", C.c_float), ("reserved", C.c_float)]
 
+
+class CBatch(C.Structure):
+    _fields_ = [("n_maps", C.c_int32), ("host_buffers", C.c_int32), ("csd", C.POINTER(C.c_void_p)),
+                ("sigma", C.POINTER(C.c_void_p)), ("sigma_kind", C.c_int32), ("reserved", C.c_int32),
+                ("seeds", C.POINTER(C.c_uint64))]
+
+
+BATCH_GROUP = 256
 
 _lib = None
 
@@ -90,7 +98,8 @@ def load_library():
     L.st_last_error.restype = C.c_char_p
     L.st_version.argtypes = []
     L.st_version.restype = C.c_char_p
-    for name in ("st_create", "st_set_workspace", "st_set_map", "st_set_map_host", "st_search", "st_track_params",
+    L.st_search_batch.argtypes = [vp, C.POINTER(CBatch), C.POINTER(CSearchParams), C.POINTER(CResult), C.POINTER(C.c_float)]
+    for name in ("st_create", "st_set_workspace", "st_set_map", "st_set_map_host", "st_search", "st_search_batch", "st_track_params",
                  "st_debug_rasterise", "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words"):
         getattr(L, name).restype = C.c_int
     _lib = L
@@ -213,12 +222,78 @@ class Stochtrack:
             p.hist_out = hist.ctypes.data_as(C.POINTER(C.c_uint64))
         r = CResult()
         self._check(self._L.st_search(self._ctx, C.byref(p), C.byref(r)))
+        return self._result(r, hist)
+
+    @staticmethod
+    def _result(r, hist):
         return SearchResult(max_snr=float(r.max_snr), max_snr_f64=float(r.max_snr_f64), arg_track=int(r.arg_track),
                             arg_tau_index=int(r.arg_tau_index), arg_tau=float(r.arg_tau),
                             arg_params=r.arg_params.as_dict(), n_evals=int(r.n_evals), n_pixels=int(r.n_pixels),
                             n_candidates=int(r.n_candidates), kernel_used=int(r.kernel_used),
                             kernel_name=KERNEL_NAMES.get(int(r.kernel_used), "?"), n_launches=int(r.n_launches),
                             flags=int(r.flags), gpu_ms=float(r.gpu_ms), hist=hist)
+
+    def search_batch(self, csd_maps, sigma_maps, seeds, n_tracks, n_min, n_max, tau_grid=None, tau_range=None,
+                     norm=NORM_SQRT_N, n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO):
+        """Batch / background mode (st_search_batch): one call over many maps.
+
+        csd_maps: sequence of complex64 [n_t][n_f] maps, all torch CUDA tensors (device path) or all
+        numpy arrays / CPU tensors (host path; pinned tensors let the copies overlap the searches).
+        sigma_maps: None or a sequence of the same length (all [n_f] or all [n_t][n_f], float32).
+        seeds: one template seed per map, or a single int used for every map.
+        Returns (list of SearchResult, gpu_ms_total); result.hist is the map's own histogram."""
+        torch = self._torch
+        n_maps = len(csd_maps)
+        on_dev = isinstance(csd_maps[0], torch.Tensor) and csd_maps[0].is_cuda
+        kind = SIGMA_NONE
+        if sigma_maps is not None:
+            shp = tuple(sigma_maps[0].shape)
+            kind = SIGMA_PER_FREQ if shp == (self.n_f,) else SIGMA_PER_PIXEL if shp == (self.n_t, self.n_f) else -1
+            if kind < 0 or len(sigma_maps) != n_maps:
+                raise ValueError("sigma_maps: one [n_f] or [n_t][n_f] array per map")
+        keep, cp, sp = [], (C.c_void_p * n_maps)(), (C.c_void_p * n_maps)()
+
+        def ptr(x, dt_t, dt_n, shape):
+            if tuple(x.shape) != shape:
+                raise ValueError(f"expected shape {shape}, got {tuple(x.shape)}")
+            if isinstance(x, torch.Tensor):
+                if x.is_cuda != on_dev or x.dtype != dt_t or not x.is_contiguous():
+                    raise ValueError("maps of a batch must be contiguous, of one dtype, and all on one side")
+                keep.append(x)
+                return x.data_ptr()
+            if on_dev:
+                raise ValueError("maps of a batch must all be CUDA tensors or all host arrays")
+            a = np.ascontiguousarray(x, dtype=dt_n)
+            keep.append(a)
+            return a.ctypes.data
+
+        for m in range(n_maps):
+            cp[m] = ptr(csd_maps[m], torch.complex64, np.complex64, (self.n_t, self.n_f))
+            if kind != SIGMA_NONE:
+                sp[m] = ptr(sigma_maps[m], torch.float32, np.float32, tuple(sigma_maps[0].shape))
+        b = CBatch()
+        b.n_maps, b.host_buffers, b.sigma_kind = n_maps, 0 if on_dev else 1, kind
+        b.csd = C.cast(cp, C.POINTER(C.c_void_p))
+        b.sigma = C.cast(sp, C.POINTER(C.c_void_p)) if kind != SIGMA_NONE else None
+        seed0 = 0
+        if np.ndim(seeds) == 0:
+            seed0 = int(seeds)
+        else:
+            sd = np.ascontiguousarray(seeds, dtype=np.uint64)
+            if sd.size != n_maps:
+                raise ValueError("seeds: one per map")
+            keep.append(sd)
+            b.seeds = sd.ctypes.data_as(C.POINTER(C.c_uint64))
+        p, k2 = self._params(n_tracks, seed0, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
+                             track_offset, kernel)
+        hist = None
+        if n_bins > 0:
+            hist = np.zeros((n_maps, n_bins), dtype=np.uint64)
+            p.hist_out = hist.ctypes.data_as(C.POINTER(C.c_uint64))
+        res = (CResult * n_maps)()
+        ms = C.c_float(0.0)
+        self._check(self._L.st_search_batch(self._ctx, C.byref(b), C.byref(p), res, C.byref(ms)))
+        return [self._result(res[m], hist[m] if hist is not None else None) for m in range(n_maps)], float(ms.value)
 
     def track_params(self, seed, track_id, n_min, n_max, tau_lo=0.0, tau_hi=0.0):
         t = CTrack()

@@ -25,7 +25,7 @@ constexpr uint64_t kMaxSamplesPerLaunch = 1ull << 31;   // keeps per-block u32 h
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t map, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, warp_best, stage_csd, stage_sigma, total;
+    size_t map, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, warp_best, stage_csd, stage_sigma, stage_csd2, stage_sigma2, b_scalars, b_result, b_hist, total;
 };
 
 Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
@@ -50,6 +50,12 @@ Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
     L.warp_best = o;   o += align_up((size_t)kWarpSlots * sizeof(st::WarpBest));
     L.stage_csd = o;   o += align_up(n_pix * sizeof(float2));
     L.stage_sigma = o; o += align_up(n_pix * sizeof(float));
+    // batch mode: second staging pair (copy of map m + 1 under the search of map m), per-map slots
+    L.stage_csd2 = o;   o += align_up(n_pix * sizeof(float2));
+    L.stage_sigma2 = o; o += align_up(n_pix * sizeof(float));
+    L.b_scalars = o;    o += align_up((size_t)ST_BATCH_GROUP * sizeof(st::Scalars));
+    L.b_result = o;     o += align_up((size_t)ST_BATCH_GROUP * sizeof(st::DeviceResult));
+    L.b_hist = o;       o += align_up((size_t)ST_BATCH_GROUP * (size_t)ST_MAX_BINS * sizeof(unsigned long long));
     L.total = o;
     return L;
 }
@@ -71,6 +77,10 @@ struct st_ctx {
     int table_kind, table_ch;          // which tables are currently built for tau_cached
     bool w_built;
     cudaEvent_t ev0, ev1;
+    cudaStream_t copy_stream;          // batch mode: host-to-device copies of the next map
+    cudaEvent_t ev_copied[2], ev_consumed[2];
+    st::DeviceResult* h_bres;          // pinned, ST_BATCH_GROUP
+    unsigned long long* h_bhist;       // pinned, ST_BATCH_GROUP x ST_MAX_BINS (allocated on first batch call)
     st::DeviceResult* h_res;           // pinned
     unsigned long long* h_hist;        // pinned, ST_MAX_BINS
     int n_sm, smem_optin;
@@ -450,13 +460,86 @@ st::ScoreArgs base_args(st_ctx* c, const st_search_params* p)
     return a;
 }
 
-int reset_search_state(st_ctx* c, int n_bins)
+// Where one search keeps its device state: the context's own slots, or the per-map slots of a batch.
+struct Slots {
+    st::Scalars* sc;
+    st::DeviceResult* res;
+    unsigned long long* hist;
+};
+Slots own_slots(st_ctx* c)
 {
-    ST_CUDA(c, cudaMemsetAsync(at<void>(c, c->L.scalars), 0, sizeof(st::Scalars), c->stream));
+    Slots s;
+    s.sc = at<st::Scalars>(c, c->L.scalars); s.res = at<st::DeviceResult>(c, c->L.result);
+    s.hist = at<unsigned long long>(c, c->L.hist);
+    return s;
+}
+Slots batch_slots(st_ctx* c, int i)
+{
+    Slots s;
+    s.sc = at<st::Scalars>(c, c->L.b_scalars) + i; s.res = at<st::DeviceResult>(c, c->L.b_result) + i;
+    s.hist = at<unsigned long long>(c, c->L.b_hist) + (size_t)i * ST_MAX_BINS;
+    return s;
+}
+
+int reset_search_state(st_ctx* c, int n_bins, const Slots& sl)
+{
+    ST_CUDA(c, cudaMemsetAsync(sl.sc, 0, sizeof(st::Scalars), c->stream));
     ST_CUDA(c, cudaMemsetAsync(at<void>(c, c->L.warp_best), 0, (size_t)kWarpSlots * sizeof(st::WarpBest), c->stream));
     if (n_bins > 0)
-        ST_CUDA(c, cudaMemsetAsync(at<void>(c, c->L.hist), 0, (size_t)n_bins * sizeof(unsigned long long), c->stream));
+        ST_CUDA(c, cudaMemsetAsync(sl.hist, 0, (size_t)n_bins * sizeof(unsigned long long), c->stream));
     // gmax_bits = 0 encodes "below every float" (enc(-inf) = 0x007FFFFF > 0)
+    return ST_OK;
+}
+
+// S1-S4 of one search, enqueued on the stream (no synchronisation): tables must be current.
+int enqueue_search(st_ctx* c, const st_search_params* p, const Plan& plan, const Slots& sl, int* n_launches,
+                   bool time_it);
+void fill_result(st_result* out, const st::DeviceResult& r, int n_tau, int kernel, int n_launches);
+
+void fill_result(st_result* out, const st::DeviceResult& r, int n_tau, int kernel, int n_launches)
+{
+    out->max_snr = r.max_snr; out->arg_tau_index = r.arg_m; out->max_snr_f64 = r.snr_f64;
+    out->arg_track = r.arg_id; out->arg_tau = r.arg_tau;
+    out->arg_params.N = r.track.N; out->arg_params.j0 = r.track.j0; out->arg_params.a = r.track.a;
+    out->arg_params.y0 = r.track.y0; out->arg_params.y1 = r.track.y1; out->arg_params.y2 = r.track.y2;
+    out->arg_params.tau = r.track.tau;
+    out->n_pixels = r.n_pixels; out->n_evals = r.n_pixels * (uint64_t)n_tau;
+    out->n_candidates = r.n_candidates; out->flags = r.flags; out->n_launches = n_launches;
+    out->kernel_used = kernel;
+}
+
+int enqueue_search(st_ctx* c, const st_search_params* p, const Plan& plan, const Slots& sl, int* n_launches,
+                   bool time_it)
+{
+    const int n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
+    int rc = reset_search_state(c, p->n_bins, sl);
+    if (rc) return rc;
+    st::ScoreArgs a = base_args(c, p);
+    a.sc = sl.sc; a.hist = sl.hist;
+    a.n_bins = p->n_bins;
+    a.hist_lo = (float)p->hist_lo;
+    a.hist_scale = p->n_bins > 0 ? (float)((double)p->n_bins / (p->hist_hi - p->hist_lo)) : 0.0f;
+    uint64_t per_launch = kMaxSamplesPerLaunch / (uint64_t)n_tau;
+    if (per_launch < 1) per_launch = 1;
+    if (time_it) ST_CUDA(c, cudaEventRecord(c->ev0, c->stream));
+    for (uint64_t done = 0; done < p->n_tracks; done += per_launch) {
+        a.track_offset = p->track_offset + done;
+        a.n_tracks = p->n_tracks - done < per_launch ? p->n_tracks - done : per_launch;
+        rc = launch_score(c, plan, a, p->n_max);
+        if (rc) return rc;
+        ++*n_launches;
+    }
+    if (time_it) ST_CUDA(c, cudaEventRecord(c->ev1, c->stream));
+    st::FinalArgs f;
+    memset(&f, 0, sizeof(f));
+    f.map = a.map; f.bp = a.bp; f.f_min = c->f_min; f.df = c->df;
+    f.norm = p->norm; f.tau_mode = p->tau_mode; f.n_tau = n_tau;
+    f.tau_d = at<double>(c, c->L.tau);
+    f.sc = a.sc; f.cand = a.cand; f.cand_cap = kCandCap; f.warp_best = a.warp_best; f.n_warp_slots = kWarpSlots;
+    f.out = sl.res;
+    st::k_finalize<<<1, 256, 0, c->stream>>>(f);
+    ST_CUDA(c, cudaGetLastError());
+    ++*n_launches;
     return ST_OK;
 }
 
@@ -482,6 +565,8 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->have_ws = c->have_map = false;
     c->table_kind = kNoTable; c->table_ch = 0; c->w_built = false;
     c->ev0 = c->ev1 = nullptr; c->h_res = nullptr; c->h_hist = nullptr;
+    c->copy_stream = nullptr; c->h_bres = nullptr; c->h_bhist = nullptr;
+    for (int i = 0; i < 2; ++i) { c->ev_copied[i] = nullptr; c->ev_consumed[i] = nullptr; }
     c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512;
     c->err[0] = 0;
     c->cheb_stride = 0; c->pick_valid = false; c->pick_dtau = 0.0; c->pick_stride = 0;
@@ -501,6 +586,13 @@ void st_destroy(st_ctx* c)
     if (c->ev1) cudaEventDestroy(c->ev1);
     if (c->h_res) cudaFreeHost(c->h_res);
     if (c->h_hist) cudaFreeHost(c->h_hist);
+    if (c->h_bres) cudaFreeHost(c->h_bres);
+    if (c->h_bhist) cudaFreeHost(c->h_bhist);
+    for (int i = 0; i < 2; ++i) {
+        if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]);
+        if (c->ev_consumed[i]) cudaEventDestroy(c->ev_consumed[i]);
+    }
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
 }
 
@@ -602,50 +694,121 @@ int st_search(st_ctx* c, const st_search_params* p, st_result* out)
     int n_launches = 0;
     rc = ensure_tables(c, p, plan, &n_launches);
     if (rc) return rc;
-    rc = reset_search_state(c, p->n_bins);
+    const Slots sl = own_slots(c);
+    rc = enqueue_search(c, p, plan, sl, &n_launches, true);
     if (rc) return rc;
-    st::ScoreArgs a = base_args(c, p);
-    a.n_bins = p->n_bins;
-    a.hist_lo = (float)p->hist_lo;
-    a.hist_scale = p->n_bins > 0 ? (float)((double)p->n_bins / (p->hist_hi - p->hist_lo)) : 0.0f;
-    uint64_t per_launch = kMaxSamplesPerLaunch / (uint64_t)n_tau;
-    if (per_launch < 1) per_launch = 1;
-    ST_CUDA(c, cudaEventRecord(c->ev0, c->stream));
-    for (uint64_t done = 0; done < p->n_tracks; done += per_launch) {
-        a.track_offset = p->track_offset + done;
-        a.n_tracks = p->n_tracks - done < per_launch ? p->n_tracks - done : per_launch;
-        rc = launch_score(c, plan, a, p->n_max);
-        if (rc) return rc;
-        ++n_launches;
-    }
-    ST_CUDA(c, cudaEventRecord(c->ev1, c->stream));
-    st::FinalArgs f;
-    memset(&f, 0, sizeof(f));
-    f.map = a.map; f.bp = a.bp; f.f_min = c->f_min; f.df = c->df;
-    f.norm = p->norm; f.tau_mode = p->tau_mode; f.n_tau = n_tau;
-    f.tau_d = at<double>(c, c->L.tau);
-    f.sc = a.sc; f.cand = a.cand; f.cand_cap = kCandCap; f.warp_best = a.warp_best; f.n_warp_slots = kWarpSlots;
-    f.out = at<st::DeviceResult>(c, c->L.result);
-    st::k_finalize<<<1, 256, 0, c->stream>>>(f);
-    ST_CUDA(c, cudaGetLastError());
-    ++n_launches;
-    ST_CUDA(c, cudaMemcpyAsync(c->h_res, f.out, sizeof(st::DeviceResult), cudaMemcpyDeviceToHost, c->stream));
+    ST_CUDA(c, cudaMemcpyAsync(c->h_res, sl.res, sizeof(st::DeviceResult), cudaMemcpyDeviceToHost, c->stream));
     if (p->n_bins > 0)
-        ST_CUDA(c, cudaMemcpyAsync(c->h_hist, a.hist, sizeof(unsigned long long) * (size_t)p->n_bins, cudaMemcpyDeviceToHost, c->stream));
+        ST_CUDA(c, cudaMemcpyAsync(c->h_hist, sl.hist, sizeof(unsigned long long) * (size_t)p->n_bins, cudaMemcpyDeviceToHost, c->stream));
     ST_CUDA(c, cudaStreamSynchronize(c->stream));
-    const st::DeviceResult& r = *c->h_res;
-    out->max_snr = r.max_snr; out->arg_tau_index = r.arg_m; out->max_snr_f64 = r.snr_f64;
-    out->arg_track = r.arg_id; out->arg_tau = r.arg_tau;
-    out->arg_params.N = r.track.N; out->arg_params.j0 = r.track.j0; out->arg_params.a = r.track.a;
-    out->arg_params.y0 = r.track.y0; out->arg_params.y1 = r.track.y1; out->arg_params.y2 = r.track.y2;
-    out->arg_params.tau = r.track.tau;
-    out->n_pixels = r.n_pixels; out->n_evals = r.n_pixels * (uint64_t)n_tau;
-    out->n_candidates = r.n_candidates; out->flags = r.flags; out->n_launches = n_launches;
+    fill_result(out, *c->h_res, n_tau, plan.kernel, n_launches);
     float ms = 0.0f;
     ST_CUDA(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
     out->gpu_ms = ms;
     if (p->n_bins > 0)
         for (int b = 0; b < p->n_bins; ++b) p->hist_out[b] = (uint64_t)c->h_hist[b];
+    return ST_OK;
+}
+
+int st_search_batch(st_ctx* c, const st_batch* b, const st_search_params* p, st_result* results, float* gpu_ms_total)
+{
+    int rc = validate(c, p, false);
+    if (rc) return rc;
+    if (!b || !results) return fail(c, ST_EINVAL, "batch / results is NULL");
+    if (b->n_maps < 1) return fail(c, ST_EINVAL, "n_maps must be >= 1");
+    if (b->reserved != 0) return fail(c, ST_EINVAL, "batch.reserved must be 0");
+    if (!b->csd) return fail(c, ST_EINVAL, "batch.csd is NULL");
+    if (b->sigma_kind < ST_SIGMA_NONE || b->sigma_kind > ST_SIGMA_PER_PIXEL) return fail(c, ST_EINVAL, "bad sigma_kind %d", b->sigma_kind);
+    if (b->sigma_kind != ST_SIGMA_NONE && !b->sigma) return fail(c, ST_EINVAL, "batch.sigma is NULL");
+    for (int m = 0; m < b->n_maps; ++m) {
+        if (!b->csd[m]) return fail(c, ST_EINVAL, "batch.csd[%d] is NULL", m);
+        if (b->sigma_kind != ST_SIGMA_NONE && !b->sigma[m]) return fail(c, ST_EINVAL, "batch.sigma[%d] is NULL", m);
+    }
+    if (p->n_bins > 0 && !p->hist_out) return fail(c, ST_EINVAL, "n_bins > 0 but hist_out is NULL");
+    Plan plan;
+    rc = make_plan(c, p, &plan);
+    if (rc) return rc;
+    const int n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
+    if (gpu_ms_total) *gpu_ms_total = 0.0f;
+    memset(results, 0, sizeof(st_result) * (size_t)b->n_maps);
+    if (p->n_tracks == 0) {
+        for (int m = 0; m < b->n_maps; ++m) {
+            results[m].kernel_used = plan.kernel; results[m].max_snr = -INFINITY; results[m].max_snr_f64 = -INFINITY;
+        }
+        if (p->n_bins > 0) memset(p->hist_out, 0, sizeof(uint64_t) * (size_t)p->n_bins * (size_t)b->n_maps);
+        return ST_OK;
+    }
+    if (!c->h_bres) ST_CUDA(c, cudaHostAlloc((void**)&c->h_bres, (size_t)ST_BATCH_GROUP * sizeof(st::DeviceResult), cudaHostAllocDefault));
+    if (p->n_bins > 0 && !c->h_bhist)
+        ST_CUDA(c, cudaHostAlloc((void**)&c->h_bhist, (size_t)ST_BATCH_GROUP * ST_MAX_BINS * sizeof(unsigned long long), cudaHostAllocDefault));
+    if (b->host_buffers) {
+        if (!c->copy_stream) ST_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            if (!c->ev_copied[i]) ST_CUDA(c, cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming));
+            if (!c->ev_consumed[i]) ST_CUDA(c, cudaEventCreateWithFlags(&c->ev_consumed[i], cudaEventDisableTiming));
+        }
+    }
+    int n_launches_tables = 0;
+    rc = ensure_tables(c, p, plan, &n_launches_tables);
+    if (rc) return rc;
+    const size_t n_pix = (size_t)c->n_t * (size_t)c->n_f;
+    const size_t n_sig = b->sigma_kind == ST_SIGMA_NONE ? 0 : b->sigma_kind == ST_SIGMA_PER_FREQ ? (size_t)c->n_f : n_pix;
+    void* stage_csd[2] = {at<void>(c, c->L.stage_csd), at<void>(c, c->L.stage_csd2)};
+    float* stage_sig[2] = {at<float>(c, c->L.stage_sigma), at<float>(c, c->L.stage_sigma2)};
+    // host buffers: copy of map m goes to staging pair m % 2 on the copy stream, once the prepare
+    // kernel of map m - 2 (which read that pair) has run
+    auto enqueue_copy = [&](int m) -> int {
+        const int sb = m & 1;
+        if (m >= 2) ST_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_consumed[sb], 0));
+        ST_CUDA(c, cudaMemcpyAsync(stage_csd[sb], b->csd[m], n_pix * sizeof(float2), cudaMemcpyHostToDevice, c->copy_stream));
+        if (n_sig) ST_CUDA(c, cudaMemcpyAsync(stage_sig[sb], b->sigma[m], n_sig * sizeof(float), cudaMemcpyHostToDevice, c->copy_stream));
+        ST_CUDA(c, cudaEventRecord(c->ev_copied[sb], c->copy_stream));
+        return ST_OK;
+    };
+    ST_CUDA(c, cudaEventRecord(c->ev0, c->stream));
+    if (b->host_buffers) {
+        // the copy stream must not run ahead of work already queued on the caller's stream
+        ST_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev0, 0));
+        rc = enqueue_copy(0);
+        if (rc) return rc;
+    }
+    st_search_params pm = *p;
+    for (int g0 = 0; g0 < b->n_maps; g0 += ST_BATCH_GROUP) {
+        const int g1 = g0 + ST_BATCH_GROUP < b->n_maps ? g0 + ST_BATCH_GROUP : b->n_maps;
+        std::vector<int> launches((size_t)(g1 - g0), 0);
+        for (int m = g0; m < g1; ++m) {
+            const int sb = m & 1;
+            if (b->host_buffers) {
+                if (m + 1 < b->n_maps) { rc = enqueue_copy(m + 1); if (rc) return rc; }
+                ST_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied[sb], 0));
+                rc = st_set_map(c, stage_csd[sb], stage_sig[sb], b->sigma_kind);
+                if (rc) return rc;
+                ST_CUDA(c, cudaEventRecord(c->ev_consumed[sb], c->stream));
+            } else {
+                rc = st_set_map(c, b->csd[m], b->sigma_kind != ST_SIGMA_NONE ? b->sigma[m] : nullptr, b->sigma_kind);
+                if (rc) return rc;
+            }
+            pm.seed = b->seeds ? b->seeds[m] : p->seed;
+            int nl = 1;                            // k_prepare_map
+            rc = enqueue_search(c, &pm, plan, batch_slots(c, m - g0), &nl, false);
+            if (rc) return rc;
+            launches[(size_t)(m - g0)] = nl;
+        }
+        ST_CUDA(c, cudaMemcpyAsync(c->h_bres, at<void>(c, c->L.b_result), (size_t)(g1 - g0) * sizeof(st::DeviceResult),
+                                   cudaMemcpyDeviceToHost, c->stream));
+        if (p->n_bins > 0)
+            ST_CUDA(c, cudaMemcpyAsync(c->h_bhist, at<void>(c, c->L.b_hist),
+                                       (size_t)(g1 - g0) * ST_MAX_BINS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+        if (g1 == b->n_maps) ST_CUDA(c, cudaEventRecord(c->ev1, c->stream));
+        ST_CUDA(c, cudaStreamSynchronize(c->stream));
+        for (int m = g0; m < g1; ++m) {
+            fill_result(&results[m], c->h_bres[m - g0], n_tau, plan.kernel, launches[(size_t)(m - g0)] + (m == 0 ? n_launches_tables : 0));
+            if (p->n_bins > 0)
+                for (int k = 0; k < p->n_bins; ++k)
+                    p->hist_out[(size_t)m * (size_t)p->n_bins + (size_t)k] = (uint64_t)c->h_bhist[(size_t)(m - g0) * ST_MAX_BINS + (size_t)k];
+        }
+    }
+    if (gpu_ms_total) ST_CUDA(c, cudaEventElapsedTime(gpu_ms_total, c->ev0, c->ev1));
     return ST_OK;
 }
 
@@ -713,7 +876,7 @@ int st_debug_scores(st_ctx* c, const st_search_params* p, uint64_t first, uint64
     int n_launches = 0;
     rc = ensure_tables(c, p, plan, &n_launches);
     if (rc) return rc;
-    rc = reset_search_state(c, 0);
+    rc = reset_search_state(c, 0, own_slots(c));
     if (rc) return rc;
     st::ScoreArgs a = base_args(c, p);
     a.track_offset = first; a.n_tracks = count; a.dump = snr_dev;

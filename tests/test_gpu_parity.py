@@ -401,3 +401,70 @@ def test_full_size_search_subrange_protocol(P, orc, cid):
     assert abs(one - ref["max_snr"]) <= 1e-12 * abs(one)
     for f in ("N", "j0", "a", "y0", "y1", "y2"):
         assert full.arg_params[f] == getattr(t, f)
+
+
+# ------------------------------------------------------------------ batch / background mode
+def _batch_inputs(orc, cfg, n_maps):
+    maps = [config_inputs(orc, cfg, m) for m in range(n_maps)]
+    seeds = [synth.map_seed(cfg, m) if cfg.n_maps > 1 else cfg.seed * 1000 + m for m in range(n_maps)]
+    return [x[0] for x in maps], (None if maps[0][1] is None else [x[1] for x in maps]), maps[0][2], seeds
+
+
+@pytest.mark.parametrize("cid,n_maps,n_tracks,side", [(1, 5, 1000, "device"), (1, 5, 1000, "host"),
+                                                      (2, 3, 6000, "host"), (4, 3, 20000, "device")])
+def test_batch_equals_individual_searches_and_oracle(P, orc, cid, n_maps, n_tracks, side):
+    """st_search_batch == n_maps x (st_set_map + st_search), bit for bit, and == the oracle's loop."""
+    import torch
+    cfg = synth.CONFIGS[cid]
+    csds, sigmas, tau, seeds = _batch_inputs(orc, cfg, n_maps)
+    st = make_ctx(P, cfg)
+    kw = dict(tau_grid=tau, n_bins=cfg.n_bins, hist_lo=cfg.hist_lo, hist_hi=cfg.hist_hi)
+    if side == "device":
+        c_in = [torch.from_numpy(c).cuda() for c in csds]
+        s_in = None if sigmas is None else [torch.from_numpy(x).cuda() for x in sigmas]
+    else:
+        c_in = [torch.from_numpy(c).pin_memory() for c in csds]
+        s_in = None if sigmas is None else [torch.from_numpy(x).pin_memory() for x in sigmas]
+    res, ms = st.search_batch(c_in, s_in, seeds, n_tracks, cfg.n_min, cfg.n_max, **kw)
+    assert len(res) == n_maps and ms > 0.0
+    refs = orc.search_batch(csds, sigmas, seeds, cfg.f_min, cfg.df, n_tracks, cfg.n_min, cfg.n_max, dump_snr=True, **kw)
+    for m in range(n_maps):
+        st.set_map(c_in[m] if side == "device" else csds[m], None if sigmas is None else (s_in[m] if side == "device" else sigmas[m]))
+        one = st.search(n_tracks, seeds[m], cfg.n_min, cfg.n_max, **kw)
+        for key in ("max_snr", "max_snr_f64", "arg_track", "arg_tau_index", "n_evals", "n_pixels", "flags", "kernel_used"):
+            assert res[m][key] == one[key], (m, key)
+        assert np.array_equal(res[m].hist, one.hist)
+        _assert_search_parity(res[m], refs[m], cfg)
+    assert len({r.arg_track for r in res}) > 1          # different maps / banks give different answers
+
+
+def test_batch_crosses_group_boundary_and_shares_a_bank(P, orc):
+    """More maps than ST_BATCH_GROUP (results come back in groups); a single seed = one shared bank."""
+    import torch
+    cfg = synth.CONFIGS[1]
+    n_maps = P.binding.BATCH_GROUP + 7
+    rng = np.random.Generator(np.random.PCG64(77))
+    base = synth.noise_csd(cfg.n_t, cfg.n_f, 123)
+    csds = [np.ascontiguousarray(np.roll(base, int(rng.integers(1, cfg.n_t)), axis=0)) for _ in range(n_maps)]   # time shifts
+    tau = synth.tau_linspace(cfg.n_tau)
+    st = make_ctx(P, cfg)
+    res, _ = st.search_batch([torch.from_numpy(c).cuda() for c in csds], None, 5, 200, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=64)
+    for m in (0, 1, P.binding.BATCH_GROUP - 1, P.binding.BATCH_GROUP, n_maps - 1):
+        ref = orc.search(orc.prepare_map(csds[m]), cfg.f_min, cfg.df, 200, 5, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=64)
+        assert (res[m].arg_track, res[m].arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+        assert abs(res[m].max_snr_f64 - ref["max_snr"]) <= 1e-11 * abs(ref["max_snr"])
+        assert int(res[m].hist.sum()) == 200 * cfg.n_tau
+
+
+def test_batch_argument_errors(P, orc):
+    import torch
+    cfg = synth.CONFIGS[1]
+    st = make_ctx(P, cfg)
+    csd = torch.from_numpy(synth.noise_csd(cfg.n_t, cfg.n_f, 1)).cuda()
+    tau = synth.tau_linspace(cfg.n_tau)
+    with pytest.raises(ValueError):
+        st.search_batch([csd, csd.cpu()], None, 1, 10, cfg.n_min, cfg.n_max, tau_grid=tau)     # mixed sides
+    with pytest.raises(ValueError):
+        st.search_batch([csd], None, [1, 2], 10, cfg.n_min, cfg.n_max, tau_grid=tau)            # seeds per map
+    res, _ = st.search_batch([csd], None, 1, 0, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=8)  # empty search
+    assert res[0].max_snr == -np.inf and int(res[0].hist.sum()) == 0
