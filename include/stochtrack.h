@@ -178,6 +178,29 @@ typedef struct {
 int st_search_batch(st_ctx *ctx, const st_batch *batch, const st_search_params *params,
                     st_result *results, float *gpu_ms_total);
 
+/* ft-map construction on the device (the step before S0; Eqs. 7 and A1-A4 at
+ * PAPER.md:96, :258-277; readings G19-G22 of DESIGN.md): two strain series -> 50 %-overlapping Hann
+ * segments of seg_len samples -> DFT -> auto-power P' from the n_neighbours non-overlapping segments
+ * on either side -> p = lambda s~_I^* s~_J, written straight into the context's map (the same state
+ * st_set_map leaves behind).  Float64 transform, float32 map.
+ *   s_i_dev, s_j_dev : DEVICE float64 [n_samples], n_samples >= (n_t + 1) * seg_len / 2
+ *   fs               : sample rate [Hz]; fs / seg_len must equal the context's df and f_min must be
+ *                      a multiple of df with f_min + n_f df <= fs / 2
+ *   seg_len          : power of two, 64 <= seg_len <= 8192
+ *   scratch_dev      : DEVICE, st_ftmap_scratch_bytes(ctx, seg_len) bytes, 256-byte aligned, caller-owned;
+ *                      after the call it holds s~_I then s~_J (float64 complex [n_t][n_f] each, parity export)
+ * Stream-ordered.  Errors: ST_EINVAL, ST_ESTATE (no workspace), ST_ENOSPC (scratch), ST_ECUDA.      */
+typedef struct {
+    double  fs;
+    int32_t seg_len;
+    int32_t n_neighbours;    /* >= 1; segments j +- 2 .. j +- (n_neighbours + 1), those inside the map (G20) */
+} st_ftmap_params;
+size_t st_ftmap_scratch_bytes(const st_ctx *ctx, int32_t seg_len);
+int st_set_map_from_strain(st_ctx *ctx, const double *s_i_dev, const double *s_j_dev, int64_t n_samples,
+                           const st_ftmap_params *params, void *scratch_dev, size_t scratch_bytes);
+/* Parity export: copy the context's current map p (complex64 [n_t][n_f]) to p_out_dev (DEVICE).   */
+int st_debug_get_map(st_ctx *ctx, void *p_out_dev);
+
 /* S1 as a pure HOST function: the control points of template `track_id`
  * (same arithmetic as the device generator).                                   */
 int st_track_params(const st_ctx *ctx, uint64_t seed, uint64_t track_id,

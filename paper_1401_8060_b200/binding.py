@@ -19,7 +19,8 @@ KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random",
 
 # every symbol include/stochtrack.h declares
 exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_workspace", "st_set_map",
-                    "st_set_map_host", "st_search", "st_search_batch", "st_track_params", "st_debug_rasterise",
+                    "st_set_map_host", "st_search", "st_search_batch", "st_ftmap_scratch_bytes", "st_set_map_from_strain", "st_debug_get_map",
+                    "st_track_params", "st_debug_rasterise",
                     "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words",
                     "st_last_error", "st_version")
 
@@ -52,6 +53,10 @@ class CResult(C.Structure):
                 ("n_evals", C.c_uint64), ("n_pixels", C.c_uint64), ("n_candidates", C.c_int32),
                 ("kernel_used", C.c_int32), ("n_launches", C.c_int32), ("flags", C.c_int32),
                 ("gpu_ms", C.c_float), ("reserved", C.c_float)]
+
+
+class CFtmapParams(C.Structure):
+    _fields_ = [("fs", C.c_double), ("seg_len", C.c_int32), ("n_neighbours", C.c_int32)]
 
 
 class CBatch(C.Structure):
@@ -98,6 +103,12 @@ def load_library():
     L.st_last_error.restype = C.c_char_p
     L.st_version.argtypes = []
     L.st_version.restype = C.c_char_p
+    L.st_ftmap_scratch_bytes.argtypes = [vp, C.c_int32]
+    L.st_ftmap_scratch_bytes.restype = C.c_size_t
+    L.st_set_map_from_strain.argtypes = [vp, vp, vp, C.c_int64, C.POINTER(CFtmapParams), vp, C.c_size_t]
+    L.st_set_map_from_strain.restype = C.c_int
+    L.st_debug_get_map.argtypes = [vp, vp]
+    L.st_debug_get_map.restype = C.c_int
     L.st_search_batch.argtypes = [vp, C.POINTER(CBatch), C.POINTER(CSearchParams), C.POINTER(CResult), C.POINTER(C.c_float)]
     for name in ("st_create", "st_set_workspace", "st_set_map", "st_set_map_host", "st_search", "st_search_batch", "st_track_params",
                  "st_debug_rasterise", "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words"):
@@ -191,6 +202,44 @@ class Stochtrack:
             if c.dtype != np.complex64 or (s is not None and s.dtype != np.float32):
                 raise ValueError("host csd must be complex64 and sigma float32")
             self._check(self._L.st_set_map_host(self._ctx, c.ctypes.data, s.ctypes.data if s is not None else 0, kind))
+
+    def set_map_from_strain(self, s_i, s_j, fs, seg_len, n_neighbours=4):
+        """ft-map construction on the device (st_set_map_from_strain): s_i, s_j float64 CUDA tensors of
+        the two strain series; the context's map becomes p = lambda s~_I^* s~_J (Eqs. 7, A4)."""
+        torch = self._torch
+        for x in (s_i, s_j):
+            if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float64 and x.is_contiguous() and x.dim() == 1):
+                raise ValueError("strain series must be contiguous 1-D float64 CUDA tensors")
+        if s_i.numel() != s_j.numel():
+            raise ValueError("the two strain series must have the same length")
+        need = self._L.st_ftmap_scratch_bytes(self._ctx, int(seg_len))
+        if need == 0:
+            raise StError(ST_EINVAL, "st_ftmap_scratch_bytes: bad seg_len")
+        if getattr(self, "_ft_scratch", None) is None or self._ft_scratch.numel() < need:
+            self._ft_scratch = torch.empty(need, dtype=torch.uint8, device=self.device)
+        fp = CFtmapParams(float(fs), int(seg_len), int(n_neighbours))
+        self._check(self._L.st_set_map_from_strain(self._ctx, s_i.data_ptr(), s_j.data_ptr(), s_i.numel(), C.byref(fp),
+                                                   self._ft_scratch.data_ptr(), self._ft_scratch.numel()))
+        self._keep = [s_i, s_j]
+
+    def debug_get_map(self):
+        """The context's current map p as a complex64 numpy array [n_t][n_f] (parity export)."""
+        torch = self._torch
+        out = torch.empty((self.n_t, self.n_f), dtype=torch.complex64, device=self.device)
+        self._check(self._L.st_debug_get_map(self._ctx, out.data_ptr()))
+        self.synchronize()
+        return out.cpu().numpy()
+
+    def debug_strain_spectra(self):
+        """s~_I, s~_J (complex128 [n_t][n_f]) left in the scratch buffer by set_map_from_strain."""
+        torch = self._torch
+        self.synchronize()
+        n = self.n_t * self.n_f
+        stride = (n * 16 + 255) // 256 * 256
+        raw = self._ft_scratch
+        a = raw[:n * 16].view(torch.complex128).reshape(self.n_t, self.n_f).cpu().numpy()
+        b = raw[stride:stride + n * 16].view(torch.complex128).reshape(self.n_t, self.n_f).cpu().numpy()
+        return a, b
 
     # ------------------------------------------------------------ S1-S4
     def _params(self, n_tracks, seed, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,

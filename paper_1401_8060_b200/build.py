@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libstochtrack_b200.so")
 MICRO = os.path.join(HERE, "st_microbench")
 SOURCES = ["stochtrack_api.cu"]
-HEADERS = ["st_kernels.cuh", "st_track.cuh", os.path.join("..", "..", "include", "stochtrack.h")]
+HEADERS = ["st_kernels.cuh", "st_track.cuh", "st_ftmap.cuh", os.path.join("..", "..", "include", "stochtrack.h")]
 # -ffp-contract=off: the host copy of the rasteriser arithmetic (st_track_params)
 # must not be contracted into FMAs (G15); device code uses *_rn intrinsics.
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -1,0 +1,112 @@
+// st_ftmap.cuh -- ft-map construction on the GPU: two strain series -> the complex SNR map p(t; f)
+// that the search consumes, with no host round trip.
+//
+//   k_ft_twiddles   W_L^t = e^{-2 pi i t / L}, t < L/2, float64 (sincospi)
+//   k_ft_segments   F1 + F2: one CTA per segment: Hann window, ONE complex FFT of length L for both
+//                   detectors (z = w (s_I + i s_J)), in shared memory, float64; the band
+//                   [k_lo, k_lo + n_f) of s~_I and s~_J is separated and stored
+//   k_ft_normalise  F3 + F4: P' from the neighbouring segments (Eq. A3),
+//                   p = sqrt(2) s~_I^* s~_J / sqrt(P'_I P'_J) (Eqs. 7, A4; readings G19-G22 of DESIGN.md)
+//
+// Float64 because strain spectra span many decades (a float32 transform leaks rounding error of the
+// loud low-frequency band into the quiet one); the transform is ~1e9 flop per map and is not the
+// bottleneck: k_ft_segments is bound by shared-memory bandwidth, k_ft_normalise by HBM/L2 traffic.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace st {
+
+constexpr int kFtMaxLen = 8192;        // L <= 8192: L double2 = 128 KB of shared memory
+constexpr int kFtThreads = 1024;
+
+__global__ void k_ft_twiddles(int L, double2* __restrict__ W)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= L / 2) return;
+    double s, c;
+    sincospi(-2.0 * (double)t / (double)L, &s, &c);
+    W[t] = make_double2(c, s);
+}
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b)
+{
+    return make_double2(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x));
+}
+
+// One CTA per segment j: samples [j L/2, j L/2 + L).  In-place radix-2 decimation-in-frequency FFT
+// (Gentleman-Sande): log2 L passes of L/2 butterflies, output in bit-reversed order.  With
+// z = w (s_I + i s_J):  s~_I(k) = (Z_k + conj Z_{L-k}) / 2,  s~_J(k) = (Z_k - conj Z_{L-k}) / (2 i).
+__global__ void __launch_bounds__(kFtThreads, 1)
+k_ft_segments(const double* __restrict__ s_i, const double* __restrict__ s_j, int L, int log2L,
+              const double2* __restrict__ W, int k_lo, int n_f,
+              double2* __restrict__ st_i, double2* __restrict__ st_j)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    double2* x = reinterpret_cast<double2*>(smem);
+    const int j = blockIdx.x;
+    const size_t base = (size_t)j * (size_t)(L / 2);
+    for (int n = threadIdx.x; n < L; n += blockDim.x) {
+        double sn, cs;
+        sincospi(2.0 * (double)n / (double)L, &sn, &cs);
+        const double w = 0.5 * (1.0 - cs);                       // Hann (G19)
+        x[n] = make_double2(w * s_i[base + n], w * s_j[base + n]);
+    }
+    __syncthreads();
+    for (int s = 0; s < log2L; ++s) {
+        const int half = L >> (s + 1);
+        for (int b = threadIdx.x; b < L / 2; b += blockDim.x) {
+            const int pos = b & (half - 1);
+            const int i0 = ((b - pos) << 1) + pos, i1 = i0 + half;
+            const double2 a = x[i0], c = x[i1];
+            x[i0] = make_double2(a.x + c.x, a.y + c.y);
+            x[i1] = cmul(make_double2(a.x - c.x, a.y - c.y), W[(size_t)pos << s]);
+        }
+        __syncthreads();
+    }
+    const int shift = 32 - log2L;
+    for (int q = threadIdx.x; q < n_f; q += blockDim.x) {
+        const int k = k_lo + q;
+        const double2 zk = x[__brev((unsigned)k) >> shift];
+        const double2 zm = x[__brev((unsigned)((L - k) & (L - 1))) >> shift];
+        // Z_k + conj Z_{L-k} = (zk.x + zm.x, zk.y - zm.y);  Z_k - conj Z_{L-k} = (zk.x - zm.x, zk.y + zm.y)
+        st_i[(size_t)j * n_f + q] = make_double2(0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y));
+        st_j[(size_t)j * n_f + q] = make_double2(0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x));
+    }
+}
+
+// P'(t_j; f) = mean |s~|^2 over j' = j +- 2 .. j +- (n_nb + 1) inside the map (G20); masked pixels -> 0.
+__global__ void __launch_bounds__(256)
+k_ft_normalise(const double2* __restrict__ st_i, const double2* __restrict__ st_j, int n_t, int n_f, int n_nb,
+               float2* __restrict__ p)
+{
+    const size_t n_pix = (size_t)n_t * (size_t)n_f;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_pix; i += (size_t)gridDim.x * blockDim.x) {
+        const int j = (int)(i / (size_t)n_f), q = (int)(i % (size_t)n_f);
+        double pi = 0.0, pj = 0.0;
+        int cnt = 0;
+        for (int d = 2; d <= n_nb + 1; ++d) {
+            for (int sgn = -1; sgn <= 1; sgn += 2) {
+                const int jj = j + sgn * d;
+                if (jj < 0 || jj >= n_t) continue;
+                const double2 a = st_i[(size_t)jj * n_f + q], b = st_j[(size_t)jj * n_f + q];
+                pi += a.x * a.x + a.y * a.y;
+                pj += b.x * b.x + b.y * b.y;
+                ++cnt;
+            }
+        }
+        float2 out = make_float2(0.0f, 0.0f);
+        if (cnt > 0) {
+            const double prod = (pi / (double)cnt) * (pj / (double)cnt);
+            if (prod > 0.0 && isfinite(prod)) {
+                const double2 a = st_i[i], b = st_j[i];
+                const double sc = sqrt(2.0) / sqrt(prod);                           // G21
+                // conj(a) * b
+                out = make_float2((float)(sc * (a.x * b.x + a.y * b.y)), (float)(sc * (a.x * b.y - a.y * b.x)));
+            }
+        }
+        p[i] = out;
+    }
+}
+
+}  // namespace st

@@ -14,6 +14,7 @@
 
 #include "../../include/stochtrack.h"
 #include "st_kernels.cuh"
+#include "st_ftmap.cuh"
 
 namespace {
 
@@ -809,6 +810,62 @@ int st_search_batch(st_ctx* c, const st_batch* b, const st_search_params* p, st_
         }
     }
     if (gpu_ms_total) ST_CUDA(c, cudaEventElapsedTime(gpu_ms_total, c->ev0, c->ev1));
+    return ST_OK;
+}
+
+size_t st_ftmap_scratch_bytes(const st_ctx* c, int32_t seg_len)
+{
+    if (!c || seg_len < 64 || seg_len > st::kFtMaxLen || (seg_len & (seg_len - 1))) return 0;
+    const size_t n_pix = (size_t)c->n_t * (size_t)c->n_f;
+    return 2 * align_up(n_pix * sizeof(double2)) + align_up((size_t)(seg_len / 2) * sizeof(double2));
+}
+
+int st_set_map_from_strain(st_ctx* c, const double* s_i, const double* s_j, int64_t n_samples,
+                           const st_ftmap_params* fp, void* scratch, size_t scratch_bytes)
+{
+    if (!c) return ST_EINVAL;
+    if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
+    if (!s_i || !s_j || !fp || !scratch) return fail(c, ST_EINVAL, "NULL argument");
+    const int L = fp->seg_len;
+    if (L < 64 || L > st::kFtMaxLen || (L & (L - 1))) return fail(c, ST_EINVAL, "seg_len %d must be a power of two in [64, %d]", L, st::kFtMaxLen);
+    if (!(fp->fs > 0.0) || !isfinite(fp->fs)) return fail(c, ST_EINVAL, "bad sample rate");
+    if (fp->n_neighbours < 1) return fail(c, ST_EINVAL, "n_neighbours must be >= 1");
+    const double df = fp->fs / (double)L;
+    if (fabs(df - c->df) > 1e-9 * c->df) return fail(c, ST_EINVAL, "fs / seg_len = %g Hz differs from the context's df = %g Hz", df, c->df);
+    const double kf = c->f_min / df;
+    const int k_lo = (int)llround(kf);
+    if (fabs(kf - (double)k_lo) > 1e-9) return fail(c, ST_EINVAL, "f_min %g is not a multiple of df %g", c->f_min, df);
+    if (k_lo + c->n_f > L / 2) return fail(c, ST_EINVAL, "the band ends above the Nyquist frequency");
+    if (n_samples < (int64_t)(c->n_t + 1) * (int64_t)(L / 2)) return fail(c, ST_EINVAL, "%lld samples hold fewer than n_t = %d segments", (long long)n_samples, c->n_t);
+    if (((uintptr_t)scratch % kAlign) != 0) return fail(c, ST_EINVAL, "scratch must be 256-byte aligned");
+    if (scratch_bytes < st_ftmap_scratch_bytes(c, L)) return fail(c, ST_ENOSPC, "scratch of %zu bytes is below %zu", scratch_bytes, st_ftmap_scratch_bytes(c, L));
+    const size_t n_pix = (size_t)c->n_t * (size_t)c->n_f;
+    double2* st_i = (double2*)scratch;
+    double2* st_j = (double2*)((unsigned char*)scratch + align_up(n_pix * sizeof(double2)));
+    double2* W = (double2*)((unsigned char*)scratch + 2 * align_up(n_pix * sizeof(double2)));
+    int log2L = 0;
+    while ((1 << log2L) < L) ++log2L;
+    st::k_ft_twiddles<<<(L / 2 + 255) / 256, 256, 0, c->stream>>>(L, W);
+    ST_CUDA(c, cudaGetLastError());
+    const size_t smem = (size_t)L * sizeof(double2);
+    int rc = set_smem(c, st::k_ft_segments, smem);
+    if (rc) return rc;
+    st::k_ft_segments<<<c->n_t, st::kFtThreads, smem, c->stream>>>(s_i, s_j, L, log2L, W, k_lo, c->n_f, st_i, st_j);
+    ST_CUDA(c, cudaGetLastError());
+    const int blocks = (int)((n_pix + 255) / 256 < (size_t)(8 * c->n_sm) ? (n_pix + 255) / 256 : (size_t)(8 * c->n_sm));
+    st::k_ft_normalise<<<blocks, 256, 0, c->stream>>>(st_i, st_j, c->n_t, c->n_f, fp->n_neighbours, at<float2>(c, c->L.map));
+    ST_CUDA(c, cudaGetLastError());
+    c->have_map = true;
+    return ST_OK;
+}
+
+int st_debug_get_map(st_ctx* c, void* p_out_dev)
+{
+    if (!c) return ST_EINVAL;
+    if (!c->have_ws || !c->have_map) return fail(c, ST_ESTATE, "no map");
+    if (!p_out_dev) return fail(c, ST_EINVAL, "output is NULL");
+    ST_CUDA(c, cudaMemcpyAsync(p_out_dev, at<void>(c, c->L.map), (size_t)c->n_t * (size_t)c->n_f * sizeof(float2),
+                               cudaMemcpyDeviceToDevice, c->stream));
     return ST_OK;
 }
 

@@ -1,0 +1,97 @@
+"""GPU parity of the ft-map construction (st_set_map_from_strain) against oracle/ftmap.py."""
+import numpy as np
+import pytest
+
+from oracle import ftmap as F
+from workloads import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1401_8060_b200 as pkg
+    from paper_1401_8060_b200 import build
+    build.build()
+    pkg.load_library()
+    return pkg
+
+
+def _coloured_noise(rng, n, fs):
+    """Gaussian noise with a steep low-frequency wall (5 decades in amplitude between 10 Hz and the band),
+    the feature of strain data that makes a float32 transform inadequate."""
+    f = np.fft.rfftfreq(n, 1.0 / fs)
+    shape = 1.0 + (60.0 / np.maximum(f, 1.0)) ** 6
+    return np.fft.irfft(np.fft.rfft(rng.standard_normal(n)) * shape, n)
+
+
+@pytest.mark.parametrize("L,fs,n_t,f_min,n_f,n_nb,coloured", [
+    (64, 64.0, 9, 3.0, 20, 2, False),            # smallest transform, ragged everything
+    (1024, 1024.0, 40, 40.0, 300, 4, True),
+    (4096, 4096.0, 250, 40.0, 961, 4, True),     # config 2 shape: 250 s x 961 bins at 1 s x 1 Hz
+    (8192, 8192.0, 120, 40.0, 2461, 8, False),   # largest transform, config 3-5 band (2461 bins from 40 Hz)
+])
+def test_ftmap_matches_oracle(P, L, fs, n_t, f_min, n_f, n_nb, coloured):
+    import torch
+    rng = np.random.default_rng(L + n_t)
+    n = (n_t + 1) * L // 2 + 13                   # a ragged tail the segmentation ignores
+    mk = (lambda: _coloured_noise(rng, n, fs)) if coloured else (lambda: rng.standard_normal(n))
+    s_i, s_j = 1e-21 * mk(), 3e-21 * mk()          # strain-like amplitudes
+    st = P.Stochtrack(n_t, n_f, fs / L, f_min, max_n_tau=64)
+    st.set_map_from_strain(torch.from_numpy(s_i).cuda(), torch.from_numpy(s_j).cuda(), fs, L, n_nb)
+    p = st.debug_get_map()
+    a, b = st.debug_strain_spectra()
+    ref, r_i, r_j, _, _ = F.ftmap(s_i, s_j, fs, L, n_t, f_min, n_f, n_nb)
+    # float64 transform on both sides: agreement to rounding, relative to the segment's largest bin IN THE
+    # WHOLE SPECTRUM (the error of an FFT scales with the rms of its input)
+    scale_i = np.sqrt(L) * np.abs(s_i).max() * 4
+    scale_j = np.sqrt(L) * np.abs(s_j).max() * 4
+    assert np.abs(a - r_i).max() <= 1e-12 * scale_i and np.abs(b - r_j).max() <= 1e-12 * scale_j
+    # the map is float32: one rounding of an O(1) number (plus the float64 error above, amplified by
+    # the dynamic range of a coloured spectrum)
+    tol = 2e-6 * np.maximum(np.abs(ref), 1.0) + (1e-5 if coloured else 0.0)
+    assert np.all(np.abs(p - ref) <= tol), float(np.abs(p - ref).max())
+    assert np.array_equal(p == 0, ref == 0)        # the same pixels are masked
+
+
+def test_ftmap_then_search_equals_oracle_chain(P, orc):
+    """strain -> map -> search, all on the device, against ftmap oracle -> search oracle."""
+    import torch
+    rng = np.random.default_rng(21)
+    fs, L, n_t, n_f, f_min = 1024.0, 1024, 64, 200, 100.0
+    n = (n_t + 1) * L // 2
+    t = np.arange(n) / fs
+    tau0 = 3e-3
+    phase = lambda x: 2 * np.pi * (150.0 * x + 1.25 * x ** 2)
+    s_i = rng.standard_normal(n) + 0.7 * np.cos(phase(t))
+    s_j = rng.standard_normal(n) + 0.7 * np.cos(phase(t - tau0))
+    st = P.Stochtrack(n_t, n_f, fs / L, f_min, max_n_tau=64)
+    st.set_map_from_strain(torch.from_numpy(s_i).cuda(), torch.from_numpy(s_j).cuda(), fs, L, 8)
+    tau = synth.tau_linspace(41, -0.01, 0.01)
+    r = st.search(20000, 3, 30, 64, tau_grid=tau, n_bins=100)
+    # the oracle searches the float32 map the device built (its own float64 map differs in the last
+    # float32 bit of each pixel; the maps themselves are compared in test_ftmap_matches_oracle)
+    ref = orc.search(st.debug_get_map().astype(np.complex128), f_min, fs / L, 20000, 3, 30, 64, tau_grid=tau, n_bins=100)
+    assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+    assert abs(r.max_snr_f64 - ref["max_snr"]) <= 1e-11 * abs(ref["max_snr"])
+    assert r.max_snr_f64 > 8.0 and abs(r.arg_tau - tau0) <= 1e-3
+    pure, *_ = F.ftmap(s_i, s_j, fs, L, n_t, f_min, n_f, 8)
+    ref2 = orc.search(pure, f_min, fs / L, 20000, 3, 30, 64, tau_grid=tau)
+    assert (ref2["arg_track"], ref2["arg_tau_index"]) == (r.arg_track, r.arg_tau_index)
+    assert abs(ref2["max_snr"] - r.max_snr_f64) <= 1e-5 * abs(ref2["max_snr"])
+
+
+def test_ftmap_argument_errors(P):
+    import torch
+    st = P.Stochtrack(10, 20, 1.0, 40.0, max_n_tau=64)
+    s = torch.zeros(11 * 512, dtype=torch.float64, device="cuda")
+    for kw in (dict(fs=1024.0, seg_len=1000),                  # not a power of two
+               dict(fs=2048.0, seg_len=1024),                  # df mismatch
+               dict(fs=64.0, seg_len=64),                      # band above Nyquist
+               dict(fs=1024.0, seg_len=1024, n_neighbours=0)):
+        with pytest.raises(P.StError):
+            st.set_map_from_strain(s, s, **kw)
+    with pytest.raises(P.StError):
+        st.set_map_from_strain(s[:1000], s[:1000], 1024.0, 1024)   # too few samples
