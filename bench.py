@@ -259,11 +259,40 @@ def run_ours(args):
                                  "frac": gbs / L2_GATHER_PEAK_GBS,
                                  "peak_how": "random 8-byte gathers from an L2-resident 19.7 MB buffer, one 32-byte sector each, "
                                              "measured by st_microbench (profiles/microbench_r01.md)"})
+    if world == 1 and args.ftmap:
+        line["ftmap"] = ftmap_timing(pkg, torch, cfg, dev)
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(cfg, csd, sigma, tau, seed, budget_s=args.cpu_budget)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def ftmap_timing(pkg, torch, cfg, dev, seg_len=8192, reps=5):
+    """The step before the hot path, timed on its own: two synthetic strain series
+    of the config's duration -> st_set_map_from_strain (float64 FFT, neighbour PSDs, p into the map)."""
+    fs = float(seg_len) * cfg.df
+    n = (cfg.n_t + 1) * seg_len // 2
+    g = torch.Generator(device=dev).manual_seed(1234)
+    s_i = torch.randn(n, dtype=torch.float64, device=dev, generator=g) * 1e-21
+    s_j = torch.randn(n, dtype=torch.float64, device=dev, generator=g) * 1e-21
+    st = pkg.Stochtrack(cfg.n_t, cfg.n_f, cfg.df, cfg.f_min, max_n_tau=64, device=dev)
+    for _ in range(3):
+        st.set_map_from_strain(s_i, s_j, fs, seg_len, 4)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    for a, b in ev:
+        a.record()
+        st.set_map_from_strain(s_i, s_j, fs, seg_len, 4)
+        b.record()
+    torch.cuda.synchronize()
+    ms = float(np.median([a.elapsed_time(b) for a, b in ev]))
+    # algorithmic bytes: both series read once (16 B per sample pair), s~ written and read back (2 x 2 x 16 B per
+    # pixel), p written (8 B per pixel)
+    n_pix = cfg.n_t * cfg.n_f
+    alg = 16.0 * n + 64.0 * n_pix + 8.0 * n_pix
+    return {"ms": ms, "n_t": cfg.n_t, "n_f": cfg.n_f, "seg_len": seg_len, "samples_per_detector": n,
+            "algorithmic_gb_per_s": alg / (ms * 1e-3) / 1e9, "launches": 3}
 
 
 def oracle_inputs(cfg):
@@ -341,6 +370,7 @@ def main():
     ap.add_argument("--maps", type=int, default=0, help="maps per batch step of config 4 (default: the config's 100)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "table", "rotation", "reinsch"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ftmap", action="store_true", help="also time st_set_map_from_strain on strain of the config's duration")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--ref-step-s", type=float, default=6.0, help="seconds of oracle work per reference step")
     args = ap.parse_args()
