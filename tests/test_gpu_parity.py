@@ -504,3 +504,29 @@ def test_full_size_background_batch_config4(P, orc):
         t = orc.track_params(seeds[m], res[m].arg_track, cfg.n_t, cfg.n_f, cfg.n_min, cfg.n_max)
         direct = orc.score_direct(p, t, orc.rasterise(t, cfg.n_f), cfg.f_min, cfg.df, tau[res[m].arg_tau_index])
         assert abs(direct - ref["max_snr"]) <= 1e-12 * abs(direct)
+
+
+def test_loudest_map_followup_combines_exactly(P, orc):
+    """the loudest maps of a run are followed up with a deeper search, and runs are
+    combined by taking the larger SNR_tot per map -- "results identical to a single search" with the
+    union of the template banks.  Batch run with T templates -> the 3 loudest maps get ids [T, 4T) ->
+    max(first, follow-up) == one search over [0, 4T), bit for bit; the oracle agrees on the deep result."""
+    import torch
+    cfg = synth.CONFIGS[1]
+    n_maps, T = 12, 500
+    csds = [synth.noise_csd(cfg.n_t, cfg.n_f, 900 + m) for m in range(n_maps)]
+    dev = [torch.from_numpy(c).cuda() for c in csds]
+    tau = synth.tau_linspace(cfg.n_tau)
+    st = make_ctx(P, cfg)
+    kw = dict(tau_grid=tau)
+    first, _ = st.search_batch(dev, None, 42, T, cfg.n_min, cfg.n_max, **kw)           # one shared bank
+    loud = sorted(range(n_maps), key=lambda m: -first[m].max_snr_f64)[:3]
+    deep, _ = st.search_batch([dev[m] for m in loud], None, 42, 3 * T, cfg.n_min, cfg.n_max, track_offset=T, **kw)
+    for m, d in zip(loud, deep):
+        best = max((first[m], d), key=lambda r: (r.max_snr_f64, -r.arg_track, -r.arg_tau_index))
+        st.set_map(dev[m])
+        whole = st.search(4 * T, 42, cfg.n_min, cfg.n_max, **kw)
+        assert (whole.max_snr_f64, whole.arg_track, whole.arg_tau_index) == (best.max_snr_f64, best.arg_track, best.arg_tau_index)
+        ref = orc.search(orc.prepare_map(csds[m]), cfg.f_min, cfg.df, 4 * T, 42, cfg.n_min, cfg.n_max, tau_grid=tau)
+        assert (ref["arg_track"], ref["arg_tau_index"]) == (whole.arg_track, whole.arg_tau_index)
+        assert abs(ref["max_snr"] - whole.max_snr_f64) <= 1e-11 * abs(ref["max_snr"])
