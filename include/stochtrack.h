@@ -150,7 +150,10 @@ int st_set_map_host(st_ctx *ctx, const void *csd_host, const float *sigma_host, 
 
 /* S1-S4 over the current map.  Fills *out (HOST) and params->hist_out (HOST).
  * Errors: ST_ESTATE (no workspace / map), ST_EINVAL, ST_ENOSPC (n_tau beyond the
- * workspace), ST_ECUDA.                                                        */
+ * workspace; in grid mode also an n_max whose pixel list, 10 bytes per column, does
+ * not fit one SM's shared memory: about 22 000 columns -- the random mode has no such
+ * limit), ST_ECUDA.  ST_KERNEL_AUTO never fails for lack of shared memory on a wide
+ * band: it falls back to the kernel whose per-bin table lives in L2.              */
 int st_search(st_ctx *ctx, const st_search_params *params, st_result *out);
 
 /* Batch / background mode (the background is estimated from many

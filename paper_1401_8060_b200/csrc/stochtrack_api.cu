@@ -248,6 +248,23 @@ struct Plan {
     double tau0, dtau;
 };
 
+// Shared memory a recurrence kernel needs with `warps` warps: histogram + per-bin tables + pixel pools.
+// AUTO only picks a kernel that keeps at least 4 warps per SM (wide bands: the per-bin tables of the
+// Chebyshev / Reinsch kernels outgrow shared memory, the rotation kernel then reads its table from L2).
+bool recur_fits(const st_ctx* c, int kernel, int n_bins, int n_max, int warps)
+{
+    const size_t stride = (size_t)((n_max + 63) & ~63);
+    const size_t hist = (size_t)((n_bins + 3) & ~3) * sizeof(uint32_t);
+    size_t need = hist;
+    if (kernel == ST_KERNEL_CHEBYSHEV)
+        need += (size_t)c->n_f * sizeof(float4) + (size_t)((c->n_f + 1) & ~1) * sizeof(float) + (size_t)warps * stride * 10;
+    else if (kernel == ST_KERNEL_REINSCH)
+        need += (size_t)(c->n_f + (c->n_f & 1)) * sizeof(float2) + (size_t)warps * (stride / 2) * 20;
+    else
+        need += (size_t)warps * stride * 10;
+    return need <= (size_t)c->smem_optin;
+}
+
 int make_plan(st_ctx* c, const st_search_params* p, Plan* plan)
 {
     plan->ch = 0; plan->tau0 = 0.0; plan->dtau = 0.0; plan->stride = 0;
@@ -256,8 +273,12 @@ int make_plan(st_ctx* c, const st_search_params* p, Plan* plan)
     int k = p->kernel;
     if (k == ST_KERNEL_AUTO) {
         if (!uni || p->n_tau < 8) k = ST_KERNEL_TABLE;
-        else if ((plan->stride = cheb_pick_stride(c, plan->dtau)) != 0) k = ST_KERNEL_CHEBYSHEV;
-        else k = reinsch_well_conditioned(c, plan->dtau) ? ST_KERNEL_REINSCH : ST_KERNEL_ROTATION;
+        else if (recur_fits(c, ST_KERNEL_CHEBYSHEV, p->n_bins, p->n_max, 4) &&
+                 (plan->stride = cheb_pick_stride(c, plan->dtau)) != 0) k = ST_KERNEL_CHEBYSHEV;
+        else if (recur_fits(c, ST_KERNEL_REINSCH, p->n_bins, p->n_max, 4) && reinsch_well_conditioned(c, plan->dtau))
+            k = ST_KERNEL_REINSCH;
+        else k = ST_KERNEL_ROTATION;
+        if (k != ST_KERNEL_TABLE) plan->stride = k == ST_KERNEL_CHEBYSHEV ? plan->stride : 0;
     }
     if (k == ST_KERNEL_CHEBYSHEV && plan->stride == 0) {
         if (uni) plan->stride = cheb_pick_stride(c, plan->dtau);

@@ -530,3 +530,35 @@ def test_loudest_map_followup_combines_exactly(P, orc):
         ref = orc.search(orc.prepare_map(csds[m]), cfg.f_min, cfg.df, 4 * T, 42, cfg.n_min, cfg.n_max, tau_grid=tau)
         assert (ref["arg_track"], ref["arg_tau_index"]) == (whole.arg_track, whole.arg_tau_index)
         assert abs(ref["max_snr"] - whole.max_snr_f64) <= 1e-11 * abs(ref["max_snr"])
+
+
+def test_wide_band_and_long_templates_limits(P, orc):
+    """Shapes beyond the five configs: a 30 000-bin band (the per-bin tables of the Chebyshev / Reinsch
+    kernels no longer fit shared memory: AUTO must fall back, not fail) and templates longer than a
+    shared-memory pixel list (grid mode: ST_ENOSPC as documented; random mode: no limit)."""
+    import torch
+    n_t, n_f = 48, 30000
+    csd = synth.noise_csd(n_t, n_f, 5)
+    st = P.Stochtrack(n_t, n_f, 0.25, 10.0, max_n_tau=64)
+    st.set_map(torch.from_numpy(csd).cuda())
+    tau = synth.tau_linspace(32, -2e-4, 2e-4)
+    r = st.search(3000, 9, 8, n_t, tau_grid=tau, n_bins=50)
+    assert r.kernel_name in ("rotation", "table")
+    ref = orc.search(orc.prepare_map(csd), 10.0, 0.25, 3000, 9, 8, n_t, tau_grid=tau, n_bins=50)
+    assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+    assert abs(r.max_snr_f64 - ref["max_snr"]) <= 1e-11 * abs(ref["max_snr"]) and int(r.hist.sum()) == 3000 * 32
+    n_t, n_f = 30000, 40
+    csd = synth.noise_csd(n_t, n_f, 6)
+    st = P.Stochtrack(n_t, n_f, 1.0, 40.0, max_n_tau=64)
+    st.set_map(torch.from_numpy(csd).cuda())
+    with pytest.raises(P.StError) as e:
+        st.search(100, 9, 10, n_t, tau_grid=synth.tau_linspace(16))
+    assert e.value.code == -3
+    r = st.search(400, 9, 10, n_t, tau_range=(-0.01, 0.01))
+    ref = orc.search(orc.prepare_map(csd), 40.0, 1.0, 400, 9, 10, n_t, tau_range=(-0.01, 0.01))
+    assert r.arg_track == ref["arg_track"] and abs(r.max_snr_f64 - ref["max_snr"]) <= 1e-11 * abs(ref["max_snr"])
+    # a long template that still fits: 20 000 columns
+    r = st.search(200, 9, 15000, 20000, tau_grid=synth.tau_linspace(16))
+    ref = orc.search(orc.prepare_map(csd), 40.0, 1.0, 200, 9, 15000, 20000, tau_grid=synth.tau_linspace(16))
+    assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+    assert abs(r.max_snr - ref["max_snr"]) <= 1e-4 * abs(ref["max_snr"])
