@@ -304,6 +304,63 @@ __global__ void k_l2_gather(const float2* __restrict__ buf, uint32_t n, float* o
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// ---- the inner loop of k_score_cheb (stride 2, two pixels per lane, 32 packed accumulators):
+// FORM 0: the recurrence as two scalar FFMAs on the halves of a register pair (round-1's first form);
+// FORM 1: one packed fma.rn.f32x2 with the coefficient as FFMA2's scalar-broadcast operand and the
+//         sign pattern ++-- (what the kernel uses now).  128 evaluations per lane per iteration.
+__device__ __forceinline__ f32x2_t mb_cheb_scalar(float g, f32x2_t cur, f32x2_t prev)
+{
+    f32x2_t r;
+    asm volatile("{\n\t.reg .f32 cl, ch, pl, ph;\n\tmov.b64 {cl, ch}, %2;\n\tmov.b64 {pl, ph}, %3;\n\t"
+                 "neg.f32 pl, pl;\n\tneg.f32 ph, ph;\n\tfma.rn.f32 pl, %1, cl, pl;\n\tfma.rn.f32 ph, %1, ch, ph;\n\t"
+                 "mov.b64 %0, {pl, ph};\n\t}" : "=l"(r) : "f"(g), "l"(cur), "l"(prev));
+    return r;
+}
+__device__ __forceinline__ f32x2_t mb_cheb_packed(float g, f32x2_t cur, f32x2_t prev)
+{
+    f32x2_t r;
+    asm volatile("{\n\t.reg .b64 gg;\n\tmov.b64 gg, {%1, %1};\n\tfma.rn.f32x2 %0, gg, %2, %3;\n\t}"
+                 : "=l"(r) : "f"(g), "l"(cur), "l"(prev));
+    return r;
+}
+template <int FORM>
+__global__ void __launch_bounds__(512, 1) k_cheb_loop(float* out, int iters, float g)
+{
+    f32x2_t f2[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) f2[i] = 0ull;
+    for (int it = 0; it < iters; ++it) {
+        const float GA = g + 1e-6f * (threadIdx.x + it), GB = g - 1e-6f * (threadIdx.x + it);
+        f32x2_t Ace = pk_make(1.f, .9f), Ape = pk_make(.8f, .95f), Aco = pk_make(.95f, .8f), Apo = pk_make(.9f, 1.f);
+        f32x2_t Bce = pk_make(.5f, .4f), Bpe = pk_make(.3f, .45f), Bco = pk_make(.45f, .3f), Bpo = pk_make(.4f, .5f);
+#pragma unroll
+        for (int i = 0; i < 32; i += 4) {
+            f2[i] = pk_add(f2[i], Ace); f2[i] = pk_add(f2[i], Bce);
+            f2[i + 1] = pk_add(f2[i + 1], Aco); f2[i + 1] = pk_add(f2[i + 1], Bco);
+            if (FORM == 0) {
+                Ape = mb_cheb_scalar(GA, Ace, Ape); Bpe = mb_cheb_scalar(GB, Bce, Bpe);
+                Apo = mb_cheb_scalar(GA, Aco, Apo); Bpo = mb_cheb_scalar(GB, Bco, Bpo);
+            } else {
+                Ape = mb_cheb_packed(GA, Ace, Ape); Bpe = mb_cheb_packed(GB, Bce, Bpe);
+                Apo = mb_cheb_packed(GA, Aco, Apo); Bpo = mb_cheb_packed(GB, Bco, Bpo);
+            }
+            f2[i + 2] = pk_add(f2[i + 2], Ape); f2[i + 2] = pk_add(f2[i + 2], Bpe);
+            f2[i + 3] = pk_add(f2[i + 3], Apo); f2[i + 3] = pk_add(f2[i + 3], Bpo);
+            if (FORM == 0) {
+                Ace = mb_cheb_scalar(GA, Ape, Ace); Bce = mb_cheb_scalar(GB, Bpe, Bce);
+                Aco = mb_cheb_scalar(GA, Apo, Aco); Bco = mb_cheb_scalar(GB, Bpo, Bco);
+            } else {
+                Ace = mb_cheb_packed(-GA, Ape, Ace); Bce = mb_cheb_packed(-GB, Bpe, Bce);
+                Aco = mb_cheb_packed(-GA, Apo, Aco); Bco = mb_cheb_packed(-GB, Bpo, Bco);
+            }
+        }
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < 32; ++i) s += pk_sum(f2[i]);
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 template <typename F>
 float time_ms(F launch, int reps = 5)
 {
@@ -405,6 +462,16 @@ int main()
         REPORT("lds64_random_gather", ms, 8.0 * kIters, "bytes");
         ms = time_ms([&] { k_lds_gather<16><<<blocks, threads, 2461 * 16>>>(out, 2461); });
         REPORT("lds128_random_gather", ms, 16.0 * kIters, "bytes");
+    }
+    for (int thr = 256; thr <= 512; thr += 256) {
+        const int iters = 20000;
+        for (int form = 0; form < 2; ++form) {
+            const float ms = form == 0 ? time_ms([&] { k_cheb_loop<0><<<n_sm, thr>>>(out, iters, 1.9f); })
+                                       : time_ms([&] { k_cheb_loop<1><<<n_sm, thr>>>(out, iters, 1.9f); });
+            printf("{\"bench\": \"cheb_loop_%s_%dw\", \"ms\": %.4f, \"per_clk_per_sm_at_max_clock\": %.2f, \"unit\": \"evals (1 FMA + 1 add each; 64 = FP32 pipe)\"}\n",
+                   form == 0 ? "scalar_ffma" : "packed_ffma2", thr / 32, ms,
+                   (double)n_sm * thr * iters * 128.0 / (ms * 1e-3) / (n_sm * ghz * 1e9));
+        }
     }
     {
         const uint32_t n = 2461u * 1000u;                 // config-5 map: 19.7 MB, L2 resident
