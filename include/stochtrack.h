@@ -201,6 +201,17 @@ typedef struct {
 size_t st_ftmap_scratch_bytes(const st_ctx *ctx, int32_t seg_len);
 int st_set_map_from_strain(st_ctx *ctx, const double *s_i_dev, const double *s_j_dev, int64_t n_samples,
                            const st_ftmap_params *params, void *scratch_dev, size_t scratch_bytes);
+/* Time-shift background from strain (significance from n_ts time-shift analyses; reading
+ * G23): the strain spectrograms are computed ONCE; for each shifts[m] (HOST, whole segments, 0 <= shift <
+ * n_t, cyclic over the map) detector J's segment (j + shift) mod n_t is paired with detector I's segment j,
+ * P' of each detector taken around its own segment, and the resulting map is searched with seeds[m]
+ * (HOST, or NULL: params->seed for every shift).  Per-shift results and histograms as st_search_batch
+ * (results HOST [n_shifts], params->hist_out HOST [n_shifts][n_bins], no host synchronisation inside a
+ * group of ST_BATCH_GROUP shifts).  On return the context's map is that of the last shift.             */
+int st_search_timeshifts(st_ctx *ctx, const double *s_i_dev, const double *s_j_dev, int64_t n_samples,
+                         const st_ftmap_params *ft_params, void *scratch_dev, size_t scratch_bytes,
+                         int32_t n_shifts, const int32_t *shifts, const uint64_t *seeds,
+                         const st_search_params *params, st_result *results, float *gpu_ms_total);
 /* Parity export: copy the context's current map p (complex64 [n_t][n_f]) to p_out_dev (DEVICE).   */
 int st_debug_get_map(st_ctx *ctx, void *p_out_dev);
 

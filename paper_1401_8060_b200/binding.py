@@ -19,7 +19,8 @@ KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random",
 
 # every symbol include/stochtrack.h declares
 exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_workspace", "st_set_map",
-                    "st_set_map_host", "st_search", "st_search_batch", "st_ftmap_scratch_bytes", "st_set_map_from_strain", "st_debug_get_map",
+                    "st_set_map_host", "st_search", "st_search_batch", "st_ftmap_scratch_bytes", "st_set_map_from_strain", "st_search_timeshifts",
+                    "st_debug_get_map",
                     "st_track_params", "st_debug_rasterise",
                     "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words",
                     "st_last_error", "st_version")
@@ -107,6 +108,10 @@ def load_library():
     L.st_ftmap_scratch_bytes.restype = C.c_size_t
     L.st_set_map_from_strain.argtypes = [vp, vp, vp, C.c_int64, C.POINTER(CFtmapParams), vp, C.c_size_t]
     L.st_set_map_from_strain.restype = C.c_int
+    L.st_search_timeshifts.argtypes = [vp, vp, vp, C.c_int64, C.POINTER(CFtmapParams), vp, C.c_size_t, C.c_int32,
+                                       C.POINTER(C.c_int32), C.POINTER(C.c_uint64), C.POINTER(CSearchParams),
+                                       C.POINTER(CResult), C.POINTER(C.c_float)]
+    L.st_search_timeshifts.restype = C.c_int
     L.st_debug_get_map.argtypes = [vp, vp]
     L.st_debug_get_map.restype = C.c_int
     L.st_search_batch.argtypes = [vp, C.POINTER(CBatch), C.POINTER(CSearchParams), C.POINTER(CResult), C.POINTER(C.c_float)]
@@ -221,6 +226,49 @@ class Stochtrack:
         self._check(self._L.st_set_map_from_strain(self._ctx, s_i.data_ptr(), s_j.data_ptr(), s_i.numel(), C.byref(fp),
                                                    self._ft_scratch.data_ptr(), self._ft_scratch.numel()))
         self._keep = [s_i, s_j]
+
+    def _ft_args(self, s_i, s_j, seg_len):
+        torch = self._torch
+        for x in (s_i, s_j):
+            if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == torch.float64 and x.is_contiguous() and x.dim() == 1):
+                raise ValueError("strain series must be contiguous 1-D float64 CUDA tensors")
+        if s_i.numel() != s_j.numel():
+            raise ValueError("the two strain series must have the same length")
+        need = self._L.st_ftmap_scratch_bytes(self._ctx, int(seg_len))
+        if need == 0:
+            raise StError(ST_EINVAL, "st_ftmap_scratch_bytes: bad seg_len")
+        if getattr(self, "_ft_scratch", None) is None or self._ft_scratch.numel() < need:
+            self._ft_scratch = torch.empty(need, dtype=torch.uint8, device=self.device)
+
+    def search_timeshifts(self, s_i, s_j, fs, seg_len, n_neighbours, shifts, seeds, n_tracks, n_min, n_max,
+                          tau_grid=None, tau_range=None, norm=NORM_SQRT_N, n_bins=0, hist_lo=-10.0, hist_hi=10.0,
+                          track_offset=0, kernel=KERNEL_AUTO):
+        """Time-shift background from strain (st_search_timeshifts): spectrograms once, one map and one
+        search per whole-segment shift of detector J.  Returns (list of SearchResult, gpu_ms_total)."""
+        self._ft_args(s_i, s_j, seg_len)
+        sh = np.ascontiguousarray(shifts, dtype=np.int32)
+        n = sh.size
+        fp = CFtmapParams(float(fs), int(seg_len), int(n_neighbours))
+        seed0, sd_p = 0, None
+        if np.ndim(seeds) == 0:
+            seed0 = int(seeds)
+        else:
+            sd = np.ascontiguousarray(seeds, dtype=np.uint64)
+            if sd.size != n:
+                raise ValueError("seeds: one per shift")
+            sd_p = sd.ctypes.data_as(C.POINTER(C.c_uint64))
+        p, keep = self._params(n_tracks, seed0, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
+                               track_offset, kernel)
+        hist = None
+        if n_bins > 0:
+            hist = np.zeros((n, n_bins), dtype=np.uint64)
+            p.hist_out = hist.ctypes.data_as(C.POINTER(C.c_uint64))
+        res = (CResult * n)()
+        ms = C.c_float(0.0)
+        self._check(self._L.st_search_timeshifts(self._ctx, s_i.data_ptr(), s_j.data_ptr(), s_i.numel(), C.byref(fp),
+                                                 self._ft_scratch.data_ptr(), self._ft_scratch.numel(), n,
+                                                 sh.ctypes.data_as(C.POINTER(C.c_int32)), sd_p, C.byref(p), res, C.byref(ms)))
+        return [self._result(res[m], hist[m] if hist is not None else None) for m in range(n)], float(ms.value)
 
     def debug_get_map(self):
         """The context's current map p as a complex64 numpy array [n_t][n_f] (parity export)."""

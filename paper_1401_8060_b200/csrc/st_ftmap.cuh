@@ -76,30 +76,38 @@ k_ft_segments(const double* __restrict__ s_i, const double* __restrict__ s_j, in
 }
 
 // P'(t_j; f) = mean |s~|^2 over j' = j +- 2 .. j +- (n_nb + 1) inside the map (G20); masked pixels -> 0.
+// `shift` (time-shifted background maps, G23): detector J's segment js = (j + shift) mod n_t meets
+// detector I's segment j; each detector's P' comes from the neighbours of ITS OWN segment.
 __global__ void __launch_bounds__(256)
 k_ft_normalise(const double2* __restrict__ st_i, const double2* __restrict__ st_j, int n_t, int n_f, int n_nb,
-               float2* __restrict__ p)
+               int shift, float2* __restrict__ p)
 {
     const size_t n_pix = (size_t)n_t * (size_t)n_f;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_pix; i += (size_t)gridDim.x * blockDim.x) {
         const int j = (int)(i / (size_t)n_f), q = (int)(i % (size_t)n_f);
+        const int js = (j + shift) % n_t;
         double pi = 0.0, pj = 0.0;
-        int cnt = 0;
+        int ci = 0, cj = 0;
         for (int d = 2; d <= n_nb + 1; ++d) {
             for (int sgn = -1; sgn <= 1; sgn += 2) {
-                const int jj = j + sgn * d;
-                if (jj < 0 || jj >= n_t) continue;
-                const double2 a = st_i[(size_t)jj * n_f + q], b = st_j[(size_t)jj * n_f + q];
-                pi += a.x * a.x + a.y * a.y;
-                pj += b.x * b.x + b.y * b.y;
-                ++cnt;
+                const int ji = j + sgn * d, jj = js + sgn * d;
+                if (ji >= 0 && ji < n_t) {
+                    const double2 a = st_i[(size_t)ji * n_f + q];
+                    pi += a.x * a.x + a.y * a.y;
+                    ++ci;
+                }
+                if (jj >= 0 && jj < n_t) {
+                    const double2 b = st_j[(size_t)jj * n_f + q];
+                    pj += b.x * b.x + b.y * b.y;
+                    ++cj;
+                }
             }
         }
         float2 out = make_float2(0.0f, 0.0f);
-        if (cnt > 0) {
-            const double prod = (pi / (double)cnt) * (pj / (double)cnt);
+        if (ci > 0 && cj > 0) {
+            const double prod = (pi / (double)ci) * (pj / (double)cj);
             if (prod > 0.0 && isfinite(prod)) {
-                const double2 a = st_i[i], b = st_j[i];
+                const double2 a = st_i[i], b = st_j[(size_t)js * n_f + q];
                 const double sc = sqrt(2.0) / sqrt(prod);                           // G21
                 // conj(a) * b
                 out = make_float2((float)(sc * (a.x * b.x + a.y * b.y)), (float)(sc * (a.x * b.y - a.y * b.x)));

@@ -841,10 +841,11 @@ size_t st_ftmap_scratch_bytes(const st_ctx* c, int32_t seg_len)
     return 2 * align_up(n_pix * sizeof(double2)) + align_up((size_t)(seg_len / 2) * sizeof(double2));
 }
 
-int st_set_map_from_strain(st_ctx* c, const double* s_i, const double* s_j, int64_t n_samples,
-                           const st_ftmap_params* fp, void* scratch, size_t scratch_bytes)
+// F1 + F2 of the ft-map construction: validation, twiddles, one FFT per segment.  On success the
+// scratch holds s~_I, s~_J; k_ft_normalise (any shift) can follow.
+static int ft_spectra(st_ctx* c, const double* s_i, const double* s_j, int64_t n_samples, const st_ftmap_params* fp,
+                      void* scratch, size_t scratch_bytes, double2** st_i_out, double2** st_j_out)
 {
-    if (!c) return ST_EINVAL;
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
     if (!s_i || !s_j || !fp || !scratch) return fail(c, ST_EINVAL, "NULL argument");
     const int L = fp->seg_len;
@@ -873,10 +874,93 @@ int st_set_map_from_strain(st_ctx* c, const double* s_i, const double* s_j, int6
     if (rc) return rc;
     st::k_ft_segments<<<c->n_t, st::kFtThreads, smem, c->stream>>>(s_i, s_j, L, log2L, W, k_lo, c->n_f, st_i, st_j);
     ST_CUDA(c, cudaGetLastError());
+    *st_i_out = st_i; *st_j_out = st_j;
+    return ST_OK;
+}
+
+// F3 + F4 for one time shift (0 = the zero-lag map) into the context's map.
+static int ft_normalise(st_ctx* c, const double2* st_i, const double2* st_j, int n_nb, int shift)
+{
+    const size_t n_pix = (size_t)c->n_t * (size_t)c->n_f;
     const int blocks = (int)((n_pix + 255) / 256 < (size_t)(8 * c->n_sm) ? (n_pix + 255) / 256 : (size_t)(8 * c->n_sm));
-    st::k_ft_normalise<<<blocks, 256, 0, c->stream>>>(st_i, st_j, c->n_t, c->n_f, fp->n_neighbours, at<float2>(c, c->L.map));
+    st::k_ft_normalise<<<blocks, 256, 0, c->stream>>>(st_i, st_j, c->n_t, c->n_f, n_nb, shift, at<float2>(c, c->L.map));
     ST_CUDA(c, cudaGetLastError());
     c->have_map = true;
+    return ST_OK;
+}
+
+int st_set_map_from_strain(st_ctx* c, const double* s_i, const double* s_j, int64_t n_samples,
+                           const st_ftmap_params* fp, void* scratch, size_t scratch_bytes)
+{
+    if (!c) return ST_EINVAL;
+    double2 *st_i = nullptr, *st_j = nullptr;
+    int rc = ft_spectra(c, s_i, s_j, n_samples, fp, scratch, scratch_bytes, &st_i, &st_j);
+    if (rc) return rc;
+    return ft_normalise(c, st_i, st_j, fp->n_neighbours, 0);
+}
+
+int st_search_timeshifts(st_ctx* c, const double* s_i, const double* s_j, int64_t n_samples, const st_ftmap_params* fp,
+                         void* scratch, size_t scratch_bytes, int32_t n_shifts, const int32_t* shifts,
+                         const uint64_t* seeds, const st_search_params* p, st_result* results, float* gpu_ms_total)
+{
+    int rc = validate(c, p, false);
+    if (rc) return rc;
+    if (!results || !shifts) return fail(c, ST_EINVAL, "shifts / results is NULL");
+    if (n_shifts < 1) return fail(c, ST_EINVAL, "n_shifts must be >= 1");
+    for (int m = 0; m < n_shifts; ++m)
+        if (shifts[m] < 0 || shifts[m] >= c->n_t) return fail(c, ST_EINVAL, "shifts[%d] = %d outside [0, n_t)", m, shifts[m]);
+    if (p->n_bins > 0 && !p->hist_out) return fail(c, ST_EINVAL, "n_bins > 0 but hist_out is NULL");
+    Plan plan;
+    rc = make_plan(c, p, &plan);
+    if (rc) return rc;
+    const int n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
+    if (gpu_ms_total) *gpu_ms_total = 0.0f;
+    memset(results, 0, sizeof(st_result) * (size_t)n_shifts);
+    if (!c->h_bres) ST_CUDA(c, cudaHostAlloc((void**)&c->h_bres, (size_t)ST_BATCH_GROUP * sizeof(st::DeviceResult), cudaHostAllocDefault));
+    if (p->n_bins > 0 && !c->h_bhist)
+        ST_CUDA(c, cudaHostAlloc((void**)&c->h_bhist, (size_t)ST_BATCH_GROUP * ST_MAX_BINS * sizeof(unsigned long long), cudaHostAllocDefault));
+    ST_CUDA(c, cudaEventRecord(c->ev0, c->stream));
+    double2 *st_i = nullptr, *st_j = nullptr;
+    rc = ft_spectra(c, s_i, s_j, n_samples, fp, scratch, scratch_bytes, &st_i, &st_j);      // once for every shift
+    if (rc) return rc;
+    if (p->n_tracks == 0) {
+        for (int m = 0; m < n_shifts; ++m) {
+            results[m].kernel_used = plan.kernel; results[m].max_snr = -INFINITY; results[m].max_snr_f64 = -INFINITY;
+        }
+        if (p->n_bins > 0) memset(p->hist_out, 0, sizeof(uint64_t) * (size_t)p->n_bins * (size_t)n_shifts);
+        return ft_normalise(c, st_i, st_j, fp->n_neighbours, shifts[n_shifts - 1]);
+    }
+    int n_launches_tables = 2;                        // k_ft_twiddles, k_ft_segments
+    rc = ensure_tables(c, p, plan, &n_launches_tables);
+    if (rc) return rc;
+    st_search_params pm = *p;
+    for (int g0 = 0; g0 < n_shifts; g0 += ST_BATCH_GROUP) {
+        const int g1 = g0 + ST_BATCH_GROUP < n_shifts ? g0 + ST_BATCH_GROUP : n_shifts;
+        std::vector<int> launches((size_t)(g1 - g0), 0);
+        for (int m = g0; m < g1; ++m) {
+            rc = ft_normalise(c, st_i, st_j, fp->n_neighbours, shifts[m]);
+            if (rc) return rc;
+            pm.seed = seeds ? seeds[m] : p->seed;
+            int nl = 1;                               // k_ft_normalise
+            rc = enqueue_search(c, &pm, plan, batch_slots(c, m - g0), &nl, false);
+            if (rc) return rc;
+            launches[(size_t)(m - g0)] = nl;
+        }
+        ST_CUDA(c, cudaMemcpyAsync(c->h_bres, at<void>(c, c->L.b_result), (size_t)(g1 - g0) * sizeof(st::DeviceResult),
+                                   cudaMemcpyDeviceToHost, c->stream));
+        if (p->n_bins > 0)
+            ST_CUDA(c, cudaMemcpyAsync(c->h_bhist, at<void>(c, c->L.b_hist),
+                                       (size_t)(g1 - g0) * ST_MAX_BINS * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+        if (g1 == n_shifts) ST_CUDA(c, cudaEventRecord(c->ev1, c->stream));
+        ST_CUDA(c, cudaStreamSynchronize(c->stream));
+        for (int m = g0; m < g1; ++m) {
+            fill_result(&results[m], c->h_bres[m - g0], n_tau, plan.kernel, launches[(size_t)(m - g0)] + (m == 0 ? n_launches_tables : 0));
+            if (p->n_bins > 0)
+                for (int k = 0; k < p->n_bins; ++k)
+                    p->hist_out[(size_t)m * (size_t)p->n_bins + (size_t)k] = (uint64_t)c->h_bhist[(size_t)(m - g0) * ST_MAX_BINS + (size_t)k];
+        }
+    }
+    if (gpu_ms_total) ST_CUDA(c, cudaEventElapsedTime(gpu_ms_total, c->ev0, c->ev1));
     return ST_OK;
 }
 

@@ -95,3 +95,45 @@ def test_ftmap_argument_errors(P):
             st.set_map_from_strain(s, s, **kw)
     with pytest.raises(P.StError):
         st.set_map_from_strain(s[:1000], s[:1000], 1024.0, 1024)   # too few samples
+
+
+def test_timeshift_background_from_strain(P, orc):
+    """st_search_timeshifts: spectrograms once, one (map, search) per whole-segment shift (G23).  Every
+    shift's map equals the oracle's ftmap_timeshift, its search equals the search oracle on that map; the
+    zero-lag entry finds the injected chirp, the shifted ones do not (the time-shift background)."""
+    import torch
+    rng = np.random.default_rng(33)
+    fs, L, n_t, n_f, f_min, n_nb = 1024.0, 1024, 64, 200, 100.0, 6
+    n = (n_t + 1) * L // 2
+    t = np.arange(n) / fs
+    tau0 = -2e-3
+    env = ((t > 4.0) & (t < 28.0)).astype(float)
+    phase = lambda x: 2 * np.pi * (150.0 * x + 1.25 * x ** 2)
+    s_i = rng.standard_normal(n) + 0.8 * env * np.cos(phase(t))
+    s_j = rng.standard_normal(n) + 0.8 * env * np.cos(phase(t - tau0))
+    shifts = [0, 1, 7, 31, 63]
+    seeds = [5, 6, 7, 8, 9]
+    tau = synth.tau_linspace(41, -0.01, 0.01)
+    st = P.Stochtrack(n_t, n_f, fs / L, f_min, max_n_tau=64)
+    res, ms = st.search_timeshifts(torch.from_numpy(s_i).cuda(), torch.from_numpy(s_j).cuda(), fs, L, n_nb, shifts, seeds,
+                                   8000, 20, 64, tau_grid=tau, n_bins=100)
+    assert len(res) == len(shifts) and ms > 0
+    _, r_i, r_j, _, _ = F.ftmap(s_i, s_j, fs, L, n_t, f_min, n_f, n_nb)
+    last = st.debug_get_map()                                     # the context keeps the last shift's map
+    ref_last = F.ftmap_timeshift(r_i, r_j, n_nb, shifts[-1])
+    assert np.all(np.abs(last - ref_last) <= 2e-6 * np.maximum(np.abs(ref_last), 1.0))
+    for m, (sh, sd) in enumerate(zip(shifts, seeds)):
+        pm = F.ftmap_timeshift(r_i, r_j, n_nb, sh)
+        ref = orc.search(pm, f_min, fs / L, 8000, sd, 20, 64, tau_grid=tau, n_bins=100)
+        # float32 map on the device vs float64 map in the oracle: same argmax unless a near tie (none here)
+        assert (res[m].arg_track, res[m].arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"]), m
+        assert abs(res[m].max_snr_f64 - ref["max_snr"]) <= 1e-5 * abs(ref["max_snr"])
+        assert int(res[m].hist.sum()) == 8000 * 41
+    assert res[0].max_snr_f64 > 8.0 and abs(res[0].arg_tau - tau0) <= 1e-3
+    assert max(r.max_snr_f64 for r in res[1:]) < 0.75 * res[0].max_snr_f64
+    # shift 0 of the batch call == st_set_map_from_strain + st_search, bit for bit
+    st.set_map_from_strain(torch.from_numpy(s_i).cuda(), torch.from_numpy(s_j).cuda(), fs, L, n_nb)
+    one = st.search(8000, seeds[0], 20, 64, tau_grid=tau, n_bins=100)
+    assert (one.max_snr_f64, one.arg_track, one.arg_tau_index) == (res[0].max_snr_f64, res[0].arg_track, res[0].arg_tau_index)
+    with pytest.raises(P.StError):
+        st.search_timeshifts(torch.from_numpy(s_i).cuda(), torch.from_numpy(s_j).cuda(), fs, L, n_nb, [n_t], 1, 10, 20, 64, tau_grid=tau)

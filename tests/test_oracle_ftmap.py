@@ -120,3 +120,33 @@ def test_F_ftmap_feeds_the_search_oracle(orc):
     tau = synth.tau_linspace(41, -0.01, 0.01)
     r = orc.search(p, f_min, fs / L, 20000, 3, 30, 64, tau_grid=tau)
     assert r["max_snr"] > 8.0 and abs(r["arg_tau"] - tau0) <= 1.0e-3
+
+
+def test_F_timeshift_zero_is_identity_and_shift_destroys_coherence():
+    """G23: shift 0 reproduces the unshifted map; a whole-segment shift of detector J leaves the noise
+    statistics unchanged but removes a transient that is coherent between the detectors (the point of
+    a time-shift background); shifting by n_t is the identity (cyclic)."""
+    rng = np.random.default_rng(8)
+    fs, L, n_t, n_f = 256.0, 256, 60, 80
+    n = int(L / 2 * (n_t + 1))
+    t = np.arange(n) / fs
+    env = ((t > 10.0) & (t < 14.0)).astype(float)
+    h = 1.2 * env * np.cos(2 * np.pi * (50.0 * t + 1.5 * (t - 10.0) ** 2))       # a 4 s chirp, 50 -> 62 Hz
+    s_i, s_j = rng.standard_normal(n) + h, rng.standard_normal(n) + h
+    p, st_i, st_j, _, _ = F.ftmap(s_i, s_j, fs, L, n_t, 20.0, n_f, 6)
+    assert np.array_equal(F.ftmap_timeshift(st_i, st_j, 6, 0), p)
+    assert np.array_equal(F.ftmap_timeshift(st_i, st_j, 6, n_t), p)
+    rows, band = slice(20, 27), slice(28, 44)              # the pixels the chirp crosses
+    n_box = 7 * 16
+    assert np.real(p[rows, band]).sum() > 5.0 * np.sqrt(n_box)            # coherent: +829 measured, noise rms ~11
+    for s in (3, 17, 31):
+        shifted = F.ftmap_timeshift(st_i, st_j, 6, s)
+        assert abs(np.real(shifted[rows, band]).sum()) < 4.0 * np.sqrt(n_box)
+        assert 0.9 < np.real(shifted[10:-10, 60:80]).var() < 1.3         # noise statistics unchanged
+    # pairing rule, spelled out on one pixel
+    shifted = F.ftmap_timeshift(st_i, st_j, 6, 17)
+    j, q, s = 20, 5, 17
+    P_i, _ = F.neighbour_power(st_i, 6)
+    P_j, _ = F.neighbour_power(st_j, 6)
+    want = np.sqrt(2) * np.conj(st_i[j, q]) * st_j[(j + s) % n_t, q] / np.sqrt(P_i[j, q] * P_j[(j + s) % n_t, q])
+    assert shifted[j, q] == pytest.approx(want, rel=1e-14)
