@@ -35,7 +35,7 @@ __device__ __forceinline__ double2 cmul(double2 a, double2 b)
 }
 
 // One CTA per segment j: samples [j L/2, j L/2 + L).  In-place radix-2 decimation-in-frequency FFT
-// (Gentleman-Sande): log2 L passes of L/2 butterflies, output in bit-reversed order.  With
+// (Gentleman-Sande), two stages per pass over shared memory, output in bit-reversed order.  With
 // z = w (s_I + i s_J):  s~_I(k) = (Z_k + conj Z_{L-k}) / 2,  s~_J(k) = (Z_k - conj Z_{L-k}) / (2 i).
 __global__ void __launch_bounds__(kFtThreads, 1)
 k_ft_segments(const double* __restrict__ s_i, const double* __restrict__ s_j, int L, int log2L,
@@ -47,13 +47,34 @@ k_ft_segments(const double* __restrict__ s_i, const double* __restrict__ s_j, in
     const int j = blockIdx.x;
     const size_t base = (size_t)j * (size_t)(L / 2);
     for (int n = threadIdx.x; n < L; n += blockDim.x) {
-        double sn, cs;
-        sincospi(2.0 * (double)n / (double)L, &sn, &cs);
-        const double w = 0.5 * (1.0 - cs);                       // Hann (G19)
+        // Hann (G19): cos(2 pi n / L) from the twiddle table (W[t].x = cos(2 pi t / L), t < L/2)
+        const double cs = n < L / 2 ? W[n].x : (n == L / 2 ? -1.0 : W[L - n].x);
+        const double w = 0.5 * (1.0 - cs);
         x[n] = make_double2(w * s_i[base + n], w * s_j[base + n]);
     }
     __syncthreads();
-    for (int s = 0; s < log2L; ++s) {
+    // two radix-2 stages per pass, fused in registers (the arithmetic and the bit-reversed output order
+    // are those of plain radix-2; shared-memory traffic and barriers are halved)
+    int s = 0;
+    for (; s + 2 <= log2L; s += 2) {
+        const int half = L >> (s + 1), quarter = half >> 1;
+        for (int b = threadIdx.x; b < L / 4; b += blockDim.x) {
+            const int pos = b & (quarter - 1);
+            const int i0 = ((b - pos) << 2) + pos, i1 = i0 + quarter, i2 = i0 + half, i3 = i2 + quarter;
+            const double2 x0 = x[i0], x1 = x[i1], x2 = x[i2], x3 = x[i3];
+            const double2 u0 = make_double2(x0.x + x2.x, x0.y + x2.y);
+            const double2 u1 = make_double2(x1.x + x3.x, x1.y + x3.y);
+            const double2 u2 = cmul(make_double2(x0.x - x2.x, x0.y - x2.y), W[(size_t)pos << s]);
+            const double2 u3 = cmul(make_double2(x1.x - x3.x, x1.y - x3.y), W[(size_t)(pos + quarter) << s]);
+            const double2 w1 = W[(size_t)pos << (s + 1)];
+            x[i0] = make_double2(u0.x + u1.x, u0.y + u1.y);
+            x[i1] = cmul(make_double2(u0.x - u1.x, u0.y - u1.y), w1);
+            x[i2] = make_double2(u2.x + u3.x, u2.y + u3.y);
+            x[i3] = cmul(make_double2(u2.x - u3.x, u2.y - u3.y), w1);
+        }
+        __syncthreads();
+    }
+    for (; s < log2L; ++s) {                                     // odd log2 L: one plain radix-2 stage
         const int half = L >> (s + 1);
         for (int b = threadIdx.x; b < L / 2; b += blockDim.x) {
             const int pos = b & (half - 1);
