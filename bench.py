@@ -38,6 +38,10 @@ DRAM_TRAFFIC_BYTES_PER_LAUNCH = {5: 19.87e6, 3: 9.88e6}
 L2_GATHER_PEAK_GBS = 9200.0          # random 32-byte sector gathers, measured (profiles/microbench_r01.md)
 
 
+def workload_tag(config):
+    return "the paper's Table III shape (PAPER.md:207-212, context)" if config == "P" else f"BASELINE.json configs[{config - 1}]"
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     sm_mhz, src = 1965.0, "fallback clock 1965 MHz"
@@ -230,7 +234,7 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({cfg.name}): {cfg.n_t}x{cfg.n_f} map, "
+        "config": {"workload": f"{workload_tag(args.config)} ({cfg.name}): {cfg.n_t}x{cfg.n_f} map, "
                                f"{n_tracks:.0e} templates per GPU" + (f" per map x {n_maps} maps in one st_search_batch call" if n_maps > 1 else "") +
                                f", {n_tau} delays ({cfg.tau_mode})",
                    "n_t": cfg.n_t, "n_f": cfg.n_f, "n_tracks_per_gpu": n_tracks, "n_tau": n_tau,
@@ -351,7 +355,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({cfg.name}): {cfg.n_t}x{cfg.n_f} map, "
+        "config": {"workload": f"{workload_tag(args.config)} ({cfg.name}): {cfg.n_t}x{cfg.n_f} map, "
                                f"{n_tau} delays ({cfg.tau_mode}); bounded sample of {n} templates per step",
                    "n_t": cfg.n_t, "n_f": cfg.n_f, "n_tau": n_tau, "tau_mode": cfg.tau_mode},
         "cpu_baseline": {"value": value, "unit": UNIT, "kind": "oracle", "cores": r["threads_used"], "sample": sample},
@@ -365,7 +369,8 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", default="5", choices=["1", "2", "3", "4", "5", "P"],
+                    help="BASELINE.json config (1-5) or P: the shape of the paper's own timing, Table III (context)")
     ap.add_argument("--tracks", type=int, default=0, help="override templates per GPU (debugging)")
     ap.add_argument("--maps", type=int, default=0, help="maps per batch step of config 4 (default: the config's 100)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "table", "rotation", "reinsch"])
@@ -374,6 +379,7 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--ref-step-s", type=float, default=6.0, help="seconds of oracle work per reference step")
     args = ap.parse_args()
+    args.config = "P" if args.config == "P" else int(args.config)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = max(args.warmup, 1)
     if args.impl == "reference":
