@@ -48,6 +48,18 @@ def test_rasteriser_indices_bit_exact(P, orc, cid, first, count):
     assert (N >= cfg.n_min).all() and (N <= cfg.n_max).all()
 
 
+@pytest.mark.parametrize("n_t,n_f,n_min,n_max,count", [(64, 65535, 1, 64, 60000), (4096, 2461, 3000, 4096, 600),
+                                                        (16, 7, 1, 16, 20000)])
+def test_rasteriser_indices_bit_exact_extreme_shapes(P, orc, n_t, n_f, n_min, n_max, count):
+    """The fast path's guard (max(1e-6, 4e-11 n_f) bins from an edge -> normative sequence) must hold at the
+    widest band the ABI allows, on long templates and on a tiny map: indices equal the oracle's, bit for bit."""
+    st = P.Stochtrack(n_t, n_f, 1.0, 0.0, max_n_tau=64)
+    k, j0, N = st.debug_rasterise(77, n_min, n_max, 10 ** 12, count)
+    p = np.zeros((n_t, n_f), dtype=np.complex128)
+    ref = orc.search(p, 0.0, 1.0, count, 77, n_min, n_max, tau_grid=np.zeros(1), track_offset=10 ** 12, dump_tracks=True)
+    assert np.array_equal(N, ref["N"]) and np.array_equal(j0, ref["j0"]) and np.array_equal(k, ref["k"])
+
+
 def test_rasteriser_explicit_tracks(P, orc):
     """Injection tracks of SURVEY 8(d) and the degenerate shapes: flat, straight, a -> 0, a -> N."""
     cfg = synth.CONFIGS[5]
