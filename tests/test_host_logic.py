@@ -78,6 +78,18 @@ def test_create_validates_arguments(lib):
         assert b"workspace" in lib.st_last_error(ctx)
         assert lib.st_set_map(ctx, 0, 0, 0) == binding.ST_ESTATE
         assert lib.st_set_workspace(ctx, 0, 1 << 30, 0) == binding.ST_EINVAL
+        # the batch / ft-map / time-shift entry points: same rule (state error before any CUDA call)
+        b = binding.CBatch()
+        b.n_maps = 1
+        res = (binding.CResult * 1)()
+        assert lib.st_search_batch(ctx, C.byref(b), C.byref(p), res, None) == binding.ST_ESTATE
+        fp = binding.CFtmapParams(8192.0, 8192, 4)
+        assert lib.st_set_map_from_strain(ctx, 1, 1, 10 ** 7, C.byref(fp), 1, 1 << 30) == binding.ST_ESTATE
+        sh = (C.c_int32 * 1)(0)
+        assert lib.st_search_timeshifts(ctx, 1, 1, 10 ** 7, C.byref(fp), 1, 1 << 30, 1, sh, None, C.byref(p), res, None) == binding.ST_ESTATE
+        assert lib.st_debug_get_map(ctx, 1) == binding.ST_ESTATE
+        assert lib.st_ftmap_scratch_bytes(ctx, 8192) >= 2 * 1000 * 2461 * 16 + 4096 * 16
+        assert lib.st_ftmap_scratch_bytes(ctx, 1000) == 0 and lib.st_ftmap_scratch_bytes(ctx, 16384) == 0
         t = binding.CTrack()
         assert lib.st_track_params(ctx, 0, 0, 10, 1001, 0.0, 0.0, C.byref(t)) == binding.ST_EINVAL
         assert lib.st_track_params(ctx, 0, 0, 0, 10, 0.0, 0.0, C.byref(t)) == binding.ST_EINVAL
