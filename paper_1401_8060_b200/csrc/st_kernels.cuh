@@ -678,7 +678,6 @@ __device__ __forceinline__ float pk_sum(f32x2_t a)
 constexpr int kChunk = 32;        // delays per accumulator chunk
 constexpr int kSuper = 256;       // delays between re-anchoring (8 chunks)
 
-template <int VAR>
 __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -695,10 +694,6 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
     for (int k = threadIdx.x; k < a.bp.n_f; k += blockDim.x) sm_kz[k] = a.kz[k];
     hist_init(sm_hist, a.n_bins);
     const float* sm_negk = reinterpret_cast<const float*>(sm_kz);     // sm_negk[2k] = -kappa_k
-#ifdef ST_EXP_NOANCHOR
-    for (int e = lane; e < P; e += kWarp) { pool_x[e] = 0ull; pool_d[e] = 0ull; pool_k[e] = 0u; }
-    __syncwarp();
-#endif
     const int n_chunks = (a.n_tau + kChunk - 1) / kChunk;
     WarpReduce wr;
     reduce_init(wr);
@@ -713,19 +708,11 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
         const float scale = norm_scale(t.N, a.norm);
 #pragma unroll 1
         for (int j = 0; j < n_chunks; ++j) {
-#ifdef ST_EXP_ONEANCHOR
-            if (j == 0) {
-#else
             if ((j & (kSuper / kChunk - 1)) == 0) {
-#endif
                 // ---- anchor phase of super-chunk s: state (x, d) of every pixel at delay s * R
                 const int s = j / (kSuper / kChunk);
                 const float2* Es = a.Es + (size_t)s * (size_t)a.bp.n_f;
-#ifdef ST_EXP_NOANCHOR
-                if (s == 0 && q > (1ull << 62)) {
-#else
                 if (s == 0) {
-#endif
                     // rasterise: four columns per lane in flight (FP64 div / sqrt chains are long)
 #pragma unroll 1
                     for (int pr = 0; pr < n_prows; pr += 2) {
@@ -742,11 +729,7 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
                 }
                 // gather p and the anchor phase factor: 16 independent L2 loads in flight per lane
 #pragma unroll 1
-#ifdef ST_EXP_NOANCHOR
-                for (int pr = 0; pr < (q > (1ull << 62) ? n_prows : 0); pr += 4) {
-#else
                 for (int pr = 0; pr < n_prows; pr += 4) {
-#endif
                     float2 pv[8], wv[8];
                     int kq[8];
 #pragma unroll
@@ -787,8 +770,7 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
             // ---- one chunk of 32 delays: four pixels of the lane in flight (two register pairs).
             // Per delay and pair: two scalar FFMAs (d += -kappa x on the halves; a packed FFMA with
             // three distinct register pairs issues at 2/3 rate), one packed add (x += d) and the
-            // accumulation.  VAR 0: four scalar adds into acc[i]; VAR 1: one packed add of the two
-            // pairs, then two scalar adds (fewer issue slots).
+            // accumulation: one packed add of the two pairs, then two scalar adds.
             float f[kChunk];
 #pragma unroll
             for (int i = 0; i < kChunk; ++i) f[i] = 0.0f;
@@ -800,45 +782,14 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
                 const uint32_t kk0 = pool_k[e0], kk1 = pool_k[e1];
                 const f32x2_t nk0 = pk_make(sm_negk[2 * (kk0 & 0xFFFFu)], sm_negk[2 * (kk0 >> 16)]);
                 const f32x2_t nk1 = pk_make(sm_negk[2 * (kk1 & 0xFFFFu)], sm_negk[2 * (kk1 >> 16)]);
-                if (VAR <= 1) {
 #pragma unroll
-                    for (int i = 0; i < kChunk; ++i) {
-                        if (VAR == 0) {
-                            f[i] += pk_lo(x0); f[i] += pk_hi(x0);
-                            f[i] += pk_lo(x1); f[i] += pk_hi(x1);
-                        } else {
-                            const f32x2_t sx = pk_add(x0, x1);
-                            f[i] += pk_lo(sx); f[i] += pk_hi(sx);
-                        }
-                        d0 = pk_fma_halves(nk0, x0, d0);
-                        d1 = pk_fma_halves(nk1, x1, d1);
-                        x0 = pk_add(x0, d0);
-                        x1 = pk_add(x1, d1);
-                    }
-                } else if (VAR == 2) {
-                    // same arithmetic, every packed value updated in place (stable register pairs)
-                    f32x2_t sx = pk_add(x0, x1);
-#pragma unroll
-                    for (int i = 0; i < kChunk; ++i) {
-                        f[i] += pk_lo(sx); f[i] += pk_hi(sx);
-                        d0 = pk_fma_halves(nk0, x0, d0);
-                        d1 = pk_fma_halves(nk1, x1, d1);
-                        x0 = pk_add(x0, d0);
-                        x1 = pk_add(x1, d1);
-                        sx = pk_add(x0, x1);
-                    }
-                } else {
-                    // all scalar: four independent chains, 32-bit operands only
-                    float a0 = pk_lo(x0), a1 = pk_hi(x0), a2 = pk_lo(x1), a3 = pk_hi(x1);
-                    float b0 = pk_lo(d0), b1 = pk_hi(d0), b2 = pk_lo(d1), b3 = pk_hi(d1);
-                    const float k0 = pk_lo(nk0), k1 = pk_hi(nk0), k2 = pk_lo(nk1), k3 = pk_hi(nk1);
-#pragma unroll
-                    for (int i = 0; i < kChunk; ++i) {
-                        f[i] += (a0 + a1) + (a2 + a3);
-                        b0 = fmaf(k0, a0, b0); b1 = fmaf(k1, a1, b1); b2 = fmaf(k2, a2, b2); b3 = fmaf(k3, a3, b3);
-                        a0 += b0; a1 += b1; a2 += b2; a3 += b3;
-                    }
-                    x0 = pk_make(a0, a1); x1 = pk_make(a2, a3); d0 = pk_make(b0, b1); d1 = pk_make(b2, b3);
+                for (int i = 0; i < kChunk; ++i) {
+                    const f32x2_t sx = pk_add(x0, x1);
+                    f[i] += pk_lo(sx); f[i] += pk_hi(sx);
+                    d0 = pk_fma_halves(nk0, x0, d0);
+                    d1 = pk_fma_halves(nk1, x1, d1);
+                    x0 = pk_add(x0, d0);
+                    x1 = pk_add(x1, d1);
                 }
                 pool_x[e0] = x0; pool_d[e0] = d0; pool_x[e1] = x1; pool_d[e1] = d1;
             }
@@ -856,7 +807,6 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
                 pool_x[e0] = x0; pool_d[e0] = d0;
             }
             // ---- fold: the transposing tree across the 32 lanes
-#ifndef ST_EXP_NOFOLD
 #pragma unroll
             for (int off = 16, n = kChunk / 2; off >= 1; off >>= 1, n >>= 1) {
                 const bool upper = (lane & off) != 0;
@@ -867,18 +817,10 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
                     f[i] = keep + __shfl_xor_sync(kFull, send, off);
                 }
             }
-#else
-#pragma unroll
-            for (int i = 1; i < kChunk; ++i) f[0] += f[i];
-#endif
             const float v[1] = {f[0] * scale};
             const uint32_t ms[1] = {(uint32_t)(j * kChunk + lane)};
             const bool ok[1] = {(int)ms[0] < a.n_tau};
-#ifndef ST_EXP_NOREDUCE
             reduce_samples<1>(a, wr, sm_hist, id, q, v, ms, ok);
-#else
-            if (v[0] == 123.456f && ok[0]) wr.pixels += ms[0];
-#endif
         }
     }
     reduce_finish(a, wr);

@@ -89,7 +89,6 @@ struct st_ctx {
     int cheb_stride;                   // stride of the tables currently on the device
     bool pick_valid; double pick_dtau; int pick_stride;   // memo of cheb_pick_stride
     std::vector<float> h_cheb;         // host-built Chebyshev tables: [n_f] float4, [n_f] float2 Ec, [n_f] float zi
-    int reinsch_chains;                // tunable: packed recurrence chains in flight per lane (1 or 2)
     char err[512];
 };
 
@@ -413,17 +412,12 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         }
         if (smem > (size_t)c->smem_optin)
             return fail(c, ST_ENOSPC, "n_f %d / n_max %d need more shared memory than one SM has", c->n_f, n_max);
-        const int var = c->reinsch_chains;
-        int rc = var == 0 ? set_smem(c, st::k_score_reinsch<0>, smem) : var == 1 ? set_smem(c, st::k_score_reinsch<1>, smem)
-               : var == 2 ? set_smem(c, st::k_score_reinsch<2>, smem) : set_smem(c, st::k_score_reinsch<3>, smem);
+        int rc = set_smem(c, st::k_score_reinsch, smem);
         if (rc) return rc;
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
-        if (var == 0) st::k_score_reinsch<0><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
-        else if (var == 1) st::k_score_reinsch<1><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
-        else if (var == 2) st::k_score_reinsch<2><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
-        else st::k_score_reinsch<3><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        st::k_score_reinsch<<<(unsigned)blocks, threads, smem, c->stream>>>(a);
     } else {
         int threads = c->recur_threads;
         const size_t bt_bytes = (size_t)c->n_f * sizeof(float4);
@@ -592,9 +586,6 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512;
     c->err[0] = 0;
     c->cheb_stride = 0; c->pick_valid = false; c->pick_dtau = 0.0; c->pick_stride = 0;
-    c->reinsch_chains = 1;
-    const char* e2 = getenv("ST_REINSCH_VAR");
-    if (e2 && atoi(e2) >= 0 && atoi(e2) <= 3) c->reinsch_chains = atoi(e2);
     const char* e = getenv("ST_RECUR_THREADS");
     if (e) { int t = atoi(e); if (t >= 32 && t <= 1024 && t % 32 == 0) c->recur_threads = t; }
     *out = c;
