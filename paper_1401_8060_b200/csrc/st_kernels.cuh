@@ -435,7 +435,7 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
         if (q >= a.n_tracks) break;
         const uint64_t id = a.track_offset + q;
         const Track t = make_track(a.bp, id);
-        const Raster r = make_raster(t, a.bp.n_f);
+        const RasterFast r = make_raster_fast(t, a.bp.n_f);
         const double u_last = int_to_double_fast(t.N - 1) + 0.5;
         const float2* col0 = a.map + (size_t)t.j0 * (size_t)a.bp.n_f;
         float acc = 0.0f;
@@ -454,7 +454,7 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
             if (redo[0] | redo[1] | redo[2] | redo[3]) {  // ~1e-5 of the time: normative sequence
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
-                    if (redo[u]) kq[u] = raster_bin(r, cq[u]);
+                    if (redo[u]) kq[u] = raster_bin_regen(a.bp, id, cq[u]);
             }
             float2 pv[4];
 #pragma unroll

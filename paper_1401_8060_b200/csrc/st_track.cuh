@@ -159,7 +159,9 @@ ST_HD int32_t raster_bin(const Raster& r, int32_t c)
 // |dy/dxi| <= 2 n_f; guard = max(1e-6, 4e-11 n_f) leaves a factor 3).
 constexpr double kRoundMagic = 6755399441055744.0;   // 1.5 * 2^52: x + M - M rounds x to the nearest integer
 
-__device__ __forceinline__ double raster_y_fast(const Raster& r, double u)
+// xi(u): root of the time polynomial, float64 MUFU seeds + one Newton step each (~6e-12)
+template <typename R>
+__device__ __forceinline__ double raster_xi_fast(const R& r, double u)
 {
     const double D  = fma(r.cc, u, r.aa);                       // >= min(a, N - a)^2 > 0
     double rs, rc;
@@ -169,25 +171,28 @@ __device__ __forceinline__ double raster_y_fast(const Raster& r, double u)
     const double den = r.a + s;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(den));
     const double q0 = u * rc;
-    const double xi = fma(fma(-den, q0, u), rc, q0);            // one Newton step on the quotient u / den
+    return fma(fma(-den, q0, u), rc, q0);                       // one Newton step on the quotient u / den
+}
+__device__ __forceinline__ double raster_y_fast(const Raster& r, double u)
+{
+    const double xi = raster_xi_fast(r, u);
     const double om = 1.0 - xi;
     return fma(om * om, r.y0, fma(2.0 * (om * xi), r.y1, (xi * xi) * r.y2));
 }
 // floor(y) as an int (clamped to [0, kmax]); redo when y is within the guard of an integer or NaN
-__device__ __forceinline__ int32_t floor_guarded(const Raster& r, double y, bool& redo)
+template <typename R>
+__device__ __forceinline__ int32_t floor_guarded(const R& r, double y, bool& redo)
 {
     const double tm = y + kRoundMagic;
-    int32_t k = __double2loint(tm);                             // the low mantissa word holds the integer
-    double yr = tm - kRoundMagic;                               // nearest integer
-    const bool above = yr > y;
-    yr = above ? yr - 1.0 : yr;                                 // floor
-    k  = above ? k - 1 : k;
-    const double fr = y - yr;
-    redo = !(fr > r.guard && fr < 1.0 - r.guard) || !(fabs(y) < 1e9);   // also true for NaN
+    const int32_t kn = __double2loint(tm);                      // the low mantissa word holds the nearest integer
+    const double d = y - (tm - kRoundMagic);                    // y - nearest integer, in [-1/2, 1/2]
+    redo = !(fabs(d) >= r.guard);                               // near a bin edge, or NaN
+    const int32_t k = d < 0.0 ? kn - 1 : kn;                    // floor
     return k < 0 ? 0 : (k > r.kmax ? r.kmax : k);
 }
 // u = column + 1/2 given as a double (callers step it without int -> double conversions)
-__device__ __forceinline__ int32_t raster_bin_fast_u(const Raster& r, double u, bool& redo)
+template <typename R>
+__device__ __forceinline__ int32_t raster_bin_fast_u(const R& r, double u, bool& redo)
 {
     return floor_guarded(r, raster_y_fast(r, u), redo);
 }
@@ -200,6 +205,32 @@ __device__ __forceinline__ int32_t raster_bin_fast(const Raster& r, int32_t c)
     bool redo;
     const int32_t k = raster_bin_fast(r, c, redo);
     return redo ? raster_bin(r, c) : k;
+}
+// The fast path's own constants (no y1, y2: the hot kernels hold these 13 registers per template and,
+// on the ~2e-6 of the pixels that need the normative sequence, regenerate the template from its id).
+struct RasterFast {
+    double a, cc, aa, y0, pb, pc, guard;
+    int32_t kmax;
+};
+__device__ __forceinline__ RasterFast make_raster_fast(const Track& t, int32_t n_f)
+{
+    const Raster r = make_raster(t, n_f);
+    RasterFast f;
+    f.a = r.a; f.cc = r.cc; f.aa = r.aa; f.y0 = r.y0; f.guard = r.guard; f.kmax = r.kmax;
+    f.pb = 2.0 * (t.y1 - t.y0);                                 // Eq. 6 in Horner form: y = y0 + xi (pb + xi pc)
+    f.pc = (t.y0 - t.y1) + (t.y2 - t.y1);
+    return f;
+}
+__device__ __forceinline__ double raster_y_fast(const RasterFast& r, double u)
+{
+    const double xi = raster_xi_fast(r, u);
+    return fma(xi, fma(xi, r.pc, r.pb), r.y0);                  // error ~1e-12 bins
+}
+// normative bin of column c of template `id` (regenerated: rare path)
+__device__ __forceinline__ int32_t raster_bin_regen(const BankParams& bp, uint64_t id, int32_t c)
+{
+    const Track t = make_track(bp, id);
+    return raster_bin(make_raster(t, bp.n_f), c);
 }
 // exact (double)k for 0 <= k < 2^31 without the I2F conversion
 __device__ __forceinline__ double int_to_double_fast(int32_t k)
