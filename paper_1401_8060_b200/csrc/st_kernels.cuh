@@ -430,9 +430,13 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
     hist_init(sm_hist, a.n_bins);
     WarpReduce wr;
     reduce_init(wr);
+    // the template counter's atomic is issued one template ahead (its result waits in lane 0)
+    unsigned long long q_pref = 0;
+    if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
     for (;;) {
-        const uint64_t q = next_track(a);
+        const uint64_t q = __shfl_sync(kFull, q_pref, 0);
         if (q >= a.n_tracks) break;
+        if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
         const uint64_t id = a.track_offset + q;
         const Track t = make_track(a.bp, id);
         const RasterFast r = make_raster_fast(t, a.bp.n_f);
