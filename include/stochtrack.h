@@ -156,6 +156,25 @@ int st_set_map_host(st_ctx *ctx, const void *csd_host, const float *sigma_host, 
  * band: it falls back to the kernel whose per-bin table lives in L2.              */
 int st_search(st_ctx *ctx, const st_search_params *params, st_result *out);
 
+/* The top_k loudest (template, delay) samples of a search, in the G12 total order (larger float64 SNR,
+ * then smaller template id, then smaller delay index) -- the candidates a follow-up looks at
+ * (PAPER.md:232).  Two passes over the bank: st_search as usual (params->n_bins must be > 0: the
+ * histogram locates the SNR of the top_k-th sample), then a second scoring pass that keeps every sample
+ * at or above the edge one bin below it, re-scores those in float64 on the device and sorts them.
+ * top_out: HOST [top_k]; *n_out = entries written (= min(top_k, samples)).  *result as st_search.
+ * Errors as st_search, plus ST_EINVAL (top_k outside [1, ST_MAX_TOP_K], n_bins == 0) and ST_ENOSPC when
+ * more than 65 536 samples lie at or above that edge (histogram too coarse: use more / narrower bins). */
+#define ST_MAX_TOP_K 4096
+typedef struct {
+    uint64_t track;
+    int32_t  tau_index;      /* 0 in random mode */
+    float    snr_f32;        /* what the scoring kernel produced */
+    double   snr_f64;        /* re-scored in float64 */
+    double   tau;            /* seconds */
+} st_top_entry;
+int st_search_topk(st_ctx *ctx, const st_search_params *params, int32_t top_k, st_top_entry *top_out,
+                   int32_t *n_out, st_result *result);
+
 /* Batch / background mode (the background is estimated from many
  * time-shifted maps, every one searched with its own template bank; BASELINE.json configs[3]):
  * S0-S4 over n_maps maps in ONE call.  Map m is searched exactly as

@@ -222,3 +222,17 @@ def search_batch(csd_maps, sigma_maps, seeds, f_min, df, n_tracks, n_min, n_max,
         seed = int(seeds[m]) if np.ndim(seeds) else int(seeds)
         out.append(search(p, f_min, df, n_tracks, seed, n_min, n_max, **kw))
     return out
+
+
+def top_k(result, k):
+    """The k loudest (template, delay) samples of a `search(..., dump_snr=True)` result, in the G12 total
+    order (larger SNR, then smaller template id, then smaller delay index): the events a follow-up looks
+    at.  Plain sort of the dumped SNR array.  Returns [(track, tau_index, snr)]."""
+    snr = result["snr"]
+    n_tracks, n_tau = snr.shape
+    first = result.get("track_offset", 0)
+    flat = snr.ravel()
+    ids = np.repeat(np.arange(n_tracks, dtype=np.int64), n_tau)
+    ms = np.tile(np.arange(n_tau, dtype=np.int64), n_tracks)
+    order = np.lexsort((ms, ids, -flat))[:k]
+    return [(int(first + ids[i]), int(ms[i]), float(flat[i])) for i in order]

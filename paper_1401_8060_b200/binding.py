@@ -19,7 +19,7 @@ KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random",
 
 # every symbol include/stochtrack.h declares
 exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_workspace", "st_set_map",
-                    "st_set_map_host", "st_search", "st_search_batch", "st_ftmap_scratch_bytes", "st_set_map_from_strain", "st_search_timeshifts",
+                    "st_set_map_host", "st_search", "st_search_topk", "st_search_batch", "st_ftmap_scratch_bytes", "st_set_map_from_strain", "st_search_timeshifts",
                     "st_debug_get_map",
                     "st_track_params", "st_debug_rasterise",
                     "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words",
@@ -54,6 +54,14 @@ class CResult(C.Structure):
                 ("n_evals", C.c_uint64), ("n_pixels", C.c_uint64), ("n_candidates", C.c_int32),
                 ("kernel_used", C.c_int32), ("n_launches", C.c_int32), ("flags", C.c_int32),
                 ("gpu_ms", C.c_float), ("reserved", C.c_float)]
+
+
+class CTopEntry(C.Structure):
+    _fields_ = [("track", C.c_uint64), ("tau_index", C.c_int32), ("snr_f32", C.c_float), ("snr_f64", C.c_double),
+                ("tau", C.c_double)]
+
+
+MAX_TOP_K = 4096
 
 
 class CFtmapParams(C.Structure):
@@ -104,6 +112,9 @@ def load_library():
     L.st_last_error.restype = C.c_char_p
     L.st_version.argtypes = []
     L.st_version.restype = C.c_char_p
+    L.st_search_topk.argtypes = [vp, C.POINTER(CSearchParams), C.c_int32, C.POINTER(CTopEntry), C.POINTER(C.c_int32),
+                                 C.POINTER(CResult)]
+    L.st_search_topk.restype = C.c_int
     L.st_ftmap_scratch_bytes.argtypes = [vp, C.c_int32]
     L.st_ftmap_scratch_bytes.restype = C.c_size_t
     L.st_set_map_from_strain.argtypes = [vp, vp, vp, C.c_int64, C.POINTER(CFtmapParams), vp, C.c_size_t]
@@ -320,6 +331,22 @@ class Stochtrack:
         r = CResult()
         self._check(self._L.st_search(self._ctx, C.byref(p), C.byref(r)))
         return self._result(r, hist)
+
+    def search_topk(self, top_k, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=None, norm=NORM_SQRT_N,
+                    n_bins=1000, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO):
+        """The top_k loudest (template, delay) samples (st_search_topk).  Returns (SearchResult, list of
+        dicts {track, tau_index, snr_f32, snr_f64, tau} in the G12 order)."""
+        p, keep = self._params(n_tracks, seed, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
+                               track_offset, kernel)
+        hist = np.zeros(max(n_bins, 1), dtype=np.uint64)
+        p.hist_out = hist.ctypes.data_as(C.POINTER(C.c_uint64))
+        top = (CTopEntry * int(top_k))()
+        n_out = C.c_int32(0)
+        r = CResult()
+        self._check(self._L.st_search_topk(self._ctx, C.byref(p), int(top_k), top, C.byref(n_out), C.byref(r)))
+        entries = [dict(track=int(e.track), tau_index=int(e.tau_index), snr_f32=float(e.snr_f32),
+                        snr_f64=float(e.snr_f64), tau=float(e.tau)) for e in top[:n_out.value]]
+        return self._result(r, hist), entries
 
     @staticmethod
     def _result(r, hist):

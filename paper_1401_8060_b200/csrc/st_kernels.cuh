@@ -84,6 +84,8 @@ struct ScoreArgs {
     float hist_lo, hist_scale;
     float* dump;              // [n_tracks][n_tau] or null
     int32_t pool_stride;      // pixels of pool space per warp (>= n_max, multiple of 32)
+    int32_t capture_mode;     // top-K second pass: keep every sample with SNR >= capture_thr, nothing else
+    float capture_thr;
 };
 
 // ------------------------------------------------------------------ helpers --
@@ -140,11 +142,24 @@ __device__ __forceinline__ void reduce_init(WarpReduce& wr)
 
 // Called by all 32 lanes with NV values per lane (sample (id, m[i]) = v[i], ignored
 // where !valid[i]).  Histogram + running max + near-max candidate capture.
-template <int NV>
+// MODE 0: search pass (compiled without the capture branch: the hot kernels' register budget is tight);
+// MODE 1: capture pass of st_search_topk; MODE 2: decided at run time by a.capture_mode (fallback kernels).
+template <int NV, int MODE = 2>
 __device__ __forceinline__ void reduce_samples(const ScoreArgs& a, WarpReduce& wr, uint32_t* sm_hist,
                                                uint64_t id, uint64_t q, const float (&v)[NV],
                                                const uint32_t (&m)[NV], const bool (&valid)[NV])
 {
+    if (MODE == 1 || (MODE == 2 && a.capture_mode)) {       // warp-uniform
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            if (valid[i] && v[i] >= a.capture_thr) {
+                const uint32_t slot = atomicAdd(&a.sc->cand_count, 1u);
+                if (slot < a.cand_cap) { Cand c; c.snr = v[i]; c.m = m[i]; c.id = id; a.cand[slot] = c; }
+                else a.sc->overflow = 1u;
+            }
+        }
+        return;
+    }
     float lmax = -INFINITY;
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
@@ -421,6 +436,7 @@ __global__ void __launch_bounds__(256) k_score_table(const ScoreArgs a)
 #ifndef ST_RANDOM_MIN_BLOCKS
 #define ST_RANDOM_MIN_BLOCKS 3
 #endif
+template <bool CAPTURE>
 __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -482,7 +498,7 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
         const float v[1] = {acc * norm_scale(t.N, a.norm)};
         const uint32_t ms[1] = {0u};
         const bool ok[1] = {lane == 0};
-        reduce_samples<1>(a, wr, sm_hist, id, q, v, ms, ok);
+        reduce_samples<1, CAPTURE ? 1 : 0>(a, wr, sm_hist, id, q, v, ms, ok);
     }
     reduce_finish(a, wr);
     hist_flush(sm_hist, a.hist, a.n_bins);
@@ -1018,7 +1034,7 @@ __device__ __forceinline__ int cheb_phase_a(const ScoreArgs& a, const Track& t, 
 
 // Phase B for one template whose merged pixels sit in (pool_v, pool_k): every delay of the grid,
 // fused S4.  pool_v is advanced in place from chunk to chunk.
-template <int STRIDE>
+template <int STRIDE, bool CAPTURE>
 __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr, uint32_t* sm_hist,
                                              const float4* sm_tab, const float* sm_zi, float2* pool_v,
                                              const uint16_t* pool_k, const int n_merged, const float scale,
@@ -1126,11 +1142,11 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
     const float v[2] = {pk_lo(f2[0]) * sscale, pk_hi(f2[0]) * sscale};
         const uint32_t ms[2] = {(uint32_t)(j * kCheb + kHalf + lane), (uint32_t)(j * kCheb + kHalf - 1 - lane)};
         const bool ok[2] = {(int)ms[0] < a.n_tau, (int)ms[1] < a.n_tau};
-        reduce_samples<2>(a, wr, sm_hist, id, q, v, ms, ok);
+        reduce_samples<2, CAPTURE ? 1 : 0>(a, wr, sm_hist, id, q, v, ms, ok);
     }
 }
 
-template <int STRIDE>
+template <int STRIDE, bool CAPTURE>
 __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -1160,7 +1176,7 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
         const Track t = make_track(a.bp, id);
         wr.pixels += (unsigned long long)t.N;
         const int n_merged = cheb_phase_a(a, t, pool_v, pool_k, lane);
-        cheb_phase_b<STRIDE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, n_merged, norm_scale(t.N, a.norm), id, q,
+        cheb_phase_b<STRIDE, CAPTURE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, n_merged, norm_scale(t.N, a.norm), id, q,
                              n_chunks, lane);
     }
     reduce_finish(a, wr);
@@ -1278,6 +1294,21 @@ __global__ void __launch_bounds__(256) k_finalize(const FinalArgs a)
             if (overflow) res.n_candidates = 1;
         }
         if (lane == 0) *a.out = res;
+    }
+}
+
+// Float64 re-score of every captured candidate (top-K second pass): one warp per candidate at a time.
+__global__ void __launch_bounds__(256) k_rescore_cands(const FinalArgs a, double* __restrict__ snr64)
+{
+    const int lane = threadIdx.x & 31;
+    const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_w = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t n_cand = a.sc->cand_count < a.cand_cap ? a.sc->cand_count : a.cand_cap;
+    for (uint32_t i = gw; i < n_cand; i += n_w) {
+        const Cand c = a.cand[i];
+        const Track t = make_track(a.bp, c.id);
+        const double tau = a.tau_mode == 0 ? a.tau_d[c.m] : t.tau;
+        const double s = score_f64(a.map, a.bp, a.f_min, a.df, t, tau, a.norm);
+        if (lane == 0) snr64[i] = s;
     }
 }
 

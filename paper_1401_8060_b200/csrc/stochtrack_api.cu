@@ -10,6 +10,7 @@
 #include <string.h>
 #include <math.h>
 #include <vector>
+#include <algorithm>
 #include <new>
 
 #include "../../include/stochtrack.h"
@@ -26,7 +27,7 @@ constexpr uint64_t kMaxSamplesPerLaunch = 1ull << 31;   // keeps per-block u32 h
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t map, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, warp_best, stage_csd, stage_sigma, stage_csd2, stage_sigma2, b_scalars, b_result, b_hist, total;
+    size_t map, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, cand64, warp_best, stage_csd, stage_sigma, stage_csd2, stage_sigma2, b_scalars, b_result, b_hist, total;
 };
 
 Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
@@ -48,6 +49,7 @@ Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
     L.scalars = o;     o += align_up(sizeof(st::Scalars));
     L.result = o;      o += align_up(sizeof(st::DeviceResult));
     L.cand = o;        o += align_up((size_t)kCandCap * sizeof(st::Cand));
+    L.cand64 = o;      o += align_up((size_t)kCandCap * sizeof(double));
     L.warp_best = o;   o += align_up((size_t)kWarpSlots * sizeof(st::WarpBest));
     L.stage_csd = o;   o += align_up(n_pix * sizeof(float2));
     L.stage_sigma = o; o += align_up(n_pix * sizeof(float));
@@ -367,7 +369,8 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         uint64_t blocks = (uint64_t)c->n_sm * 8;
         const uint64_t need = (want_warps + 7) / 8;
         if (blocks > need) blocks = need;
-        st::k_score_random<<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        if (a.capture_mode) st::k_score_random<true><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        else st::k_score_random<false><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
     } else if (plan.kernel == ST_KERNEL_TABLE) {
         int threads = 256;
         size_t smem;
@@ -395,13 +398,18 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         if (smem > (size_t)c->smem_optin)
             return fail(c, ST_ENOSPC, "n_f %d / n_max %d need more shared memory than one SM has", c->n_f, n_max);
         const bool pk = plan.stride == 2;
-        int rc = pk ? set_smem(c, st::k_score_cheb<2>, smem) : set_smem(c, st::k_score_cheb<1>, smem);
-        if (rc) return rc;
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
-        if (pk) st::k_score_cheb<2><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
-        else st::k_score_cheb<1><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+#define ST_LAUNCH_CHEB(STRIDE, CAPTURE)                                                           \
+    do {                                                                                          \
+        int rc_ = set_smem(c, st::k_score_cheb<STRIDE, CAPTURE>, smem);                           \
+        if (rc_) return rc_;                                                                      \
+        st::k_score_cheb<STRIDE, CAPTURE><<<(unsigned)blocks, threads, smem, c->stream>>>(a);     \
+    } while (0)
+        if (pk) { if (a.capture_mode) ST_LAUNCH_CHEB(2, true); else ST_LAUNCH_CHEB(2, false); }
+        else    { if (a.capture_mode) ST_LAUNCH_CHEB(1, true); else ST_LAUNCH_CHEB(1, false); }
+#undef ST_LAUNCH_CHEB
     } else if (plan.kernel == ST_KERNEL_REINSCH) {
         int threads = c->recur_threads;
         size_t smem;
@@ -720,6 +728,89 @@ int st_search(st_ctx* c, const st_search_params* p, st_result* out)
     out->gpu_ms = ms;
     if (p->n_bins > 0)
         for (int b = 0; b < p->n_bins; ++b) p->hist_out[b] = (uint64_t)c->h_hist[b];
+    return ST_OK;
+}
+
+int st_search_topk(st_ctx* c, const st_search_params* p, int32_t top_k, st_top_entry* top_out, int32_t* n_out,
+                   st_result* result)
+{
+    if (!c) return ST_EINVAL;
+    if (!p || !top_out || !n_out || !result) return fail(c, ST_EINVAL, "NULL argument");
+    if (top_k < 1 || top_k > ST_MAX_TOP_K) return fail(c, ST_EINVAL, "top_k %d outside [1, %d]", top_k, ST_MAX_TOP_K);
+    if (p->n_bins < 1) return fail(c, ST_EINVAL, "st_search_topk needs a histogram (n_bins > 0)");
+    *n_out = 0;
+    int rc = st_search(c, p, result);                       // pass 1: maximum, histogram
+    if (rc) return rc;
+    if (p->n_tracks == 0) return ST_OK;
+    // the bin holding the top_k-th largest sample, then one bin lower (a sample near an edge may have been
+    // binned on either side of it in float32)
+    uint64_t cum = 0;
+    int b = p->n_bins;
+    while (b > 0 && cum < (uint64_t)top_k) cum += p->hist_out[--b];
+    if (b > 0) cum += p->hist_out[--b];
+    if (cum > (uint64_t)kCandCap)
+        return fail(c, ST_ENOSPC, "%llu samples at or above the bin of the top_k-th: histogram too coarse (cap %u)",
+                    (unsigned long long)cum, kCandCap);
+    const double width = (p->hist_hi - p->hist_lo) / (double)p->n_bins;
+    const float thr = b == 0 ? -INFINITY : (float)(p->hist_lo + (double)b * width - 1e-4 * width);
+    // pass 2: capture
+    Plan plan;
+    rc = make_plan(c, p, &plan);
+    if (rc) return rc;
+    const int n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
+    const Slots sl = own_slots(c);
+    rc = reset_search_state(c, 0, sl);
+    if (rc) return rc;
+    st::ScoreArgs a = base_args(c, p);
+    a.capture_mode = 1; a.capture_thr = thr;
+    uint64_t per_launch = kMaxSamplesPerLaunch / (uint64_t)n_tau;
+    if (per_launch < 1) per_launch = 1;
+    for (uint64_t done = 0; done < p->n_tracks; done += per_launch) {
+        a.track_offset = p->track_offset + done;
+        a.n_tracks = p->n_tracks - done < per_launch ? p->n_tracks - done : per_launch;
+        rc = launch_score(c, plan, a, p->n_max);
+        if (rc) return rc;
+        ++result->n_launches;
+    }
+    st::FinalArgs f;
+    memset(&f, 0, sizeof(f));
+    f.map = a.map; f.bp = a.bp; f.f_min = c->f_min; f.df = c->df;
+    f.norm = p->norm; f.tau_mode = p->tau_mode; f.n_tau = n_tau;
+    f.tau_d = at<double>(c, c->L.tau);
+    f.sc = a.sc; f.cand = a.cand; f.cand_cap = kCandCap;
+    st::k_rescore_cands<<<c->n_sm * 4, 256, 0, c->stream>>>(f, at<double>(c, c->L.cand64));
+    ST_CUDA(c, cudaGetLastError());
+    ++result->n_launches;
+    st::Scalars hsc;
+    ST_CUDA(c, cudaMemcpyAsync(&hsc, a.sc, sizeof(hsc), cudaMemcpyDeviceToHost, c->stream));
+    ST_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (hsc.overflow || hsc.cand_count > kCandCap) return fail(c, ST_ENOSPC, "candidate list overflowed in the capture pass");
+    const uint32_t n = hsc.cand_count;
+    std::vector<st::Cand> hc(n);
+    std::vector<double> h64(n);
+    if (n) {
+        ST_CUDA(c, cudaMemcpy(hc.data(), a.cand, (size_t)n * sizeof(st::Cand), cudaMemcpyDeviceToHost));
+        ST_CUDA(c, cudaMemcpy(h64.data(), at<double>(c, c->L.cand64), (size_t)n * sizeof(double), cudaMemcpyDeviceToHost));
+    }
+    std::vector<uint32_t> order(n);
+    for (uint32_t i = 0; i < n; ++i) order[i] = i;
+    std::sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) {     // G12 total order
+        if (h64[x] != h64[y]) return h64[x] > h64[y];
+        if (hc[x].id != hc[y].id) return hc[x].id < hc[y].id;
+        return hc[x].m < hc[y].m;
+    });
+    const uint32_t k_out = n < (uint32_t)top_k ? n : (uint32_t)top_k;
+    for (uint32_t i = 0; i < k_out; ++i) {
+        const uint32_t e = order[i];
+        top_out[i].track = hc[e].id; top_out[i].tau_index = (int32_t)hc[e].m;
+        top_out[i].snr_f32 = hc[e].snr; top_out[i].snr_f64 = h64[e];
+        if (p->tau_mode == ST_TAU_GRID) top_out[i].tau = p->tau_grid[hc[e].m];
+        else {
+            st::BankParams bp = bank(c, p);
+            top_out[i].tau = st::make_track(bp, hc[e].id).tau;
+        }
+    }
+    *n_out = (int32_t)k_out;
     return ST_OK;
 }
 

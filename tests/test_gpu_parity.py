@@ -574,3 +574,41 @@ def test_wide_band_and_long_templates_limits(P, orc):
     ref = orc.search(orc.prepare_map(csd), 40.0, 1.0, 200, 9, 15000, 20000, tau_grid=synth.tau_linspace(16))
     assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
     assert abs(r.max_snr - ref["max_snr"]) <= 1e-4 * abs(ref["max_snr"])
+
+
+@pytest.mark.parametrize("cid,n_tracks,k", [(1, 1000, 10), (2, 100000, 25), (3, 200000, 10)])
+def test_top_k_loudest_samples(P, orc, cid, n_tracks, k):
+    """st_search_topk == the oracle's sorted head: the same (template, delay) pairs in the same order, float64
+    SNRs to the re-score's accuracy; the first entry is the search's argmax."""
+    cfg = synth.CONFIGS[cid]
+    csd, sigma, tau = config_inputs(orc, cfg, 0)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    kw = dict(tau_grid=tau) if cfg.tau_mode == "grid" else dict(tau_range=(-synth.TAU_MAX, synth.TAU_MAX))
+    r, top = st.search_topk(k, n_tracks, cfg.seed, cfg.n_min, cfg.n_max, n_bins=cfg.n_bins, hist_lo=cfg.hist_lo,
+                            hist_hi=cfg.hist_hi, **kw)
+    ref = orc.search(orc.prepare_map(csd, sigma), cfg.f_min, cfg.df, n_tracks, cfg.seed, cfg.n_min, cfg.n_max,
+                     dump_snr=True, **kw)
+    want = orc.top_k(ref, k)
+    assert len(top) == k
+    assert [(e["track"], e["tau_index"]) for e in top] == [w[:2] for w in want]
+    rel64 = 1e-11 if cfg.sigma == "none" else 2e-7
+    for e, w in zip(top, want):
+        assert abs(e["snr_f64"] - w[2]) <= rel64 * abs(w[2]) and abs(e["snr_f32"] - w[2]) <= 1e-4 * max(abs(w[2]), S0_UNIT)
+    assert (top[0]["track"], top[0]["tau_index"]) == (r.arg_track, r.arg_tau_index) and top[0]["snr_f64"] == r.max_snr_f64
+    if cfg.tau_mode == "grid":
+        assert top[3]["tau"] == tau[top[3]["tau_index"]]
+
+
+def test_top_k_limits(P, orc):
+    cfg = synth.CONFIGS[1]
+    csd, sigma, tau = config_inputs(orc, cfg, 0)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    r, top = st.search_topk(50, 2, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau[:4], n_bins=100)     # fewer samples than k
+    assert len(top) == 8 and sorted(t["snr_f64"] for t in top)[::-1] == [t["snr_f64"] for t in top]
+    with pytest.raises(P.StError):
+        st.search_topk(10, 100, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=0)
+    with pytest.raises(P.StError) as e:                 # one coarse bin holds everything: 1e5 x 16 samples > 65 536
+        st.search_topk(10, 100000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=2, hist_lo=-50.0, hist_hi=50.0)
+    assert e.value.code == -3

@@ -43,7 +43,8 @@ int main(void) {
          offsetof(st_search_params, tau_grid), offsetof(st_search_params, hist_out), offsetof(st_search_params, kernel),
          offsetof(st_result, arg_params), offsetof(st_result, gpu_ms), sizeof(st_batch), offsetof(st_batch, csd),
          offsetof(st_batch, seeds));
-  printf("%zu %zu\n", sizeof(st_ftmap_params), offsetof(st_ftmap_params, n_neighbours));
+  printf("%zu %zu ", sizeof(st_ftmap_params), offsetof(st_ftmap_params, n_neighbours));
+  printf("%zu %zu %zu\n", sizeof(st_top_entry), offsetof(st_top_entry, snr_f64), offsetof(st_top_entry, tau));
   return 0; }
 """)
     exe = tmp_path / "layout"
@@ -53,7 +54,8 @@ int main(void) {
     want = [C.sizeof(B.CTrack), C.sizeof(B.CSearchParams), C.sizeof(B.CResult), B.CSearchParams.tau_grid.offset,
             B.CSearchParams.hist_out.offset, B.CSearchParams.kernel.offset, B.CResult.arg_params.offset,
             B.CResult.gpu_ms.offset, C.sizeof(B.CBatch), B.CBatch.csd.offset, B.CBatch.seeds.offset,
-            C.sizeof(B.CFtmapParams), B.CFtmapParams.n_neighbours.offset]
+            C.sizeof(B.CFtmapParams), B.CFtmapParams.n_neighbours.offset,
+            C.sizeof(B.CTopEntry), B.CTopEntry.snr_f64.offset, B.CTopEntry.tau.offset]
     assert B.BATCH_GROUP == int(re.search(r"#define ST_BATCH_GROUP\s+(\d+)", open(os.path.join(ROOT, "include", "stochtrack.h")).read()).group(1))
     assert got == want
 

@@ -443,3 +443,17 @@ def test_random_tau_mode_uses_track_delay(orc):
         assert r["snr"][i, 0] == orc.score_direct(p, t, k, cfg.f_min, cfg.df, t.tau, 0)
     i = int(np.argmax(r["snr"][:, 0]))
     assert r["arg_track"] == i and r["arg_tau"] == orc.track_params(3, i, cfg.n_t, cfg.n_f, 8, 64, -0.01, 0.01).tau
+
+
+def test_top_k_is_the_sorted_head_of_all_samples(orc):
+    """oracle.top_k against brute force on a tiny search (explicit Python sort of every sample), ties
+    included: an all-zero map makes every SNR equal, so the order is by template id, then delay index."""
+    cfg = synth.CONFIGS[1]
+    csd, sigma, tau = synth.config_inputs(cfg)
+    r = orc.search(orc.prepare_map(csd, sigma), cfg.f_min, cfg.df, 60, 3, cfg.n_min, cfg.n_max, tau_grid=tau, dump_snr=True)
+    brute = sorted(((-r["snr"][i, m], i, m) for i in range(60) for m in range(cfg.n_tau)))[:25]
+    assert orc.top_k(r, 25) == [(i, m, -s) for s, i, m in brute]
+    assert orc.top_k(r, 1)[0][:2] == (r["arg_track"], r["arg_tau_index"])
+    z = orc.search(np.zeros((cfg.n_t, cfg.n_f), dtype=np.complex128), cfg.f_min, cfg.df, 5, 3, cfg.n_min, cfg.n_max,
+                   tau_grid=tau[:3], dump_snr=True)
+    assert [e[:2] for e in orc.top_k(z, 5)] == [(0, 0), (0, 1), (0, 2), (1, 0), (1, 1)]
