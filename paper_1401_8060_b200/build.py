@@ -35,6 +35,18 @@ def _stale(target, deps):
     return any(os.path.getmtime(d) > t for d in deps if os.path.exists(d))
 
 
+LIB_CHECKED = os.path.join(HERE, "libstochtrack_b200_checked.so")
+
+
+def build_checked(force=False):
+    """The same library with -DST_CHECKED: device-side assertions on every index (for the GPU tests)."""
+    srcs = [os.path.join(CSRC, s) for s in SOURCES]
+    deps = srcs + [os.path.join(CSRC, h) for h in HEADERS]
+    if force or _stale(LIB_CHECKED, deps):
+        subprocess.check_call([_nvcc(), *NVCC_FLAGS, "-DST_CHECKED", "-shared", "-o", LIB_CHECKED, *srcs])
+    return LIB_CHECKED
+
+
 def build(force=False, verbose=False):
     """Compile libstochtrack_b200.so (and the microbenchmark binary). Returns the .so path."""
     srcs = [os.path.join(CSRC, s) for s in SOURCES]
@@ -52,4 +64,7 @@ def build(force=False, verbose=False):
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--checked" in sys.argv:
+        print(build_checked(force="--force" in sys.argv))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -18,6 +18,16 @@
 #include <stdint.h>
 #include "st_track.cuh"
 
+// -DST_CHECKED (python -m paper_1401_8060_b200.build --checked): device-side assertions on every index the
+// kernels form (compute-sanitizer is not available on the GPU pool); a failed one traps the kernel and the
+// next API call returns ST_ECUDA.  Compiled out of the production library.
+#ifdef ST_CHECKED
+#include <assert.h>
+#define ST_ASSERT(cond) assert(cond)
+#else
+#define ST_ASSERT(cond) ((void)0)
+#endif
+
 namespace st {
 
 constexpr int kWarp = 32;
@@ -168,6 +178,7 @@ __device__ __forceinline__ void reduce_samples(const ScoreArgs& a, WarpReduce& w
             if (a.n_bins > 0) {
                 int b = __float2int_rd((v[i] - a.hist_lo) * a.hist_scale);
                 b = b < 0 ? 0 : (b >= a.n_bins ? a.n_bins - 1 : b);
+                ST_ASSERT(b >= 0 && b < a.n_bins && (int)m[i] < a.n_tau);
                 atomicAdd(&sm_hist[b], 1u);
             }
             if (a.dump) a.dump[q * (uint64_t)a.n_tau + m[i]] = v[i];
@@ -195,6 +206,7 @@ __device__ __forceinline__ void reduce_samples(const ScoreArgs& a, WarpReduce& w
                     if (slot < a.cand_cap) { Cand c; c.snr = v[i]; c.m = m[i]; c.id = id; a.cand[slot] = c; }
                     else a.sc->overflow = 1u;
                 }
+                ST_ASSERT(id >= a.track_offset && id < a.track_offset + a.n_tracks);
                 if (v[i] > bs || (v[i] == bs && m[i] < bm)) { bs = v[i]; bm = m[i]; }
             }
         }
@@ -478,8 +490,10 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
             }
             float2 pv[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
+            for (int u = 0; u < 4; ++u) {
+                ST_ASSERT(kq[u] >= 0 && kq[u] < a.bp.n_f && cq[u] >= 0 && t.j0 + cq[u] < a.bp.n_t);
                 pv[u] = __ldg(col0 + (size_t)cq[u] * (size_t)a.bp.n_f + (size_t)kq[u]);
+            }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const double cyc = (a.f_min + int_to_double_fast(kq[u]) * a.df) * t.tau;
@@ -964,6 +978,8 @@ __device__ __forceinline__ void cheb_fetch(const ScoreArgs& a, const ChebFetchCt
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
+        ST_ASSERT(E.k[u] >= 0 && E.k[u] < a.bp.n_f && cc[u] >= 0 &&
+                  (size_t)(f.col0 - a.map) / (size_t)a.bp.n_f + (size_t)cc[u] < (size_t)a.bp.n_t);
         E.p[u] = __ldg(f.col0 + (size_t)cc[u] * (size_t)a.bp.n_f + (size_t)E.k[u]);
         E.e[u] = __ldg(&a.Ec[E.k[u]]);
     }
@@ -1053,6 +1069,7 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
             const int e0 = row * kWarp + lane, e1 = e0 + kWarp;
             const float2 v0 = pool_v[e0], v1 = pool_v[e1];
             const int k0 = pool_k[e0], k1 = pool_k[e1];
+            ST_ASSERT(k0 >= 0 && k0 < a.bp.n_f && k1 >= 0 && k1 < a.bp.n_f);
             const float4 t0 = sm_tab[k0], t1 = sm_tab[k1];
             const float zi0 = sm_zi[k0], zi1 = sm_zi[k1];
             // next chunk's anchors: v e^{i 64 theta}   (t.w = cos 64 theta, zi = sin 64 theta)
@@ -1176,6 +1193,8 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
         const Track t = make_track(a.bp, id);
         wr.pixels += (unsigned long long)t.N;
         const int n_merged = cheb_phase_a(a, t, pool_v, pool_k, lane);
+        ST_ASSERT(n_merged >= 1 && n_merged <= t.N && ((n_merged + kWarp - 1) & ~(kWarp - 1)) <= S &&
+                  t.N >= a.bp.n_min && t.N <= a.bp.n_max && t.j0 >= 0 && t.j0 + t.N <= a.bp.n_t);
         cheb_phase_b<STRIDE, CAPTURE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, n_merged, norm_scale(t.N, a.norm), id, q,
                              n_chunks, lane);
     }
