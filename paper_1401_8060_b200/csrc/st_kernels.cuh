@@ -438,13 +438,78 @@ __global__ void __launch_bounds__(256) k_score_table(const ScoreArgs a)
 }
 
 // ----------------------------------------- S1-S4, the paper's random-tau mode --
-// One delay per template.  Lanes over columns, four columns per lane in flight:
-// branch-free bins, then the four L2 gathers together.  The phase f_k tau (up to 25 cycles) is
-// formed and reduced to [-1/2, 1/2] in float64, its sine and cosine taken by MUFU in float32
-// (abs error 5e-7); partial sums meet in a warp shuffle tree.  Per pixel the XU pipe sees five
-// operations (two float64 seeds of the rasteriser, one F2F, MUFU.SIN, MUFU.COS): everything else
-// (floor, int <-> double, rounding to the nearest cycle) runs on the FP64 pipe through the
-// 1.5 * 2^52 constant, so that the binding unit is the L2 sector gather, not conversions.
+// One delay per template: one Eq. 8 term per pixel, so the kernel is a gather.  Measured:
+// neither the rasteriser nor the phase factor bound it (removing either changes nothing) -- the chain
+// counter -> Philox -> rasteriser -> L2 gather -> reduce of ONE template per warp does.  So a warp works
+// on several templates at once, kRandGroup lanes each: their chains run in the same instructions (SIMT),
+// the per-template fixed work costs a fraction of the issue slots, and a 255-column template fills its
+// lanes where 32 lanes idled on its ragged last pass.  Measured on config 3 / the paper's Table III shape
+// (fraction of the L2 gather rate): 32 lanes 0.71 / 0.91, 16 lanes 0.84 / 0.95, 8 lanes 0.82 / 0.94,
+// 4 lanes 0.79 / 0.92.
+// Per pixel: branch-free bin (fast path), the gather, the phase f_k tau reduced to [-1/2, 1/2] in float64
+// on the FP64 pipe (1.5 * 2^52 rounding), MUFU sin / cos in float32 (abs error 5e-7); 5 XU operations.
+#ifndef ST_RAND_GROUP
+#define ST_RAND_GROUP 16
+#endif
+constexpr int kRandGroup = ST_RAND_GROUP;   // lanes per template
+constexpr int kRandPerWarp = kWarp / kRandGroup;
+
+// S4 for up to one sample per lane, each with its own template id (m = 0): histogram, running maximum,
+// near-max candidates, per-warp best under the G12 order.
+template <int MODE>
+__device__ __forceinline__ void reduce_samples_multi(const ScoreArgs& a, WarpReduce& wr, uint32_t* sm_hist,
+                                                     const uint64_t id, const uint64_t q, const float v, const bool valid)
+{
+    if (MODE == 1) {
+        if (valid && v >= a.capture_thr) {
+            const uint32_t slot = atomicAdd(&a.sc->cand_count, 1u);
+            if (slot < a.cand_cap) { Cand c; c.snr = v; c.m = 0u; c.id = id; a.cand[slot] = c; }
+            else a.sc->overflow = 1u;
+        }
+        return;
+    }
+    if (valid) {
+        if (a.n_bins > 0) {
+            int b = __float2int_rd((v - a.hist_lo) * a.hist_scale);
+            b = b < 0 ? 0 : (b >= a.n_bins ? a.n_bins - 1 : b);
+            ST_ASSERT(b >= 0 && b < a.n_bins);
+            atomicAdd(&sm_hist[b], 1u);
+        }
+        if (a.dump) a.dump[q] = v;
+    }
+    float wmax = valid ? v : -INFINITY;
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) wmax = fmaxf(wmax, __shfl_xor_sync(kFull, wmax, off));
+    if (wmax >= wr.cached_max - near_margin(wr.cached_max)) {
+        const int lane = threadIdx.x & 31;
+        uint32_t old = 0;
+        if (lane == 0) old = atomicMax(&a.sc->gmax_bits, enc_f32(wmax));
+        old = __shfl_sync(kFull, old, 0);
+        const float gm = fmaxf(dec_f32(old), wmax);
+        wr.cached_max = gm;
+        const float thr = gm - near_margin(gm);
+        const bool full = *(volatile uint32_t*)&a.sc->overflow != 0;
+        float bs = -INFINITY; uint64_t bid = 0;
+        if (valid && v >= thr) {
+            if (!full) {
+                const uint32_t slot = atomicAdd(&a.sc->cand_count, 1u);
+                if (slot < a.cand_cap) { Cand c; c.snr = v; c.m = 0u; c.id = id; a.cand[slot] = c; }
+                else a.sc->overflow = 1u;
+            }
+            bs = v; bid = id;
+        }
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) {
+            const float os = __shfl_xor_sync(kFull, bs, off);
+            const uint64_t oid = __shfl_xor_sync(kFull, bid, off);
+            if (os > bs || (os == bs && os > -INFINITY && oid < bid)) { bs = os; bid = oid; }
+        }
+        if (bs > -INFINITY && (!wr.best.valid || better(bs, bid, 0u, wr.best.snr, wr.best.id, wr.best.m))) {
+            wr.best.snr = bs; wr.best.m = 0u; wr.best.id = bid; wr.best.valid = 1;
+        }
+    }
+}
+
 #ifndef ST_RANDOM_MIN_BLOCKS
 #define ST_RANDOM_MIN_BLOCKS 3
 #endif
@@ -454,34 +519,41 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
     const int lane = threadIdx.x & 31;
-    const double u_lane = (double)lane + 0.5;
+    const int sub = lane & (kRandGroup - 1), grp = lane / kRandGroup;
+    const double u_sub = (double)sub + 0.5;
     hist_init(sm_hist, a.n_bins);
     WarpReduce wr;
     reduce_init(wr);
-    // the template counter's atomic is issued one template ahead (its result waits in lane 0)
+    // kRandPerWarp templates are claimed per atomic, one claim ahead (the result waits in lane 0)
     unsigned long long q_pref = 0;
-    if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
+    if (lane == 0) q_pref = atomicAdd(&a.sc->counter, (unsigned long long)kRandPerWarp);
     for (;;) {
-        const uint64_t q = __shfl_sync(kFull, q_pref, 0);
-        if (q >= a.n_tracks) break;
-        if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
-        const uint64_t id = a.track_offset + q;
+        const uint64_t q0 = __shfl_sync(kFull, q_pref, 0);
+        if (q0 >= a.n_tracks) break;
+        if (lane == 0) q_pref = atomicAdd(&a.sc->counter, (unsigned long long)kRandPerWarp);
+        const uint64_t q = q0 + (uint64_t)grp;
+        const bool live = q < a.n_tracks;                    // the last claim may be ragged
+        const uint64_t id = a.track_offset + (live ? q : q0);
         const Track t = make_track(a.bp, id);
         const RasterFast r = make_raster_fast(t, a.bp.n_f);
+        const int N = live ? t.N : 0;
+        int n_max = N;
+#pragma unroll
+        for (int off = 16; off >= kRandGroup; off >>= 1) n_max = max(n_max, __shfl_xor_sync(kFull, n_max, off));
         const double u_last = int_to_double_fast(t.N - 1) + 0.5;
         const float2* col0 = a.map + (size_t)t.j0 * (size_t)a.bp.n_f;
         float acc = 0.0f;
-        double ub = u_lane;                               // column centre of this lane in the current group
+        double ub = u_sub;                                    // column centre of this lane in the current pass
 #pragma unroll 1
-        for (int c0 = lane; c0 < t.N; c0 += 4 * kWarp, ub += 128.0) {
+        for (int c0 = sub; c0 < n_max; c0 += 4 * kRandGroup, ub += 4.0 * kRandGroup) {
             int kq[4], cq[4];
             bool redo[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int c = c0 + u * kWarp;
-                const bool in = c < t.N;
+                const int c = c0 + u * kRandGroup;
+                const bool in = c < N;
                 cq[u] = in ? c : t.N - 1;                 // clamped: discarded below
-                kq[u] = raster_bin_fast_u(r, in ? ub + 32.0 * u : u_last, redo[u]);
+                kq[u] = raster_bin_fast_u(r, in ? ub + (double)(u * kRandGroup) : u_last, redo[u]);
             }
             if (redo[0] | redo[1] | redo[2] | redo[3]) {  // ~1e-5 of the time: normative sequence
 #pragma unroll
@@ -500,19 +572,23 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
                 const double fr = cyc - ((cyc + kRoundMagic) - kRoundMagic);     // cyc - rint(cyc), |cyc| < 2^51
                 const float ph = 6.283185307179586f * (float)fr;
                 const float s = __sinf(ph), co = __cosf(ph);
-                if (c0 + u * kWarp < t.N) {
+                if (c0 + u * kRandGroup < N) {
                     acc = fmaf(co, pv[u].x, acc);
                     acc = fmaf(-s, pv[u].y, acc);
                 }
             }
         }
 #pragma unroll
-        for (int off = 16; off >= 1; off >>= 1) acc += __shfl_xor_sync(kFull, acc, off);
-        wr.pixels += (unsigned long long)t.N;
-        const float v[1] = {acc * norm_scale(t.N, a.norm)};
-        const uint32_t ms[1] = {0u};
-        const bool ok[1] = {lane == 0};
-        reduce_samples<1, CAPTURE ? 1 : 0>(a, wr, sm_hist, id, q, v, ms, ok);
+        for (int off = kRandGroup / 2; off >= 1; off >>= 1) acc += __shfl_xor_sync(kFull, acc, off);
+        if (sub == 0) wr.pixels += (unsigned long long)N;
+        reduce_samples_multi<CAPTURE ? 1 : 0>(a, wr, sm_hist, id, q, acc * norm_scale(t.N, a.norm), live && sub == 0);
+    }
+    // wr.pixels was accumulated by the four group leaders: fold them into lane 0 for reduce_finish
+    {
+        unsigned long long px = wr.pixels;
+#pragma unroll
+        for (int off = 16; off >= kRandGroup; off >>= 1) px += __shfl_xor_sync(kFull, px, off);
+        wr.pixels = px;
     }
     reduce_finish(a, wr);
     hist_flush(sm_hist, a.hist, a.n_bins);

@@ -367,7 +367,7 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         const int threads = 256;
         const size_t smem = hist_bytes(a.n_bins);
         uint64_t blocks = (uint64_t)c->n_sm * 8;
-        const uint64_t need = (want_warps + 7) / 8;
+        const uint64_t need = ((want_warps + st::kRandPerWarp - 1) / st::kRandPerWarp + 7) / 8;   // a warp scores kRandPerWarp templates at a time
         if (blocks > need) blocks = need;
         if (a.capture_mode) st::k_score_random<true><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
         else st::k_score_random<false><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
