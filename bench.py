@@ -382,6 +382,16 @@ def main():
     args.config = "P" if args.config == "P" else int(args.config)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = max(args.warmup, 1)
+    # --gpus N is a request for N ranks, one per GPU.  Under torchrun WORLD_SIZE must agree with it; started
+    # as a plain `python bench.py --gpus N` (N > 1) the script re-executes itself under torch.distributed.run.
+    world = os.environ.get("WORLD_SIZE")
+    if world is None and args.gpus > 1:
+        port = os.environ.get("MASTER_PORT", "29531")
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", port, os.path.abspath(__file__), *sys.argv[1:]]
+        raise SystemExit(subprocess.call(cmd))
+    if world is not None and int(world) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch {args.gpus} ranks or pass --gpus {world}")
     if args.impl == "reference":
         run_reference(args)
     else:

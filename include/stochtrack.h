@@ -220,7 +220,7 @@ typedef struct {
 size_t st_ftmap_scratch_bytes(const st_ctx *ctx, int32_t seg_len);
 int st_set_map_from_strain(st_ctx *ctx, const double *s_i_dev, const double *s_j_dev, int64_t n_samples,
                            const st_ftmap_params *params, void *scratch_dev, size_t scratch_bytes);
-/* Time-shift background from strain (PAPER.md:165: significance from n_ts time-shift analyses; reading
+/* Time-shift background from strain (PAPER.md:173: significance from n_ts time-shift analyses; reading
  * G23): the strain spectrograms are computed ONCE; for each shifts[m] (HOST, whole segments, 0 <= shift <
  * n_t, cyclic over the map) detector J's segment (j + shift) mod n_t is paired with detector I's segment j,
  * P' of each detector taken around its own segment, and the resulting map is searched with seeds[m]

@@ -25,7 +25,7 @@ Readings (G19-G22), where the paper is silent:
        p = sqrt(2) s~_I^* s~_J / sqrt(P'_I P'_J), which makes Re[e^{i phi} p] unit variance on
        stationary independent Gaussian noise in the limit of many neighbours (A1-A3).
   G22  a pixel whose P'_I P'_J is zero or not finite is masked (p = 0), as G11.
-  G23  time shifts (PAPER.md:165) are whole segments, cyclic over the map: J's segment (j + s) mod n_t
+  G23  time shifts (PAPER.md:173) are whole segments, cyclic over the map: J's segment (j + s) mod n_t
        meets I's segment j; P'_J is taken around J's own segment.
 """
 import numpy as np
@@ -91,7 +91,7 @@ def ftmap(s_i, s_j, fs, seg_len, n_t, f_min, n_f, n_nb):
 
 
 def ftmap_timeshift(st_i, st_j, n_nb, shift):
-    """Time-shifted background map (PAPER.md:165: significance is evaluated from n_ts time-shift analyses;
+    """Time-shifted background map (PAPER.md:173: significance is evaluated from n_ts time-shift analyses;
     reading G23): detector J's segment (j + shift) mod n_t is paired with detector I's segment j, so
     that no astrophysical signal is coherent between the two; every detector's P' is taken around its
     own segment.  st_i, st_j: the strain spectrograms of `ftmap` (F1 + F2).  shift = 0 is `ftmap`."""

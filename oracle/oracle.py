@@ -208,7 +208,7 @@ def search(p, f_min, df, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=
             "arg_tau_index": int(res.arg_tau_index), "arg_tau": res.arg_tau,
             "n_evals": int(res.n_evals), "n_pixels": int(res.n_pixels),
             "threads_used": int(res.threads_used), "hist": hist, "snr": snr,
-            "k": kd, "j0": j0, "N": Nn}
+            "k": kd, "j0": j0, "N": Nn, "track_offset": int(track_offset)}
 
 
 def search_batch(csd_maps, sigma_maps, seeds, f_min, df, n_tracks, n_min, n_max, **kw):
@@ -230,7 +230,7 @@ def top_k(result, k):
     at.  Plain sort of the dumped SNR array.  Returns [(track, tau_index, snr)]."""
     snr = result["snr"]
     n_tracks, n_tau = snr.shape
-    first = result.get("track_offset", 0)
+    first = result["track_offset"]                     # ids are global: row q of the dump is template first + q
     flat = snr.ravel()
     ids = np.repeat(np.arange(n_tracks, dtype=np.int64), n_tau)
     ms = np.tile(np.arange(n_tau, dtype=np.int64), n_tracks)

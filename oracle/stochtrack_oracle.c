@@ -29,10 +29,15 @@
  *                      720 us / 72 us, periodicity / rotation / shift invariants (P3-P6)
  *   or_search        : injected-track self recovery, null variance, chunk combination,
  *                      histogram total (P7-P10)
- *   or_track_params  : "parity unpinned" beyond its stated ranges/uniformity: the
- *                      word -> parameter maps are conventions (G3, G4), pinned only by
- *                      being written down in DESIGN.md; their statistical properties
- *                      (ranges, means, t_start < t_mid < t_end) are tested.
+ *   or_track_params  : what the text fixes (PAPER.md:75 durations >= t_min and t_start < t_mid
+ *                      < t_end, :86 six independent random numbers, :100 a uniform, independent
+ *                      delay; configs[0] full-duration templates) as statistical statements
+ *                      on its output: both end values of N and of j0 | N attained, chi-square
+ *                      uniformity of N and of j0 given N, KS uniformity of a/N, y/n_f, tau,
+ *                      pairwise independence of all seven parameters
+ *                      (tests/test_oracle_track_params_pins.py, which also rebuilds this file
+ *                      with eight plausible slips and requires every one to fail).  Which
+ *                      Philox word feeds which parameter remains a convention (G5).
  */
 #include <math.h>
 #include <stdint.h>

@@ -6,8 +6,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# ST_LIB_PATH selects another build of the same C ABI (e.g. a tuning variant)
-_LIB_PATH = os.environ.get("ST_LIB_PATH") or os.path.join(_HERE, "libstochtrack_b200.so")
+_LIB_PATH = os.path.join(_HERE, "libstochtrack_b200.so")
 
 ST_OK, ST_EINVAL, ST_ESTATE, ST_ENOSPC, ST_ECUDA = 0, -1, -2, -3, -4
 _CODES = {ST_EINVAL: "ST_EINVAL", ST_ESTATE: "ST_ESTATE", ST_ENOSPC: "ST_ENOSPC", ST_ECUDA: "ST_ECUDA"}
@@ -83,11 +82,16 @@ def library_path():
     return _LIB_PATH
 
 
-def load_library():
-    """dlopen the C-ABI library.  Fails loudly when it has not been built."""
-    global _lib
+def load_library(path=None):
+    """dlopen the C-ABI library.  Fails loudly when it has not been built.  `path` (first call only) names
+    another build of the same C ABI, e.g. the -DST_CHECKED library of build.build_checked()."""
+    global _lib, _LIB_PATH
     if _lib is not None:
+        if path is not None and os.path.abspath(path) != os.path.abspath(_LIB_PATH):
+            raise RuntimeError(f"a different library is already loaded: {_LIB_PATH}")
         return _lib
+    if path is not None:
+        _LIB_PATH = path
     if not os.path.exists(_LIB_PATH):
         raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_1401_8060_b200.build` "
                           "(there is no CPU fallback)")

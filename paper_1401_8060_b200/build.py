@@ -1,6 +1,6 @@
 """Build the C-ABI shared library (hand-written CUDA, sm_100a only) in-tree.
 
-    python -m paper_1401_8060_b200.build [--force]
+    python -m paper_1401_8060_b200.build [--force] [--checked | --microbench]
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the
 GPU box with the repo snapshot.
@@ -47,8 +47,16 @@ def build_checked(force=False):
     return LIB_CHECKED
 
 
+def build_microbench(force=False):
+    """The issue-rate / gather-rate microbenchmarks behind profiles/microbench_*.md (not part of the library)."""
+    micro_src = os.path.join(CSRC, "st_microbench.cu")
+    if force or _stale(MICRO, [micro_src]):
+        subprocess.check_call([_nvcc(), *NVCC_FLAGS, "-o", MICRO, micro_src])
+    return MICRO
+
+
 def build(force=False, verbose=False):
-    """Compile libstochtrack_b200.so (and the microbenchmark binary). Returns the .so path."""
+    """Compile libstochtrack_b200.so. Returns the .so path."""
     srcs = [os.path.join(CSRC, s) for s in SOURCES]
     deps = srcs + [os.path.join(CSRC, h) for h in HEADERS]
     if force or _stale(LIB, deps):
@@ -57,14 +65,13 @@ def build(force=False, verbose=False):
             cmd.insert(1, "-Xptxas=-v")
             print(" ".join(cmd))
         subprocess.check_call(cmd)
-    micro_src = os.path.join(CSRC, "st_microbench.cu")
-    if os.path.exists(micro_src) and (force or _stale(MICRO, [micro_src])):
-        subprocess.check_call([_nvcc(), *NVCC_FLAGS, "-o", MICRO, micro_src])
     return LIB
 
 
 if __name__ == "__main__":
     if "--checked" in sys.argv:
         print(build_checked(force="--force" in sys.argv))
+    elif "--microbench" in sys.argv:
+        print(build_microbench(force="--force" in sys.argv))
     else:
         print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

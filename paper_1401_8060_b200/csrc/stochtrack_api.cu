@@ -594,8 +594,6 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512;
     c->err[0] = 0;
     c->cheb_stride = 0; c->pick_valid = false; c->pick_dtau = 0.0; c->pick_stride = 0;
-    const char* e = getenv("ST_RECUR_THREADS");
-    if (e) { int t = atoi(e); if (t >= 32 && t <= 1024 && t % 32 == 0) c->recur_threads = t; }
     *out = c;
     return ST_OK;
 }

@@ -16,6 +16,7 @@ import json, sys
 import numpy as np, torch
 sys.path.insert(0, %(root)r)
 import paper_1401_8060_b200 as P
+P.load_library(%(lib)r)
 from workloads import synth
 out = {}
 for cid, n in ((1, 1000), (2, 20000), (3, 30000), (5, 3000)):
@@ -42,13 +43,8 @@ print(json.dumps(out))
 
 
 def _run(lib_path):
-    env = dict(os.environ)
-    if lib_path:
-        env["ST_LIB_PATH"] = lib_path
-    else:
-        env.pop("ST_LIB_PATH", None)
-    out = subprocess.run([sys.executable, "-c", SCRIPT % {"root": ROOT}], capture_output=True, text=True, timeout=600,
-                         cwd=ROOT, env=env)
+    out = subprocess.run([sys.executable, "-c", SCRIPT % {"root": ROOT, "lib": lib_path}], capture_output=True, text=True,
+                         timeout=600, cwd=ROOT)
     assert out.returncode == 0, out.stderr[-3000:]
     return json.loads(out.stdout.strip().splitlines()[-1])
 
@@ -60,6 +56,6 @@ def test_checked_build_trips_no_assertion_and_matches_production():
     build.build()
     checked = build.build_checked()
     got = _run(checked)
-    want = _run(None)
+    want = _run(build.LIB)
     assert got == want
     assert len(got) >= 12

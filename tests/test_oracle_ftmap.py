@@ -125,7 +125,7 @@ def test_F_ftmap_feeds_the_search_oracle(orc):
 def test_F_timeshift_zero_is_identity_and_shift_destroys_coherence():
     """G23: shift 0 reproduces the unshifted map; a whole-segment shift of detector J leaves the noise
     statistics unchanged but removes a transient that is coherent between the detectors (the point of
-    a time-shift background, PAPER.md:165); shifting by n_t is the identity (cyclic)."""
+    a time-shift background, PAPER.md:173); shifting by n_t is the identity (cyclic)."""
     rng = np.random.default_rng(8)
     fs, L, n_t, n_f = 256.0, 256, 60, 80
     n = int(L / 2 * (n_t + 1))
