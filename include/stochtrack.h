@@ -175,6 +175,31 @@ typedef struct {
 int st_search_topk(st_ctx *ctx, const st_search_params *params, int32_t top_k, st_top_entry *top_out,
                    int32_t *n_out, st_result *result);
 
+/* st_search plus, for every template of the search, its maximum over the delays and the delay that attains
+ * it (a template "tries to guess ... the appropriate phase factor"): computed in
+ * the fused S4 epilogue of the scoring kernels, nothing is dumped.
+ *   snr_max_dev   : DEVICE float32 [n_tracks], max_m SNR(track_offset + q, m) as the kernel scored it
+ *   tau_index_dev : DEVICE int32   [n_tracks], the smallest delay index attaining it (0 in random mode)
+ * Decided in float32 (reading G24 of DESIGN.md): where two delays of one template tie to float32 accuracy
+ * the index may differ from a float64 evaluation; the value agrees within the G13 tolerance.
+ * Errors as st_search, plus ST_EINVAL for a NULL output.  Synchronous on return.                    */
+int st_search_track_max(st_ctx *ctx, const st_search_params *params, float *snr_max_dev,
+                        int32_t *tau_index_dev, st_result *out);
+
+/* Eq. 8 for EXPLICIT templates instead of bank members: the targeted use of the statistic
+ * (Eq. 5: a fixed set of clusters Gamma) and the parity export for track shapes the bank
+ * produces with vanishing probability (flat, near-flat, full-length).
+ *   tracks  : HOST [count] templates in the st_track parameterisation (1 <= N, 0 <= j0, j0 + N <= n_t,
+ *             0 < a < N, finite control points); in random mode each template's own `tau` is its delay
+ *   snr_dev : DEVICE float32 [count][n_tau] (n_tau = 1 in random mode), same scoring kernel as st_search
+ *             with the same params (tau grid / range, norm, kernel); n_tracks, track_offset, seed, n_min,
+ *             n_max and the histogram fields of params are ignored.
+ * Errors: ST_EINVAL (a template outside the map, count outside [0, ST_MAX_SCORE_TRACKS]), otherwise as
+ * st_search.  Synchronous on return.                                                               */
+#define ST_MAX_SCORE_TRACKS 4096
+int st_score_tracks(st_ctx *ctx, const st_search_params *params, const st_track *tracks, int32_t count,
+                    float *snr_dev);
+
 /* Batch / background mode (the background is estimated from many
  * time-shifted maps, every one searched with its own template bank; BASELINE.json configs[3]):
  * S0-S4 over n_maps maps in ONE call.  Map m is searched exactly as
@@ -244,6 +269,11 @@ int st_track_params(const st_ctx *ctx, uint64_t seed, uint64_t track_id,
  * Uses params->seed, n_min, n_max.                                             */
 int st_debug_rasterise(st_ctx *ctx, const st_search_params *params, uint64_t first, uint64_t count,
                        int32_t *k_out_dev, int32_t *j0_dev, int32_t *N_dev);
+/* The same export through the random-delay kernel's OWN rasteriser (its fast path evaluates Eq. 6 in
+ * Horner form and regenerates the template on the normative fallback): runs k_score_random over ids
+ * [first, first+count) with params (ST_TAU_RANDOM) and writes the bins it used.  Needs a map.        */
+int st_debug_rasterise_random(st_ctx *ctx, const st_search_params *params, uint64_t first, uint64_t count,
+                              int32_t *k_out_dev, int32_t *j0_dev, int32_t *N_dev);
 /* Rasterise one explicit template (HOST st_track in, DEVICE int32 [N] out).    */
 int st_debug_rasterise_track(st_ctx *ctx, const st_track *track, int32_t *k_out_dev);
 /* snr_dev float32 [count][n_tau] (n_tau = 1 in random mode): every SNR(i, tau)

@@ -18,7 +18,8 @@ KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random",
 
 # every symbol include/stochtrack.h declares
 exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_workspace", "st_set_map",
-                    "st_set_map_host", "st_search", "st_search_topk", "st_search_batch", "st_ftmap_scratch_bytes", "st_set_map_from_strain", "st_search_timeshifts",
+                    "st_set_map_host", "st_search", "st_search_topk", "st_search_batch", "st_search_track_max",
+                    "st_score_tracks", "st_debug_rasterise_random", "st_ftmap_scratch_bytes", "st_set_map_from_strain", "st_search_timeshifts",
                     "st_debug_get_map",
                     "st_track_params", "st_debug_rasterise",
                     "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words",
@@ -61,6 +62,7 @@ class CTopEntry(C.Structure):
 
 
 MAX_TOP_K = 4096
+MAX_SCORE_TRACKS = 4096
 
 
 class CFtmapParams(C.Structure):
@@ -130,6 +132,12 @@ def load_library(path=None):
     L.st_debug_get_map.argtypes = [vp, vp]
     L.st_debug_get_map.restype = C.c_int
     L.st_search_batch.argtypes = [vp, C.POINTER(CBatch), C.POINTER(CSearchParams), C.POINTER(CResult), C.POINTER(C.c_float)]
+    L.st_search_track_max.argtypes = [vp, C.POINTER(CSearchParams), vp, vp, C.POINTER(CResult)]
+    L.st_search_track_max.restype = C.c_int
+    L.st_score_tracks.argtypes = [vp, C.POINTER(CSearchParams), C.POINTER(CTrack), C.c_int32, vp]
+    L.st_score_tracks.restype = C.c_int
+    L.st_debug_rasterise_random.argtypes = [vp, C.POINTER(CSearchParams), C.c_uint64, C.c_uint64, vp, vp, vp]
+    L.st_debug_rasterise_random.restype = C.c_int
     for name in ("st_create", "st_set_workspace", "st_set_map", "st_set_map_host", "st_search", "st_search_batch", "st_track_params",
                  "st_debug_rasterise", "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words"):
         getattr(L, name).restype = C.c_int
@@ -336,6 +344,38 @@ class Stochtrack:
         self._check(self._L.st_search(self._ctx, C.byref(p), C.byref(r)))
         return self._result(r, hist)
 
+    def search_track_max(self, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=None, norm=NORM_SQRT_N,
+                         n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO):
+        """st_search_track_max: the search result plus, per template, its maximum over the delays and the delay
+        index attaining it.  Returns (SearchResult, snr_max float32 [n_tracks], tau_index int32 [n_tracks])."""
+        torch = self._torch
+        p, keep = self._params(n_tracks, seed, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
+                               track_offset, kernel)
+        hist = None
+        if n_bins > 0:
+            hist = np.zeros(n_bins, dtype=np.uint64)
+            p.hist_out = hist.ctypes.data_as(C.POINTER(C.c_uint64))
+        snr = torch.empty(max(int(n_tracks), 1), dtype=torch.float32, device=self.device)
+        idx = torch.empty(max(int(n_tracks), 1), dtype=torch.int32, device=self.device)
+        r = CResult()
+        self._check(self._L.st_search_track_max(self._ctx, C.byref(p), snr.data_ptr(), idx.data_ptr(), C.byref(r)))
+        return self._result(r, hist), snr[:int(n_tracks)].cpu().numpy(), idx[:int(n_tracks)].cpu().numpy()
+
+    def score_tracks(self, tracks, tau_grid=None, tau_range=None, norm=NORM_SQRT_N, kernel=KERNEL_AUTO):
+        """st_score_tracks: Eq. 8 for explicit templates.  tracks: sequence of (N, j0, a, y0, y1, y2[, tau]).
+        Returns float32 [count][n_tau] (n_tau = 1 in random mode, where each template's own tau is its delay)."""
+        torch = self._torch
+        n = len(tracks)
+        arr = (CTrack * max(n, 1))()
+        for i, t in enumerate(tracks):
+            arr[i] = CTrack(int(t[0]), int(t[1]), float(t[2]), float(t[3]), float(t[4]), float(t[5]),
+                            float(t[6]) if len(t) > 6 else 0.0)
+        p, keep = self._params(n, 0, 1, 1, tau_grid, tau_range if tau_range is not None else (0.0, 0.0), norm, 0, -10.0, 10.0, 0, kernel)
+        n_tau = p.n_tau if p.tau_mode == TAU_GRID else 1
+        snr = torch.empty((max(n, 1), n_tau), dtype=torch.float32, device=self.device)
+        self._check(self._L.st_score_tracks(self._ctx, C.byref(p), arr, n, snr.data_ptr()))
+        return snr[:n].cpu().numpy()
+
     def search_topk(self, top_k, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=None, norm=NORM_SQRT_N,
                     n_bins=1000, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO):
         """The top_k loudest (template, delay) samples (st_search_topk).  Returns (SearchResult, list of
@@ -437,6 +477,18 @@ class Stochtrack:
         N = torch.empty(count, dtype=torch.int32, device=self.device)
         self._check(self._L.st_debug_rasterise(self._ctx, C.byref(p), int(first), int(count), k.data_ptr(),
                                                j0.data_ptr(), N.data_ptr()))
+        self.synchronize()
+        return k.cpu().numpy(), j0.cpu().numpy(), N.cpu().numpy()
+
+    def debug_rasterise_random(self, seed, n_min, n_max, first, count, tau_range=(-0.01, 0.01)):
+        """Bins decided by the random-delay kernel's own rasteriser (st_debug_rasterise_random)."""
+        torch = self._torch
+        p, _ = self._params(count, seed, n_min, n_max, None, tau_range, 0, 0, -10, 10, 0, 0)
+        k = torch.empty((count, self.n_t), dtype=torch.int32, device=self.device)
+        j0 = torch.empty(count, dtype=torch.int32, device=self.device)
+        N = torch.empty(count, dtype=torch.int32, device=self.device)
+        self._check(self._L.st_debug_rasterise_random(self._ctx, C.byref(p), int(first), int(count), k.data_ptr(),
+                                                      j0.data_ptr(), N.data_ptr()))
         self.synchronize()
         return k.cpu().numpy(), j0.cpu().numpy(), N.cpu().numpy()
 

@@ -88,7 +88,8 @@ struct ScoreArgs {
     Scalars* sc;
     Cand* cand;
     uint32_t cand_cap;
-    WarpBest* warp_best;
+    WarpBest* warp_best;      // [warp_slots] one record per resident warp of a launch
+    uint32_t warp_slots;
     unsigned long long* hist; // [n_bins] global counts
     int32_t n_bins;
     float hist_lo, hist_scale;
@@ -96,7 +97,41 @@ struct ScoreArgs {
     int32_t pool_stride;      // pixels of pool space per warp (>= n_max, multiple of 32)
     int32_t capture_mode;     // top-K second pass: keep every sample with SNR >= capture_thr, nothing else
     float capture_thr;
+    const Track* tracks;      // explicit templates [n_tracks] (st_score_tracks) or null: template q = make_track(seed, id)
+    float* tmax_snr;          // per-template maximum over the delays [n_tracks] (st_search_track_max) or null
+    int32_t* tmax_m;          // its delay index [n_tracks]
+    int32_t* k_dump;          // parity export of k_score_random's own rasteriser: [n_tracks][n_t] (pre-filled with -1)
+    int32_t* j0_dump;         //   with [n_tracks] first columns
+    int32_t* N_dump;          //   and [n_tracks] durations
 };
+
+// Template q of the launch: regenerated from (seed, id), or read from the caller's explicit list.
+__device__ __forceinline__ Track load_track(const ScoreArgs& a, uint64_t q, uint64_t id)
+{
+    return a.tracks ? a.tracks[q] : make_track(a.bp, id);
+}
+
+// Per-template maximum over the delays (the delay that "minimises the timing error" of a
+// template), G12 order inside a template: larger float32 SNR, then smaller delay index.
+struct TrackMax { float v; int32_t m; };
+__device__ __forceinline__ void tmax_init(TrackMax& t) { t.v = -INFINITY; t.m = 0x7FFFFFFF; }
+template <int NV>
+__device__ __forceinline__ void tmax_update(TrackMax& t, const float (&v)[NV], const uint32_t (&m)[NV], const bool (&ok)[NV])
+{
+#pragma unroll
+    for (int i = 0; i < NV; ++i)
+        if (ok[i] && (v[i] > t.v || (v[i] == t.v && (int32_t)m[i] < t.m))) { t.v = v[i]; t.m = (int32_t)m[i]; }
+}
+__device__ __forceinline__ void tmax_finish(const ScoreArgs& a, TrackMax t, uint64_t q)
+{
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        const float ov = __shfl_xor_sync(kFull, t.v, off);
+        const int32_t om = __shfl_xor_sync(kFull, t.m, off);
+        if (ov > t.v || (ov == t.v && om < t.m)) { t.v = ov; t.m = om; }
+    }
+    if ((threadIdx.x & 31) == 0) { a.tmax_snr[q] = t.v; a.tmax_m[q] = t.m; }
+}
 
 // ------------------------------------------------------------------ helpers --
 __device__ __forceinline__ uint32_t enc_f32(float f)
@@ -230,6 +265,7 @@ __device__ __forceinline__ void reduce_finish(const ScoreArgs& a, WarpReduce& wr
         if (wr.pixels) atomicAdd(&a.sc->n_pixels, wr.pixels);
         if (wr.best.valid) {
             const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+            ST_ASSERT(gw < a.warp_slots);       // the host clamps every grid to warp_slots resident warps
             WarpBest cur = a.warp_best[gw];     // slot owned by this warp across launches
             if (!cur.valid || better(wr.best.snr, wr.best.id, wr.best.m, cur.snr, cur.id, cur.m))
                 a.warp_best[gw] = wr.best;
@@ -404,7 +440,7 @@ __global__ void __launch_bounds__(256) k_score_table(const ScoreArgs a)
         const uint64_t q = next_track(a);
         if (q >= a.n_tracks) break;
         const uint64_t id = a.track_offset + q;
-        const Track t = make_track(a.bp, id);
+        const Track t = load_track(a, q, id);
         const Raster r = make_raster(t, a.bp.n_f);
         for (int c = lane; c < t.N; c += kWarp) {
             const int k = raster_bin_fast(r, c);
@@ -414,6 +450,8 @@ __global__ void __launch_bounds__(256) k_score_table(const ScoreArgs a)
         __syncwarp();
         wr.pixels += (unsigned long long)t.N;
         const float scale = norm_scale(t.N, a.norm);
+        TrackMax tm;
+        tmax_init(tm);
         for (int mb = 0; mb < a.n_tau; mb += kWarp) {
             const int m = mb + lane;
             const int mm = m < a.n_tau ? m : a.n_tau - 1;
@@ -430,7 +468,9 @@ __global__ void __launch_bounds__(256) k_score_table(const ScoreArgs a)
             const uint32_t ms[1] = {(uint32_t)m};
             const bool ok[1] = {m < a.n_tau};
             reduce_samples<1>(a, wr, sm_hist, id, q, v, ms, ok);
+            tmax_update<1>(tm, v, ms, ok);
         }
+        if (a.tmax_snr) tmax_finish(a, tm, q);
         __syncwarp();
     }
     reduce_finish(a, wr);
@@ -476,6 +516,7 @@ __device__ __forceinline__ void reduce_samples_multi(const ScoreArgs& a, WarpRed
             atomicAdd(&sm_hist[b], 1u);
         }
         if (a.dump) a.dump[q] = v;
+        if (a.tmax_snr) { a.tmax_snr[q] = v; a.tmax_m[q] = 0; }     // one delay per template: it is its own maximum
     }
     float wmax = valid ? v : -INFINITY;
 #pragma unroll
@@ -513,7 +554,9 @@ __device__ __forceinline__ void reduce_samples_multi(const ScoreArgs& a, WarpRed
 #ifndef ST_RANDOM_MIN_BLOCKS
 #define ST_RANDOM_MIN_BLOCKS 3
 #endif
-template <bool CAPTURE>
+// KDUMP: parity export -- the bins this kernel's own fast path (Horner form, regenerate-on-fallback) decides
+// are written to a.k_dump next to the scores (st_debug_rasterise_random).
+template <bool CAPTURE, bool KDUMP>
 __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -534,7 +577,7 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
         const uint64_t q = q0 + (uint64_t)grp;
         const bool live = q < a.n_tracks;                    // the last claim may be ragged
         const uint64_t id = a.track_offset + (live ? q : q0);
-        const Track t = make_track(a.bp, id);
+        const Track t = load_track(a, live ? q : q0, id);
         const RasterFast r = make_raster_fast(t, a.bp.n_f);
         const int N = live ? t.N : 0;
         int n_max = N;
@@ -558,7 +601,13 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
             if (redo[0] | redo[1] | redo[2] | redo[3]) {  // ~1e-5 of the time: normative sequence
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
-                    if (redo[u]) kq[u] = raster_bin_regen(a.bp, id, cq[u]);
+                    if (redo[u]) kq[u] = raster_bin(make_raster(load_track(a, live ? q : q0, id), a.bp.n_f), cq[u]);
+            }
+            if (KDUMP) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (c0 + u * kRandGroup < N) a.k_dump[q * (uint64_t)a.bp.n_t + (uint64_t)cq[u]] = kq[u];
+                if (live && sub == 0) { a.j0_dump[q] = t.j0; a.N_dump[q] = t.N; }
             }
             float2 pv[4];
 #pragma unroll
@@ -630,8 +679,10 @@ __global__ void __launch_bounds__(512, 1) k_score_recur(const ScoreArgs a)
         const uint64_t q = next_track(a);
         if (q >= a.n_tracks) break;
         const uint64_t id = a.track_offset + q;
-        const Track t = make_track(a.bp, id);
+        const Track t = load_track(a, q, id);
         const Raster r = make_raster(t, a.bp.n_f);
+        TrackMax tm;
+        tmax_init(tm);
         // ---- phase A: rasterise, gather, rotate to tau_0
         const int n_pad = (t.N + 63) & ~63;          // pairs of 32-pixel rows
 #pragma unroll 2
@@ -710,8 +761,10 @@ __global__ void __launch_bounds__(512, 1) k_score_recur(const ScoreArgs a)
                 v[i] = acc[i] * scale;
             }
             reduce_samples<NV>(a, wr, sm_hist, id, q, v, ms, ok);
+            tmax_update<NV>(tm, v, ms, ok);
             __syncwarp();
         }
+        if (a.tmax_snr) tmax_finish(a, tm, q);
     }
     reduce_finish(a, wr);
     hist_flush(sm_hist, a.hist, a.n_bins);
@@ -811,8 +864,10 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
         const uint64_t q = next_track(a);
         if (q >= a.n_tracks) break;
         const uint64_t id = a.track_offset + q;
-        const Track t = make_track(a.bp, id);
+        const Track t = load_track(a, q, id);
         const Raster r = make_raster(t, a.bp.n_f);
+        TrackMax tm;
+        tmax_init(tm);
         const int n_prows = (t.N + 63) >> 6;         // packed rows: columns [64 pr, 64 pr + 64)
         wr.pixels += (unsigned long long)t.N;
         const float scale = norm_scale(t.N, a.norm);
@@ -931,7 +986,9 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
             const uint32_t ms[1] = {(uint32_t)(j * kChunk + lane)};
             const bool ok[1] = {(int)ms[0] < a.n_tau};
             reduce_samples<1>(a, wr, sm_hist, id, q, v, ms, ok);
+            tmax_update<1>(tm, v, ms, ok);
         }
+        if (a.tmax_snr) tmax_finish(a, tm, q);
     }
     reduce_finish(a, wr);
     hist_flush(sm_hist, a.hist, a.n_bins);
@@ -1126,13 +1183,16 @@ __device__ __forceinline__ int cheb_phase_a(const ScoreArgs& a, const Track& t, 
 
 // Phase B for one template whose merged pixels sit in (pool_v, pool_k): every delay of the grid,
 // fused S4.  pool_v is advanced in place from chunk to chunk.
-template <int STRIDE, bool CAPTURE>
+// MODE 0: search; 1: capture pass of st_search_topk; 2: search + per-template maximum over the delays
+template <int STRIDE, int MODE>
 __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr, uint32_t* sm_hist,
                                              const float4* sm_tab, const float* sm_zi, float2* pool_v,
                                              const uint16_t* pool_k, const int n_merged, const float scale,
                                              const uint64_t id, const uint64_t q, const int n_chunks, const int lane)
 {
     const int n_rows = (n_merged + kWarp - 1) >> 5;
+    TrackMax tm;
+    tmax_init(tm);
     // ---- phase B: chunks of 64 delays; f2[i] = (sum x_{mc+i}, sum x_{mc-1-i}) over this lane's pixels
 #pragma unroll 1
     for (int j = 0; j < n_chunks; ++j) {
@@ -1235,11 +1295,13 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
     const float v[2] = {pk_lo(f2[0]) * sscale, pk_hi(f2[0]) * sscale};
         const uint32_t ms[2] = {(uint32_t)(j * kCheb + kHalf + lane), (uint32_t)(j * kCheb + kHalf - 1 - lane)};
         const bool ok[2] = {(int)ms[0] < a.n_tau, (int)ms[1] < a.n_tau};
-        reduce_samples<2, CAPTURE ? 1 : 0>(a, wr, sm_hist, id, q, v, ms, ok);
+        reduce_samples<2, MODE == 1 ? 1 : 0>(a, wr, sm_hist, id, q, v, ms, ok);
+        if (MODE == 2) tmax_update<2>(tm, v, ms, ok);
     }
+    if (MODE == 2) tmax_finish(a, tm, q);
 }
 
-template <int STRIDE, bool CAPTURE>
+template <int STRIDE, int MODE>
 __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -1266,12 +1328,12 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
         if (q >= a.n_tracks) break;
         if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
         const uint64_t id = a.track_offset + q;
-        const Track t = make_track(a.bp, id);
+        const Track t = load_track(a, q, id);
         wr.pixels += (unsigned long long)t.N;
         const int n_merged = cheb_phase_a(a, t, pool_v, pool_k, lane);
         ST_ASSERT(n_merged >= 1 && n_merged <= t.N && ((n_merged + kWarp - 1) & ~(kWarp - 1)) <= S &&
-                  t.N >= a.bp.n_min && t.N <= a.bp.n_max && t.j0 >= 0 && t.j0 + t.N <= a.bp.n_t);
-        cheb_phase_b<STRIDE, CAPTURE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, n_merged, norm_scale(t.N, a.norm), id, q,
+                  (a.tracks || (t.N >= a.bp.n_min && t.N <= a.bp.n_max)) && t.j0 >= 0 && t.j0 + t.N <= a.bp.n_t);
+        cheb_phase_b<STRIDE, MODE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, n_merged, norm_scale(t.N, a.norm), id, q,
                              n_chunks, lane);
     }
     reduce_finish(a, wr);

@@ -27,7 +27,7 @@ constexpr uint64_t kMaxSamplesPerLaunch = 1ull << 31;   // keeps per-block u32 h
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t map, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, cand64, warp_best, stage_csd, stage_sigma, stage_csd2, stage_sigma2, b_scalars, b_result, b_hist, total;
+    size_t map, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, cand64, warp_best, stage_csd, stage_sigma, stage_csd2, stage_sigma2, b_scalars, b_result, b_hist, tracks, total;
 };
 
 Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
@@ -59,6 +59,7 @@ Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
     L.b_scalars = o;    o += align_up((size_t)ST_BATCH_GROUP * sizeof(st::Scalars));
     L.b_result = o;     o += align_up((size_t)ST_BATCH_GROUP * sizeof(st::DeviceResult));
     L.b_hist = o;       o += align_up((size_t)ST_BATCH_GROUP * (size_t)ST_MAX_BINS * sizeof(unsigned long long));
+    L.tracks = o;       o += align_up((size_t)ST_MAX_SCORE_TRACKS * sizeof(st::Track));
     L.total = o;
     return L;
 }
@@ -87,6 +88,7 @@ struct st_ctx {
     st::DeviceResult* h_res;           // pinned
     unsigned long long* h_hist;        // pinned, ST_MAX_BINS
     int n_sm, smem_optin;
+    int device;                        // ordinal of the device the workspace lives on (every call runs there)
     int recur_threads;                 // tunable: threads per block of the recurrence kernels
     int cheb_stride;                   // stride of the tables currently on the device
     bool pick_valid; double pick_dtau; int pick_stride;   // memo of cheb_pick_stride
@@ -106,6 +108,17 @@ int fail(st_ctx* c, int code, const char* fmt, ...)
     }
     return code;
 }
+
+// Every device entry point runs on the workspace's device, whatever device is current in the calling thread.
+struct DevGuard {
+    int prev; bool switched;
+    explicit DevGuard(const st_ctx* c) : prev(-1), switched(false)
+    {
+        if (c && c->have_ws && cudaGetDevice(&prev) == cudaSuccess && prev != c->device)
+            switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DevGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 #define ST_CUDA(ctx, call)                                                                   \
     do {                                                                                     \
@@ -369,8 +382,10 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         uint64_t blocks = (uint64_t)c->n_sm * 8;
         const uint64_t need = ((want_warps + st::kRandPerWarp - 1) / st::kRandPerWarp + 7) / 8;   // a warp scores kRandPerWarp templates at a time
         if (blocks > need) blocks = need;
-        if (a.capture_mode) st::k_score_random<true><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
-        else st::k_score_random<false><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        if (blocks > kWarpSlots / 8) blocks = kWarpSlots / 8;         // one per-warp record slot per resident warp
+        if (a.k_dump) st::k_score_random<false, true><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        else if (a.capture_mode) st::k_score_random<true, false><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        else st::k_score_random<false, false><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
     } else if (plan.kernel == ST_KERNEL_TABLE) {
         int threads = 256;
         size_t smem;
@@ -386,6 +401,7 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         uint64_t blocks = (uint64_t)c->n_sm * (uint64_t)per_sm;
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
+        if (blocks > kWarpSlots / (uint64_t)(threads / 32)) blocks = kWarpSlots / (uint64_t)(threads / 32);
         st::k_score_table<<<(unsigned)blocks, threads, smem, c->stream>>>(a);
     } else if (plan.kernel == ST_KERNEL_CHEBYSHEV) {
         int threads = c->recur_threads;
@@ -401,14 +417,15 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
-#define ST_LAUNCH_CHEB(STRIDE, CAPTURE)                                                           \
+#define ST_LAUNCH_CHEB(STRIDE, MODE)                                                              \
     do {                                                                                          \
-        int rc_ = set_smem(c, st::k_score_cheb<STRIDE, CAPTURE>, smem);                           \
+        int rc_ = set_smem(c, st::k_score_cheb<STRIDE, MODE>, smem);                              \
         if (rc_) return rc_;                                                                      \
-        st::k_score_cheb<STRIDE, CAPTURE><<<(unsigned)blocks, threads, smem, c->stream>>>(a);     \
+        st::k_score_cheb<STRIDE, MODE><<<(unsigned)blocks, threads, smem, c->stream>>>(a);        \
     } while (0)
-        if (pk) { if (a.capture_mode) ST_LAUNCH_CHEB(2, true); else ST_LAUNCH_CHEB(2, false); }
-        else    { if (a.capture_mode) ST_LAUNCH_CHEB(1, true); else ST_LAUNCH_CHEB(1, false); }
+        const int mode = a.capture_mode ? 1 : (a.tmax_snr ? 2 : 0);
+        if (pk) { if (mode == 1) ST_LAUNCH_CHEB(2, 1); else if (mode == 2) ST_LAUNCH_CHEB(2, 2); else ST_LAUNCH_CHEB(2, 0); }
+        else    { if (mode == 1) ST_LAUNCH_CHEB(1, 1); else if (mode == 2) ST_LAUNCH_CHEB(1, 2); else ST_LAUNCH_CHEB(1, 0); }
 #undef ST_LAUNCH_CHEB
     } else if (plan.kernel == ST_KERNEL_REINSCH) {
         int threads = c->recur_threads;
@@ -478,6 +495,7 @@ st::ScoreArgs base_args(st_ctx* c, const st_search_params* p)
     a.cand = at<st::Cand>(c, c->L.cand);
     a.cand_cap = kCandCap;
     a.warp_best = at<st::WarpBest>(c, c->L.warp_best);
+    a.warp_slots = kWarpSlots;
     a.hist = at<unsigned long long>(c, c->L.hist);
     a.n_bins = 0; a.hist_lo = 0.0f; a.hist_scale = 0.0f;
     a.dump = nullptr;
@@ -517,7 +535,7 @@ int reset_search_state(st_ctx* c, int n_bins, const Slots& sl)
 
 // S1-S4 of one search, enqueued on the stream (no synchronisation): tables must be current.
 int enqueue_search(st_ctx* c, const st_search_params* p, const Plan& plan, const Slots& sl, int* n_launches,
-                   bool time_it);
+                   bool time_it, float* tmax_snr = nullptr, int32_t* tmax_m = nullptr);
 void fill_result(st_result* out, const st::DeviceResult& r, int n_tau, int kernel, int n_launches);
 
 void fill_result(st_result* out, const st::DeviceResult& r, int n_tau, int kernel, int n_launches)
@@ -533,7 +551,7 @@ void fill_result(st_result* out, const st::DeviceResult& r, int n_tau, int kerne
 }
 
 int enqueue_search(st_ctx* c, const st_search_params* p, const Plan& plan, const Slots& sl, int* n_launches,
-                   bool time_it)
+                   bool time_it, float* tmax_snr, int32_t* tmax_m)
 {
     const int n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
     int rc = reset_search_state(c, p->n_bins, sl);
@@ -549,6 +567,8 @@ int enqueue_search(st_ctx* c, const st_search_params* p, const Plan& plan, const
     for (uint64_t done = 0; done < p->n_tracks; done += per_launch) {
         a.track_offset = p->track_offset + done;
         a.n_tracks = p->n_tracks - done < per_launch ? p->n_tracks - done : per_launch;
+        a.tmax_snr = tmax_snr ? tmax_snr + done : nullptr;
+        a.tmax_m = tmax_m ? tmax_m + done : nullptr;
         rc = launch_score(c, plan, a, p->n_max);
         if (rc) return rc;
         ++*n_launches;
@@ -591,7 +611,7 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->ev0 = c->ev1 = nullptr; c->h_res = nullptr; c->h_hist = nullptr;
     c->copy_stream = nullptr; c->h_bres = nullptr; c->h_bhist = nullptr;
     for (int i = 0; i < 2; ++i) { c->ev_copied[i] = nullptr; c->ev_consumed[i] = nullptr; }
-    c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512;
+    c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512; c->device = 0;
     c->err[0] = 0;
     c->cheb_stride = 0; c->pick_valid = false; c->pick_dtau = 0.0; c->pick_stride = 0;
     *out = c;
@@ -633,12 +653,14 @@ int st_set_workspace(st_ctx* c, void* ws, size_t bytes, void* cuda_stream)
         const int mid = (lo + hi + 1) / 2;
         if (make_layout(c->n_t, c->n_f, mid).total <= bytes) lo = mid; else hi = mid - 1;
     }
-    int dev = 0;
-    ST_CUDA(c, cudaGetDevice(&dev));
     cudaPointerAttributes pa;
     ST_CUDA(c, cudaPointerGetAttributes(&pa, ws));
     if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)
         return fail(c, ST_EINVAL, "workspace is not device memory");
+    const int dev = pa.device;                      // the context lives on the workspace's device
+    c->device = dev; c->have_ws = true;             // (have_ws lets the guard below switch to it)
+    DevGuard dev_guard(c);
+    c->have_ws = false;
     ST_CUDA(c, cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev));
     ST_CUDA(c, cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     if (!c->ev0) ST_CUDA(c, cudaEventCreate(&c->ev0));
@@ -655,6 +677,7 @@ int st_set_workspace(st_ctx* c, void* ws, size_t bytes, void* cuda_stream)
 
 int st_set_map(st_ctx* c, const void* csd_dev, const float* sigma_dev, int32_t sigma_kind)
 {
+    DevGuard dev_guard(c);
     if (!c) return ST_EINVAL;
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
     if (!csd_dev) return fail(c, ST_EINVAL, "csd is NULL");
@@ -676,6 +699,7 @@ int st_set_map(st_ctx* c, const void* csd_dev, const float* sigma_dev, int32_t s
 
 int st_set_map_host(st_ctx* c, const void* csd_host, const float* sigma_host, int32_t sigma_kind)
 {
+    DevGuard dev_guard(c);
     if (!c) return ST_EINVAL;
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
     if (!csd_host) return fail(c, ST_EINVAL, "csd is NULL");
@@ -693,7 +717,23 @@ int st_set_map_host(st_ctx* c, const void* csd_host, const float* sigma_host, in
     return ST_OK;
 }
 
+static int search_impl(st_ctx* c, const st_search_params* p, st_result* out, float* tmax_snr, int32_t* tmax_m);
+
 int st_search(st_ctx* c, const st_search_params* p, st_result* out)
+{
+    DevGuard dev_guard(c);
+    return search_impl(c, p, out, nullptr, nullptr);
+}
+
+int st_search_track_max(st_ctx* c, const st_search_params* p, float* snr_max_dev, int32_t* tau_index_dev, st_result* out)
+{
+    DevGuard dev_guard(c);
+    if (!c) return ST_EINVAL;
+    if (!snr_max_dev || !tau_index_dev) return fail(c, ST_EINVAL, "per-template output pointer is NULL");
+    return search_impl(c, p, out, snr_max_dev, tau_index_dev);
+}
+
+static int search_impl(st_ctx* c, const st_search_params* p, st_result* out, float* tmax_snr, int32_t* tmax_m)
 {
     int rc = validate(c, p, true);
     if (rc) return rc;
@@ -714,7 +754,7 @@ int st_search(st_ctx* c, const st_search_params* p, st_result* out)
     rc = ensure_tables(c, p, plan, &n_launches);
     if (rc) return rc;
     const Slots sl = own_slots(c);
-    rc = enqueue_search(c, p, plan, sl, &n_launches, true);
+    rc = enqueue_search(c, p, plan, sl, &n_launches, true, tmax_snr, tmax_m);
     if (rc) return rc;
     ST_CUDA(c, cudaMemcpyAsync(c->h_res, sl.res, sizeof(st::DeviceResult), cudaMemcpyDeviceToHost, c->stream));
     if (p->n_bins > 0)
@@ -732,6 +772,7 @@ int st_search(st_ctx* c, const st_search_params* p, st_result* out)
 int st_search_topk(st_ctx* c, const st_search_params* p, int32_t top_k, st_top_entry* top_out, int32_t* n_out,
                    st_result* result)
 {
+    DevGuard dev_guard(c);
     if (!c) return ST_EINVAL;
     if (!p || !top_out || !n_out || !result) return fail(c, ST_EINVAL, "NULL argument");
     if (top_k < 1 || top_k > ST_MAX_TOP_K) return fail(c, ST_EINVAL, "top_k %d outside [1, %d]", top_k, ST_MAX_TOP_K);
@@ -750,7 +791,10 @@ int st_search_topk(st_ctx* c, const st_search_params* p, int32_t top_k, st_top_e
         return fail(c, ST_ENOSPC, "%llu samples at or above the bin of the top_k-th: histogram too coarse (cap %u)",
                     (unsigned long long)cum, kCandCap);
     const double width = (p->hist_hi - p->hist_lo) / (double)p->n_bins;
-    const float thr = b == 0 ? -INFINITY : (float)(p->hist_lo + (double)b * width - 1e-4 * width);
+    // the capture threshold sits below that edge by more than the float32 score error (relative 1e-4, the
+    // G13 tolerance, whatever the bin width): the final order is decided by the float64 re-score
+    const double edge = p->hist_lo + (double)b * width;
+    const float thr = b == 0 ? -INFINITY : (float)(edge - 1e-4 * width - 1e-4 * (fabs(edge) > 1.0 ? fabs(edge) : 1.0));
     // pass 2: capture
     Plan plan;
     rc = make_plan(c, p, &plan);
@@ -812,7 +856,22 @@ int st_search_topk(st_ctx* c, const st_search_params* p, int32_t top_k, st_top_e
     return ST_OK;
 }
 
+static int batch_impl(st_ctx* c, const st_batch* b, const st_search_params* p, st_result* results, float* gpu_ms_total);
+
 int st_search_batch(st_ctx* c, const st_batch* b, const st_search_params* p, st_result* results, float* gpu_ms_total)
+{
+    DevGuard dev_guard(c);
+    const int rc = batch_impl(c, b, p, results, gpu_ms_total);
+    if (rc && c && c->have_ws) {
+        // an error part-way through: host-to-device copies from the caller's buffers may still be in flight
+        // on the internal stream, and searches on the caller's; both drain before the buffers are handed back
+        if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
+        cudaStreamSynchronize(c->stream);
+    }
+    return rc;
+}
+
+static int batch_impl(st_ctx* c, const st_batch* b, const st_search_params* p, st_result* results, float* gpu_ms_total)
 {
     int rc = validate(c, p, false);
     if (rc) return rc;
@@ -972,6 +1031,7 @@ static int ft_normalise(st_ctx* c, const double2* st_i, const double2* st_j, int
 int st_set_map_from_strain(st_ctx* c, const double* s_i, const double* s_j, int64_t n_samples,
                            const st_ftmap_params* fp, void* scratch, size_t scratch_bytes)
 {
+    DevGuard dev_guard(c);
     if (!c) return ST_EINVAL;
     double2 *st_i = nullptr, *st_j = nullptr;
     int rc = ft_spectra(c, s_i, s_j, n_samples, fp, scratch, scratch_bytes, &st_i, &st_j);
@@ -983,6 +1043,7 @@ int st_search_timeshifts(st_ctx* c, const double* s_i, const double* s_j, int64_
                          void* scratch, size_t scratch_bytes, int32_t n_shifts, const int32_t* shifts,
                          const uint64_t* seeds, const st_search_params* p, st_result* results, float* gpu_ms_total)
 {
+    DevGuard dev_guard(c);
     int rc = validate(c, p, false);
     if (rc) return rc;
     if (!results || !shifts) return fail(c, ST_EINVAL, "shifts / results is NULL");
@@ -1046,6 +1107,7 @@ int st_search_timeshifts(st_ctx* c, const double* s_i, const double* s_j, int64_
 
 int st_debug_get_map(st_ctx* c, void* p_out_dev)
 {
+    DevGuard dev_guard(c);
     if (!c) return ST_EINVAL;
     if (!c->have_ws || !c->have_map) return fail(c, ST_ESTATE, "no map");
     if (!p_out_dev) return fail(c, ST_EINVAL, "output is NULL");
@@ -1078,6 +1140,7 @@ int st_debug_track_words(uint64_t seed, uint64_t track_id, uint32_t* out_host)
 int st_debug_rasterise(st_ctx* c, const st_search_params* p, uint64_t first, uint64_t count,
                        int32_t* k_out_dev, int32_t* j0_dev, int32_t* N_dev)
 {
+    DevGuard dev_guard(c);
     if (!c) return ST_EINVAL;
     if (!p) return fail(c, ST_EINVAL, "params is NULL");
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
@@ -1093,6 +1156,7 @@ int st_debug_rasterise(st_ctx* c, const st_search_params* p, uint64_t first, uin
 
 int st_debug_rasterise_track(st_ctx* c, const st_track* t, int32_t* k_out_dev)
 {
+    DevGuard dev_guard(c);
     if (!c) return ST_EINVAL;
     if (!t || !k_out_dev) return fail(c, ST_EINVAL, "NULL argument");
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
@@ -1104,8 +1168,73 @@ int st_debug_rasterise_track(st_ctx* c, const st_track* t, int32_t* k_out_dev)
     return ST_OK;
 }
 
+int st_debug_rasterise_random(st_ctx* c, const st_search_params* p, uint64_t first, uint64_t count,
+                              int32_t* k_out_dev, int32_t* j0_dev, int32_t* N_dev)
+{
+    DevGuard dev_guard(c);
+    int rc = validate(c, p, true);
+    if (rc) return rc;
+    if (p->tau_mode != ST_TAU_RANDOM) return fail(c, ST_EINVAL, "st_debug_rasterise_random needs ST_TAU_RANDOM");
+    if (!k_out_dev || !j0_dev || !N_dev) return fail(c, ST_EINVAL, "output pointer is NULL");
+    if (count == 0) return ST_OK;
+    if (count > kMaxSamplesPerLaunch) return fail(c, ST_EINVAL, "count too large for one debug launch");
+    Plan plan;
+    rc = make_plan(c, p, &plan);
+    if (rc) return rc;
+    rc = reset_search_state(c, 0, own_slots(c));
+    if (rc) return rc;
+    ST_CUDA(c, cudaMemsetAsync(k_out_dev, 0xFF, (size_t)count * (size_t)c->n_t * sizeof(int32_t), c->stream));   // -1 beyond N
+    st::ScoreArgs a = base_args(c, p);
+    a.track_offset = first; a.n_tracks = count;
+    a.k_dump = k_out_dev; a.j0_dump = j0_dev; a.N_dump = N_dev;
+    return launch_score(c, plan, a, p->n_max);
+}
+
+int st_score_tracks(st_ctx* c, const st_search_params* p, const st_track* tracks, int32_t count, float* snr_dev)
+{
+    DevGuard dev_guard(c);
+    if (!c) return ST_EINVAL;
+    if (!p) return fail(c, ST_EINVAL, "params is NULL");
+    if (!tracks || !snr_dev) return fail(c, ST_EINVAL, "tracks / snr_dev is NULL");
+    if (count < 0 || count > ST_MAX_SCORE_TRACKS) return fail(c, ST_EINVAL, "count %d outside [0, %d]", count, ST_MAX_SCORE_TRACKS);
+    if (count == 0) return ST_OK;
+    st_search_params q = *p;                         // the durations come from the list, not from params
+    q.n_min = c->n_t; q.n_max = 1; q.n_tracks = (uint64_t)count; q.track_offset = 0; q.n_bins = 0; q.hist_out = nullptr;
+    std::vector<st::Track> h((size_t)count);
+    for (int i = 0; i < count; ++i) {
+        const st_track& t = tracks[i];
+        if (t.N < 1 || t.j0 < 0 || (int64_t)t.j0 + (int64_t)t.N > (int64_t)c->n_t)
+            return fail(c, ST_EINVAL, "tracks[%d] lies outside the map", i);
+        if (!(t.a > 0.0) || !(t.a < (double)t.N) || !isfinite(t.y0) || !isfinite(t.y1) || !isfinite(t.y2) || !isfinite(t.tau))
+            return fail(c, ST_EINVAL, "tracks[%d]: need 0 < a < N and finite control points / delay", i);
+        h[(size_t)i].N = t.N; h[(size_t)i].j0 = t.j0; h[(size_t)i].a = t.a;
+        h[(size_t)i].y0 = t.y0; h[(size_t)i].y1 = t.y1; h[(size_t)i].y2 = t.y2; h[(size_t)i].tau = t.tau;
+        if (t.N < q.n_min) q.n_min = t.N;
+        if (t.N > q.n_max) q.n_max = t.N;
+    }
+    int rc = validate(c, &q, true);
+    if (rc) return rc;
+    Plan plan;
+    rc = make_plan(c, &q, &plan);
+    if (rc) return rc;
+    int n_launches = 0;
+    rc = ensure_tables(c, &q, plan, &n_launches);
+    if (rc) return rc;
+    rc = reset_search_state(c, 0, own_slots(c));
+    if (rc) return rc;
+    st::Track* d_tracks = at<st::Track>(c, c->L.tracks);
+    ST_CUDA(c, cudaMemcpyAsync(d_tracks, h.data(), (size_t)count * sizeof(st::Track), cudaMemcpyHostToDevice, c->stream));
+    st::ScoreArgs a = base_args(c, &q);
+    a.track_offset = 0; a.n_tracks = (uint64_t)count; a.dump = snr_dev; a.tracks = d_tracks;
+    rc = launch_score(c, plan, a, q.n_max);
+    if (rc) return rc;
+    ST_CUDA(c, cudaStreamSynchronize(c->stream));    // the pageable staging vector goes out of scope
+    return ST_OK;
+}
+
 int st_debug_scores(st_ctx* c, const st_search_params* p, uint64_t first, uint64_t count, float* snr_dev)
 {
+    DevGuard dev_guard(c);
     int rc = validate(c, p, true);
     if (rc) return rc;
     if (!snr_dev) return fail(c, ST_EINVAL, "snr_dev is NULL");

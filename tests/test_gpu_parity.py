@@ -612,3 +612,190 @@ def test_top_k_limits(P, orc):
     with pytest.raises(P.StError) as e:                 # one coarse bin holds everything: 1e5 x 16 samples > 65 536
         st.search_topk(10, 100000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=2, hist_lo=-50.0, hist_hi=50.0)
     assert e.value.code == -3
+
+
+# ------------------------------------------------------------------ round 2: holes named by the round-1 review
+def _oracle_tracks(orc, n_t, n_f, f_min, df, seed, n_min, n_max, first, count, tau_range=None):
+    p = np.zeros((n_t, n_f), dtype=np.complex128)
+    kw = dict(tau_range=tau_range) if tau_range is not None else dict(tau_grid=np.zeros(1))
+    return orc.search(p, f_min, df, count, seed, n_min, n_max, track_offset=first, dump_tracks=True, **kw)
+
+
+@pytest.mark.parametrize("n_t,n_f,f_min,seed,n_min,n_max,first,count", [
+    (500, 2461, 40.0, 2, 10, 500, 0, 100_000),                 # config 3
+    (500, 151, 100.0, 5, 70, 500, 7_000_000, 100_000),         # config P (Table III shape)
+    (64, 65535, 0.0, 77, 1, 64, 10 ** 12, 60_000),             # widest band the ABI allows
+    (4096, 2461, 0.0, 77, 3000, 4096, 10 ** 12, 600),          # long templates
+    (16, 7, 0.0, 77, 1, 16, 10 ** 12, 20_000)])                # tiny map
+def test_random_kernel_own_rasteriser_indices_bit_exact(P, orc, n_t, n_f, f_min, seed, n_min, n_max, first, count):
+    """k_score_random rasterises with its own fast path (Eq. 6 in Horner form, template regenerated on the
+    normative fallback) -- not the one st_debug_rasterise exports.  Its bins, dumped by the scoring kernel
+    itself, must equal the oracle's bit for bit (Eq. 6; G2, G15)."""
+    st = P.Stochtrack(n_t, n_f, 1.0, f_min, max_n_tau=64)
+    st.set_map(np.zeros((n_t, n_f), dtype=np.complex64))
+    step = 25_000
+    for off in range(0, count, step):
+        n = min(step, count - off)
+        k, j0, N = st.debug_rasterise_random(seed, n_min, n_max, first + off, n, tau_range=(-0.01, 0.01))
+        ref = _oracle_tracks(orc, n_t, n_f, f_min, 1.0, seed, n_min, n_max, first + off, n, tau_range=(-0.01, 0.01))
+        assert np.array_equal(N, ref["N"]) and np.array_equal(j0, ref["j0"])
+        assert np.array_equal(k, ref["k"])
+
+
+def test_top_k_at_a_large_track_offset(P, orc):
+    """Template ids are global: the K loudest samples of ids [2^33 + 5, ...) carry those ids on both sides."""
+    cfg = synth.CONFIGS[2]
+    csd, sigma, tau = config_inputs(orc, cfg, 0)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    first, n, k = 2 ** 33 + 5, 30_000, 20
+    r, top = st.search_topk(k, n, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=cfg.n_bins, track_offset=first)
+    ref = orc.search(orc.prepare_map(csd, sigma), cfg.f_min, cfg.df, n, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau,
+                     track_offset=first, dump_snr=True)
+    want = orc.top_k(ref, k)
+    assert min(w[0] for w in want) >= first
+    assert [(e["track"], e["tau_index"]) for e in top] == [w[:2] for w in want]
+    for e, w in zip(top, want):
+        assert abs(e["snr_f64"] - w[2]) <= 2e-7 * abs(w[2])
+    assert (top[0]["track"], top[0]["tau_index"]) == (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+
+
+FLAT_TRACKS = [      # (N, j0, a, y0, y1, y2): flat and near-flat full-length templates on the config-5 shape
+    (1000, 0, 500.0, 0.5, 0.5, 0.5),                 # flat in the lowest bin: every lane merges ~31 columns into one run
+    (1000, 0, 500.0, 1230.5, 1230.5, 1230.5),        # flat mid-band
+    (1000, 0, 137.0, 2460.5, 2460.5, 2460.5),        # flat in the top bin, t_mid off-centre
+    (1000, 0, 500.0, 100.1, 100.9, 101.7),           # near-flat: two bins over 1000 columns
+    (1000, 0, 900.0, 7.2, 9.9, 7.3),                 # near-flat with a turning point
+    (999, 1, 3.0, 2000.4, 2001.2, 1999.9),
+    (33, 500, 16.5, 40.5, 40.5, 40.5), (64, 936, 20.0, 1.5, 1.5, 2.5)]
+
+
+def _oracle_scores_explicit(orc, p, f_min, df, tracks, tau, norm=0):
+    W = orc.build_table(p.shape[1], f_min, df, tau)
+    out = []
+    for tr in tracks:
+        t = orc.make_track(*tr)
+        out.append(orc.score_table(p, t, orc.rasterise(t, p.shape[1]), W, norm))
+    return np.array(out)
+
+
+@pytest.mark.parametrize("kname", ["auto", "table", "rotation", "reinsch", "chebyshev"])
+def test_scores_flat_and_near_flat_full_length_explicit_tracks(P, orc, kname):
+    """Track shapes the random bank all but never draws: flat / near-flat full-length templates merge up to 32
+    columns per lane into one run before the rotation (float32 sum of p) -- scored through st_score_tracks by
+    the same kernels as a search and compared at every delay of the 512-point grid (G13)."""
+    cfg = synth.CONFIGS[5]
+    csd, sigma, tau = config_inputs(orc, cfg)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    p = orc.prepare_map(csd, sigma)
+    got = st.score_tracks(FLAT_TRACKS, tau_grid=tau, kernel=KERNELS.get(kname, 0))
+    ref = _oracle_scores_explicit(orc, p, cfg.f_min, cfg.df, FLAT_TRACKS, tau)
+    ok, worst = snr_close(got, ref)
+    assert ok, f"{kname}: worst error {worst:.3f} x tolerance"
+    # the paper's one-delay mode: each explicit template carries its own delay
+    taus = [-0.0093, 0.0, 0.004, 0.0099, -0.001, 0.0025, 0.0071, -0.0042]
+    got1 = st.score_tracks([tr + (x,) for tr, x in zip(FLAT_TRACKS, taus)], tau_range=(-0.01, 0.01))
+    ref1 = np.array([orc.score_direct(p, orc.make_track(*tr), orc.rasterise(orc.make_track(*tr), cfg.n_f), cfg.f_min, cfg.df, x)
+                     for tr, x in zip(FLAT_TRACKS, taus)])
+    ok, worst = snr_close(got1[:, 0], ref1)
+    assert ok, worst
+
+
+@pytest.mark.parametrize("kbin,snr", [(0, 10.0), (0, 16.0), (3, 12.0), (40, 10.0), (2460, 10.0)])
+def test_loud_coherent_flat_injection_every_delay(P, orc, kbin, snr):
+    """A loud flat injection (SNR 10-16) in one bin of the config-5 map, scored by its own matched template at
+    every one of the 512 delays: SNR(tau) = A cos(2 pi f (tau - tau0)) + noise swings through zero, where the
+    G13 tolerance is 1e-4 s0 ABSOLUTE while a systematic phase error of the recurrence scales with A.  The
+    production kernel (AUTO) must hold G13 at every delay and find the argmax (Eq. 3)."""
+    cfg = synth.CONFIGS[5]
+    csd = synth.noise_csd(cfg.n_t, cfg.n_f, 4)
+    sigma = synth.make_sigma(cfg.sigma, cfg.sigma_scale, cfg.n_t, cfg.n_f, 4)
+    tau = synth.tau_linspace(cfg.n_tau)
+    tr = (cfg.n_t, 0, 500.0, kbin + 0.5, kbin + 0.5, kbin + 0.5)
+    synth.add_injection(csd, sigma, np.arange(cfg.n_t), np.full(cfg.n_t, kbin), -6.1e-3, snr, cfg.f_min, cfg.df)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    p = orc.prepare_map(csd, sigma)
+    ref = _oracle_scores_explicit(orc, p, cfg.f_min, cfg.df, [tr], tau)
+    assert ref.max() > 0.8 * snr
+    got = st.score_tracks([tr], tau_grid=tau)
+    ok, worst = snr_close(got, ref)
+    assert ok, f"bin {kbin}: worst error {worst:.3f} x tolerance"
+    assert int(np.argmax(got[0])) == int(np.argmax(ref[0]))
+
+
+def test_patch_of_sky_delay_prior(P, orc):
+    """the delay drawn 'from a distribution corresponding to a particular patch of sky' -- a narrow,
+    asymmetric (tau_lo, tau_hi) in the random mode, and the same patch as a fine grid."""
+    cfg = synth.CONFIGS[3]
+    csd, sigma, _ = config_inputs(orc, cfg)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    p = orc.prepare_map(csd, sigma)
+    lo, hi, n = 2.0e-3, 3.5e-3, 30_000
+    got = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, 500_000, n, tau_range=(lo, hi))
+    ref = orc.search(p, cfg.f_min, cfg.df, n, cfg.seed, cfg.n_min, cfg.n_max, tau_range=(lo, hi), track_offset=500_000,
+                     dump_snr=True, n_bins=cfg.n_bins)
+    ok, worst = snr_close(got, ref["snr"])
+    assert ok, worst
+    r = st.search(n, cfg.seed, cfg.n_min, cfg.n_max, tau_range=(lo, hi), track_offset=500_000, n_bins=cfg.n_bins)
+    assert r.arg_track == ref["arg_track"] and lo < r.arg_tau < hi and r.arg_tau == ref["arg_tau"]
+    assert abs(r.max_snr_f64 - ref["max_snr"]) <= 1e-11 * abs(ref["max_snr"])
+    ok, why = hist_rule_ok(r.hist, ref["snr"], cfg.hist_lo, cfg.hist_hi, cfg.n_bins)
+    assert ok, why
+    grid = synth.tau_linspace(64, lo, hi)
+    got = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, 0, 2000, tau_grid=grid)
+    ref = orc.search(p, cfg.f_min, cfg.df, 2000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=grid, dump_snr=True)
+    ok, worst = snr_close(got, ref["snr"])
+    assert ok, worst
+
+
+@pytest.mark.parametrize("cid,n,first,n_tau,kname", [(1, 1000, 0, None, "auto"), (2, 20_000, 50_000, None, "auto"),
+                                                      (2, 3000, 0, None, "table"), (2, 3000, 0, None, "rotation"),
+                                                      (2, 3000, 0, None, "reinsch"), (5, 2000, 9_000_000, None, "auto"),
+                                                      (5, 500, 0, 200, "auto"), (3, 20_000, 0, None, "auto")])
+def test_per_template_maximum_over_delays(P, orc, cid, n, first, n_tau, kname):
+    """st_search_track_max: for every template its best delay and SNR, computed in the
+    fused epilogue.  Values within G13 of the oracle's row maximum; the index is decided in float32 (G24), so
+    it equals the oracle's or names a delay whose oracle SNR is within the tolerance of the row maximum."""
+    cfg = synth.CONFIGS[cid]
+    csd, sigma, tau = config_inputs(orc, cfg)
+    if n_tau is not None:
+        tau = synth.tau_linspace(n_tau)
+    st = make_ctx(P, cfg, max_n_tau=max(64, 0 if tau is None else len(tau)))
+    st.set_map(csd, sigma)
+    kw = dict(tau_grid=tau) if cfg.tau_mode == "grid" else dict(tau_range=(-synth.TAU_MAX, synth.TAU_MAX))
+    r, vmax, imax = st.search_track_max(n, cfg.seed, cfg.n_min, cfg.n_max, track_offset=first, n_bins=cfg.n_bins,
+                                        kernel=KERNELS.get(kname, 0), **kw)
+    ref = orc.search(orc.prepare_map(csd, sigma), cfg.f_min, cfg.df, n, cfg.seed, cfg.n_min, cfg.n_max,
+                     track_offset=first, dump_snr=True, n_bins=cfg.n_bins, **kw)
+    snr = ref["snr"]
+    rows = np.arange(n)
+    want_v, want_i = snr.max(axis=1), snr.argmax(axis=1)
+    ok, worst = snr_close(vmax, want_v)
+    assert ok, worst
+    tol = 1e-4 * np.maximum(np.abs(want_v), S0_UNIT)
+    assert ((imax == want_i) | (want_v - snr[rows, imax] <= 2 * tol)).all()
+    assert (imax == want_i).mean() > 0.999
+    # the search result itself is unchanged by asking for the per-template output
+    plain = st.search(n, cfg.seed, cfg.n_min, cfg.n_max, track_offset=first, n_bins=cfg.n_bins, kernel=KERNELS.get(kname, 0), **kw)
+    assert (r.arg_track, r.arg_tau_index, r.max_snr_f64) == (plain.arg_track, plain.arg_tau_index, plain.max_snr_f64)
+    assert np.array_equal(r.hist, plain.hist)
+    assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+    assert float(vmax.max()) == r.max_snr and int(imax[r.arg_track - first]) == r.arg_tau_index
+
+
+def test_context_on_a_device_that_is_not_current(P, orc):
+    """Every entry point runs on the workspace's device whatever device is current in the calling thread."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one GPU")
+    cfg = synth.CONFIGS[1]
+    csd, sigma, tau = config_inputs(orc, cfg)
+    torch.cuda.set_device(0)
+    st = P.Stochtrack(cfg.n_t, cfg.n_f, cfg.df, cfg.f_min, max_n_tau=64, device="cuda:1")
+    st.set_map(csd, sigma)
+    r = st.search(cfg.n_tracks, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau)
+    ref = orc.search(orc.prepare_map(csd, sigma), cfg.f_min, cfg.df, cfg.n_tracks, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau)
+    assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
