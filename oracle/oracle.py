@@ -29,7 +29,7 @@ def build(force=False):
 class Track(C.Structure):
     _fields_ = [("N", C.c_int32), ("j0", C.c_int32), ("a", C.c_double),
                 ("y0", C.c_double), ("y1", C.c_double), ("y2", C.c_double),
-                ("tau", C.c_double)]
+                ("tau", C.c_double), ("y3", C.c_double), ("family", C.c_int32)]
 
     def as_dict(self):
         return {f: getattr(self, f) for f, _ in self._fields_}
@@ -42,7 +42,8 @@ class _SearchParams(C.Structure):
                 ("tau_lo", C.c_double), ("tau_hi", C.c_double),
                 ("norm_mode", C.c_int32), ("n_bins", C.c_int32),
                 ("hist_lo", C.c_double), ("hist_hi", C.c_double),
-                ("score_mode", C.c_int32), ("n_threads", C.c_int32)]
+                ("score_mode", C.c_int32), ("n_threads", C.c_int32),
+                ("family", C.c_int32), ("pad", C.c_int32)]
 
 
 class _SearchResult(C.Structure):
@@ -66,6 +67,13 @@ def lib():
         L.or_track_params.argtypes = [C.c_uint64, C.c_uint64, C.c_int32, C.c_int32, C.c_int32,
                                       C.c_int32, C.c_double, C.c_double, C.POINTER(Track)]
         L.or_track_params.restype = C.c_int
+        L.or_track_params_family.argtypes = [C.c_uint64, C.c_uint64, C.c_int32, C.c_int32, C.c_int32,
+                                             C.c_int32, C.c_double, C.c_double, C.c_int32, C.POINTER(Track)]
+        L.or_track_params_family.restype = C.c_int
+        L.or_prepare_inv_sigma.argtypes = [f32p, C.c_int, C.c_int32, C.c_int32, f64p]
+        L.or_score_direct_w.argtypes = [f64p, f64p, C.c_int32, C.POINTER(Track), i32p, C.c_double, C.c_double, C.c_double]
+        L.or_score_direct_w.restype = C.c_double
+        L.or_score_table_w.argtypes = [f64p, f64p, C.c_int32, C.POINTER(Track), i32p, f64p, C.c_int32, f64p]
         L.or_rasterise.argtypes = [C.POINTER(Track), C.c_int32, i32p]
         L.or_prepare_map.argtypes = [f32p, f32p, C.c_int, C.c_int32, C.c_int32, f64p]
         L.or_score_direct.argtypes = [f64p, C.c_int32, C.POINTER(Track), i32p,
@@ -76,7 +84,7 @@ def lib():
                                      C.c_int, f64p]
         L.or_search.argtypes = [f64p, C.c_int32, C.c_int32, C.c_double, C.c_double, f64p,
                                 C.POINTER(_SearchParams), C.POINTER(_SearchResult),
-                                u64p, f64p, i32p, i32p, i32p]
+                                u64p, f64p, i32p, i32p, i32p, f64p]
         L.or_search.restype = C.c_int
         _lib = L
     return _lib
@@ -86,7 +94,8 @@ def _p(a, ctype):
     return a.ctypes.data_as(C.POINTER(ctype)) if a is not None else None
 
 
-NORM_SQRT_N, NORM_MEAN = 0, 1
+NORM_SQRT_N, NORM_MEAN, NORM_INVVAR = 0, 1, 2
+FAMILY_QUADRATIC, FAMILY_CUBIC = 0, 1
 TAU_GRID, TAU_RANDOM = 0, 1
 
 
@@ -104,16 +113,22 @@ def track_words(seed, track_id):
     return out
 
 
-def track_params(seed, track_id, n_t, n_f, n_min, n_max, tau_lo=0.0, tau_hi=0.0):
+def track_params(seed, track_id, n_t, n_f, n_min, n_max, tau_lo=0.0, tau_hi=0.0, family=FAMILY_QUADRATIC):
     t = Track()
-    rc = lib().or_track_params(seed, track_id, n_t, n_f, n_min, n_max, tau_lo, tau_hi, C.byref(t))
+    if family == FAMILY_QUADRATIC:
+        rc = lib().or_track_params(seed, track_id, n_t, n_f, n_min, n_max, tau_lo, tau_hi, C.byref(t))
+    else:
+        rc = lib().or_track_params_family(seed, track_id, n_t, n_f, n_min, n_max, tau_lo, tau_hi, family, C.byref(t))
     if rc != 0:
         raise ValueError("or_track_params: invalid arguments")
     return t
 
 
-def make_track(N, j0, a, y0, y1, y2, tau=0.0):
-    return Track(int(N), int(j0), float(a), float(y0), float(y1), float(y2), float(tau))
+def make_track(N, j0, a, y0, y1, y2, tau=0.0, y3=None):
+    """A quadratic template (Eq. 6), or with y3 a cubic one: frequency control points y0, y1, y2, y3 (G26)."""
+    if y3 is None:
+        return Track(int(N), int(j0), float(a), float(y0), float(y1), float(y2), float(tau), 0.0, FAMILY_QUADRATIC)
+    return Track(int(N), int(j0), float(a), float(y0), float(y1), float(y2), float(tau), float(y3), FAMILY_CUBIC)
 
 
 def rasterise(track, n_f):
@@ -140,6 +155,40 @@ def prepare_map(csd, sigma=None):
     lib().or_prepare_map(_p(csd.view(np.float32), C.c_float), _p(s, C.c_float), kind, n_t, n_f,
                          _p(p.view(np.float64), C.c_double))
     return p
+
+
+def prepare_inv_sigma(shape, sigma=None):
+    """1 / sigma per pixel as float64 [n_t][n_f] (0 where the pixel is masked, G11): the weights of O4w."""
+    n_t, n_f = shape
+    kind, s = 0, None
+    if sigma is not None:
+        s = np.ascontiguousarray(sigma, dtype=np.float32)
+        kind = 1 if s.shape == (n_f,) else 2
+        if s.shape not in ((n_f,), (n_t, n_f)):
+            raise ValueError("sigma must be None, [n_f] or [n_t][n_f]")
+    r = np.zeros((n_t, n_f), dtype=np.float64)
+    lib().or_prepare_inv_sigma(_p(s, C.c_float), kind, n_t, n_f, _p(r, C.c_double))
+    return r
+
+
+def score_direct_w(p, inv_sigma, track, k, f_min, df, tau):
+    """Inverse-variance weighted statistic (fn. 23, G25) of one template at one delay."""
+    p = np.ascontiguousarray(p, dtype=np.complex128)
+    r = np.ascontiguousarray(inv_sigma, dtype=np.float64)
+    k = np.ascontiguousarray(k, dtype=np.int32)
+    return lib().or_score_direct_w(_p(p.view(np.float64), C.c_double), _p(r, C.c_double), p.shape[1], C.byref(track),
+                                   _p(k, C.c_int32), f_min, df, tau)
+
+
+def score_table_w(p, inv_sigma, track, k, W):
+    p = np.ascontiguousarray(p, dtype=np.complex128)
+    r = np.ascontiguousarray(inv_sigma, dtype=np.float64)
+    k = np.ascontiguousarray(k, dtype=np.int32)
+    W = np.ascontiguousarray(W, dtype=np.complex128)
+    snr = np.zeros(W.shape[1], dtype=np.float64)
+    lib().or_score_table_w(_p(p.view(np.float64), C.c_double), _p(r, C.c_double), p.shape[1], C.byref(track),
+                           _p(k, C.c_int32), _p(W.view(np.float64), C.c_double), W.shape[1], _p(snr, C.c_double))
+    return snr
 
 
 def score_direct(p, track, k, f_min, df, tau, norm=NORM_SQRT_N):
@@ -170,11 +219,14 @@ def score_table(p, track, k, W, norm=NORM_SQRT_N):
 
 def search(p, f_min, df, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=None,
            norm=NORM_SQRT_N, n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0,
-           score_mode=0, n_threads=0, dump_snr=False, dump_tracks=False):
+           score_mode=0, n_threads=0, dump_snr=False, dump_tracks=False, family=FAMILY_QUADRATIC,
+           inv_sigma=None):
     """Whole path O1-O5 for ids [track_offset, track_offset + n_tracks).
 
     tau_grid (array) selects grid mode; tau_range=(lo, hi) selects the paper's
-    random-tau mode.  Returns a dict.
+    random-tau mode.  family selects the template family (G26); norm=NORM_INVVAR
+    the inverse-variance weighting (G25) and then needs inv_sigma = prepare_inv_sigma(...).
+    Returns a dict.
     """
     p = np.ascontiguousarray(p, dtype=np.complex128)
     n_t, n_f = p.shape
@@ -191,6 +243,14 @@ def search(p, f_min, df, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=
     sp.norm_mode, sp.n_bins = int(norm), int(n_bins)
     sp.hist_lo, sp.hist_hi = float(hist_lo), float(hist_hi)
     sp.score_mode, sp.n_threads = int(score_mode), int(n_threads)
+    sp.family = int(family)
+    rs = None
+    if int(norm) == NORM_INVVAR:
+        if inv_sigma is None:
+            raise ValueError("norm=NORM_INVVAR needs inv_sigma")
+        rs = np.ascontiguousarray(inv_sigma, dtype=np.float64)
+        if rs.shape != (n_t, n_f):
+            raise ValueError("inv_sigma must be [n_t][n_f]")
     n_tau = sp.n_tau
     hist = np.zeros(n_bins, dtype=np.uint64) if n_bins > 0 else None
     snr = np.zeros((n_tracks, n_tau), dtype=np.float64) if dump_snr else None
@@ -201,7 +261,7 @@ def search(p, f_min, df, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=
     rc = lib().or_search(_p(p.view(np.float64), C.c_double), n_t, n_f, f_min, df,
                          _p(tau, C.c_double), C.byref(sp), C.byref(res),
                          _p(hist, C.c_uint64), _p(snr, C.c_double),
-                         _p(kd, C.c_int32), _p(j0, C.c_int32), _p(Nn, C.c_int32))
+                         _p(kd, C.c_int32), _p(j0, C.c_int32), _p(Nn, C.c_int32), _p(rs, C.c_double))
     if rc != 0:
         raise ValueError(f"or_search failed with {rc}")
     return {"max_snr": res.max_snr, "arg_track": int(res.arg_track),
@@ -218,9 +278,13 @@ def search_batch(csd_maps, sigma_maps, seeds, f_min, df, n_tracks, n_min, n_max,
     O1-O5 (search) with seed seeds[m].  Returns the list of per-map result dicts."""
     out = []
     for m, csd in enumerate(csd_maps):
-        p = prepare_map(csd, None if sigma_maps is None else sigma_maps[m])
+        sig = None if sigma_maps is None else sigma_maps[m]
+        p = prepare_map(csd, sig)
         seed = int(seeds[m]) if np.ndim(seeds) else int(seeds)
-        out.append(search(p, f_min, df, n_tracks, seed, n_min, n_max, **kw))
+        kw_m = dict(kw)
+        if kw.get("norm", NORM_SQRT_N) == NORM_INVVAR:
+            kw_m["inv_sigma"] = prepare_inv_sigma(p.shape, sig)
+        out.append(search(p, f_min, df, n_tracks, seed, n_min, n_max, **kw_m))
     return out
 
 

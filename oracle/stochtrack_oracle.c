@@ -20,6 +20,9 @@
  *   O3  rasterisation       Eq. 6 -> one bin per time column  PAPER.md:83, :73  (G2, G15)
  *   O4  score               Eq. 8 (with Eq. 7's p = CSD/sigma) PAPER.md:104, :96 (G1, G6, G7)
  *   O5  reduce              max / argmax / histogram          PAPER.md:68, :234 (G12, G14)
+ * Variants (readings G25, G26 of DESIGN.md):
+ *   O4w inverse-variance weighting of SNR_tot (fn. 23): norm_mode 2
+ *   O2c/O3c the cubic template family (PAPER.md:75 "other parameterizable curves", :246-252, :287)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"):
  *   or_philox4x32_10 : cuRAND host generator CURAND_RNG_PSEUDO_PHILOX4_32_10 (P1)
@@ -38,6 +41,12 @@
  *                      (tests/test_oracle_track_params_pins.py, which also rebuilds this file
  *                      with eight plausible slips and requires every one to fail).  Which
  *                      Philox word feeds which parameter remains a convention (G5).
+ *   or_score_*_w     : reduction to the sqrt(N) statistic for constant sigma, a two-pixel closed
+ *                      form, optimality against random weightings, masked pixels dropping out,
+ *                      unit null variance under strongly varying sigma (tests/test_oracle_variants.py)
+ *   cubic family     : 60-digit decimal brute force of the cubic Bernstein form, end points, convex
+ *                      hull, the degree-elevated quadratic reproducing the quadratic family's pixels,
+ *                      uniformity / independence of the fourth control point (same file)
  */
 #include <math.h>
 #include <stdint.h>
@@ -94,6 +103,8 @@ typedef struct {
     double  a;       /* P1.t - P0.t in columns, 0 < a < N (G3)                          */
     double  y0, y1, y2; /* f_start, f_mid, f_end in bin units, bin k covers [k, k+1)    */
     double  tau;     /* the track's own delay (random-tau mode); else 0    */
+    double  y3;      /* cubic family only: f_end; then y1, y2 are the two inner control points */
+    int32_t family;  /* 0 quadratic Bezier (Eq. 6), 1 cubic in frequency (G26)          */
 } or_track;
 
 /* O2: "each template can be quickly generated from just six random numbers"
@@ -102,6 +113,7 @@ int or_track_params(uint64_t seed, uint64_t id, int32_t n_t, int32_t n_f,
                     int32_t n_min, int32_t n_max, double tau_lo, double tau_hi,
                     or_track *t)
 {
+    t->y3 = 0.0; t->family = 0;
     if (n_t < 1 || n_f < 1 || n_min < 1 || n_max < n_min || n_max > n_t) return -1;
     uint32_t r[8];
     or_track_words(seed, id, r);
@@ -126,6 +138,26 @@ int or_track_params(uint64_t seed, uint64_t id, int32_t n_t, int32_t n_f,
     return 0;
 }
 
+/* O2c (G26): the cubic family.  "Other parameterizable curves such as spline can be used as well"
+ * (PAPER.md:75); a compact-binary chirp "is not especially well-described with a second-order Bezier
+ * curve".  Reading: a cubic Bezier curve whose TIME control points are the degree-elevated
+ * quadratic of O2 (so t(xi) stays the monotone quadratic and O3's root is reused) and whose FREQUENCY has
+ * four control points y0, y1, y2, y3, each uniform over the band and independent: the one extra random
+ * number is the Philox word O2 leaves unused (r7).  N, j0, a, y0, y1, y2, tau are exactly O2's.          */
+int or_track_params_family(uint64_t seed, uint64_t id, int32_t n_t, int32_t n_f,
+                           int32_t n_min, int32_t n_max, double tau_lo, double tau_hi,
+                           int32_t family, or_track *t)
+{
+    if (family != 0 && family != 1) return -1;
+    int rc = or_track_params(seed, id, n_t, n_f, n_min, n_max, tau_lo, tau_hi, t);
+    if (rc != 0 || family == 0) return rc;
+    uint32_t r[8];
+    or_track_words(seed, id, r);
+    t->family = 1;
+    t->y3 = ((double)r[7] + 0.5) * (double)n_f * (1.0 / 4294967296.0);
+    return 0;
+}
+
 /* ------------------------------------------------------------------ O3 -- */
 /* Eq. 6: t(xi) = (1-xi)^2 t0 + 2(1-xi)xi t1 + xi^2 t2 with
  * t0 = j0, t1 = j0 + a, t2 = j0 + N gives t(xi) - j0 = (N - 2a) xi^2 + 2a xi.
@@ -146,10 +178,23 @@ void or_rasterise(const or_track *t, int32_t n_f, int32_t *k_out)
         double den = a + s;
         double xi  = u / den;
         double om  = 1.0 - xi;
-        double b0  = om * om;
-        double b1  = 2.0 * (om * xi);
-        double b2  = xi * xi;
-        double y   = (b0 * t->y0 + b1 * t->y1) + b2 * t->y2;
+        double y;
+        if (t->family == 0) {
+            double b0  = om * om;
+            double b1  = 2.0 * (om * xi);
+            double b2  = xi * xi;
+            y = (b0 * t->y0 + b1 * t->y1) + b2 * t->y2;
+        } else {
+            /* O3c (G26): f(xi) = (1-xi)^3 y0 + 3 (1-xi)^2 xi y1 + 3 (1-xi) xi^2 y2 + xi^3 y3, the cubic
+             * Bernstein form of Eq. 6's construction; NORMATIVE order, single rounded operations.   */
+            double om2 = om * om;
+            double xi2 = xi * xi;
+            double b0  = om2 * om;
+            double b1  = 3.0 * (om2 * xi);
+            double b2  = 3.0 * (om * xi2);
+            double b3  = xi2 * xi;
+            y = ((b0 * t->y0 + b1 * t->y1) + b2 * t->y2) + b3 * t->y3;
+        }
         double fl  = floor(y);
         int32_t k;
         if (!(fl >= 0.0)) k = 0;
@@ -232,6 +277,55 @@ void or_score_table(const double *p, int32_t n_f, const or_track *t, const int32
     for (int32_t m = 0; m < n_tau; ++m) snr[m] /= nrm;
 }
 
+/* ----------------------------------------------------------------- O4w -- */
+/* fn. 23: "alternative definitions of SNR_tot (with a different weighting scheme) are also
+ * possible".  Reading G25: the inverse-variance combination of the per-pixel cross-power estimates of
+ * Appendix A.  A pixel carries Y = Re[e^{i phi} CSD] with variance sigma^2 (A1-A3); the
+ * minimum-variance combination of the Y's is sum(Y / sigma^2) / sum(1 / sigma^2) with variance
+ * 1 / sum(1 / sigma^2), so its signal-to-noise ratio is
+ *       SNR_w = sum_Gamma (Y / sigma^2) / sqrt( sum_Gamma 1 / sigma^2 )
+ *             = sum_Gamma (rho / sigma)   / sqrt( sum_Gamma 1 / sigma^2 ),     rho = Re[e^{i phi} p].
+ * For constant sigma this is sum(rho) / sqrt(N): G1's alpha = 1/2 statistic.  Masked pixels (G11) have
+ * p = 0 and 1/sigma := 0: they drop out of both sums; a template with every pixel masked scores 0.   */
+void or_prepare_inv_sigma(const float *sigma, int sigma_kind, int32_t n_t, int32_t n_f, double *r /* [n_t][n_f] */)
+{
+    for (int32_t j = 0; j < n_t; ++j)
+        for (int32_t k = 0; k < n_f; ++k) {
+            double s = or_sigma_at(sigma, sigma_kind, n_f, j, k);
+            r[(size_t)j * (size_t)n_f + (size_t)k] = (!(s > 0.0) || !isfinite(s)) ? 0.0 : 1.0 / s;
+        }
+}
+
+double or_score_direct_w(const double *p, const double *r, int32_t n_f, const or_track *t, const int32_t *k,
+                         double f_min, double df, double tau)
+{
+    double S = 0.0, Wt = 0.0;
+    for (int32_t c = 0; c < t->N; ++c) {
+        size_t px = (size_t)(t->j0 + c) * (size_t)n_f + (size_t)k[c];
+        double phi = OR_TWO_PI * (f_min + (double)k[c] * df) * tau;
+        double rho = cos(phi) * p[2 * px] - sin(phi) * p[2 * px + 1];
+        S  += rho * r[px];
+        Wt += r[px] * r[px];
+    }
+    return Wt > 0.0 ? S / sqrt(Wt) : 0.0;
+}
+
+void or_score_table_w(const double *p, const double *r, int32_t n_f, const or_track *t, const int32_t *k,
+                      const double *W, int32_t n_tau, double *snr /* [n_tau] */)
+{
+    double Wt = 0.0;
+    for (int32_t m = 0; m < n_tau; ++m) snr[m] = 0.0;
+    for (int32_t c = 0; c < t->N; ++c) {
+        size_t px = (size_t)(t->j0 + c) * (size_t)n_f + (size_t)k[c];
+        const double pr = p[2 * px], pi = p[2 * px + 1], rc = r[px];
+        const double *w = W + (size_t)k[c] * (size_t)n_tau * 2;
+        for (int32_t m = 0; m < n_tau; ++m)
+            snr[m] += (w[2 * m] * pr - w[2 * m + 1] * pi) * rc;
+        Wt += rc * rc;
+    }
+    for (int32_t m = 0; m < n_tau; ++m) snr[m] = Wt > 0.0 ? snr[m] / sqrt(Wt) : 0.0;
+}
+
 /* ------------------------------------------------------------------ O5 -- */
 /* Total order of G12: larger SNR, then smaller track id, then smaller tau index. */
 static int or_better(double s, uint64_t id, int32_t m, double bs, uint64_t bid, int32_t bm)
@@ -257,11 +351,13 @@ typedef struct {
     int32_t  tau_mode;        /* 0 grid, 1 random (one tau per track) */
     int32_t  n_tau;           /* grid size (grid mode); 1 in random mode            */
     double   tau_lo, tau_hi;  /* random mode range                                   */
-    int32_t  norm_mode;       /* 0 sqrt(N), 1 N                                      */
+    int32_t  norm_mode;       /* 0 sqrt(N), 1 N, 2 inverse-variance weighting (O4w)  */
     int32_t  n_bins;          /* 0 = no histogram                                    */
     double   hist_lo, hist_hi;
     int32_t  score_mode;      /* 0 table, 1 direct (grid mode only; random is direct) */
     int32_t  n_threads;       /* OpenMP threads; <= 0 = library default              */
+    int32_t  family;          /* 0 quadratic, 1 cubic templates (O2c / O3c)          */
+    int32_t  pad;
 } or_search_params;
 
 typedef struct {
@@ -280,10 +376,13 @@ typedef struct {
  * k_dump: int32[n_tracks][n_t] (-1 padded), j0_dump/N_dump: int32[n_tracks], or NULL. */
 int or_search(const double *p, int32_t n_t, int32_t n_f, double f_min, double df,
               const double *tau_grid, const or_search_params *sp, or_search_result *res,
-              uint64_t *hist, double *snr_dump, int32_t *k_dump, int32_t *j0_dump, int32_t *N_dump)
+              uint64_t *hist, double *snr_dump, int32_t *k_dump, int32_t *j0_dump, int32_t *N_dump,
+              const double *inv_sigma /* [n_t][n_f] from or_prepare_inv_sigma; only read when norm_mode == 2 */)
 {
     const int32_t n_tau = sp->tau_mode == 0 ? sp->n_tau : 1;
     if (n_tau < 1) return -1;
+    if (sp->norm_mode == 2 && !inv_sigma) return -1;
+    if (sp->family != 0 && sp->family != 1) return -1;
     if (sp->n_min < 1 || sp->n_max < sp->n_min || sp->n_max > n_t) return -1;
     double *W = NULL;
     if (sp->tau_mode == 0 && sp->score_mode == 0) {
@@ -323,9 +422,17 @@ int or_search(const double *p, int32_t n_t, int32_t n_f, double f_min, double df
         for (int64_t q = 0; q < (int64_t)sp->n_tracks; ++q) {
             uint64_t id = sp->track_offset + (uint64_t)q;
             or_track t;
-            or_track_params(sp->seed, id, n_t, n_f, sp->n_min, sp->n_max, sp->tau_lo, sp->tau_hi, &t);
+            or_track_params_family(sp->seed, id, n_t, n_f, sp->n_min, sp->n_max, sp->tau_lo, sp->tau_hi, sp->family, &t);
             or_rasterise(&t, n_f, k);
-            if (sp->tau_mode == 0) {
+            if (sp->norm_mode == 2) {
+                if (sp->tau_mode == 0) {
+                    if (sp->score_mode == 0) or_score_table_w(p, inv_sigma, n_f, &t, k, W, n_tau, snr);
+                    else for (int32_t m = 0; m < n_tau; ++m)
+                        snr[m] = or_score_direct_w(p, inv_sigma, n_f, &t, k, f_min, df, tau_grid[m]);
+                } else {
+                    snr[0] = or_score_direct_w(p, inv_sigma, n_f, &t, k, f_min, df, t.tau);
+                }
+            } else if (sp->tau_mode == 0) {
                 if (sp->score_mode == 0) or_score_table(p, n_f, &t, k, W, n_tau, sp->norm_mode, snr);
                 else for (int32_t m = 0; m < n_tau; ++m)
                     snr[m] = or_score_direct(p, n_f, &t, k, f_min, df, tau_grid[m], sp->norm_mode);

@@ -19,13 +19,20 @@ int main(void)
     or_search_params sp;
     sp.n_tracks = T; sp.track_offset = (1ull << 40) + 3; sp.seed = 99; sp.n_min = 1; sp.n_max = NT;
     sp.tau_mode = 0; sp.n_tau = NTAU; sp.tau_lo = -0.01; sp.tau_hi = 0.01; sp.norm_mode = 0; sp.n_bins = NB;
-    sp.hist_lo = -5.0; sp.hist_hi = 5.0; sp.score_mode = 0; sp.n_threads = 2;
+    sp.hist_lo = -5.0; sp.hist_hi = 5.0; sp.score_mode = 0; sp.n_threads = 2; sp.family = 0; sp.pad = 0;
     or_search_result r;
     for (int mode = 0; mode < 3; ++mode) {
         sp.score_mode = mode == 1; sp.tau_mode = mode == 2; if (mode == 2) sp.n_tau = 1;
-        if (or_search(p, NT, NF, 40.0, 1.0, tau, &sp, &r, hist, snr, kd, j0, Nn) != 0) return 2;
+        if (or_search(p, NT, NF, 40.0, 1.0, tau, &sp, &r, hist, snr, kd, j0, Nn, NULL) != 0) return 2;
         printf("%d %.17g %llu %d %llu\n", mode, r.max_snr, (unsigned long long)r.arg_track, r.arg_tau_index,
                (unsigned long long)r.n_evals);
     }
+    /* variants: cubic templates, inverse-variance weighting (their own output row is not compared) */
+    static double inv_sigma[NT * NF];
+    or_prepare_inv_sigma(sigma, 2, NT, NF, inv_sigma);
+    sp.tau_mode = 0; sp.n_tau = NTAU; sp.score_mode = 0; sp.family = 1; sp.norm_mode = 2;
+    if (or_search(p, NT, NF, 40.0, 1.0, tau, &sp, &r, hist, snr, kd, j0, Nn, inv_sigma) != 0) return 3;
+    sp.score_mode = 1;
+    if (or_search(p, NT, NF, 40.0, 1.0, tau, &sp, &r, hist, snr, kd, j0, Nn, inv_sigma) != 0) return 3;
     return 0;
 }

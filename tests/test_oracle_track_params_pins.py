@@ -35,7 +35,7 @@ ORACLE_SRC = os.path.join(os.path.dirname(HERE), "oracle", "stochtrack_oracle.c"
 
 class _Track(C.Structure):
     _fields_ = [("N", C.c_int32), ("j0", C.c_int32), ("a", C.c_double), ("y0", C.c_double),
-                ("y1", C.c_double), ("y2", C.c_double), ("tau", C.c_double)]
+                ("y1", C.c_double), ("y2", C.c_double), ("tau", C.c_double), ("y3", C.c_double), ("family", C.c_int32)]
 
 
 def _sampler(lib):
@@ -118,7 +118,7 @@ def check_track_param_pins(sample):
 
 
 def test_track_params_pinned(orc):
-    check_track_param_pins(_sampler(orc.lib()))
+    check_track_param_pins(_sampler(C.CDLL(orc.build())))       # its own handle: argtypes are set on it
 
 
 # One plausible slip per entry: (what goes wrong, regex on the oracle source, replacement).
