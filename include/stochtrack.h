@@ -59,6 +59,21 @@ extern "C" {
  * statistic; alpha = 1 is Eq. 8 exactly as printed.           */
 #define ST_NORM_SQRT_N 0
 #define ST_NORM_MEAN   1
+/* fn. 23: "alternative definitions of SNR_tot (with a different weighting scheme)".  Reading
+ * G25: the inverse-variance combination of Appendix A's per-pixel estimates,
+ *     SNR_w = sum_Gamma (rho / sigma) / sqrt( sum_Gamma 1 / sigma^2 ),   rho = Re[e^{2 pi i f tau} p],
+ * equal to the SQRT_N statistic for constant sigma; masked pixels leave both sums.  Needs the map to have
+ * been set with its sigma (st_set_map, st_set_map_host, st_search_batch), else ST_ESTATE.             */
+#define ST_NORM_INVVAR 2
+
+/* template families ("other parameterizable curves such as spline can be used as well";
+ * a chirp "is not especially well-described with a second-order Bezier curve").
+ * CUBIC (reading G26): a cubic Bezier curve whose time control points are the degree-elevated quadratic
+ * (t(xi) is the quadratic family's) and whose frequency has four control points y0, y1, y2, y3, each
+ * uniform over the band; N, j0, a, y0, y1, y2, tau of template i are those of the quadratic template i,
+ * y3 comes from the one Philox word the quadratic family leaves unused.                              */
+#define ST_FAMILY_QUADRATIC 0
+#define ST_FAMILY_CUBIC     1
 
 /* scoring kernel selection (grid mode).  AUTO picks CHEBYSHEV when the grid is
  * uniform and every bin's step angle is well conditioned, else REINSCH / ROTATION
@@ -81,6 +96,7 @@ typedef struct {
     double  a;      /* t_mid - t_start in columns, 0 < a < N (G3)               */
     double  y0, y1, y2;
     double  tau;    /* seconds                                                  */
+    double  y3;     /* ST_FAMILY_CUBIC: f_end (y1, y2 are then the inner control points); else ignored */
 } st_track;
 
 typedef struct {
@@ -93,12 +109,12 @@ typedef struct {
     int32_t  n_tau;          /* grid size (grid mode), ignored in random mode           */
     const double *tau_grid;  /* HOST, n_tau delays in seconds (grid mode)               */
     double   tau_lo, tau_hi; /* random mode: tau ~ U(tau_lo, tau_hi)     */
-    int32_t  norm;           /* ST_NORM_SQRT_N | ST_NORM_MEAN                           */
+    int32_t  norm;           /* ST_NORM_SQRT_N | ST_NORM_MEAN | ST_NORM_INVVAR          */
     int32_t  n_bins;         /* histogram bins, 0 = no histogram, <= ST_MAX_BINS        */
     double   hist_lo, hist_hi; /* bin = floor((snr-lo)/(hi-lo)*n_bins) clamped (G14)    */
     uint64_t *hist_out;      /* HOST, n_bins counts (overwritten) or NULL               */
     int32_t  kernel;         /* ST_KERNEL_* request (grid mode)                         */
-    int32_t  reserved;       /* must be 0                                               */
+    int32_t  family;         /* ST_FAMILY_QUADRATIC (0) | ST_FAMILY_CUBIC               */
 } st_search_params;
 
 typedef struct {
@@ -192,8 +208,8 @@ int st_search_track_max(st_ctx *ctx, const st_search_params *params, float *snr_
  *   tracks  : HOST [count] templates in the st_track parameterisation (1 <= N, 0 <= j0, j0 + N <= n_t,
  *             0 < a < N, finite control points); in random mode each template's own `tau` is its delay
  *   snr_dev : DEVICE float32 [count][n_tau] (n_tau = 1 in random mode), same scoring kernel as st_search
- *             with the same params (tau grid / range, norm, kernel); n_tracks, track_offset, seed, n_min,
- *             n_max and the histogram fields of params are ignored.
+ *             with the same params (tau grid / range, norm, kernel, family); n_tracks, track_offset, seed,
+ *             n_min, n_max and the histogram fields of params are ignored.
  * Errors: ST_EINVAL (a template outside the map, count outside [0, ST_MAX_SCORE_TRACKS]), otherwise as
  * st_search.  Synchronous on return.                                                               */
 #define ST_MAX_SCORE_TRACKS 4096
@@ -263,10 +279,13 @@ int st_debug_get_map(st_ctx *ctx, void *p_out_dev);
  * (same arithmetic as the device generator).                                   */
 int st_track_params(const st_ctx *ctx, uint64_t seed, uint64_t track_id,
                     int32_t n_min, int32_t n_max, double tau_lo, double tau_hi, st_track *out);
+/* The same for either template family (st_track_params is the quadratic one).   */
+int st_track_params_family(const st_ctx *ctx, uint64_t seed, uint64_t track_id, int32_t n_min, int32_t n_max,
+                           double tau_lo, double tau_hi, int32_t family, st_track *out);
 
 /* Parity exports (stream-ordered, outputs DEVICE).  Ids [first, first+count):
  * k_out_dev int32 [count][n_t] (-1 beyond N), j0_dev / N_dev int32 [count].
- * Uses params->seed, n_min, n_max.                                             */
+ * Uses params->seed, n_min, n_max, family.                                     */
 int st_debug_rasterise(st_ctx *ctx, const st_search_params *params, uint64_t first, uint64_t count,
                        int32_t *k_out_dev, int32_t *j0_dev, int32_t *N_dev);
 /* The same export through the random-delay kernel's OWN rasteriser (its fast path evaluates Eq. 6 in
@@ -274,8 +293,8 @@ int st_debug_rasterise(st_ctx *ctx, const st_search_params *params, uint64_t fir
  * [first, first+count) with params (ST_TAU_RANDOM) and writes the bins it used.  Needs a map.        */
 int st_debug_rasterise_random(st_ctx *ctx, const st_search_params *params, uint64_t first, uint64_t count,
                               int32_t *k_out_dev, int32_t *j0_dev, int32_t *N_dev);
-/* Rasterise one explicit template (HOST st_track in, DEVICE int32 [N] out).    */
-int st_debug_rasterise_track(st_ctx *ctx, const st_track *track, int32_t *k_out_dev);
+/* Rasterise one explicit template of the given family (HOST st_track in, DEVICE int32 [N] out). */
+int st_debug_rasterise_track(st_ctx *ctx, const st_track *track, int32_t family, int32_t *k_out_dev);
 /* snr_dev float32 [count][n_tau] (n_tau = 1 in random mode): every SNR(i, tau)
  * the scoring kernel selected by params->kernel produces.                      */
 int st_debug_scores(st_ctx *ctx, const st_search_params *params, uint64_t first, uint64_t count,

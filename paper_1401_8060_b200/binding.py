@@ -12,7 +12,8 @@ ST_OK, ST_EINVAL, ST_ESTATE, ST_ENOSPC, ST_ECUDA = 0, -1, -2, -3, -4
 _CODES = {ST_EINVAL: "ST_EINVAL", ST_ESTATE: "ST_ESTATE", ST_ENOSPC: "ST_ENOSPC", ST_ECUDA: "ST_ECUDA"}
 SIGMA_NONE, SIGMA_PER_FREQ, SIGMA_PER_PIXEL = 0, 1, 2
 TAU_GRID, TAU_RANDOM = 0, 1
-NORM_SQRT_N, NORM_MEAN = 0, 1
+NORM_SQRT_N, NORM_MEAN, NORM_INVVAR = 0, 1, 2
+FAMILY_QUADRATIC, FAMILY_CUBIC = 0, 1
 KERNEL_AUTO, KERNEL_TABLE, KERNEL_ROTATION, KERNEL_REINSCH, KERNEL_RANDOM, KERNEL_CHEBYSHEV = 0, 1, 2, 3, 4, 5
 KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random", 5: "chebyshev"}
 
@@ -21,7 +22,7 @@ exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_wor
                     "st_set_map_host", "st_search", "st_search_topk", "st_search_batch", "st_search_track_max",
                     "st_score_tracks", "st_debug_rasterise_random", "st_ftmap_scratch_bytes", "st_set_map_from_strain", "st_search_timeshifts",
                     "st_debug_get_map",
-                    "st_track_params", "st_debug_rasterise",
+                    "st_track_params", "st_track_params_family", "st_debug_rasterise",
                     "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words",
                     "st_last_error", "st_version")
 
@@ -34,7 +35,7 @@ class StError(RuntimeError):
 
 class CTrack(C.Structure):
     _fields_ = [("N", C.c_int32), ("j0", C.c_int32), ("a", C.c_double), ("y0", C.c_double),
-                ("y1", C.c_double), ("y2", C.c_double), ("tau", C.c_double)]
+                ("y1", C.c_double), ("y2", C.c_double), ("tau", C.c_double), ("y3", C.c_double)]
 
     def as_dict(self):
         return {f: getattr(self, f) for f, _ in self._fields_}
@@ -45,7 +46,7 @@ class CSearchParams(C.Structure):
                 ("n_min", C.c_int32), ("n_max", C.c_int32), ("tau_mode", C.c_int32), ("n_tau", C.c_int32),
                 ("tau_grid", C.POINTER(C.c_double)), ("tau_lo", C.c_double), ("tau_hi", C.c_double),
                 ("norm", C.c_int32), ("n_bins", C.c_int32), ("hist_lo", C.c_double), ("hist_hi", C.c_double),
-                ("hist_out", C.POINTER(C.c_uint64)), ("kernel", C.c_int32), ("reserved", C.c_int32)]
+                ("hist_out", C.POINTER(C.c_uint64)), ("kernel", C.c_int32), ("family", C.c_int32)]
 
 
 class CResult(C.Structure):
@@ -111,7 +112,10 @@ def load_library(path=None):
     L.st_track_params.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_int32, C.c_int32, C.c_double, C.c_double,
                                   C.POINTER(CTrack)]
     L.st_debug_rasterise.argtypes = [vp, C.POINTER(CSearchParams), C.c_uint64, C.c_uint64, vp, vp, vp]
-    L.st_debug_rasterise_track.argtypes = [vp, C.POINTER(CTrack), vp]
+    L.st_track_params_family.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_int32, C.c_int32, C.c_double, C.c_double,
+                                         C.c_int32, C.POINTER(CTrack)]
+    L.st_track_params_family.restype = C.c_int
+    L.st_debug_rasterise_track.argtypes = [vp, C.POINTER(CTrack), C.c_int32, vp]
     L.st_debug_scores.argtypes = [vp, C.POINTER(CSearchParams), C.c_uint64, C.c_uint64, vp]
     L.st_debug_track_words.argtypes = [C.c_uint64, C.c_uint64, C.POINTER(C.c_uint32)]
     L.st_last_error.argtypes = [vp]
@@ -265,7 +269,7 @@ class Stochtrack:
 
     def search_timeshifts(self, s_i, s_j, fs, seg_len, n_neighbours, shifts, seeds, n_tracks, n_min, n_max,
                           tau_grid=None, tau_range=None, norm=NORM_SQRT_N, n_bins=0, hist_lo=-10.0, hist_hi=10.0,
-                          track_offset=0, kernel=KERNEL_AUTO):
+                          track_offset=0, kernel=KERNEL_AUTO, family=FAMILY_QUADRATIC):
         """Time-shift background from strain (st_search_timeshifts): spectrograms once, one map and one
         search per whole-segment shift of detector J.  Returns (list of SearchResult, gpu_ms_total)."""
         self._ft_args(s_i, s_j, seg_len)
@@ -281,7 +285,7 @@ class Stochtrack:
                 raise ValueError("seeds: one per shift")
             sd_p = sd.ctypes.data_as(C.POINTER(C.c_uint64))
         p, keep = self._params(n_tracks, seed0, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
-                               track_offset, kernel)
+                               track_offset, kernel, family)
         hist = None
         if n_bins > 0:
             hist = np.zeros((n, n_bins), dtype=np.uint64)
@@ -314,7 +318,7 @@ class Stochtrack:
 
     # ------------------------------------------------------------ S1-S4
     def _params(self, n_tracks, seed, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
-                track_offset, kernel):
+                track_offset, kernel, family=FAMILY_QUADRATIC):
         p = CSearchParams()
         p.n_tracks, p.track_offset, p.seed = int(n_tracks), int(track_offset), int(seed)
         p.n_min, p.n_max = int(n_min), int(n_max)
@@ -330,12 +334,13 @@ class Stochtrack:
         p.norm, p.n_bins = int(norm), int(n_bins)
         p.hist_lo, p.hist_hi = float(hist_lo), float(hist_hi)
         p.kernel = int(kernel)
+        p.family = int(family)
         return p, keep
 
     def search(self, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=None, norm=NORM_SQRT_N,
-               n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO):
+               n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO, family=FAMILY_QUADRATIC):
         p, keep = self._params(n_tracks, seed, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
-                               track_offset, kernel)
+                               track_offset, kernel, family)
         hist = None
         if n_bins > 0:
             hist = np.zeros(n_bins, dtype=np.uint64)
@@ -345,12 +350,12 @@ class Stochtrack:
         return self._result(r, hist)
 
     def search_track_max(self, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=None, norm=NORM_SQRT_N,
-                         n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO):
+                         n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO, family=FAMILY_QUADRATIC):
         """st_search_track_max: the search result plus, per template, its maximum over the delays and the delay
         index attaining it.  Returns (SearchResult, snr_max float32 [n_tracks], tau_index int32 [n_tracks])."""
         torch = self._torch
         p, keep = self._params(n_tracks, seed, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
-                               track_offset, kernel)
+                               track_offset, kernel, family)
         hist = None
         if n_bins > 0:
             hist = np.zeros(n_bins, dtype=np.uint64)
@@ -361,27 +366,27 @@ class Stochtrack:
         self._check(self._L.st_search_track_max(self._ctx, C.byref(p), snr.data_ptr(), idx.data_ptr(), C.byref(r)))
         return self._result(r, hist), snr[:int(n_tracks)].cpu().numpy(), idx[:int(n_tracks)].cpu().numpy()
 
-    def score_tracks(self, tracks, tau_grid=None, tau_range=None, norm=NORM_SQRT_N, kernel=KERNEL_AUTO):
-        """st_score_tracks: Eq. 8 for explicit templates.  tracks: sequence of (N, j0, a, y0, y1, y2[, tau]).
+    def score_tracks(self, tracks, tau_grid=None, tau_range=None, norm=NORM_SQRT_N, kernel=KERNEL_AUTO, family=FAMILY_QUADRATIC):
+        """st_score_tracks: Eq. 8 for explicit templates.  tracks: sequence of (N, j0, a, y0, y1, y2[, tau[, y3]]).
         Returns float32 [count][n_tau] (n_tau = 1 in random mode, where each template's own tau is its delay)."""
         torch = self._torch
         n = len(tracks)
         arr = (CTrack * max(n, 1))()
         for i, t in enumerate(tracks):
             arr[i] = CTrack(int(t[0]), int(t[1]), float(t[2]), float(t[3]), float(t[4]), float(t[5]),
-                            float(t[6]) if len(t) > 6 else 0.0)
-        p, keep = self._params(n, 0, 1, 1, tau_grid, tau_range if tau_range is not None else (0.0, 0.0), norm, 0, -10.0, 10.0, 0, kernel)
+                            float(t[6]) if len(t) > 6 else 0.0, float(t[7]) if len(t) > 7 else 0.0)
+        p, keep = self._params(n, 0, 1, 1, tau_grid, tau_range if tau_range is not None else (0.0, 0.0), norm, 0, -10.0, 10.0, 0, kernel, family)
         n_tau = p.n_tau if p.tau_mode == TAU_GRID else 1
         snr = torch.empty((max(n, 1), n_tau), dtype=torch.float32, device=self.device)
         self._check(self._L.st_score_tracks(self._ctx, C.byref(p), arr, n, snr.data_ptr()))
         return snr[:n].cpu().numpy()
 
     def search_topk(self, top_k, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=None, norm=NORM_SQRT_N,
-                    n_bins=1000, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO):
+                    n_bins=1000, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO, family=FAMILY_QUADRATIC):
         """The top_k loudest (template, delay) samples (st_search_topk).  Returns (SearchResult, list of
         dicts {track, tau_index, snr_f32, snr_f64, tau} in the G12 order)."""
         p, keep = self._params(n_tracks, seed, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
-                               track_offset, kernel)
+                               track_offset, kernel, family)
         hist = np.zeros(max(n_bins, 1), dtype=np.uint64)
         p.hist_out = hist.ctypes.data_as(C.POINTER(C.c_uint64))
         top = (CTopEntry * int(top_k))()
@@ -402,7 +407,7 @@ class Stochtrack:
                             flags=int(r.flags), gpu_ms=float(r.gpu_ms), hist=hist)
 
     def search_batch(self, csd_maps, sigma_maps, seeds, n_tracks, n_min, n_max, tau_grid=None, tau_range=None,
-                     norm=NORM_SQRT_N, n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO):
+                     norm=NORM_SQRT_N, n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO, family=FAMILY_QUADRATIC):
         """Batch / background mode (st_search_batch): one call over many maps.
 
         csd_maps: sequence of complex64 [n_t][n_f] maps, all torch CUDA tensors (device path) or all
@@ -453,7 +458,7 @@ class Stochtrack:
             keep.append(sd)
             b.seeds = sd.ctypes.data_as(C.POINTER(C.c_uint64))
         p, k2 = self._params(n_tracks, seed0, n_min, n_max, tau_grid, tau_range, norm, n_bins, hist_lo, hist_hi,
-                             track_offset, kernel)
+                             track_offset, kernel, family)
         hist = None
         if n_bins > 0:
             hist = np.zeros((n_maps, n_bins), dtype=np.uint64)
@@ -463,15 +468,15 @@ class Stochtrack:
         self._check(self._L.st_search_batch(self._ctx, C.byref(b), C.byref(p), res, C.byref(ms)))
         return [self._result(res[m], hist[m] if hist is not None else None) for m in range(n_maps)], float(ms.value)
 
-    def track_params(self, seed, track_id, n_min, n_max, tau_lo=0.0, tau_hi=0.0):
+    def track_params(self, seed, track_id, n_min, n_max, tau_lo=0.0, tau_hi=0.0, family=FAMILY_QUADRATIC):
         t = CTrack()
-        self._check(self._L.st_track_params(self._ctx, seed, track_id, n_min, n_max, tau_lo, tau_hi, C.byref(t)))
+        self._check(self._L.st_track_params_family(self._ctx, seed, track_id, n_min, n_max, tau_lo, tau_hi, int(family), C.byref(t)))
         return t
 
     # ------------------------------------------------------ parity exports
-    def debug_rasterise(self, seed, n_min, n_max, first, count):
+    def debug_rasterise(self, seed, n_min, n_max, first, count, family=FAMILY_QUADRATIC):
         torch = self._torch
-        p, _ = self._params(count, seed, n_min, n_max, None, (0.0, 0.0), 0, 0, -10, 10, 0, 0)
+        p, _ = self._params(count, seed, n_min, n_max, None, (0.0, 0.0), 0, 0, -10, 10, 0, 0, family)
         k = torch.empty((count, self.n_t), dtype=torch.int32, device=self.device)
         j0 = torch.empty(count, dtype=torch.int32, device=self.device)
         N = torch.empty(count, dtype=torch.int32, device=self.device)
@@ -480,10 +485,10 @@ class Stochtrack:
         self.synchronize()
         return k.cpu().numpy(), j0.cpu().numpy(), N.cpu().numpy()
 
-    def debug_rasterise_random(self, seed, n_min, n_max, first, count, tau_range=(-0.01, 0.01)):
+    def debug_rasterise_random(self, seed, n_min, n_max, first, count, tau_range=(-0.01, 0.01), family=FAMILY_QUADRATIC):
         """Bins decided by the random-delay kernel's own rasteriser (st_debug_rasterise_random)."""
         torch = self._torch
-        p, _ = self._params(count, seed, n_min, n_max, None, tau_range, 0, 0, -10, 10, 0, 0)
+        p, _ = self._params(count, seed, n_min, n_max, None, tau_range, 0, 0, -10, 10, 0, 0, family)
         k = torch.empty((count, self.n_t), dtype=torch.int32, device=self.device)
         j0 = torch.empty(count, dtype=torch.int32, device=self.device)
         N = torch.empty(count, dtype=torch.int32, device=self.device)
@@ -492,18 +497,20 @@ class Stochtrack:
         self.synchronize()
         return k.cpu().numpy(), j0.cpu().numpy(), N.cpu().numpy()
 
-    def debug_rasterise_track(self, N, j0, a, y0, y1, y2):
+    def debug_rasterise_track(self, N, j0, a, y0, y1, y2, y3=None):
+        """Bins of one explicit template; with y3 a cubic one (frequency control points y0, y1, y2, y3)."""
         torch = self._torch
-        t = CTrack(int(N), int(j0), float(a), float(y0), float(y1), float(y2), 0.0)
+        t = CTrack(int(N), int(j0), float(a), float(y0), float(y1), float(y2), 0.0, 0.0 if y3 is None else float(y3))
         k = torch.empty(int(N), dtype=torch.int32, device=self.device)
-        self._check(self._L.st_debug_rasterise_track(self._ctx, C.byref(t), k.data_ptr()))
+        self._check(self._L.st_debug_rasterise_track(self._ctx, C.byref(t), FAMILY_QUADRATIC if y3 is None else FAMILY_CUBIC,
+                                                     k.data_ptr()))
         self.synchronize()
         return k.cpu().numpy()
 
     def debug_scores(self, seed, n_min, n_max, first, count, tau_grid=None, tau_range=None, norm=NORM_SQRT_N,
-                     kernel=KERNEL_AUTO):
+                     kernel=KERNEL_AUTO, family=FAMILY_QUADRATIC):
         torch = self._torch
-        p, keep = self._params(count, seed, n_min, n_max, tau_grid, tau_range, norm, 0, -10, 10, first, kernel)
+        p, keep = self._params(count, seed, n_min, n_max, tau_grid, tau_range, norm, 0, -10, 10, first, kernel, family)
         n_tau = p.n_tau if p.tau_mode == TAU_GRID else 1
         snr = torch.empty((count, n_tau), dtype=torch.float32, device=self.device)
         self._check(self._L.st_debug_scores(self._ctx, C.byref(p), int(first), int(count), snr.data_ptr()))
@@ -511,7 +518,8 @@ class Stochtrack:
         return snr.cpu().numpy()
 
 
-def st_track_params(n_t, n_f, seed, track_id, n_min, n_max, tau_lo=0.0, tau_hi=0.0, df=1.0, f_min=0.0):
+def st_track_params(n_t, n_f, seed, track_id, n_min, n_max, tau_lo=0.0, tau_hi=0.0, df=1.0, f_min=0.0,
+                    family=FAMILY_QUADRATIC):
     """S1 as a pure host function (no GPU needed)."""
     L = load_library()
     ctx = C.c_void_p()
@@ -520,7 +528,7 @@ def st_track_params(n_t, n_f, seed, track_id, n_min, n_max, tau_lo=0.0, tau_hi=0
         raise StError(rc, "st_create")
     try:
         t = CTrack()
-        rc = L.st_track_params(ctx, seed, track_id, n_min, n_max, tau_lo, tau_hi, C.byref(t))
+        rc = L.st_track_params_family(ctx, seed, track_id, n_min, n_max, tau_lo, tau_hi, int(family), C.byref(t))
         if rc:
             raise StError(rc, "st_track_params: invalid arguments")
         return t

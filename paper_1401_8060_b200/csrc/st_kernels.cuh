@@ -71,6 +71,7 @@ struct DeviceResult {
 
 struct ScoreArgs {
     const float2* map;        // p[j * n_f + k]
+    const float* isig;        // 1 / sigma per pixel (0 where masked): the weights of norm 2 (G25)
     BankParams bp;
     double f_min, df;
     uint64_t track_offset;    // id of template 0 of this launch
@@ -169,6 +170,23 @@ __host__ __device__ __forceinline__ float norm_scale(int32_t N, int32_t norm)
 #else
     return norm == 0 ? (float)(1.0 / sqrt((double)N)) : (float)(1.0 / (double)N);
 #endif
+}
+
+// The per-template scale of Eq. 8: N^-alpha, or for the inverse-variance weighting (norm 2; fn. 23,
+// PAPER.md:342, reading G25) 1 / sqrt(sum_Gamma 1/sigma^2) from the partial sums w2 of `width` adjacent lanes.
+__device__ __forceinline__ float inv_sqrt_pos(float w)
+{
+    if (!(w > 0.0f)) return 0.0f;              // every pixel masked: the template scores 0
+    const float y = rsqrtf(w);
+    return y * fmaf(-0.5f * w * y, y, 1.5f);
+}
+template <int WIDTH = 32>
+__device__ __forceinline__ float track_scale(const int32_t norm, const int32_t N, float w2)
+{
+    if (norm != 2) return norm_scale(N, norm);
+#pragma unroll
+    for (int off = WIDTH / 2; off >= 1; off >>= 1) w2 += __shfl_xor_sync(kFull, w2, off);
+    return inv_sqrt_pos(w2);
 }
 
 // Per-warp reduction state (S4).
@@ -304,12 +322,18 @@ __device__ __forceinline__ float2 prepare_pixel(float2 c, float s)
     if (!(s > 0.0f) || isinf(s)) return make_float2(0.0f, 0.0f);
     return make_float2(__fdiv_rn(c.x, s), __fdiv_rn(c.y, s));
 }
+// 1 / sigma, 0 where the pixel is masked: the weight plane of the inverse-variance statistic (G25)
+__device__ __forceinline__ float inv_sigma_pixel(float s)
+{
+    return (!(s > 0.0f) || isinf(s)) ? 0.0f : __fdiv_rn(1.0f, s);
+}
 // HBM bound (16 B read + 8 B written per pixel with a per-pixel sigma).  VEC: two pixels per thread
 // per iteration through 16-byte loads and stores (the host checks alignment and parity), two
 // iterations in flight.
 template <bool VEC>
 __global__ void __launch_bounds__(256) k_prepare_map(const float2* __restrict__ csd, const float* __restrict__ sigma,
-                                                     int sigma_kind, int n_f, size_t n_pix, float2* __restrict__ p)
+                                                     int sigma_kind, int n_f, size_t n_pix, float2* __restrict__ p,
+                                                     float* __restrict__ isig)
 {
     const size_t stride = (size_t)gridDim.x * blockDim.x, t0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (VEC) {
@@ -338,12 +362,17 @@ __global__ void __launch_bounds__(256) k_prepare_map(const float2* __restrict__ 
             }
             p4[i] = make_float4(r0.x, r0.y, r1.x, r1.y);
             if (two) p4[j] = make_float4(r2.x, r2.y, r3.x, r3.y);
+            float2* i2 = reinterpret_cast<float2*>(isig);
+            i2[i] = sigma_kind != 0 ? make_float2(inv_sigma_pixel(sa.x), inv_sigma_pixel(sa.y)) : make_float2(1.0f, 1.0f);
+            if (two) i2[j] = sigma_kind != 0 ? make_float2(inv_sigma_pixel(sb.x), inv_sigma_pixel(sb.y)) : make_float2(1.0f, 1.0f);
         }
     } else {
         for (size_t i = t0; i < n_pix; i += stride) {
             float2 c = csd[i];
-            if (sigma_kind != 0) c = prepare_pixel(c, sigma_kind == 1 ? sigma[i % (size_t)n_f] : sigma[i]);
+            const float sg = sigma_kind == 0 ? 1.0f : (sigma_kind == 1 ? sigma[i % (size_t)n_f] : sigma[i]);
+            if (sigma_kind != 0) c = prepare_pixel(c, sg);
             p[i] = c;
+            isig[i] = inv_sigma_pixel(sg);
         }
     }
 }
@@ -441,15 +470,19 @@ __global__ void __launch_bounds__(256) k_score_table(const ScoreArgs a)
         if (q >= a.n_tracks) break;
         const uint64_t id = a.track_offset + q;
         const Track t = load_track(a, q, id);
-        const Raster r = make_raster(t, a.bp.n_f);
+        const Raster r = make_raster(t, a.bp.n_f, a.bp.family);
+        float w2 = 0.0f;
         for (int c = lane; c < t.N; c += kWarp) {
             const int k = raster_bin_fast(r, c);
-            pool_p[c] = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k]);
+            const size_t pix = (size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k;
+            float2 pv = __ldg(&a.map[pix]);
+            if (a.norm == 2) { const float rs = __ldg(&a.isig[pix]); pv.x *= rs; pv.y *= rs; w2 = fmaf(rs, rs, w2); }
+            pool_p[c] = pv;
             pool_k[c] = (uint16_t)k;
         }
         __syncwarp();
         wr.pixels += (unsigned long long)t.N;
-        const float scale = norm_scale(t.N, a.norm);
+        const float scale = track_scale(a.norm, t.N, w2);
         TrackMax tm;
         tmax_init(tm);
         for (int mb = 0; mb < a.n_tau; mb += kWarp) {
@@ -556,7 +589,8 @@ __device__ __forceinline__ void reduce_samples_multi(const ScoreArgs& a, WarpRed
 #endif
 // KDUMP: parity export -- the bins this kernel's own fast path (Horner form, regenerate-on-fallback) decides
 // are written to a.k_dump next to the scores (st_debug_rasterise_random).
-template <bool CAPTURE, bool KDUMP>
+// GEN as in the Chebyshev kernel: false = quadratic bank templates with N^-alpha (options compiled in as constants).
+template <bool CAPTURE, bool KDUMP, bool GEN>
 __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -577,15 +611,17 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
         const uint64_t q = q0 + (uint64_t)grp;
         const bool live = q < a.n_tracks;                    // the last claim may be ragged
         const uint64_t id = a.track_offset + (live ? q : q0);
-        const Track t = load_track(a, live ? q : q0, id);
-        const RasterFast r = make_raster_fast(t, a.bp.n_f);
+        const Track t = GEN ? load_track(a, live ? q : q0, id) : make_track(a.bp, id);
+        const int family = GEN ? a.bp.family : 0;
+        const int norm = GEN ? a.norm : (a.norm == 1 ? 1 : 0);
+        const RasterFast r = make_raster_fast(t, a.bp.n_f, family);
         const int N = live ? t.N : 0;
         int n_max = N;
 #pragma unroll
         for (int off = 16; off >= kRandGroup; off >>= 1) n_max = max(n_max, __shfl_xor_sync(kFull, n_max, off));
         const double u_last = int_to_double_fast(t.N - 1) + 0.5;
         const float2* col0 = a.map + (size_t)t.j0 * (size_t)a.bp.n_f;
-        float acc = 0.0f;
+        float acc = 0.0f, w2 = 0.0f;
         double ub = u_sub;                                    // column centre of this lane in the current pass
 #pragma unroll 1
         for (int c0 = sub; c0 < n_max; c0 += 4 * kRandGroup, ub += 4.0 * kRandGroup) {
@@ -601,7 +637,7 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
             if (redo[0] | redo[1] | redo[2] | redo[3]) {  // ~1e-5 of the time: normative sequence
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
-                    if (redo[u]) kq[u] = raster_bin(make_raster(load_track(a, live ? q : q0, id), a.bp.n_f), cq[u]);
+                    if (redo[u]) kq[u] = raster_bin(make_raster(GEN ? load_track(a, live ? q : q0, id) : make_track(a.bp, id), a.bp.n_f, family), cq[u]);
             }
             if (KDUMP) {
 #pragma unroll
@@ -614,6 +650,14 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
             for (int u = 0; u < 4; ++u) {
                 ST_ASSERT(kq[u] >= 0 && kq[u] < a.bp.n_f && cq[u] >= 0 && t.j0 + cq[u] < a.bp.n_t);
                 pv[u] = __ldg(col0 + (size_t)cq[u] * (size_t)a.bp.n_f + (size_t)kq[u]);
+            }
+            if (GEN && norm == 2) {                       // inverse-variance weights (G25): one more gather per pixel
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const float rs = __ldg(a.isig + ((size_t)(t.j0 + cq[u]) * (size_t)a.bp.n_f + (size_t)kq[u]));
+                    pv[u].x *= rs; pv[u].y *= rs;
+                    if (c0 + u * kRandGroup < N) w2 = fmaf(rs, rs, w2);
+                }
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
@@ -630,7 +674,7 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
 #pragma unroll
         for (int off = kRandGroup / 2; off >= 1; off >>= 1) acc += __shfl_xor_sync(kFull, acc, off);
         if (sub == 0) wr.pixels += (unsigned long long)N;
-        reduce_samples_multi<CAPTURE ? 1 : 0>(a, wr, sm_hist, id, q, acc * norm_scale(t.N, a.norm), live && sub == 0);
+        reduce_samples_multi<CAPTURE ? 1 : 0>(a, wr, sm_hist, id, q, acc * track_scale<kRandGroup>(norm, t.N, w2), live && sub == 0);
     }
     // wr.pixels was accumulated by the four group leaders: fold them into lane 0 for reduce_finish
     {
@@ -680,18 +724,21 @@ __global__ void __launch_bounds__(512, 1) k_score_recur(const ScoreArgs a)
         if (q >= a.n_tracks) break;
         const uint64_t id = a.track_offset + q;
         const Track t = load_track(a, q, id);
-        const Raster r = make_raster(t, a.bp.n_f);
+        const Raster r = make_raster(t, a.bp.n_f, a.bp.family);
         TrackMax tm;
         tmax_init(tm);
         // ---- phase A: rasterise, gather, rotate to tau_0
         const int n_pad = (t.N + 63) & ~63;          // pairs of 32-pixel rows
+        float w2 = 0.0f;
 #pragma unroll 2
         for (int c = lane; c < n_pad; c += kWarp) {
             float2 v = make_float2(0.0f, 0.0f);
             int k = 0;
             if (c < t.N) {
                 k = raster_bin_fast(r, c);
-                const float2 p = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k]);
+                const size_t pix = (size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)k;
+                float2 p = __ldg(&a.map[pix]);
+                if (a.norm == 2) { const float rs = __ldg(&a.isig[pix]); p.x *= rs; p.y *= rs; w2 = fmaf(rs, rs, w2); }
                 const float2 e = __ldg(&a.E0[k]);
                 v.x = p.x * e.x - p.y * e.y;
                 v.y = p.x * e.y + p.y * e.x;
@@ -701,7 +748,7 @@ __global__ void __launch_bounds__(512, 1) k_score_recur(const ScoreArgs a)
         }
         __syncwarp();
         wr.pixels += (unsigned long long)t.N;
-        const float scale = norm_scale(t.N, a.norm);
+        const float scale = track_scale(a.norm, t.N, w2);
         // ---- phase B: chunks of CH delays
         for (int j = 0; j < n_chunks; ++j) {
             float acc[CH];
@@ -865,12 +912,12 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
         if (q >= a.n_tracks) break;
         const uint64_t id = a.track_offset + q;
         const Track t = load_track(a, q, id);
-        const Raster r = make_raster(t, a.bp.n_f);
+        const Raster r = make_raster(t, a.bp.n_f, a.bp.family);
         TrackMax tm;
         tmax_init(tm);
         const int n_prows = (t.N + 63) >> 6;         // packed rows: columns [64 pr, 64 pr + 64)
         wr.pixels += (unsigned long long)t.N;
-        const float scale = norm_scale(t.N, a.norm);
+        float scale = 0.0f, w2 = 0.0f;
 #pragma unroll 1
         for (int j = 0; j < n_chunks; ++j) {
             if ((j & (kSuper / kChunk - 1)) == 0) {
@@ -909,8 +956,15 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
                         const int prow = pr + (u >> 1) < n_prows ? pr + (u >> 1) : n_prows - 1;
                         int c = prow * 64 + (u & 1) * kWarp + lane;
                         c = c < t.N ? c : t.N - 1;       // clamped: the value is discarded below
-                        pv[u] = __ldg(&a.map[(size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)kq[u]]);
+                        const size_t pix = (size_t)(t.j0 + c) * (size_t)a.bp.n_f + (size_t)kq[u];
+                        pv[u] = __ldg(&a.map[pix]);
                         wv[u] = __ldg(&Es[kq[u]]);
+                        if (a.norm == 2) {
+                            const float rs = __ldg(&a.isig[pix]);
+                            pv[u].x *= rs; pv[u].y *= rs;
+                            const int cu = prow * 64 + (u & 1) * kWarp + lane;          // unclamped column of this slot
+                            if (s == 0 && pr + (u >> 1) < n_prows && cu < t.N) w2 = fmaf(rs, rs, w2);
+                        }
                     }
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
@@ -931,6 +985,7 @@ __global__ void __launch_bounds__(512, 1) k_score_reinsch(const ScoreArgs a)
                         }
                     }
                 }
+                if (s == 0) scale = track_scale(a.norm, t.N, w2);
             }
             // ---- one chunk of 32 delays: four pixels of the lane in flight (two register pairs).
             // Per delay and pair: two scalar FFMAs (d += -kappa x on the halves; a packed FFMA with
@@ -1080,18 +1135,22 @@ struct ChebFetchCtx {          // what fetching needs to know about a template
     const float2* col0;        // map row of the template's first column
     int32_t N, L, cbase;       // columns, columns per lane, first column of this lane
 };
-struct ChebElem { int k[4]; float2 p[4], e[4]; };
-struct ChebMergeState { int run_k, n_merged; float ax, ay; float2 run_e; };
+struct ChebElem { int k[4]; float2 p[4], e[4]; float r[4]; };     // r: 1 / sigma, only loaded for norm 2
+struct ChebMergeState { int run_k, n_merged; float ax, ay; float2 run_e; float w2; };
 
+// GEN = false compiles the default search (quadratic templates, N^-alpha normalisation) with the template
+// family and the weighting as constants; GEN = true reads both from the arguments (cubic family, norm 2).
+template <bool GEN>
 __device__ __forceinline__ void cheb_fetch_ctx(const ScoreArgs& a, const Track& t, const int lane, ChebFetchCtx& f)
 {
-    f.r = make_raster(t, a.bp.n_f);
+    f.r = make_raster(t, a.bp.n_f, GEN ? a.bp.family : 0);
     f.N = t.N;
     f.L = (t.N + kWarp - 1) >> 5;
     f.cbase = lane * f.L;
     f.u_last = int_to_double_fast(t.N - 1) + 0.5;
     f.col0 = a.map + (size_t)t.j0 * (size_t)a.bp.n_f;
 }
+template <bool GEN>
 __device__ __forceinline__ void cheb_fetch(const ScoreArgs& a, const ChebFetchCtx& f, const int i, ChebElem& E)
 {
     bool redo[4];
@@ -1116,10 +1175,15 @@ __device__ __forceinline__ void cheb_fetch(const ScoreArgs& a, const ChebFetchCt
         E.p[u] = __ldg(f.col0 + (size_t)cc[u] * (size_t)a.bp.n_f + (size_t)E.k[u]);
         E.e[u] = __ldg(&a.Ec[E.k[u]]);
     }
+    if (GEN && a.norm == 2) {                          // inverse-variance weights (G25): one more gather per pixel
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            E.r[u] = __ldg(a.isig + ((size_t)(f.col0 - a.map) + (size_t)cc[u] * (size_t)a.bp.n_f + (size_t)E.k[u]));
+    }
 }
 __device__ __forceinline__ void cheb_merge_init(ChebMergeState& m)
 {
-    m.run_k = -1; m.n_merged = 0; m.ax = 0.0f; m.ay = 0.0f; m.run_e = make_float2(0.0f, 0.0f);
+    m.run_k = -1; m.n_merged = 0; m.ax = 0.0f; m.ay = 0.0f; m.run_e = make_float2(0.0f, 0.0f); m.w2 = 0.0f;
 }
 // append the finished runs of the lanes flagged `emit` (a warp-wide ballot keeps the pool compact)
 __device__ __forceinline__ void cheb_emit(ChebMergeState& m, const bool emit, float2* pool_v, uint16_t* pool_k, const int lane)
@@ -1132,7 +1196,7 @@ __device__ __forceinline__ void cheb_emit(ChebMergeState& m, const bool emit, fl
     }
     m.n_merged += __popc(em);
 }
-__device__ __forceinline__ void cheb_merge(const int N, const int L, const int cbase, const int i, const ChebElem& E,
+__device__ __forceinline__ void cheb_merge(const int norm, const int N, const int L, const int cbase, const int i, const ChebElem& E,
                                            ChebMergeState& m, float2* pool_v, uint16_t* pool_k, const int lane)
 {
 #pragma unroll
@@ -1141,7 +1205,12 @@ __device__ __forceinline__ void cheb_merge(const int N, const int L, const int c
         const bool brk = valid && E.k[u] != m.run_k;   // a new run starts at this column
         cheb_emit(m, brk && m.run_k >= 0, pool_v, pool_k, lane);
         // branch-free update: a break restarts the sums, a column outside the template adds zero
-        const float px = valid ? E.p[u].x : 0.0f, py = valid ? E.p[u].y : 0.0f;
+        float px = valid ? E.p[u].x : 0.0f, py = valid ? E.p[u].y : 0.0f;
+        if (norm == 2) {                               // warp-uniform
+            const float rs = valid ? E.r[u] : 0.0f;
+            px *= rs; py *= rs;
+            m.w2 = fmaf(rs, rs, m.w2);
+        }
         m.ax = brk ? px : m.ax + px;
         m.ay = brk ? py : m.ay + py;
         m.run_k = brk ? E.k[u] : m.run_k;
@@ -1160,24 +1229,27 @@ __device__ __forceinline__ int cheb_merge_finish(ChebMergeState& m, float2* pool
 }
 
 // Phase A for one template, start to finish (the next element is in flight while one is merged).
+template <bool GEN>
 __device__ __forceinline__ int cheb_phase_a(const ScoreArgs& a, const Track& t, float2* pool_v, uint16_t* pool_k,
-                                            const int lane)
+                                            const int lane, float& scale)
 {
     ChebFetchCtx f;
-    cheb_fetch_ctx(a, t, lane, f);
+    cheb_fetch_ctx<GEN>(a, t, lane, f);
+    const int norm = GEN ? a.norm : (a.norm == 1 ? 1 : 0);
     ChebMergeState m;
     cheb_merge_init(m);
     ChebElem E0, E1;                                   // ping-pong: no register copies between elements
     __syncwarp();                                      // the previous template's pool reads are done
-    cheb_fetch(a, f, 0, E0);
+    cheb_fetch<GEN>(a, f, 0, E0);
 #pragma unroll 1
     for (int i = 0; i < f.L; i += 8) {
-        if (i + 4 < f.L) cheb_fetch(a, f, i + 4, E1);  // warp-uniform
-        cheb_merge(f.N, f.L, f.cbase, i, E0, m, pool_v, pool_k, lane);
+        if (i + 4 < f.L) cheb_fetch<GEN>(a, f, i + 4, E1);  // warp-uniform
+        cheb_merge(norm, f.N, f.L, f.cbase, i, E0, m, pool_v, pool_k, lane);
         if (i + 4 >= f.L) break;
-        if (i + 8 < f.L) cheb_fetch(a, f, i + 8, E0);
-        cheb_merge(f.N, f.L, f.cbase, i + 4, E1, m, pool_v, pool_k, lane);
+        if (i + 8 < f.L) cheb_fetch<GEN>(a, f, i + 8, E0);
+        cheb_merge(norm, f.N, f.L, f.cbase, i + 4, E1, m, pool_v, pool_k, lane);
     }
+    scale = track_scale(norm, t.N, m.w2);
     return cheb_merge_finish(m, pool_v, pool_k, lane);
 }
 
@@ -1301,7 +1373,7 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
     if (MODE == 2) tmax_finish(a, tm, q);
 }
 
-template <int STRIDE, int MODE>
+template <int STRIDE, int MODE, bool GEN>
 __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -1328,12 +1400,13 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
         if (q >= a.n_tracks) break;
         if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
         const uint64_t id = a.track_offset + q;
-        const Track t = load_track(a, q, id);
+        const Track t = GEN ? load_track(a, q, id) : make_track(a.bp, id);     // explicit templates take the general build
         wr.pixels += (unsigned long long)t.N;
-        const int n_merged = cheb_phase_a(a, t, pool_v, pool_k, lane);
+        float scale;
+        const int n_merged = cheb_phase_a<GEN>(a, t, pool_v, pool_k, lane, scale);
         ST_ASSERT(n_merged >= 1 && n_merged <= t.N && ((n_merged + kWarp - 1) & ~(kWarp - 1)) <= S &&
                   (a.tracks || (t.N >= a.bp.n_min && t.N <= a.bp.n_max)) && t.j0 >= 0 && t.j0 + t.N <= a.bp.n_t);
-        cheb_phase_b<STRIDE, MODE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, n_merged, norm_scale(t.N, a.norm), id, q,
+        cheb_phase_b<STRIDE, MODE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, n_merged, scale, id, q,
                              n_chunks, lane);
     }
     reduce_finish(a, wr);
@@ -1343,27 +1416,35 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
 // ----------------------------------------------------------------------- S4 --
 // Float64 score of one (template, delay): Eq. 8 with cos/sin of 2 pi f tau in
 // double, lanes over columns, fixed-order shuffle tree.  All lanes return it.
-__device__ __forceinline__ double score_f64(const float2* __restrict__ map, const BankParams& bp,
+__device__ __forceinline__ double score_f64(const float2* __restrict__ map, const float* __restrict__ isig, const BankParams& bp,
                                             double f_min, double df, const Track& t, double tau, int norm)
 {
     const int lane = threadIdx.x & 31;
-    const Raster r = make_raster(t, bp.n_f);
-    double acc = 0.0;
+    const Raster r = make_raster(t, bp.n_f, bp.family);
+    double acc = 0.0, w2 = 0.0;
     for (int c = lane; c < t.N; c += kWarp) {
         const int k = raster_bin_fast(r, c);
-        const float2 p = map[(size_t)(t.j0 + c) * (size_t)bp.n_f + (size_t)k];
+        const size_t pix = (size_t)(t.j0 + c) * (size_t)bp.n_f + (size_t)k;
+        const float2 p = map[pix];
         const double phi = kTwoPi * (f_min + (double)k * df) * tau;
         double s, co;
         sincos(phi, &s, &co);
-        acc += co * (double)p.x - s * (double)p.y;
+        const double rho = co * (double)p.x - s * (double)p.y;
+        if (norm == 2) { const double rs = (double)isig[pix]; acc += rho * rs; w2 += rs * rs; }
+        else acc += rho;
     }
 #pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) acc += __shfl_xor_sync(kFull, acc, off);
+    for (int off = 16; off >= 1; off >>= 1) {
+        acc += __shfl_xor_sync(kFull, acc, off);
+        w2 += __shfl_xor_sync(kFull, w2, off);
+    }
+    if (norm == 2) return w2 > 0.0 ? acc / sqrt(w2) : 0.0;
     return acc / (norm == 0 ? sqrt((double)t.N) : (double)t.N);
 }
 
 struct FinalArgs {
     const float2* map;
+    const float* isig;
     BankParams bp;
     double f_min, df;
     int32_t norm, tau_mode, n_tau;
@@ -1401,7 +1482,7 @@ __global__ void __launch_bounds__(256) k_finalize(const FinalArgs a)
             if (!(c.snr >= thr)) continue;
             const Track t = make_track(a.bp, c.id);
             const double tau = a.tau_mode == 0 ? a.tau_d[c.m] : t.tau;
-            const double s = score_f64(a.map, a.bp, a.f_min, a.df, t, tau, a.norm);
+            const double s = score_f64(a.map, a.isig, a.bp, a.f_min, a.df, t, tau, a.norm);
             ++n_scored;
             if (!have || s > best || (s == best && (c.id < bid || (c.id == bid && c.m < bm)))) {
                 have = 1; best = s; bid = c.id; bm = c.m; bf32 = c.snr;
@@ -1441,12 +1522,12 @@ __global__ void __launch_bounds__(256) k_finalize(const FinalArgs a)
         }
         DeviceResult res;
         res.max_snr = gmax; res.arg_m = 0; res.snr_f64 = 0.0; res.arg_id = 0; res.arg_tau = 0.0;
-        res.track.N = 0; res.track.j0 = 0; res.track.a = res.track.y0 = res.track.y1 = res.track.y2 = res.track.tau = 0.0;
+        res.track.N = 0; res.track.j0 = 0; res.track.a = res.track.y0 = res.track.y1 = res.track.y2 = res.track.tau = res.track.y3 = 0.0;
         res.n_candidates = total; res.flags = overflow ? 1 : 0; res.n_pixels = a.sc->n_pixels;
         if (have) {
             const Track t = make_track(a.bp, bid);
             const double tau = a.tau_mode == 0 ? a.tau_d[bm] : t.tau;
-            const double s = overflow ? score_f64(a.map, a.bp, a.f_min, a.df, t, tau, a.norm) : best;
+            const double s = overflow ? score_f64(a.map, a.isig, a.bp, a.f_min, a.df, t, tau, a.norm) : best;
             res.arg_m = (int32_t)bm; res.snr_f64 = s; res.arg_id = bid; res.arg_tau = tau; res.track = t;
             if (overflow) res.n_candidates = 1;
         }
@@ -1464,7 +1545,7 @@ __global__ void __launch_bounds__(256) k_rescore_cands(const FinalArgs a, double
         const Cand c = a.cand[i];
         const Track t = make_track(a.bp, c.id);
         const double tau = a.tau_mode == 0 ? a.tau_d[c.m] : t.tau;
-        const double s = score_f64(a.map, a.bp, a.f_min, a.df, t, tau, a.norm);
+        const double s = score_f64(a.map, a.isig, a.bp, a.f_min, a.df, t, tau, a.norm);
         if (lane == 0) snr64[i] = s;
     }
 }
@@ -1479,16 +1560,16 @@ __global__ void k_debug_rasterise(BankParams bp, uint64_t first, uint64_t count,
     const uint64_t n_w = ((uint64_t)gridDim.x * blockDim.x) >> 5;
     for (uint64_t q = gw; q < count; q += n_w) {
         const Track t = make_track(bp, first + q);
-        const Raster r = make_raster(t, bp.n_f);
+        const Raster r = make_raster(t, bp.n_f, bp.family);
         int32_t* row = k_out + q * (uint64_t)bp.n_t;
         for (int c = lane; c < bp.n_t; c += kWarp) row[c] = c < t.N ? raster_bin_fast(r, c) : -1;
         if (lane == 0) { j0_out[q] = t.j0; N_out[q] = t.N; }
     }
 }
 
-__global__ void k_debug_rasterise_track(Track t, int32_t n_f, int32_t* __restrict__ k_out)
+__global__ void k_debug_rasterise_track(Track t, int32_t n_f, int32_t family, int32_t* __restrict__ k_out)
 {
-    const Raster r = make_raster(t, n_f);
+    const Raster r = make_raster(t, n_f, family);
     for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < t.N; c += gridDim.x * blockDim.x)
         k_out[c] = raster_bin_fast(r, c);
 }

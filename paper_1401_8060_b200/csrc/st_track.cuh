@@ -3,6 +3,9 @@
 // S1: PAPER.md:75, :86 ("each template can be quickly generated from just six
 //     random numbers"), :100 (Delta tau ~ U(+-Delta tau_max)); readings G3-G5 of DESIGN.md.
 // S2: PAPER.md:83 (Eq. 6), :73 (N = pixels in Gamma); readings G2, G15.
+// Second template family (PAPER.md:75 "other parameterizable curves", :246-252, :287; reading G26): a cubic
+// Bezier curve whose time control points are the degree-elevated quadratic (so t(xi) and its root are those
+// of the quadratic family) and whose frequency has four control points; the extra random number is r7.
 //
 // Everything here is __host__ __device__ so that st_track_params (host, pure)
 // and the kernels share one statement of the arithmetic.  The rasteriser is a
@@ -73,12 +76,15 @@ ST_HD Words8 track_words(uint64_t seed, uint64_t id)
 struct Track {
     int32_t N, j0;
     double a, y0, y1, y2, tau;
+    double y3;            // cubic family: f_end (then y1, y2 are the inner control points); else unused
 };
 
 struct BankParams {       // what S1 needs besides (seed, id)
     uint64_t seed;
     int32_t n_t, n_f, n_min, n_max;
     double tau_lo, tau_hi;
+    int32_t family;       // 0 quadratic (Eq. 6), 1 cubic in frequency (G26)
+    int32_t pad;
 };
 
 // S1.  N uniform in [n_min, n_max]; first column uniform among the feasible
@@ -99,25 +105,36 @@ ST_HD Track make_track(const BankParams& bp, uint64_t id)
     t.y2 = ST_DMUL(ST_DMUL((double)w.r[5] + 0.5, dF), kTwoM32);
     const double u = ST_DMUL((double)w.r[6] + 0.5, kTwoM32);
     t.tau = ST_DADD(bp.tau_lo, ST_DMUL(ST_DSUB(bp.tau_hi, bp.tau_lo), u));
+    t.y3 = bp.family ? ST_DMUL(ST_DMUL((double)w.r[7] + 0.5, dF), kTwoM32) : 0.0;
     return t;
 }
 
 // Per-track constants of S2.
 struct Raster {
-    double a, cc, aa, y0, y1, y2;
+    double a, cc, aa, y0, y1, y2, y3;
     double guard;      // fast path: distance from a bin edge below which the normative sequence decides
     int32_t kmax;
+    int32_t family;
 };
 
-ST_HD Raster make_raster(const Track& t, int32_t n_f)
+// guard of the fast path: |y_fast - y_normative| <= |dy/dxi| * 6e-12 with |dy/dxi| <= 2 n_f (quadratic) or
+// 3 n_f (cubic); a factor 3 is left on top
+ST_HD double raster_guard(int32_t n_f, int32_t family)
+{
+    const double g = (family ? 6e-11 : 4e-11) * (double)n_f;
+    return g > 1e-6 ? g : 1e-6;
+}
+
+ST_HD Raster make_raster(const Track& t, int32_t n_f, int32_t family)
 {
     Raster r;
     r.a  = t.a;
     r.cc = ST_DSUB((double)t.N, ST_DMUL(2.0, t.a));   // N - 2a
     r.aa = ST_DMUL(t.a, t.a);
-    r.y0 = t.y0; r.y1 = t.y1; r.y2 = t.y2;
+    r.y0 = t.y0; r.y1 = t.y1; r.y2 = t.y2; r.y3 = t.y3;
     r.kmax = n_f - 1;
-    r.guard = 4e-11 * (double)n_f > 1e-6 ? 4e-11 * (double)n_f : 1e-6;
+    r.family = family;
+    r.guard = raster_guard(n_f, family);
     return r;
 }
 
@@ -134,10 +151,22 @@ ST_HD int32_t raster_bin(const Raster& r, int32_t c)
     const double den = ST_DADD(r.a, s);
     const double xi  = ST_DDIV(u, den);
     const double om  = ST_DSUB(1.0, xi);
-    const double b0  = ST_DMUL(om, om);
-    const double b1  = ST_DMUL(2.0, ST_DMUL(om, xi));
-    const double b2  = ST_DMUL(xi, xi);
-    const double y   = ST_DADD(ST_DADD(ST_DMUL(b0, r.y0), ST_DMUL(b1, r.y1)), ST_DMUL(b2, r.y2));
+    double y;
+    if (r.family == 0) {
+        const double b0  = ST_DMUL(om, om);
+        const double b1  = ST_DMUL(2.0, ST_DMUL(om, xi));
+        const double b2  = ST_DMUL(xi, xi);
+        y = ST_DADD(ST_DADD(ST_DMUL(b0, r.y0), ST_DMUL(b1, r.y1)), ST_DMUL(b2, r.y2));
+    } else {
+        // cubic Bernstein form, normative order ((b0 y0 + b1 y1) + b2 y2) + b3 y3 (G26)
+        const double om2 = ST_DMUL(om, om);
+        const double xi2 = ST_DMUL(xi, xi);
+        const double b0  = ST_DMUL(om2, om);
+        const double b1  = ST_DMUL(3.0, ST_DMUL(om2, xi));
+        const double b2  = ST_DMUL(3.0, ST_DMUL(om, xi2));
+        const double b3  = ST_DMUL(xi2, xi);
+        y = ST_DADD(ST_DADD(ST_DADD(ST_DMUL(b0, r.y0), ST_DMUL(b1, r.y1)), ST_DMUL(b2, r.y2)), ST_DMUL(b3, r.y3));
+    }
     const double fl  = floor(y);
     int32_t k;
     if (!(fl >= 0.0)) k = 0;
@@ -177,7 +206,10 @@ __device__ __forceinline__ double raster_y_fast(const Raster& r, double u)
 {
     const double xi = raster_xi_fast(r, u);
     const double om = 1.0 - xi;
-    return fma(om * om, r.y0, fma(2.0 * (om * xi), r.y1, (xi * xi) * r.y2));
+    if (r.family == 0) return fma(om * om, r.y0, fma(2.0 * (om * xi), r.y1, (xi * xi) * r.y2));
+    // cubic: de Casteljau-like nesting ((y0 om + 3 y1 xi) om + 3 y2 xi^2) om + y3 xi^3
+    const double xi2 = xi * xi;
+    return fma(fma(fma(r.y0, om, 3.0 * r.y1 * xi), om, 3.0 * r.y2 * xi2), om, r.y3 * (xi2 * xi));
 }
 // floor(y) as an int (clamped to [0, kmax]); redo when y is within the guard of an integer or NaN
 template <typename R>
@@ -209,28 +241,35 @@ __device__ __forceinline__ int32_t raster_bin_fast(const Raster& r, int32_t c)
 // The fast path's own constants (no y1, y2: the hot kernels hold these 13 registers per template and,
 // on the ~2e-6 of the pixels that need the normative sequence, regenerate the template from its id).
 struct RasterFast {
-    double a, cc, aa, y0, pb, pc, guard;
+    double a, cc, aa, y0, pb, pc, pd, guard;
     int32_t kmax;
 };
-__device__ __forceinline__ RasterFast make_raster_fast(const Track& t, int32_t n_f)
+__device__ __forceinline__ RasterFast make_raster_fast(const Track& t, int32_t n_f, int32_t family)
 {
-    const Raster r = make_raster(t, n_f);
+    const Raster r = make_raster(t, n_f, family);
     RasterFast f;
     f.a = r.a; f.cc = r.cc; f.aa = r.aa; f.y0 = r.y0; f.guard = r.guard; f.kmax = r.kmax;
-    f.pb = 2.0 * (t.y1 - t.y0);                                 // Eq. 6 in Horner form: y = y0 + xi (pb + xi pc)
-    f.pc = (t.y0 - t.y1) + (t.y2 - t.y1);
+    if (family == 0) {
+        f.pb = 2.0 * (t.y1 - t.y0);                             // Eq. 6 in Horner form: y = y0 + xi (pb + xi pc)
+        f.pc = (t.y0 - t.y1) + (t.y2 - t.y1);
+        f.pd = 0.0;
+    } else {                                                    // cubic: y = y0 + xi (pb + xi (pc + xi pd))
+        f.pb = 3.0 * (t.y1 - t.y0);
+        f.pc = 3.0 * ((t.y0 - t.y1) + (t.y2 - t.y1));
+        f.pd = (t.y3 - t.y0) + 3.0 * (t.y1 - t.y2);
+    }
     return f;
 }
 __device__ __forceinline__ double raster_y_fast(const RasterFast& r, double u)
 {
     const double xi = raster_xi_fast(r, u);
-    return fma(xi, fma(xi, r.pc, r.pb), r.y0);                  // error ~1e-12 bins
+    return fma(xi, fma(xi, fma(xi, r.pd, r.pc), r.pb), r.y0);   // error ~1e-12 n_f / 2461 bins (pd = 0: the quadratic, bit for bit)
 }
 // normative bin of column c of template `id` (regenerated: rare path)
 __device__ __forceinline__ int32_t raster_bin_regen(const BankParams& bp, uint64_t id, int32_t c)
 {
     const Track t = make_track(bp, id);
-    return raster_bin(make_raster(t, bp.n_f), c);
+    return raster_bin(make_raster(t, bp.n_f, bp.family), c);
 }
 // exact (double)k for 0 <= k < 2^31 without the I2F conversion
 __device__ __forceinline__ double int_to_double_fast(int32_t k)

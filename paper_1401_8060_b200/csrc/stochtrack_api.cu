@@ -27,7 +27,7 @@ constexpr uint64_t kMaxSamplesPerLaunch = 1ull << 31;   // keeps per-block u32 h
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t map, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, cand64, warp_best, stage_csd, stage_sigma, stage_csd2, stage_sigma2, b_scalars, b_result, b_hist, tracks, total;
+    size_t map, isig, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, cand64, warp_best, stage_csd, stage_sigma, stage_csd2, stage_sigma2, b_scalars, b_result, b_hist, tracks, total;
 };
 
 Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
@@ -36,6 +36,7 @@ Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
     Layout L;
     size_t o = 0;
     L.map = o;         o += align_up(n_pix * sizeof(float2));
+    L.isig = o;        o += align_up(n_pix * sizeof(float));
     L.e0 = o;          o += align_up((size_t)n_f * sizeof(float2));
     L.bintab = o;      o += align_up((size_t)n_f * sizeof(float4));
     L.es = o;          o += align_up((size_t)n_f * (size_t)((max_n_tau + st::kSuper - 1) / st::kSuper) * sizeof(float2));
@@ -77,6 +78,7 @@ struct st_ctx {
     Layout L;
     cudaStream_t stream;
     bool have_ws, have_map;
+    bool have_isig;                    // the 1 / sigma plane matches the map (set by st_set_map, not by the ft-map path)
     std::vector<double> tau_cached;    // grid currently on the device
     int table_kind, table_ch;          // which tables are currently built for tau_cached
     bool w_built;
@@ -137,6 +139,7 @@ st::BankParams bank(const st_ctx* c, const st_search_params* p)
     bp.n_t = c->n_t; bp.n_f = c->n_f; bp.n_min = p->n_min; bp.n_max = p->n_max;
     bp.tau_lo = p->tau_mode == ST_TAU_RANDOM ? p->tau_lo : 0.0;
     bp.tau_hi = p->tau_mode == ST_TAU_RANDOM ? p->tau_hi : 0.0;
+    bp.family = p->family; bp.pad = 0;
     return bp;
 }
 
@@ -159,12 +162,14 @@ int validate(st_ctx* c, const st_search_params* p, bool need_map)
         if (!isfinite(p->tau_lo) || !isfinite(p->tau_hi) || p->tau_hi < p->tau_lo)
             return fail(c, ST_EINVAL, "bad random-tau range");
     }
-    if (p->norm != ST_NORM_SQRT_N && p->norm != ST_NORM_MEAN) return fail(c, ST_EINVAL, "bad norm %d", p->norm);
+    if (p->norm != ST_NORM_SQRT_N && p->norm != ST_NORM_MEAN && p->norm != ST_NORM_INVVAR) return fail(c, ST_EINVAL, "bad norm %d", p->norm);
+    if (p->norm == ST_NORM_INVVAR && need_map && !c->have_isig)
+        return fail(c, ST_ESTATE, "ST_NORM_INVVAR needs sigma: set the map through st_set_map / st_set_map_host / st_search_batch");
+    if (p->family != ST_FAMILY_QUADRATIC && p->family != ST_FAMILY_CUBIC) return fail(c, ST_EINVAL, "bad template family %d", p->family);
     if (p->n_bins < 0 || p->n_bins > ST_MAX_BINS) return fail(c, ST_EINVAL, "n_bins %d outside [0, %d]", p->n_bins, ST_MAX_BINS);
     if (p->n_bins > 0 && !(p->hist_hi > p->hist_lo)) return fail(c, ST_EINVAL, "need hist_hi > hist_lo");
     if (p->kernel < ST_KERNEL_AUTO || p->kernel > ST_KERNEL_CHEBYSHEV || p->kernel == ST_KERNEL_RANDOM)
         return fail(c, ST_EINVAL, "bad kernel %d", p->kernel);
-    if (p->reserved != 0) return fail(c, ST_EINVAL, "reserved must be 0");
     if (p->n_tracks > (1ull << 62) || p->track_offset > (1ull << 62)) return fail(c, ST_EINVAL, "n_tracks / track_offset too large");
     return ST_OK;
 }
@@ -383,9 +388,17 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         const uint64_t need = ((want_warps + st::kRandPerWarp - 1) / st::kRandPerWarp + 7) / 8;   // a warp scores kRandPerWarp templates at a time
         if (blocks > need) blocks = need;
         if (blocks > kWarpSlots / 8) blocks = kWarpSlots / 8;         // one per-warp record slot per resident warp
-        if (a.k_dump) st::k_score_random<false, true><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
-        else if (a.capture_mode) st::k_score_random<true, false><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
-        else st::k_score_random<false, false><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        const bool gen = a.bp.family != 0 || a.norm == 2 || a.tracks != nullptr;
+        if (a.k_dump) {
+            if (gen) st::k_score_random<false, true, true><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+            else st::k_score_random<false, true, false><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        } else if (a.capture_mode) {
+            if (gen) st::k_score_random<true, false, true><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+            else st::k_score_random<true, false, false><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        } else {
+            if (gen) st::k_score_random<false, false, true><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+            else st::k_score_random<false, false, false><<<(unsigned)blocks, threads, smem, c->stream>>>(a);
+        }
     } else if (plan.kernel == ST_KERNEL_TABLE) {
         int threads = 256;
         size_t smem;
@@ -417,15 +430,25 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
-#define ST_LAUNCH_CHEB(STRIDE, MODE)                                                              \
+#define ST_LAUNCH_CHEB(STRIDE, MODE, GEN)                                                         \
     do {                                                                                          \
-        int rc_ = set_smem(c, st::k_score_cheb<STRIDE, MODE>, smem);                              \
+        int rc_ = set_smem(c, st::k_score_cheb<STRIDE, MODE, GEN>, smem);                         \
         if (rc_) return rc_;                                                                      \
-        st::k_score_cheb<STRIDE, MODE><<<(unsigned)blocks, threads, smem, c->stream>>>(a);        \
+        st::k_score_cheb<STRIDE, MODE, GEN><<<(unsigned)blocks, threads, smem, c->stream>>>(a);   \
+    } while (0)
+#define ST_LAUNCH_CHEB_MODE(STRIDE, GEN)                                                          \
+    do {                                                                                          \
+        if (mode == 1) ST_LAUNCH_CHEB(STRIDE, 1, GEN);                                            \
+        else if (mode == 2) ST_LAUNCH_CHEB(STRIDE, 2, GEN);                                       \
+        else ST_LAUNCH_CHEB(STRIDE, 0, GEN);                                                      \
     } while (0)
         const int mode = a.capture_mode ? 1 : (a.tmax_snr ? 2 : 0);
-        if (pk) { if (mode == 1) ST_LAUNCH_CHEB(2, 1); else if (mode == 2) ST_LAUNCH_CHEB(2, 2); else ST_LAUNCH_CHEB(2, 0); }
-        else    { if (mode == 1) ST_LAUNCH_CHEB(1, 1); else if (mode == 2) ST_LAUNCH_CHEB(1, 2); else ST_LAUNCH_CHEB(1, 0); }
+        // the general build (cubic family, inverse-variance weighting, explicit templates) reads its options
+        // at run time; the default search is compiled with them as constants
+        const bool gen = a.bp.family != 0 || a.norm == 2 || a.tracks != nullptr;
+        if (pk) { if (gen) ST_LAUNCH_CHEB_MODE(2, true); else ST_LAUNCH_CHEB_MODE(2, false); }
+        else    { if (gen) ST_LAUNCH_CHEB_MODE(1, true); else ST_LAUNCH_CHEB_MODE(1, false); }
+#undef ST_LAUNCH_CHEB_MODE
 #undef ST_LAUNCH_CHEB
     } else if (plan.kernel == ST_KERNEL_REINSCH) {
         int threads = c->recur_threads;
@@ -479,6 +502,7 @@ st::ScoreArgs base_args(st_ctx* c, const st_search_params* p)
     st::ScoreArgs a;
     memset(&a, 0, sizeof(a));
     a.map = at<float2>(c, c->L.map);
+    a.isig = at<float>(c, c->L.isig);
     a.bp = bank(c, p);
     a.f_min = c->f_min; a.df = c->df;
     a.n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
@@ -544,7 +568,7 @@ void fill_result(st_result* out, const st::DeviceResult& r, int n_tau, int kerne
     out->arg_track = r.arg_id; out->arg_tau = r.arg_tau;
     out->arg_params.N = r.track.N; out->arg_params.j0 = r.track.j0; out->arg_params.a = r.track.a;
     out->arg_params.y0 = r.track.y0; out->arg_params.y1 = r.track.y1; out->arg_params.y2 = r.track.y2;
-    out->arg_params.tau = r.track.tau;
+    out->arg_params.tau = r.track.tau; out->arg_params.y3 = r.track.y3;
     out->n_pixels = r.n_pixels; out->n_evals = r.n_pixels * (uint64_t)n_tau;
     out->n_candidates = r.n_candidates; out->flags = r.flags; out->n_launches = n_launches;
     out->kernel_used = kernel;
@@ -576,7 +600,7 @@ int enqueue_search(st_ctx* c, const st_search_params* p, const Plan& plan, const
     if (time_it) ST_CUDA(c, cudaEventRecord(c->ev1, c->stream));
     st::FinalArgs f;
     memset(&f, 0, sizeof(f));
-    f.map = a.map; f.bp = a.bp; f.f_min = c->f_min; f.df = c->df;
+    f.map = a.map; f.isig = a.isig; f.bp = a.bp; f.f_min = c->f_min; f.df = c->df;
     f.norm = p->norm; f.tau_mode = p->tau_mode; f.n_tau = n_tau;
     f.tau_d = at<double>(c, c->L.tau);
     f.sc = a.sc; f.cand = a.cand; f.cand_cap = kCandCap; f.warp_best = a.warp_best; f.n_warp_slots = kWarpSlots;
@@ -606,7 +630,7 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     if (!c) return ST_EINVAL;
     c->n_t = n_t; c->n_f = n_f; c->df = df; c->f_min = f_min;
     c->ws = nullptr; c->ws_bytes = 0; c->max_n_tau = 0; c->stream = nullptr;
-    c->have_ws = c->have_map = false;
+    c->have_ws = c->have_map = false; c->have_isig = false;
     c->table_kind = kNoTable; c->table_ch = 0; c->w_built = false;
     c->ev0 = c->ev1 = nullptr; c->h_res = nullptr; c->h_hist = nullptr;
     c->copy_stream = nullptr; c->h_bres = nullptr; c->h_bhist = nullptr;
@@ -670,7 +694,7 @@ int st_set_workspace(st_ctx* c, void* ws, size_t bytes, void* cuda_stream)
     c->ws = (unsigned char*)ws; c->ws_bytes = bytes; c->max_n_tau = lo;
     c->L = make_layout(c->n_t, c->n_f, lo);
     c->stream = (cudaStream_t)cuda_stream;
-    c->have_ws = true; c->have_map = false;
+    c->have_ws = true; c->have_map = false; c->have_isig = false;
     c->tau_cached.clear(); c->table_kind = kNoTable; c->w_built = false;
     return ST_OK;
 }
@@ -689,11 +713,11 @@ int st_set_map(st_ctx* c, const void* csd_dev, const float* sigma_dev, int32_t s
     const bool vec = (n_pix % 2 == 0) && ((uintptr_t)csd_dev % 16 == 0) &&
                      (sigma_kind != ST_SIGMA_PER_PIXEL || (uintptr_t)sigma_dev % 8 == 0);
     if (vec) st::k_prepare_map<true><<<blocks, 256, 0, c->stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, c->n_f, n_pix,
-                                                                    at<float2>(c, c->L.map));
+                                                                    at<float2>(c, c->L.map), at<float>(c, c->L.isig));
     else st::k_prepare_map<false><<<blocks, 256, 0, c->stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, c->n_f, n_pix,
-                                                                  at<float2>(c, c->L.map));
+                                                                  at<float2>(c, c->L.map), at<float>(c, c->L.isig));
     ST_CUDA(c, cudaGetLastError());
-    c->have_map = true;
+    c->have_map = true; c->have_isig = true;
     return ST_OK;
 }
 
@@ -816,7 +840,7 @@ int st_search_topk(st_ctx* c, const st_search_params* p, int32_t top_k, st_top_e
     }
     st::FinalArgs f;
     memset(&f, 0, sizeof(f));
-    f.map = a.map; f.bp = a.bp; f.f_min = c->f_min; f.df = c->df;
+    f.map = a.map; f.isig = a.isig; f.bp = a.bp; f.f_min = c->f_min; f.df = c->df;
     f.norm = p->norm; f.tau_mode = p->tau_mode; f.n_tau = n_tau;
     f.tau_d = at<double>(c, c->L.tau);
     f.sc = a.sc; f.cand = a.cand; f.cand_cap = kCandCap;
@@ -1024,7 +1048,7 @@ static int ft_normalise(st_ctx* c, const double2* st_i, const double2* st_j, int
     const int blocks = (int)((n_pix + 255) / 256 < (size_t)(8 * c->n_sm) ? (n_pix + 255) / 256 : (size_t)(8 * c->n_sm));
     st::k_ft_normalise<<<blocks, 256, 0, c->stream>>>(st_i, st_j, c->n_t, c->n_f, n_nb, shift, at<float2>(c, c->L.map));
     ST_CUDA(c, cudaGetLastError());
-    c->have_map = true;
+    c->have_map = true; c->have_isig = false;      // the ft-map path forms p directly: no sigma plane
     return ST_OK;
 }
 
@@ -1116,17 +1140,25 @@ int st_debug_get_map(st_ctx* c, void* p_out_dev)
     return ST_OK;
 }
 
-int st_track_params(const st_ctx* c, uint64_t seed, uint64_t track_id, int32_t n_min, int32_t n_max,
-                    double tau_lo, double tau_hi, st_track* out)
+int st_track_params_family(const st_ctx* c, uint64_t seed, uint64_t track_id, int32_t n_min, int32_t n_max,
+                           double tau_lo, double tau_hi, int32_t family, st_track* out)
 {
     if (!c || !out) return ST_EINVAL;
     if (n_min < 1 || n_max < n_min || n_max > c->n_t) return ST_EINVAL;
+    if (family != ST_FAMILY_QUADRATIC && family != ST_FAMILY_CUBIC) return ST_EINVAL;
     st::BankParams bp;
     bp.seed = seed; bp.n_t = c->n_t; bp.n_f = c->n_f; bp.n_min = n_min; bp.n_max = n_max;
-    bp.tau_lo = tau_lo; bp.tau_hi = tau_hi;
+    bp.tau_lo = tau_lo; bp.tau_hi = tau_hi; bp.family = family; bp.pad = 0;
     const st::Track t = st::make_track(bp, track_id);
     out->N = t.N; out->j0 = t.j0; out->a = t.a; out->y0 = t.y0; out->y1 = t.y1; out->y2 = t.y2; out->tau = t.tau;
+    out->y3 = t.y3;
     return ST_OK;
+}
+
+int st_track_params(const st_ctx* c, uint64_t seed, uint64_t track_id, int32_t n_min, int32_t n_max,
+                    double tau_lo, double tau_hi, st_track* out)
+{
+    return st_track_params_family(c, seed, track_id, n_min, n_max, tau_lo, tau_hi, ST_FAMILY_QUADRATIC, out);
 }
 
 int st_debug_track_words(uint64_t seed, uint64_t track_id, uint32_t* out_host)
@@ -1145,6 +1177,7 @@ int st_debug_rasterise(st_ctx* c, const st_search_params* p, uint64_t first, uin
     if (!p) return fail(c, ST_EINVAL, "params is NULL");
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
     if (p->n_min < 1 || p->n_max < p->n_min || p->n_max > c->n_t) return fail(c, ST_EINVAL, "need 1 <= n_min <= n_max <= n_t");
+    if (p->family != ST_FAMILY_QUADRATIC && p->family != ST_FAMILY_CUBIC) return fail(c, ST_EINVAL, "bad template family %d", p->family);
     if (!k_out_dev || !j0_dev || !N_dev) return fail(c, ST_EINVAL, "output pointer is NULL");
     if (count == 0) return ST_OK;
     const uint64_t need = (count + 7) / 8;
@@ -1154,16 +1187,17 @@ int st_debug_rasterise(st_ctx* c, const st_search_params* p, uint64_t first, uin
     return ST_OK;
 }
 
-int st_debug_rasterise_track(st_ctx* c, const st_track* t, int32_t* k_out_dev)
+int st_debug_rasterise_track(st_ctx* c, const st_track* t, int32_t family, int32_t* k_out_dev)
 {
     DevGuard dev_guard(c);
     if (!c) return ST_EINVAL;
     if (!t || !k_out_dev) return fail(c, ST_EINVAL, "NULL argument");
+    if (family != ST_FAMILY_QUADRATIC && family != ST_FAMILY_CUBIC) return fail(c, ST_EINVAL, "bad template family %d", family);
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
     if (t->N < 1 || t->j0 < 0 || t->j0 + t->N > c->n_t) return fail(c, ST_EINVAL, "track outside the map");
     st::Track d;
-    d.N = t->N; d.j0 = t->j0; d.a = t->a; d.y0 = t->y0; d.y1 = t->y1; d.y2 = t->y2; d.tau = t->tau;
-    st::k_debug_rasterise_track<<<(t->N + 127) / 128, 128, 0, c->stream>>>(d, c->n_f, k_out_dev);
+    d.N = t->N; d.j0 = t->j0; d.a = t->a; d.y0 = t->y0; d.y1 = t->y1; d.y2 = t->y2; d.tau = t->tau; d.y3 = t->y3;
+    st::k_debug_rasterise_track<<<(t->N + 127) / 128, 128, 0, c->stream>>>(d, c->n_f, family, k_out_dev);
     ST_CUDA(c, cudaGetLastError());
     return ST_OK;
 }
@@ -1205,10 +1239,12 @@ int st_score_tracks(st_ctx* c, const st_search_params* p, const st_track* tracks
         const st_track& t = tracks[i];
         if (t.N < 1 || t.j0 < 0 || (int64_t)t.j0 + (int64_t)t.N > (int64_t)c->n_t)
             return fail(c, ST_EINVAL, "tracks[%d] lies outside the map", i);
-        if (!(t.a > 0.0) || !(t.a < (double)t.N) || !isfinite(t.y0) || !isfinite(t.y1) || !isfinite(t.y2) || !isfinite(t.tau))
+        if (!(t.a > 0.0) || !(t.a < (double)t.N) || !isfinite(t.y0) || !isfinite(t.y1) || !isfinite(t.y2) || !isfinite(t.tau) ||
+            !isfinite(t.y3))
             return fail(c, ST_EINVAL, "tracks[%d]: need 0 < a < N and finite control points / delay", i);
         h[(size_t)i].N = t.N; h[(size_t)i].j0 = t.j0; h[(size_t)i].a = t.a;
         h[(size_t)i].y0 = t.y0; h[(size_t)i].y1 = t.y1; h[(size_t)i].y2 = t.y2; h[(size_t)i].tau = t.tau;
+        h[(size_t)i].y3 = t.y3;
         if (t.N < q.n_min) q.n_min = t.N;
         if (t.N > q.n_max) q.n_max = t.N;
     }

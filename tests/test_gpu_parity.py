@@ -799,3 +799,157 @@ def test_context_on_a_device_that_is_not_current(P, orc):
     r = st.search(cfg.n_tracks, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau)
     ref = orc.search(orc.prepare_map(csd, sigma), cfg.f_min, cfg.df, cfg.n_tracks, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau)
     assert (r.arg_track, r.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+
+
+# ------------------------------------------------------------------ statistic variant: inverse-variance weighting (G25)
+@pytest.mark.parametrize("kname", ["auto", "table", "rotation", "reinsch", "chebyshev", "random"])
+def test_inverse_variance_weighted_statistic(P, orc, kname):
+    """ST_NORM_INVVAR (fn. 23; G25): SNR_w = sum(rho / sigma) / sqrt(sum 1 / sigma^2) on the config-5
+    shape with lognormal(0, 0.3) per-pixel sigma plus masked pixels, every kernel: scores within G13, whole search
+    (argmax, float64 re-score, histogram) against the oracle."""
+    cfg = synth.CONFIGS[5]
+    csd, sigma, tau = config_inputs(orc, cfg)
+    sigma = sigma.copy()
+    sigma[:, 700:720] = 0.0                      # a notch (G11): drops out of both sums
+    sigma[333, :] = np.inf
+    tau = synth.tau_linspace(128)
+    st = make_ctx(P, cfg, max_n_tau=128)
+    st.set_map(csd, sigma)
+    p = orc.prepare_map(csd, sigma)
+    r = orc.prepare_inv_sigma(p.shape, sigma)
+    n, first = 1500, 4_000_000
+    kw = dict(tau_range=(-synth.TAU_MAX, synth.TAU_MAX)) if kname == "random" else dict(tau_grid=tau, kernel=KERNELS.get(kname, 0))
+    okw = dict(tau_range=(-synth.TAU_MAX, synth.TAU_MAX)) if kname == "random" else dict(tau_grid=tau)
+    got = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, first, n, norm=P.NORM_INVVAR, **kw)
+    ref = orc.search(p, cfg.f_min, cfg.df, n, cfg.seed, cfg.n_min, cfg.n_max, track_offset=first, norm=orc.NORM_INVVAR,
+                     inv_sigma=r, dump_snr=True, n_bins=cfg.n_bins, **okw)
+    ok, worst = snr_close(got, ref["snr"])
+    assert ok, f"{kname}: worst error {worst:.3f} x tolerance"
+    res = st.search(n, cfg.seed, cfg.n_min, cfg.n_max, track_offset=first, norm=P.NORM_INVVAR, n_bins=cfg.n_bins, **kw)
+    assert (res.arg_track, res.arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+    assert abs(res.max_snr_f64 - ref["max_snr"]) <= 3e-7 * abs(ref["max_snr"])      # float32 p and 1 / sigma
+    ok, why = hist_rule_ok(res.hist, ref["snr"], cfg.hist_lo, cfg.hist_hi, cfg.n_bins)
+    assert ok, why
+    # constant sigma: the weighted statistic IS the sqrt(N) statistic
+    sig_c = np.full((cfg.n_t, cfg.n_f), 0.5, dtype=np.float32)
+    st.set_map(csd, sig_c)
+    a = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, first, 300, norm=P.NORM_INVVAR, **kw)
+    b = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, first, 300, norm=P.NORM_SQRT_N, **kw)
+    assert np.abs(a - b).max() <= 2e-5 * max(1.0, np.abs(b).max())
+
+
+def test_inverse_variance_needs_sigma_and_batches(P, orc):
+    """The weighting needs the map's sigma: after st_set_map_from_strain (no sigma plane) it is ST_ESTATE; in a batch
+    every map brings its own sigma."""
+    import torch
+    cfg = synth.CONFIGS[2]
+    csds = [synth.noise_csd(cfg.n_t, cfg.n_f, 70 + m) for m in range(3)]
+    sigs = [synth.make_sigma("per_pixel", 0.4, cfg.n_t, cfg.n_f, 70 + m) for m in range(3)]
+    tau = synth.tau_linspace(cfg.n_tau)
+    st = make_ctx(P, cfg)
+    res, _ = st.search_batch([torch.from_numpy(c).cuda() for c in csds], [torch.from_numpy(s).cuda() for s in sigs], [5, 6, 7],
+                             4000, cfg.n_min, cfg.n_max, tau_grid=tau, norm=P.NORM_INVVAR, n_bins=cfg.n_bins)
+    refs = orc.search_batch(csds, sigs, [5, 6, 7], cfg.f_min, cfg.df, 4000, cfg.n_min, cfg.n_max, tau_grid=tau,
+                            norm=orc.NORM_INVVAR, n_bins=cfg.n_bins)
+    for a, b in zip(res, refs):
+        assert (a.arg_track, a.arg_tau_index) == (b["arg_track"], b["arg_tau_index"])
+        assert abs(a.max_snr_f64 - b["max_snr"]) <= 3e-7 * abs(b["max_snr"])
+    L = 256
+    n_t, n_f = 24, 60
+    rng = np.random.default_rng(3)
+    s_i, s_j = rng.standard_normal((n_t + 1) * L // 2), rng.standard_normal((n_t + 1) * L // 2)
+    st2 = P.Stochtrack(n_t, n_f, 1.0, 20.0, max_n_tau=64)
+    st2.set_map_from_strain(torch.from_numpy(s_i).cuda(), torch.from_numpy(s_j).cuda(), float(L), L, 4)
+    with pytest.raises(P.StError) as e:
+        st2.search(10, 0, 4, n_t, tau_grid=synth.tau_linspace(16), norm=P.NORM_INVVAR)
+    assert e.value.code == -2
+
+
+# ------------------------------------------------------------------ second template family: cubic (G26)
+@pytest.mark.parametrize("n_t,n_f,f_min,seed,n_min,n_max,first,count", [
+    (1000, 2461, 40.0, 4, 10, 1000, 0, 3000), (1000, 2461, 40.0, 4, 10, 1000, 9_990_000, 1500),
+    (250, 961, 40.0, 1, 10, 250, 2 ** 33 + 5, 3000), (64, 65535, 0.0, 77, 1, 64, 10 ** 12, 60_000),
+    (4096, 2461, 0.0, 77, 3000, 4096, 10 ** 12, 600), (16, 7, 0.0, 77, 1, 16, 10 ** 12, 20_000)])
+def test_cubic_family_indices_bit_exact(P, orc, n_t, n_f, f_min, seed, n_min, n_max, first, count):
+    """S1 + S2 of the cubic family: parameters and every pixel index equal the oracle's bit for bit, through both
+    rasteriser fast paths (the Bernstein form of the grid kernels and the Horner form of the random-delay kernel)."""
+    st = P.Stochtrack(n_t, n_f, 1.0, f_min, max_n_tau=64)
+    st.set_map(np.zeros((n_t, n_f), dtype=np.complex64))
+    p = np.zeros((n_t, n_f), dtype=np.complex128)
+    ref = orc.search(p, f_min, 1.0, count, seed, n_min, n_max, tau_range=(-0.01, 0.01), track_offset=first,
+                     dump_tracks=True, family=orc.FAMILY_CUBIC)
+    k, j0, N = st.debug_rasterise(seed, n_min, n_max, first, count, family=P.FAMILY_CUBIC)
+    assert np.array_equal(N, ref["N"]) and np.array_equal(j0, ref["j0"]) and np.array_equal(k, ref["k"])
+    k, j0, N = st.debug_rasterise_random(seed, n_min, n_max, first, count, family=P.FAMILY_CUBIC)
+    assert np.array_equal(N, ref["N"]) and np.array_equal(j0, ref["j0"]) and np.array_equal(k, ref["k"])
+    for tid in (first, first + count - 1):
+        a = st.track_params(seed, tid, n_min, n_max, -0.01, 0.01, family=P.FAMILY_CUBIC)
+        b = orc.track_params(seed, tid, n_t, n_f, n_min, n_max, -0.01, 0.01, family=orc.FAMILY_CUBIC)
+        assert (a.N, a.j0, a.a, a.y0, a.y1, a.y2, a.tau, a.y3) == (b.N, b.j0, b.a, b.y0, b.y1, b.y2, b.tau, b.y3)
+
+
+def test_cubic_family_explicit_tracks(P, orc):
+    cfg = synth.CONFIGS[5]
+    st = make_ctx(P, cfg)
+    for tr in [(1000, 0, 500.0, 100.5, 100.5, 2400.5, 2400.5), (777, 100, 3.0, 2460.999999, 0.0000001, 2460.999999, 0.5),
+               (10, 5, 1e-9, 100.0, 2000.0, 50.0, 1999.0), (1, 999, 0.5, 7.3, 9.9, 1.2, 2460.99), (500, 250, 250.0, 7.5, 7.5, 7.5, 7.5)]:
+        got = st.debug_rasterise_track(*tr[:6], y3=tr[6])
+        want = orc.rasterise(orc.make_track(*tr[:6], y3=tr[6]), cfg.n_f)
+        assert np.array_equal(got, want), tr
+
+
+@pytest.mark.parametrize("cid,kname,n", [(2, "auto", 20_000), (2, "table", 3000), (2, "rotation", 3000), (2, "reinsch", 3000),
+                                         (5, "auto", 1500), (3, "random", 30_000)])
+def test_cubic_family_search_parity(P, orc, cid, kname, n):
+    """Whole searches with the cubic bank: SNRs within G13, argmax / histogram / float64 re-score against the oracle,
+    and the argmax template's control points (y3 included) bit-exact."""
+    cfg = synth.CONFIGS[cid]
+    csd, sigma, tau = config_inputs(orc, cfg)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    p = orc.prepare_map(csd, sigma)
+    first = 123_456
+    kw = dict(tau_range=(-synth.TAU_MAX, synth.TAU_MAX)) if cfg.tau_mode == "random" else dict(tau_grid=tau, kernel=KERNELS.get(kname, 0))
+    okw = dict(tau_range=(-synth.TAU_MAX, synth.TAU_MAX)) if cfg.tau_mode == "random" else dict(tau_grid=tau)
+    ref = orc.search(p, cfg.f_min, cfg.df, n, cfg.seed, cfg.n_min, cfg.n_max, track_offset=first, family=orc.FAMILY_CUBIC,
+                     dump_snr=True, n_bins=cfg.n_bins, **okw)
+    got = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, first, n, family=P.FAMILY_CUBIC, **kw)
+    ok, worst = snr_close(got, ref["snr"])
+    assert ok, f"{kname}: worst error {worst:.3f} x tolerance"
+    r = st.search(n, cfg.seed, cfg.n_min, cfg.n_max, track_offset=first, family=P.FAMILY_CUBIC, n_bins=cfg.n_bins, **kw)
+    _assert_search_parity(r, ref, cfg)
+    o = orc.track_params(cfg.seed, ref["arg_track"], cfg.n_t, cfg.n_f, cfg.n_min, cfg.n_max, -synth.TAU_MAX if cfg.tau_mode == "random" else 0.0,
+                         synth.TAU_MAX if cfg.tau_mode == "random" else 0.0, family=orc.FAMILY_CUBIC)
+    for f in ("N", "j0", "a", "y0", "y1", "y2", "y3"):
+        assert r.arg_params[f] == getattr(o, f)
+    # the quadratic bank is untouched by the new field
+    rq = st.search(2000, cfg.seed, cfg.n_min, cfg.n_max, n_bins=cfg.n_bins, **kw)
+    refq = orc.search(p, cfg.f_min, cfg.df, 2000, cfg.seed, cfg.n_min, cfg.n_max, **okw)
+    assert (rq.arg_track, rq.arg_tau_index) == (refq["arg_track"], refq["arg_tau_index"])
+
+
+def test_cubic_family_self_recovery_and_explicit_scores(P, orc):
+    """P7 for the family: an injected cubic bank member is returned exactly; st_score_tracks scores explicit cubic
+    templates (an S-shaped track no quadratic can follow) like the oracle."""
+    cfg = synth.CONFIGS[2]
+    tau = synth.tau_linspace(64)
+    i_star, m_star, snr = 4321, 17, 9.0
+    t = orc.track_params(cfg.seed, i_star, cfg.n_t, cfg.n_f, cfg.n_min, cfg.n_max, family=orc.FAMILY_CUBIC)
+    k = orc.rasterise(t, cfg.n_f)
+    csd = np.zeros((cfg.n_t, cfg.n_f), dtype=np.complex64)
+    synth.add_injection(csd, None, t.j0 + np.arange(t.N), k, tau[m_star], snr, cfg.f_min, cfg.df)
+    st = make_ctx(P, cfg)
+    st.set_map(csd)
+    r = st.search(10000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, family=P.FAMILY_CUBIC)
+    assert (r.arg_track, r.arg_tau_index) == (i_star, m_star) and r.max_snr_f64 == pytest.approx(snr, rel=1e-6)
+    assert r.arg_params["y3"] == t.y3 and r.arg_params["y1"] == t.y1
+    csd, sigma, _ = config_inputs(orc, cfg)
+    st.set_map(csd, sigma)
+    p = orc.prepare_map(csd, sigma)
+    tracks = [(250, 0, 125.0, 100.5, 100.5, 800.5, 0.0, 800.5), (200, 20, 60.0, 900.25, 50.5, 950.75, 0.0, 10.5)]
+    got = st.score_tracks(tracks, tau_grid=tau, family=P.FAMILY_CUBIC)
+    W = orc.build_table(cfg.n_f, cfg.f_min, cfg.df, tau)
+    ref = np.array([orc.score_table(p, orc.make_track(*tr[:6], y3=tr[7]), orc.rasterise(orc.make_track(*tr[:6], y3=tr[7]), cfg.n_f), W)
+                    for tr in tracks])
+    ok, worst = snr_close(got, ref)
+    assert ok, worst
