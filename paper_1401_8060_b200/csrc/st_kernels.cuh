@@ -54,7 +54,7 @@ struct Scalars {         // device scalars of one search, zeroed by the host
     uint32_t gmax_bits;             // ordered-uint encoding of the float32 maximum
     uint32_t cand_count;
     uint32_t overflow;
-    uint32_t pad;
+    uint32_t n_deferred;            // templates the fast Chebyshev build handed to the two-class build (per launch)
 };
 
 struct DeviceResult {
@@ -104,6 +104,11 @@ struct ScoreArgs {
     int32_t* k_dump;          // parity export of k_score_random's own rasteriser: [n_tracks][n_t] (pre-filled with -1)
     int32_t* j0_dump;         //   with [n_tracks] first columns
     int32_t* N_dump;          //   and [n_tracks] durations
+    uint32_t* deferred;       // Chebyshev kernel: list of launch-relative template indices handed from the fast build
+                              // (which appends) to the two-class build (which, with defer_in set, works through it)
+    uint32_t deferred_cap;
+    int32_t defer_in;         // 1: this launch scores the templates of `deferred` (count in sc->n_deferred)
+    float defer_limit;        // fast build: largest scale * sum |v| over class B pixels it may score itself
 };
 
 // Template q of the launch: regenerated from (seed, id), or read from the caller's explicit list.
@@ -846,6 +851,12 @@ __device__ __forceinline__ f32x2_t pk_add(f32x2_t a, f32x2_t b)
     asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
     return r;
 }
+__device__ __forceinline__ f32x2_t pk_sub(f32x2_t a, f32x2_t b)      // FADD2 with the second operand negated
+{
+    f32x2_t r;
+    asm volatile("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
 // d = fma(nk, x, d) on the two halves with scalar FFMAs: fma.rn.f32x2 with three distinct
 // register-pair operands issues at 2/3 rate (register-file bandwidth; st_microbench
 // ffma2_3distinct), two scalar FFMAs cost the same pipe time as one full-rate packed op.
@@ -1136,7 +1147,8 @@ struct ChebFetchCtx {          // what fetching needs to know about a template
     int32_t N, L, cbase;       // columns, columns per lane, first column of this lane
 };
 struct ChebElem { int k[4]; float2 p[4], e[4]; float r[4]; };     // r: 1 / sigma, only loaded for norm 2
-struct ChebMergeState { int run_k, n_merged; float ax, ay; float2 run_e; float w2; };
+struct ChebMergeState { int run_k, n_a, n_b; float ax, ay; float2 run_e; float w2, bamp; };
+struct ChebCounts { int n_a, n_b; };       // pool entries of class A (front of the pool) and class B (back)
 
 // GEN = false compiles the default search (quadratic templates, N^-alpha normalisation) with the template
 // family and the weighting as constants; GEN = true reads both from the arguments (cubic family, norm 2).
@@ -1183,27 +1195,55 @@ __device__ __forceinline__ void cheb_fetch(const ScoreArgs& a, const ChebFetchCt
 }
 __device__ __forceinline__ void cheb_merge_init(ChebMergeState& m)
 {
-    m.run_k = -1; m.n_merged = 0; m.ax = 0.0f; m.ay = 0.0f; m.run_e = make_float2(0.0f, 0.0f); m.w2 = 0.0f;
+    m.run_k = -1; m.n_a = 0; m.n_b = 0; m.ax = 0.0f; m.ay = 0.0f; m.run_e = make_float2(0.0f, 0.0f); m.w2 = 0.0f; m.bamp = 0.0f;
 }
-// append the finished runs of the lanes flagged `emit` (a warp-wide ballot keeps the pool compact)
-__device__ __forceinline__ void cheb_emit(ChebMergeState& m, const bool emit, float2* pool_v, uint16_t* pool_k, const int lane)
+// Append the finished runs of the lanes flagged `emit` (warp-wide ballots keep the pool compact).  A pixel's
+// CLASS is a property of its bin, carried by the lowest mantissa bit of the anchor phase factor Ec[k].x the
+// host uploads: class A bins run the Chebyshev recurrence; in class B bins the float32 coefficient
+// 2 cos(S theta) would drift the phase by more than kChebClassDrift over half a chunk (small theta: fine grids,
+// low frequencies), which mis-scores a loud coherent signal where SNR(tau) crosses zero.
+//   TWO = true (the general build): class A fills the pool from the front, class B from the back (entries
+//     S-1, S-2, ...) and is advanced by Reinsch's form, whose coefficient 4 sin^2(theta/2) keeps its relative
+//     precision as theta -> 0;
+//   TWO = false (the fast build): one pool; the amplitude |Re v| + |Im v| >= |v| parked in class B bins is
+//     summed, and a template whose worst-case drift error  d_max * scale * sum_B |v|  could reach a fraction of
+//     the G13 tolerance is not scored here but handed to the general build (cheb_defer).
+template <bool TWO>
+__device__ __forceinline__ void cheb_emit(ChebMergeState& m, const bool emit, float2* pool_v, uint16_t* pool_k, const int lane,
+                                          const int S)
 {
-    const uint32_t em = __ballot_sync(kFull, emit);
-    if (emit) {
-        const int e = m.n_merged + __popc(em & ((1u << lane) - 1u));
-        pool_v[e] = make_float2(m.ax * m.run_e.x - m.ay * m.run_e.y, m.ax * m.run_e.y + m.ay * m.run_e.x);
-        pool_k[e] = (uint16_t)m.run_k;
+    const bool cls_b = (__float_as_uint(m.run_e.x) & 1u) != 0u;
+    if (TWO) {
+        const uint32_t em_a = __ballot_sync(kFull, emit && !cls_b);
+        const uint32_t em_b = __ballot_sync(kFull, emit && cls_b);
+        if (emit) {
+            const uint32_t below = (1u << lane) - 1u;
+            const int e = cls_b ? S - 1 - (m.n_b + __popc(em_b & below)) : m.n_a + __popc(em_a & below);
+            pool_v[e] = make_float2(m.ax * m.run_e.x - m.ay * m.run_e.y, m.ax * m.run_e.y + m.ay * m.run_e.x);
+            pool_k[e] = (uint16_t)m.run_k;
+        }
+        m.n_a += __popc(em_a);
+        m.n_b += __popc(em_b);
+    } else {
+        const uint32_t em = __ballot_sync(kFull, emit);
+        if (emit) {
+            const int e = m.n_a + __popc(em & ((1u << lane) - 1u));
+            pool_v[e] = make_float2(m.ax * m.run_e.x - m.ay * m.run_e.y, m.ax * m.run_e.y + m.ay * m.run_e.x);
+            pool_k[e] = (uint16_t)m.run_k;
+            if (cls_b) m.bamp += fabsf(m.ax) + fabsf(m.ay);
+        }
+        m.n_a += __popc(em);
     }
-    m.n_merged += __popc(em);
 }
+template <bool TWO>
 __device__ __forceinline__ void cheb_merge(const int norm, const int N, const int L, const int cbase, const int i, const ChebElem& E,
-                                           ChebMergeState& m, float2* pool_v, uint16_t* pool_k, const int lane)
+                                           ChebMergeState& m, float2* pool_v, uint16_t* pool_k, const int lane, const int S)
 {
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
         const bool valid = (i + u < L) && (cbase + i + u < N);
         const bool brk = valid && E.k[u] != m.run_k;   // a new run starts at this column
-        cheb_emit(m, brk && m.run_k >= 0, pool_v, pool_k, lane);
+        cheb_emit<TWO>(m, brk && m.run_k >= 0, pool_v, pool_k, lane, S);
         // branch-free update: a break restarts the sums, a column outside the template adds zero
         float px = valid ? E.p[u].x : 0.0f, py = valid ? E.p[u].y : 0.0f;
         if (norm == 2) {                               // warp-uniform
@@ -1218,21 +1258,31 @@ __device__ __forceinline__ void cheb_merge(const int norm, const int N, const in
         m.run_e.y = brk ? E.e[u].y : m.run_e.y;
     }
 }
-// the lanes' last runs, then zero-fill up to a multiple of 32 entries; returns the merged count
-__device__ __forceinline__ int cheb_merge_finish(ChebMergeState& m, float2* pool_v, uint16_t* pool_k, const int lane)
+// the lanes' last runs, then zero-fill both classes up to whole rows of 32 entries; returns the two counts
+template <bool TWO>
+__device__ __forceinline__ ChebCounts cheb_merge_finish(ChebMergeState& m, float2* pool_v, uint16_t* pool_k, const int lane,
+                                                        const int S)
 {
-    cheb_emit(m, m.run_k >= 0, pool_v, pool_k, lane);
-    const int e = m.n_merged + lane;
-    if (e < ((m.n_merged + kWarp - 1) & ~(kWarp - 1))) { pool_v[e] = make_float2(0.0f, 0.0f); pool_k[e] = 0; }
+    cheb_emit<TWO>(m, m.run_k >= 0, pool_v, pool_k, lane, S);
+    const int ea = m.n_a + lane;
+    if (ea < ((m.n_a + kWarp - 1) & ~(kWarp - 1))) { pool_v[ea] = make_float2(0.0f, 0.0f); pool_k[ea] = 0; }
+    if (TWO) {
+        const int eb = S - 1 - (m.n_b + lane);
+        if (eb >= S - ((m.n_b + kWarp - 1) & ~(kWarp - 1))) { pool_v[eb] = make_float2(0.0f, 0.0f); pool_k[eb] = 0; }
+    }
     __syncwarp();
-    return m.n_merged;
+    ChebCounts c;
+    c.n_a = m.n_a; c.n_b = m.n_b;
+    return c;
 }
 
 // Phase A for one template, start to finish (the next element is in flight while one is merged).
+// `defer` (fast build only): the template must be scored by the two-class build instead (see cheb_emit).
 template <bool GEN>
-__device__ __forceinline__ int cheb_phase_a(const ScoreArgs& a, const Track& t, float2* pool_v, uint16_t* pool_k,
-                                            const int lane, float& scale)
+__device__ __forceinline__ ChebCounts cheb_phase_a(const ScoreArgs& a, const Track& t, float2* pool_v, uint16_t* pool_k,
+                                                   const int lane, float& scale, bool& defer)
 {
+    const int S = a.pool_stride;
     ChebFetchCtx f;
     cheb_fetch_ctx<GEN>(a, t, lane, f);
     const int norm = GEN ? a.norm : (a.norm == 1 ? 1 : 0);
@@ -1244,25 +1294,36 @@ __device__ __forceinline__ int cheb_phase_a(const ScoreArgs& a, const Track& t, 
 #pragma unroll 1
     for (int i = 0; i < f.L; i += 8) {
         if (i + 4 < f.L) cheb_fetch<GEN>(a, f, i + 4, E1);  // warp-uniform
-        cheb_merge(norm, f.N, f.L, f.cbase, i, E0, m, pool_v, pool_k, lane);
+        cheb_merge<GEN>(norm, f.N, f.L, f.cbase, i, E0, m, pool_v, pool_k, lane, S);
         if (i + 4 >= f.L) break;
         if (i + 8 < f.L) cheb_fetch<GEN>(a, f, i + 8, E0);
-        cheb_merge(norm, f.N, f.L, f.cbase, i + 4, E1, m, pool_v, pool_k, lane);
+        cheb_merge<GEN>(norm, f.N, f.L, f.cbase, i + 4, E1, m, pool_v, pool_k, lane, S);
     }
     scale = track_scale(norm, t.N, m.w2);
-    return cheb_merge_finish(m, pool_v, pool_k, lane);
+    const ChebCounts cnt = cheb_merge_finish<GEN>(m, pool_v, pool_k, lane, S);
+    defer = false;
+    if (!GEN && a.defer_limit < 3.0e38f) {             // the grid has class B bins (warp-uniform)
+        float b = m.bamp;
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) b += __shfl_xor_sync(kFull, b, off);
+        defer = b * scale > a.defer_limit;
+    }
+    return cnt;
 }
 
 // Phase B for one template whose merged pixels sit in (pool_v, pool_k): every delay of the grid,
 // fused S4.  pool_v is advanced in place from chunk to chunk.
 // MODE 0: search; 1: capture pass of st_search_topk; 2: search + per-template maximum over the delays
-template <int STRIDE, int MODE>
+// TWO: the pool holds class B rows at its back (general build)
+template <int STRIDE, int MODE, bool TWO>
 __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr, uint32_t* sm_hist,
                                              const float4* sm_tab, const float* sm_zi, float2* pool_v,
-                                             const uint16_t* pool_k, const int n_merged, const float scale,
+                                             const uint16_t* pool_k, const ChebCounts cnt, const float scale,
                                              const uint64_t id, const uint64_t q, const int n_chunks, const int lane)
 {
-    const int n_rows = (n_merged + kWarp - 1) >> 5;
+    const int n_rows = (cnt.n_a + kWarp - 1) >> 5;          // class A rows, from the front of the pool
+    const int n_rows_b = TWO ? (cnt.n_b + kWarp - 1) >> 5 : 0;   // class B rows, from its back
+    const int S = a.pool_stride;
     TrackMax tm;
     tmax_init(tm);
     // ---- phase B: chunks of 64 delays; f2[i] = (sum x_{mc+i}, sum x_{mc-1-i}) over this lane's pixels
@@ -1351,6 +1412,35 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
                 }
             }
         }
+        // ---- class B rows (Reinsch's form, stride 1): x_{n+1} = x_n + d_{n+1}, d_{n+1} = d_n - kappa x_n with
+        // kappa = 4 sin^2(theta/2); pair = (forward, backward) as above, the
+        // backward half runs the same recurrence from d = -(x_mc - x_{mc-1}).  Three packed operations per
+        // two evaluations; the accumulators take x with the sign the Chebyshev chains carry at that offset.
+        if (TWO) {
+#pragma unroll 1
+        for (int rb = 0; rb < n_rows_b; ++rb) {
+            const int e0 = S - kWarp * (rb + 1) + lane;
+            const float2 v0 = pool_v[e0];
+            const int k0 = pool_k[e0];
+            ST_ASSERT(e0 >= 0 && k0 >= 0 && k0 < a.bp.n_f);
+            const float4 t0 = sm_tab[k0];
+            const float zi0 = sm_zi[k0];
+            pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
+            // kappa = 2 (1 - cos theta) = 2 sin^2 theta / (1 + cos theta): from the float32 (cos, sin) of the table
+            // without cancellation (relative error <= 3e-7: 5e-6 |theta| rad over half a chunk, |theta| <= 0.6)
+            const float kap = __fdiv_rn(2.0f * t0.z * t0.z, 1.0f + t0.y);
+            // x_mc - x_{mc-1} = Re v (1 - cos theta) - Im v sin theta, 1 - cos theta = kappa / 2
+            const float dlt = fmaf(0.5f * kap, v0.x, -(v0.y * t0.z));
+            f32x2_t x = pk_make(v0.x, v0.x - dlt), d = pk_make(dlt, -dlt);
+            const float nk = -kap;
+#pragma unroll
+            for (int i = 0; i < kHalf; ++i) {
+                f2[i] = ((i >> STRIDE) & 1) ? pk_sub(f2[i], x) : pk_add(f2[i], x);
+                d = pk_step(nk, x, d);
+                x = pk_add(x, d);
+            }
+        }
+        }
         // ---- fold across the 32 lanes (transposing tree on register pairs): lane l keeps pair l
 #pragma unroll
         for (int off = 16, n = kHalf / 2; off >= 1; off >>= 1, n >>= 1) {
@@ -1395,18 +1485,32 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
     // stays in lane 0 until the next iteration broadcasts it
     unsigned long long q_pref = 0;
     if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
+    // a launch works through its own id range, or (general build, defer_in) through the list of templates the
+    // fast build handed over: the list is complete, the fast launch precedes this one on the stream
+    const uint64_t n_items = (GEN && a.defer_in) ? (uint64_t)min(a.sc->n_deferred, a.deferred_cap) : a.n_tracks;
     for (;;) {
-        const uint64_t q = __shfl_sync(kFull, q_pref, 0);
-        if (q >= a.n_tracks) break;
+        const uint64_t item = __shfl_sync(kFull, q_pref, 0);
+        if (item >= n_items) break;
         if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
+        const uint64_t q = (GEN && a.defer_in) ? (uint64_t)a.deferred[item] : item;
         const uint64_t id = a.track_offset + q;
         const Track t = GEN ? load_track(a, q, id) : make_track(a.bp, id);     // explicit templates take the general build
-        wr.pixels += (unsigned long long)t.N;
         float scale;
-        const int n_merged = cheb_phase_a<GEN>(a, t, pool_v, pool_k, lane, scale);
-        ST_ASSERT(n_merged >= 1 && n_merged <= t.N && ((n_merged + kWarp - 1) & ~(kWarp - 1)) <= S &&
+        bool defer;
+        const ChebCounts cnt = cheb_phase_a<GEN>(a, t, pool_v, pool_k, lane, scale, defer);
+        if (!GEN && defer) {                       // warp-uniform: too much amplitude in class B bins for this build
+            if (lane == 0) {
+                const uint32_t slot = atomicAdd(&a.sc->n_deferred, 1u);
+                ST_ASSERT(slot < a.deferred_cap);
+                if (slot < a.deferred_cap) a.deferred[slot] = (uint32_t)q;
+            }
+            continue;
+        }
+        wr.pixels += (unsigned long long)t.N;
+        ST_ASSERT(cnt.n_a + cnt.n_b >= 1 && cnt.n_a + cnt.n_b <= t.N &&
+                  ((cnt.n_a + kWarp - 1) & ~(kWarp - 1)) + ((cnt.n_b + kWarp - 1) & ~(kWarp - 1)) <= S &&
                   (a.tracks || (t.N >= a.bp.n_min && t.N <= a.bp.n_max)) && t.j0 >= 0 && t.j0 + t.N <= a.bp.n_t);
-        cheb_phase_b<STRIDE, MODE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, n_merged, scale, id, q,
+        cheb_phase_b<STRIDE, MODE, GEN>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, cnt, scale, id, q,
                              n_chunks, lane);
     }
     reduce_finish(a, wr);

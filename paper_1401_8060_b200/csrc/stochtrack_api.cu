@@ -23,11 +23,12 @@ constexpr size_t kAlign = 256;
 constexpr uint32_t kCandCap = 1u << 16;
 constexpr uint32_t kWarpSlots = 1u << 14;
 constexpr uint64_t kMaxSamplesPerLaunch = 1ull << 31;   // keeps per-block u32 histogram bins exact
+constexpr uint32_t kDeferCap = 1u << 22;                // templates per Chebyshev launch = size of its hand-over list
 
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t map, isig, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, cand64, warp_best, stage_csd, stage_sigma, stage_csd2, stage_sigma2, b_scalars, b_result, b_hist, tracks, total;
+    size_t map, isig, e0, bintab, es, kz, ec, cheb, cheb_zi, w, tau, hist, scalars, result, cand, cand64, warp_best, stage_csd, stage_sigma, stage_csd2, stage_sigma2, b_scalars, b_result, b_hist, tracks, deferred, total;
 };
 
 Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
@@ -61,6 +62,7 @@ Layout make_layout(int32_t n_t, int32_t n_f, int32_t max_n_tau)
     L.b_result = o;     o += align_up((size_t)ST_BATCH_GROUP * sizeof(st::DeviceResult));
     L.b_hist = o;       o += align_up((size_t)ST_BATCH_GROUP * (size_t)ST_MAX_BINS * sizeof(unsigned long long));
     L.tracks = o;       o += align_up((size_t)ST_MAX_SCORE_TRACKS * sizeof(st::Track));
+    L.deferred = o;     o += align_up((size_t)kDeferCap * sizeof(uint32_t));
     L.total = o;
     return L;
 }
@@ -93,6 +95,8 @@ struct st_ctx {
     int device;                        // ordinal of the device the workspace lives on (every call runs there)
     int recur_threads;                 // tunable: threads per block of the recurrence kernels
     int cheb_stride;                   // stride of the tables currently on the device
+    int cheb_n_class_b;                // class B bins of those tables
+    double cheb_dmax;                  // largest Chebyshev drift among them [rad over half a chunk]
     bool pick_valid; double pick_dtau; int pick_stride;   // memo of cheb_pick_stride
     std::vector<float> h_cheb;         // host-built Chebyshev tables: [n_f] float4, [n_f] float2 Ec, [n_f] float zi
     char err[512];
@@ -198,15 +202,28 @@ bool reinsch_well_conditioned(const st_ctx* c, double dtau)
     return true;
 }
 
-// Chebyshev tables for stride S (built on the host so that the conditioning test sees the very
-// float32 coefficients the kernel uses).  The coefficient G = fl32(2 cos(S theta)) is the exact
-// coefficient of a slightly different angle; over the 32 delays between an anchor and the edge of
-// its chunk the phase drifts by (32 / S) |acos(G/2) - S theta|.  Returns the worst drift over bins.
-double build_cheb_tables(const st_ctx* c, double tau0, double dtau, int stride, std::vector<float>* out)
+// Chebyshev tables for stride S (built on the host so that the conditioning test sees the very float32
+// coefficients the kernel uses).  The coefficient G = fl32(2 cos(S theta)) is the exact coefficient of a slightly
+// different angle; over the 32 delays between an anchor and the edge of its chunk the phase drifts by
+// (32 / S) |acos(G/2) - S theta|.  A coherent signal of amplitude A (in SNR units) is then mis-scored by up to
+// A x drift where SNR(tau) crosses zero, against an absolute tolerance of 1e-4 s0 there (G13): bins whose drift
+// exceeds kChebClassDrift become CLASS B; the general build of the kernel advances them by Reinsch's form
+// (coefficient kappa = 4 sin^2(theta/2), relative precision kept as theta -> 0), the fast build scores a template
+// itself only when its amplitude in class B bins bounds the drift error below kChebDeferBudget (launch_score).
+// Returns the number of class B bins, or -1 when some bin suits neither form (then the grid goes to the rotation
+// kernel).  Table per bin: (G, cos theta, sin theta, cos 64 theta), Ec = anchor phase factor of chunk 0 with the
+// class in the lowest mantissa bit of its real part, zi = sin 64 theta.
+#ifndef ST_CLASS_DRIFT
+#define ST_CLASS_DRIFT 3e-6
+#endif
+constexpr double kChebClassDrift = ST_CLASS_DRIFT;   // rad over half a chunk: A = 16 stays inside half the G13 tolerance
+
+int build_cheb_tables(const st_ctx* c, double tau0, double dtau, int stride, std::vector<float>* out, double* d_max = nullptr)
 {
     const int n_f = c->n_f;
     if (out) out->assign((size_t)n_f * 7, 0.0f);
-    double worst = 0.0;
+    int n_class_b = 0;
+    if (d_max) *d_max = 0.0;
     for (int k = 0; k < n_f; ++k) {
         const double f = c->f_min + (double)k * c->df;
         double cyc = f * dtau;
@@ -217,8 +234,16 @@ double build_cheb_tables(const st_ctx* c, double tau0, double dtau, int stride, 
         const float G = (float)(2.0 * cos(sth));
         double half = 0.5 * (double)G;
         half = half > 1.0 ? 1.0 : (half < -1.0 ? -1.0 : half);
-        const double drift = (32.0 / (double)stride) * fabs(acos(half) - fabs(sth));
-        if (drift > worst) worst = drift;
+        const double drift_a = (32.0 / (double)stride) * fabs(acos(half) - fabs(sth));
+        bool class_b = false;
+        if (drift_a > kChebClassDrift) {
+            // Reinsch's form at stride 1 with kappa = 2 sin^2 theta / (1 + cos theta) formed in float32 from the
+            // table's (cos theta, sin theta): relative error <= 3e-7, i.e. <= 32 x 1.5e-7 |theta| rad of drift
+            const double drift_b = 4.8e-6 * fabs(theta);
+            if (drift_b > kChebClassDrift) return -1;
+            class_b = true; ++n_class_b;
+            if (d_max && drift_a > *d_max) *d_max = drift_a;
+        }
         if (out) {
             double c64 = cyc * 64.0;
             c64 -= rint(c64);
@@ -228,15 +253,19 @@ double build_cheb_tables(const st_ctx* c, double tau0, double dtau, int stride, 
             t4[0] = G; t4[1] = (float)cos(theta); t4[2] = (float)sin(theta); t4[3] = (float)cos(st::kTwoPi * c64);
             float* ec = out->data() + (size_t)n_f * 4 + (size_t)k * 2;
             ec[0] = (float)cos(st::kTwoPi * c0); ec[1] = (float)sin(st::kTwoPi * c0);
+            uint32_t bits;                                  // the class rides in the lowest mantissa bit of Ec.x
+            memcpy(&bits, &ec[0], sizeof(bits));
+            bits = (bits & ~1u) | (class_b ? 1u : 0u);
+            memcpy(&ec[0], &bits, sizeof(bits));
             (*out)[(size_t)n_f * 6 + (size_t)k] = (float)sin(st::kTwoPi * c64);
         }
     }
-    return worst;
+    return n_class_b;
 }
 
-constexpr double kChebMaxDrift = 3e-5;   // rad: worst-case relative error of a coherent signal's SNR
-
-// Stride 2 needs 2 theta inside (0, pi) for every bin; pick the stride with the smaller drift.
+// Stride 2 needs 2 theta inside (0, pi) for every bin; of the usable strides take the one with fewer class B
+// bins (their rows cost 3 packed operations per 2 evaluations instead of 2), stride 2 on a tie (more independent
+// chains per pixel).  0 = the Chebyshev kernel does not suit this grid.
 int cheb_pick_stride(st_ctx* c, double dtau)
 {
     if (c->pick_valid && c->pick_dtau == dtau) return c->pick_stride;
@@ -246,12 +275,14 @@ int cheb_pick_stride(st_ctx* c, double dtau)
         cyc -= rint(cyc);
         if (fabs(cyc) > max_abs_cyc) max_abs_cyc = fabs(cyc);
     }
-    const double d1 = build_cheb_tables(c, 0.0, dtau, 1, nullptr);
-    const double d2 = max_abs_cyc < 0.22 ? build_cheb_tables(c, 0.0, dtau, 2, nullptr) : 1e9;
-    const int s = d2 < d1 ? 2 : 1;
-    c->pick_valid = true; c->pick_dtau = dtau;
-    c->pick_stride = (s == 2 ? d2 : d1) <= kChebMaxDrift ? s : 0;
-    return c->pick_stride;
+    const int b1 = build_cheb_tables(c, 0.0, dtau, 1, nullptr);
+    const int b2 = max_abs_cyc < 0.22 ? build_cheb_tables(c, 0.0, dtau, 2, nullptr) : -1;
+    int s = 0;
+    if (b1 >= 0 && b2 >= 0) s = b2 <= b1 ? 2 : 1;
+    else if (b2 >= 0) s = 2;
+    else if (b1 >= 0) s = 1;
+    c->pick_valid = true; c->pick_dtau = dtau; c->pick_stride = s;
+    return s;
 }
 
 int pick_chunk(int n_tau)
@@ -270,9 +301,13 @@ struct Plan {
 // Shared memory a recurrence kernel needs with `warps` warps: histogram + per-bin tables + pixel pools.
 // AUTO only picks a kernel that keeps at least 4 warps per SM (wide bands: the per-bin tables of the
 // Chebyshev / Reinsch kernels outgrow shared memory, the rotation kernel then reads its table from L2).
+// Pool entries per warp of the Chebyshev kernel: class A rows from the front, class B rows from the back, each
+// zero-filled to whole rows of 32 (ceil32(a) + ceil32(b) <= ceil32(a + b) + 32).
+int cheb_pool_stride(int n_max) { return ((n_max + 31) & ~31) + 32; }
+
 bool recur_fits(const st_ctx* c, int kernel, int n_bins, int n_max, int warps)
 {
-    const size_t stride = (size_t)((n_max + 63) & ~63);
+    const size_t stride = kernel == ST_KERNEL_CHEBYSHEV ? (size_t)cheb_pool_stride(n_max) : (size_t)((n_max + 63) & ~63);
     const size_t hist = (size_t)((n_bins + 3) & ~3) * sizeof(uint32_t);
     size_t need = hist;
     if (kernel == ST_KERNEL_CHEBYSHEV)
@@ -302,7 +337,7 @@ int make_plan(st_ctx* c, const st_search_params* p, Plan* plan)
     if (k == ST_KERNEL_CHEBYSHEV && plan->stride == 0) {
         if (uni) plan->stride = cheb_pick_stride(c, plan->dtau);
         if (uni && plan->stride == 0)
-            return fail(c, ST_EINVAL, "the Chebyshev kernel is ill conditioned on this delay grid (drift > %.1e rad)", kChebMaxDrift);
+            return fail(c, ST_EINVAL, "the Chebyshev kernel is ill conditioned on this delay grid (a bin suits neither recurrence within %.1e rad)", kChebClassDrift);
     }
     if ((k == ST_KERNEL_ROTATION || k == ST_KERNEL_REINSCH || k == ST_KERNEL_CHEBYSHEV) && !uni)
         return fail(c, ST_EINVAL, "recurrence kernels need a uniform tau grid");
@@ -344,7 +379,7 @@ int ensure_tables(st_ctx* c, const st_search_params* p, const Plan& plan, int* n
         }
     } else if (plan.kernel == ST_KERNEL_CHEBYSHEV) {
         if (c->table_kind != kChebTable || c->cheb_stride != plan.stride) {
-            build_cheb_tables(c, plan.tau0, plan.dtau, plan.stride, &c->h_cheb);
+            c->cheb_n_class_b = build_cheb_tables(c, plan.tau0, plan.dtau, plan.stride, &c->h_cheb, &c->cheb_dmax);
             const size_t n = (size_t)c->n_f;
             ST_CUDA(c, cudaMemcpyAsync(at<void>(c, c->L.cheb), c->h_cheb.data(), n * 4 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
             ST_CUDA(c, cudaMemcpyAsync(at<void>(c, c->L.ec), c->h_cheb.data() + n * 4, n * 2 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
@@ -375,7 +410,12 @@ int set_smem(st_ctx* c, K kernel, size_t bytes)
 size_t hist_bytes(int n_bins) { return (size_t)((n_bins + 3) & ~3) * sizeof(uint32_t); }
 
 // Launch the scoring kernel of the plan on templates [a.track_offset, +a.n_tracks).
-int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
+// Absolute error (in SNR units) the fast Chebyshev build may owe to coefficient drift in class B bins: half the
+// G13 tolerance at a zero crossing of SNR(tau) on the configs' data (1e-4 x s0, s0 = 0.707).  Class A bins add
+// at most kChebClassDrift x A for a coherent amplitude A (3e-5 at SNR 10).
+constexpr double kChebDeferBudget = 3.5e-5;
+
+int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max, int* extra_launches = nullptr)
 {
     const int stride = (n_max + 63) & ~63;
     a.pool_stride = stride;
@@ -419,9 +459,11 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
     } else if (plan.kernel == ST_KERNEL_CHEBYSHEV) {
         int threads = c->recur_threads;
         size_t smem;
+        const int cstride = cheb_pool_stride(n_max);
+        a.pool_stride = cstride;
         for (;; threads -= 32) {
             smem = hist_bytes(a.n_bins) + (size_t)c->n_f * sizeof(float4) + (size_t)((c->n_f + 1) & ~1) * sizeof(float) +
-                   (size_t)(threads / 32) * (size_t)stride * (sizeof(float2) + sizeof(uint16_t));
+                   (size_t)(threads / 32) * (size_t)cstride * (sizeof(float2) + sizeof(uint16_t));
             if (smem <= (size_t)c->smem_optin || threads == 32) break;
         }
         if (smem > (size_t)c->smem_optin)
@@ -446,8 +488,28 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max)
         // the general build (cubic family, inverse-variance weighting, explicit templates) reads its options
         // at run time; the default search is compiled with them as constants
         const bool gen = a.bp.family != 0 || a.norm == 2 || a.tracks != nullptr;
+        // Grids with class B bins (coefficient drift, see build_cheb_tables): the fast build scores every template
+        // whose amplitude in those bins bounds the drift error below kChebDeferBudget and lists the others; a
+        // second launch of the general (two-class) build scores the listed ones.  Results are order independent.
+        const bool two_pass = !gen && c->cheb_n_class_b > 0;
+        a.deferred = at<uint32_t>(c, c->L.deferred); a.deferred_cap = kDeferCap; a.defer_in = 0;
+        a.defer_limit = two_pass ? (float)(kChebDeferBudget / c->cheb_dmax) : 3.4e38f;
+        if (two_pass) {
+            if (a.n_tracks > kDeferCap) return fail(c, ST_EINVAL, "internal: Chebyshev launch of %llu templates exceeds its hand-over list", (unsigned long long)a.n_tracks);
+            ST_CUDA(c, cudaMemsetAsync(&a.sc->n_deferred, 0, sizeof(uint32_t), c->stream));
+        }
         if (pk) { if (gen) ST_LAUNCH_CHEB_MODE(2, true); else ST_LAUNCH_CHEB_MODE(2, false); }
         else    { if (gen) ST_LAUNCH_CHEB_MODE(1, true); else ST_LAUNCH_CHEB_MODE(1, false); }
+        if (two_pass) {
+            ST_CUDA(c, cudaGetLastError());
+            ST_CUDA(c, cudaMemsetAsync(&a.sc->counter, 0, sizeof(unsigned long long), c->stream));
+            a.defer_in = 1; a.defer_limit = 3.4e38f;
+            blocks = (uint64_t)c->n_sm;
+            if (blocks > need) blocks = need;
+            if (pk) ST_LAUNCH_CHEB_MODE(2, true); else ST_LAUNCH_CHEB_MODE(1, true);
+            a.defer_in = 0;
+            if (extra_launches) ++*extra_launches;
+        }
 #undef ST_LAUNCH_CHEB_MODE
 #undef ST_LAUNCH_CHEB
     } else if (plan.kernel == ST_KERNEL_REINSCH) {
@@ -587,13 +649,14 @@ int enqueue_search(st_ctx* c, const st_search_params* p, const Plan& plan, const
     a.hist_scale = p->n_bins > 0 ? (float)((double)p->n_bins / (p->hist_hi - p->hist_lo)) : 0.0f;
     uint64_t per_launch = kMaxSamplesPerLaunch / (uint64_t)n_tau;
     if (per_launch < 1) per_launch = 1;
+    if (plan.kernel == ST_KERNEL_CHEBYSHEV && per_launch > kDeferCap) per_launch = kDeferCap;
     if (time_it) ST_CUDA(c, cudaEventRecord(c->ev0, c->stream));
     for (uint64_t done = 0; done < p->n_tracks; done += per_launch) {
         a.track_offset = p->track_offset + done;
         a.n_tracks = p->n_tracks - done < per_launch ? p->n_tracks - done : per_launch;
         a.tmax_snr = tmax_snr ? tmax_snr + done : nullptr;
         a.tmax_m = tmax_m ? tmax_m + done : nullptr;
-        rc = launch_score(c, plan, a, p->n_max);
+        rc = launch_score(c, plan, a, p->n_max, n_launches);
         if (rc) return rc;
         ++*n_launches;
     }
@@ -637,7 +700,7 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     for (int i = 0; i < 2; ++i) { c->ev_copied[i] = nullptr; c->ev_consumed[i] = nullptr; }
     c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512; c->device = 0;
     c->err[0] = 0;
-    c->cheb_stride = 0; c->pick_valid = false; c->pick_dtau = 0.0; c->pick_stride = 0;
+    c->cheb_stride = 0; c->cheb_n_class_b = 0; c->cheb_dmax = 0.0; c->pick_valid = false; c->pick_dtau = 0.0; c->pick_stride = 0;
     *out = c;
     return ST_OK;
 }
@@ -831,10 +894,11 @@ int st_search_topk(st_ctx* c, const st_search_params* p, int32_t top_k, st_top_e
     a.capture_mode = 1; a.capture_thr = thr;
     uint64_t per_launch = kMaxSamplesPerLaunch / (uint64_t)n_tau;
     if (per_launch < 1) per_launch = 1;
+    if (plan.kernel == ST_KERNEL_CHEBYSHEV && per_launch > kDeferCap) per_launch = kDeferCap;
     for (uint64_t done = 0; done < p->n_tracks; done += per_launch) {
         a.track_offset = p->track_offset + done;
         a.n_tracks = p->n_tracks - done < per_launch ? p->n_tracks - done : per_launch;
-        rc = launch_score(c, plan, a, p->n_max);
+        rc = launch_score(c, plan, a, p->n_max, &result->n_launches);
         if (rc) return rc;
         ++result->n_launches;
     }
@@ -1279,7 +1343,7 @@ int st_debug_scores(st_ctx* c, const st_search_params* p, uint64_t first, uint64
     rc = make_plan(c, p, &plan);
     if (rc) return rc;
     const int n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
-    if (count > kMaxSamplesPerLaunch / (uint64_t)n_tau) return fail(c, ST_EINVAL, "count too large for one debug launch");
+    if (count > kMaxSamplesPerLaunch / (uint64_t)n_tau || count > kDeferCap) return fail(c, ST_EINVAL, "count too large for one debug launch");
     int n_launches = 0;
     rc = ensure_tables(c, p, plan, &n_launches);
     if (rc) return rc;
