@@ -149,6 +149,9 @@ def run_ours(args):
         maps_h = [csd_h] + [torch.from_numpy(synth.config_inputs(cfg, m)[0]).pin_memory() for m in range(1, n_maps)]
         maps_d = [h.to(dev) for h in maps_h]
         seeds = [synth.map_seed(cfg, m) for m in range(n_maps)]
+        if args.shared_bank:
+            seeds = synth.map_seed(cfg, 0)
+            st.enable_bank_cache(n_mine, cfg.n_max)
 
         def run_batch(maps):
             res, ms = st.search_batch(maps, None, seeds, n_mine, cfg.n_min, cfg.n_max, track_offset=first, **kw)
@@ -373,6 +376,9 @@ def main():
                     help="BASELINE.json config (1-5) or P: the shape of the paper's own timing, Table III (context)")
     ap.add_argument("--tracks", type=int, default=0, help="override templates per GPU (debugging)")
     ap.add_argument("--maps", type=int, default=0, help="maps per batch step of config 4 (default: the config's 100)")
+    ap.add_argument("--shared-bank", action="store_true",
+                    help="config 4 with ONE template bank for every map (seed of map 0) and the bank cache attached: "
+                         "S1 + S2 run once, the other maps read the rasterised bank back (SURVEY 8(f) NEXT-2)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "table", "rotation", "reinsch"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ftmap", action="store_true", help="also time st_set_map_from_strain on strain of the config's duration")

@@ -129,10 +129,14 @@ typedef struct {
     int32_t  n_candidates;   /* near-max samples re-scored in float64                    */
     int32_t  kernel_used;    /* ST_KERNEL_* actually launched                            */
     int32_t  n_launches;     /* kernels launched by this call                            */
-    int32_t  flags;          /* bit 0: candidate list overflowed, argmax from float32    */
+    int32_t  flags;          /* ST_FLAG_* bits                                           */
     float    gpu_ms;         /* device time of the scoring launches (CUDA events)        */
     float    reserved;
 } st_result;
+
+#define ST_FLAG_CAND_OVERFLOW 1   /* candidate list overflowed: argmax decided by the float32 records      */
+#define ST_FLAG_BANK_READ     2   /* S1 + S2 came from the bank cache (st_set_bank_cache)                 */
+#define ST_FLAG_BANK_FILLED   4   /* this search filled the bank cache                                     */
 
 #define ST_MAX_BINS 4096
 #define ST_MAX_N_T  1048576
@@ -153,6 +157,19 @@ size_t st_workspace_bytes(const st_ctx *ctx, int32_t max_n_tau);
  * context's use) and the CUDA stream (cudaStream_t as void*, NULL = default
  * stream) every later call is ordered on.  Errors: ST_ENOSPC, ST_EINVAL, ST_ECUDA. */
 int st_set_workspace(st_ctx *ctx, void *workspace_dev, size_t bytes, void *cuda_stream);
+
+/* Bank cache: the rasterised template bank kept on the device and reused across maps (n_ts
+ * time-shifted maps per analysis; follow-ups and repeated runs over the same spectrograms).
+ * When the caller hands in a buffer, a grid search of quadratic templates (ST_KERNEL_CHEBYSHEV path, sqrt(N) /
+ * mean normalisation) that uses a NEW bank -- (seed, track_offset, n_tracks, n_min, n_max) -- and fits writes
+ * (N, j0) and the bins of every template while it scores them (ST_FLAG_BANK_FILLED); every later search with the
+ * SAME bank on whatever map reads them back instead of running S1 + S2 (ST_FLAG_BANK_READ): 2 bytes per template
+ * column from HBM instead of the Philox rounds and the float64 rasteriser.  Results are bit-identical either way.
+ * st_search_batch / st_search_timeshifts with one seed for every map use it from the second map on.
+ *   st_bank_cache_bytes : bytes for a bank of n_tracks templates of at most n_max columns (0 on bad arguments)
+ *   st_set_bank_cache   : DEVICE buffer, 256-byte aligned, caller-owned; NULL detaches.  Invalidates the cache. */
+size_t st_bank_cache_bytes(const st_ctx *ctx, uint64_t n_tracks, int32_t n_max);
+int st_set_bank_cache(st_ctx *ctx, void *cache_dev, size_t bytes);
 
 /* S0 (Eq. 7): p = CSD / sigma into the workspace.  csd_dev: DEVICE
  * complex64 [n_t][n_f] (frequency contiguous, interleaved re/im); sigma_dev: DEVICE

@@ -20,7 +20,7 @@ KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random",
 # every symbol include/stochtrack.h declares
 exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_workspace", "st_set_map",
                     "st_set_map_host", "st_search", "st_search_topk", "st_search_batch", "st_search_track_max",
-                    "st_score_tracks", "st_debug_rasterise_random", "st_ftmap_scratch_bytes", "st_set_map_from_strain", "st_search_timeshifts",
+                    "st_score_tracks", "st_debug_rasterise_random", "st_bank_cache_bytes", "st_set_bank_cache", "st_ftmap_scratch_bytes", "st_set_map_from_strain", "st_search_timeshifts",
                     "st_debug_get_map",
                     "st_track_params", "st_track_params_family", "st_debug_rasterise",
                     "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words",
@@ -136,6 +136,10 @@ def load_library(path=None):
     L.st_debug_get_map.argtypes = [vp, vp]
     L.st_debug_get_map.restype = C.c_int
     L.st_search_batch.argtypes = [vp, C.POINTER(CBatch), C.POINTER(CSearchParams), C.POINTER(CResult), C.POINTER(C.c_float)]
+    L.st_bank_cache_bytes.argtypes = [vp, C.c_uint64, C.c_int32]
+    L.st_bank_cache_bytes.restype = C.c_size_t
+    L.st_set_bank_cache.argtypes = [vp, vp, C.c_size_t]
+    L.st_set_bank_cache.restype = C.c_int
     L.st_search_track_max.argtypes = [vp, C.POINTER(CSearchParams), vp, vp, C.POINTER(CResult)]
     L.st_search_track_max.restype = C.c_int
     L.st_score_tracks.argtypes = [vp, C.POINTER(CSearchParams), C.POINTER(CTrack), C.c_int32, vp]
@@ -201,6 +205,20 @@ class Stochtrack:
 
     def synchronize(self):
         self._stream.synchronize()
+
+    def enable_bank_cache(self, n_tracks, n_max):
+        """Allocate and attach a bank cache for banks of n_tracks templates of at most n_max columns
+        (st_bank_cache_bytes / st_set_bank_cache).  Returns its size in bytes."""
+        nbytes = self._L.st_bank_cache_bytes(self._ctx, int(n_tracks), int(n_max))
+        if nbytes == 0:
+            raise StError(ST_EINVAL, "st_bank_cache_bytes: bad arguments")
+        self._bank = self._torch.empty(nbytes, dtype=self._torch.uint8, device=self.device)
+        self._check(self._L.st_set_bank_cache(self._ctx, self._bank.data_ptr(), nbytes))
+        return nbytes
+
+    def disable_bank_cache(self):
+        self._check(self._L.st_set_bank_cache(self._ctx, None, 0))
+        self._bank = None
 
     # ---------------------------------------------------------------- S0
     def set_map(self, csd, sigma=None):

@@ -109,6 +109,13 @@ struct ScoreArgs {
     uint32_t deferred_cap;
     int32_t defer_in;         // 1: this launch scores the templates of `deferred` (count in sc->n_deferred)
     float defer_limit;        // fast build: largest scale * sum |v| over class B pixels it may score itself
+    // bank cache (Chebyshev fast build): S1 + S2 of a template bank kept in HBM so that further maps searched with
+    // the same bank skip Philox and the rasteriser (PAPER.md:173 time shifts, :232-234 follow-ups)
+    uint16_t* kcache;         // [templates][kcache_stride] bins, lane-major: entry lane * ceil4(L) + i
+    int2* kmeta;              // [templates] (N, j0)
+    uint32_t kcache_stride;   // uint16 entries per template = 32 * ceil4(ceil(n_max / 32))
+    uint64_t kcache_base;     // cache row of template 0 of this launch
+    int32_t kcache_mode;      // 0 unused, 1 this launch fills the cache, 2 it reads it
 };
 
 // Template q of the launch: regenerated from (seed, id), or read from the caller's explicit list.
@@ -1142,6 +1149,7 @@ struct ChebPixel {
 // caller can keep the next element in flight while it merges the current one.
 struct ChebFetchCtx {          // what fetching needs to know about a template
     Raster r;
+    uint16_t* krow;            // bank cache: this lane's slice of the template's row
     double u_last;             // centre of the last column (clamp target of out-of-range lanes)
     const float2* col0;        // map row of the template's first column
     int32_t N, L, cbase;       // columns, columns per lane, first column of this lane
@@ -1152,33 +1160,44 @@ struct ChebCounts { int n_a, n_b; };       // pool entries of class A (front of 
 
 // GEN = false compiles the default search (quadratic templates, N^-alpha normalisation) with the template
 // family and the weighting as constants; GEN = true reads both from the arguments (cubic family, norm 2).
-template <bool GEN>
-__device__ __forceinline__ void cheb_fetch_ctx(const ScoreArgs& a, const Track& t, const int lane, ChebFetchCtx& f)
+// BANK: 0 no bank cache, 1 this launch fills it, 2 this launch reads it (S1 + S2 skipped)
+template <bool GEN, int BANK>
+__device__ __forceinline__ void cheb_fetch_ctx(const ScoreArgs& a, const Track& t, const uint64_t q, const int lane, ChebFetchCtx& f)
 {
-    f.r = make_raster(t, a.bp.n_f, GEN ? a.bp.family : 0);
+    if (BANK != 2) f.r = make_raster(t, a.bp.n_f, GEN ? a.bp.family : 0);
     f.N = t.N;
     f.L = (t.N + kWarp - 1) >> 5;
     f.cbase = lane * f.L;
+    if (BANK != 0) f.krow = a.kcache + (a.kcache_base + q) * (uint64_t)a.kcache_stride + (uint32_t)lane * (uint32_t)((f.L + 3) & ~3);
     f.u_last = int_to_double_fast(t.N - 1) + 0.5;
     f.col0 = a.map + (size_t)t.j0 * (size_t)a.bp.n_f;
 }
-template <bool GEN>
+template <bool GEN, int BANK>
 __device__ __forceinline__ void cheb_fetch(const ScoreArgs& a, const ChebFetchCtx& f, const int i, ChebElem& E)
 {
-    bool redo[4];
     int cc[4];
-    const double ub = int_to_double_fast(f.cbase + i) + 0.5;
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
         const int c = f.cbase + i + u;
-        const bool in = c < f.N;
-        cc[u] = in ? c : f.N - 1;                      // clamped: discarded by the merge
-        E.k[u] = raster_bin_fast_u(f.r, in ? ub + (double)u : f.u_last, redo[u]);   // branch-free: the four chains interleave
+        cc[u] = c < f.N ? c : f.N - 1;                 // clamped: discarded by the merge
     }
-    if (redo[0] | redo[1] | redo[2] | redo[3]) {       // ~1e-5 of the time: normative sequence
+    if (BANK == 2) {                                   // the four bins of this element: one 8-byte read
+        const uint2 w = __ldg(reinterpret_cast<const uint2*>(f.krow + i));
+        E.k[0] = (int)(w.x & 0xFFFFu); E.k[1] = (int)(w.x >> 16); E.k[2] = (int)(w.y & 0xFFFFu); E.k[3] = (int)(w.y >> 16);
+    } else {
+        bool redo[4];
+        const double ub = int_to_double_fast(f.cbase + i) + 0.5;
 #pragma unroll
         for (int u = 0; u < 4; ++u)
-            if (redo[u]) E.k[u] = raster_bin(f.r, cc[u]);
+            E.k[u] = raster_bin_fast_u(f.r, f.cbase + i + u < f.N ? ub + (double)u : f.u_last, redo[u]);   // branch-free: the four chains interleave
+        if (redo[0] | redo[1] | redo[2] | redo[3]) {   // ~1e-5 of the time: normative sequence
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (redo[u]) E.k[u] = raster_bin(f.r, cc[u]);
+        }
+        if (BANK == 1)
+            *reinterpret_cast<uint2*>(f.krow + i) = make_uint2((uint32_t)E.k[0] | ((uint32_t)E.k[1] << 16),
+                                                              (uint32_t)E.k[2] | ((uint32_t)E.k[3] << 16));
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
@@ -1278,25 +1297,25 @@ __device__ __forceinline__ ChebCounts cheb_merge_finish(ChebMergeState& m, float
 
 // Phase A for one template, start to finish (the next element is in flight while one is merged).
 // `defer` (fast build only): the template must be scored by the two-class build instead (see cheb_emit).
-template <bool GEN>
-__device__ __forceinline__ ChebCounts cheb_phase_a(const ScoreArgs& a, const Track& t, float2* pool_v, uint16_t* pool_k,
-                                                   const int lane, float& scale, bool& defer)
+template <bool GEN, int BANK>
+__device__ __forceinline__ ChebCounts cheb_phase_a(const ScoreArgs& a, const Track& t, const uint64_t q, float2* pool_v,
+                                                   uint16_t* pool_k, const int lane, float& scale, bool& defer)
 {
     const int S = a.pool_stride;
     ChebFetchCtx f;
-    cheb_fetch_ctx<GEN>(a, t, lane, f);
+    cheb_fetch_ctx<GEN, BANK>(a, t, q, lane, f);
     const int norm = GEN ? a.norm : (a.norm == 1 ? 1 : 0);
     ChebMergeState m;
     cheb_merge_init(m);
     ChebElem E0, E1;                                   // ping-pong: no register copies between elements
     __syncwarp();                                      // the previous template's pool reads are done
-    cheb_fetch<GEN>(a, f, 0, E0);
+    cheb_fetch<GEN, BANK>(a, f, 0, E0);
 #pragma unroll 1
     for (int i = 0; i < f.L; i += 8) {
-        if (i + 4 < f.L) cheb_fetch<GEN>(a, f, i + 4, E1);  // warp-uniform
+        if (i + 4 < f.L) cheb_fetch<GEN, BANK>(a, f, i + 4, E1);  // warp-uniform
         cheb_merge<GEN>(norm, f.N, f.L, f.cbase, i, E0, m, pool_v, pool_k, lane, S);
         if (i + 4 >= f.L) break;
-        if (i + 8 < f.L) cheb_fetch<GEN>(a, f, i + 8, E0);
+        if (i + 8 < f.L) cheb_fetch<GEN, BANK>(a, f, i + 8, E0);
         cheb_merge<GEN>(norm, f.N, f.L, f.cbase, i + 4, E1, m, pool_v, pool_k, lane, S);
     }
     scale = track_scale(norm, t.N, m.w2);
@@ -1341,7 +1360,8 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
             ST_ASSERT(k0 >= 0 && k0 < a.bp.n_f && k1 >= 0 && k1 < a.bp.n_f);
             const float4 t0 = sm_tab[k0], t1 = sm_tab[k1];
             const float zi0 = sm_zi[k0], zi1 = sm_zi[k1];
-            // next chunk's anchors: v e^{i 64 theta}   (t.w = cos 64 theta, zi = sin 64 theta)
+            // next chunk's anchors: v e^{i 64 theta}   (t.w = cos 64 theta, zi = sin 64 theta).  Unconditional: skipping
+            // the advance on the last chunk (a warp-uniform branch here) cost 4-7 % (measured, round 2)
             pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
             pool_v[e1] = make_float2(fmaf(v1.x, t1.w, -(v1.y * zi1)), fmaf(v1.x, zi1, v1.y * t1.w));
             ChebPixel<STRIDE> A, B;
@@ -1463,7 +1483,7 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
     if (MODE == 2) tmax_finish(a, tm, q);
 }
 
-template <int STRIDE, int MODE, bool GEN>
+template <int STRIDE, int MODE, bool GEN, int BANK>
 __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -1494,10 +1514,17 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
         if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
         const uint64_t q = (GEN && a.defer_in) ? (uint64_t)a.deferred[item] : item;
         const uint64_t id = a.track_offset + q;
-        const Track t = GEN ? load_track(a, q, id) : make_track(a.bp, id);     // explicit templates take the general build
+        Track t;
+        if (BANK == 2) {                           // S1 from the bank cache: only N and j0 are needed downstream
+            const int2 nj = __ldg(&a.kmeta[a.kcache_base + q]);
+            t.N = nj.x; t.j0 = nj.y; t.a = t.y0 = t.y1 = t.y2 = t.tau = t.y3 = 0.0;
+        } else {
+            t = GEN ? load_track(a, q, id) : make_track(a.bp, id);             // explicit templates take the general build
+            if (BANK == 1 && lane == 0) a.kmeta[a.kcache_base + q] = make_int2(t.N, t.j0);
+        }
         float scale;
         bool defer;
-        const ChebCounts cnt = cheb_phase_a<GEN>(a, t, pool_v, pool_k, lane, scale, defer);
+        const ChebCounts cnt = cheb_phase_a<GEN, BANK>(a, t, q, pool_v, pool_k, lane, scale, defer);
         if (!GEN && defer) {                       // warp-uniform: too much amplitude in class B bins for this build
             if (lane == 0) {
                 const uint32_t slot = atomicAdd(&a.sc->n_deferred, 1u);

@@ -95,6 +95,10 @@ struct st_ctx {
     int device;                        // ordinal of the device the workspace lives on (every call runs there)
     int recur_threads;                 // tunable: threads per block of the recurrence kernels
     int cheb_stride;                   // stride of the tables currently on the device
+    // bank cache (st_set_bank_cache): S1 + S2 of one template bank, reused by every search with the same bank
+    unsigned char* bank; size_t bank_bytes; bool bank_valid;
+    int last_bank_mode;                // what the last enqueued search did with it: 0 nothing, 1 filled, 2 read
+    struct { uint64_t seed, offset, n_tracks; int32_t n_min, n_max; } bank_key;
     int cheb_n_class_b;                // class B bins of those tables
     double cheb_dmax;                  // largest Chebyshev drift among them [rad over half a chunk]
     bool pick_valid; double pick_dtau; int pick_stride;   // memo of cheb_pick_stride
@@ -410,6 +414,13 @@ int set_smem(st_ctx* c, K kernel, size_t bytes)
 size_t hist_bytes(int n_bins) { return (size_t)((n_bins + 3) & ~3) * sizeof(uint32_t); }
 
 // Launch the scoring kernel of the plan on templates [a.track_offset, +a.n_tracks).
+// Bank cache layout: [n_tracks] (N, j0) records, then per template 32 lanes x ceil4(ceil(n_max / 32)) uint16 bins.
+uint32_t bank_row_entries(int n_max) { return 32u * (uint32_t)((((n_max + 31) >> 5) + 3) & ~3); }
+size_t bank_bytes_for(uint64_t n_tracks, int n_max)
+{
+    return align_up((size_t)n_tracks * sizeof(int2)) + align_up((size_t)n_tracks * (size_t)bank_row_entries(n_max) * sizeof(uint16_t));
+}
+
 // Absolute error (in SNR units) the fast Chebyshev build may owe to coefficient drift in class B bins: half the
 // G13 tolerance at a zero crossing of SNR(tau) on the configs' data (1e-4 x s0, s0 = 0.707).  Class A bins add
 // at most kChebClassDrift x A for a coherent amplitude A (3e-5 at SNR 10).
@@ -472,17 +483,19 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max, int* 
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
-#define ST_LAUNCH_CHEB(STRIDE, MODE, GEN)                                                         \
+#define ST_LAUNCH_CHEB(STRIDE, MODE, GEN, BANK)                                                   \
     do {                                                                                          \
-        int rc_ = set_smem(c, st::k_score_cheb<STRIDE, MODE, GEN>, smem);                         \
+        int rc_ = set_smem(c, st::k_score_cheb<STRIDE, MODE, GEN, BANK>, smem);                   \
         if (rc_) return rc_;                                                                      \
-        st::k_score_cheb<STRIDE, MODE, GEN><<<(unsigned)blocks, threads, smem, c->stream>>>(a);   \
+        st::k_score_cheb<STRIDE, MODE, GEN, BANK><<<(unsigned)blocks, threads, smem, c->stream>>>(a); \
     } while (0)
 #define ST_LAUNCH_CHEB_MODE(STRIDE, GEN)                                                          \
     do {                                                                                          \
-        if (mode == 1) ST_LAUNCH_CHEB(STRIDE, 1, GEN);                                            \
-        else if (mode == 2) ST_LAUNCH_CHEB(STRIDE, 2, GEN);                                       \
-        else ST_LAUNCH_CHEB(STRIDE, 0, GEN);                                                      \
+        if (mode == 1) ST_LAUNCH_CHEB(STRIDE, 1, GEN, 0);                                         \
+        else if (mode == 2) ST_LAUNCH_CHEB(STRIDE, 2, GEN, 0);                                    \
+        else if (!GEN && a.kcache_mode == 1) ST_LAUNCH_CHEB(STRIDE, 0, false, 1);                 \
+        else if (!GEN && a.kcache_mode == 2) ST_LAUNCH_CHEB(STRIDE, 0, false, 2);                 \
+        else ST_LAUNCH_CHEB(STRIDE, 0, GEN, 0);                                                   \
     } while (0)
         const int mode = a.capture_mode ? 1 : (a.tmax_snr ? 2 : 0);
         // the general build (cubic family, inverse-variance weighting, explicit templates) reads its options
@@ -650,17 +663,40 @@ int enqueue_search(st_ctx* c, const st_search_params* p, const Plan& plan, const
     uint64_t per_launch = kMaxSamplesPerLaunch / (uint64_t)n_tau;
     if (per_launch < 1) per_launch = 1;
     if (plan.kernel == ST_KERNEL_CHEBYSHEV && per_launch > kDeferCap) per_launch = kDeferCap;
+    // bank cache: a plain Chebyshev search of quadratic templates reads S1 + S2 from the cache when it holds this
+    // bank (same seed, id range, duration range), else fills it when the range fits
+    int bank_mode = 0;
+    if (c->bank && plan.kernel == ST_KERNEL_CHEBYSHEV && p->family == ST_FAMILY_QUADRATIC && p->norm != ST_NORM_INVVAR &&
+        !tmax_snr && p->n_tracks > 0) {
+        const uint32_t stride = bank_row_entries(p->n_max);
+        const bool same = c->bank_valid && c->bank_key.seed == p->seed && c->bank_key.offset == p->track_offset &&
+                          c->bank_key.n_tracks == p->n_tracks && c->bank_key.n_min == p->n_min && c->bank_key.n_max == p->n_max;
+        if (same) bank_mode = 2;
+        else if (bank_bytes_for(p->n_tracks, p->n_max) <= c->bank_bytes) {
+            bank_mode = 1;
+            c->bank_valid = false;
+            c->bank_key.seed = p->seed; c->bank_key.offset = p->track_offset; c->bank_key.n_tracks = p->n_tracks;
+            c->bank_key.n_min = p->n_min; c->bank_key.n_max = p->n_max;
+        }
+        a.kcache_stride = stride;
+        a.kmeta = reinterpret_cast<int2*>(c->bank);
+        a.kcache = reinterpret_cast<uint16_t*>(c->bank + align_up((size_t)p->n_tracks * sizeof(int2)));
+    }
+    a.kcache_mode = bank_mode;
     if (time_it) ST_CUDA(c, cudaEventRecord(c->ev0, c->stream));
     for (uint64_t done = 0; done < p->n_tracks; done += per_launch) {
         a.track_offset = p->track_offset + done;
         a.n_tracks = p->n_tracks - done < per_launch ? p->n_tracks - done : per_launch;
         a.tmax_snr = tmax_snr ? tmax_snr + done : nullptr;
         a.tmax_m = tmax_m ? tmax_m + done : nullptr;
+        a.kcache_base = done;
         rc = launch_score(c, plan, a, p->n_max, n_launches);
         if (rc) return rc;
         ++*n_launches;
     }
     if (time_it) ST_CUDA(c, cudaEventRecord(c->ev1, c->stream));
+    if (bank_mode == 1) c->bank_valid = true;       // every launch of the filling search has been enqueued
+    c->last_bank_mode = bank_mode;
     st::FinalArgs f;
     memset(&f, 0, sizeof(f));
     f.map = a.map; f.isig = a.isig; f.bp = a.bp; f.f_min = c->f_min; f.df = c->df;
@@ -698,8 +734,9 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->ev0 = c->ev1 = nullptr; c->h_res = nullptr; c->h_hist = nullptr;
     c->copy_stream = nullptr; c->h_bres = nullptr; c->h_bhist = nullptr;
     for (int i = 0; i < 2; ++i) { c->ev_copied[i] = nullptr; c->ev_consumed[i] = nullptr; }
-    c->n_sm = 0; c->smem_optin = 0; c->recur_threads = 512; c->device = 0;
+    c->n_sm = 0; c->smem_optin = 0; c->recur_threads = ST_CHEB_MAX_THREADS; c->device = 0;
     c->err[0] = 0;
+    c->bank = nullptr; c->bank_bytes = 0; c->bank_valid = false; c->last_bank_mode = 0; memset(&c->bank_key, 0, sizeof(c->bank_key));
     c->cheb_stride = 0; c->cheb_n_class_b = 0; c->cheb_dmax = 0.0; c->pick_valid = false; c->pick_dtau = 0.0; c->pick_stride = 0;
     *out = c;
     return ST_OK;
@@ -759,6 +796,20 @@ int st_set_workspace(st_ctx* c, void* ws, size_t bytes, void* cuda_stream)
     c->stream = (cudaStream_t)cuda_stream;
     c->have_ws = true; c->have_map = false; c->have_isig = false;
     c->tau_cached.clear(); c->table_kind = kNoTable; c->w_built = false;
+    return ST_OK;
+}
+
+size_t st_bank_cache_bytes(const st_ctx* c, uint64_t n_tracks, int32_t n_max)
+{
+    if (!c || n_tracks == 0 || n_tracks > (1ull << 40) || n_max < 1 || n_max > c->n_t) return 0;
+    return bank_bytes_for(n_tracks, n_max);
+}
+
+int st_set_bank_cache(st_ctx* c, void* cache_dev, size_t bytes)
+{
+    if (!c) return ST_EINVAL;
+    if (cache_dev && ((uintptr_t)cache_dev % kAlign) != 0) return fail(c, ST_EINVAL, "bank cache must be 256-byte aligned");
+    c->bank = (unsigned char*)cache_dev; c->bank_bytes = cache_dev ? bytes : 0; c->bank_valid = false;
     return ST_OK;
 }
 
@@ -848,6 +899,7 @@ static int search_impl(st_ctx* c, const st_search_params* p, st_result* out, flo
         ST_CUDA(c, cudaMemcpyAsync(c->h_hist, sl.hist, sizeof(unsigned long long) * (size_t)p->n_bins, cudaMemcpyDeviceToHost, c->stream));
     ST_CUDA(c, cudaStreamSynchronize(c->stream));
     fill_result(out, *c->h_res, n_tau, plan.kernel, n_launches);
+    out->flags |= c->last_bank_mode == 2 ? ST_FLAG_BANK_READ : (c->last_bank_mode == 1 ? ST_FLAG_BANK_FILLED : 0);
     float ms = 0.0f;
     ST_CUDA(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
     out->gpu_ms = ms;
@@ -1024,7 +1076,7 @@ static int batch_impl(st_ctx* c, const st_batch* b, const st_search_params* p, s
     st_search_params pm = *p;
     for (int g0 = 0; g0 < b->n_maps; g0 += ST_BATCH_GROUP) {
         const int g1 = g0 + ST_BATCH_GROUP < b->n_maps ? g0 + ST_BATCH_GROUP : b->n_maps;
-        std::vector<int> launches((size_t)(g1 - g0), 0);
+        std::vector<int> launches((size_t)(g1 - g0), 0), bank_modes((size_t)(g1 - g0), 0);
         for (int m = g0; m < g1; ++m) {
             const int sb = m & 1;
             if (b->host_buffers) {
@@ -1042,6 +1094,7 @@ static int batch_impl(st_ctx* c, const st_batch* b, const st_search_params* p, s
             rc = enqueue_search(c, &pm, plan, batch_slots(c, m - g0), &nl, false);
             if (rc) return rc;
             launches[(size_t)(m - g0)] = nl;
+            bank_modes[(size_t)(m - g0)] = c->last_bank_mode;
         }
         ST_CUDA(c, cudaMemcpyAsync(c->h_bres, at<void>(c, c->L.b_result), (size_t)(g1 - g0) * sizeof(st::DeviceResult),
                                    cudaMemcpyDeviceToHost, c->stream));
@@ -1052,6 +1105,7 @@ static int batch_impl(st_ctx* c, const st_batch* b, const st_search_params* p, s
         ST_CUDA(c, cudaStreamSynchronize(c->stream));
         for (int m = g0; m < g1; ++m) {
             fill_result(&results[m], c->h_bres[m - g0], n_tau, plan.kernel, launches[(size_t)(m - g0)] + (m == 0 ? n_launches_tables : 0));
+            results[m].flags |= bank_modes[(size_t)(m - g0)] == 2 ? ST_FLAG_BANK_READ : (bank_modes[(size_t)(m - g0)] == 1 ? ST_FLAG_BANK_FILLED : 0);
             if (p->n_bins > 0)
                 for (int k = 0; k < p->n_bins; ++k)
                     p->hist_out[(size_t)m * (size_t)p->n_bins + (size_t)k] = (uint64_t)c->h_bhist[(size_t)(m - g0) * ST_MAX_BINS + (size_t)k];
@@ -1165,7 +1219,7 @@ int st_search_timeshifts(st_ctx* c, const double* s_i, const double* s_j, int64_
     st_search_params pm = *p;
     for (int g0 = 0; g0 < n_shifts; g0 += ST_BATCH_GROUP) {
         const int g1 = g0 + ST_BATCH_GROUP < n_shifts ? g0 + ST_BATCH_GROUP : n_shifts;
-        std::vector<int> launches((size_t)(g1 - g0), 0);
+        std::vector<int> launches((size_t)(g1 - g0), 0), bank_modes((size_t)(g1 - g0), 0);
         for (int m = g0; m < g1; ++m) {
             rc = ft_normalise(c, st_i, st_j, fp->n_neighbours, shifts[m]);
             if (rc) return rc;
@@ -1174,6 +1228,7 @@ int st_search_timeshifts(st_ctx* c, const double* s_i, const double* s_j, int64_
             rc = enqueue_search(c, &pm, plan, batch_slots(c, m - g0), &nl, false);
             if (rc) return rc;
             launches[(size_t)(m - g0)] = nl;
+            bank_modes[(size_t)(m - g0)] = c->last_bank_mode;
         }
         ST_CUDA(c, cudaMemcpyAsync(c->h_bres, at<void>(c, c->L.b_result), (size_t)(g1 - g0) * sizeof(st::DeviceResult),
                                    cudaMemcpyDeviceToHost, c->stream));
@@ -1184,6 +1239,7 @@ int st_search_timeshifts(st_ctx* c, const double* s_i, const double* s_j, int64_
         ST_CUDA(c, cudaStreamSynchronize(c->stream));
         for (int m = g0; m < g1; ++m) {
             fill_result(&results[m], c->h_bres[m - g0], n_tau, plan.kernel, launches[(size_t)(m - g0)] + (m == 0 ? n_launches_tables : 0));
+            results[m].flags |= bank_modes[(size_t)(m - g0)] == 2 ? ST_FLAG_BANK_READ : (bank_modes[(size_t)(m - g0)] == 1 ? ST_FLAG_BANK_FILLED : 0);
             if (p->n_bins > 0)
                 for (int k = 0; k < p->n_bins; ++k)
                     p->hist_out[(size_t)m * (size_t)p->n_bins + (size_t)k] = (uint64_t)c->h_bhist[(size_t)(m - g0) * ST_MAX_BINS + (size_t)k];

@@ -953,3 +953,64 @@ def test_cubic_family_self_recovery_and_explicit_scores(P, orc):
                     for tr in tracks])
     ok, worst = snr_close(got, ref)
     assert ok, worst
+
+
+# ------------------------------------------------------------------ bank cache: S1 + S2 reused across maps (NEXT-2)
+def test_bank_cache_reuses_the_rasterised_bank_across_maps(P, orc):
+    """PAPER.md:173 / :232-234: many maps searched with one template bank.  With a bank cache attached the first
+    search of a bank fills it (ST_FLAG_BANK_FILLED), every later search with the same bank -- on another map, in a
+    batch, after other calls -- reads S1 + S2 back (ST_FLAG_BANK_READ); all results are bit-identical to searches
+    without the cache and agree with the oracle.  A different bank (seed, id range or duration range) refills it."""
+    import torch
+    cfg = synth.CONFIGS[4]
+    tau = synth.tau_linspace(cfg.n_tau)
+    maps = [synth.noise_csd(cfg.n_t, cfg.n_f, 500 + m) for m in range(4)]
+    dev = [torch.from_numpy(x).cuda() for x in maps]
+    T, seed, first = 30_000, 77, 2 ** 33 + 11
+    kw = dict(tau_grid=tau, n_bins=cfg.n_bins, track_offset=first)
+    plain = P.Stochtrack(cfg.n_t, cfg.n_f, cfg.df, cfg.f_min, max_n_tau=cfg.n_tau)
+    want = []
+    for d in dev:
+        plain.set_map(d)
+        want.append(plain.search(T, seed, cfg.n_min, cfg.n_max, **kw))
+    assert all(w.flags & 6 == 0 for w in want)
+    st = P.Stochtrack(cfg.n_t, cfg.n_f, cfg.df, cfg.f_min, max_n_tau=cfg.n_tau)
+    assert st.enable_bank_cache(T, cfg.n_max) > 0
+    got = []
+    for d in dev:
+        st.set_map(d)
+        got.append(st.search(T, seed, cfg.n_min, cfg.n_max, **kw))
+    assert got[0].flags & 4 and not got[0].flags & 2 and all(g.flags & 2 for g in got[1:])
+    for g, w in zip(got, want):
+        for key in ("max_snr", "max_snr_f64", "arg_track", "arg_tau_index", "n_evals", "n_pixels", "n_candidates"):
+            assert g[key] == w[key], key
+        assert np.array_equal(g.hist, w.hist)
+    ref = orc.search(orc.prepare_map(maps[2]), cfg.f_min, cfg.df, T, seed, cfg.n_min, cfg.n_max, tau_grid=tau, track_offset=first,
+                     n_bins=cfg.n_bins, dump_snr=True)
+    _assert_search_parity(SimpleFlags(got[2]), ref, cfg)
+    # one batch call with a shared seed: map 0 reads too (the bank is still cached), results identical
+    res, _ = st.search_batch(dev, None, seed, T, cfg.n_min, cfg.n_max, **kw)
+    assert all(r.flags & 2 for r in res)
+    for r, w in zip(res, want):
+        assert (r.max_snr_f64, r.arg_track, r.arg_tau_index) == (w.max_snr_f64, w.arg_track, w.arg_tau_index) and np.array_equal(r.hist, w.hist)
+    # another bank refills; a bank too large for the buffer is searched without the cache
+    st.set_map(dev[0])
+    other = st.search(T, seed + 1, cfg.n_min, cfg.n_max, **kw)
+    assert other.flags & 4
+    again = st.search(T, seed + 1, cfg.n_min, cfg.n_max, **kw)
+    assert again.flags & 2 and (again.max_snr_f64, again.arg_track) == (other.max_snr_f64, other.arg_track)
+    big = st.search(T + 1000, seed + 1, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=cfg.n_bins)
+    assert big.flags & 6 == 0
+    # per-map seeds (G16): every map brings its own bank, so each one refills
+    res, _ = st.search_batch(dev[:2], None, [5, 6], T, cfg.n_min, cfg.n_max, tau_grid=tau)
+    assert all(r.flags & 4 for r in res)
+    st.disable_bank_cache()
+    assert st.search(T, seed, cfg.n_min, cfg.n_max, **kw).flags & 6 == 0
+
+
+class SimpleFlags(dict):
+    """A search result with the bank-cache bits masked out of `flags` (for _assert_search_parity)."""
+    def __init__(self, r):
+        super().__init__(r)
+        self["flags"] = r["flags"] & ~6
+    __getattr__ = dict.__getitem__
