@@ -122,6 +122,35 @@ def run_ours(args):
     build.build()
     pkg.load_library()
     dev = f"cuda:{local}"
+    env = dict(torch=torch, pkg=pkg, sharding=sharding, dist=dist, world=world, rank=rank, local=local, dev=dev)
+    line = measure(args, env)
+    if rank == 0:
+        # short driver-visible runs of the other workloads (W = 3 warm-up, 2 timed steps each): config 3 (the
+        # paper's random-delay mode), config 4 as the one-call background batch with per-map banks (G16) and with one
+        # shared bank + bank cache, config P (the paper's Table III shape)
+        if world == 1 and args.config == 5 and not args.no_other_configs and not args.tracks:
+            import copy
+            others = []
+            for cid, extra in ((3, {}), (4, dict(maps=20)), (4, dict(maps=20, shared_bank=True)), ("P", {})):
+                a2 = copy.copy(args)
+                a2.config, a2.steps, a2.warmup, a2.no_cpu_baseline, a2.ftmap, a2.maps, a2.shared_bank = cid, 2, 3, True, False, 0, False
+                for k, v in extra.items():
+                    setattr(a2, k, v)
+                o = measure(a2, env)
+                others.append({"config": o["config"]["workload"], "value": o["value"], "unit": o["unit"], "ms_per_step": o["ms_per_step"],
+                               "steps": o["steps"], "warmup": o["warmup"], "tracks_tau_per_s": o["tracks_tau_per_s"],
+                               "e2e_value": o["e2e"]["value"], "gpu_launches": o["gpu_launches"], "clocks": o["clocks"],
+                               "roofline": {k: o["roofline"][k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac")}})
+            line["other_configs"] = others
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def measure(args, env):
+    """One workload, timed as the module docstring says; returns the JSON line as a dict on rank 0 (None elsewhere)."""
+    torch, pkg, sharding, dist = env["torch"], env["pkg"], env["sharding"], env["dist"]
+    world, rank, local, dev = env["world"], env["rank"], env["local"], env["dev"]
     cfg = synth.CONFIGS[args.config]
     n_tracks = args.tracks or cfg.n_tracks
     st = pkg.Stochtrack(cfg.n_t, cfg.n_f, cfg.df, cfg.f_min, max_n_tau=max(cfg.n_tau, 64), device=dev)
@@ -158,6 +187,7 @@ def run_ours(args):
             a = _Agg()
             a.gpu_ms, a.n_launches, a.n_evals = ms, sum(x.n_launches for x in res) - 1, sum(x.n_evals for x in res)
             a.kernel_name, a.best = res[0].kernel_name, max(res, key=lambda x: x.max_snr_f64)
+            a.n_deferred = sum(x.n_deferred for x in res)
             a.maxima = [x.max_snr_f64 for x in res]
             return a
 
@@ -223,9 +253,7 @@ def run_ours(args):
     else:
         combined = r if n_maps == 1 else r.best
     if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
-        return
+        return None
     peak, peak_how = peaks()
     value = evals / (dev_ms * 1e-3)
     per_launch_evals = evals / world / args.steps            # one scoring launch sequence per step per rank
@@ -238,7 +266,7 @@ def run_ours(args):
         "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{workload_tag(args.config)} ({cfg.name}): {cfg.n_t}x{cfg.n_f} map, "
-                               f"{n_tracks:.0e} templates per GPU" + (f" per map x {n_maps} maps in one st_search_batch call" if n_maps > 1 else "") +
+                               f"{n_tracks:.0e} templates per GPU" + (f" per map x {n_maps} maps in one st_search_batch call" + (" (shared bank)" if args.shared_bank else "") if n_maps > 1 else "") +
                                f", {n_tau} delays ({cfg.tau_mode})",
                    "n_t": cfg.n_t, "n_f": cfg.n_f, "n_tracks_per_gpu": n_tracks, "n_tau": n_tau,
                    "tau_mode": cfg.tau_mode, "kernel": r.kernel_name, "l2": "flushed between timed steps (256 MB write)",
@@ -253,10 +281,11 @@ def run_ours(args):
                      "unit": "TFLOP/s", "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
                      "peak_how": peak_how + "; algorithmic 4 flop per track-pixel evaluation (DESIGN.md)"},
         "result": {"max_snr": combined["max_snr_f64"], "arg_track": combined["arg_track"],
-                   "arg_tau_index": combined["arg_tau_index"]},
+                   "arg_tau_index": combined["arg_tau_index"], "n_deferred_last_step": int(r.n_deferred)},
     }
     if n_maps > 1:
         line["config"]["n_maps"] = n_maps
+        line["config"]["bank"] = "one shared bank, bank cache attached" if args.shared_bank else "one bank per map (G16)"
         line["result"]["per_map_max_snr"] = {"min": min(r.maxima), "median": float(np.median(r.maxima)), "max": max(r.maxima)}
         line["roofline"]["peak_how"] += "; batch mode: the kernel time is the device time of the whole call (S0, S1-S4, finalize of every map)"
     if cfg.tau_mode == "random":
@@ -270,9 +299,7 @@ def run_ours(args):
         line["ftmap"] = ftmap_timing(pkg, torch, cfg, dev)
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(cfg, csd, sigma, tau, seed, budget_s=args.cpu_budget)
-    print(json.dumps(line))
-    if dist is not None:
-        dist.destroy_process_group()
+    return line
 
 
 def ftmap_timing(pkg, torch, cfg, dev, seg_len=8192, reps=5):
@@ -381,6 +408,7 @@ def main():
                          "S1 + S2 run once, the other maps read the rasterised bank back (SURVEY 8(f) NEXT-2)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "table", "rotation", "reinsch"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="default run: skip the short runs of configs 3, 4, P")
     ap.add_argument("--ftmap", action="store_true", help="also time st_set_map_from_strain on strain of the config's duration")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--ref-step-s", type=float, default=6.0, help="seconds of oracle work per reference step")

@@ -131,7 +131,8 @@ typedef struct {
     int32_t  n_launches;     /* kernels launched by this call                            */
     int32_t  flags;          /* ST_FLAG_* bits                                           */
     float    gpu_ms;         /* device time of the scoring launches (CUDA events)        */
-    float    reserved;
+    int32_t  n_deferred;     /* Chebyshev path: templates re-scored by the two-class build because their
+                                amplitude in drift-prone (class B) bins was too large for the fast build */
 } st_result;
 
 #define ST_FLAG_CAND_OVERFLOW 1   /* candidate list overflowed: argmax decided by the float32 records      */

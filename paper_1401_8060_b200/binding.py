@@ -54,7 +54,7 @@ class CResult(C.Structure):
                 ("arg_track", C.c_uint64), ("arg_tau", C.c_double), ("arg_params", CTrack),
                 ("n_evals", C.c_uint64), ("n_pixels", C.c_uint64), ("n_candidates", C.c_int32),
                 ("kernel_used", C.c_int32), ("n_launches", C.c_int32), ("flags", C.c_int32),
-                ("gpu_ms", C.c_float), ("reserved", C.c_float)]
+                ("gpu_ms", C.c_float), ("n_deferred", C.c_int32)]
 
 
 class CTopEntry(C.Structure):
@@ -422,7 +422,7 @@ class Stochtrack:
                             arg_params=r.arg_params.as_dict(), n_evals=int(r.n_evals), n_pixels=int(r.n_pixels),
                             n_candidates=int(r.n_candidates), kernel_used=int(r.kernel_used),
                             kernel_name=KERNEL_NAMES.get(int(r.kernel_used), "?"), n_launches=int(r.n_launches),
-                            flags=int(r.flags), gpu_ms=float(r.gpu_ms), hist=hist)
+                            flags=int(r.flags), gpu_ms=float(r.gpu_ms), n_deferred=int(r.n_deferred), hist=hist)
 
     def search_batch(self, csd_maps, sigma_maps, seeds, n_tracks, n_min, n_max, tau_grid=None, tau_range=None,
                      norm=NORM_SQRT_N, n_bins=0, hist_lo=-10.0, hist_hi=10.0, track_offset=0, kernel=KERNEL_AUTO, family=FAMILY_QUADRATIC):

@@ -55,6 +55,8 @@ struct Scalars {         // device scalars of one search, zeroed by the host
     uint32_t cand_count;
     uint32_t overflow;
     uint32_t n_deferred;            // templates the fast Chebyshev build handed to the two-class build (per launch)
+    uint32_t n_deferred_total;      // the same summed over the launches of the search
+    uint32_t pad;
 };
 
 struct DeviceResult {
@@ -67,6 +69,8 @@ struct DeviceResult {
     int32_t  n_candidates;
     int32_t  flags;
     unsigned long long n_pixels;
+    uint32_t n_deferred;
+    uint32_t pad;
 };
 
 struct ScoreArgs {
@@ -903,6 +907,42 @@ __device__ __forceinline__ float pk_sum(f32x2_t a)
     return lo + hi;
 }
 
+// Shared-memory accesses of the Chebyshev kernel's row loops through explicit 32-bit shared addresses: with
+// generic pointers the compiler re-derived every base address from the kernel parameters inside the loop
+// (~25 integer / uniform instructions per row pair, the IMADs among them on the FMA pipe).
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+template <int OFF>
+__device__ __forceinline__ float2 lds_f2(uint32_t addr)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2+%3];" : "=f"(v.x), "=f"(v.y) : "r"(addr), "n"(OFF));
+    return v;
+}
+template <int OFF>
+__device__ __forceinline__ void sts_f2(uint32_t addr, float x, float y)
+{
+    asm volatile("st.shared.v2.f32 [%0+%1], {%2, %3};" :: "r"(addr), "n"(OFF), "f"(x), "f"(y) : "memory");
+}
+template <int OFF>
+__device__ __forceinline__ uint32_t lds_u16(uint32_t addr)
+{
+    uint32_t k;
+    asm volatile("{\n\t.reg .u16 t;\n\tld.shared.u16 t, [%1+%2];\n\tcvt.u32.u16 %0, t;\n\t}" : "=r"(k) : "r"(addr), "n"(OFF));
+    return k;
+}
+__device__ __forceinline__ float4 lds_f4(uint32_t addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds_f1(uint32_t addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+
 constexpr int kChunk = 32;        // delays per accumulator chunk
 constexpr int kSuper = 256;       // delays between re-anchoring (8 chunks)
 
@@ -1158,6 +1198,14 @@ struct ChebElem { int k[4]; float2 p[4], e[4]; float r[4]; };     // r: 1 / sigm
 struct ChebMergeState { int run_k, n_a, n_b; float ax, ay; float2 run_e; float w2, bamp; };
 struct ChebCounts { int n_a, n_b; };       // pool entries of class A (front of the pool) and class B (back)
 
+// The normative rasteriser sequence of the rare fallback.  Measured as an out-of-line call (-DST_COLD_CALL: 19 %
+// less code in the kernel): config 4 +0.5 %, config 5 -1.4 % -- inlined it stays.
+#ifndef ST_COLD_CALL
+__device__ __forceinline__ int32_t raster_bin_cold(const Raster& r, int32_t c) { return raster_bin(r, c); }
+#else
+__device__ __noinline__ int32_t raster_bin_cold(const Raster r, int32_t c) { return raster_bin(r, c); }
+#endif
+
 // GEN = false compiles the default search (quadratic templates, N^-alpha normalisation) with the template
 // family and the weighting as constants; GEN = true reads both from the arguments (cubic family, norm 2).
 // BANK: 0 no bank cache, 1 this launch fills it, 2 this launch reads it (S1 + S2 skipped)
@@ -1193,7 +1241,7 @@ __device__ __forceinline__ void cheb_fetch(const ScoreArgs& a, const ChebFetchCt
         if (redo[0] | redo[1] | redo[2] | redo[3]) {   // ~1e-5 of the time: normative sequence
 #pragma unroll
             for (int u = 0; u < 4; ++u)
-                if (redo[u]) E.k[u] = raster_bin(f.r, cc[u]);
+                if (redo[u]) E.k[u] = raster_bin_cold(f.r, cc[u]);
         }
         if (BANK == 1)
             *reinterpret_cast<uint2*>(f.krow + i) = make_uint2((uint32_t)E.k[0] | ((uint32_t)E.k[1] << 16),
@@ -1345,6 +1393,10 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
     const int S = a.pool_stride;
     TrackMax tm;
     tmax_init(tm);
+#ifndef ST_PLAIN_ADDR
+    const uint32_t pv_base = smem_u32(pool_v) + (uint32_t)lane * 8u, pk_base = smem_u32(pool_k) + (uint32_t)lane * 2u;
+    const uint32_t tab_base = smem_u32(sm_tab), zi_base = smem_u32(sm_zi);
+#endif
     // ---- phase B: chunks of 64 delays; f2[i] = (sum x_{mc+i}, sum x_{mc-1-i}) over this lane's pixels
 #pragma unroll 1
     for (int j = 0; j < n_chunks; ++j) {
@@ -1352,6 +1404,21 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
 #pragma unroll
         for (int i = 0; i < kHalf; ++i) f2[i] = 0ull;
         int row = 0;
+#ifndef ST_PLAIN_ADDR
+        uint32_t pv = pv_base, pk = pk_base;           // this lane's entry of the current row
+#pragma unroll 1
+        for (; row + 2 <= n_rows; row += 2, pv += 2 * kWarp * 8, pk += 2 * kWarp * 2) {
+            const float2 v0 = lds_f2<0>(pv), v1 = lds_f2<kWarp * 8>(pv);
+            const uint32_t k0 = lds_u16<0>(pk), k1 = lds_u16<kWarp * 2>(pk);
+            ST_ASSERT(k0 < (uint32_t)a.bp.n_f && k1 < (uint32_t)a.bp.n_f);
+            const float4 t0 = lds_f4(tab_base + k0 * 16u), t1 = lds_f4(tab_base + k1 * 16u);
+            const float zi0 = lds_f1(zi_base + k0 * 4u), zi1 = lds_f1(zi_base + k1 * 4u);
+            // next chunk's anchors: v e^{i 64 theta}   (t.w = cos 64 theta, zi = sin 64 theta).  Unconditional: skipping
+            // the advance on the last chunk (a warp-uniform branch here) cost 4-7 % (measured, round 2)
+            sts_f2<0>(pv, fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
+            sts_f2<kWarp * 8>(pv, fmaf(v1.x, t1.w, -(v1.y * zi1)), fmaf(v1.x, zi1, v1.y * t1.w));
+            ChebPixel<STRIDE> A, B;
+#else
 #pragma unroll 1
         for (; row + 2 <= n_rows; row += 2) {
             const int e0 = row * kWarp + lane, e1 = e0 + kWarp;
@@ -1360,11 +1427,10 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
             ST_ASSERT(k0 >= 0 && k0 < a.bp.n_f && k1 >= 0 && k1 < a.bp.n_f);
             const float4 t0 = sm_tab[k0], t1 = sm_tab[k1];
             const float zi0 = sm_zi[k0], zi1 = sm_zi[k1];
-            // next chunk's anchors: v e^{i 64 theta}   (t.w = cos 64 theta, zi = sin 64 theta).  Unconditional: skipping
-            // the advance on the last chunk (a warp-uniform branch here) cost 4-7 % (measured, round 2)
             pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
             pool_v[e1] = make_float2(fmaf(v1.x, t1.w, -(v1.y * zi1)), fmaf(v1.x, zi1, v1.y * t1.w));
             ChebPixel<STRIDE> A, B;
+#endif
             A.anchor(v0, t0);
             B.anchor(v1, t1);
             if (STRIDE == 1) {
@@ -1402,12 +1468,20 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
             }
         }
         if (row < n_rows) {          // odd tail row
+#ifndef ST_PLAIN_ADDR
+            const float2 v0 = lds_f2<0>(pv);
+            const uint32_t k0 = lds_u16<0>(pk);
+            const float4 t0 = lds_f4(tab_base + k0 * 16u);
+            const float zi0 = lds_f1(zi_base + k0 * 4u);
+            sts_f2<0>(pv, fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
+#else
             const int e0 = row * kWarp + lane;
             const float2 v0 = pool_v[e0];
             const int k0 = pool_k[e0];
             const float4 t0 = sm_tab[k0];
             const float zi0 = sm_zi[k0];
             pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
+#endif
             ChebPixel<STRIDE> A;
             A.anchor(v0, t0);
             if (STRIDE == 1) {
@@ -1508,6 +1582,7 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
     // a launch works through its own id range, or (general build, defer_in) through the list of templates the
     // fast build handed over: the list is complete, the fast launch precedes this one on the stream
     const uint64_t n_items = (GEN && a.defer_in) ? (uint64_t)min(a.sc->n_deferred, a.deferred_cap) : a.n_tracks;
+    if (GEN && a.defer_in && blockIdx.x == 0 && threadIdx.x == 0) a.sc->n_deferred_total += (uint32_t)n_items;
     for (;;) {
         const uint64_t item = __shfl_sync(kFull, q_pref, 0);
         if (item >= n_items) break;
@@ -1655,6 +1730,7 @@ __global__ void __launch_bounds__(256) k_finalize(const FinalArgs a)
         res.max_snr = gmax; res.arg_m = 0; res.snr_f64 = 0.0; res.arg_id = 0; res.arg_tau = 0.0;
         res.track.N = 0; res.track.j0 = 0; res.track.a = res.track.y0 = res.track.y1 = res.track.y2 = res.track.tau = res.track.y3 = 0.0;
         res.n_candidates = total; res.flags = overflow ? 1 : 0; res.n_pixels = a.sc->n_pixels;
+        res.n_deferred = a.sc->n_deferred_total; res.pad = 0;
         if (have) {
             const Track t = make_track(a.bp, bid);
             const double tau = a.tau_mode == 0 ? a.tau_d[bm] : t.tau;

@@ -424,7 +424,10 @@ size_t bank_bytes_for(uint64_t n_tracks, int n_max)
 // Absolute error (in SNR units) the fast Chebyshev build may owe to coefficient drift in class B bins: half the
 // G13 tolerance at a zero crossing of SNR(tau) on the configs' data (1e-4 x s0, s0 = 0.707).  Class A bins add
 // at most kChebClassDrift x A for a coherent amplitude A (3e-5 at SNR 10).
-constexpr double kChebDeferBudget = 3.5e-5;
+#ifndef ST_DEFER_BUDGET
+#define ST_DEFER_BUDGET 3.5e-5
+#endif
+constexpr double kChebDeferBudget = ST_DEFER_BUDGET;
 
 int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max, int* extra_launches = nullptr)
 {
@@ -646,6 +649,7 @@ void fill_result(st_result* out, const st::DeviceResult& r, int n_tau, int kerne
     out->arg_params.tau = r.track.tau; out->arg_params.y3 = r.track.y3;
     out->n_pixels = r.n_pixels; out->n_evals = r.n_pixels * (uint64_t)n_tau;
     out->n_candidates = r.n_candidates; out->flags = r.flags; out->n_launches = n_launches;
+    out->n_deferred = (int32_t)r.n_deferred;
     out->kernel_used = kernel;
 }
 
