@@ -120,6 +120,7 @@ struct ScoreArgs {
     uint32_t kcache_stride;   // uint16 entries per template = 32 * ceil4(ceil(n_max / 32))
     uint64_t kcache_base;     // cache row of template 0 of this launch
     int32_t kcache_mode;      // 0 unused, 1 this launch fills the cache, 2 it reads it
+    uint32_t fold_offset;     // Chebyshev kernel, shared-memory fold: byte offset of the per-warp fold scratch
 };
 
 // Template q of the launch: regenerated from (seed, id), or read from the caller's explicit list.
@@ -1179,6 +1180,7 @@ struct ChebPixel {
 #ifndef ST_CHEB_MAX_THREADS
 #define ST_CHEB_MAX_THREADS 512
 #endif
+#define ST_CHEB_PIPE_THREADS 384      // builds with the software-pipelined phase B: 168 registers per thread
 // ---- Phase A of the Chebyshev kernels: rasterise, gather p, merge runs of consecutive columns
 // that fall in the same bin (their terms share the phase factor, so Eq. 8 only needs the sum of
 // their p), compact into the pool, rotate to the anchor of chunk 0.  A lane owns L = ceil(N / 32)
@@ -1187,6 +1189,13 @@ struct ChebPixel {
 // through a ballot.  The work is cut into ELEMENTS of four columns per lane: cheb_fetch issues the
 // four rasteriser chains and the L2 gathers of an element, cheb_merge consumes them, so that a
 // caller can keep the next element in flight while it merges the current one.
+// A map pixel is used once per template: gathered past L1 so that the per-bin tables stay there.
+__device__ __forceinline__ float2 ldg_stream_f2(const float2* p)
+{
+    float2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
 struct ChebFetchCtx {          // what fetching needs to know about a template
     Raster r;
     uint16_t* krow;            // bank cache: this lane's slice of the template's row
@@ -1251,7 +1260,11 @@ __device__ __forceinline__ void cheb_fetch(const ScoreArgs& a, const ChebFetchCt
     for (int u = 0; u < 4; ++u) {
         ST_ASSERT(E.k[u] >= 0 && E.k[u] < a.bp.n_f && cc[u] >= 0 &&
                   (size_t)(f.col0 - a.map) / (size_t)a.bp.n_f + (size_t)cc[u] < (size_t)a.bp.n_t);
+#ifdef ST_X_NOALLOC
+        E.p[u] = ldg_stream_f2(f.col0 + (size_t)cc[u] * (size_t)a.bp.n_f + (size_t)E.k[u]);
+#else
         E.p[u] = __ldg(f.col0 + (size_t)cc[u] * (size_t)a.bp.n_f + (size_t)E.k[u]);
+#endif
         E.e[u] = __ldg(&a.Ec[E.k[u]]);
     }
     if (GEN && a.norm == 2) {                          // inverse-variance weights (G25): one more gather per pixel
@@ -1557,8 +1570,299 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
     if (MODE == 2) tmax_finish(a, tm, q);
 }
 
-template <int STRIDE, int MODE, bool GEN, int BANK>
-__global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const ScoreArgs a)
+// Phase B, delay-split form (PB 1, 2): the two half-warps work on TWO chunks of the same 16 pool entries
+// per row -- lanes 0-15 on chunk 2 jp (anchor v as stored), lanes 16-31 on chunk 2 jp + 1 (anchor
+// v e^{i 64 theta}) -- so one fold and one S4 epilogue serve 128 delays, rows are padded to 16 entries
+// instead of 32, and the two halves read the same pool and table words (broadcasts, half the bank
+// conflicts).  The anchor of the next pass, v e^{i 128 theta}, is formed as (v z64) z64: the same two
+// float32 rotations the one-chunk form applies in two steps.
+//   FOLD 0: transposing shuffle tree over the 16 lanes of a half (30 packed shuffles per pass; lane l of
+//           a half ends with accumulators 2 l and 2 l + 1);
+//   FOLD 1: through shared memory in two rounds of 16 accumulators (8 STS.128, 16 LDS.64 and 15 packed
+//           adds per round; lane l ends with accumulators l and 16 + l); needs kFoldWords floats per warp.
+//   SINGLE: the grid has at most two chunks: one pass, no anchor is stored back.
+constexpr int kFoldRow = 36;                    // floats per lane row of the fold scratch: 16 pairs + 16 B (conflict-free)
+constexpr int kFoldWords = kWarp * kFoldRow;    // floats of fold scratch per warp (4608 B)
+__device__ __forceinline__ void sts_f4(uint32_t addr, f32x2_t a, f32x2_t b)
+{
+    asm volatile("st.shared.v2.b64 [%0], {%1, %2};" :: "r"(addr), "l"(a), "l"(b) : "memory");
+}
+__device__ __forceinline__ f32x2_t lds_pk(uint32_t addr)
+{
+    f32x2_t v;
+    asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr));
+    return v;
+}
+// One row pair of the delay-split phase B on its way from the pool to its chain heads, in three stages.
+struct ChebStage { float2 v0, v1; uint32_t k0, k1; float4 t0, t1; float zi0, zi1; };
+__device__ __forceinline__ void cheb_stage_load(ChebStage& g, const uint32_t pv, const uint32_t pk)
+{
+    g.v0 = lds_f2<0>(pv); g.v1 = lds_f2<16 * 8>(pv);
+    g.k0 = lds_u16<0>(pk); g.k1 = lds_u16<16 * 2>(pk);
+}
+__device__ __forceinline__ void cheb_stage_table(ChebStage& g, const uint32_t tab_base, const uint32_t zi_base)
+{
+    g.t0 = lds_f4(tab_base + g.k0 * 16u); g.t1 = lds_f4(tab_base + g.k1 * 16u);
+    g.zi0 = lds_f1(zi_base + g.k0 * 4u); g.zi1 = lds_f1(zi_base + g.k1 * 4u);
+}
+__device__ __forceinline__ void sts_f2_if(const bool p, const uint32_t addr, const float x, const float y)
+{
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %0, 0;\n\t@q st.shared.v2.f32 [%1], {%2, %3};\n\t}"
+                 :: "r"((uint32_t)p), "r"(addr), "f"(x), "f"(y) : "memory");
+}
+template <int STRIDE, bool SINGLE>
+__device__ __forceinline__ void cheb_stage_anchor(const ChebStage& g, const bool upper, const bool store, const uint32_t pv,
+                                                  ChebPixel<STRIDE>& A, ChebPixel<STRIDE>& B)
+{
+    const float r0x = fmaf(g.v0.x, g.t0.w, -(g.v0.y * g.zi0)), r0y = fmaf(g.v0.x, g.zi0, g.v0.y * g.t0.w);   // v e^{i 64 theta}
+    const float r1x = fmaf(g.v1.x, g.t1.w, -(g.v1.y * g.zi1)), r1y = fmaf(g.v1.x, g.zi1, g.v1.y * g.t1.w);
+    if (!SINGLE) {                                          // the next pass's anchor, (v z64) z64, kept by the lower half
+        sts_f2_if(store, pv, fmaf(r0x, g.t0.w, -(r0y * g.zi0)), fmaf(r0x, g.zi0, r0y * g.t0.w));
+        sts_f2_if(store, pv + 16 * 8, fmaf(r1x, g.t1.w, -(r1y * g.zi1)), fmaf(r1x, g.zi1, r1y * g.t1.w));
+    }
+    A.anchor(make_float2(upper ? r0x : g.v0.x, upper ? r0y : g.v0.y), g.t0);
+    B.anchor(make_float2(upper ? r1x : g.v1.x, upper ? r1y : g.v1.y), g.t1);
+}
+template <int STRIDE, int MODE, bool TWO, int FOLD, bool SINGLE, bool PIPE>
+__device__ __forceinline__ void cheb_phase_b_split(const ScoreArgs& a, WarpReduce& wr, uint32_t* sm_hist,
+                                                   const float4* sm_tab, const float* sm_zi, float2* pool_v,
+                                                   const uint16_t* pool_k, float* fold, const ChebCounts cnt, const float scale,
+                                                   const uint64_t id, const uint64_t q, const int n_chunks, const int lane)
+{
+    constexpr int kW = 16;                                  // pool entries per row
+    // class A rows of 16 entries, from the front of the pool (zero-filled to whole rows of 32: the pipelined form
+    // takes rows in pairs, the plain form handles an odd last row on its own)
+    const int n_rows = PIPE ? ((cnt.n_a + kWarp - 1) >> 5) << 1 : (cnt.n_a + kW - 1) >> 4;
+    const int n_rows_b = TWO ? (cnt.n_b + kW - 1) >> 4 : 0; // class B rows, from its back
+    const int S = a.pool_stride;
+    const int l16 = lane & 15;
+    const bool upper = (lane & 16) != 0;
+    TrackMax tm;
+    tmax_init(tm);
+    const uint32_t pv_base = smem_u32(pool_v) + (uint32_t)l16 * 8u, pk_base = smem_u32(pool_k) + (uint32_t)l16 * 2u;
+    const uint32_t tab_base = smem_u32(sm_tab), zi_base = smem_u32(sm_zi);
+    const int n_pass = SINGLE ? 1 : (n_chunks + 1) >> 1;
+#pragma unroll 1
+    for (int jp = 0; jp < n_pass; ++jp) {
+        f32x2_t f2[kHalf];
+#pragma unroll
+        for (int i = 0; i < kHalf; ++i) f2[i] = 0ull;
+        if (!PIPE) {
+        int row = 0;
+        uint32_t pv = pv_base, pk = pk_base;
+#pragma unroll 1
+        for (; row + 2 <= n_rows; row += 2, pv += 2 * kW * 8, pk += 2 * kW * 2) {
+            ChebStage g;
+            cheb_stage_load(g, pv, pk);
+            ST_ASSERT(g.k0 < (uint32_t)a.bp.n_f && g.k1 < (uint32_t)a.bp.n_f);
+            cheb_stage_table(g, tab_base, zi_base);
+            ChebPixel<STRIDE> A, B;
+            cheb_stage_anchor<STRIDE, SINGLE>(g, upper, !upper, pv, A, B);
+            if (STRIDE == 1) {
+#pragma unroll
+                for (int i = 0; i < kHalf; i += 2) {
+                    f2[i] = pk_add(f2[i], A.ce);
+                    f2[i] = pk_add(f2[i], B.ce);
+                    A.pe = pk_step(A.G, A.ce, A.pe);
+                    B.pe = pk_step(B.G, B.ce, B.pe);
+                    f2[i + 1] = pk_add(f2[i + 1], A.pe);
+                    f2[i + 1] = pk_add(f2[i + 1], B.pe);
+                    A.ce = pk_step(-A.G, A.pe, A.ce);
+                    B.ce = pk_step(-B.G, B.pe, B.ce);
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < kHalf; i += 4) {
+                    f2[i] = pk_add(f2[i], A.ce);
+                    f2[i] = pk_add(f2[i], B.ce);
+                    f2[i + 1] = pk_add(f2[i + 1], A.co);
+                    f2[i + 1] = pk_add(f2[i + 1], B.co);
+                    A.pe = pk_step(A.G, A.ce, A.pe);
+                    B.pe = pk_step(B.G, B.ce, B.pe);
+                    A.po = pk_step(A.G, A.co, A.po);
+                    B.po = pk_step(B.G, B.co, B.po);
+                    f2[i + 2] = pk_add(f2[i + 2], A.pe);
+                    f2[i + 2] = pk_add(f2[i + 2], B.pe);
+                    f2[i + 3] = pk_add(f2[i + 3], A.po);
+                    f2[i + 3] = pk_add(f2[i + 3], B.po);
+                    A.ce = pk_step(-A.G, A.pe, A.ce);
+                    B.ce = pk_step(-B.G, B.pe, B.ce);
+                    A.co = pk_step(-A.G, A.po, A.co);
+                    B.co = pk_step(-B.G, B.po, B.co);
+                }
+            }
+        }
+        if (row < n_rows) {          // odd last row
+            const float2 v0 = lds_f2<0>(pv);
+            const uint32_t k0 = lds_u16<0>(pk);
+            const float4 t0 = lds_f4(tab_base + k0 * 16u);
+            const float zi0 = lds_f1(zi_base + k0 * 4u);
+            const float r0x = fmaf(v0.x, t0.w, -(v0.y * zi0)), r0y = fmaf(v0.x, zi0, v0.y * t0.w);
+            if (!SINGLE) sts_f2_if(!upper, pv, fmaf(r0x, t0.w, -(r0y * zi0)), fmaf(r0x, zi0, r0y * t0.w));
+            ChebPixel<STRIDE> A;
+            A.anchor(make_float2(upper ? r0x : v0.x, upper ? r0y : v0.y), t0);
+            if (STRIDE == 1) {
+#pragma unroll
+                for (int i = 0; i < kHalf; i += 2) {
+                    f2[i] = pk_add(f2[i], A.ce);
+                    A.pe = pk_step(A.G, A.ce, A.pe);
+                    f2[i + 1] = pk_add(f2[i + 1], A.pe);
+                    A.ce = pk_step(-A.G, A.pe, A.ce);
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < kHalf; i += 4) {
+                    f2[i] = pk_add(f2[i], A.ce);
+                    f2[i + 1] = pk_add(f2[i + 1], A.co);
+                    A.pe = pk_step(A.G, A.ce, A.pe);
+                    A.po = pk_step(A.G, A.co, A.po);
+                    f2[i + 2] = pk_add(f2[i + 2], A.pe);
+                    f2[i + 3] = pk_add(f2[i + 3], A.po);
+                    A.ce = pk_step(-A.G, A.pe, A.ce);
+                    A.co = pk_step(-A.G, A.po, A.co);
+                }
+            }
+        }
+        } else {
+        // Row pairs, software-pipelined: the pool / table reads, the anchor rotation and the chain heads of the
+        // NEXT pair are issued at fixed points under the 32 steps of the current one (every access and every packed
+        // operation here is a volatile asm statement, so the source order is the issue order).  On the last pair the
+        // "next" pair is the current one again (a harmless re-read, its store predicated off).
+        uint32_t pv = pv_base, pk = pk_base;
+        ChebPixel<STRIDE> A, B;
+        if (n_rows > 0) {                                   // (a template of class B pixels only has no class A row)
+            ChebStage g;
+            cheb_stage_load(g, pv, pk);
+            cheb_stage_table(g, tab_base, zi_base);
+            cheb_stage_anchor<STRIDE, SINGLE>(g, upper, !upper, pv, A, B);
+        }
+#pragma unroll 1
+        for (int row = 0; row < n_rows; row += 2) {
+            const bool has_next = row + 2 < n_rows;
+            const uint32_t pvn = has_next ? pv + 2 * kW * 8 : pv, pkn = has_next ? pk + 2 * kW * 2 : pk;
+            ChebStage g;
+            ChebPixel<STRIDE> An, Bn;
+            if (STRIDE == 1) {
+#pragma unroll
+                for (int i = 0; i < kHalf; i += 2) {
+                    if (i == 0) cheb_stage_load(g, pvn, pkn);
+                    if (i == 8) cheb_stage_table(g, tab_base, zi_base);
+                    if (i == 20) cheb_stage_anchor<STRIDE, SINGLE>(g, upper, has_next && !upper, pvn, An, Bn);
+                    f2[i] = pk_add(f2[i], A.ce);
+                    f2[i] = pk_add(f2[i], B.ce);
+                    A.pe = pk_step(A.G, A.ce, A.pe);
+                    B.pe = pk_step(B.G, B.ce, B.pe);
+                    f2[i + 1] = pk_add(f2[i + 1], A.pe);
+                    f2[i + 1] = pk_add(f2[i + 1], B.pe);
+                    A.ce = pk_step(-A.G, A.pe, A.ce);
+                    B.ce = pk_step(-B.G, B.pe, B.ce);
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < kHalf; i += 4) {
+                    if (i == 0) cheb_stage_load(g, pvn, pkn);
+                    if (i == 8) cheb_stage_table(g, tab_base, zi_base);
+                    if (i == 20) cheb_stage_anchor<STRIDE, SINGLE>(g, upper, has_next && !upper, pvn, An, Bn);
+                    f2[i] = pk_add(f2[i], A.ce);
+                    f2[i] = pk_add(f2[i], B.ce);
+                    f2[i + 1] = pk_add(f2[i + 1], A.co);
+                    f2[i + 1] = pk_add(f2[i + 1], B.co);
+                    A.pe = pk_step(A.G, A.ce, A.pe);
+                    B.pe = pk_step(B.G, B.ce, B.pe);
+                    A.po = pk_step(A.G, A.co, A.po);
+                    B.po = pk_step(B.G, B.co, B.po);
+                    f2[i + 2] = pk_add(f2[i + 2], A.pe);
+                    f2[i + 2] = pk_add(f2[i + 2], B.pe);
+                    f2[i + 3] = pk_add(f2[i + 3], A.po);
+                    f2[i + 3] = pk_add(f2[i + 3], B.po);
+                    A.ce = pk_step(-A.G, A.pe, A.ce);
+                    B.ce = pk_step(-B.G, B.pe, B.ce);
+                    A.co = pk_step(-A.G, A.po, A.co);
+                    B.co = pk_step(-B.G, B.po, B.co);
+                }
+            }
+            A = An; B = Bn; pv = pvn; pk = pkn;
+        }
+        }
+        // ---- class B rows (Reinsch's form, see the one-chunk form above), 16 entries per row from the back
+        if (TWO) {
+#pragma unroll 1
+        for (int rb = 0; rb < n_rows_b; ++rb) {
+            const int e0 = S - kW * (rb + 1) + l16;
+            const float2 v0 = pool_v[e0];
+            const int k0 = pool_k[e0];
+            ST_ASSERT(e0 >= 0 && k0 >= 0 && k0 < a.bp.n_f);
+            const float4 t0 = sm_tab[k0];
+            const float zi0 = sm_zi[k0];
+            const float r0x = fmaf(v0.x, t0.w, -(v0.y * zi0)), r0y = fmaf(v0.x, zi0, v0.y * t0.w);
+            if (!SINGLE) {
+                const float n0x = fmaf(r0x, t0.w, -(r0y * zi0)), n0y = fmaf(r0x, zi0, r0y * t0.w);
+                __syncwarp();                              // both halves have read the entry
+                if (!upper) pool_v[e0] = make_float2(n0x, n0y);
+            }
+            const float ax = upper ? r0x : v0.x, ay = upper ? r0y : v0.y;
+            const float kap = __fdiv_rn(2.0f * t0.z * t0.z, 1.0f + t0.y);
+            const float dlt = fmaf(0.5f * kap, ax, -(ay * t0.z));
+            f32x2_t x = pk_make(ax, ax - dlt), d = pk_make(dlt, -dlt);
+            const float nk = -kap;
+#pragma unroll
+            for (int i = 0; i < kHalf; ++i) {
+                f2[i] = ((i >> STRIDE) & 1) ? pk_sub(f2[i], x) : pk_add(f2[i], x);
+                d = pk_step(nk, x, d);
+                x = pk_add(x, d);
+            }
+        }
+        }
+        // ---- fold over the 16 lanes of each half; this lane's two accumulators are i0 and i1
+        int i0, i1;
+        f32x2_t g0, g1;
+        if (FOLD == 0) {
+#pragma unroll
+            for (int off = 8, n = kHalf / 2; off >= 1; off >>= 1, n >>= 1) {
+                const bool up = (lane & off) != 0;
+#pragma unroll
+                for (int i = 0; i < n; ++i) {
+                    const f32x2_t send = up ? f2[i] : f2[i + n];
+                    const f32x2_t keep = up ? f2[i + n] : f2[i];
+                    f2[i] = pk_add(keep, __shfl_xor_sync(kFull, send, off));
+                }
+            }
+            g0 = f2[0]; g1 = f2[1]; i0 = 2 * l16; i1 = i0 + 1;
+        } else {
+            const uint32_t fs = smem_u32(fold);
+            const uint32_t wr_addr = fs + (uint32_t)lane * (kFoldRow * 4u);
+            const uint32_t rd_addr = fs + (uint32_t)(lane & 16) * (kFoldRow * 4u) + (uint32_t)l16 * 8u;
+            f32x2_t g[2];
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {
+                __syncwarp();
+#pragma unroll
+                for (int i = 0; i < 16; i += 2) sts_f4(wr_addr + (uint32_t)i * 8u, f2[16 * r + i], f2[16 * r + i + 1]);
+                __syncwarp();
+                f32x2_t s[16];
+#pragma unroll
+                for (int rr = 0; rr < 16; ++rr) s[rr] = lds_pk(rd_addr + (uint32_t)rr * (kFoldRow * 4u));
+#pragma unroll
+                for (int w = 8; w >= 1; w >>= 1)
+#pragma unroll
+                    for (int rr = 0; rr < w; ++rr) s[rr] = pk_add(s[rr], s[rr + w]);
+                g[r] = s[0];
+            }
+            g0 = g[0]; g1 = g[1]; i0 = l16; i1 = l16 + 16;
+        }
+        const int mc = (2 * jp + (upper ? 1 : 0)) * kCheb + kHalf;
+        const float s0 = ((i0 >> STRIDE) & 1) ? -scale : scale, s1 = ((i1 >> STRIDE) & 1) ? -scale : scale;
+        const float v[4] = {pk_lo(g0) * s0, pk_hi(g0) * s0, pk_lo(g1) * s1, pk_hi(g1) * s1};
+        const uint32_t ms[4] = {(uint32_t)(mc + i0), (uint32_t)(mc - 1 - i0), (uint32_t)(mc + i1), (uint32_t)(mc - 1 - i1)};
+        const bool ok[4] = {(int)ms[0] < a.n_tau, (int)ms[1] < a.n_tau, (int)ms[2] < a.n_tau, (int)ms[3] < a.n_tau};
+        reduce_samples<4, MODE == 1 ? 1 : 0>(a, wr, sm_hist, id, q, v, ms, ok);
+        if (MODE == 2) tmax_update<4>(tm, v, ms, ok);
+    }
+    if (MODE == 2) tmax_finish(a, tm, q);
+}
+
+template <int STRIDE, int MODE, bool GEN, int BANK, int PB = 0, bool PIPE = false>
+__global__ void __launch_bounds__(PIPE ? ST_CHEB_PIPE_THREADS : ST_CHEB_MAX_THREADS, 1) k_score_cheb(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
@@ -1570,6 +1874,8 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
     float2* pool_v = reinterpret_cast<float2*>(sm_tab + a.bp.n_f) + (size_t)warp * S;
     float* sm_zi = reinterpret_cast<float*>(reinterpret_cast<float2*>(sm_tab + a.bp.n_f) + (size_t)n_warps * S);
     uint16_t* pool_k = reinterpret_cast<uint16_t*>(sm_zi + ((a.bp.n_f + 1) & ~1)) + (size_t)warp * S;
+    // PB 2, 4: per-warp fold scratch behind the bin pools (16-byte aligned: the host pads the pools)
+    float* fold = reinterpret_cast<float*>(smem + a.fold_offset) + (size_t)warp * kFoldWords;
     for (int k = threadIdx.x; k < a.bp.n_f; k += blockDim.x) { sm_tab[k] = a.cheb[k]; sm_zi[k] = a.cheb_zi[k]; }
     hist_init(sm_hist, a.n_bins);
     const int n_chunks = (a.n_tau + kCheb - 1) / kCheb;
@@ -1612,8 +1918,13 @@ __global__ void __launch_bounds__(ST_CHEB_MAX_THREADS, 1) k_score_cheb(const Sco
         ST_ASSERT(cnt.n_a + cnt.n_b >= 1 && cnt.n_a + cnt.n_b <= t.N &&
                   ((cnt.n_a + kWarp - 1) & ~(kWarp - 1)) + ((cnt.n_b + kWarp - 1) & ~(kWarp - 1)) <= S &&
                   (a.tracks || (t.N >= a.bp.n_min && t.N <= a.bp.n_max)) && t.j0 >= 0 && t.j0 + t.N <= a.bp.n_t);
-        cheb_phase_b<STRIDE, MODE, GEN>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, cnt, scale, id, q,
-                             n_chunks, lane);
+        // PB: 0 one chunk per pass; 1 / 2 two chunks per pass (shuffle / shared-memory fold); 3 / 4 the same for
+        // grids of at most two chunks (one pass)
+        if (PB == 0)
+            cheb_phase_b<STRIDE, MODE, GEN>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k, cnt, scale, id, q, n_chunks, lane);
+        else
+            cheb_phase_b_split<STRIDE, MODE, GEN, (PB == 2 || PB == 4) ? 1 : 0, (PB >= 3), PIPE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k,
+                                                                                          fold, cnt, scale, id, q, n_chunks, lane);
     }
     reduce_finish(a, wr);
     hist_flush(sm_hist, a.hist, a.n_bins);

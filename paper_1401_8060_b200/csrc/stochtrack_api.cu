@@ -482,25 +482,52 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max, int* 
         }
         if (smem > (size_t)c->smem_optin)
             return fail(c, ST_ENOSPC, "n_f %d / n_max %d need more shared memory than one SM has", c->n_f, n_max);
+        // Phase B form (st_kernels.cuh): grids of two or more chunks take the delay-split form (two chunks per pass);
+        // which form runs is a property of the grid alone, so every build of the kernel (search, capture, per-template
+        // maximum, general, bank cache) sums a template's terms in the same order.  The default search of a grid of
+        // at most two chunks has a one-pass build, with the fold through shared memory when the scratch fits.
+        const int n_chunks = (a.n_tau + st::kCheb - 1) / st::kCheb;
+        const int pb = n_chunks >= 2 ? 1 : 0;
+        int pb_single = pb;
+        a.fold_offset = 0;
+        if (pb && n_chunks <= 2) {
+            pb_single = 3;
+            const size_t fold_off = (smem + 15) & ~(size_t)15;
+            const size_t with_fold = fold_off + (size_t)(threads / 32) * (size_t)st::kFoldWords * sizeof(float);
+            if (with_fold <= (size_t)c->smem_optin) { smem = with_fold; a.fold_offset = (uint32_t)fold_off; pb_single = 4; }
+        }
         const bool pk = plan.stride == 2;
         uint64_t blocks = (uint64_t)c->n_sm;            // persistent: one block per SM
         const uint64_t need = (want_warps + (uint64_t)(threads / 32) - 1) / (uint64_t)(threads / 32);
         if (blocks > need) blocks = need;
-#define ST_LAUNCH_CHEB(STRIDE, MODE, GEN, BANK)                                                   \
+#define ST_LAUNCH_CHEB(STRIDE, MODE, GEN, BANK, PB)                                               \
     do {                                                                                          \
-        int rc_ = set_smem(c, st::k_score_cheb<STRIDE, MODE, GEN, BANK>, smem);                   \
+        int rc_ = set_smem(c, st::k_score_cheb<STRIDE, MODE, GEN, BANK, PB>, smem);               \
         if (rc_) return rc_;                                                                      \
-        st::k_score_cheb<STRIDE, MODE, GEN, BANK><<<(unsigned)blocks, threads, smem, c->stream>>>(a); \
+        st::k_score_cheb<STRIDE, MODE, GEN, BANK, PB><<<(unsigned)blocks, threads, smem, c->stream>>>(a); \
+    } while (0)
+#define ST_LAUNCH_CHEB_FORM(STRIDE, MODE, GEN, BANK)                                              \
+    do {                                                                                          \
+        if (pb_ == 0) ST_LAUNCH_CHEB(STRIDE, MODE, GEN, BANK, 0);                                 \
+        else ST_LAUNCH_CHEB(STRIDE, MODE, GEN, BANK, 1);                                          \
+    } while (0)
+#define ST_LAUNCH_CHEB_SEARCH(STRIDE, BANK)                                                       \
+    do {                                                                                          \
+        if (pb_ == 3) ST_LAUNCH_CHEB(STRIDE, 0, false, BANK, 3);                                  \
+        else if (pb_ == 4) ST_LAUNCH_CHEB(STRIDE, 0, false, BANK, 4);                             \
+        else ST_LAUNCH_CHEB_FORM(STRIDE, 0, false, BANK);                                         \
     } while (0)
 #define ST_LAUNCH_CHEB_MODE(STRIDE, GEN)                                                          \
     do {                                                                                          \
-        if (mode == 1) ST_LAUNCH_CHEB(STRIDE, 1, GEN, 0);                                         \
-        else if (mode == 2) ST_LAUNCH_CHEB(STRIDE, 2, GEN, 0);                                    \
-        else if (!GEN && a.kcache_mode == 1) ST_LAUNCH_CHEB(STRIDE, 0, false, 1);                 \
-        else if (!GEN && a.kcache_mode == 2) ST_LAUNCH_CHEB(STRIDE, 0, false, 2);                 \
-        else ST_LAUNCH_CHEB(STRIDE, 0, GEN, 0);                                                   \
+        if (mode == 1) ST_LAUNCH_CHEB_FORM(STRIDE, 1, GEN, 0);                                    \
+        else if (mode == 2) ST_LAUNCH_CHEB_FORM(STRIDE, 2, GEN, 0);                               \
+        else if (GEN) ST_LAUNCH_CHEB_FORM(STRIDE, 0, true, 0);                                    \
+        else if (a.kcache_mode == 1) ST_LAUNCH_CHEB_SEARCH(STRIDE, 1);                            \
+        else if (a.kcache_mode == 2) ST_LAUNCH_CHEB_SEARCH(STRIDE, 2);                            \
+        else ST_LAUNCH_CHEB_SEARCH(STRIDE, 0);                                                    \
     } while (0)
         const int mode = a.capture_mode ? 1 : (a.tmax_snr ? 2 : 0);
+        int pb_ = pb_single;
         // the general build (cubic family, inverse-variance weighting, explicit templates) reads its options
         // at run time; the default search is compiled with them as constants
         const bool gen = a.bp.family != 0 || a.norm == 2 || a.tracks != nullptr;
@@ -520,6 +547,7 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max, int* 
             ST_CUDA(c, cudaGetLastError());
             ST_CUDA(c, cudaMemsetAsync(&a.sc->counter, 0, sizeof(unsigned long long), c->stream));
             a.defer_in = 1; a.defer_limit = 3.4e38f;
+            pb_ = pb;
             blocks = (uint64_t)c->n_sm;
             if (blocks > need) blocks = need;
             if (pk) ST_LAUNCH_CHEB_MODE(2, true); else ST_LAUNCH_CHEB_MODE(1, true);
@@ -527,6 +555,8 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max, int* 
             if (extra_launches) ++*extra_launches;
         }
 #undef ST_LAUNCH_CHEB_MODE
+#undef ST_LAUNCH_CHEB_SEARCH
+#undef ST_LAUNCH_CHEB_FORM
 #undef ST_LAUNCH_CHEB
     } else if (plan.kernel == ST_KERNEL_REINSCH) {
         int threads = c->recur_threads;
