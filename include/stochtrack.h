@@ -77,7 +77,10 @@ extern "C" {
 
 /* scoring kernel selection (grid mode).  AUTO picks CHEBYSHEV when the grid is
  * uniform and every bin's step angle is well conditioned, else REINSCH / ROTATION
- * when uniform, else TABLE.                                                     */
+ * when uniform, else TABLE.  A kernel asked for by name on a grid it cannot score
+ * within the 1e-4 contract (REINSCH / CHEBYSHEV: a bin's step angle 2 pi f dtau too
+ * close to 0 or pi; any recurrence kernel: a non-uniform grid) is refused with
+ * ST_EINVAL rather than run.                                                    */
 #define ST_KERNEL_AUTO     0
 #define ST_KERNEL_TABLE    1   /* twiddle table W[k][m] read from L2, any grid          */
 #define ST_KERNEL_ROTATION 2   /* complex rotation recurrence along a uniform tau grid  */

@@ -1277,7 +1277,9 @@ __device__ __forceinline__ void cheb_merge_init(ChebMergeState& m)
 {
     m.run_k = -1; m.n_a = 0; m.n_b = 0; m.ax = 0.0f; m.ay = 0.0f; m.run_e = make_float2(0.0f, 0.0f); m.w2 = 0.0f; m.bamp = 0.0f;
 }
-// Append the finished runs of the lanes flagged `emit` (warp-wide ballots keep the pool compact).  A pixel's
+// Append the finished runs of the lanes flagged `emit` (warp-wide ballots keep the pool compact); the rotation
+// to the anchor is written with explicit roundings (one multiply, one FMA per component), so every build of the
+// kernel forms bit-identical pool entries whatever the assembler would have contracted.  A pixel's
 // CLASS is a property of its bin, carried by the lowest mantissa bit of the anchor phase factor Ec[k].x the
 // host uploads: class A bins run the Chebyshev recurrence; in class B bins the float32 coefficient
 // 2 cos(S theta) would drift the phase by more than kChebClassDrift over half a chunk (small theta: fine grids,
@@ -1299,7 +1301,7 @@ __device__ __forceinline__ void cheb_emit(ChebMergeState& m, const bool emit, fl
         if (emit) {
             const uint32_t below = (1u << lane) - 1u;
             const int e = cls_b ? S - 1 - (m.n_b + __popc(em_b & below)) : m.n_a + __popc(em_a & below);
-            pool_v[e] = make_float2(m.ax * m.run_e.x - m.ay * m.run_e.y, m.ax * m.run_e.y + m.ay * m.run_e.x);
+            pool_v[e] = make_float2(fmaf(m.ax, m.run_e.x, -__fmul_rn(m.ay, m.run_e.y)), fmaf(m.ax, m.run_e.y, __fmul_rn(m.ay, m.run_e.x)));
             pool_k[e] = (uint16_t)m.run_k;
         }
         m.n_a += __popc(em_a);
@@ -1308,7 +1310,7 @@ __device__ __forceinline__ void cheb_emit(ChebMergeState& m, const bool emit, fl
         const uint32_t em = __ballot_sync(kFull, emit);
         if (emit) {
             const int e = m.n_a + __popc(em & ((1u << lane) - 1u));
-            pool_v[e] = make_float2(m.ax * m.run_e.x - m.ay * m.run_e.y, m.ax * m.run_e.y + m.ay * m.run_e.x);
+            pool_v[e] = make_float2(fmaf(m.ax, m.run_e.x, -__fmul_rn(m.ay, m.run_e.y)), fmaf(m.ax, m.run_e.y, __fmul_rn(m.ay, m.run_e.x)));
             pool_k[e] = (uint16_t)m.run_k;
             if (cls_b) m.bamp += fabsf(m.ax) + fabsf(m.ay);
         }

@@ -345,6 +345,8 @@ int make_plan(st_ctx* c, const st_search_params* p, Plan* plan)
     }
     if ((k == ST_KERNEL_ROTATION || k == ST_KERNEL_REINSCH || k == ST_KERNEL_CHEBYSHEV) && !uni)
         return fail(c, ST_EINVAL, "recurrence kernels need a uniform tau grid");
+    if (k == ST_KERNEL_REINSCH && p->kernel == ST_KERNEL_REINSCH && !reinsch_well_conditioned(c, plan->dtau))
+        return fail(c, ST_EINVAL, "the Reinsch kernel is ill conditioned on this delay grid (a bin's step angle is within 0.1 rad of pi)");
     plan->kernel = k;
     if (k == ST_KERNEL_ROTATION) plan->ch = pick_chunk(p->n_tau);
     if (k == ST_KERNEL_REINSCH) plan->ch = st::kChunk;
@@ -490,6 +492,15 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max, int* 
         const int pb = n_chunks >= 2 ? 1 : 0;
         int pb_single = pb;
         a.fold_offset = 0;
+        // the one-pass search build is compiled for ST_CHEB_PIPE_THREADS threads (12 warps at 168 registers:
+        // its phase B is software-pipelined, see cheb_phase_b_split)
+        const bool one_pass_search = pb && n_chunks <= 2 && !a.capture_mode && !a.tmax_snr &&
+                                     a.bp.family == 0 && a.norm != 2 && a.tracks == nullptr;
+        if (one_pass_search && threads > ST_CHEB_PIPE_THREADS) {
+            threads = ST_CHEB_PIPE_THREADS;
+            smem = hist_bytes(a.n_bins) + (size_t)c->n_f * sizeof(float4) + (size_t)((c->n_f + 1) & ~1) * sizeof(float) +
+                   (size_t)(threads / 32) * (size_t)cstride * (sizeof(float2) + sizeof(uint16_t));
+        }
         if (pb && n_chunks <= 2) {
             pb_single = 3;
             const size_t fold_off = (smem + 15) & ~(size_t)15;
@@ -511,10 +522,16 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max, int* 
         if (pb_ == 0) ST_LAUNCH_CHEB(STRIDE, MODE, GEN, BANK, 0);                                 \
         else ST_LAUNCH_CHEB(STRIDE, MODE, GEN, BANK, 1);                                          \
     } while (0)
+#define ST_LAUNCH_CHEB_PIPE(STRIDE, BANK, PB)                                                     \
+    do {                                                                                          \
+        int rc_ = set_smem(c, st::k_score_cheb<STRIDE, 0, false, BANK, PB, true>, smem);          \
+        if (rc_) return rc_;                                                                      \
+        st::k_score_cheb<STRIDE, 0, false, BANK, PB, true><<<(unsigned)blocks, threads, smem, c->stream>>>(a); \
+    } while (0)
 #define ST_LAUNCH_CHEB_SEARCH(STRIDE, BANK)                                                       \
     do {                                                                                          \
-        if (pb_ == 3) ST_LAUNCH_CHEB(STRIDE, 0, false, BANK, 3);                                  \
-        else if (pb_ == 4) ST_LAUNCH_CHEB(STRIDE, 0, false, BANK, 4);                             \
+        if (pb_ == 3) ST_LAUNCH_CHEB_PIPE(STRIDE, BANK, 3);                                       \
+        else if (pb_ == 4) ST_LAUNCH_CHEB_PIPE(STRIDE, BANK, 4);                                  \
         else ST_LAUNCH_CHEB_FORM(STRIDE, 0, false, BANK);                                         \
     } while (0)
 #define ST_LAUNCH_CHEB_MODE(STRIDE, GEN)                                                          \
@@ -556,6 +573,7 @@ int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max, int* 
         }
 #undef ST_LAUNCH_CHEB_MODE
 #undef ST_LAUNCH_CHEB_SEARCH
+#undef ST_LAUNCH_CHEB_PIPE
 #undef ST_LAUNCH_CHEB_FORM
 #undef ST_LAUNCH_CHEB
     } else if (plan.kernel == ST_KERNEL_REINSCH) {

@@ -99,17 +99,19 @@ def test_scores_grid_kernels_vs_oracle(P, orc, kname, cid, count):
 
 
 @pytest.mark.parametrize("kname", ["table", "rotation", "reinsch", "chebyshev"])
-@pytest.mark.parametrize("n_tau", [1, 7, 33, 50, 128, 200, 600])
+@pytest.mark.parametrize("n_tau", [1, 7, 33, 50, 100, 128, 150, 200, 300, 600])
 def test_scores_ragged_tau_counts(P, orc, kname, n_tau):
     """Grid sizes that are not multiples of the 32/64-delay chunks, on the config-5 shape
-    with per-pixel sigma (several 32-column rows and a ragged tail per track)."""
+    with per-pixel sigma (several 32-column rows and a ragged tail per track).  For the Chebyshev kernel the
+    counts cover every form of its phase B: one chunk (1, 7, 33, 50), the one-pass delay-split build (100, 128),
+    odd chunk counts whose last pass leaves one half-warp idle (150: 3, 300: 5) and even ones (200: 4, 600: 10)."""
     cfg = synth.CONFIGS[5]
     try:
         got, ref = _score_case(P, orc, cfg, KERNELS[kname], 300, first=12345, n_tau=n_tau)
     except P.StError as e:
-        # coarse grids alias some bins onto theta ~ 0 or pi: the Chebyshev kernel refuses them
+        # coarse grids alias some bins onto theta ~ 0 or pi: the Chebyshev and Reinsch kernels refuse them
         # (ST_EINVAL) rather than lose accuracy; AUTO must then pick another kernel and still agree
-        assert kname == "chebyshev" and e.code == -1 and n_tau in (7, 33, 50)
+        assert kname in ("chebyshev", "reinsch") and e.code == -1 and n_tau in (7, 33, 50, 100)
         got, ref = _score_case(P, orc, cfg, 0, 300, first=12345, n_tau=n_tau)
     ok, worst = snr_close(got, ref)
     assert ok, f"{kname} n_tau {n_tau}: worst error {worst:.3f} x tolerance"
@@ -754,7 +756,8 @@ def test_patch_of_sky_delay_prior(P, orc):
 @pytest.mark.parametrize("cid,n,first,n_tau,kname", [(1, 1000, 0, None, "auto"), (2, 20_000, 50_000, None, "auto"),
                                                       (2, 3000, 0, None, "table"), (2, 3000, 0, None, "rotation"),
                                                       (2, 3000, 0, None, "reinsch"), (5, 2000, 9_000_000, None, "auto"),
-                                                      (5, 500, 0, 200, "auto"), (3, 20_000, 0, None, "auto")])
+                                                      (5, 500, 0, 200, "auto"), (3, 20_000, 0, None, "auto"),
+                                                      (5, 600, 77, 128, "auto"), (5, 600, 77, 100, "auto"), (5, 400, 5, 300, "auto")])
 def test_per_template_maximum_over_delays(P, orc, cid, n, first, n_tau, kname):
     """st_search_track_max: for every template its best delay and SNR, computed in the
     fused epilogue.  Values within G13 of the oracle's row maximum; the index is decided in float32 (G24), so
