@@ -254,9 +254,8 @@ __device__ __forceinline__ void reduce_samples(const ScoreArgs& a, WarpReduce& w
             if (a.dump) a.dump[q * (uint64_t)a.n_tau + m[i]] = v[i];
         }
     }
-    float wmax = lmax;
-#pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) wmax = fmaxf(wmax, __shfl_xor_sync(kFull, wmax, off));
+    // warp maximum through the order-preserving integer encoding: one REDUX instead of five shuffle + max steps
+    const float wmax = dec_f32(__reduce_max_sync(kFull, enc_f32(lmax)));
     if (wmax >= wr.cached_max - near_margin(wr.cached_max)) {
         // slow path: this template comes within the margin of the global maximum
         const int lane = threadIdx.x & 31;
@@ -1385,10 +1384,10 @@ __device__ __forceinline__ ChebCounts cheb_phase_a(const ScoreArgs& a, const Tra
     const ChebCounts cnt = cheb_merge_finish<GEN>(m, pool_v, pool_k, lane, S);
     defer = false;
     if (!GEN && a.defer_limit < 3.0e38f) {             // the grid has class B bins (warp-uniform)
-        float b = m.bamp;
-#pragma unroll
-        for (int off = 16; off >= 1; off >>= 1) b += __shfl_xor_sync(kFull, b, off);
-        defer = b * scale > a.defer_limit;
+        // warp sum in fixed point (1 / 1024, every lane rounded up: never below the float sum) through one REDUX
+        // instead of five dependent shuffle + add steps
+        const uint32_t bq = __reduce_add_sync(kFull, __float2uint_ru(fminf(m.bamp, 3.0e4f) * 1024.0f));
+        defer = (float)bq * (scale * (1.0f / 1024.0f)) > a.defer_limit;
     }
     return cnt;
 }
