@@ -321,12 +321,28 @@ __device__ __forceinline__ void hist_flush(uint32_t* sm_hist, unsigned long long
     }
 }
 
+// The template counter's fetch-and-add.  An integer atomic (atomicAdd(), or atom.global.add.u64 in PTX) under
+// `if (lane == 0)` gets the assembler's warp-aggregation pattern -- leader atomic, then a SHFL of the result to
+// the active lanes -- and that shuffle waits for the L2 round trip on the spot (~500 clocks per template in the
+// profile; issuing the atomic "one template ahead" hid nothing).  A float64 atomic is not aggregated: the counter
+// is kept as a double (exact below 2^53; the all-zero bit pattern the host writes is 0.0), the raw result stays
+// pending in a register and is converted at its first use, one template later (claim_value).
+__device__ __forceinline__ unsigned long long claim_add(unsigned long long* counter, unsigned long long n)
+{
+    unsigned long long old;
+    asm volatile("atom.global.add.f64 %0, [%1], %2;" : "=l"(old) : "l"(counter), "d"((double)n) : "memory");
+    return old;                                         // bits of the previous count as a double
+}
+__device__ __forceinline__ uint64_t claim_value(unsigned long long bits)
+{
+    return (uint64_t)__double2ll_rn(__longlong_as_double((long long)bits));
+}
 // Next template of the launch for this warp (dynamic: durations vary 100x).
 __device__ __forceinline__ uint64_t next_track(const ScoreArgs& a)
 {
     unsigned long long q = 0;
-    if ((threadIdx.x & 31) == 0) q = atomicAdd(&a.sc->counter, 1ull);
-    return __shfl_sync(kFull, q, 0);
+    if ((threadIdx.x & 31) == 0) q = claim_add(&a.sc->counter, 1ull);
+    return claim_value(__shfl_sync(kFull, q, 0));
 }
 
 __device__ __forceinline__ uint32_t hist_smem_words(int n_bins) { return (uint32_t)((n_bins + 3) & ~3); }
@@ -619,11 +635,11 @@ __global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(cons
     reduce_init(wr);
     // kRandPerWarp templates are claimed per atomic, one claim ahead (the result waits in lane 0)
     unsigned long long q_pref = 0;
-    if (lane == 0) q_pref = atomicAdd(&a.sc->counter, (unsigned long long)kRandPerWarp);
+    if (lane == 0) q_pref = claim_add(&a.sc->counter, (unsigned long long)kRandPerWarp);
     for (;;) {
-        const uint64_t q0 = __shfl_sync(kFull, q_pref, 0);
+        const uint64_t q0 = claim_value(__shfl_sync(kFull, q_pref, 0));
         if (q0 >= a.n_tracks) break;
-        if (lane == 0) q_pref = atomicAdd(&a.sc->counter, (unsigned long long)kRandPerWarp);
+        if (lane == 0) q_pref = claim_add(&a.sc->counter, (unsigned long long)kRandPerWarp);
         const uint64_t q = q0 + (uint64_t)grp;
         const bool live = q < a.n_tracks;                    // the last claim may be ragged
         const uint64_t id = a.track_offset + (live ? q : q0);
@@ -1885,15 +1901,15 @@ __global__ void __launch_bounds__(PIPE ? ST_CHEB_PIPE_THREADS : ST_CHEB_MAX_THRE
     // the template counter's L2 atomic (~1 us round trip) is issued one template ahead; its result
     // stays in lane 0 until the next iteration broadcasts it
     unsigned long long q_pref = 0;
-    if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
+    if (lane == 0) q_pref = claim_add(&a.sc->counter, 1ull);
     // a launch works through its own id range, or (general build, defer_in) through the list of templates the
     // fast build handed over: the list is complete, the fast launch precedes this one on the stream
     const uint64_t n_items = (GEN && a.defer_in) ? (uint64_t)min(a.sc->n_deferred, a.deferred_cap) : a.n_tracks;
     if (GEN && a.defer_in && blockIdx.x == 0 && threadIdx.x == 0) a.sc->n_deferred_total += (uint32_t)n_items;
     for (;;) {
-        const uint64_t item = __shfl_sync(kFull, q_pref, 0);
+        const uint64_t item = claim_value(__shfl_sync(kFull, q_pref, 0));
         if (item >= n_items) break;
-        if (lane == 0) q_pref = atomicAdd(&a.sc->counter, 1ull);
+        if (lane == 0) q_pref = claim_add(&a.sc->counter, 1ull);
         const uint64_t q = (GEN && a.defer_in) ? (uint64_t)a.deferred[item] : item;
         const uint64_t id = a.track_offset + q;
         Track t;
