@@ -32,9 +32,12 @@ METRIC = "track_pixel_evals_per_s"
 UNIT = "evals/s"
 N_SM, FP32_LANES = 148, 128           # B200: 148 SMs x 128 FP32 lanes (B200_PROFILING.md, blackwell guide)
 FLOP_PER_EVAL = 4                     # Eq. 8 needs 2 FMA per (pixel, delay) once the phase factor is known
-# dram__bytes_read.sum + dram__bytes_write.sum of k_score_cheb from the ncu --set full capture in
-# profiles/r01_kernels.md (config 5: the 19.69 MB map is read from HBM once, then served by L2)
-DRAM_TRAFFIC_BYTES_PER_LAUNCH = {5: 19.87e6, 3: 9.88e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the `ncu --set full` capture
+# named beside it (profiles/; the command is in the file's first line).  The map is read from HBM once per launch
+# and then served by L2; a config without a capture reports null.
+DRAM_TRAFFIC = {5: (19.85e6, "profiles/r02_ncu_cheb_c5.txt"),      # algorithmic: the 19.69 MB map once
+                4: (9.97e6, "profiles/r02_ncu_cheb_c4.txt"),       # per map of the batch: the 9.84 MB map once
+                3: (9.88e6, "profiles/r02_ncu_random.txt")}
 L2_GATHER_PEAK_GBS = 9200.0          # random 32-byte sector gathers, measured (profiles/microbench_r01.md)
 
 
@@ -140,7 +143,7 @@ def run_ours(args):
                 others.append({"config": o["config"]["workload"], "value": o["value"], "unit": o["unit"], "ms_per_step": o["ms_per_step"],
                                "steps": o["steps"], "warmup": o["warmup"], "tracks_tau_per_s": o["tracks_tau_per_s"],
                                "e2e_value": o["e2e"]["value"], "gpu_launches": o["gpu_launches"], "clocks": o["clocks"],
-                               "roofline": {k: o["roofline"][k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac")}})
+                               "roofline": {k: o["roofline"][k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic")}})
             line["other_configs"] = others
         print(json.dumps(line))
     if dist is not None:
@@ -278,7 +281,8 @@ def measure(args, env):
         "clocks": clocks,
         "roofline": {"bound": "alu", "kernel": {"chebyshev": "k_score_cheb", "reinsch": "k_score_reinsch", "rotation": "k_score_recur",
                                                 "table": "k_score_table", "random": "k_score_random"}.get(r.kernel_name, r.kernel_name), "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": DRAM_TRAFFIC.get(args.config, (None, None))[0],
+                     "traffic_from": DRAM_TRAFFIC.get(args.config, (None, None))[1],
                      "peak_how": peak_how + "; algorithmic 4 flop per track-pixel evaluation (DESIGN.md)"},
         "result": {"max_snr": combined["max_snr_f64"], "arg_track": combined["arg_track"],
                    "arg_tau_index": combined["arg_tau_index"], "n_deferred_last_step": int(r.n_deferred)},
