@@ -19,7 +19,7 @@ import paper_1401_8060_b200 as P
 P.load_library(%(lib)r)
 from workloads import synth
 out = {}
-for cid, n in ((1, 1000), (2, 20000), (3, 30000), (5, 3000)):
+for cid, n in ((1, 1000), (2, 20000), (3, 30000), (4, 20000), (5, 3000)):
     cfg = synth.CONFIGS[cid]
     st = P.Stochtrack(cfg.n_t, cfg.n_f, cfg.df, cfg.f_min, max_n_tau=max(cfg.n_tau, 64))
     csd = synth.noise_csd(cfg.n_t, cfg.n_f, 40 + cid)
@@ -34,6 +34,13 @@ for cid, n in ((1, 1000), (2, 20000), (3, 30000), (5, 3000)):
     kw = dict(tau_grid=tau) if tau is not None else dict(tau_range=(-0.01, 0.01))
     r, top = st.search_topk(7, n, 7, cfg.n_min, cfg.n_max, n_bins=400, **kw)
     out["c%%d_top" %% cid] = [[e["track"], e["tau_index"], e["snr_f64"]] for e in top]
+    if cid in (4, 5):      # the delay-split builds: per-template maximum, and the bank cache filled then read
+        r, vmax, imax = st.search_track_max(n, 7, cfg.n_min, cfg.n_max, n_bins=200, **kw)
+        out["c%%d_tmax" %% cid] = [float(vmax.max()), int(imax.sum()), r.arg_track]
+        st.enable_bank_cache(n, cfg.n_max)
+        for rep in range(2):
+            r = st.search(n, 7, cfg.n_min, cfg.n_max, n_bins=200, **kw)
+            out["c%%d_bank%%d" %% (cid, rep)] = [r.max_snr_f64, r.arg_track, r.arg_tau_index, int(r.hist.sum()), int(r.flags)]
     if cid == 1:
         res, _ = st.search_batch([torch.from_numpy(csd).cuda()] * 3, None, [1, 2, 3], 500, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=50)
         out["batch"] = [[x.max_snr_f64, x.arg_track] for x in res]
@@ -58,4 +65,4 @@ def test_checked_build_trips_no_assertion_and_matches_production():
     got = _run(checked)
     want = _run(build.LIB)
     assert got == want
-    assert len(got) >= 12
+    assert len(got) >= 24
