@@ -1295,21 +1295,23 @@ __device__ __forceinline__ void cheb_merge_init(ChebMergeState& m)
 // Append the finished runs of the lanes flagged `emit` (warp-wide ballots keep the pool compact); the rotation
 // to the anchor is written with explicit roundings (one multiply, one FMA per component), so every build of the
 // kernel forms bit-identical pool entries whatever the assembler would have contracted.  A pixel's
-// CLASS is a property of its bin, carried by the lowest mantissa bit of the anchor phase factor Ec[k].x the
-// host uploads: class A bins run the Chebyshev recurrence; in class B bins the float32 coefficient
+// CLASS is a property of its bin, carried by the two lowest mantissa bits of the anchor phase factor Ec[k].x the
+// host uploads (0 = class A; 1, 2, 3 = class B with a drift of at most d_max / 4, d_max / 2, d_max): class A bins run the Chebyshev recurrence; in class B bins the float32 coefficient
 // 2 cos(S theta) would drift the phase by more than kChebClassDrift over half a chunk (small theta: fine grids,
 // low frequencies), which mis-scores a loud coherent signal where SNR(tau) crosses zero.
 //   TWO = true (the general build): class A fills the pool from the front, class B from the back (entries
 //     S-1, S-2, ...) and is advanced by Reinsch's form, whose coefficient 4 sin^2(theta/2) keeps its relative
 //     precision as theta -> 0;
 //   TWO = false (the fast build): one pool; the amplitude |Re v| + |Im v| >= |v| parked in class B bins is
-//     summed, and a template whose worst-case drift error  d_max * scale * sum_B |v|  could reach a fraction of
-//     the G13 tolerance is not scored here but handed to the general build (cheb_defer).
+//     summed, weighted by the bin's drift level, and a template whose worst-case drift error
+//     scale * sum_B d_k |v|  (d_k rounded up to d_max / 4, / 2 or d_max) could reach a fraction of the G13
+//     tolerance is not scored here but handed to the general build (cheb_defer).
 template <bool TWO>
 __device__ __forceinline__ void cheb_emit(ChebMergeState& m, const bool emit, float2* pool_v, uint16_t* pool_k, const int lane,
                                           const int S)
 {
-    const bool cls_b = (__float_as_uint(m.run_e.x) & 1u) != 0u;
+    const uint32_t level = __float_as_uint(m.run_e.x) & 3u;         // 0: class A; 1-3: class B, drift <= d_max / 4, / 2, d_max
+    const bool cls_b = level != 0u;
     if (TWO) {
         const uint32_t em_a = __ballot_sync(kFull, emit && !cls_b);
         const uint32_t em_b = __ballot_sync(kFull, emit && cls_b);
@@ -1327,7 +1329,7 @@ __device__ __forceinline__ void cheb_emit(ChebMergeState& m, const bool emit, fl
             const int e = m.n_a + __popc(em & ((1u << lane) - 1u));
             pool_v[e] = make_float2(fmaf(m.ax, m.run_e.x, -__fmul_rn(m.ay, m.run_e.y)), fmaf(m.ax, m.run_e.y, __fmul_rn(m.ay, m.run_e.x)));
             pool_k[e] = (uint16_t)m.run_k;
-            if (cls_b) m.bamp += fabsf(m.ax) + fabsf(m.ay);
+            if (cls_b) m.bamp = fmaf(fabsf(m.ax) + fabsf(m.ay), __uint_as_float((124u + level) << 23), m.bamp);   // x 2^(level - 3)
         }
         m.n_a += __popc(em);
     }

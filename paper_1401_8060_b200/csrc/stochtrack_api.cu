@@ -227,7 +227,8 @@ int build_cheb_tables(const st_ctx* c, double tau0, double dtau, int stride, std
     const int n_f = c->n_f;
     if (out) out->assign((size_t)n_f * 7, 0.0f);
     int n_class_b = 0;
-    if (d_max) *d_max = 0.0;
+    double dmax = 0.0;
+    std::vector<double> drift((size_t)n_f, 0.0);        // class B bins: their drift over half a chunk (0 = class A)
     for (int k = 0; k < n_f; ++k) {
         const double f = c->f_min + (double)k * c->df;
         double cyc = f * dtau;
@@ -239,14 +240,14 @@ int build_cheb_tables(const st_ctx* c, double tau0, double dtau, int stride, std
         double half = 0.5 * (double)G;
         half = half > 1.0 ? 1.0 : (half < -1.0 ? -1.0 : half);
         const double drift_a = (32.0 / (double)stride) * fabs(acos(half) - fabs(sth));
-        bool class_b = false;
         if (drift_a > kChebClassDrift) {
             // Reinsch's form at stride 1 with kappa = 2 sin^2 theta / (1 + cos theta) formed in float32 from the
             // table's (cos theta, sin theta): relative error <= 3e-7, i.e. <= 32 x 1.5e-7 |theta| rad of drift
             const double drift_b = 4.8e-6 * fabs(theta);
             if (drift_b > kChebClassDrift) return -1;
-            class_b = true; ++n_class_b;
-            if (d_max && drift_a > *d_max) *d_max = drift_a;
+            ++n_class_b;
+            drift[(size_t)k] = drift_a;
+            if (drift_a > dmax) dmax = drift_a;
         }
         if (out) {
             double c64 = cyc * 64.0;
@@ -257,11 +258,22 @@ int build_cheb_tables(const st_ctx* c, double tau0, double dtau, int stride, std
             t4[0] = G; t4[1] = (float)cos(theta); t4[2] = (float)sin(theta); t4[3] = (float)cos(st::kTwoPi * c64);
             float* ec = out->data() + (size_t)n_f * 4 + (size_t)k * 2;
             ec[0] = (float)cos(st::kTwoPi * c0); ec[1] = (float)sin(st::kTwoPi * c0);
-            uint32_t bits;                                  // the class rides in the lowest mantissa bit of Ec.x
-            memcpy(&bits, &ec[0], sizeof(bits));
-            bits = (bits & ~1u) | (class_b ? 1u : 0u);
-            memcpy(&ec[0], &bits, sizeof(bits));
             (*out)[(size_t)n_f * 6 + (size_t)k] = (float)sin(st::kTwoPi * c64);
+        }
+    }
+    if (d_max) *d_max = dmax;
+    if (out) {
+        // The class rides in the two lowest mantissa bits of Ec.x: 0 = class A; 1, 2, 3 = class B with a drift of at most
+        // d_max / 4, d_max / 2, d_max: the fast build weighs a pixel's amplitude by 2^(level - 3) x 2 in its bound of
+        // the drift error, so the many mildly drifting bins do not count as the worst one.
+        for (int k = 0; k < n_f; ++k) {
+            float* ec = out->data() + (size_t)n_f * 4 + (size_t)k * 2;
+            const double d = drift[(size_t)k];
+            const uint32_t level = d == 0.0 ? 0u : (d <= 0.25 * dmax ? 1u : (d <= 0.5 * dmax ? 2u : 3u));
+            uint32_t bits;
+            memcpy(&bits, &ec[0], sizeof(bits));
+            bits = (bits & ~3u) | level;
+            memcpy(&ec[0], &bits, sizeof(bits));
         }
     }
     return n_class_b;
