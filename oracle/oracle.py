@@ -95,7 +95,7 @@ def _p(a, ctype):
 
 
 NORM_SQRT_N, NORM_MEAN, NORM_INVVAR = 0, 1, 2
-FAMILY_QUADRATIC, FAMILY_CUBIC = 0, 1
+FAMILY_QUADRATIC, FAMILY_CUBIC, FAMILY_CHIRP = 0, 1, 2
 TAU_GRID, TAU_RANDOM = 0, 1
 
 
@@ -124,8 +124,11 @@ def track_params(seed, track_id, n_t, n_f, n_min, n_max, tau_lo=0.0, tau_hi=0.0,
     return t
 
 
-def make_track(N, j0, a, y0, y1, y2, tau=0.0, y3=None):
-    """A quadratic template (Eq. 6), or with y3 a cubic one: frequency control points y0, y1, y2, y3 (G26)."""
+def make_track(N, j0, a, y0, y1, y2, tau=0.0, y3=None, family=None):
+    """A quadratic template (Eq. 6), or with y3 a cubic one: frequency control points y0, y1, y2, y3 (G26);
+    family=FAMILY_CHIRP: the chirp-law template of G27 (N, j0, a, y0 are used)."""
+    if family == FAMILY_CHIRP:
+        return Track(int(N), int(j0), float(a), float(y0), float(y1), float(y2), float(tau), 0.0, FAMILY_CHIRP)
     if y3 is None:
         return Track(int(N), int(j0), float(a), float(y0), float(y1), float(y2), float(tau), 0.0, FAMILY_QUADRATIC)
     return Track(int(N), int(j0), float(a), float(y0), float(y1), float(y2), float(tau), float(y3), FAMILY_CUBIC)
@@ -224,7 +227,7 @@ def search(p, f_min, df, n_tracks, seed, n_min, n_max, tau_grid=None, tau_range=
     """Whole path O1-O5 for ids [track_offset, track_offset + n_tracks).
 
     tau_grid (array) selects grid mode; tau_range=(lo, hi) selects the paper's
-    random-tau mode.  family selects the template family (G26); norm=NORM_INVVAR
+    random-tau mode.  family selects the template family (G26, G27); norm=NORM_INVVAR
     the inverse-variance weighting (G25) and then needs inv_sigma = prepare_inv_sigma(...).
     Returns a dict.
     """

@@ -23,6 +23,7 @@
  * Variants (readings G25, G26 of DESIGN.md):
  *   O4w inverse-variance weighting of SNR_tot (fn. 23): norm_mode 2
  *   O2c/O3c the cubic template family (PAPER.md:75 "other parameterizable curves", :246-252, :287)
+ *   O2k/O3k the chirp-law template family f ~ (t_c - t)^(-3/8) (reading G27)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"):
  *   or_philox4x32_10 : cuRAND host generator CURAND_RNG_PSEUDO_PHILOX4_32_10 (P1)
@@ -44,6 +45,9 @@
  *   or_score_*_w     : reduction to the sqrt(N) statistic for constant sigma, a two-pixel closed
  *                      form, optimality against random weightings, masked pixels dropping out,
  *                      unit null variance under strongly varying sigma (tests/test_oracle_variants.py)
+ *   chirp family     : 60-digit decimal evaluation of y0 (T_c / (T_c - u))^(3/8), f^(-8/3) linear in time,
+ *                      the closed form f_end = 8 f_start at a = N / 256, monotone pixels, the band clamp,
+ *                      self-recovery of an injected bank member (tests/test_oracle_variants.py)
  *   cubic family     : 60-digit decimal brute force of the cubic Bernstein form, end points, convex
  *                      hull, the degree-elevated quadratic reproducing the quadratic family's pixels,
  *                      uniformity / independence of the fourth control point (same file)
@@ -104,7 +108,7 @@ typedef struct {
     double  y0, y1, y2; /* f_start, f_mid, f_end in bin units, bin k covers [k, k+1)    */
     double  tau;     /* the track's own delay (random-tau mode); else 0    */
     double  y3;      /* cubic family only: f_end; then y1, y2 are the two inner control points */
-    int32_t family;  /* 0 quadratic Bezier (Eq. 6), 1 cubic in frequency (G26)          */
+    int32_t family;  /* 0 quadratic Bezier (Eq. 6), 1 cubic in frequency (G26), 2 chirp law (G27) */
 } or_track;
 
 /* O2: "each template can be quickly generated from just six random numbers"
@@ -148,9 +152,18 @@ int or_track_params_family(uint64_t seed, uint64_t id, int32_t n_t, int32_t n_f,
                            int32_t n_min, int32_t n_max, double tau_lo, double tau_hi,
                            int32_t family, or_track *t)
 {
-    if (family != 0 && family != 1) return -1;
+    if (family != 0 && family != 1 && family != 2) return -1;
     int rc = or_track_params(seed, id, n_t, n_f, n_min, n_max, tau_lo, tau_hi, t);
     if (rc != 0 || family == 0) return rc;
+    if (family == 2) {
+        /* O2k (G27): the chirp-law family.  A compact-binary inspiral sweeps as f ~ (t_c - t)^(-3/8) (the signal of
+         * PAPER.md:252 and Fig. 2, which a quadratic "does not describe especially well"): the track is
+         * f(u) = y0 (T_c / (T_c - u))^(3/8) from its first column on.  N, j0, y0 (the frequency at the start) and tau
+         * are O2's; the time to coalescence from the start is T_c = N^2 / (N - a) > N with O2's a, so that the
+         * fraction of T_c left at the track's end, a / N, is uniform in (0, 1).  y1, y2 are not used.            */
+        t->family = 2;
+        return 0;
+    }
     uint32_t r[8];
     or_track_words(seed, id, r);
     t->family = 1;
@@ -170,6 +183,30 @@ void or_rasterise(const or_track *t, int32_t n_f, int32_t *k_out)
     const double a  = t->a;
     const double cc = (double)t->N - 2.0 * a;
     const double aa = a * a;
+    if (t->family == 2) {
+        /* O3k (G27): y(u) = y0 r^(3/8), r = T_c / (T_c - u) = N^2 / (N^2 - u (N - a)), at the column centre u = c + 1/2;
+         * r^(1/8) by three square roots.  NORMATIVE order, every operation a single correctly rounded double op
+         * (sqrt and division are; pow is not, so it is not used).                                              */
+        const double nn = (double)t->N * (double)t->N;      /* exact: N < 2^26 */
+        const double w  = (double)t->N - a;
+        for (int32_t c = 0; c < t->N; ++c) {
+            double u  = (double)c + 0.5;
+            double m  = u * w;
+            double D  = nn - m;                              /* > 0: u < N, w < N */
+            double r  = nn / D;
+            double s  = sqrt(sqrt(sqrt(r)));
+            double s2 = s * s;
+            double s3 = s2 * s;
+            double y  = s3 * t->y0;
+            double fl = floor(y);
+            int32_t k;
+            if (!(fl >= 0.0)) k = 0;
+            else if (fl > (double)(n_f - 1)) k = n_f - 1;
+            else k = (int32_t)fl;
+            k_out[c] = k;
+        }
+        return;
+    }
     for (int32_t c = 0; c < t->N; ++c) {
         double u   = (double)c + 0.5;
         double D   = aa + cc * u;
@@ -356,7 +393,7 @@ typedef struct {
     double   hist_lo, hist_hi;
     int32_t  score_mode;      /* 0 table, 1 direct (grid mode only; random is direct) */
     int32_t  n_threads;       /* OpenMP threads; <= 0 = library default              */
-    int32_t  family;          /* 0 quadratic, 1 cubic templates (O2c / O3c)          */
+    int32_t  family;          /* 0 quadratic, 1 cubic (O2c / O3c), 2 chirp-law templates (O2k / O3k) */
     int32_t  pad;
 } or_search_params;
 
@@ -382,7 +419,7 @@ int or_search(const double *p, int32_t n_t, int32_t n_f, double f_min, double df
     const int32_t n_tau = sp->tau_mode == 0 ? sp->n_tau : 1;
     if (n_tau < 1) return -1;
     if (sp->norm_mode == 2 && !inv_sigma) return -1;
-    if (sp->family != 0 && sp->family != 1) return -1;
+    if (sp->family != 0 && sp->family != 1 && sp->family != 2) return -1;
     if (sp->n_min < 1 || sp->n_max < sp->n_min || sp->n_max > n_t) return -1;
     double *W = NULL;
     if (sp->tau_mode == 0 && sp->score_mode == 0) {

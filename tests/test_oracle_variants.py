@@ -3,6 +3,7 @@ fix -- none of these tests touches the CUDA path.
 
   O4w  inverse-variance weighting of SNR_tot (fn. 23; Appendix A; reading G25)
   O2c / O3c  the cubic template family (reading G26)
+  O2k / O3k  the chirp-law template family f ~ (t_c - t)^(-3/8) (reading G27)
 """
 from decimal import Decimal, getcontext
 
@@ -235,3 +236,85 @@ def test_cubic_search_path(orc):
     assert np.array_equal(r["k"][i_star, :t.N], k) and (r["k"][i_star, t.N:] == -1).all()
     rq = orc.search(p, cfg.f_min, cfg.df, 1000, cfg.seed, 8, 64, tau_grid=taus)
     assert rq["max_snr"] < r["max_snr"]
+
+
+# ------------------------------------------------------------------------------------- O2k / O3k: chirp-law family (G27)
+def _decimal_chirp(t, n_f):
+    """y(u) = y0 (T_c / (T_c - u))^(3/8), T_c = N^2 / (N - a), in 60-digit arithmetic, written differently from the
+    oracle (the power through ln / exp, T_c formed explicitly)."""
+    getcontext().prec = 60
+    N, a, y0 = Decimal(t.N), Decimal(t.a), Decimal(t.y0)
+    t_c = N * N / (N - a)
+    ks, ys = [], []
+    for c in range(t.N):
+        u = Decimal(c) + Decimal("0.5")
+        y = y0 * ((t_c / (t_c - u)).ln() * Decimal(3) / Decimal(8)).exp()
+        ys.append(y)
+        ks.append(min(max(int(y.to_integral_value(rounding="ROUND_FLOOR")), 0), n_f - 1))
+    return ks, ys
+
+
+def test_chirp_rasteriser_vs_60_digit_brute_force(orc):
+    n_pix = n_mis = 0
+    for seed, n_t, n_f, n_min, n_max, count in ((4, 1000, 2461, 10, 1000, 60), (1, 250, 961, 10, 250, 150), (0, 64, 64, 64, 64, 100)):
+        for tid in range(count):
+            t = orc.track_params(seed, tid, n_t, n_f, n_min, n_max, family=orc.FAMILY_CHIRP)
+            assert t.family == 2
+            k = orc.rasterise(t, n_f)
+            ks, ys = _decimal_chirp(t, n_f)
+            n_pix += t.N
+            for c in range(t.N):
+                if k[c] != ks[c]:
+                    n_mis += 1
+                    assert abs(ys[c] - ys[c].to_integral_value()) < Decimal("1e-9"), (seed, tid, c)
+            assert (np.diff(k) >= 0).all() and k[0] >= int(np.floor(t.y0))          # an up-chirp from y0
+    assert n_pix > 40000 and n_mis <= 2
+
+
+def test_chirp_law_closed_forms(orc):
+    """f^(-8/3) is linear in time (the chirp law); at a = N / 256 the frequency at the END of the track
+    is 256^(3/8) = 8 times the start; the band clamp; T_c -> infinity (a -> N) is a flat track."""
+    n_f = 4096
+    N, y0 = 400, 100.5
+    t = orc.make_track(N, 7, N / 256.0, y0, 0.0, 0.0, family=orc.FAMILY_CHIRP)
+    k = orc.rasterise(t, n_f)
+    _, ys = _decimal_chirp(t, n_f)
+    u = np.arange(N) + 0.5
+    t_c = N * N / (N - t.a)
+    lin = np.array([float((y / Decimal(y0)) ** (Decimal(-8) / Decimal(3))) for y in ys])
+    assert np.allclose(lin, 1.0 - u / t_c, rtol=0, atol=1e-12)
+    # end of the track: u = N gives (T_c - N) / T_c = a / N = 1 / 256, so f = 8 y0; the last column centre is half a
+    # column earlier: f = y0 (T_c / (T_c - N + 1/2))^(3/8)
+    want_last = y0 * (t_c / (t_c - N + 0.5)) ** 0.375
+    assert k[-1] == int(np.floor(want_last)) and abs(want_last / y0 - 8.0) < 0.8
+    assert k[0] == int(np.floor(y0 * (t_c / (t_c - 0.5)) ** 0.375))
+    # leaving the band: the pixels ride the top bin (clamp), as for the Bezier families
+    hot = orc.rasterise(orc.make_track(300, 0, 300 / 256.0, 900.0, 0.0, 0.0, family=orc.FAMILY_CHIRP), 2461)
+    assert hot.max() == 2460 and (np.diff(hot) >= 0).all() and (hot == 2460).sum() > 3
+    # a -> N: T_c -> infinity, the track is flat at y0
+    flat = orc.rasterise(orc.make_track(200, 0, 200 - 1e-9, 333.5, 0.0, 0.0, family=orc.FAMILY_CHIRP), n_f)
+    assert (flat == 333).all()
+
+
+def test_chirp_family_parameters_and_search_path(orc):
+    """N, j0, a, y0, tau are those of the quadratic template with the same id; or_search with family 2 dumps
+    or_rasterise's pixels and recovers a noise-free injected bank member exactly (P7 for the family)."""
+    n_t, n_f = 500, 2461
+    for i in range(500):
+        q = orc.track_params(2, i, n_t, n_f, 10, 500, -0.01, 0.01)
+        c = orc.track_params(2, i, n_t, n_f, 10, 500, -0.01, 0.01, family=orc.FAMILY_CHIRP)
+        assert (q.N, q.j0, q.a, q.y0, q.tau) == (c.N, c.j0, c.a, c.y0, c.tau) and c.family == 2
+    cfg = synth.CONFIGS[1]
+    taus = synth.tau_linspace(cfg.n_tau)
+    f = cfg.f_min + cfg.df * np.arange(cfg.n_f)
+    i_star, m_star = 127, 9
+    t = orc.track_params(cfg.seed, i_star, cfg.n_t, cfg.n_f, 8, 64, family=orc.FAMILY_CHIRP)
+    k = orc.rasterise(t, cfg.n_f)
+    csd = np.zeros((cfg.n_t, cfg.n_f), dtype=np.complex64)
+    j = t.j0 + np.arange(t.N)
+    csd[j, k] = (2.0 * np.exp(-2j * np.pi * f[k] * taus[m_star])).astype(np.complex64)
+    p = orc.prepare_map(csd)
+    r = orc.search(p, cfg.f_min, cfg.df, 1000, cfg.seed, 8, 64, tau_grid=taus, family=orc.FAMILY_CHIRP, dump_tracks=True)
+    assert (r["arg_track"], r["arg_tau_index"]) == (i_star, m_star)
+    assert abs(r["max_snr"] - 2.0 * np.sqrt(t.N)) < 1e-5
+    assert np.array_equal(r["k"][i_star, :t.N], k) and (r["k"][i_star, t.N:] == -1).all()
