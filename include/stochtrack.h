@@ -71,9 +71,14 @@ extern "C" {
  * CUBIC (reading G26): a cubic Bezier curve whose time control points are the degree-elevated quadratic
  * (t(xi) is the quadratic family's) and whose frequency has four control points y0, y1, y2, y3, each
  * uniform over the band; N, j0, a, y0, y1, y2, tau of template i are those of the quadratic template i,
- * y3 comes from the one Philox word the quadratic family leaves unused.                              */
+ * y3 comes from the one Philox word the quadratic family leaves unused.
+ * CHIRP (reading G27): the leading-order inspiral sweep f ~ (t_c - t)^(-3/8) (the binary
+ * neutron star study): f(u) = y0 (T_c / (T_c - u))^(3/8) from the template's first column,
+ * T_c = N^2 / (N - a); N, j0, a, y0, tau are those of the quadratic template i; y1, y2, y3 are not used; a
+ * sweep that leaves the band rides its top bin.  Scored by the general builds of the kernels.          */
 #define ST_FAMILY_QUADRATIC 0
 #define ST_FAMILY_CUBIC     1
+#define ST_FAMILY_CHIRP     2
 
 /* scoring kernel selection (grid mode).  AUTO picks CHEBYSHEV when the grid is
  * uniform and every bin's step angle is well conditioned, else REINSCH / ROTATION
@@ -117,7 +122,7 @@ typedef struct {
     double   hist_lo, hist_hi; /* bin = floor((snr-lo)/(hi-lo)*n_bins) clamped (G14)    */
     uint64_t *hist_out;      /* HOST, n_bins counts (overwritten) or NULL               */
     int32_t  kernel;         /* ST_KERNEL_* request (grid mode)                         */
-    int32_t  family;         /* ST_FAMILY_QUADRATIC (0) | ST_FAMILY_CUBIC               */
+    int32_t  family;         /* ST_FAMILY_QUADRATIC (0) | ST_FAMILY_CUBIC | ST_FAMILY_CHIRP */
 } st_search_params;
 
 typedef struct {

@@ -10,4 +10,4 @@ CUDA device is present.
 from .binding import (Stochtrack, StError, SearchResult, st_track_params, st_track_words,  # noqa: F401
                       library_path, load_library, exported_symbols,
                       KERNEL_AUTO, KERNEL_TABLE, KERNEL_ROTATION, KERNEL_REINSCH, KERNEL_RANDOM, KERNEL_CHEBYSHEV,
-                      NORM_SQRT_N, NORM_MEAN, NORM_INVVAR, FAMILY_QUADRATIC, FAMILY_CUBIC, TAU_GRID, TAU_RANDOM)
+                      NORM_SQRT_N, NORM_MEAN, NORM_INVVAR, FAMILY_QUADRATIC, FAMILY_CUBIC, FAMILY_CHIRP, TAU_GRID, TAU_RANDOM)

@@ -13,7 +13,7 @@ _CODES = {ST_EINVAL: "ST_EINVAL", ST_ESTATE: "ST_ESTATE", ST_ENOSPC: "ST_ENOSPC"
 SIGMA_NONE, SIGMA_PER_FREQ, SIGMA_PER_PIXEL = 0, 1, 2
 TAU_GRID, TAU_RANDOM = 0, 1
 NORM_SQRT_N, NORM_MEAN, NORM_INVVAR = 0, 1, 2
-FAMILY_QUADRATIC, FAMILY_CUBIC = 0, 1
+FAMILY_QUADRATIC, FAMILY_CUBIC, FAMILY_CHIRP = 0, 1, 2
 KERNEL_AUTO, KERNEL_TABLE, KERNEL_ROTATION, KERNEL_REINSCH, KERNEL_RANDOM, KERNEL_CHEBYSHEV = 0, 1, 2, 3, 4, 5
 KERNEL_NAMES = {0: "auto", 1: "table", 2: "rotation", 3: "reinsch", 4: "random", 5: "chebyshev"}
 
@@ -515,13 +515,14 @@ class Stochtrack:
         self.synchronize()
         return k.cpu().numpy(), j0.cpu().numpy(), N.cpu().numpy()
 
-    def debug_rasterise_track(self, N, j0, a, y0, y1, y2, y3=None):
-        """Bins of one explicit template; with y3 a cubic one (frequency control points y0, y1, y2, y3)."""
+    def debug_rasterise_track(self, N, j0, a, y0, y1, y2, y3=None, family=None):
+        """Bins of one explicit template; with y3 a cubic one (frequency control points y0, y1, y2, y3); with
+        family=FAMILY_CHIRP the chirp-law template of (N, j0, a, y0)."""
         torch = self._torch
         t = CTrack(int(N), int(j0), float(a), float(y0), float(y1), float(y2), 0.0, 0.0 if y3 is None else float(y3))
         k = torch.empty(int(N), dtype=torch.int32, device=self.device)
-        self._check(self._L.st_debug_rasterise_track(self._ctx, C.byref(t), FAMILY_QUADRATIC if y3 is None else FAMILY_CUBIC,
-                                                     k.data_ptr()))
+        fam = family if family is not None else (FAMILY_QUADRATIC if y3 is None else FAMILY_CUBIC)
+        self._check(self._L.st_debug_rasterise_track(self._ctx, C.byref(t), int(fam), k.data_ptr()))
         self.synchronize()
         return k.cpu().numpy()
 

@@ -6,6 +6,7 @@
 // Second template family (PAPER.md:75 "other parameterizable curves", :246-252, :287; reading G26): a cubic
 // Bezier curve whose time control points are the degree-elevated quadratic (so t(xi) and its root are those
 // of the quadratic family) and whose frequency has four control points; the extra random number is r7.
+// Third family (reading G27): the chirp law f(u) = y0 (T_c / (T_c - u))^(3/8), T_c = N^2 / (N - a).
 //
 // Everything here is __host__ __device__ so that st_track_params (host, pure)
 // and the kernels share one statement of the arithmetic.  The rasteriser is a
@@ -83,7 +84,7 @@ struct BankParams {       // what S1 needs besides (seed, id)
     uint64_t seed;
     int32_t n_t, n_f, n_min, n_max;
     double tau_lo, tau_hi;
-    int32_t family;       // 0 quadratic (Eq. 6), 1 cubic in frequency (G26)
+    int32_t family;       // 0 quadratic (Eq. 6), 1 cubic in frequency (G26), 2 chirp law (G27)
     int32_t pad;
 };
 
@@ -105,7 +106,7 @@ ST_HD Track make_track(const BankParams& bp, uint64_t id)
     t.y2 = ST_DMUL(ST_DMUL((double)w.r[5] + 0.5, dF), kTwoM32);
     const double u = ST_DMUL((double)w.r[6] + 0.5, kTwoM32);
     t.tau = ST_DADD(bp.tau_lo, ST_DMUL(ST_DSUB(bp.tau_hi, bp.tau_lo), u));
-    t.y3 = bp.family ? ST_DMUL(ST_DMUL((double)w.r[7] + 0.5, dF), kTwoM32) : 0.0;
+    t.y3 = bp.family == 1 ? ST_DMUL(ST_DMUL((double)w.r[7] + 0.5, dF), kTwoM32) : 0.0;
     return t;
 }
 
@@ -121,7 +122,8 @@ struct Raster {
 // 3 n_f (cubic); a factor 3 is left on top
 ST_HD double raster_guard(int32_t n_f, int32_t family)
 {
-    const double g = (family ? 6e-11 : 4e-11) * (double)n_f;
+    // (chirp family: y = y0 r^(3/8) <= n_f inside the band, each of the four Newton-refined factors good to ~1e-12)
+    const double g = (family == 2 ? 1e-10 : (family ? 6e-11 : 4e-11)) * (double)n_f;
     return g > 1e-6 ? g : 1e-6;
 }
 
@@ -129,8 +131,13 @@ ST_HD Raster make_raster(const Track& t, int32_t n_f, int32_t family)
 {
     Raster r;
     r.a  = t.a;
-    r.cc = ST_DSUB((double)t.N, ST_DMUL(2.0, t.a));   // N - 2a
-    r.aa = ST_DMUL(t.a, t.a);
+    if (family == 2) {                                 // chirp law (G27): cc = N - a, aa = N^2 (exact)
+        r.cc = ST_DSUB((double)t.N, t.a);
+        r.aa = ST_DMUL((double)t.N, (double)t.N);
+    } else {
+        r.cc = ST_DSUB((double)t.N, ST_DMUL(2.0, t.a));   // N - 2a
+        r.aa = ST_DMUL(t.a, t.a);
+    }
     r.y0 = t.y0; r.y1 = t.y1; r.y2 = t.y2; r.y3 = t.y3;
     r.kmax = n_f - 1;
     r.family = family;
@@ -145,6 +152,18 @@ ST_HD Raster make_raster(const Track& t, int32_t n_f, int32_t family)
 ST_HD int32_t raster_bin(const Raster& r, int32_t c)
 {
     const double u   = (double)c + 0.5;
+    if (r.family == 2) {
+        // chirp law (G27): y = y0 r^(3/8), r = N^2 / (N^2 - u (N - a)); r^(1/8) by three square roots.  Normative
+        // order, every operation correctly rounded (the oracle's O3k).
+        const double D  = ST_DSUB(r.aa, ST_DMUL(u, r.cc));
+        const double q  = ST_DDIV(r.aa, D);
+        const double s  = ST_DSQRT(ST_DSQRT(ST_DSQRT(q)));
+        const double y  = ST_DMUL(ST_DMUL(ST_DMUL(s, s), s), r.y0);
+        const double fl = floor(y);
+        if (!(fl >= 0.0)) return 0;
+        if (fl > (double)r.kmax) return r.kmax;
+        return (int32_t)fl;
+    }
     double D         = ST_DADD(r.aa, ST_DMUL(r.cc, u));
     D                = D < 0.0 ? 0.0 : D;
     const double s   = ST_DSQRT(D);
@@ -202,8 +221,25 @@ __device__ __forceinline__ double raster_xi_fast(const R& r, double u)
     const double q0 = u * rc;
     return fma(fma(-den, q0, u), rc, q0);                       // one Newton step on the quotient u / den
 }
+// sqrt(x), x >= 1, from the MUFU seed and one Newton step (~1e-12)
+__device__ __forceinline__ double sqrt_fast(double x)
+{
+    double rs;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(rs) : "d"(x));
+    const double s0 = x * rs;
+    return fma(fma(-s0, s0, x), 0.5 * rs, s0);
+}
 __device__ __forceinline__ double raster_y_fast(const Raster& r, double u)
 {
+    if (r.family == 2) {                                            // chirp law (G27)
+        const double D = fma(-u, r.cc, r.aa);                       // N^2 - u (N - a) > 0
+        double rc;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(D));
+        const double q0 = r.aa * rc;
+        const double q  = fma(fma(-D, q0, r.aa), rc, q0);           // N^2 / D, one Newton step on the quotient
+        const double s  = sqrt_fast(sqrt_fast(sqrt_fast(q)));
+        return (s * s) * (s * r.y0);
+    }
     const double xi = raster_xi_fast(r, u);
     const double om = 1.0 - xi;
     if (r.family == 0) return fma(om * om, r.y0, fma(2.0 * (om * xi), r.y1, (xi * xi) * r.y2));
@@ -249,7 +285,11 @@ __device__ __forceinline__ RasterFast make_raster_fast(const Track& t, int32_t n
     const Raster r = make_raster(t, n_f, family);
     RasterFast f;
     f.a = r.a; f.cc = r.cc; f.aa = r.aa; f.y0 = r.y0; f.guard = r.guard; f.kmax = r.kmax;
-    if (family == 0) {
+    if (family == 2) {
+        // the chirp law has no fast path in this struct: a NaN polynomial sends every pixel to the normative
+        // sequence (the random-delay kernel's regenerate path), correct by construction
+        f.pb = f.pc = f.pd = __longlong_as_double(0x7FF8000000000000ll);
+    } else if (family == 0) {
         f.pb = 2.0 * (t.y1 - t.y0);                             // Eq. 6 in Horner form: y = y0 + xi (pb + xi pc)
         f.pc = (t.y0 - t.y1) + (t.y2 - t.y1);
         f.pd = 0.0;

@@ -173,7 +173,7 @@ int validate(st_ctx* c, const st_search_params* p, bool need_map)
     if (p->norm != ST_NORM_SQRT_N && p->norm != ST_NORM_MEAN && p->norm != ST_NORM_INVVAR) return fail(c, ST_EINVAL, "bad norm %d", p->norm);
     if (p->norm == ST_NORM_INVVAR && need_map && !c->have_isig)
         return fail(c, ST_ESTATE, "ST_NORM_INVVAR needs sigma: set the map through st_set_map / st_set_map_host / st_search_batch");
-    if (p->family != ST_FAMILY_QUADRATIC && p->family != ST_FAMILY_CUBIC) return fail(c, ST_EINVAL, "bad template family %d", p->family);
+    if (p->family != ST_FAMILY_QUADRATIC && p->family != ST_FAMILY_CUBIC && p->family != ST_FAMILY_CHIRP) return fail(c, ST_EINVAL, "bad template family %d", p->family);
     if (p->n_bins < 0 || p->n_bins > ST_MAX_BINS) return fail(c, ST_EINVAL, "n_bins %d outside [0, %d]", p->n_bins, ST_MAX_BINS);
     if (p->n_bins > 0 && !(p->hist_hi > p->hist_lo)) return fail(c, ST_EINVAL, "need hist_hi > hist_lo");
     if (p->kernel < ST_KERNEL_AUTO || p->kernel > ST_KERNEL_CHEBYSHEV || p->kernel == ST_KERNEL_RANDOM)
@@ -1329,7 +1329,7 @@ int st_track_params_family(const st_ctx* c, uint64_t seed, uint64_t track_id, in
 {
     if (!c || !out) return ST_EINVAL;
     if (n_min < 1 || n_max < n_min || n_max > c->n_t) return ST_EINVAL;
-    if (family != ST_FAMILY_QUADRATIC && family != ST_FAMILY_CUBIC) return ST_EINVAL;
+    if (family != ST_FAMILY_QUADRATIC && family != ST_FAMILY_CUBIC && family != ST_FAMILY_CHIRP) return ST_EINVAL;
     st::BankParams bp;
     bp.seed = seed; bp.n_t = c->n_t; bp.n_f = c->n_f; bp.n_min = n_min; bp.n_max = n_max;
     bp.tau_lo = tau_lo; bp.tau_hi = tau_hi; bp.family = family; bp.pad = 0;
@@ -1361,7 +1361,7 @@ int st_debug_rasterise(st_ctx* c, const st_search_params* p, uint64_t first, uin
     if (!p) return fail(c, ST_EINVAL, "params is NULL");
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
     if (p->n_min < 1 || p->n_max < p->n_min || p->n_max > c->n_t) return fail(c, ST_EINVAL, "need 1 <= n_min <= n_max <= n_t");
-    if (p->family != ST_FAMILY_QUADRATIC && p->family != ST_FAMILY_CUBIC) return fail(c, ST_EINVAL, "bad template family %d", p->family);
+    if (p->family != ST_FAMILY_QUADRATIC && p->family != ST_FAMILY_CUBIC && p->family != ST_FAMILY_CHIRP) return fail(c, ST_EINVAL, "bad template family %d", p->family);
     if (!k_out_dev || !j0_dev || !N_dev) return fail(c, ST_EINVAL, "output pointer is NULL");
     if (count == 0) return ST_OK;
     const uint64_t need = (count + 7) / 8;
@@ -1376,7 +1376,7 @@ int st_debug_rasterise_track(st_ctx* c, const st_track* t, int32_t family, int32
     DevGuard dev_guard(c);
     if (!c) return ST_EINVAL;
     if (!t || !k_out_dev) return fail(c, ST_EINVAL, "NULL argument");
-    if (family != ST_FAMILY_QUADRATIC && family != ST_FAMILY_CUBIC) return fail(c, ST_EINVAL, "bad template family %d", family);
+    if (family != ST_FAMILY_QUADRATIC && family != ST_FAMILY_CUBIC && family != ST_FAMILY_CHIRP) return fail(c, ST_EINVAL, "bad template family %d", family);
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
     if (t->N < 1 || t->j0 < 0 || t->j0 + t->N > c->n_t) return fail(c, ST_EINVAL, "track outside the map");
     st::Track d;

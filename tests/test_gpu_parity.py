@@ -1017,3 +1017,87 @@ class SimpleFlags(dict):
         super().__init__(r)
         self["flags"] = r["flags"] & ~6
     __getattr__ = dict.__getitem__
+
+
+# ------------------------------------------------------------------ third template family: chirp law (G27)
+@pytest.mark.parametrize("n_t,n_f,f_min,seed,n_min,n_max,first,count", [
+    (1000, 2461, 40.0, 4, 10, 1000, 0, 3000), (250, 961, 40.0, 1, 10, 250, 2 ** 33 + 5, 3000),
+    (64, 65535, 0.0, 77, 1, 64, 10 ** 12, 60_000), (4096, 2461, 0.0, 77, 3000, 4096, 10 ** 12, 400),
+    (16, 7, 0.0, 77, 1, 16, 10 ** 12, 20_000)])
+def test_chirp_family_indices_bit_exact(P, orc, n_t, n_f, f_min, seed, n_min, n_max, first, count):
+    """S1 + S2 of the chirp-law family (f ~ (t_c - t)^(-3/8); G27): parameters and every pixel index equal
+    the oracle's bit for bit, through the grid kernels' fast path (MUFU seeds + Newton for the quotient and the three
+    square roots, guarded) and the random-delay kernel's normative path."""
+    st = P.Stochtrack(n_t, n_f, 1.0, f_min, max_n_tau=64)
+    st.set_map(np.zeros((n_t, n_f), dtype=np.complex64))
+    p = np.zeros((n_t, n_f), dtype=np.complex128)
+    ref = orc.search(p, f_min, 1.0, count, seed, n_min, n_max, tau_range=(-0.01, 0.01), track_offset=first,
+                     dump_tracks=True, family=orc.FAMILY_CHIRP)
+    k, j0, N = st.debug_rasterise(seed, n_min, n_max, first, count, family=P.FAMILY_CHIRP)
+    assert np.array_equal(N, ref["N"]) and np.array_equal(j0, ref["j0"]) and np.array_equal(k, ref["k"])
+    k, j0, N = st.debug_rasterise_random(seed, n_min, n_max, first, min(count, 3000), family=P.FAMILY_CHIRP)
+    m = min(count, 3000)
+    assert np.array_equal(N, ref["N"][:m]) and np.array_equal(j0, ref["j0"][:m]) and np.array_equal(k, ref["k"][:m])
+    for tid in (first, first + count - 1):
+        a = st.track_params(seed, tid, n_min, n_max, -0.01, 0.01, family=P.FAMILY_CHIRP)
+        b = orc.track_params(seed, tid, n_t, n_f, n_min, n_max, -0.01, 0.01, family=orc.FAMILY_CHIRP)
+        assert (a.N, a.j0, a.a, a.y0, a.tau) == (b.N, b.j0, b.a, b.y0, b.tau)
+
+
+def test_chirp_family_explicit_tracks(P, orc):
+    cfg = synth.CONFIGS[5]
+    st = make_ctx(P, cfg)
+    for tr in [(1000, 0, 1000 / 256.0, 100.5), (777, 100, 3.0, 2460.999999), (10, 5, 1e-9, 100.0), (10, 5, 10 - 1e-9, 100.0),
+               (1, 999, 0.5, 7.3), (500, 250, 250.0, 7.5), (1000, 0, 999.999, 0.0000001), (300, 0, 300 / 256.0, 900.0)]:
+        got = st.debug_rasterise_track(tr[0], tr[1], tr[2], tr[3], 0.0, 0.0, family=P.FAMILY_CHIRP)
+        want = orc.rasterise(orc.make_track(tr[0], tr[1], tr[2], tr[3], 0.0, 0.0, family=orc.FAMILY_CHIRP), cfg.n_f)
+        assert np.array_equal(got, want), tr
+
+
+@pytest.mark.parametrize("cid,kname,n", [(2, "auto", 20_000), (2, "table", 3000), (2, "rotation", 3000), (5, "auto", 1500),
+                                         (3, "random", 20_000)])
+def test_chirp_family_search_parity(P, orc, cid, kname, n):
+    """Whole searches with the chirp bank: SNRs within G13, argmax / histogram / float64 re-score against the oracle."""
+    cfg = synth.CONFIGS[cid]
+    csd, sigma, tau = config_inputs(orc, cfg)
+    st = make_ctx(P, cfg)
+    st.set_map(csd, sigma)
+    p = orc.prepare_map(csd, sigma)
+    first = 654_321
+    kw = dict(tau_range=(-synth.TAU_MAX, synth.TAU_MAX)) if cfg.tau_mode == "random" else dict(tau_grid=tau, kernel=KERNELS.get(kname, 0))
+    okw = dict(tau_range=(-synth.TAU_MAX, synth.TAU_MAX)) if cfg.tau_mode == "random" else dict(tau_grid=tau)
+    ref = orc.search(p, cfg.f_min, cfg.df, n, cfg.seed, cfg.n_min, cfg.n_max, track_offset=first, family=orc.FAMILY_CHIRP,
+                     dump_snr=True, n_bins=cfg.n_bins, **okw)
+    got = st.debug_scores(cfg.seed, cfg.n_min, cfg.n_max, first, n, family=P.FAMILY_CHIRP, **kw)
+    ok, worst = snr_close(got, ref["snr"])
+    assert ok, f"{kname}: worst error {worst:.3f} x tolerance"
+    r = st.search(n, cfg.seed, cfg.n_min, cfg.n_max, track_offset=first, family=P.FAMILY_CHIRP, n_bins=cfg.n_bins, **kw)
+    _assert_search_parity(r, ref, cfg)
+
+
+def test_chirp_family_self_recovery_and_explicit_scores(P, orc):
+    """P7 for the family: an injected chirp bank member is returned exactly, and the quadratic bank does not reach its
+    SNR (the reason for the family); st_score_tracks scores explicit chirp templates like the oracle."""
+    cfg = synth.CONFIGS[2]
+    tau = synth.tau_linspace(64)
+    i_star, m_star, snr = 1234, 40, 9.0
+    t = orc.track_params(cfg.seed, i_star, cfg.n_t, cfg.n_f, cfg.n_min, cfg.n_max, family=orc.FAMILY_CHIRP)
+    k = orc.rasterise(t, cfg.n_f)
+    csd = np.zeros((cfg.n_t, cfg.n_f), dtype=np.complex64)
+    synth.add_injection(csd, None, t.j0 + np.arange(t.N), k, tau[m_star], snr, cfg.f_min, cfg.df)
+    st = make_ctx(P, cfg)
+    st.set_map(csd)
+    r = st.search(10000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau, family=P.FAMILY_CHIRP)
+    assert (r.arg_track, r.arg_tau_index) == (i_star, m_star) and r.max_snr_f64 == pytest.approx(snr, rel=1e-6)
+    rq = st.search(10000, cfg.seed, cfg.n_min, cfg.n_max, tau_grid=tau)
+    assert rq.max_snr_f64 < r.max_snr_f64
+    csd, sigma, _ = config_inputs(orc, cfg)
+    st.set_map(csd, sigma)
+    p = orc.prepare_map(csd, sigma)
+    tracks = [(250, 0, 250 / 64.0, 100.5, 0.0, 0.0, 0.0, 0.0), (200, 20, 60.0, 300.25, 0.0, 0.0, 0.0, 0.0)]
+    got = st.score_tracks(tracks, tau_grid=tau, family=P.FAMILY_CHIRP)
+    W = orc.build_table(cfg.n_f, cfg.f_min, cfg.df, tau)
+    ref = np.array([orc.score_table(p, orc.make_track(*tr[:6], family=orc.FAMILY_CHIRP),
+                                    orc.rasterise(orc.make_track(*tr[:6], family=orc.FAMILY_CHIRP), cfg.n_f), W) for tr in tracks])
+    ok, worst = snr_close(got, ref)
+    assert ok, worst
