@@ -904,16 +904,14 @@ __device__ __forceinline__ f32x2_t pk_make(float lo, float hi)
 }
 __device__ __forceinline__ float pk_lo(f32x2_t a)
 {
-    float lo, hi;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a));
-    (void)hi;
+    float lo;
+    asm("{\n\t.reg .b32 t;\n\tmov.b64 {%0, t}, %1;\n\t}" : "=f"(lo) : "l"(a));
     return lo;
 }
 __device__ __forceinline__ float pk_hi(f32x2_t a)
 {
-    float lo, hi;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a));
-    (void)lo;
+    float hi;
+    asm("{\n\t.reg .b32 t;\n\tmov.b64 {t, %0}, %1;\n\t}" : "=f"(hi) : "l"(a));
     return hi;
 }
 __device__ __forceinline__ float pk_sum(f32x2_t a)
