@@ -35,7 +35,7 @@ FLOP_PER_EVAL = 4                     # Eq. 8 needs 2 FMA per (pixel, delay) onc
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the `ncu --set full` capture
 # named beside it (profiles/; the command is in the file's first line).  The map is read from HBM once per launch
 # and then served by L2; a config without a capture reports null.
-DRAM_TRAFFIC = {5: (19.85e6, "profiles/r02_ncu_cheb_c5.txt"),      # algorithmic: the 19.69 MB map once
+DRAM_TRAFFIC = {5: (19.83e6, "profiles/r02_ncu_cheb_c5.txt"),      # algorithmic: the 19.69 MB map once
                 4: (9.97e6, "profiles/r02_ncu_cheb_c4.txt"),       # per map of the batch: the 9.84 MB map once
                 3: (9.88e6, "profiles/r02_ncu_random.txt")}
 L2_GATHER_PEAK_GBS = 9200.0          # random 32-byte sector gathers, measured (profiles/microbench_r01.md)
