@@ -616,14 +616,12 @@ __device__ __forceinline__ void reduce_samples_multi(const ScoreArgs& a, WarpRed
     }
 }
 
-#ifndef ST_RANDOM_MIN_BLOCKS
-#define ST_RANDOM_MIN_BLOCKS 3
-#endif
+constexpr int kRandMinBlocks = 3;
 // KDUMP: parity export -- the bins this kernel's own fast path (Horner form, regenerate-on-fallback) decides
 // are written to a.k_dump next to the scores (st_debug_rasterise_random).
 // GEN as in the Chebyshev kernel: false = quadratic bank templates with N^-alpha (options compiled in as constants).
 template <bool CAPTURE, bool KDUMP, bool GEN>
-__global__ void __launch_bounds__(256, ST_RANDOM_MIN_BLOCKS) k_score_random(const ScoreArgs a)
+__global__ void __launch_bounds__(256, kRandMinBlocks) k_score_random(const ScoreArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t* sm_hist = reinterpret_cast<uint32_t*>(smem);
@@ -1202,13 +1200,6 @@ struct ChebPixel {
 // through a ballot.  The work is cut into ELEMENTS of four columns per lane: cheb_fetch issues the
 // four rasteriser chains and the L2 gathers of an element, cheb_merge consumes them, so that a
 // caller can keep the next element in flight while it merges the current one.
-// A map pixel is used once per template: gathered past L1 so that the per-bin tables stay there.
-__device__ __forceinline__ float2 ldg_stream_f2(const float2* p)
-{
-    float2 v;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
-    return v;
-}
 struct ChebFetchCtx {          // what fetching needs to know about a template
     Raster r;
     uint16_t* krow;            // bank cache: this lane's slice of the template's row
@@ -1220,13 +1211,9 @@ struct ChebElem { int k[4]; float2 p[4], e[4]; float r[4]; };     // r: 1 / sigm
 struct ChebMergeState { int run_k, n_a, n_b; float ax, ay; float2 run_e; float w2, bamp; };
 struct ChebCounts { int n_a, n_b; };       // pool entries of class A (front of the pool) and class B (back)
 
-// The normative rasteriser sequence of the rare fallback.  Measured as an out-of-line call (-DST_COLD_CALL: 19 %
-// less code in the kernel): config 4 +0.5 %, config 5 -1.4 % -- inlined it stays.
-#ifndef ST_COLD_CALL
+// The normative rasteriser sequence of the rare fallback (inlined: as an out-of-line call the kernel has 19 % less
+// code, config 4 +0.5 %, config 5 -1.4 %).
 __device__ __forceinline__ int32_t raster_bin_cold(const Raster& r, int32_t c) { return raster_bin(r, c); }
-#else
-__device__ __noinline__ int32_t raster_bin_cold(const Raster r, int32_t c) { return raster_bin(r, c); }
-#endif
 
 // GEN = false compiles the default search (quadratic templates, N^-alpha normalisation) with the template
 // family and the weighting as constants; GEN = true reads both from the arguments (cubic family, norm 2).
@@ -1273,11 +1260,7 @@ __device__ __forceinline__ void cheb_fetch(const ScoreArgs& a, const ChebFetchCt
     for (int u = 0; u < 4; ++u) {
         ST_ASSERT(E.k[u] >= 0 && E.k[u] < a.bp.n_f && cc[u] >= 0 &&
                   (size_t)(f.col0 - a.map) / (size_t)a.bp.n_f + (size_t)cc[u] < (size_t)a.bp.n_t);
-#ifdef ST_X_NOALLOC
-        E.p[u] = ldg_stream_f2(f.col0 + (size_t)cc[u] * (size_t)a.bp.n_f + (size_t)E.k[u]);
-#else
         E.p[u] = __ldg(f.col0 + (size_t)cc[u] * (size_t)a.bp.n_f + (size_t)E.k[u]);
-#endif
         E.e[u] = __ldg(&a.Ec[E.k[u]]);
     }
     if (GEN && a.norm == 2) {                          // inverse-variance weights (G25): one more gather per pixel
@@ -1423,10 +1406,8 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
     const int S = a.pool_stride;
     TrackMax tm;
     tmax_init(tm);
-#ifndef ST_PLAIN_ADDR
     const uint32_t pv_base = smem_u32(pool_v) + (uint32_t)lane * 8u, pk_base = smem_u32(pool_k) + (uint32_t)lane * 2u;
     const uint32_t tab_base = smem_u32(sm_tab), zi_base = smem_u32(sm_zi);
-#endif
     // ---- phase B: chunks of 64 delays; f2[i] = (sum x_{mc+i}, sum x_{mc-1-i}) over this lane's pixels
 #pragma unroll 1
     for (int j = 0; j < n_chunks; ++j) {
@@ -1434,7 +1415,6 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
 #pragma unroll
         for (int i = 0; i < kHalf; ++i) f2[i] = 0ull;
         int row = 0;
-#ifndef ST_PLAIN_ADDR
         uint32_t pv = pv_base, pk = pk_base;           // this lane's entry of the current row
 #pragma unroll 1
         for (; row + 2 <= n_rows; row += 2, pv += 2 * kWarp * 8, pk += 2 * kWarp * 2) {
@@ -1448,19 +1428,6 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
             sts_f2<0>(pv, fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
             sts_f2<kWarp * 8>(pv, fmaf(v1.x, t1.w, -(v1.y * zi1)), fmaf(v1.x, zi1, v1.y * t1.w));
             ChebPixel<STRIDE> A, B;
-#else
-#pragma unroll 1
-        for (; row + 2 <= n_rows; row += 2) {
-            const int e0 = row * kWarp + lane, e1 = e0 + kWarp;
-            const float2 v0 = pool_v[e0], v1 = pool_v[e1];
-            const int k0 = pool_k[e0], k1 = pool_k[e1];
-            ST_ASSERT(k0 >= 0 && k0 < a.bp.n_f && k1 >= 0 && k1 < a.bp.n_f);
-            const float4 t0 = sm_tab[k0], t1 = sm_tab[k1];
-            const float zi0 = sm_zi[k0], zi1 = sm_zi[k1];
-            pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
-            pool_v[e1] = make_float2(fmaf(v1.x, t1.w, -(v1.y * zi1)), fmaf(v1.x, zi1, v1.y * t1.w));
-            ChebPixel<STRIDE> A, B;
-#endif
             A.anchor(v0, t0);
             B.anchor(v1, t1);
             if (STRIDE == 1) {
@@ -1498,20 +1465,11 @@ __device__ __forceinline__ void cheb_phase_b(const ScoreArgs& a, WarpReduce& wr,
             }
         }
         if (row < n_rows) {          // odd tail row
-#ifndef ST_PLAIN_ADDR
             const float2 v0 = lds_f2<0>(pv);
             const uint32_t k0 = lds_u16<0>(pk);
             const float4 t0 = lds_f4(tab_base + k0 * 16u);
             const float zi0 = lds_f1(zi_base + k0 * 4u);
             sts_f2<0>(pv, fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
-#else
-            const int e0 = row * kWarp + lane;
-            const float2 v0 = pool_v[e0];
-            const int k0 = pool_k[e0];
-            const float4 t0 = sm_tab[k0];
-            const float zi0 = sm_zi[k0];
-            pool_v[e0] = make_float2(fmaf(v0.x, t0.w, -(v0.y * zi0)), fmaf(v0.x, zi0, v0.y * t0.w));
-#endif
             ChebPixel<STRIDE> A;
             A.anchor(v0, t0);
             if (STRIDE == 1) {

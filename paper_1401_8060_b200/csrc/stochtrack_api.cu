@@ -217,10 +217,7 @@ bool reinsch_well_conditioned(const st_ctx* c, double dtau)
 // Returns the number of class B bins, or -1 when some bin suits neither form (then the grid goes to the rotation
 // kernel).  Table per bin: (G, cos theta, sin theta, cos 64 theta), Ec = anchor phase factor of chunk 0 with the
 // class in the lowest mantissa bit of its real part, zi = sin 64 theta.
-#ifndef ST_CLASS_DRIFT
-#define ST_CLASS_DRIFT 3e-6
-#endif
-constexpr double kChebClassDrift = ST_CLASS_DRIFT;   // rad over half a chunk: A = 16 stays inside half the G13 tolerance
+constexpr double kChebClassDrift = 3e-6;   // rad over half a chunk: A = 16 stays inside half the G13 tolerance
 
 int build_cheb_tables(const st_ctx* c, double tau0, double dtau, int stride, std::vector<float>* out, double* d_max = nullptr)
 {
@@ -438,10 +435,7 @@ size_t bank_bytes_for(uint64_t n_tracks, int n_max)
 // Absolute error (in SNR units) the fast Chebyshev build may owe to coefficient drift in class B bins: half the
 // G13 tolerance at a zero crossing of SNR(tau) on the configs' data (1e-4 x s0, s0 = 0.707).  Class A bins add
 // at most kChebClassDrift x A for a coherent amplitude A (3e-5 at SNR 10).
-#ifndef ST_DEFER_BUDGET
-#define ST_DEFER_BUDGET 3.5e-5
-#endif
-constexpr double kChebDeferBudget = ST_DEFER_BUDGET;
+constexpr double kChebDeferBudget = 3.5e-5;
 
 int launch_score(st_ctx* c, const Plan& plan, st::ScoreArgs& a, int n_max, int* extra_launches = nullptr)
 {
