@@ -137,3 +137,32 @@ def test_timeshift_background_from_strain(P, orc):
     assert (one.max_snr_f64, one.arg_track, one.arg_tau_index) == (res[0].max_snr_f64, res[0].arg_track, res[0].arg_tau_index)
     with pytest.raises(P.StError):
         st.search_timeshifts(torch.from_numpy(s_i).cuda(), torch.from_numpy(s_j).cuda(), fs, L, n_nb, [n_t], 1, 10, 20, 64, tau_grid=tau)
+
+
+def test_timeshift_background_with_one_bank_and_the_bank_cache(P, orc):
+    """The paper's background workflow with ONE template bank for every time shift ("arrays of Bezier
+    curves", :173 n_ts time-shift analyses): with the bank cache attached the first shift fills it, the others read
+    S1 + S2 back; every result is bit-identical to the call without a cache and agrees with the oracle."""
+    import torch
+    rng = np.random.default_rng(34)
+    fs, L, n_t, n_f, f_min, n_nb = 1024.0, 1024, 64, 200, 100.0, 6
+    n = (n_t + 1) * L // 2
+    s_i, s_j = rng.standard_normal(n), rng.standard_normal(n)
+    shifts, seed, T = [0, 3, 9, 27, 40], 11, 6000
+    tau = synth.tau_linspace(100, -0.01, 0.01)                    # two chunks: the one-pass build
+    di, dj = torch.from_numpy(s_i).cuda(), torch.from_numpy(s_j).cuda()
+    plain = P.Stochtrack(n_t, n_f, fs / L, f_min, max_n_tau=128)
+    want, _ = plain.search_timeshifts(di, dj, fs, L, n_nb, shifts, seed, T, 20, 64, tau_grid=tau, n_bins=100)
+    assert all(w.flags & 6 == 0 for w in want)
+    st = P.Stochtrack(n_t, n_f, fs / L, f_min, max_n_tau=128)
+    assert st.enable_bank_cache(T, 64) > 0
+    got, _ = st.search_timeshifts(di, dj, fs, L, n_nb, shifts, seed, T, 20, 64, tau_grid=tau, n_bins=100)
+    assert got[0].flags & 4 and all(g.flags & 2 for g in got[1:])
+    for g, w in zip(got, want):
+        assert (g.max_snr, g.max_snr_f64, g.arg_track, g.arg_tau_index, g.n_evals) == (w.max_snr, w.max_snr_f64, w.arg_track, w.arg_tau_index, w.n_evals)
+        assert np.array_equal(g.hist, w.hist)
+    _, r_i, r_j, _, _ = F.ftmap(s_i, s_j, fs, L, n_t, f_min, n_f, n_nb)
+    for m in (1, 4):
+        ref = orc.search(F.ftmap_timeshift(r_i, r_j, n_nb, shifts[m]), f_min, fs / L, T, seed, 20, 64, tau_grid=tau, n_bins=100)
+        assert (got[m].arg_track, got[m].arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
+        assert abs(got[m].max_snr_f64 - ref["max_snr"]) <= 1e-5 * abs(ref["max_snr"])
