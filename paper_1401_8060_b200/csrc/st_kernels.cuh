@@ -583,9 +583,7 @@ __device__ __forceinline__ void reduce_samples_multi(const ScoreArgs& a, WarpRed
         if (a.dump) a.dump[q] = v;
         if (a.tmax_snr) { a.tmax_snr[q] = v; a.tmax_m[q] = 0; }     // one delay per template: it is its own maximum
     }
-    float wmax = valid ? v : -INFINITY;
-#pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) wmax = fmaxf(wmax, __shfl_xor_sync(kFull, wmax, off));
+    const float wmax = dec_f32(__reduce_max_sync(kFull, enc_f32(valid ? v : -INFINITY)));     // one REDUX (see reduce_samples)
     if (wmax >= wr.cached_max - near_margin(wr.cached_max)) {
         const int lane = threadIdx.x & 31;
         uint32_t old = 0;
