@@ -111,6 +111,15 @@ def test_host_track_generator_matches_oracle_bit_for_bit(lib, orc):
             o = orc.track_params(seed, tid, n_t, n_f, n_min, n_max, -0.01, 0.01)
             for f in ("N", "j0", "a", "y0", "y1", "y2", "tau"):
                 assert getattr(g, f) == getattr(o, f), (seed, tid, f)
+    # the other template families (G26: y3 from the eighth Philox word; G27: the chirp law uses N, j0, a, y0, tau)
+    for family in (P.FAMILY_CUBIC, P.FAMILY_CHIRP):
+        for tid in ids[:60] + ids[-4:]:
+            g = P.st_track_params(500, 2461, 2, tid, 10, 500, -0.01, 0.01, family=family)
+            o = orc.track_params(2, tid, 500, 2461, 10, 500, -0.01, 0.01, family=family)
+            for f in ("N", "j0", "a", "y0", "y1", "y2", "tau", "y3"):
+                assert getattr(g, f) == getattr(o, f), (family, tid, f)
+    with pytest.raises(P.StError):
+        P.st_track_params(500, 2461, 2, 0, 10, 500, family=3)
 
 
 def test_binding_fails_loudly_without_gpu():
