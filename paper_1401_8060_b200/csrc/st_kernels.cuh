@@ -3,12 +3,19 @@
 //   k_prepare_map      S0  p = CSD / sigma                     Eq. 7
 //   k_build_w_table    twiddles W[k][m] = e^{2 pi i f_k tau_m}        (G6, G7)
 //   k_build_bin_tables per-bin constants of the uniform-grid recurrences
+//   k_score_cheb       S1-S4, uniform tau grid, the production kernel: lanes over pixels, the term of
+//                      Eq. 8 advanced along tau by a packed two-sided Chebyshev recurrence (one FFMA2 +
+//                      one FADD2 per two evaluations); builds: search / capture / per-template maximum,
+//                      fast / general (two-class, cubic and chirp families, inverse-variance weighting,
+//                      explicit templates), bank cache fill / read, one chunk or two chunks per pass,
+//                      one-pass software-pipelined
+//   k_score_reinsch    S1-S4, uniform tau grid: Reinsch's form of the recurrence (3 operations per evaluation)
+//   k_score_recur      S1-S4, uniform tau grid: complex rotation recurrence (5 operations, any step angle)
 //   k_score_table      S1-S4, any tau grid: lanes over tau, W read through L1/L2
-//   k_score_recur      S1-S4, uniform tau grid: lanes over pixels, the phase factor
-//                      advanced along tau by a recurrence in registers
 //   k_score_random     S1-S4, the paper's mode: one random delay per template
 //   k_finalize         S4: float64 re-score of the near-max candidates, argmax (G12)
-//   k_debug_rasterise  parity export of S1+S2
+//   k_rescore_cands    float64 scores of the captured samples (st_search_topk)
+//   k_debug_rasterise  parity exports of S1+S2
 //
 // One warp owns one template at a time (templates are independent: PAPER.md:25,
 // :242 "embarrassingly parallel").  No tensor cores: per template the sum of
