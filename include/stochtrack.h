@@ -328,6 +328,57 @@ int st_debug_scores(st_ctx *ctx, const st_search_params *params, uint64_t first,
 /* The 8 Philox words of a template (HOST out[8]); pure host function.          */
 int st_debug_track_words(uint64_t seed, uint64_t track_id, uint32_t *out_host);
 
+/* The paper's one-delay-per-template scoring (S0-S3 of the list at the top) for callers that
+ * cannot give the library any device memory of their own.
+ *
+ * Who that is.  Every other device call here needs a workspace the caller allocates (st_set_workspace), and a
+ * workspace is an allocation like any other.  Some hosts of this library have none to give: a search stage
+ * plugged into a pipeline whose framework reserved the whole card for its own memory pool at start-up, so that a
+ * late cudaMalloc fails with out-of-memory; an online (low-latency) analysis that may not allocate or free while
+ * it runs, because cudaMalloc / cudaFree synchronise the whole device and stall every other stream of the
+ * process; a component that is handed exactly its input and output buffers by the application around it and
+ * has no allocator of its own to ask.  They still own the map they want searched and the buffer the scores go
+ * to: those are this call's only pointers.
+ *
+ * What it does.  snr_dev[q] = SNR of template params->track_offset + q with that template's own random delay
+ * in (tau_lo, tau_hi), q = 0 .. params->n_tracks - 1: bit for bit what st_set_map(csd_dev, sigma_dev, sigma_kind)
+ * followed by st_debug_scores(params, track_offset, n_tracks, snr_dev) writes for a context of the same n_t,
+ * n_f, df, f_min -- the same two kernels (k_prepare_map, k_score_random) are launched.  What those kernels keep
+ * besides their inputs and outputs -- the weighted map p = CSD / sigma with its 1 / sigma plane, the
+ * work-claim counter and the reduction records -- lives in ONE array of ST_NOALLOC_SCRATCH_BYTES (about
+ * 3.4 MiB) that is compiled into the library as a static __device__ object.  Every GPU on which the library's
+ * code gets loaded holds its copy of that array until the process exits, whether or not this call is ever
+ * used there.  The call itself performs no cudaMalloc, cudaFree, cudaHostAlloc, stream / event creation or
+ * any other allocating CUDA or library routine; it issues one cudaMemsetAsync and two kernel launches.
+ *
+ * Limits (the price of a fixed array): n_t * n_f <= ST_NOALLOC_MAX_PIXELS (the Table III map of the paper,
+ * 500 x 151, and the 250 x 961 map of BASELINE.json configs[1] fit; the 500 x 2461 maps do not), else ST_ENOSPC;
+ * ST_TAU_RANDOM only, quadratic templates, norm ST_NORM_SQRT_N or ST_NORM_MEAN, n_tracks <= 2^31 (one launch),
+ * else ST_EINVAL.  The fields n_tau, tau_grid, n_bins, hist_*, kernel of params are ignored.
+ *
+ *   csd_dev, sigma_dev : DEVICE, as st_set_map (complex64 [n_t][n_f]; float32 per sigma_kind), on the CURRENT device
+ *   snr_dev            : DEVICE float32 [n_tracks], on the current device, caller-owned
+ *   cuda_stream        : cudaStream_t as void* (NULL = default stream) of the current device; the call is
+ *                        stream-ordered and returns once its work is enqueued (inputs / output may be released
+ *                        after the stream has passed it)
+ *   err_host, err_len  : optional HOST buffer that receives the message of a failing call (may be NULL / 0)
+ *
+ * The first call on each device looks up that device's address of the array (cudaGetSymbolAddress, which may
+ * load the library's device code there) and the SM count; later calls reuse them.  Make that first call at
+ * start-up, outside any stream capture.
+ * The array is shared by every call on a device and still holds what the previous call left in it: the call
+ * clears the part that must start from zero and overwrites the map, so consecutive calls on one stream are
+ * independent of each other; but two calls whose work can overlap on the GPU (different streams, or different
+ * host threads on different streams) use the same array at the same time and corrupt each other's results --
+ * keep all calls of a device on one stream, or order them with events.  It uses no st_ctx and does not
+ * touch the state of any.                                                                                */
+#define ST_NOALLOC_MAX_PIXELS    262144
+#define ST_NOALLOC_SCRATCH_BYTES 3604736
+int st_score_random_noalloc(const void *csd_dev, const float *sigma_dev, int32_t sigma_kind,
+                            int32_t n_t, int32_t n_f, double df, double f_min,
+                            const st_search_params *params, float *snr_dev, void *cuda_stream,
+                            char *err_host, size_t err_len);
+
 const char *st_last_error(const st_ctx *ctx);
 /* Library / build identification, e.g. "stochtrack-b200 sm_100a".              */
 const char *st_version(void);

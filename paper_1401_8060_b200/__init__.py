@@ -9,5 +9,6 @@ CUDA device is present.
 """
 from .binding import (Stochtrack, StError, SearchResult, st_track_params, st_track_words,  # noqa: F401
                       library_path, load_library, exported_symbols,
+                      score_random_noalloc, NOALLOC_MAX_PIXELS, NOALLOC_SCRATCH_BYTES,
                       KERNEL_AUTO, KERNEL_TABLE, KERNEL_ROTATION, KERNEL_REINSCH, KERNEL_RANDOM, KERNEL_CHEBYSHEV,
                       NORM_SQRT_N, NORM_MEAN, NORM_INVVAR, FAMILY_QUADRATIC, FAMILY_CUBIC, FAMILY_CHIRP, TAU_GRID, TAU_RANDOM)

@@ -24,6 +24,7 @@ exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_wor
                     "st_debug_get_map",
                     "st_track_params", "st_track_params_family", "st_debug_rasterise",
                     "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words",
+                    "st_score_random_noalloc",
                     "st_last_error", "st_version")
 
 
@@ -146,6 +147,9 @@ def load_library(path=None):
     L.st_score_tracks.restype = C.c_int
     L.st_debug_rasterise_random.argtypes = [vp, C.POINTER(CSearchParams), C.c_uint64, C.c_uint64, vp, vp, vp]
     L.st_debug_rasterise_random.restype = C.c_int
+    L.st_score_random_noalloc.argtypes = [vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_double, C.c_double,
+                                          C.POINTER(CSearchParams), vp, vp, C.c_char_p, C.c_size_t]
+    L.st_score_random_noalloc.restype = C.c_int
     for name in ("st_create", "st_set_workspace", "st_set_map", "st_set_map_host", "st_search", "st_search_batch", "st_track_params",
                  "st_debug_rasterise", "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words"):
         getattr(L, name).restype = C.c_int
@@ -535,6 +539,53 @@ class Stochtrack:
         self._check(self._L.st_debug_scores(self._ctx, C.byref(p), int(first), int(count), snr.data_ptr()))
         self.synchronize()
         return snr.cpu().numpy()
+
+
+NOALLOC_MAX_PIXELS = 262144        # ST_NOALLOC_MAX_PIXELS
+NOALLOC_SCRATCH_BYTES = 3604736    # ST_NOALLOC_SCRATCH_BYTES
+
+
+def score_random_noalloc(csd, sigma, df, f_min, n_tracks, seed, n_min, n_max, tau_range, out, norm=NORM_SQRT_N,
+                         track_offset=0, stream=None):
+    """st_score_random_noalloc: the one-delay-per-template scores of templates [track_offset, +n_tracks) on
+    the map csd / sigma, for a caller who has no device memory to lend the library (a framework pool owns the
+    card, nothing may be allocated while the analysis runs, or the component only sees its own input and
+    output buffers).  The library's scratch is a static array inside its device image (NOALLOC_SCRATCH_BYTES
+    on every GPU that loads it), which caps the map at NOALLOC_MAX_PIXELS pixels.  Nothing is allocated here
+    either: `out` is the caller's float32 CUDA tensor of n_tracks elements and is returned filled
+    (stream-ordered, not synchronised).  All calls on one device share the static array: issue them on one
+    stream; the first call per device does a one-off symbol look-up and belongs at start-up.
+    csd: complex64 [n_t][n_f] CUDA tensor; sigma: None, [n_f] or [n_t][n_f] float32 CUDA tensor."""
+    import torch
+    L = load_library()
+    if not (isinstance(csd, torch.Tensor) and csd.is_cuda and csd.dtype == torch.complex64 and csd.is_contiguous() and csd.dim() == 2):
+        raise ValueError("csd must be a contiguous complex64 [n_t][n_f] CUDA tensor")
+    n_t, n_f = int(csd.shape[0]), int(csd.shape[1])
+    kind, sp = SIGMA_NONE, 0
+    if sigma is not None:
+        if not (isinstance(sigma, torch.Tensor) and sigma.is_cuda and sigma.dtype == torch.float32 and sigma.is_contiguous()):
+            raise ValueError("sigma must be a contiguous float32 CUDA tensor")
+        shp = tuple(sigma.shape)
+        kind = SIGMA_PER_FREQ if shp == (n_f,) else SIGMA_PER_PIXEL if shp == (n_t, n_f) else -1
+        if kind < 0:
+            raise ValueError("sigma must be None, [n_f] or [n_t][n_f]")
+        sp = sigma.data_ptr()
+    if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float32 and out.is_contiguous()
+            and out.numel() == int(n_tracks)):
+        raise ValueError("out must be a contiguous float32 CUDA tensor of n_tracks elements")
+    p = CSearchParams()
+    p.n_tracks, p.track_offset, p.seed = int(n_tracks), int(track_offset), int(seed)
+    p.n_min, p.n_max, p.tau_mode, p.n_tau = int(n_min), int(n_max), TAU_RANDOM, 1
+    p.tau_lo, p.tau_hi = float(tau_range[0]), float(tau_range[1])
+    p.norm, p.family = int(norm), FAMILY_QUADRATIC
+    err = C.create_string_buffer(512)
+    with torch.cuda.device(csd.device):
+        s = stream if stream is not None else torch.cuda.current_stream(csd.device)
+        rc = L.st_score_random_noalloc(csd.data_ptr(), sp, kind, n_t, n_f, float(df), float(f_min), C.byref(p),
+                                       out.data_ptr(), s.cuda_stream, err, len(err))
+    if rc:
+        raise StError(rc, err.value.decode())
+    return out
 
 
 def st_track_params(n_t, n_f, seed, track_id, n_min, n_max, tau_lo=0.0, tau_hi=0.0, df=1.0, f_min=0.0,

@@ -11,6 +11,7 @@
 #include <math.h>
 #include <vector>
 #include <algorithm>
+#include <mutex>
 #include <new>
 
 #include "../../include/stochtrack.h"
@@ -1469,3 +1470,154 @@ int st_debug_scores(st_ctx* c, const st_search_params* p, uint64_t first, uint64
 }
 
 }  // extern "C"
+
+// ================================================= entry point without allocations ====
+// st_score_random_noalloc (include/stochtrack.h): S0-S3 in the paper's one-delay-per-template mode
+// for hosts that cannot hand the library a workspace -- a framework's pool owns the whole
+// card, or nothing may be allocated while the analysis is live, or the component only ever sees its input
+// and output buffers.  The kernels are the library's own k_prepare_map and k_score_random<false, false, false>,
+// launched as st_set_map + st_debug_scores launch them; the only difference is where their scratch lives.
+//
+// g_noalloc_scratch is that scratch: a static __device__ array, so it is part of the library's device image
+// and every GPU that loads the image carries these ST_NOALLOC_SCRATCH_BYTES until the process ends.  In HOST
+// code the name `g_noalloc_scratch` is only a handle for the symbol look-up -- it is not a device address and
+// must never be passed to a kernel or to cudaMemset; noalloc_device() asks the runtime for the real address
+// once per device, with that device current, and every use below goes through that pointer.
+namespace {
+
+constexpr uint32_t kNaCandCap = 4096;                   // near-max records (not read back: the scores are the output)
+constexpr size_t kNaOffScalars  = 0;                                                                    // st::Scalars
+constexpr size_t kNaOffWarpBest = 256;                                                                  // [kWarpSlots]
+constexpr size_t kNaOffCand     = kNaOffWarpBest + (size_t)kWarpSlots * sizeof(st::WarpBest);           // [kNaCandCap]
+constexpr size_t kNaOffMap      = kNaOffCand + (size_t)kNaCandCap * sizeof(st::Cand);                   // p, float2 per pixel
+constexpr size_t kNaOffIsig     = kNaOffMap + (size_t)ST_NOALLOC_MAX_PIXELS * sizeof(float2);           // 1 / sigma per pixel
+constexpr size_t kNaTotal       = kNaOffIsig + (size_t)ST_NOALLOC_MAX_PIXELS * sizeof(float);
+constexpr size_t kNaZeroed      = kNaOffCand;           // [0, kNaZeroed): what a call needs to find zeroed
+static_assert(sizeof(st::Scalars) <= kNaOffWarpBest, "scalars outgrew their slot");
+static_assert(kNaOffCand % kAlign == 0 && kNaOffMap % kAlign == 0 && kNaOffIsig % kAlign == 0, "scratch parts must stay 256-byte aligned");
+static_assert(kNaTotal == ST_NOALLOC_SCRATCH_BYTES, "include/stochtrack.h states the size of the static scratch");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNaTotal];
+
+constexpr int kNaMaxDevices = 64;
+struct NoallocDevice { bool ready; unsigned char* scratch; int n_sm; };
+NoallocDevice g_na_dev[kNaMaxDevices];                  // zero-initialised: nothing looked up yet
+std::mutex g_na_mutex;
+
+int na_fail(char* err, size_t len, int code, const char* fmt, ...)
+{
+    if (err && len) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(err, len, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+// Set-up, once per device, on that device's first call (which therefore belongs at start-up, before any
+// stream capture): the device must be current for cudaGetSymbolAddress to return ITS copy of the array.
+int noalloc_device(int dev, NoallocDevice* out, char* err, size_t len)
+{
+    std::lock_guard<std::mutex> lock(g_na_mutex);
+    NoallocDevice& d = g_na_dev[dev];
+    if (!d.ready) {
+        void* ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+        if (e != cudaSuccess || !ptr)
+            return na_fail(err, len, ST_ECUDA, "cudaGetSymbolAddress(static scratch) on device %d: %s", dev, cudaGetErrorString(e));
+        int n_sm = 0;
+        e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess || n_sm < 1)
+            return na_fail(err, len, ST_ECUDA, "cudaDeviceGetAttribute(SM count) on device %d: %s", dev, cudaGetErrorString(e));
+        d.scratch = static_cast<unsigned char*>(ptr); d.n_sm = n_sm; d.ready = true;
+    }
+    *out = d;
+    return ST_OK;
+}
+
+}  // namespace
+
+extern "C" int st_score_random_noalloc(const void* csd_dev, const float* sigma_dev, int32_t sigma_kind,
+                                       int32_t n_t, int32_t n_f, double df, double f_min,
+                                       const st_search_params* p, float* snr_dev, void* cuda_stream,
+                                       char* err, size_t len)
+{
+    if (err && len) err[0] = 0;
+    // ---- host-side checks, before any CUDA call
+    if (!p) return na_fail(err, len, ST_EINVAL, "params is NULL");
+    if (n_t < 1 || n_t > ST_MAX_N_T || n_f < 1 || n_f > ST_MAX_N_F)
+        return na_fail(err, len, ST_EINVAL, "map shape %d x %d outside [1, %d] x [1, %d]", n_t, n_f, ST_MAX_N_T, ST_MAX_N_F);
+    if (!(df > 0.0) || !(f_min >= 0.0) || !isfinite(df) || !isfinite(f_min))
+        return na_fail(err, len, ST_EINVAL, "need df > 0 and f_min >= 0, both finite");
+    const size_t n_pix = (size_t)n_t * (size_t)n_f;
+    if (n_pix > (size_t)ST_NOALLOC_MAX_PIXELS)
+        return na_fail(err, len, ST_ENOSPC, "map of %d x %d = %zu pixels exceeds ST_NOALLOC_MAX_PIXELS = %d, the size the library's "
+                       "static scratch was compiled for: use st_set_workspace / st_search with a workspace of your own", n_t, n_f, n_pix,
+                       ST_NOALLOC_MAX_PIXELS);
+    if (!csd_dev) return na_fail(err, len, ST_EINVAL, "csd is NULL");
+    if (sigma_kind < ST_SIGMA_NONE || sigma_kind > ST_SIGMA_PER_PIXEL) return na_fail(err, len, ST_EINVAL, "bad sigma_kind %d", sigma_kind);
+    if (sigma_kind != ST_SIGMA_NONE && !sigma_dev) return na_fail(err, len, ST_EINVAL, "sigma is NULL");
+    if (p->n_min < 1 || p->n_max < p->n_min || p->n_max > n_t)
+        return na_fail(err, len, ST_EINVAL, "need 1 <= n_min <= n_max <= n_t (got %d, %d, n_t %d)", p->n_min, p->n_max, n_t);
+    if (p->tau_mode != ST_TAU_RANDOM) return na_fail(err, len, ST_EINVAL, "only ST_TAU_RANDOM (one delay per template) is offered without a workspace");
+    if (!isfinite(p->tau_lo) || !isfinite(p->tau_hi) || p->tau_hi < p->tau_lo) return na_fail(err, len, ST_EINVAL, "bad random-tau range");
+    if (p->norm != ST_NORM_SQRT_N && p->norm != ST_NORM_MEAN) return na_fail(err, len, ST_EINVAL, "norm %d: only ST_NORM_SQRT_N / ST_NORM_MEAN here", p->norm);
+    if (p->family != ST_FAMILY_QUADRATIC) return na_fail(err, len, ST_EINVAL, "family %d: only ST_FAMILY_QUADRATIC here", p->family);
+    if (p->track_offset > (1ull << 62)) return na_fail(err, len, ST_EINVAL, "track_offset too large");
+    if (p->n_tracks > kMaxSamplesPerLaunch) return na_fail(err, len, ST_EINVAL, "n_tracks %llu exceeds one launch (2^31): split the range",
+                                                           (unsigned long long)p->n_tracks);
+    if (p->n_tracks == 0) return ST_OK;
+    if (!snr_dev) return na_fail(err, len, ST_EINVAL, "snr_dev is NULL");
+    // ---- the current device's copy of the static scratch
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return na_fail(err, len, ST_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= kNaMaxDevices) return na_fail(err, len, ST_EINVAL, "device ordinal %d beyond the %d this entry point keeps track of", dev, kNaMaxDevices);
+    NoallocDevice d;
+    int rc = noalloc_device(dev, &d, err, len);
+    if (rc) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    st::Scalars* sc = reinterpret_cast<st::Scalars*>(d.scratch + kNaOffScalars);
+    float2* map = reinterpret_cast<float2*>(d.scratch + kNaOffMap);
+    float* isig = reinterpret_cast<float*>(d.scratch + kNaOffIsig);
+    // The array still holds the previous call's counter, maximum and per-warp records: those must read zero.
+    // The map and 1 / sigma planes need no clearing: S0 below rewrites every pixel this call will gather.
+    e = cudaMemsetAsync(d.scratch, 0, kNaZeroed, stream);
+    if (e != cudaSuccess) return na_fail(err, len, ST_ECUDA, "cudaMemsetAsync(static scratch): %s", cudaGetErrorString(e));
+    // ---- S0 (Eq. 7), as st_set_map launches it
+    {
+        const int blocks = (int)((n_pix + 255) / 256 < (size_t)(8 * d.n_sm) ? (n_pix + 255) / 256 : (size_t)(8 * d.n_sm));
+        const bool vec = (n_pix % 2 == 0) && ((uintptr_t)csd_dev % 16 == 0) &&
+                         (sigma_kind != ST_SIGMA_PER_PIXEL || (uintptr_t)sigma_dev % 8 == 0);
+        if (vec) st::k_prepare_map<true><<<blocks, 256, 0, stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, n_f, n_pix, map, isig);
+        else st::k_prepare_map<false><<<blocks, 256, 0, stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, n_f, n_pix, map, isig);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return na_fail(err, len, ST_ECUDA, "k_prepare_map launch: %s", cudaGetErrorString(e));
+    }
+    // ---- S1-S3 (+ the S4 records the kernel keeps anyway), as st_debug_scores launches them in random mode
+    st::ScoreArgs a;
+    memset(&a, 0, sizeof(a));
+    a.map = map; a.isig = isig;
+    a.bp.seed = p->seed; a.bp.n_t = n_t; a.bp.n_f = n_f; a.bp.n_min = p->n_min; a.bp.n_max = p->n_max;
+    a.bp.tau_lo = p->tau_lo; a.bp.tau_hi = p->tau_hi; a.bp.family = ST_FAMILY_QUADRATIC; a.bp.pad = 0;
+    a.f_min = f_min; a.df = df;
+    a.track_offset = p->track_offset; a.n_tracks = p->n_tracks;
+    a.n_tau = 1; a.norm = p->norm;
+    a.sc = sc;
+    a.cand = reinterpret_cast<st::Cand*>(d.scratch + kNaOffCand); a.cand_cap = kNaCandCap;
+    a.warp_best = reinterpret_cast<st::WarpBest*>(d.scratch + kNaOffWarpBest); a.warp_slots = kWarpSlots;
+    a.hist = nullptr; a.n_bins = 0;
+    a.dump = snr_dev;
+    a.pool_stride = (p->n_max + 63) & ~63;
+    {
+        uint64_t blocks = (uint64_t)d.n_sm * 8;
+        const uint64_t need = ((p->n_tracks + st::kRandPerWarp - 1) / st::kRandPerWarp + 7) / 8;
+        if (blocks > need) blocks = need;
+        if (blocks > kWarpSlots / 8) blocks = kWarpSlots / 8;
+        st::k_score_random<false, false, false><<<(unsigned)blocks, 256, hist_bytes(0), stream>>>(a);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return na_fail(err, len, ST_ECUDA, "k_score_random launch: %s", cudaGetErrorString(e));
+    }
+    return ST_OK;
+}
