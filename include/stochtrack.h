@@ -63,7 +63,8 @@ extern "C" {
  * G25: the inverse-variance combination of Appendix A's per-pixel estimates,
  *     SNR_w = sum_Gamma (rho / sigma) / sqrt( sum_Gamma 1 / sigma^2 ),   rho = Re[e^{2 pi i f tau} p],
  * equal to the SQRT_N statistic for constant sigma; masked pixels leave both sums.  Needs the map to have
- * been set with its sigma (st_set_map, st_set_map_host, st_search_batch), else ST_ESTATE.             */
+ * been set with its sigma (st_set_map, st_set_map_host, or a st_search_batch run with this norm: a batch with
+ * another norm does not write the 1 / sigma plane and leaves its last map without one), else ST_ESTATE. */
 #define ST_NORM_INVVAR 2
 
 /* template families ("other parameterizable curves such as spline can be used as well";
@@ -232,7 +233,10 @@ int st_search_track_max(st_ctx *ctx, const st_search_params *params, float *snr_
  * (Eq. 5: a fixed set of clusters Gamma) and the parity export for track shapes the bank
  * produces with vanishing probability (flat, near-flat, full-length).
  *   tracks  : HOST [count] templates in the st_track parameterisation (1 <= N, 0 <= j0, j0 + N <= n_t,
- *             0 < a < N, finite control points); in random mode each template's own `tau` is its delay
+ *             0 < a < N, finite values, and the frequency control points the family uses -- y0, y1, y2; y3 too
+ *             for CUBIC; y0 alone for CHIRP -- inside the band, 0 <= y <= n_f in bin units, as every bank
+ *             member's are: the rasteriser's bit-exactness guard is sized for that range); in random mode
+ *             each template's own `tau` is its delay
  *   snr_dev : DEVICE float32 [count][n_tau] (n_tau = 1 in random mode), same scoring kernel as st_search
  *             with the same params (tau grid / range, norm, kernel, family); n_tracks, track_offset, seed,
  *             n_min, n_max and the histogram fields of params are ignored.
@@ -293,7 +297,9 @@ int st_set_map_from_strain(st_ctx *ctx, const double *s_i_dev, const double *s_j
  * P' of each detector taken around its own segment, and the resulting map is searched with seeds[m]
  * (HOST, or NULL: params->seed for every shift).  Per-shift results and histograms as st_search_batch
  * (results HOST [n_shifts], params->hist_out HOST [n_shifts][n_bins], no host synchronisation inside a
- * group of ST_BATCH_GROUP shifts).  On return the context's map is that of the last shift.             */
+ * group of ST_BATCH_GROUP shifts).  On return the context's map is that of the last shift.
+ * ST_NORM_INVVAR is refused (ST_EINVAL): a map built from strain has no 1 / sigma plane; likewise st_search on
+ * a map set by st_set_map_from_strain returns ST_ESTATE for that norm.                                   */
 int st_search_timeshifts(st_ctx *ctx, const double *s_i_dev, const double *s_j_dev, int64_t n_samples,
                          const st_ftmap_params *ft_params, void *scratch_dev, size_t scratch_bytes,
                          int32_t n_shifts, const int32_t *shifts, const uint64_t *seeds,
@@ -319,7 +325,8 @@ int st_debug_rasterise(st_ctx *ctx, const st_search_params *params, uint64_t fir
  * [first, first+count) with params (ST_TAU_RANDOM) and writes the bins it used.  Needs a map.        */
 int st_debug_rasterise_random(st_ctx *ctx, const st_search_params *params, uint64_t first, uint64_t count,
                               int32_t *k_out_dev, int32_t *j0_dev, int32_t *N_dev);
-/* Rasterise one explicit template of the given family (HOST st_track in, DEVICE int32 [N] out). */
+/* Rasterise one explicit template of the given family (HOST st_track in, DEVICE int32 [N] out); the template
+ * must satisfy the conditions listed at st_score_tracks (ST_EINVAL otherwise). */
 int st_debug_rasterise_track(st_ctx *ctx, const st_track *track, int32_t family, int32_t *k_out_dev);
 /* snr_dev float32 [count][n_tau] (n_tau = 1 in random mode): every SNR(i, tau)
  * the scoring kernel selected by params->kernel produces.                      */

@@ -366,10 +366,12 @@ __device__ __forceinline__ float inv_sigma_pixel(float s)
 {
     return (!(s > 0.0f) || isinf(s)) ? 0.0f : __fdiv_rn(1.0f, s);
 }
-// HBM bound (16 B read + 8 B written per pixel with a per-pixel sigma).  VEC: two pixels per thread
-// per iteration through 16-byte loads and stores (the host checks alignment and parity), two
-// iterations in flight.
-template <bool VEC>
+// HBM bound: per pixel 8 B of CSD (+ 4 B of a per-pixel sigma) read, 8 B of p written, and -- ISIG -- 4 B of the
+// 1 / sigma plane written.  Only ST_NORM_INVVAR reads that plane: st_set_map writes it (a later search may ask for
+// that norm), the batch call knows its norm before S0 and leaves the plane out otherwise (1/6 to 1/5 of S0's
+// traffic).  VEC: two pixels per thread per iteration through 16-byte loads and stores (the host checks alignment
+// and parity), two iterations in flight.
+template <bool VEC, bool ISIG = true>
 __global__ void __launch_bounds__(256) k_prepare_map(const float2* __restrict__ csd, const float* __restrict__ sigma,
                                                      int sigma_kind, int n_f, size_t n_pix, float2* __restrict__ p,
                                                      float* __restrict__ isig)
@@ -401,9 +403,11 @@ __global__ void __launch_bounds__(256) k_prepare_map(const float2* __restrict__ 
             }
             p4[i] = make_float4(r0.x, r0.y, r1.x, r1.y);
             if (two) p4[j] = make_float4(r2.x, r2.y, r3.x, r3.y);
-            float2* i2 = reinterpret_cast<float2*>(isig);
-            i2[i] = sigma_kind != 0 ? make_float2(inv_sigma_pixel(sa.x), inv_sigma_pixel(sa.y)) : make_float2(1.0f, 1.0f);
-            if (two) i2[j] = sigma_kind != 0 ? make_float2(inv_sigma_pixel(sb.x), inv_sigma_pixel(sb.y)) : make_float2(1.0f, 1.0f);
+            if (ISIG) {
+                float2* i2 = reinterpret_cast<float2*>(isig);
+                i2[i] = sigma_kind != 0 ? make_float2(inv_sigma_pixel(sa.x), inv_sigma_pixel(sa.y)) : make_float2(1.0f, 1.0f);
+                if (two) i2[j] = sigma_kind != 0 ? make_float2(inv_sigma_pixel(sb.x), inv_sigma_pixel(sb.y)) : make_float2(1.0f, 1.0f);
+            }
         }
     } else {
         for (size_t i = t0; i < n_pix; i += stride) {
@@ -411,7 +415,7 @@ __global__ void __launch_bounds__(256) k_prepare_map(const float2* __restrict__ 
             const float sg = sigma_kind == 0 ? 1.0f : (sigma_kind == 1 ? sigma[i % (size_t)n_f] : sigma[i]);
             if (sigma_kind != 0) c = prepare_pixel(c, sg);
             p[i] = c;
-            isig[i] = inv_sigma_pixel(sg);
+            if (ISIG) isig[i] = inv_sigma_pixel(sg);
         }
     }
 }

@@ -94,6 +94,7 @@ struct st_ctx {
     unsigned long long* h_hist;        // pinned, ST_MAX_BINS
     int n_sm, smem_optin;
     int device;                        // ordinal of the device the workspace lives on (every call runs there)
+    int ev_device;                     // device the context's events (and batch stream) were created on, -1 = none yet
     int recur_threads;                 // tunable: threads per block of the recurrence kernels
     int cheb_stride;                   // stride of the tables currently on the device
     // bank cache (st_set_bank_cache): S1 + S2 of one template bank, reused by every search with the same bank
@@ -123,12 +124,14 @@ int fail(st_ctx* c, int code, const char* fmt, ...)
 // Every device entry point runs on the workspace's device, whatever device is current in the calling thread.
 struct DevGuard {
     int prev; bool switched;
-    explicit DevGuard(const st_ctx* c) : prev(-1), switched(false)
-    {
-        if (c && c->have_ws && cudaGetDevice(&prev) == cudaSuccess && prev != c->device)
-            switched = cudaSetDevice(c->device) == cudaSuccess;
-    }
+    explicit DevGuard(const st_ctx* c) : prev(-1), switched(false) { if (c && c->have_ws) enter(c->device); }
+    explicit DevGuard(int device) : prev(-1), switched(false) { enter(device); }     // before a context knows its device
     ~DevGuard() { if (switched) cudaSetDevice(prev); }
+private:
+    void enter(int device)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+    }
 };
 
 #define ST_CUDA(ctx, call)                                                                   \
@@ -712,6 +715,10 @@ int enqueue_search(st_ctx* c, const st_search_params* p, const Plan& plan, const
                    bool time_it, float* tmax_snr, int32_t* tmax_m)
 {
     const int n_tau = p->tau_mode == ST_TAU_GRID ? p->n_tau : 1;
+    // every search passes here, so no caller can score with a 1 / sigma plane that does not belong to the map
+    // (the ft-map path forms p directly and leaves the plane of an earlier st_set_map, or nothing, behind)
+    if (p->norm == ST_NORM_INVVAR && !c->have_isig)
+        return fail(c, ST_ESTATE, "ST_NORM_INVVAR needs sigma: set the map through st_set_map / st_set_map_host / st_search_batch");
     int rc = reset_search_state(c, p->n_bins, sl);
     if (rc) return rc;
     st::ScoreArgs a = base_args(c, p);
@@ -769,6 +776,25 @@ int enqueue_search(st_ctx* c, const st_search_params* p, const Plan& plan, const
     return ST_OK;
 }
 
+// An explicit template (st_score_tracks, st_debug_rasterise_track) must lie where bank members lie: 0 < a < N and
+// the control points its family uses inside the band, 0 <= y <= n_f.  The rasteriser's fast path decides a bin
+// without the normative sequence when y is further than raster_guard() from an edge, and that guard is sized for
+// |dy/dxi| <= 2 n_f (quadratic) / 3 n_f (cubic), i.e. for control points inside the band; outside it the fast bin
+// could differ from the normative one without a redo, which is exactly what these exports promise not to happen.
+const char* explicit_track_problem(const st_ctx* c, const st_track& t, int32_t family)
+{
+    if (t.N < 1 || t.j0 < 0 || (int64_t)t.j0 + (int64_t)t.N > (int64_t)c->n_t) return "lies outside the map";
+    if (!(t.a > 0.0) || !(t.a < (double)t.N)) return "needs 0 < a < N";
+    if (!isfinite(t.y0) || !isfinite(t.y1) || !isfinite(t.y2) || !isfinite(t.y3) || !isfinite(t.tau))
+        return "needs finite control points and delay";
+    const double top = (double)c->n_f;
+    const int n_used = family == ST_FAMILY_CHIRP ? 1 : (family == ST_FAMILY_CUBIC ? 4 : 3);
+    const double y[4] = {t.y0, t.y1, t.y2, t.y3};
+    for (int i = 0; i < n_used; ++i)
+        if (y[i] < 0.0 || y[i] > top) return "needs its frequency control points inside the band, 0 <= y <= n_f (bin units)";
+    return nullptr;
+}
+
 }  // namespace
 
 // ================================================================== C ABI ====
@@ -793,7 +819,7 @@ int st_create(st_ctx** out, int32_t n_t, int32_t n_f, double df, double f_min)
     c->ev0 = c->ev1 = nullptr; c->h_res = nullptr; c->h_hist = nullptr;
     c->copy_stream = nullptr; c->h_bres = nullptr; c->h_bhist = nullptr;
     for (int i = 0; i < 2; ++i) { c->ev_copied[i] = nullptr; c->ev_consumed[i] = nullptr; }
-    c->n_sm = 0; c->smem_optin = 0; c->recur_threads = ST_CHEB_MAX_THREADS; c->device = 0;
+    c->n_sm = 0; c->smem_optin = 0; c->recur_threads = ST_CHEB_MAX_THREADS; c->device = 0; c->ev_device = -1;
     c->err[0] = 0;
     c->bank = nullptr; c->bank_bytes = 0; c->bank_valid = false; c->last_bank_mode = 0; memset(&c->bank_key, 0, sizeof(c->bank_key));
     c->cheb_stride = 0; c->cheb_n_class_b = 0; c->cheb_dmax = 0.0; c->pick_valid = false; c->pick_dtau = 0.0; c->pick_stride = 0;
@@ -841,20 +867,56 @@ int st_set_workspace(st_ctx* c, void* ws, size_t bytes, void* cuda_stream)
     if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)
         return fail(c, ST_EINVAL, "workspace is not device memory");
     const int dev = pa.device;                      // the context lives on the workspace's device
-    c->device = dev; c->have_ws = true;             // (have_ws lets the guard below switch to it)
-    DevGuard dev_guard(c);
-    c->have_ws = false;
-    ST_CUDA(c, cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev));
-    ST_CUDA(c, cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-    if (!c->ev0) ST_CUDA(c, cudaEventCreate(&c->ev0));
-    if (!c->ev1) ST_CUDA(c, cudaEventCreate(&c->ev1));
-    if (!c->h_res) ST_CUDA(c, cudaHostAlloc((void**)&c->h_res, sizeof(st::DeviceResult), cudaHostAllocDefault));
-    if (!c->h_hist) ST_CUDA(c, cudaHostAlloc((void**)&c->h_hist, ST_MAX_BINS * sizeof(unsigned long long), cudaHostAllocDefault));
+    // Everything fallible happens first, into locals: a failure below leaves the context exactly as it was (an
+    // attached workspace stays attached and usable on its own device).
+    DevGuard dev_guard(dev);
+    int n_sm = 0, smem_optin = 0;
+    ST_CUDA(c, cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    ST_CUDA(c, cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    // events belong to the device they were created on: a move to another device gets its own pair
+    const bool new_events = !c->ev0 || !c->ev1 || c->ev_device != dev;
+    cudaEvent_t ev0 = c->ev0, ev1 = c->ev1;
+    if (new_events) {
+        ev0 = ev1 = nullptr;
+        ST_CUDA(c, cudaEventCreate(&ev0));
+        const cudaError_t e1 = cudaEventCreate(&ev1);
+        if (e1 != cudaSuccess) { cudaEventDestroy(ev0); return fail(c, ST_ECUDA, "cudaEventCreate: %s", cudaGetErrorString(e1)); }
+    }
+    if (!c->h_res || !c->h_hist) {
+        st::DeviceResult* h_res = c->h_res;
+        unsigned long long* h_hist = c->h_hist;
+        cudaError_t e = cudaSuccess;
+        if (!h_res) e = cudaHostAlloc((void**)&h_res, sizeof(st::DeviceResult), cudaHostAllocDefault);
+        if (e == cudaSuccess && !h_hist) e = cudaHostAlloc((void**)&h_hist, ST_MAX_BINS * sizeof(unsigned long long), cudaHostAllocDefault);
+        if (e != cudaSuccess) {
+            if (h_res && !c->h_res) cudaFreeHost(h_res);
+            if (new_events) { cudaEventDestroy(ev0); cudaEventDestroy(ev1); }
+            return fail(c, ST_ECUDA, "cudaHostAlloc: %s", cudaGetErrorString(e));
+        }
+        c->h_res = h_res; c->h_hist = h_hist;       // pinned host memory serves any device: kept across re-attachments
+    }
+    // ---- commit (no CUDA call below can fail the attachment)
+    if (new_events) {
+        if (c->ev0) cudaEventDestroy(c->ev0);
+        if (c->ev1) cudaEventDestroy(c->ev1);
+        c->ev0 = ev0; c->ev1 = ev1;
+        if (c->ev_device != dev) {                  // the batch mode's stream and events are re-made lazily on the new device
+            for (int i = 0; i < 2; ++i) {
+                if (c->ev_copied[i]) { cudaEventDestroy(c->ev_copied[i]); c->ev_copied[i] = nullptr; }
+                if (c->ev_consumed[i]) { cudaEventDestroy(c->ev_consumed[i]); c->ev_consumed[i] = nullptr; }
+            }
+            if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); c->copy_stream = nullptr; }
+        }
+        c->ev_device = dev;
+    }
+    c->device = dev; c->n_sm = n_sm; c->smem_optin = smem_optin;
     c->ws = (unsigned char*)ws; c->ws_bytes = bytes; c->max_n_tau = lo;
     c->L = make_layout(c->n_t, c->n_f, lo);
     c->stream = (cudaStream_t)cuda_stream;
     c->have_ws = true; c->have_map = false; c->have_isig = false;
     c->tau_cached.clear(); c->table_kind = kNoTable; c->w_built = false;
+    // a bank cache filled on the previous stream or device is not ordered against reads on the new one
+    c->bank_valid = false;
     return ST_OK;
 }
 
@@ -872,9 +934,17 @@ int st_set_bank_cache(st_ctx* c, void* cache_dev, size_t bytes)
     return ST_OK;
 }
 
+// S0 into the workspace.  want_isig: also write the 1 / sigma plane (read by ST_NORM_INVVAR only).
+static int set_map_impl(st_ctx* c, const void* csd_dev, const float* sigma_dev, int32_t sigma_kind, bool want_isig);
+
 int st_set_map(st_ctx* c, const void* csd_dev, const float* sigma_dev, int32_t sigma_kind)
 {
     DevGuard dev_guard(c);
+    return set_map_impl(c, csd_dev, sigma_dev, sigma_kind, true);     // whichever norm a later search asks for
+}
+
+static int set_map_impl(st_ctx* c, const void* csd_dev, const float* sigma_dev, int32_t sigma_kind, bool want_isig)
+{
     if (!c) return ST_EINVAL;
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
     if (!csd_dev) return fail(c, ST_EINVAL, "csd is NULL");
@@ -885,12 +955,14 @@ int st_set_map(st_ctx* c, const void* csd_dev, const float* sigma_dev, int32_t s
     // two pixels per thread through 16-byte accesses when the pointers and the pixel count allow
     const bool vec = (n_pix % 2 == 0) && ((uintptr_t)csd_dev % 16 == 0) &&
                      (sigma_kind != ST_SIGMA_PER_PIXEL || (uintptr_t)sigma_dev % 8 == 0);
-    if (vec) st::k_prepare_map<true><<<blocks, 256, 0, c->stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, c->n_f, n_pix,
-                                                                    at<float2>(c, c->L.map), at<float>(c, c->L.isig));
-    else st::k_prepare_map<false><<<blocks, 256, 0, c->stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, c->n_f, n_pix,
-                                                                  at<float2>(c, c->L.map), at<float>(c, c->L.isig));
+#define ST_LAUNCH_PREPARE(VEC, ISIG)                                                                              \
+    st::k_prepare_map<VEC, ISIG><<<blocks, 256, 0, c->stream>>>((const float2*)csd_dev, sigma_dev, sigma_kind, c->n_f, n_pix, \
+                                                                at<float2>(c, c->L.map), at<float>(c, c->L.isig))
+    if (vec) { if (want_isig) ST_LAUNCH_PREPARE(true, true); else ST_LAUNCH_PREPARE(true, false); }
+    else     { if (want_isig) ST_LAUNCH_PREPARE(false, true); else ST_LAUNCH_PREPARE(false, false); }
+#undef ST_LAUNCH_PREPARE
     ST_CUDA(c, cudaGetLastError());
-    c->have_map = true; c->have_isig = true;
+    c->have_map = true; c->have_isig = want_isig;
     return ST_OK;
 }
 
@@ -916,10 +988,19 @@ int st_set_map_host(st_ctx* c, const void* csd_host, const float* sigma_host, in
 
 static int search_impl(st_ctx* c, const st_search_params* p, st_result* out, float* tmax_snr, int32_t* tmax_m);
 
+// The bank cache's validity is host-side book-keeping: it is set once a filling search has been ENQUEUED.  Any call
+// that then fails (a launch or synchronisation error, an error in a later map of a batch) may leave the cache
+// partly written, so every failing search drops it; the next search with that bank fills it again.
+static int drop_bank_on_error(st_ctx* c, int rc)
+{
+    if (rc && c) c->bank_valid = false;
+    return rc;
+}
+
 int st_search(st_ctx* c, const st_search_params* p, st_result* out)
 {
     DevGuard dev_guard(c);
-    return search_impl(c, p, out, nullptr, nullptr);
+    return drop_bank_on_error(c, search_impl(c, p, out, nullptr, nullptr));
 }
 
 int st_search_track_max(st_ctx* c, const st_search_params* p, float* snr_max_dev, int32_t* tau_index_dev, st_result* out)
@@ -927,7 +1008,7 @@ int st_search_track_max(st_ctx* c, const st_search_params* p, float* snr_max_dev
     DevGuard dev_guard(c);
     if (!c) return ST_EINVAL;
     if (!snr_max_dev || !tau_index_dev) return fail(c, ST_EINVAL, "per-template output pointer is NULL");
-    return search_impl(c, p, out, snr_max_dev, tau_index_dev);
+    return drop_bank_on_error(c, search_impl(c, p, out, snr_max_dev, tau_index_dev));
 }
 
 static int search_impl(st_ctx* c, const st_search_params* p, st_result* out, float* tmax_snr, int32_t* tmax_m)
@@ -1067,7 +1148,7 @@ int st_search_batch(st_ctx* c, const st_batch* b, const st_search_params* p, st_
         if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
         cudaStreamSynchronize(c->stream);
     }
-    return rc;
+    return drop_bank_on_error(c, rc);
 }
 
 static int batch_impl(st_ctx* c, const st_batch* b, const st_search_params* p, st_result* results, float* gpu_ms_total)
@@ -1133,6 +1214,9 @@ static int batch_impl(st_ctx* c, const st_batch* b, const st_search_params* p, s
         if (rc) return rc;
     }
     st_search_params pm = *p;
+    // the batch knows its norm before S0: the 1 / sigma plane is written only for the statistic that reads it
+    // (afterwards the context's map is the last one, without the plane: a later INVVAR search gets ST_ESTATE)
+    const bool want_isig = p->norm == ST_NORM_INVVAR;
     for (int g0 = 0; g0 < b->n_maps; g0 += ST_BATCH_GROUP) {
         const int g1 = g0 + ST_BATCH_GROUP < b->n_maps ? g0 + ST_BATCH_GROUP : b->n_maps;
         std::vector<int> launches((size_t)(g1 - g0), 0), bank_modes((size_t)(g1 - g0), 0);
@@ -1141,11 +1225,11 @@ static int batch_impl(st_ctx* c, const st_batch* b, const st_search_params* p, s
             if (b->host_buffers) {
                 if (m + 1 < b->n_maps) { rc = enqueue_copy(m + 1); if (rc) return rc; }
                 ST_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied[sb], 0));
-                rc = st_set_map(c, stage_csd[sb], stage_sig[sb], b->sigma_kind);
+                rc = set_map_impl(c, stage_csd[sb], stage_sig[sb], b->sigma_kind, want_isig);
                 if (rc) return rc;
                 ST_CUDA(c, cudaEventRecord(c->ev_consumed[sb], c->stream));
             } else {
-                rc = st_set_map(c, b->csd[m], b->sigma_kind != ST_SIGMA_NONE ? b->sigma[m] : nullptr, b->sigma_kind);
+                rc = set_map_impl(c, b->csd[m], b->sigma_kind != ST_SIGMA_NONE ? b->sigma[m] : nullptr, b->sigma_kind, want_isig);
                 if (rc) return rc;
             }
             pm.seed = b->seeds ? b->seeds[m] : p->seed;
@@ -1240,13 +1324,28 @@ int st_set_map_from_strain(st_ctx* c, const double* s_i, const double* s_j, int6
     return ft_normalise(c, st_i, st_j, fp->n_neighbours, 0);
 }
 
+static int timeshifts_impl(st_ctx* c, const double* s_i, const double* s_j, int64_t n_samples, const st_ftmap_params* fp,
+                           void* scratch, size_t scratch_bytes, int32_t n_shifts, const int32_t* shifts,
+                           const uint64_t* seeds, const st_search_params* p, st_result* results, float* gpu_ms_total);
+
 int st_search_timeshifts(st_ctx* c, const double* s_i, const double* s_j, int64_t n_samples, const st_ftmap_params* fp,
                          void* scratch, size_t scratch_bytes, int32_t n_shifts, const int32_t* shifts,
                          const uint64_t* seeds, const st_search_params* p, st_result* results, float* gpu_ms_total)
 {
     DevGuard dev_guard(c);
+    return drop_bank_on_error(c, timeshifts_impl(c, s_i, s_j, n_samples, fp, scratch, scratch_bytes, n_shifts, shifts, seeds, p,
+                                                 results, gpu_ms_total));
+}
+
+static int timeshifts_impl(st_ctx* c, const double* s_i, const double* s_j, int64_t n_samples, const st_ftmap_params* fp,
+                           void* scratch, size_t scratch_bytes, int32_t n_shifts, const int32_t* shifts,
+                           const uint64_t* seeds, const st_search_params* p, st_result* results, float* gpu_ms_total)
+{
     int rc = validate(c, p, false);
     if (rc) return rc;
+    // the maps of this call come from strain (k_ft_normalise writes p only): there is no per-pixel sigma to weight by
+    if (p->norm == ST_NORM_INVVAR)
+        return fail(c, ST_EINVAL, "ST_NORM_INVVAR is not available for maps built from strain (no 1 / sigma plane): use ST_NORM_SQRT_N");
     if (!results || !shifts) return fail(c, ST_EINVAL, "shifts / results is NULL");
     if (n_shifts < 1) return fail(c, ST_EINVAL, "n_shifts must be >= 1");
     for (int m = 0; m < n_shifts; ++m)
@@ -1372,8 +1471,8 @@ int st_debug_rasterise_track(st_ctx* c, const st_track* t, int32_t family, int32
     if (!c) return ST_EINVAL;
     if (!t || !k_out_dev) return fail(c, ST_EINVAL, "NULL argument");
     if (family != ST_FAMILY_QUADRATIC && family != ST_FAMILY_CUBIC && family != ST_FAMILY_CHIRP) return fail(c, ST_EINVAL, "bad template family %d", family);
+    if (const char* why = explicit_track_problem(c, *t, family)) return fail(c, ST_EINVAL, "track %s", why);
     if (!c->have_ws) return fail(c, ST_ESTATE, "no workspace: call st_set_workspace first");
-    if (t->N < 1 || t->j0 < 0 || t->j0 + t->N > c->n_t) return fail(c, ST_EINVAL, "track outside the map");
     st::Track d;
     d.N = t->N; d.j0 = t->j0; d.a = t->a; d.y0 = t->y0; d.y1 = t->y1; d.y2 = t->y2; d.tau = t->tau; d.y3 = t->y3;
     st::k_debug_rasterise_track<<<(t->N + 127) / 128, 128, 0, c->stream>>>(d, c->n_f, family, k_out_dev);
@@ -1411,16 +1510,13 @@ int st_score_tracks(st_ctx* c, const st_search_params* p, const st_track* tracks
     if (!tracks || !snr_dev) return fail(c, ST_EINVAL, "tracks / snr_dev is NULL");
     if (count < 0 || count > ST_MAX_SCORE_TRACKS) return fail(c, ST_EINVAL, "count %d outside [0, %d]", count, ST_MAX_SCORE_TRACKS);
     if (count == 0) return ST_OK;
+    if (p->family != ST_FAMILY_QUADRATIC && p->family != ST_FAMILY_CUBIC && p->family != ST_FAMILY_CHIRP) return fail(c, ST_EINVAL, "bad template family %d", p->family);
     st_search_params q = *p;                         // the durations come from the list, not from params
     q.n_min = c->n_t; q.n_max = 1; q.n_tracks = (uint64_t)count; q.track_offset = 0; q.n_bins = 0; q.hist_out = nullptr;
     std::vector<st::Track> h((size_t)count);
     for (int i = 0; i < count; ++i) {
         const st_track& t = tracks[i];
-        if (t.N < 1 || t.j0 < 0 || (int64_t)t.j0 + (int64_t)t.N > (int64_t)c->n_t)
-            return fail(c, ST_EINVAL, "tracks[%d] lies outside the map", i);
-        if (!(t.a > 0.0) || !(t.a < (double)t.N) || !isfinite(t.y0) || !isfinite(t.y1) || !isfinite(t.y2) || !isfinite(t.tau) ||
-            !isfinite(t.y3))
-            return fail(c, ST_EINVAL, "tracks[%d]: need 0 < a < N and finite control points / delay", i);
+        if (const char* why = explicit_track_problem(c, t, p->family)) return fail(c, ST_EINVAL, "tracks[%d] %s", i, why);
         h[(size_t)i].N = t.N; h[(size_t)i].j0 = t.j0; h[(size_t)i].a = t.a;
         h[(size_t)i].y0 = t.y0; h[(size_t)i].y1 = t.y1; h[(size_t)i].y2 = t.y2; h[(size_t)i].tau = t.tau;
         h[(size_t)i].y3 = t.y3;

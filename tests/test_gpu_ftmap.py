@@ -166,3 +166,33 @@ def test_timeshift_background_with_one_bank_and_the_bank_cache(P, orc):
         ref = orc.search(F.ftmap_timeshift(r_i, r_j, n_nb, shifts[m]), f_min, fs / L, T, seed, 20, 64, tau_grid=tau, n_bins=100)
         assert (got[m].arg_track, got[m].arg_tau_index) == (ref["arg_track"], ref["arg_tau_index"])
         assert abs(got[m].max_snr_f64 - ref["max_snr"]) <= 1e-5 * abs(ref["max_snr"])
+
+
+def test_inverse_variance_norm_is_refused_on_maps_built_from_strain(P):
+    """A map built from strain carries no 1 / sigma plane (k_ft_normalise forms p directly), so the inverse-variance
+    statistic (G25) has nothing to weight by: the time-shift call refuses it up front (ST_EINVAL) and a plain search
+    on such a map reports the missing state (ST_ESTATE) -- even when an earlier st_set_map left a plane of its own in
+    the workspace (the silent-wrong-result case the refusal closes).  The context stays usable."""
+    import torch
+    rng = np.random.default_rng(35)
+    fs, L, n_t, n_f, f_min, n_nb = 1024.0, 1024, 32, 100, 100.0, 4
+    n = (n_t + 1) * L // 2
+    di, dj = torch.from_numpy(rng.standard_normal(n)).cuda(), torch.from_numpy(rng.standard_normal(n)).cuda()
+    tau = synth.tau_linspace(16, -0.01, 0.01)
+    st = P.Stochtrack(n_t, n_f, fs / L, f_min, max_n_tau=64)
+    # a map with its own sigma first: the plane it leaves behind must not be picked up by the strain path
+    st.set_map(synth.noise_csd(n_t, n_f, 5), synth.make_sigma("per_pixel", 0.3, n_t, n_f, 5))
+    ok = st.search(500, 3, 10, 32, tau_grid=tau, norm=P.NORM_INVVAR)
+    assert np.isfinite(ok.max_snr_f64)
+    with pytest.raises(P.StError) as e:
+        st.search_timeshifts(di, dj, fs, L, n_nb, [0, 5], 3, 500, 10, 32, tau_grid=tau, norm=P.NORM_INVVAR)
+    assert e.value.code == -1 and "ST_NORM_INVVAR" in str(e.value)
+    st.set_map_from_strain(di, dj, fs, L, n_nb)
+    for call in (lambda: st.search(500, 3, 10, 32, tau_grid=tau, norm=P.NORM_INVVAR),
+                 lambda: st.search(500, 3, 10, 32, tau_range=(-0.01, 0.01), norm=P.NORM_INVVAR),
+                 lambda: st.debug_scores(3, 10, 32, 0, 100, tau_grid=tau, norm=P.NORM_INVVAR)):
+        with pytest.raises(P.StError) as e:
+            call()
+        assert e.value.code == -2 and "sigma" in str(e.value)
+    res, _ = st.search_timeshifts(di, dj, fs, L, n_nb, [0, 5], 3, 500, 10, 32, tau_grid=tau)
+    assert len(res) == 2 and all(np.isfinite(r.max_snr_f64) for r in res)

@@ -1101,3 +1101,47 @@ def test_chirp_family_self_recovery_and_explicit_scores(P, orc):
                                     orc.rasterise(orc.make_track(*tr[:6], family=orc.FAMILY_CHIRP), cfg.n_f), W) for tr in tracks])
     ok, worst = snr_close(got, ref)
     assert ok, worst
+
+
+def test_bank_cache_is_dropped_by_a_failed_search_and_by_a_new_workspace(P):
+    """The cache's validity is host-side book-keeping set when a filling search is enqueued; a search that then fails
+    may have left it partly written, and a workspace re-attachment may move the context to another stream, so both
+    drop it: the next search with the same bank fills it again (ST_FLAG_BANK_FILLED) instead of reading, with
+    identical results.  A refused re-attachment (buffer too small / not device memory) leaves the context usable."""
+    import ctypes as C
+    import torch
+    cfg = synth.CONFIGS[2]
+    tau = synth.tau_linspace(cfg.n_tau)
+    csd = torch.from_numpy(synth.noise_csd(cfg.n_t, cfg.n_f, 77)).cuda()
+    st = make_ctx(P, cfg)
+    st.set_map(csd)
+    T = 5000
+    assert st.enable_bank_cache(T, cfg.n_max) > 0
+    kw = dict(tau_grid=tau, n_bins=100)
+    a = st.search(T, 5, cfg.n_min, cfg.n_max, **kw)
+    b = st.search(T, 5, cfg.n_min, cfg.n_max, **kw)
+    assert a.flags & 4 and b.flags & 2
+    with pytest.raises(P.StError):                    # a failing search: grid beyond the workspace's max_n_tau
+        st.search(T, 5, cfg.n_min, cfg.n_max, tau_grid=synth.tau_linspace(4096), n_bins=100)
+    c = st.search(T, 5, cfg.n_min, cfg.n_max, **kw)
+    assert c.flags & 4 and not c.flags & 2
+    assert st.search(T, 5, cfg.n_min, cfg.n_max, **kw).flags & 2
+    # refused re-attachments change nothing: the map, the tables and the cache are still there
+    L = st._L
+    assert L.st_set_workspace(st._ctx, st._ws.data_ptr(), 1024, st._stream.cuda_stream) == -3
+    host = np.zeros(64, dtype=np.uint8)
+    assert L.st_set_workspace(st._ctx, C.c_void_p(host.ctypes.data + (-host.ctypes.data) % 256 if host.ctypes.data % 256 else host.ctypes.data),
+                              st.workspace_bytes, st._stream.cuda_stream) in (-1, -4)
+    d = st.search(T, 5, cfg.n_min, cfg.n_max, **kw)
+    assert d.flags & 2
+    # an accepted re-attachment (same buffer) resets the context: the map must be set again, the cache is refilled
+    assert L.st_set_workspace(st._ctx, st._ws.data_ptr(), st.workspace_bytes, st._stream.cuda_stream) == 0
+    with pytest.raises(P.StError) as e:
+        st.search(T, 5, cfg.n_min, cfg.n_max, **kw)
+    assert e.value.code == -2
+    st.set_map(csd)
+    f = st.search(T, 5, cfg.n_min, cfg.n_max, **kw)
+    assert f.flags & 4 and not f.flags & 2
+    for r in (b, c, d, f):
+        assert (r.max_snr, r.max_snr_f64, r.arg_track, r.arg_tau_index, r.n_pixels) == (a.max_snr, a.max_snr_f64, a.arg_track, a.arg_tau_index, a.n_pixels)
+        assert np.array_equal(r.hist, a.hist)

@@ -99,6 +99,43 @@ def test_create_validates_arguments(lib):
         lib.st_destroy(ctx)
 
 
+def test_explicit_templates_outside_the_band_are_refused(lib):
+    """st_score_tracks / st_debug_rasterise_track: the rasteriser's fast-path guard is sized for control points inside
+    the band (as every bank member's are), so explicit templates beyond it are refused on the host (ST_EINVAL) rather
+    than rasterised without the bit-exactness guarantee; templates inside pass on to the next check (here: no
+    workspace, ST_ESTATE).  No CUDA call is reached."""
+    ctx = C.c_void_p()
+    assert lib.st_create(C.byref(ctx), 100, 50, 1.0, 40.0) == 0
+    try:
+        p = binding.CSearchParams()
+        p.tau_mode, p.tau_hi = binding.TAU_RANDOM, 0.01
+        good = dict(N=50, j0=10, a=20.0, y0=0.0, y1=50.0, y2=25.5, tau=0.0, y3=0.0)
+
+        def score(family=0, **kw):
+            p.family = family
+            t = (binding.CTrack * 1)(binding.CTrack(**{**good, **kw}))
+            return lib.st_score_tracks(ctx, C.byref(p), t, 1, 256), lib.st_last_error(ctx).decode()
+
+        def raster(family=0, **kw):
+            t = binding.CTrack(**{**good, **kw})
+            return lib.st_debug_rasterise_track(ctx, C.byref(t), family, 256), lib.st_last_error(ctx).decode()
+
+        for call in (score, raster):
+            assert call()[0] == binding.ST_ESTATE                           # inside the band, edges included
+            for bad in (dict(y0=-1e-9), dict(y1=50.000001), dict(y2=1e9), dict(y1=float("nan")), dict(a=0.0), dict(a=50.0),
+                        dict(j0=51), dict(N=0)):
+                rc, msg = call(**bad)
+                assert rc == binding.ST_EINVAL, (call.__name__, bad)
+            assert "inside the band" in call(y2=-3.0)[1]
+            # y3 counts for the cubic family only; the chirp law uses y0 alone
+            assert call(y3=77.0)[0] == binding.ST_ESTATE and call(binding.FAMILY_CUBIC, y3=77.0)[0] == binding.ST_EINVAL
+            assert call(binding.FAMILY_CHIRP, y1=-5.0, y2=1e6, y3=99.0)[0] == binding.ST_ESTATE
+            assert call(binding.FAMILY_CHIRP, y0=50.5)[0] == binding.ST_EINVAL
+            assert call(3)[0] == binding.ST_EINVAL
+    finally:
+        lib.st_destroy(ctx)
+
+
 def test_host_track_generator_matches_oracle_bit_for_bit(lib, orc):
     """S1 on the host side of the product == O1 + O2 of the oracle (words and parameters)."""
     shapes = [(0, 64, 64, 64, 64), (1, 250, 961, 10, 250), (2, 500, 2461, 10, 500), (4, 1000, 2461, 10, 1000),
