@@ -430,6 +430,46 @@ def test_P9_P10_chunk_combination_and_histogram(orc):
     assert np.array_equal(dire["snr"], snr)
 
 
+def test_histogram_bins_by_their_definition(orc):
+    """G14 pinned by what a histogram IS, not by re-typing the oracle's floor formula: bin i counts the samples with
+    lo + i w <= SNR < lo + (i + 1) w (explicit edges, np.searchsorted on the oracle's own SNR dump), samples below lo
+    go to bin 0 and samples at or above hi to the last bin.  A range narrower than the data exercises both clamps, a
+    width that is not a power of two keeps the edges off round numbers.  Then constructed maps whose every SNR is one
+    exactly known value -- a constant real map at tau = 0 under the mean normalisation scores exactly that constant --
+    put samples ON edges, just inside bins and outside the range: a round-to-nearest, a ceil, an open-left edge or a
+    dropped clamp each fail here."""
+    cfg = synth.CONFIGS[1]
+    csd, sigma, taus = synth.config_inputs(cfg)
+    p = orc.prepare_map(csd, sigma)
+    lo, hi, nb = -1.0, 1.5, 37
+    r = orc.search(p, cfg.f_min, cfg.df, 700, 5, 8, 64, tau_grid=taus, n_bins=nb, hist_lo=lo, hist_hi=hi, dump_snr=True)
+    snr = np.sort(r["snr"].ravel())
+    assert snr[0] < lo - 0.2 and snr[-1] > hi + 0.2            # both clamps are exercised
+    edges = lo + (hi - lo) * np.arange(nb + 1) / nb
+    near = np.abs(snr[:, None] - edges[None, :]).min(axis=1) < 1e-12
+    assert near.sum() == 0                                      # no sample sits on an edge of this seeded case
+    cum = np.searchsorted(snr, edges, side="left")              # samples strictly below each edge
+    want = np.diff(cum).astype(np.int64)
+    want[0] += cum[0]                                           # below lo -> first bin
+    want[-1] += snr.size - cum[-1]                              # at or above hi -> last bin
+    assert np.array_equal(r["hist"], want) and int(r["hist"].sum()) == 700 * cfg.n_tau
+    # samples of exactly known value: constant map, tau = 0, alpha = 1 -> SNR = c for every template
+    lo, hi, nb = -4.0, 4.0, 64
+    w = (hi - lo) / nb                                          # 0.125: edges and the values below are exact in binary
+    eps = 2.0 ** -20                                            # dyadic: sums of up to 64 copies stay exact
+    cases = [(0.0, 32), (w, 33), (-w, 31), (0.5 * w, 32), (0.75 * w, 32), (0.9375 * w, 32), (-0.25 * w, 31), (-0.75 * w, 31),
+             (lo, 0), (lo + 0.5 * w, 0), (hi - w, 63), (hi - 0.5 * w, 63), (hi, 63), (100.0, 63), (-100.0, 0),
+             (lo - eps, 0), (w - eps, 32), (-w - eps, 30), (hi - eps, 63), (3 * w + eps, 35)]
+    for c, want_bin in cases:
+        flat = np.full((cfg.n_t, cfg.n_f), c, dtype=np.complex128)
+        z = orc.search(flat, cfg.f_min, cfg.df, 20, 1, 8, 64, tau_grid=np.zeros(1), norm=orc.NORM_MEAN, n_bins=nb, hist_lo=lo,
+                       hist_hi=hi, dump_snr=True)
+        assert (z["snr"] == c).all(), c
+        expect = np.zeros(nb, dtype=np.int64)
+        expect[want_bin] = 20
+        assert np.array_equal(z["hist"], expect), (c, want_bin, np.flatnonzero(z["hist"]))
+
+
 def test_random_tau_mode_uses_track_delay(orc):
     """each template carries its own random delay."""
     cfg = synth.CONFIGS[1]
