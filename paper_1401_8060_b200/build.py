@@ -1,6 +1,6 @@
 """Build the C-ABI shared library (hand-written CUDA, sm_100a only) in-tree.
 
-    python -m paper_1401_8060_b200.build [--force] [--checked | --microbench]
+    python -m paper_1401_8060_b200.build [--force] [--checked | --microbench | --sass-summary]
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the
 GPU box with the repo snapshot.
@@ -68,8 +68,59 @@ def build(force=False, verbose=False):
     return LIB
 
 
+def sass_summary(lib=None):
+    """Markdown table of what the assembler made of every kernel in the built library: registers, local (spill)
+    bytes and the counts of the sm_100 instructions the design leans on (packed FP32 FFMA2 / FADD2, warp REDUX,
+    the float64 atomic of the template counter, float64 MUFU seeds), from `cuobjdump -res-usage` and `-sass`."""
+    import collections
+    import re
+    lib = lib or build()
+    cuobjdump = os.path.join(os.path.dirname(_nvcc()), "cuobjdump") if os.path.isabs(_nvcc()) else "cuobjdump"
+    res = subprocess.run([cuobjdump, "-res-usage", lib], capture_output=True, text=True, check=True).stdout
+    usage, cur = {}, None
+    for line in res.splitlines():
+        m = re.search(r"Function (\S+):", line)
+        if m:
+            cur = m.group(1)
+            continue
+        m = re.search(r"REG:(\d+).*?SHARED:(\d+).*?LOCAL:(\d+)", line)
+        if m and cur:
+            usage[cur], cur = tuple(int(x) for x in m.groups()), None
+    pat = collections.OrderedDict([
+        ("FFMA2", r"\bFFMA2\b"), ("FADD2", r"\bFADD2\b"), ("FFMA", r"\bFFMA\b"), ("REDUX", r"\bC?REDUX\b"),
+        ("ATOMG.ADD.F64", r"ATOMG\.E\.ADD\.F64"), ("MUFU.*64H", r"MUFU\.\w+64H"), ("DFMA", r"\bDFMA\b"), ("LDS", r"\bLDS\b"),
+        ("SHFL", r"\bSHFL\b"), ("instructions", r"^\s+/\*[0-9a-f]{4}\*/")])
+    sass = subprocess.run([cuobjdump, "-sass", lib], capture_output=True, text=True, check=True).stdout
+    counts, cur = collections.OrderedDict(), None
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            cur = m.group(1)
+            counts[cur] = collections.Counter()
+            continue
+        if cur is not None:
+            for k, rx in pat.items():
+                if re.search(rx, line):
+                    counts[cur][k] += 1
+    filt = os.path.join(os.path.dirname(cuobjdump), "cu++filt") if os.path.isabs(cuobjdump) else "cu++filt"
+    names = subprocess.run([filt] + list(counts), capture_output=True, text=True, check=True).stdout.splitlines()
+    rows, total = [], collections.Counter()
+    for sym, name in zip(counts, names):
+        name = re.sub(r"\((bool|int)\)", "", re.sub(r"^void ", "", name))         # <(bool)1, (int)2> -> <1, 2>
+        name = re.sub(r"\(.*$", "", name).replace("st::", "")
+        rows.append((name, usage.get(sym, (0, 0, 0)), counts[sym]))
+        total.update(counts[sym])
+    out = ["| kernel build | registers | local (spill) B | " + " | ".join(pat) + " |", "|---|---|---|" + "---|" * len(pat)]
+    for name, u, c in sorted(rows):
+        out.append(f"| `{name}` | {u[0]} | {u[2]} | " + " | ".join(str(c[k]) for k in pat) + " |")
+    out.append(f"| **all {len(rows)} kernel builds** | | | " + " | ".join(str(total[k]) for k in pat) + " |")
+    return "\n".join(out)
+
+
 if __name__ == "__main__":
-    if "--checked" in sys.argv:
+    if "--sass-summary" in sys.argv:
+        print(sass_summary())
+    elif "--checked" in sys.argv:
         print(build_checked(force="--force" in sys.argv))
     elif "--microbench" in sys.argv:
         print(build_microbench(force="--force" in sys.argv))
