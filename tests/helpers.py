@@ -45,3 +45,17 @@ def hist_rule_ok(h_gpu, ref_snr, lo, hi, n_bins, s0=S0_UNIT, rel=1e-4):
         i = int(np.flatnonzero(~ok)[0])
         return False, f"edge {edges[i]}: gpu cum {cum_gpu[i]} not in [{lo_cnt[i]}, {hi_cnt[i]}]"
     return True, ""
+
+
+def argmax_ok(arg_track, arg_m, ref, first=0, gap=2e-6):
+    """G12 with its pre-declared near-tie clause: the (template, delay) the GPU returns is the
+    oracle's, or the oracle's OWN float64 value at the sample the GPU chose lies within a relative `gap` of the
+    oracle's maximum -- then the two samples tie to float64 rounding noise (libm vs device sincos decide) and either
+    is accepted.  Needs ref["snr"] (dump_snr=True).  Returns (ok, was_near_tie)."""
+    if (int(arg_track), int(arg_m)) == (int(ref["arg_track"]), int(ref["arg_tau_index"])):
+        return True, False
+    q = int(arg_track) - int(first)
+    if not (0 <= q < ref["snr"].shape[0] and 0 <= int(arg_m) < ref["snr"].shape[1]):
+        return False, False
+    v = float(ref["snr"][q, int(arg_m)])
+    return abs(float(ref["max_snr"]) - v) <= gap * abs(float(ref["max_snr"])), True
