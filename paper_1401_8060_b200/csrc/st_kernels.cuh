@@ -673,7 +673,7 @@ __global__ void __launch_bounds__(256, kRandMinBlocks) k_score_random(const Scor
                 cq[u] = in ? c : t.N - 1;                 // clamped: discarded below
                 kq[u] = raster_bin_fast_u(r, in ? ub + (double)(u * kRandGroup) : u_last, redo[u]);
             }
-            if (redo[0] | redo[1] | redo[2] | redo[3]) {  // ~1e-5 of the time: normative sequence
+            if (redo[0] | redo[1] | redo[2] | redo[3]) {  // ~1e-5 of the time (any family): normative sequence
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
                     if (redo[u]) kq[u] = raster_bin(make_raster(GEN ? load_track(a, live ? q : q0, id) : make_track(a.bp, id), a.bp.n_f, family), cq[u]);

@@ -279,16 +279,18 @@ __device__ __forceinline__ int32_t raster_bin_fast(const Raster& r, int32_t c)
 struct RasterFast {
     double a, cc, aa, y0, pb, pc, pd, guard;
     int32_t kmax;
+    int32_t chirp;     // 1: the chirp law (G27), evaluated from cc = N - a, aa = N^2, y0; the polynomial is unused
 };
 __device__ __forceinline__ RasterFast make_raster_fast(const Track& t, int32_t n_f, int32_t family)
 {
     const Raster r = make_raster(t, n_f, family);
     RasterFast f;
     f.a = r.a; f.cc = r.cc; f.aa = r.aa; f.y0 = r.y0; f.guard = r.guard; f.kmax = r.kmax;
+    f.chirp = family == 2;         // a compile-time 0 in the builds whose family is a constant
     if (family == 2) {
-        // the chirp law has no fast path in this struct: a NaN polynomial sends every pixel to the normative
-        // sequence (the random-delay kernel's regenerate path), correct by construction
-        f.pb = f.pc = f.pd = __longlong_as_double(0x7FF8000000000000ll);
+        // the chirp law is not a polynomial in xi: raster_y_fast evaluates it from (cc, aa, y0) as the grid kernels'
+        // fast path does (MUFU seeds + one Newton step for the quotient and each of the three square roots)
+        f.pb = f.pc = f.pd = 0.0;
     } else if (family == 0) {
         f.pb = 2.0 * (t.y1 - t.y0);                             // Eq. 6 in Horner form: y = y0 + xi (pb + xi pc)
         f.pc = (t.y0 - t.y1) + (t.y2 - t.y1);
@@ -302,6 +304,15 @@ __device__ __forceinline__ RasterFast make_raster_fast(const Track& t, int32_t n
 }
 __device__ __forceinline__ double raster_y_fast(const RasterFast& r, double u)
 {
+    if (r.chirp) {                                                  // as raster_y_fast(const Raster&), family 2
+        const double D = fma(-u, r.cc, r.aa);                       // N^2 - u (N - a) > 0
+        double rc;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(D));
+        const double q0 = r.aa * rc;
+        const double q  = fma(fma(-D, q0, r.aa), rc, q0);
+        const double s  = sqrt_fast(sqrt_fast(sqrt_fast(q)));
+        return (s * s) * (s * r.y0);
+    }
     const double xi = raster_xi_fast(r, u);
     return fma(xi, fma(xi, fma(xi, r.pd, r.pc), r.pb), r.y0);   // error ~1e-12 n_f / 2461 bins (pd = 0: the quadratic, bit for bit)
 }

@@ -1027,7 +1027,8 @@ class SimpleFlags(dict):
 def test_chirp_family_indices_bit_exact(P, orc, n_t, n_f, f_min, seed, n_min, n_max, first, count):
     """S1 + S2 of the chirp-law family (f ~ (t_c - t)^(-3/8); G27): parameters and every pixel index equal
     the oracle's bit for bit, through the grid kernels' fast path (MUFU seeds + Newton for the quotient and the three
-    square roots, guarded) and the random-delay kernel's normative path."""
+    square roots, guarded) and the random-delay kernel's own copy of that fast path (RasterFast, regenerate-on-guard),
+    every template of every shape."""
     st = P.Stochtrack(n_t, n_f, 1.0, f_min, max_n_tau=64)
     st.set_map(np.zeros((n_t, n_f), dtype=np.complex64))
     p = np.zeros((n_t, n_f), dtype=np.complex128)
@@ -1035,9 +1036,8 @@ def test_chirp_family_indices_bit_exact(P, orc, n_t, n_f, f_min, seed, n_min, n_
                      dump_tracks=True, family=orc.FAMILY_CHIRP)
     k, j0, N = st.debug_rasterise(seed, n_min, n_max, first, count, family=P.FAMILY_CHIRP)
     assert np.array_equal(N, ref["N"]) and np.array_equal(j0, ref["j0"]) and np.array_equal(k, ref["k"])
-    k, j0, N = st.debug_rasterise_random(seed, n_min, n_max, first, min(count, 3000), family=P.FAMILY_CHIRP)
-    m = min(count, 3000)
-    assert np.array_equal(N, ref["N"][:m]) and np.array_equal(j0, ref["j0"][:m]) and np.array_equal(k, ref["k"][:m])
+    k, j0, N = st.debug_rasterise_random(seed, n_min, n_max, first, count, family=P.FAMILY_CHIRP)
+    assert np.array_equal(N, ref["N"]) and np.array_equal(j0, ref["j0"]) and np.array_equal(k, ref["k"])
     for tid in (first, first + count - 1):
         a = st.track_params(seed, tid, n_min, n_max, -0.01, 0.01, family=P.FAMILY_CHIRP)
         b = orc.track_params(seed, tid, n_t, n_f, n_min, n_max, -0.01, 0.01, family=orc.FAMILY_CHIRP)
