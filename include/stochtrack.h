@@ -335,6 +335,21 @@ int st_debug_scores(st_ctx *ctx, const st_search_params *params, uint64_t first,
 /* The 8 Philox words of a template (HOST out[8]); pure host function.          */
 int st_debug_track_words(uint64_t seed, uint64_t track_id, uint32_t *out_host);
 
+/* S4 across runs (independent runs over disjoint template-id ranges -- other GPUs, other jobs, resumed
+ * chunks -- are combined by taking the maximum, "results identical"): the G12 rule as one HOST function, so that no
+ * caller has to restate it.  Pure host code, no CUDA call, no context.
+ *   results   : HOST [n] results of searches over disjoint id ranges of the SAME map, delay grid and norm
+ *   hists     : HOST [n] pointers to their n_bins-bin histograms (entries may be NULL), or NULL
+ *   out       : the combination: the entry that wins under the G12 total order among the runs that scored anything
+ *               (larger max_snr_f64, then smaller arg_track, then smaller arg_tau_index) with n_evals, n_pixels,
+ *               n_candidates, n_launches, n_deferred summed, flags OR-ed, max_snr and gpu_ms the maxima; when no
+ *               run scored anything, results[0]
+ *   hist_out  : HOST [n_bins] sum of the histograms given (exact, u64), or NULL
+ *   best_index: optional, receives the index of the winning entry
+ * Errors: ST_EINVAL (n < 1, NULL results / out, n_bins outside [0, ST_MAX_BINS], hist_out without hists).       */
+int st_combine_results(const st_result *results, const uint64_t *const *hists, int32_t n, int32_t n_bins,
+                       st_result *out, uint64_t *hist_out, int32_t *best_index);
+
 /* The paper's one-delay-per-template scoring (S0-S3 of the list at the top) for callers that
  * cannot give the library any device memory of their own.
  *

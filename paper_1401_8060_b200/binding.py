@@ -24,7 +24,7 @@ exported_symbols = ("st_create", "st_destroy", "st_workspace_bytes", "st_set_wor
                     "st_debug_get_map",
                     "st_track_params", "st_track_params_family", "st_debug_rasterise",
                     "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words",
-                    "st_score_random_noalloc",
+                    "st_score_random_noalloc", "st_combine_results",
                     "st_last_error", "st_version")
 
 
@@ -150,6 +150,9 @@ def load_library(path=None):
     L.st_score_random_noalloc.argtypes = [vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_double, C.c_double,
                                           C.POINTER(CSearchParams), vp, vp, C.c_char_p, C.c_size_t]
     L.st_score_random_noalloc.restype = C.c_int
+    L.st_combine_results.argtypes = [C.POINTER(CResult), C.POINTER(C.POINTER(C.c_uint64)), C.c_int32, C.c_int32,
+                                     C.POINTER(CResult), C.POINTER(C.c_uint64), C.POINTER(C.c_int32)]
+    L.st_combine_results.restype = C.c_int
     for name in ("st_create", "st_set_workspace", "st_set_map", "st_set_map_host", "st_search", "st_search_batch", "st_track_params",
                  "st_debug_rasterise", "st_debug_rasterise_track", "st_debug_scores", "st_debug_track_words"):
         getattr(L, name).restype = C.c_int

@@ -1567,6 +1567,47 @@ int st_debug_scores(st_ctx* c, const st_search_params* p, uint64_t first, uint64
 
 }  // extern "C"
 
+// S4 across runs: host only.
+extern "C" int st_combine_results(const st_result* results, const uint64_t* const* hists, int32_t n, int32_t n_bins,
+                                  st_result* out, uint64_t* hist_out, int32_t* best_index)
+{
+    if (!results || !out || n < 1 || n_bins < 0 || n_bins > ST_MAX_BINS) return ST_EINVAL;
+    if (hist_out && !hists) return ST_EINVAL;
+    int best = -1;
+    for (int i = 0; i < n; ++i) {
+        const st_result& r = results[i];
+        if (r.n_evals == 0) continue;                                  // a run that scored nothing has no maximum
+        if (best < 0) { best = i; continue; }
+        const st_result& b = results[best];
+        // G12: larger float64 SNR, then smaller template id, then smaller delay index
+        const bool wins = r.max_snr_f64 != b.max_snr_f64 ? r.max_snr_f64 > b.max_snr_f64
+                        : r.arg_track != b.arg_track     ? r.arg_track < b.arg_track
+                                                         : r.arg_tau_index < b.arg_tau_index;
+        if (wins) best = i;
+    }
+    st_result c = results[best < 0 ? 0 : best];
+    if (best >= 0) {
+        c.n_evals = 0; c.n_pixels = 0; c.n_candidates = 0; c.n_launches = 0; c.n_deferred = 0; c.flags = 0; c.gpu_ms = 0.0f;
+        for (int i = 0; i < n; ++i) {
+            const st_result& r = results[i];
+            c.n_evals += r.n_evals; c.n_pixels += r.n_pixels; c.n_launches += r.n_launches; c.flags |= r.flags;
+            if (r.gpu_ms > c.gpu_ms) c.gpu_ms = r.gpu_ms;
+            if (r.n_evals == 0) continue;
+            c.n_candidates += r.n_candidates; c.n_deferred += r.n_deferred;
+            if (r.max_snr > c.max_snr) c.max_snr = r.max_snr;
+        }
+    }
+    if (hist_out) {
+        for (int b = 0; b < n_bins; ++b) hist_out[b] = 0;
+        for (int i = 0; i < n; ++i)
+            if (hists[i])
+                for (int b = 0; b < n_bins; ++b) hist_out[b] += hists[i][b];
+    }
+    *out = c;
+    if (best_index) *best_index = best < 0 ? 0 : best;
+    return ST_OK;
+}
+
 // ================================================= entry point without allocations ====
 // st_score_random_noalloc (include/stochtrack.h): S0-S3 in the paper's one-delay-per-template mode
 // for hosts that cannot hand the library a workspace -- a framework's pool owns the whole

@@ -21,23 +21,37 @@ def split_range(n_tracks_total, world_size, rank, base_offset=0):
     return base_offset + first, q + (1 if rank < rem else 0)
 
 
-def _key(r):
-    # G12: larger SNR, then smaller template id, then smaller delay index
-    return (-r["max_snr_f64"], r["arg_track"], r["arg_tau_index"])
-
-
 def combine(results):
-    """Combine per-range search results (dicts as returned by Stochtrack.search)."""
-    live = [r for r in results if r["n_evals"] > 0]
-    if not live:
-        return dict(results[0])
-    best = dict(min(live, key=_key))
-    best["n_evals"] = sum(r["n_evals"] for r in results)
-    best["n_pixels"] = sum(r["n_pixels"] for r in results)
-    best["n_candidates"] = sum(r["n_candidates"] for r in live)
-    best["max_snr"] = max(r["max_snr"] for r in live)
-    hists = [r["hist"] for r in results if r.get("hist") is not None]
-    best["hist"] = np.sum(np.stack(hists), axis=0).astype(np.uint64) if hists else None
+    """Combine per-range search results (dicts as returned by Stochtrack.search): marshalling around the C ABI's
+    st_combine_results, which holds the rule (G12 total order, sums, histogram sum); no step of S4 lives here."""
+    import ctypes as C
+    from . import binding as B
+    L = B.load_library()
+    n = len(results)
+    arr = (B.CResult * n)()
+    hists, keep = (C.POINTER(C.c_uint64) * n)(), []
+    n_bins = 0
+    for i, r in enumerate(results):
+        for f in ("max_snr", "max_snr_f64", "arg_tau"):
+            setattr(arr[i], f, float(r.get(f, 0.0)))
+        for f in ("arg_tau_index", "arg_track", "n_evals", "n_pixels", "n_candidates", "n_launches", "flags", "n_deferred"):
+            setattr(arr[i], f, int(r.get(f, 0)))
+        h = r.get("hist")
+        if h is not None:
+            h = np.ascontiguousarray(h, dtype=np.uint64)
+            keep.append(h)
+            hists[i] = h.ctypes.data_as(C.POINTER(C.c_uint64))
+            n_bins = h.size
+    out, idx = B.CResult(), C.c_int32(0)
+    hist_out = np.zeros(n_bins, dtype=np.uint64) if keep else None
+    rc = L.st_combine_results(arr, hists, n, n_bins, C.byref(out),
+                              hist_out.ctypes.data_as(C.POINTER(C.c_uint64)) if keep else None, C.byref(idx))
+    if rc:
+        raise B.StError(rc, "st_combine_results: bad arguments")
+    best = dict(results[idx.value])                   # keeps the winner's arg_params, arg_tau, kernel name, ...
+    for f in ("max_snr", "n_evals", "n_pixels", "n_candidates"):
+        best[f] = getattr(out, f)
+    best["hist"] = hist_out
     return best
 
 

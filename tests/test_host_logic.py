@@ -159,6 +159,43 @@ def test_host_track_generator_matches_oracle_bit_for_bit(lib, orc):
         P.st_track_params(500, 2461, 2, 0, 10, 500, family=3)
 
 
+def test_combine_results_through_the_c_abi(lib):
+    """st_combine_results (G12), called through ctypes with no binding in between: the winner under
+    (larger float64 SNR, smaller template id, smaller delay index), runs that scored nothing ignored, counts summed,
+    histograms summed exactly, flags OR-ed; argument errors refused."""
+    R = binding.CResult
+
+    def res(snr, track, m, evals=10, **kw):
+        r = R()
+        r.max_snr, r.max_snr_f64, r.arg_track, r.arg_tau_index, r.n_evals, r.n_pixels, r.n_candidates = snr, snr, track, m, evals, evals // 2, 1
+        for k, v in kw.items():
+            setattr(r, k, v)
+        return r
+
+    runs = [res(1.0, 9, 3, flags=2), res(1.0, 4, 7, n_launches=3), res(float("-inf"), 0, 0, evals=0), res(1.0, 4, 2, gpu_ms=2.5),
+            res(0.5, 1, 0, n_deferred=7)]
+    arr = (R * len(runs))(*runs)
+    h = [np.arange(4, dtype=np.uint64) + i for i in range(len(runs))]
+    h[2][:] = 0
+    hp = (C.POINTER(C.c_uint64) * len(runs))(*[x.ctypes.data_as(C.POINTER(C.c_uint64)) for x in h])
+    hp[4] = None                                           # a run without a histogram
+    out, idx, hist = R(), C.c_int32(-1), np.full(4, 99, dtype=np.uint64)
+    assert lib.st_combine_results(arr, hp, len(runs), 4, C.byref(out), hist.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(idx)) == 0
+    assert idx.value == 3 and (out.arg_track, out.arg_tau_index, out.max_snr_f64) == (4, 2, 1.0)
+    assert (out.n_evals, out.n_pixels, out.n_candidates, out.n_launches, out.n_deferred, out.flags) == (40, 20, 4, 3, 7, 2)
+    assert out.gpu_ms == 2.5 and out.max_snr == 1.0
+    assert hist.tolist() == (h[0] + h[1] + h[3]).tolist()
+    # a larger float64 value wins whatever the ids; nothing scored anywhere -> the first entry comes back
+    arr2 = (R * 2)(res(2.0, 100, 9), res(2.5, 200, 11))
+    assert lib.st_combine_results(arr2, None, 2, 0, C.byref(out), None, C.byref(idx)) == 0 and idx.value == 1 and out.arg_track == 200
+    arr3 = (R * 2)(res(float("-inf"), 5, 0, evals=0), res(float("-inf"), 6, 0, evals=0))
+    assert lib.st_combine_results(arr3, None, 2, 0, C.byref(out), None, None) == 0 and out.arg_track == 5 and out.n_evals == 0
+    for bad in ((None, None, 2, 0, C.byref(out), None, None), (arr2, None, 0, 0, C.byref(out), None, None),
+                (arr2, None, 2, 5000, C.byref(out), None, None), (arr2, None, 2, 4, C.byref(out), hist.ctypes.data_as(C.POINTER(C.c_uint64)), None),
+                (arr2, None, 2, 0, None, None, None)):
+        assert lib.st_combine_results(*bad) == binding.ST_EINVAL
+
+
 def test_binding_fails_loudly_without_gpu():
     import torch
     if torch.cuda.is_available():
