@@ -123,7 +123,7 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     build.build()
-    pkg.load_library()
+    pkg.load_library(args.lib or None)
     dev = f"cuda:{local}"
     env = dict(torch=torch, pkg=pkg, sharding=sharding, dist=dist, world=world, rank=rank, local=local, dev=dev)
     line = measure(args, env)
@@ -312,6 +312,8 @@ def measure(args, env):
         "result": {"max_snr": combined["max_snr_f64"], "arg_track": combined["arg_track"],
                    "arg_tau_index": combined["arg_tau_index"], "n_deferred_last_step": int(r.n_deferred)},
     }
+    if args.lib:
+        line["config"]["library"] = os.path.basename(args.lib) + " (NOT the production build: a measurement build, results meaningless)"
     if n_maps > 1:
         line["config"]["n_maps"] = n_maps
         line["config"]["bank"] = "one shared bank, bank cache attached" if args.shared_bank else "one bank per map (G16)"
@@ -485,6 +487,8 @@ def main():
     ap.add_argument("--call", default="search", choices=["search", "topk", "track_max"],
                     help="entry point a step goes through: st_search, st_search_topk (K = 100) or st_search_track_max; "
                          "with config 4 the latter two run on one map of its shape")
+    ap.add_argument("--lib", default="", help="load another build of the same C ABI (the -DST_ABLATE measurement builds of "
+                                              "`python -m paper_1401_8060_b200.build --ablate N`); never a bench value")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="default run: skip the short runs of configs 3, 4, P")
     ap.add_argument("--ftmap", action="store_true", help="also time st_set_map_from_strain on strain of the config's duration")

@@ -1,6 +1,6 @@
 """Build the C-ABI shared library (hand-written CUDA, sm_100a only) in-tree.
 
-    python -m paper_1401_8060_b200.build [--force] [--checked | --microbench | --sass-summary]
+    python -m paper_1401_8060_b200.build [--force] [--checked | --microbench | --sass-summary | --ablate 1|2]
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the
 GPU box with the repo snapshot.
@@ -45,6 +45,20 @@ def build_checked(force=False):
     if force or _stale(LIB_CHECKED, deps):
         subprocess.check_call([_nvcc(), *NVCC_FLAGS, "-DST_CHECKED", "-shared", "-o", LIB_CHECKED, *srcs])
     return LIB_CHECKED
+
+
+def build_ablate(which, force=False):
+    """Measurement builds of the Chebyshev kernel (-DST_ABLATE=1: phase B alone, 2: phase A alone; st_kernels.cuh).
+    Their results are meaningless; only `bench.py --lib <path>` loads them (profiles/r03_ablation.md)."""
+    which = int(which)
+    if which not in (1, 2):
+        raise ValueError("--ablate takes 1 (phase B alone) or 2 (phase A alone)")
+    out = os.path.join(HERE, f"libstochtrack_b200_ablate{which}.so")
+    srcs = [os.path.join(CSRC, s) for s in SOURCES]
+    deps = srcs + [os.path.join(CSRC, h) for h in HEADERS]
+    if force or _stale(out, deps):
+        subprocess.check_call([_nvcc(), *NVCC_FLAGS, f"-DST_ABLATE={which}", "-shared", "-o", out, *srcs])
+    return out
 
 
 def build_microbench(force=False):
@@ -120,6 +134,8 @@ def sass_summary(lib=None):
 if __name__ == "__main__":
     if "--sass-summary" in sys.argv:
         print(sass_summary())
+    elif "--ablate" in sys.argv:
+        print(build_ablate(sys.argv[sys.argv.index("--ablate") + 1], force="--force" in sys.argv))
     elif "--checked" in sys.argv:
         print(build_checked(force="--force" in sys.argv))
     elif "--microbench" in sys.argv:

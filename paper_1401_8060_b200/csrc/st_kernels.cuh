@@ -1845,6 +1845,18 @@ __device__ __forceinline__ void cheb_phase_b_split(const ScoreArgs& a, WarpReduc
     if (MODE == 2) tmax_finish(a, tm, q);
 }
 
+// -DST_ABLATE=1 | 2 (python -m paper_1401_8060_b200.build --ablate N): MEASUREMENT builds of the Chebyshev kernel that
+// bound where its time goes (profiles/r03_ablation.md); their results are meaningless and no test loads them.
+//   1  phase B alone: a warp runs S1 + S2 + phase A for one claim in 16 and re-scores that pool for the 15 claims
+//      that follow (the epilogue, fold and S4 run as usual): no Philox, rasteriser, gather, merge on 15/16 of the
+//      claims.  The periodic refresh keeps the mix of pool sizes that of the bank: with the work claimed
+//      dynamically, a warp that kept one short pool for the whole launch would take more than its share of claims;
+//   2  phase A alone: S1 + S2 + gather + merge + compaction into the pool for every template, phase B skipped.
+// n_pixels (hence bench.py's evals) still counts N x n_tau of what each claim stood for.
+#ifndef ST_ABLATE
+#define ST_ABLATE 0
+#endif
+
 template <int STRIDE, int MODE, bool GEN, int BANK, int PB = 0, bool PIPE = false>
 __global__ void __launch_bounds__(PIPE ? ST_CHEB_PIPE_THREADS : ST_CHEB_MAX_THREADS, 1) k_score_cheb(const ScoreArgs a)
 {
@@ -1873,6 +1885,9 @@ __global__ void __launch_bounds__(PIPE ? ST_CHEB_PIPE_THREADS : ST_CHEB_MAX_THRE
     // fast build handed over: the list is complete, the fast launch precedes this one on the stream
     const uint64_t n_items = (GEN && a.defer_in) ? (uint64_t)min(a.sc->n_deferred, a.deferred_cap) : a.n_tracks;
     if (GEN && a.defer_in && blockIdx.x == 0 && threadIdx.x == 0) a.sc->n_deferred_total += (uint32_t)n_items;
+#if ST_ABLATE == 1
+    bool abl_have = false; Track abl_t; ChebCounts abl_cnt; float abl_scale = 0.0f; uint32_t abl_age = 0;
+#endif
     for (;;) {
         const uint64_t item = claim_value(__shfl_sync(kFull, q_pref, 0));
         if (item >= n_items) break;
@@ -1880,6 +1895,13 @@ __global__ void __launch_bounds__(PIPE ? ST_CHEB_PIPE_THREADS : ST_CHEB_MAX_THRE
         const uint64_t q = (GEN && a.defer_in) ? (uint64_t)a.deferred[item] : item;
         const uint64_t id = a.track_offset + q;
         Track t;
+        float scale;
+        bool defer;
+        ChebCounts cnt;
+#if ST_ABLATE == 1
+        if (abl_have && (++abl_age & 15u) != 0u) { t = abl_t; cnt = abl_cnt; scale = abl_scale; defer = false; }
+        else {
+#endif
         if (BANK == 2) {                           // S1 from the bank cache: only N and j0 are needed downstream
             const int2 nj = __ldg(&a.kmeta[a.kcache_base + q]);
             t.N = nj.x; t.j0 = nj.y; t.a = t.y0 = t.y1 = t.y2 = t.tau = t.y3 = 0.0;
@@ -1887,9 +1909,11 @@ __global__ void __launch_bounds__(PIPE ? ST_CHEB_PIPE_THREADS : ST_CHEB_MAX_THRE
             t = GEN ? load_track(a, q, id) : make_track(a.bp, id);             // explicit templates take the general build
             if (BANK == 1 && lane == 0) a.kmeta[a.kcache_base + q] = make_int2(t.N, t.j0);
         }
-        float scale;
-        bool defer;
-        const ChebCounts cnt = cheb_phase_a<GEN, BANK>(a, t, q, pool_v, pool_k, lane, scale, defer);
+        cnt = cheb_phase_a<GEN, BANK>(a, t, q, pool_v, pool_k, lane, scale, defer);
+#if ST_ABLATE == 1
+        abl_have = GEN || !defer; abl_t = t; abl_cnt = cnt; abl_scale = scale;
+        }
+#endif
         if (!GEN && defer) {                       // warp-uniform: too much amplitude in class B bins for this build
             if (lane == 0) {
                 const uint32_t slot = atomicAdd(&a.sc->n_deferred, 1u);
@@ -1899,6 +1923,9 @@ __global__ void __launch_bounds__(PIPE ? ST_CHEB_PIPE_THREADS : ST_CHEB_MAX_THRE
             continue;
         }
         wr.pixels += (unsigned long long)t.N;
+#if ST_ABLATE == 2
+        continue;                                  // phase A alone
+#endif
         ST_ASSERT(cnt.n_a + cnt.n_b >= 1 && cnt.n_a + cnt.n_b <= t.N &&
                   ((cnt.n_a + kWarp - 1) & ~(kWarp - 1)) + ((cnt.n_b + kWarp - 1) & ~(kWarp - 1)) <= S &&
                   (a.tracks || (t.N >= a.bp.n_min && t.N <= a.bp.n_max)) && t.j0 >= 0 && t.j0 + t.N <= a.bp.n_t);
@@ -1910,6 +1937,9 @@ __global__ void __launch_bounds__(PIPE ? ST_CHEB_PIPE_THREADS : ST_CHEB_MAX_THRE
             cheb_phase_b_split<STRIDE, MODE, GEN, (PB == 2 || PB == 4) ? 1 : 0, (PB >= 3), PIPE>(a, wr, sm_hist, sm_tab, sm_zi, pool_v, pool_k,
                                                                                           fold, cnt, scale, id, q, n_chunks, lane);
     }
+#if ST_ABLATE == 2
+    if (pool_v[lane].x == 123.456f && pool_k[lane] == 54321) a.sc->overflow = 1u;      // keeps the pool stores observable
+#endif
     reduce_finish(a, wr);
     hist_flush(sm_hist, a.hist, a.n_bins);
 }
