@@ -39,6 +39,17 @@ DRAM_TRAFFIC = {5: (19.83e6, "profiles/r02_ncu_cheb_c5.txt"),      # algorithmic
                 4: (9.97e6, "profiles/r02_ncu_cheb_c4.txt"),       # per map of the batch: the 9.84 MB map once
                 3: (9.88e6, "profiles/r02_ncu_random.txt")}
 L2_GATHER_PEAK_GBS = 9200.0          # random 32-byte sector gathers, measured (profiles/microbench_r01.md)
+L2_GATHER_FROM = "profiles/microbench_r01.md (built-in fallback)"
+# The figures above are fallbacks: profiles/peaks.json (a tracked data file: each entry with the raw file, command, date
+# and lease it comes from) replaces them when present, so that a new capture updates the line without an edit here.
+_PEAKS_FILE = os.path.join(ROOT, "profiles", "peaks.json")
+if os.path.exists(_PEAKS_FILE):
+    with open(_PEAKS_FILE) as _f:
+        _pk = json.load(_f)
+    if "l2_gather" in _pk:
+        L2_GATHER_PEAK_GBS, L2_GATHER_FROM = float(_pk["l2_gather"]["sector_GBps"]), _pk["l2_gather"]["from"] + " via profiles/peaks.json"
+    for _c, _e in _pk.get("dram_traffic_bytes_per_launch", {}).items():
+        DRAM_TRAFFIC["P" if _c == "P" else int(_c)] = (float(_e["bytes"]), _e["from"] + " via profiles/peaks.json")
 
 
 def workload_tag(config):
@@ -325,7 +336,7 @@ def measure(args, env):
         line["roofline"].update({"bound": "l2-gather", "achieved": gbs, "peak": L2_GATHER_PEAK_GBS, "unit": "GB/s",
                                  "frac": gbs / L2_GATHER_PEAK_GBS,
                                  "peak_how": "random 8-byte gathers from an L2-resident 19.7 MB buffer, one 32-byte sector each, "
-                                             "measured by st_microbench (profiles/microbench_r01.md)"})
+                                             f"measured by st_microbench ({L2_GATHER_FROM})"})
     if world == 1 and args.ftmap:
         line["ftmap"] = ftmap_timing(pkg, torch, cfg, dev)
     if world == 1 and not args.no_cpu_baseline:
