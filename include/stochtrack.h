@@ -387,7 +387,7 @@ int st_combine_results(const st_result *results, const uint64_t *const *hists, i
  *
  * The first call on each device looks up that device's address of the array (cudaGetSymbolAddress, which may
  * load the library's device code there) and the SM count; later calls reuse them.  Make that first call at
- * start-up, outside any stream capture.
+ * start-up, before any stream capture begins.
  * The array is shared by every call on a device and still holds what the previous call left in it: the call
  * clears the part that must start from zero and overwrites the map, so consecutive calls on one stream are
  * independent of each other; but two calls whose work can overlap on the GPU (different streams, or different

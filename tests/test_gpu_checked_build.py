@@ -44,6 +44,15 @@ for cid, n in ((1, 1000), (2, 20000), (3, 30000), (4, 20000), (5, 3000)):
     if cid == 1:
         res, _ = st.search_batch([torch.from_numpy(csd).cuda()] * 3, None, [1, 2, 3], 500, cfg.n_min, cfg.n_max, tau_grid=tau, n_bins=50)
         out["batch"] = [[x.max_snr_f64, x.arg_track] for x in res]
+# the call without a workspace (static scratch inside the library): same kernels, same index assertions
+cfg = synth.CONFIGS[2]
+csd = torch.from_numpy(synth.noise_csd(cfg.n_t, cfg.n_f, 61)).cuda()
+sig = torch.from_numpy(synth.make_sigma(cfg.sigma, cfg.sigma_scale, cfg.n_t, cfg.n_f, 61)).cuda()
+snr = torch.empty(7001, dtype=torch.float32, device="cuda")
+for rep in range(2):
+    P.score_random_noalloc(csd, sig, cfg.df, cfg.f_min, 7001, 7 + rep, cfg.n_min, cfg.n_max, (-0.01, 0.01), snr, track_offset=2 ** 33)
+    torch.cuda.synchronize()
+    out["noalloc%%d" %% rep] = [float(snr.double().sum()), float(snr.max()), int(snr.argmax())]
 torch.cuda.synchronize()
 print(json.dumps(out))
 """
@@ -65,4 +74,4 @@ def test_checked_build_trips_no_assertion_and_matches_production():
     got = _run(checked)
     want = _run(build.LIB)
     assert got == want
-    assert len(got) >= 24
+    assert len(got) >= 26 and "noalloc1" in got
